@@ -1,0 +1,130 @@
+/* gwl.h -- C ABI of libgwl: the B200 (sm_100a) hot path of the Lanczos full-frequency GW method
+ * of Gao, Tang, Zhao and Chelikowsky, arXiv 2310.20103 ("PAPER.md" below = /root/reference/PAPER.md).
+ *
+ * What the library computes (all FP64; units eV; arrays row-major, last index fastest):
+ *   C      = (A-B)^{1/2}(A+B)(A-B)^{1/2}                                    PAPER.md:52  (Eq. 4)
+ *          = diag(Delta^2) + 2 diag(sqrt Delta) K^T V K diag(sqrt Delta),   PAPER.md:41-45 (Eq. 2-3), :122 (Eq. 16)
+ *            Delta_vc = eps_c - eps_v,  K[mu, vc] = phi_v(r_mu) phi_c(r_mu),  V = (alpha|beta)  PAPER.md:125 (Eq. 17)
+ *   |P_nm> : (P_nm)_vc = (nm|vc) sqrt(Delta_vc)
+ *   Lanczos tridiagonalisation started from |P_nm>, one chain per (n,m)      PAPER.md:87-90 (Eq. 13)
+ *   <P|(zeta - Op)^{-1}|P> by the Haydock continued fraction                 PAPER.md:92-99 (Eq. 14)
+ *   Sigma^corr_mm(omega, n) and its sum over n                               PAPER.md:73-83 (Eq. 10-12)
+ * Pair index vc = v*n_c + c.  "delta" of the paper (the broadening) is the argument `eta`.
+ *
+ * Conventions
+ *   - Every entry point returns a gwl_status; the library never throws, aborts or prints.
+ *     gwl_last_error() gives a context-owned, NUL-terminated description of the last failure.
+ *   - The caller owns every buffer it passes.  set_* calls COPY their inputs; no caller pointer is
+ *     kept after a call returns.  Outputs are written into caller-allocated buffers.
+ *   - Pointer mode 0 (default): all array arguments are HOST pointers.  Pointer mode 1: all array
+ *     arguments of gwl_casida_matvec / gwl_lanczos / gwl_resolvent / gwl_selfenergy /
+ *     gwl_set_start_vectors(p) are DEVICE pointers on the context's device (used for timing with the
+ *     data already resident in HBM).  Index arrays (n_idx, m_idx, sgn_n, eps_n) and set_orbitals /
+ *     set_energies / set_kernel / set_polynomial inputs are always HOST pointers.
+ *   - Calls are synchronous on return in pointer mode 0.  In pointer mode 1 work is enqueued on the
+ *     context's stream (gwl_set_stream) and the call returns without synchronising, except gwl_lanczos
+ *     which synchronises only if a host-side decision is needed (never in the default path).
+ *   - One in-flight call per context; contexts are independent.
+ *   - Calls out of order (e.g. gwl_lanczos before gwl_set_kernel) return GWL_ESTATE.
+ *   - There is no CPU fallback: without a CUDA device gwl_create returns GWL_ECUDA.
+ */
+#ifndef GWL_H
+#define GWL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gwl_ctx gwl_ctx; /* opaque; owns its device memory */
+
+typedef enum {
+    GWL_OK = 0,
+    GWL_EINVAL = 1, /* bad argument (NULL, non-positive size, eps_c <= eps_v, ...) */
+    GWL_ESTATE = 2, /* call out of order */
+    GWL_ENOMEM = 3, /* device or host allocation failed */
+    GWL_ECUDA = 4   /* CUDA runtime/driver error; see gwl_last_error */
+} gwl_status;
+
+/* Create a context for N_v occupied, N_c empty orbitals and N_mu fitting points on the CURRENT CUDA
+ * device.  PAPER.md:39 (N_vc = N_v N_c), :117-120 (N_mu).  All sizes >= 1. */
+gwl_status gwl_create(gwl_ctx** out, int64_t n_v, int64_t n_c, int64_t n_mu);
+void gwl_destroy(gwl_ctx* ctx);                 /* NULL-safe; frees all device memory */
+const char* gwl_last_error(const gwl_ctx* ctx); /* "" if none; NULL-safe */
+
+gwl_status gwl_set_pointer_mode(gwl_ctx* ctx, int device_ptrs); /* 0 host (default), 1 device */
+/* Run all work on `cuda_stream` (a cudaStream_t / CUstream handle; NULL = the legacy default
+ * stream).  The stream stays owned by the caller and must outlive the context's use of it. */
+gwl_status gwl_set_stream(gwl_ctx* ctx, void* cuda_stream);
+
+/* Orbitals at the fitting points, PAPER.md:117-123 (C^mu_nm = phi_n(r_mu) phi_m(r_mu)).
+ * phi_v [n_mu][n_v], phi_c [n_mu][n_c], host. */
+gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi_c);
+/* Kohn-Sham energies.  eps_v [n_v], eps_c [n_c], host.
+ * GWL_EINVAL unless min(eps_c) > max(eps_v) (Delta > 0 is needed for (A-B)^{1/2}). */
+gwl_status gwl_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps_c);
+/* Two-centre integrals (alpha|beta), PAPER.md:125 (Eq. 17).  V [n_mu][n_mu], host, symmetric
+ * (only V itself is used; symmetry is the caller's responsibility). */
+gwl_status gwl_set_kernel(gwl_ctx* ctx, const double* V);
+/* Optional polynomial square root D ~ p_g(C).  cheb[g+1] are coefficients in
+ * the Chebyshev basis on [lo, hi]: p_g(x) = sum_j cheb[j] T_j((2x-hi-lo)/(hi-lo)).  g >= 1 switches
+ * gwl_lanczos to Op = p_g(C) and gwl_selfenergy to Eq. 12 + Eq. 14 ("poly mode"); g = 0 (cheb may be
+ * NULL) clears it: Op = C and gwl_selfenergy evaluates Eq. 11 on the Ritz pairs of T_L ("direct mode"). */
+gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo, double hi);
+
+/* y = C x for nvec vectors, PAPER.md:52 with the factorisation of PAPER.md:128, :383-389:
+ * y = Delta^2 o x + 2 sqrt(Delta) o K^T ( V ( K ( sqrt(Delta) o x ) ) ).  Always C, never p_g(C).
+ * x, y [nvec][n_v][n_c]; x and y must not overlap.  nvec >= 0 (0 is a no-op). */
+gwl_status gwl_casida_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec);
+
+/* Chains by orbital indices: chain j starts from |P_{n_j m_j}>.  An index in
+ * [0, n_v + n_c): < n_v is the occupied orbital of that number (eta_n = +1), otherwise the empty
+ * orbital idx - n_v (eta_n = -1).  eps_n and eta_n of PAPER.md:62, :79 are taken from n_idx.  Host arrays. */
+gwl_status gwl_set_chains(gwl_ctx* ctx, int64_t n_chains, const int32_t* n_idx, const int32_t* m_idx);
+/* Alternative: explicit start vectors p [n_chains][n_v][n_c] (pointer mode applies to p) with
+ * eps_n [n_chains], sgn_n [n_chains] (+1/-1), host. */
+gwl_status gwl_set_start_vectors(gwl_ctx* ctx, int64_t n_chains, const double* p,
+                                 const double* eps_n, const int32_t* sgn_n);
+
+/* Lanczos tridiagonalisation of Op (C, or p_g(C) in poly mode) for the first n_chains chains set
+ * above, `block` chains at a time (the last block may be short), PAPER.md:87-90 (Eq. 13).
+ * steps = number of Op applications = dimension of T_L.  reorth: 0 off, 1 two-pass full
+ * reorthogonalisation against all previous Lanczos vectors of the same chain.
+ * Outputs (may be NULL to skip; the context keeps its own copy for gwl_resolvent/gwl_selfenergy):
+ *   alpha [n_chains][steps]  a_0 .. a_{L-1}
+ *   beta  [n_chains][steps]  beta[k] = b_{k+1}; beta[steps-1] is returned but not part of T_L
+ *   norm2 [n_chains]         <P|P>
+ *   len   [n_chains]         effective length <= steps: on breakdown (b_{k+1} <= 1e-12 max_i(|a_i|+b_i))
+ *                            len = k+1, b_{k+1} is stored as 0 and the tail is zero-filled. */
+gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t block, int reorth,
+                       double* alpha, double* beta, double* norm2, int32_t* len);
+
+/* r[j][i] = <P_j|(zeta_i - Op)^{-1}|P_j> by Eq. 14 from the tridiagonals of the last
+ * gwl_lanczos: norm2 / (zeta - a_0 - b_1^2/(zeta - a_1 - ...)), truncated at len_j.
+ * zeta [n_zeta][2] (re, im); r [n_chains][n_zeta][2]. */
+gwl_status gwl_resolvent(gwl_ctx* ctx, const double* zeta, int64_t n_zeta, double* r);
+
+/* Sigma^corr_mm(omega, n_j) for every chain of the last gwl_lanczos, PAPER.md:77-83 (Eq. 11-12), with
+ * z_n = omega - eps_n - i eta_n eta (eta > 0 is the paper's delta), and optionally
+ * the sum over chains, PAPER.md:73 (Eq. 10).
+ * omega [n_omega]; sigma [n_chains][n_omega][2] (may be NULL); sigma_sum [n_omega][2] (may be NULL). */
+gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, double eta,
+                          double* sigma, double* sigma_sum);
+
+/* CUDA-event totals (ms) of the last gwl_lanczos: time inside Casida products (S2), inside the Lanczos
+ * vector kernels (S4) and overall.  Any pointer may be NULL.  Synchronises the stream. */
+gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total);
+
+/* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
+gwl_status gwl_get_launch_count(gwl_ctx* ctx, int64_t* n_launches);
+
+/* Measurement helper, not part of the method: run a register-resident mma.sync.m8n8k4.f64 (kind 0) or
+ * DFMA (kind 1) loop on every SM of the current device and return the achieved FP64 TFLOP/s.
+ * This is the denominator DESIGN.md uses for the FP64 tensor roofline. */
+gwl_status gwl_probe_fp64_peak(int kind, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GWL_H */

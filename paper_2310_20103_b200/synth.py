@@ -1,0 +1,139 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs.
+
+This module is INPUT GENERATION ONLY.  It holds none of the method's arithmetic
+(no Casida product, no Lanczos, no continued fraction) and imports neither the
+oracle nor the CUDA binding; the tests, bench.py and smoke() hand the very same
+host arrays to both sides.
+
+Recipe (BASELINE.json:configs): numpy.random.default_rng(seed),
+draw order r, Phi_v, Phi_c, eps_v, eps_c.
+  r_mu      uniform in a cube of side `box` (configs 0-3) or in a sphere of
+            DIAMETER `box` (config 4, reading Q16)
+  Phi_v/c   i.i.d. N(0,1)/sqrt(N_mu)       -- stand-ins for the orbitals at the
+            ISDF points; real orbitals are not in the container
+  eps_v     U[ev_lo, ev_hi], eps_c U[ec_lo, ec_hi], both sorted ascending (eV)
+  V         14.4 / sqrt(|r_mu - r_nu|^2 + 0.25) eV, stand-in for (alpha|beta),
+            PAPER.md:125 (Eq. 17); inverse multiquadric, positive definite
+  omega     uniform grid on [-20, 20] eV, broadening 0.1 eV (the paper's delta)
+  chains    (n, m) = {first a valence} x {first b conduction}, row-major (Q11);
+            orbital index in [0, N_v + N_c): < N_v valence, else conduction
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+
+@dataclass(frozen=True)
+class Config:
+    name: str
+    n_v: int
+    n_c: int
+    n_mu: int
+    box: float            # cube side or sphere diameter, Angstrom
+    sphere: bool
+    ev: tuple             # (lo, hi) of eps_v
+    ec: tuple             # (lo, hi) of eps_c
+    chains_a: int         # number of valence n
+    chains_b: int         # number of conduction m
+    block: int
+    steps: int
+    n_omega: int
+    omega_lo: float = -20.0
+    omega_hi: float = 20.0
+    eta: float = 0.1      # BASELINE's eta = the paper's delta (eV)
+
+    @property
+    def n_vc(self) -> int:
+        return self.n_v * self.n_c
+
+    @property
+    def n_chains(self) -> int:
+        return self.chains_a * self.chains_b
+
+    def flop_per_vector(self) -> float:
+        """F/B = 4 N_mu N_vc + 2 N_mu^2."""
+        return 4.0 * self.n_mu * self.n_vc + 2.0 * self.n_mu * self.n_mu
+
+
+CONFIGS = (
+    Config("cfg0_tiny", 8, 24, 192, 10.0, False, (-10.0, -5.0), (-3.0, 20.0), 2, 2, 4, 60, 201),
+    Config("cfg1_small_molecule", 64, 256, 1536, 15.0, False, (-10.0, -5.0), (-3.0, 20.0), 8, 8, 64, 200, 401),
+    Config("cfg2_100_atom_cluster", 256, 1024, 6144, 20.0, False, (-10.0, -5.0), (-3.0, 20.0), 16, 16, 256, 300, 401),
+    Config("cfg3_defect_cell", 512, 2048, 12288, 25.0, False, (-10.0, -5.0), (-3.0, 20.0), 16, 32, 256, 300, 401),
+    Config("cfg4_si_quantum_dot", 1024, 4096, 20480, 40.0, True, (-12.0, -4.0), (-2.0, 25.0), 16, 16, 128, 200, 801),
+)
+
+
+@dataclass
+class Problem:
+    cfg: Config
+    r: np.ndarray          # [n_mu, 3]
+    phi_v: np.ndarray      # [n_mu, n_v]
+    phi_c: np.ndarray      # [n_mu, n_c]
+    eps_v: np.ndarray      # [n_v]
+    eps_c: np.ndarray      # [n_c]
+    omega: np.ndarray      # [n_omega]
+    n_idx: np.ndarray      # [n_chains] int32
+    m_idx: np.ndarray      # [n_chains] int32
+    _V: np.ndarray | None = field(default=None, repr=False)
+
+    @property
+    def V(self) -> np.ndarray:
+        if self._V is None:
+            self._V = coulomb_kernel(self.r)
+        return self._V
+
+
+def coulomb_kernel(r: np.ndarray, row_chunk: int = 1024) -> np.ndarray:
+    """V[mu,nu] = 14.4 / sqrt(|r_mu - r_nu|^2 + 0.25), built in row chunks."""
+    n = r.shape[0]
+    V = np.empty((n, n), dtype=np.float64)
+    for i in range(0, n, row_chunk):
+        d = r[i:i + row_chunk, None, :] - r[None, :, :]
+        V[i:i + row_chunk] = 14.4 / np.sqrt(np.einsum("ijk,ijk->ij", d, d) + 0.25)
+    return V
+
+
+def chain_list(cfg: Config):
+    """(n, m) pairs of Q11: n over the first `a` valence, m over the first `b` conduction."""
+    n = np.repeat(np.arange(cfg.chains_a, dtype=np.int32), cfg.chains_b)
+    m = np.tile(np.arange(cfg.chains_b, dtype=np.int32), cfg.chains_a) + np.int32(cfg.n_v)
+    return n, m
+
+
+def make_problem(cfg: Config | int, seed: int = 0) -> Problem:
+    if isinstance(cfg, int):
+        cfg = CONFIGS[cfg]
+    rng = np.random.default_rng(seed)
+    if cfg.sphere:
+        # uniform in a ball of diameter `box`: R u^(1/3) times a unit vector
+        u = rng.random(cfg.n_mu)
+        g = rng.standard_normal((cfg.n_mu, 3))
+        g /= np.linalg.norm(g, axis=1, keepdims=True)
+        r = (0.5 * cfg.box) * np.cbrt(u)[:, None] * g
+    else:
+        r = rng.random((cfg.n_mu, 3)) * cfg.box
+    phi_v = rng.standard_normal((cfg.n_mu, cfg.n_v)) / np.sqrt(cfg.n_mu)
+    phi_c = rng.standard_normal((cfg.n_mu, cfg.n_c)) / np.sqrt(cfg.n_mu)
+    eps_v = np.sort(rng.uniform(cfg.ev[0], cfg.ev[1], cfg.n_v))
+    eps_c = np.sort(rng.uniform(cfg.ec[0], cfg.ec[1], cfg.n_c))
+    omega = np.linspace(cfg.omega_lo, cfg.omega_hi, cfg.n_omega)
+    n_idx, m_idx = chain_list(cfg)
+    return Problem(cfg, r, phi_v, phi_c, eps_v, eps_c, omega, n_idx, m_idx)
+
+
+def make_custom(n_v: int, n_c: int, n_mu: int, box: float = 10.0, seed: int = 0,
+                n_omega: int = 101, chains_a: int = 2, chains_b: int = 2,
+                steps: int = 20, block: int = 4) -> Problem:
+    """Same generators at arbitrary (ragged) sizes, for edge-case tests."""
+    cfg = Config(f"custom_{n_v}_{n_c}_{n_mu}", n_v, n_c, n_mu, box, False,
+                 (-10.0, -5.0), (-3.0, 20.0), chains_a, chains_b, block, steps, n_omega)
+    return make_problem(cfg, seed)
+
+
+def random_block(cfg: Config, nvec: int, seed: int = 1) -> np.ndarray:
+    """A seeded block of test vectors X[nvec][n_v][n_c] ~ N(0,1)."""
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((nvec, cfg.n_v, cfg.n_c))

@@ -1,0 +1,352 @@
+"""Pins for oracle/gw_oracle.py: every oracle function is checked
+against something other than itself -- the paper's defining equations evaluated by
+brute force or by a library eigen-solver, closed forms, and algebraic invariants.
+CPU only; runs in seconds on config 0 (N_vc = 192) and smaller inputs."""
+import numpy as np
+import pytest
+import scipy.linalg as sla
+
+from oracle import gw_oracle as orc
+from paper_2310_20103_b200 import synth
+
+DLT = 0.1
+
+
+@pytest.fixture(scope="module")
+def dense0(cfg0):
+    p = cfg0
+    delta = orc.delta_vc(p.eps_v, p.eps_c)
+    K = orc.khatri_rao(p.phi_v, p.phi_c)
+    Kt = orc.coupling_dense(K, p.V)
+    C = orc.casida_dense(delta, Kt)
+    lam, Z = sla.eigh(C)
+    return dict(delta=delta, K=K, Kt=Kt, C=C, lam=lam, Z=Z)
+
+
+def _tiny(seed=3, n_v=2, n_c=3, n_mu=5):
+    return synth.make_custom(n_v, n_c, n_mu, seed=seed)
+
+
+# ---- definitions by brute force ------------------------------------------------
+def test_delta_and_pair_index_bruteforce():
+    p = _tiny()
+    d = orc.delta_vc(p.eps_v, p.eps_c)
+    for v in range(2):
+        for c in range(3):
+            assert d[v * 3 + c] == p.eps_c[c] - p.eps_v[v]
+    assert d.min() > 0
+
+
+def test_coupling_bruteforce_eq16():
+    """(vc|v'c') = sum_ab C^a_vc (a|b) C^b_v'c' with C^mu_vc = phi_v phi_c: explicit loops. PAPER.md:122."""
+    p = _tiny()
+    K = orc.khatri_rao(p.phi_v, p.phi_c)
+    Kt = orc.coupling_dense(K, p.V)
+    n_v, n_c, n_mu = 2, 3, 5
+    for v in range(n_v):
+        for c in range(n_c):
+            for v2 in range(n_v):
+                for c2 in range(n_c):
+                    acc = 0.0
+                    for a in range(n_mu):
+                        for b in range(n_mu):
+                            acc += p.phi_v[a, v] * p.phi_c[a, c] * p.V[a, b] * p.phi_v[b, v2] * p.phi_c[b, c2]
+                    assert abs(Kt[v * n_c + c, v2 * n_c + c2] - acc) < 1e-13 * (1 + abs(acc))
+
+
+def test_start_vector_bruteforce():
+    """(P_nm)_vc = (nm|vc) sqrt(eps_c - eps_v), loops; covers valence and conduction n."""
+    p = _tiny()
+    d = orc.delta_vc(p.eps_v, p.eps_c)
+    for n_idx, m_idx in [(0, 2), (1, 4), (3, 1), (4, 4)]:
+        P = orc.start_vector(p.phi_v, p.phi_c, p.V, d, n_idx, m_idx)
+        phi_all = np.concatenate([p.phi_v, p.phi_c], axis=1)
+        for v in range(2):
+            for c in range(3):
+                acc = 0.0
+                for a in range(5):
+                    for b in range(5):
+                        acc += phi_all[a, n_idx] * phi_all[a, m_idx] * p.V[a, b] * p.phi_v[b, v] * p.phi_c[b, c]
+                ref = acc * np.sqrt(p.eps_c[c] - p.eps_v[v])
+                assert abs(P[v * 3 + c] - ref) < 1e-13 * (1 + abs(ref))
+    assert orc.orbital_energy_sign(p.eps_v, p.eps_c, 1) == (p.eps_v[1], 1)
+    assert orc.orbital_energy_sign(p.eps_v, p.eps_c, 3) == (p.eps_c[1], -1)
+
+
+# ---- P1-P4: the operator ---------------------------------------------------------
+def test_P1_symmetric_psd(dense0):
+    C, delta, lam = dense0["C"], dense0["delta"], dense0["lam"]
+    assert np.abs(C - C.T).max() <= 1e-13 * np.abs(C).max()
+    assert lam.min() > 0
+    assert lam.min() >= (delta ** 2).min() - 1e-9          # C >= diag(Delta^2) as V is PSD
+    rng = np.random.default_rng(5)
+    x, y = rng.standard_normal((2, C.shape[0]))
+    assert abs(x @ (C @ y) - y @ (C @ x)) <= 1e-12 * abs(x @ (C @ y))
+
+
+def test_P2_casida_eq1_spectrum(dense0):
+    """Positive eigenvalues of [[A,B],[-B,-A]] (Eq. 1) are sqrt(eig(C)) (Eq. 4); fails for Delta instead of Delta^2."""
+    A, B = orc.casida_AB(dense0["delta"], dense0["Kt"])
+    M = np.block([[A, B], [-B, -A]])
+    ev = sla.eigvals(M)
+    assert np.abs(ev.imag).max() < 1e-8
+    pos = np.sort(ev.real[ev.real > 0])
+    assert len(pos) == A.shape[0]
+    O = np.sqrt(dense0["lam"])
+    assert np.abs(pos - O).max() <= 1e-10 * O.max()
+    neg = np.sort(-ev.real[ev.real < 0])
+    assert np.abs(neg - O).max() <= 1e-10 * O.max()
+
+
+def test_P3_sqrtm_form(dense0):
+    A, B = orc.casida_AB(dense0["delta"], dense0["Kt"])
+    S = sla.sqrtm(A - B).real
+    C2 = S @ (A + B) @ S
+    assert np.abs(C2 - dense0["C"]).max() <= 1e-13 * np.abs(C2).max()
+
+
+def test_P4_factored_vs_dense(cfg0, dense0):
+    p, C, delta = cfg0, dense0["C"], dense0["delta"]
+    X = synth.random_block(p.cfg, 5).reshape(5, -1)
+    Y = orc.casida_matvec_factored(p.phi_v, p.phi_c, p.V, delta, X)
+    ref = X @ C
+    assert np.abs(Y - ref).max() <= 1e-13 * np.abs(ref).max()
+    # shape [nvec, n_v, n_c] accepted and preserved
+    Y3 = orc.casida_matvec_factored(p.phi_v, p.phi_c, p.V, delta, X.reshape(5, p.cfg.n_v, p.cfg.n_c))
+    assert Y3.shape == (5, p.cfg.n_v, p.cfg.n_c) and np.array_equal(Y3.reshape(5, -1), Y)
+    # per-v matmul loop form
+    yl = orc.casida_matvec_loop(p.phi_v, p.phi_c, p.V, delta, X[0])
+    assert np.abs(yl - ref[0]).max() <= 1e-13 * np.abs(ref).max()
+    # V = 0 -> Delta^2 o x exactly
+    Y0 = orc.casida_matvec_factored(p.phi_v, p.phi_c, np.zeros_like(p.V), delta, X)
+    assert np.array_equal(Y0, delta ** 2 * X)
+    # unit vectors give the columns of C
+    E = np.eye(C.shape[0])[[0, 7, 191]]
+    Ye = orc.casida_matvec_factored(p.phi_v, p.phi_c, p.V, delta, E)
+    assert np.abs(Ye - C[[0, 7, 191]]).max() <= 1e-13 * np.abs(C).max()
+
+
+# ---- P5: closed form N_v = N_c = 1 ------------------------------------------------
+def test_P5_one_by_one_closed_form():
+    p = synth.make_custom(1, 1, 7, seed=11)
+    delta = orc.delta_vc(p.eps_v, p.eps_c)
+    rho = p.phi_v[:, 0] * p.phi_c[:, 0]
+    k = rho @ p.V @ rho
+    Cs = delta[0] ** 2 + 2 * delta[0] * k
+    y = orc.casida_matvec_factored(p.phi_v, p.phi_c, p.V, delta, np.ones((1, 1)))
+    assert abs(y[0, 0] - Cs) <= 1e-14 * Cs
+    P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, 0, 1)      # (n,m) = (v0, c0)
+    assert abs(P[0] - k * np.sqrt(delta[0])) <= 1e-14 * abs(P[0])
+    a, b, n2, ln = orc.lanczos(lambda x: Cs * x, P, 3)
+    assert ln == 1 and abs(a[0] - Cs) <= 1e-14 * Cs and b[0] == 0.0
+    om = np.linspace(-20, 20, 9)
+    for n_idx in (0, 1):
+        eps_n, sgn = orc.orbital_energy_sign(p.eps_v, p.eps_c, n_idx)
+        sig = orc.sigma_direct(a, b, n2, ln, om, eps_n, sgn, DLT)
+        O = np.sqrt(Cs)
+        z = om - eps_n - 1j * sgn * DLT
+        ref = P[0] ** 2 * sgn / (O * (O + sgn * z))
+        assert np.abs(sig - ref).max() <= 1e-14 * np.abs(ref).max()
+
+
+# ---- P6-P7: Lanczos ---------------------------------------------------------------
+def test_P6_moments(cfg0, dense0):
+    C, delta, p = dense0["C"], dense0["delta"], cfg0
+    P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, 0, p.cfg.n_v)
+    L = 6
+    a, b, n2, ln = orc.lanczos(lambda x: C @ x, P, L)
+    T = orc.tridiagonal(a, b, ln)
+    s = P / np.sqrt(n2)
+    e1 = np.zeros(L); e1[0] = 1
+    v, t = s.copy(), e1.copy()
+    for k in range(2 * L):
+        assert abs(e1 @ t - s @ v) <= 1e-12 * abs(s @ v), k
+        v, t = C @ v, T @ t
+    # the first moment beyond 2L-1 must differ (the fraction is not exact)
+    assert abs(e1 @ t - s @ v) > 1e-10 * abs(s @ v)
+
+
+def test_P7_full_length_lanczos(cfg0, dense0):
+    C, delta, p = dense0["C"], dense0["delta"], cfg0
+    n = C.shape[0]
+    P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, 1, p.cfg.n_v + 1)
+    a, b, n2, ln, Q = orc.lanczos(lambda x: C @ x, P, n, reorth=True, return_basis=True)
+    assert ln == n
+    T = orc.tridiagonal(a, b, ln)
+    assert np.abs(Q @ Q.T - np.eye(n)).max() < 1e-12
+    assert np.abs(Q @ C @ Q.T - T).max() < 1e-9 * np.abs(C).max()
+    assert np.abs(np.sort(sla.eigvalsh(T)) - dense0["lam"]).max() < 1e-9 * dense0["lam"].max()
+    assert b[n - 1] < 1e-7 * np.abs(a).max()
+    assert abs(n2 - P @ P) == 0
+
+
+def test_lanczos_three_term_recurrence(cfg0, dense0):
+    """C q_k = b_k q_{k-1} + a_k q_k + b_{k+1} q_{k+1} and beta indexing beta[k] = b_{k+1} (Eq. 13, Q6)."""
+    C, delta, p = dense0["C"], dense0["delta"], cfg0
+    P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, 0, p.cfg.n_v + 1)
+    a, b, n2, ln, Q = orc.lanczos(lambda x: C @ x, P, 12, return_basis=True)
+    assert np.allclose(Q[0], P / np.linalg.norm(P), rtol=0, atol=1e-15)
+    for k in range(1, 11):
+        r = C @ Q[k] - b[k - 1] * Q[k - 1] - a[k] * Q[k] - b[k] * Q[k + 1]
+        assert np.abs(r).max() < 1e-10 * np.abs(a).max()
+    assert np.all(b[:12] > 0)
+
+
+def test_breakdown_invariant_subspace():
+    """Q9: a start vector inside a 3-dimensional invariant subspace stops after 3 steps."""
+    d = np.array([1.0, 2.0, 3.0, 4.0, 5.0, 6.0])
+    P = np.array([1.0, 0.0, 2.0, 0.0, 0.0, -1.0])
+    a, b, n2, ln = orc.lanczos(lambda x: d * x, P, 6)
+    assert ln == 3 and np.all(a[3:] == 0) and np.all(b[2:] == 0)
+    th, w = orc.ritz(a, b, ln)
+    assert np.allclose(th, [1.0, 3.0, 6.0], atol=1e-12)
+    assert np.allclose(w * n2, [1.0, 4.0, 1.0], atol=1e-12)
+
+
+# ---- P8, P11: continued fraction -------------------------------------------------------
+def test_P8_continued_fraction_vs_ritz_and_exact(cfg0, dense0):
+    C, delta, p, lam, Z = dense0["C"], dense0["delta"], cfg0, dense0["lam"], dense0["Z"]
+    P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, 0, p.cfg.n_v)
+    zeta = (np.linspace(-50, 900, 23) + 0.37j) ** 1
+    for L in (1, 2, 9, 40):
+        a, b, n2, ln = orc.lanczos(lambda x: C @ x, P, L, reorth=True)
+        th, w = orc.ritz(a, b, ln)
+        ref = n2 * (w[None, :] / (zeta[:, None] - th[None, :])).sum(axis=1)
+        got = orc.continued_fraction(a, b, n2, zeta, ln)
+        assert np.abs(got - ref).max() <= 1e-11 * np.abs(ref).max(), L
+    a, b, n2, ln = orc.lanczos(lambda x: C @ x, P, C.shape[0], reorth=True)
+    got = orc.continued_fraction(a, b, n2, zeta, ln)
+    ref = orc.resolvent_exact(lam, Z, P, zeta)
+    assert np.abs(got - ref).max() <= 1e-9 * np.abs(ref).max()
+    # asymptotics: zeta R(zeta) -> <P|P> (the norm factor of Q5)
+    big = np.array([1e9 + 1e9j])
+    assert abs(big[0] * orc.continued_fraction(a, b, n2, big, 30)[0] - n2) < 1e-5 * n2
+
+
+def test_P11_diagonal_operator_closed_form():
+    rng = np.random.default_rng(2)
+    d = rng.uniform(2.0, 9.0, 7) ** 2
+    s = rng.standard_normal(7)
+    a, b, n2, ln = orc.lanczos(lambda x: d * x, s, 7, reorth=True)
+    zeta = np.array([1.0 + 0.5j, -3.0 + 0.1j, 50.0 - 2.0j])
+    ref = (s[None, :] ** 2 / (zeta[:, None] - d[None, :])).sum(axis=1)
+    got = orc.continued_fraction(a, b, n2, zeta, ln)
+    assert np.abs(got - ref).max() <= 1e-10 * np.abs(ref).max()
+
+
+def test_continued_fraction_two_level_by_hand():
+    """L = 2 written out: n2 / (z - a0 - b1^2/(z - a1)); b_2 (beta[1]) must not enter (Q6, Q7)."""
+    a = np.array([2.0, 5.0]); b = np.array([0.7, 123.0]); z = np.array([1.0 + 1.0j])
+    ref = 3.0 / (z - 2.0 - 0.49 / (z - 5.0))
+    assert np.abs(orc.continued_fraction(a, b, 3.0, z) - ref).max() < 1e-15
+
+
+# ---- P9, P10: self-energy -------------------------------------------------------------
+def test_P9_eq7_eq11_eq12(cfg0, dense0):
+    C, delta, p, lam, Z = dense0["C"], dense0["delta"], cfg0, dense0["lam"], dense0["Z"]
+    om = p.omega
+    D = (Z * np.sqrt(lam)[None, :]) @ Z.T                       # exact D, D^2 = C
+    assert np.abs(D @ D - C).max() < 1e-10 * np.abs(C).max()
+    for n_idx, m_idx in [(0, p.cfg.n_v), (p.cfg.n_v + 2, p.cfg.n_v - 1)]:
+        P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, n_idx, m_idx)
+        eps_n, sgn = orc.orbital_energy_sign(p.eps_v, p.eps_c, n_idx)
+        s7 = orc.sigma_exact_eq7(lam, Z, P, om, eps_n, sgn, DLT)
+        s11 = orc.sigma_exact_eq11(lam, Z, P, om, eps_n, sgn, DLT)
+        assert np.abs(s7 - s11).max() < 1e-13
+        a, b, n2, ln = orc.lanczos(lambda x: D @ x, P, C.shape[0], reorth=True)
+        s12 = orc.sigma_poly(a, b, n2, ln, om, eps_n, sgn, DLT)
+        assert np.abs(s12 - s7).max() < 1e-11
+        # Herglotz: Im Sigma has the sign of sgn_n for every omega
+        assert np.all(sgn * s7.imag > 0)
+
+
+def test_P10_direct_mode_converges_to_eq7(cfg0, dense0):
+    C, delta, p, lam, Z = dense0["C"], dense0["delta"], cfg0, dense0["lam"], dense0["Z"]
+    for n_idx, m_idx in [(1, p.cfg.n_v + 1), (p.cfg.n_v, 0)]:
+        P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, n_idx, m_idx)
+        eps_n, sgn = orc.orbital_energy_sign(p.eps_v, p.eps_c, n_idx)
+        a, b, n2, ln = orc.lanczos(lambda x: C @ x, P, C.shape[0], reorth=True)
+        sd = orc.sigma_direct(a, b, n2, ln, p.omega, eps_n, sgn, DLT)
+        s7 = orc.sigma_exact_eq7(lam, Z, P, p.omega, eps_n, sgn, DLT)
+        assert np.abs(sd - s7).max() < 1e-11
+    # truncated: error decreases with L
+    P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, 0, p.cfg.n_v)
+    eps_n, sgn = orc.orbital_energy_sign(p.eps_v, p.eps_c, 0)
+    s7 = orc.sigma_exact_eq7(lam, Z, P, p.omega, eps_n, sgn, DLT)
+    errs = []
+    for L in (5, 20, 80):
+        a, b, n2, ln = orc.lanczos(lambda x: C @ x, P, L, reorth=True)
+        errs.append(np.abs(orc.sigma_direct(a, b, n2, ln, p.omega, eps_n, sgn, DLT) - s7).max())
+    assert errs[0] > errs[1] > errs[2]
+
+
+def test_sigma_sum_eq10():
+    s = np.arange(12).reshape(3, 4) * (1 + 2j)
+    assert np.array_equal(orc.sigma_sum(s), s[0] + s[1] + s[2])
+
+
+# ---- polynomial square root ------------------------------------------------------------
+def test_poly_matrix_function(cfg0, dense0):
+    """p_g(C) x = Z p_g(Omega^2) Z^T x, and the Q12 range contains the spectrum."""
+    C, delta, lam, Z = dense0["C"], dense0["delta"], dense0["lam"], dense0["Z"]
+    lo, hi = 0.8 * (delta ** 2).min(), 1.25 * (delta ** 2).max()
+    assert lo < lam.min() and lam.max() < hi
+    rng = np.random.default_rng(8)
+    x = rng.standard_normal(C.shape[0])
+    for g in (0, 1, 7, 8):
+        c = orc.fit_sqrt_chebyshev(g, lo, hi)
+        y = orc.poly_apply(lambda v: C @ v, c, lo, hi, x)
+        ref = Z @ (orc.poly_eval_scalar(c, lo, hi, lam) * (Z.T @ x))
+        assert np.abs(y - ref).max() <= 1e-11 * np.abs(ref).max(), g
+        # the scalar evaluator agrees with numpy's own Chebyshev evaluation
+        t = (2 * lam - (hi + lo)) / (hi - lo)
+        assert np.abs(orc.poly_eval_scalar(c, lo, hi, lam) - np.polynomial.chebyshev.chebval(t, c)).max() < 1e-12
+
+
+def test_P12_sqrt_fit_trend():
+    """the error grows with hi/lo and is largest near lo; g = 8 is already good on [0.1, 10]."""
+    errs = {}
+    for lo, hi in [(0.1, 10.0), (0.05, 20.0), (0.01, 100.0)]:
+        x = np.geomspace(lo, hi, 4001)
+        for g in (8, 18, 24):
+            c = orc.fit_sqrt_chebyshev(g, lo, hi)
+            e = np.abs(orc.poly_eval_scalar(c, lo, hi, x) - np.sqrt(x))
+            errs[(lo, g)] = e.max()
+            assert x[np.argmax(e)] < lo + 0.05 * (hi - lo)
+    assert errs[(0.1, 8)] < errs[(0.05, 8)] < errs[(0.01, 8)]
+    assert errs[(0.1, 8)] < 0.05
+    assert errs[(0.01, 24)] > 0.2 * errs[(0.01, 18)]       # no systematic improvement from 18 to 24
+
+
+def test_poly_mode_close_to_exact_on_narrow_spectrum():
+    """Poly mode (Eq. 12 + 14 on p_g(C)) approaches Eq. 7 when the fit is good."""
+    p = synth.make_custom(3, 4, 24, seed=4)
+    delta = orc.delta_vc(p.eps_v, p.eps_c)
+    K = orc.khatri_rao(p.phi_v, p.phi_c)
+    C = orc.casida_dense(delta, orc.coupling_dense(K, p.V))
+    lam, Z = sla.eigh(C)
+    lo, hi = 0.8 * (delta ** 2).min(), 1.25 * (delta ** 2).max()
+    c = orc.fit_sqrt_chebyshev(10, lo, hi)
+    P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, 0, 3)
+    eps_n, sgn = orc.orbital_energy_sign(p.eps_v, p.eps_c, 0)
+    a, b, n2, ln = orc.lanczos(lambda x: orc.poly_apply(lambda v: C @ v, c, lo, hi, x), P, 12, reorth=True)
+    s = orc.sigma_poly(a, b, n2, ln, p.omega, eps_n, sgn, DLT)
+    s7 = orc.sigma_exact_eq7(lam, Z, P, p.omega, eps_n, sgn, DLT)
+    fit_err = np.abs(orc.poly_eval_scalar(c, lo, hi, lam) - np.sqrt(lam)).max()
+    assert np.abs(s - s7).max() < 50 * fit_err * np.abs(s7).max() + 1e-12
+
+
+# ---- the whole path ---------------------------------------------------------------------
+def test_run_chains_config0(cfg0, dense0):
+    p = cfg0
+    out = orc.run_chains(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, p.n_idx, p.m_idx,
+                         30, p.omega, DLT, reorth=True)
+    C, delta = dense0["C"], dense0["delta"]
+    assert list(p.n_idx) == [0, 0, 1, 1] and list(p.m_idx) == [8, 9, 8, 9]       # Q11
+    for j in range(4):
+        P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, int(p.n_idx[j]), int(p.m_idx[j]))
+        a, b, n2, ln = orc.lanczos(lambda x: C @ x, P, 30, reorth=True)
+        assert np.abs(out["alpha"][j] - a).max() <= 1e-10 * np.abs(a).max()
+        assert np.abs(out["beta"][j] - b).max() <= 1e-10 * np.abs(a).max()
+        assert abs(out["norm2"][j] - n2) <= 1e-13 * n2
+    assert np.abs(out["sigma_sum"] - out["sigma"].sum(axis=0)).max() == 0
