@@ -1,0 +1,778 @@
+// C ABI of libgwl (include/gwl.h): context, input staging, and the host driver that strings the kernels
+// together.  There is no host<->device traffic and no host synchronisation inside the Lanczos step loop:
+// alpha/beta/len live on the device and are copied out once at the end.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "gwl_internal.h"
+
+using namespace gwl;
+
+namespace {
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t bytes = 0;
+    cudaError_t ensure(size_t need, cudaStream_t st) {
+        if (need <= bytes && p != nullptr) return cudaSuccess;
+        if (p) {
+            cudaError_t e0 = cudaStreamSynchronize(st);
+            if (e0 != cudaSuccess) return e0;
+            cudaFree(p);
+            p = nullptr;
+            bytes = 0;
+        }
+        if (need == 0) need = 8;
+        cudaError_t e = cudaMalloc(&p, need);
+        if (e != cudaSuccess) {
+            p = nullptr;
+            return e;
+        }
+        bytes = need;
+        return cudaMemsetAsync(p, 0, need, st);
+    }
+    void release() {
+        if (p) cudaFree(p);
+        p = nullptr;
+        bytes = 0;
+    }
+    template <class T>
+    T* as() const {
+        return static_cast<T*>(p);
+    }
+};
+
+}  // namespace
+
+struct gwl_ctx {
+    int n_v = 0, n_c = 0, n_mu = 0;
+    int64_t n_vc = 0;
+    int n_cp = 0, n_mup = 0;
+    int n_sm = 148;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int device_ptrs = 0;
+    std::string err;
+    int64_t launches = 0;
+
+    bool have_orb = false, have_eps = false, have_V = false;
+    DevBuf phi_c, phi_cT, phi_vT, V, eps_v, eps_c, d2, s;
+    std::vector<double> h_eps_v, h_eps_c;
+
+    int g = 0;
+    std::vector<double> cheb;
+    double lo = 0.0, hi = 0.0;
+
+    int chain_mode = 0;  // 0 none, 1 indices, 2 explicit vectors
+    int64_t n_chains_set = 0;
+    DevBuf d_nidx, d_midx, d_start, d_eps_n, d_sgn_n;
+
+    // results of the last gwl_lanczos
+    int64_t run_chains = 0;
+    int run_steps = 0;
+    int run_poly = 0;
+    DevBuf alpha, beta, norm2, len, scale, alive;
+
+    // workspaces
+    DevBuf xs, T, W, part, dotpart, normpart, basis, coefpart, tA, tB, tC, u;
+    DevBuf theta, wgt, ritz_info, d_omega, d_zeta, d_sigma, d_sigsum, io_x, io_y;
+
+    // timing
+    std::vector<cudaEvent_t> ev;
+    size_t ev_used = 0;
+    std::vector<size_t> ev_marks;  // triples: op start, op end, step end
+
+    gwl_status fail(gwl_status st, const std::string& msg) {
+        err = msg;
+        return st;
+    }
+    gwl_status cuda_fail(cudaError_t e, const char* where) {
+        err = std::string(where) + ": " + cudaGetErrorString(e);
+        return e == cudaErrorMemoryAllocation ? GWL_ENOMEM : GWL_ECUDA;
+    }
+    cudaEvent_t next_event() {
+        if (ev_used == ev.size()) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            ev.push_back(e);
+        }
+        return ev[ev_used++];
+    }
+};
+
+#define CK(call)                                                  \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return ctx->cuda_fail(e__, #call); \
+    } while (0)
+
+namespace {
+
+struct LaunchScope {
+    explicit LaunchScope(gwl_ctx* c) { g_launch_counter = &c->launches; }
+    ~LaunchScope() { g_launch_counter = nullptr; }
+};
+
+gwl_status ensure_workspace(gwl_ctx* ctx, int nb) {
+    cudaStream_t st = ctx->stream;
+    const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
+    CK(ctx->xs.ensure((size_t)nb * ldxs * 8, st));
+    CK(ctx->T.ensure((size_t)nb * ctx->n_mup * 8, st));
+    CK(ctx->W.ensure((size_t)nb * ctx->n_mup * 8, st));
+    const int kt_f = ctx->n_v * (ctx->n_cp / BK), kt_v = ctx->n_mup / BK;
+    const GemmPlan pf = plan_gemm(MODE_FWD, ctx->n_mu, nb, kt_f, ctx->n_cp / BK, ctx->n_sm);
+    const GemmPlan pv = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
+    const int smax = std::max(pf.splits, pv.splits);
+    CK(ctx->part.ensure((size_t)smax * nb * ctx->n_mup * 8, st));
+    const int npart = vec_parts(ctx->n_vc);
+    const int64_t ndot = std::max<int64_t>((int64_t)ctx->n_v * ceil_div(ctx->n_c, 128), npart);
+    CK(ctx->dotpart.ensure((size_t)nb * ndot * 8, st));
+    CK(ctx->normpart.ensure((size_t)nb * npart * 8, st));
+    return GWL_OK;
+}
+
+// T[b][mu] <- K (xs);  W <- V T;  then the K^T product with the requested epilogue.
+// xs must already hold sqrt(Delta) o x in the padded [nb][n_v][n_cp] layout.
+gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64_t ldy, int nb,
+                             double* dotpart, int dot_stride) {
+    cudaStream_t st = ctx->stream;
+    const int kt_c = ctx->n_cp / BK, kt_f = ctx->n_v * kt_c, kt_v = ctx->n_mup / BK;
+    const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
+    const int64_t ldm = ctx->n_mup;
+    {
+        GemmPlan pl = plan_gemm(MODE_FWD, ctx->n_mu, nb, kt_f, kt_c, ctx->n_sm);
+        GemmParams p{};
+        p.A = ctx->phi_c.as<double>();
+        p.lda = ctx->n_cp;
+        p.B = ctx->xs.as<double>();
+        p.ldb = ldxs;
+        p.M = ctx->n_mu;
+        p.N = nb;
+        p.kt_total = kt_f;
+        p.a_wrap = kt_c;
+        p.kt_per_split = pl.kt_per_split;
+        p.scale = ctx->phi_vT.as<double>();
+        p.lds = ldm;
+        if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
+        p.out = pl.splits == 1 ? ctx->T.as<double>() : ctx->part.as<double>();
+        p.ldo = ldm;
+        p.out_split_stride = (int64_t)nb * ldm;
+        CK(launch_gemm(MODE_FWD, EPI_STORE, pl, p, pl.splits, st));
+        if (pl.splits > 1)
+            CK(launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->T.as<double>(), ldm,
+                                    ctx->n_mu, nb, st));
+    }
+    {
+        GemmPlan pl = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
+        GemmParams p{};
+        p.A = ctx->V.as<double>();
+        p.lda = ldm;
+        p.B = ctx->T.as<double>();
+        p.ldb = ldm;
+        p.M = ctx->n_mu;
+        p.N = nb;
+        p.kt_total = kt_v;
+        p.a_wrap = kt_v;
+        p.kt_per_split = pl.kt_per_split;
+        if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
+        p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
+        p.ldo = ldm;
+        p.out_split_stride = (int64_t)nb * ldm;
+        CK(launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
+        if (pl.splits > 1)
+            CK(launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
+                                    ctx->n_mu, nb, st));
+    }
+    {
+        GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, kt_v, kt_v, ctx->n_sm);
+        GemmParams p{};
+        p.A = ctx->phi_cT.as<double>();
+        p.lda = ldm;
+        p.B = ctx->W.as<double>();
+        p.ldb = ldm;
+        p.M = ctx->n_c;
+        p.N = nb;
+        p.kt_total = kt_v;
+        p.a_wrap = kt_v;
+        p.kt_per_split = kt_v;
+        p.scale = ctx->phi_vT.as<double>();
+        p.lds = ldm;
+        p.out = y;
+        p.ldo = ldy;
+        p.X = x;
+        p.ldx = ldx;
+        p.d2 = ctx->d2.as<double>();
+        p.s = ctx->s.as<double>();
+        p.dotpart = dotpart;
+        p.dot_stride = dot_stride;
+        p.n_c = ctx->n_c;
+        CK(launch_gemm(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, pl, p, ctx->n_v, st));
+    }
+    return GWL_OK;
+}
+
+int casida_ndot(const gwl_ctx* ctx) { return ctx->n_v * (int)ceil_div(ctx->n_c, 128); }
+
+// S1: P_j = sqrt(Delta) o K^T (V rho_j) for index chains j0..j0+nb; writes P and sum(P^2) partials.
+gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, double* normpart, int dot_stride) {
+    cudaStream_t st = ctx->stream;
+    const int64_t ldm = ctx->n_mup;
+    const int kt_v = ctx->n_mup / BK;
+    CK(launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
+                  ctx->d_nidx.as<int32_t>() + j0, ctx->d_midx.as<int32_t>() + j0, ctx->T.as<double>(), ldm, nb, st));
+    {
+        GemmPlan pl = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
+        GemmParams p{};
+        p.A = ctx->V.as<double>();
+        p.lda = ldm;
+        p.B = ctx->T.as<double>();
+        p.ldb = ldm;
+        p.M = ctx->n_mu;
+        p.N = nb;
+        p.kt_total = kt_v;
+        p.a_wrap = kt_v;
+        p.kt_per_split = pl.kt_per_split;
+        if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
+        p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
+        p.ldo = ldm;
+        p.out_split_stride = (int64_t)nb * ldm;
+        CK(launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
+        if (pl.splits > 1)
+            CK(launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
+                                    ctx->n_mu, nb, st));
+    }
+    {
+        GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, kt_v, kt_v, ctx->n_sm);
+        GemmParams p{};
+        p.A = ctx->phi_cT.as<double>();
+        p.lda = ldm;
+        p.B = ctx->W.as<double>();
+        p.ldb = ldm;
+        p.M = ctx->n_c;
+        p.N = nb;
+        p.kt_total = kt_v;
+        p.a_wrap = kt_v;
+        p.kt_per_split = kt_v;
+        p.scale = ctx->phi_vT.as<double>();
+        p.lds = ldm;
+        p.out = P;
+        p.ldo = ctx->n_vc;
+        p.X = nullptr;
+        p.ldx = ctx->n_vc;
+        p.d2 = ctx->d2.as<double>();
+        p.s = ctx->s.as<double>();
+        p.dotpart = normpart;
+        p.dot_stride = dot_stride;
+        p.n_c = ctx->n_c;
+        CK(launch_gemm(MODE_BWD, EPI_START, pl, p, ctx->n_v, st));
+    }
+    return GWL_OK;
+}
+
+bool ready(const gwl_ctx* ctx) { return ctx->have_orb && ctx->have_eps && ctx->have_V; }
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+gwl_status gwl_create(gwl_ctx** out, int64_t n_v, int64_t n_c, int64_t n_mu) {
+    if (out == nullptr) return GWL_EINVAL;
+    *out = nullptr;
+    if (n_v < 1 || n_c < 1 || n_mu < 1 || n_v > (1 << 20) || n_c > (1 << 20) || n_mu > (1 << 24)) return GWL_EINVAL;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return GWL_ECUDA;
+    }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return GWL_ECUDA;
+    }
+    gwl_ctx* ctx = new (std::nothrow) gwl_ctx();
+    if (ctx == nullptr) return GWL_ENOMEM;
+    ctx->n_v = (int)n_v;
+    ctx->n_c = (int)n_c;
+    ctx->n_mu = (int)n_mu;
+    ctx->n_vc = n_v * n_c;
+    ctx->n_cp = (int)round_up(n_c, BK);
+    ctx->n_mup = (int)round_up(n_mu, BK);
+    ctx->n_sm = prop.multiProcessorCount;
+    ctx->device = dev;
+    *out = ctx;
+    return GWL_OK;
+}
+
+void gwl_destroy(gwl_ctx* ctx) {
+    if (ctx == nullptr) return;
+    cudaStreamSynchronize(ctx->stream);
+    DevBuf* bufs[] = {&ctx->phi_c, &ctx->phi_cT, &ctx->phi_vT, &ctx->V, &ctx->eps_v, &ctx->eps_c, &ctx->d2, &ctx->s,
+                      &ctx->d_nidx, &ctx->d_midx, &ctx->d_start, &ctx->d_eps_n, &ctx->d_sgn_n, &ctx->alpha,
+                      &ctx->beta, &ctx->norm2, &ctx->len, &ctx->scale, &ctx->alive, &ctx->xs, &ctx->T, &ctx->W,
+                      &ctx->part, &ctx->dotpart, &ctx->normpart, &ctx->basis, &ctx->coefpart, &ctx->tA, &ctx->tB,
+                      &ctx->tC, &ctx->u, &ctx->theta, &ctx->wgt, &ctx->ritz_info, &ctx->d_omega, &ctx->d_zeta,
+                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y};
+    for (DevBuf* b : bufs) b->release();
+    for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    delete ctx;
+}
+
+const char* gwl_last_error(const gwl_ctx* ctx) { return ctx ? ctx->err.c_str() : ""; }
+
+gwl_status gwl_set_pointer_mode(gwl_ctx* ctx, int device_ptrs) {
+    if (ctx == nullptr || (device_ptrs != 0 && device_ptrs != 1)) return GWL_EINVAL;
+    ctx->device_ptrs = device_ptrs;
+    return GWL_OK;
+}
+
+gwl_status gwl_set_stream(gwl_ctx* ctx, void* cuda_stream) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    return GWL_OK;
+}
+
+gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi_c) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (phi_v == nullptr || phi_c == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_orbitals: NULL input");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const size_t nv = (size_t)ctx->n_mu * ctx->n_v, nc = (size_t)ctx->n_mu * ctx->n_c;
+    DevBuf tmp;
+    CK(tmp.ensure(std::max(nv, nc) * 8, st));
+    CK(ctx->phi_c.ensure((size_t)ctx->n_mu * ctx->n_cp * 8, st));
+    CK(ctx->phi_cT.ensure((size_t)ctx->n_c * ctx->n_mup * 8, st));
+    CK(ctx->phi_vT.ensure((size_t)ctx->n_v * ctx->n_mup * 8, st));
+    CK(cudaMemsetAsync(ctx->phi_c.p, 0, ctx->phi_c.bytes, st));
+    CK(cudaMemsetAsync(ctx->phi_cT.p, 0, ctx->phi_cT.bytes, st));
+    CK(cudaMemsetAsync(ctx->phi_vT.p, 0, ctx->phi_vT.bytes, st));
+    CK(cudaMemcpyAsync(tmp.p, phi_c, nc * 8, cudaMemcpyHostToDevice, st));
+    CK(launch_copy_pad(tmp.as<double>(), ctx->n_mu, ctx->n_c, ctx->phi_c.as<double>(), ctx->n_cp, st));
+    CK(launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_c, ctx->phi_cT.as<double>(), ctx->n_mup, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaMemcpyAsync(tmp.p, phi_v, nv * 8, cudaMemcpyHostToDevice, st));
+    CK(launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_v, ctx->phi_vT.as<double>(), ctx->n_mup, st));
+    CK(cudaStreamSynchronize(st));
+    tmp.release();
+    ctx->have_orb = true;
+    return GWL_OK;
+}
+
+gwl_status gwl_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps_c) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (eps_v == nullptr || eps_c == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_energies: NULL input");
+    double vmax = -INFINITY, cmin = INFINITY;
+    for (int i = 0; i < ctx->n_v; ++i) {
+        if (!std::isfinite(eps_v[i])) return ctx->fail(GWL_EINVAL, "gwl_set_energies: non-finite eps_v");
+        vmax = std::max(vmax, eps_v[i]);
+    }
+    for (int i = 0; i < ctx->n_c; ++i) {
+        if (!std::isfinite(eps_c[i])) return ctx->fail(GWL_EINVAL, "gwl_set_energies: non-finite eps_c");
+        cmin = std::min(cmin, eps_c[i]);
+    }
+    if (!(cmin > vmax)) return ctx->fail(GWL_EINVAL, "gwl_set_energies: need min(eps_c) > max(eps_v)");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    ctx->h_eps_v.assign(eps_v, eps_v + ctx->n_v);
+    ctx->h_eps_c.assign(eps_c, eps_c + ctx->n_c);
+    CK(ctx->eps_v.ensure((size_t)ctx->n_v * 8, st));
+    CK(ctx->eps_c.ensure((size_t)ctx->n_c * 8, st));
+    CK(ctx->d2.ensure((size_t)ctx->n_vc * 8, st));
+    CK(ctx->s.ensure((size_t)ctx->n_vc * 8, st));
+    CK(cudaMemcpyAsync(ctx->eps_v.p, eps_v, (size_t)ctx->n_v * 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctx->eps_c.p, eps_c, (size_t)ctx->n_c * 8, cudaMemcpyHostToDevice, st));
+    CK(launch_build_delta(ctx->eps_v.as<double>(), ctx->eps_c.as<double>(), ctx->n_v, ctx->n_c, ctx->d2.as<double>(),
+                          ctx->s.as<double>(), st));
+    CK(cudaStreamSynchronize(st));
+    ctx->have_eps = true;
+    return GWL_OK;
+}
+
+gwl_status gwl_set_kernel(gwl_ctx* ctx, const double* V) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (V == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_kernel: NULL input");
+    cudaStream_t st = ctx->stream;
+    CK(ctx->V.ensure((size_t)ctx->n_mu * ctx->n_mup * 8, st));
+    CK(cudaMemsetAsync(ctx->V.p, 0, ctx->V.bytes, st));
+    CK(cudaMemcpy2DAsync(ctx->V.p, (size_t)ctx->n_mup * 8, V, (size_t)ctx->n_mu * 8, (size_t)ctx->n_mu * 8,
+                         (size_t)ctx->n_mu, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    ctx->have_V = true;
+    return GWL_OK;
+}
+
+gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo, double hi) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (g < 0 || g > 64) return ctx->fail(GWL_EINVAL, "gwl_set_polynomial: g out of range [0, 64]");
+    if (g == 0) {
+        ctx->g = 0;
+        ctx->cheb.clear();
+        return GWL_OK;
+    }
+    if (cheb == nullptr || !(hi > lo) || !std::isfinite(lo) || !std::isfinite(hi))
+        return ctx->fail(GWL_EINVAL, "gwl_set_polynomial: need cheb != NULL and hi > lo");
+    ctx->g = g;
+    ctx->cheb.assign(cheb, cheb + g + 1);
+    ctx->lo = lo;
+    ctx->hi = hi;
+    return GWL_OK;
+}
+
+gwl_status gwl_casida_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (nvec < 0) return ctx->fail(GWL_EINVAL, "gwl_casida_matvec: nvec < 0");
+    if (nvec == 0) return GWL_OK;
+    if (x == nullptr || y == nullptr) return ctx->fail(GWL_EINVAL, "gwl_casida_matvec: NULL vector");
+    if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_casida_matvec: orbitals, energies and kernel must be set");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int chunk = (int)std::min<int64_t>(nvec, 256);
+    gwl_status rs = ensure_workspace(ctx, chunk);
+    if (rs != GWL_OK) return rs;
+    const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
+    if (!ctx->device_ptrs) {
+        CK(ctx->io_x.ensure((size_t)chunk * ctx->n_vc * 8, st));
+        CK(ctx->io_y.ensure((size_t)chunk * ctx->n_vc * 8, st));
+    }
+    for (int64_t j0 = 0; j0 < nvec; j0 += chunk) {
+        const int nb = (int)std::min<int64_t>(chunk, nvec - j0);
+        const double* xd;
+        double* yd;
+        if (ctx->device_ptrs) {
+            xd = x + j0 * ctx->n_vc;
+            yd = y + j0 * ctx->n_vc;
+        } else {
+            CK(cudaMemcpyAsync(ctx->io_x.p, x + j0 * ctx->n_vc, (size_t)nb * ctx->n_vc * 8, cudaMemcpyHostToDevice, st));
+            xd = ctx->io_x.as<double>();
+            yd = ctx->io_y.as<double>();
+        }
+        CK(launch_prescale(xd, ctx->n_vc, ctx->xs.as<double>(), ldxs, ctx->s.as<double>(), ctx->n_v, ctx->n_c,
+                           ctx->n_cp, nb, st));
+        rs = apply_casida_core(ctx, xd, ctx->n_vc, yd, ctx->n_vc, nb, nullptr, 0);
+        if (rs != GWL_OK) return rs;
+        if (!ctx->device_ptrs) {
+            CK(cudaMemcpyAsync(y + j0 * ctx->n_vc, yd, (size_t)nb * ctx->n_vc * 8, cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+        }
+    }
+    return GWL_OK;
+}
+
+gwl_status gwl_set_chains(gwl_ctx* ctx, int64_t n_chains, const int32_t* n_idx, const int32_t* m_idx) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (n_chains < 0 || (n_chains > 0 && (n_idx == nullptr || m_idx == nullptr)))
+        return ctx->fail(GWL_EINVAL, "gwl_set_chains: bad arguments");
+    if (!ctx->have_eps) return ctx->fail(GWL_ESTATE, "gwl_set_chains: energies must be set first");
+    const int n_orb = ctx->n_v + ctx->n_c;
+    std::vector<double> eps(n_chains);
+    std::vector<int32_t> sgn(n_chains);
+    for (int64_t j = 0; j < n_chains; ++j) {
+        if (n_idx[j] < 0 || n_idx[j] >= n_orb || m_idx[j] < 0 || m_idx[j] >= n_orb)
+            return ctx->fail(GWL_EINVAL, "gwl_set_chains: orbital index out of range");
+        const bool occ = n_idx[j] < ctx->n_v;
+        eps[j] = occ ? ctx->h_eps_v[n_idx[j]] : ctx->h_eps_c[n_idx[j] - ctx->n_v];
+        sgn[j] = occ ? 1 : -1;
+    }
+    cudaStream_t st = ctx->stream;
+    CK(ctx->d_nidx.ensure((size_t)n_chains * 4, st));
+    CK(ctx->d_midx.ensure((size_t)n_chains * 4, st));
+    CK(ctx->d_eps_n.ensure((size_t)n_chains * 8, st));
+    CK(ctx->d_sgn_n.ensure((size_t)n_chains * 4, st));
+    if (n_chains > 0) {
+        CK(cudaMemcpyAsync(ctx->d_nidx.p, n_idx, (size_t)n_chains * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->d_midx.p, m_idx, (size_t)n_chains * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->d_eps_n.p, eps.data(), (size_t)n_chains * 8, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->d_sgn_n.p, sgn.data(), (size_t)n_chains * 4, cudaMemcpyHostToDevice, st));
+    }
+    CK(cudaStreamSynchronize(st));
+    ctx->chain_mode = 1;
+    ctx->n_chains_set = n_chains;
+    ctx->run_chains = 0;
+    return GWL_OK;
+}
+
+gwl_status gwl_set_start_vectors(gwl_ctx* ctx, int64_t n_chains, const double* p, const double* eps_n,
+                                 const int32_t* sgn_n) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (n_chains < 0 || (n_chains > 0 && (p == nullptr || eps_n == nullptr || sgn_n == nullptr)))
+        return ctx->fail(GWL_EINVAL, "gwl_set_start_vectors: bad arguments");
+    for (int64_t j = 0; j < n_chains; ++j)
+        if (sgn_n[j] != 1 && sgn_n[j] != -1) return ctx->fail(GWL_EINVAL, "gwl_set_start_vectors: sgn_n must be +1/-1");
+    cudaStream_t st = ctx->stream;
+    CK(ctx->d_start.ensure((size_t)n_chains * ctx->n_vc * 8, st));
+    CK(ctx->d_eps_n.ensure((size_t)n_chains * 8, st));
+    CK(ctx->d_sgn_n.ensure((size_t)n_chains * 4, st));
+    if (n_chains > 0) {
+        CK(cudaMemcpyAsync(ctx->d_start.p, p, (size_t)n_chains * ctx->n_vc * 8,
+                           ctx->device_ptrs ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->d_eps_n.p, eps_n, (size_t)n_chains * 8, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->d_sgn_n.p, sgn_n, (size_t)n_chains * 4, cudaMemcpyHostToDevice, st));
+    }
+    CK(cudaStreamSynchronize(st));
+    ctx->chain_mode = 2;
+    ctx->n_chains_set = n_chains;
+    ctx->run_chains = 0;
+    return GWL_OK;
+}
+
+gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t block, int reorth, double* alpha,
+                       double* beta, double* norm2, int32_t* len) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (n_chains < 0 || steps < 1 || steps > 100000 || block < 1 || (reorth != 0 && reorth != 1))
+        return ctx->fail(GWL_EINVAL, "gwl_lanczos: bad arguments");
+    if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_lanczos: orbitals, energies and kernel must be set");
+    if (ctx->chain_mode == 0) return ctx->fail(GWL_ESTATE, "gwl_lanczos: no chains set");
+    if (n_chains > ctx->n_chains_set) return ctx->fail(GWL_EINVAL, "gwl_lanczos: more chains than were set");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int L = (int)steps;
+    const int nbmax = (int)std::min<int64_t>(block, std::max<int64_t>(n_chains, 1));
+    const int64_t n_vc = ctx->n_vc;
+    const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
+    const int npart = vec_parts(n_vc);
+    const bool poly = ctx->g > 0;
+
+    ctx->run_chains = 0;
+    ctx->ev_used = 0;
+    ctx->ev_marks.clear();
+    CK(ctx->alpha.ensure((size_t)std::max<int64_t>(n_chains, 1) * L * 8, st));
+    CK(ctx->beta.ensure((size_t)std::max<int64_t>(n_chains, 1) * L * 8, st));
+    CK(ctx->norm2.ensure((size_t)std::max<int64_t>(n_chains, 1) * 8, st));
+    CK(ctx->len.ensure((size_t)std::max<int64_t>(n_chains, 1) * 4, st));
+    CK(cudaMemsetAsync(ctx->alpha.p, 0, ctx->alpha.bytes, st));
+    CK(cudaMemsetAsync(ctx->beta.p, 0, ctx->beta.bytes, st));
+    if (n_chains > 0) {
+        gwl_status rs = ensure_workspace(ctx, nbmax);
+        if (rs != GWL_OK) return rs;
+        CK(ctx->scale.ensure((size_t)2 * nbmax * 8, st));
+        CK(ctx->alive.ensure((size_t)2 * nbmax * 4, st));
+        const int nslots = reorth ? L + 1 : 3;
+        CK(ctx->basis.ensure((size_t)nslots * nbmax * n_vc * 8, st));
+        if (reorth) CK(ctx->coefpart.ensure((size_t)nbmax * L * npart * 8, st));
+        if (poly) {
+            CK(ctx->tA.ensure((size_t)nbmax * n_vc * 8, st));
+            CK(ctx->tB.ensure((size_t)nbmax * n_vc * 8, st));
+            CK(ctx->tC.ensure((size_t)nbmax * n_vc * 8, st));
+            CK(ctx->u.ensure((size_t)nbmax * n_vc * 8, st));
+        }
+    }
+    const int ndot_c = casida_ndot(ctx);
+
+    for (int64_t j0 = 0; j0 < n_chains; j0 += nbmax) {
+        const int nb = (int)std::min<int64_t>(nbmax, n_chains - j0);
+        const int64_t slot_stride = (int64_t)nb * n_vc;
+        double* basis = ctx->basis.as<double>();
+        auto slot = [&](int k) -> double* { return basis + (int64_t)(reorth ? k : ((k % 3) + 3) % 3) * slot_stride; };
+        LanczosState S;
+        S.alpha = ctx->alpha.as<double>() + j0 * L;
+        S.beta = ctx->beta.as<double>() + j0 * L;
+        S.norm2 = ctx->norm2.as<double>() + j0;
+        S.len = ctx->len.as<int32_t>() + j0;
+        S.scale = ctx->scale.as<double>();
+        S.alive = ctx->alive.as<int32_t>();
+        S.steps = L;
+        double* dotpart = ctx->dotpart.as<double>();
+        double* normpart = ctx->normpart.as<double>();
+
+        // ---- S1: start vectors into slot 0 ----
+        if (ctx->chain_mode == 1) {
+            gwl_status rs = build_start_vectors(ctx, j0, nb, slot(0), dotpart, ndot_c);
+            if (rs != GWL_OK) return rs;
+            CK(launch_lanczos_init(slot(0), n_vc, nb, dotpart, ndot_c, S, ctx->xs.as<double>(), ldxs,
+                                   ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
+        } else {
+            CK(cudaMemcpyAsync(slot(0), ctx->d_start.as<double>() + j0 * n_vc, (size_t)nb * n_vc * 8,
+                               cudaMemcpyDeviceToDevice, st));
+            CK(launch_dot_partials(slot(0), slot(0), n_vc, n_vc, nb, normpart, npart, st));
+            CK(launch_lanczos_init(slot(0), n_vc, nb, normpart, npart, S, ctx->xs.as<double>(), ldxs,
+                                   ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
+        }
+
+        // ---- S2-S4: the step loop; nothing below touches the host ----
+        for (int k = 0; k < L; ++k) {
+            double* q = slot(k);
+            double* w = slot(k + 1);
+            const double* qp = k > 0 ? slot(k - 1) : nullptr;
+            cudaEvent_t e0 = ctx->next_event(), e1 = ctx->next_event(), e2 = ctx->next_event();
+            CK(cudaEventRecord(e0, st));
+            int ndot, dstride;
+            if (!poly) {
+                gwl_status rs = apply_casida_core(ctx, q, n_vc, w, n_vc, nb, dotpart, ndot_c);
+                if (rs != GWL_OK) return rs;
+                ndot = ndot_c;
+                dstride = ndot_c;
+            } else {
+                // w = p_g(C) q by the Chebyshev three-term recurrence on Ct = (2C - (hi+lo))/(hi-lo)
+                const double hl = ctx->hi - ctx->lo, hs = ctx->hi + ctx->lo;
+                const int64_t ntot = (int64_t)nb * n_vc;
+                double* u = ctx->u.as<double>();
+                double* tb[3] = {ctx->tA.as<double>(), ctx->tB.as<double>(), ctx->tC.as<double>()};
+                gwl_status rs = apply_casida_core(ctx, q, n_vc, u, n_vc, nb, nullptr, 0);  // xs = s o q is ready
+                if (rs != GWL_OK) return rs;
+                const double* t0 = q;
+                double* t1 = tb[0];
+                CK(launch_axpby3(t1, 2.0 / hl, u, -hs / hl, q, 0.0, nullptr, ntot, st));
+                CK(launch_axpby3(w, ctx->cheb[0], q, ctx->cheb[1], t1, 0.0, nullptr, ntot, st));
+                int nxt = 1;
+                for (int jj = 2; jj <= ctx->g; ++jj) {
+                    CK(launch_prescale(t1, n_vc, ctx->xs.as<double>(), ldxs, ctx->s.as<double>(), ctx->n_v, ctx->n_c,
+                                       ctx->n_cp, nb, st));
+                    rs = apply_casida_core(ctx, t1, n_vc, u, n_vc, nb, nullptr, 0);
+                    if (rs != GWL_OK) return rs;
+                    double* t2 = tb[nxt];
+                    // t2 may alias t0 (three rotating buffers, t0 is read element-wise before the write)
+                    CK(launch_axpby3(t2, 4.0 / hl, u, -2.0 * hs / hl, t1, -1.0, t0, ntot, st));
+                    CK(launch_axpby3(w, 1.0, w, ctx->cheb[jj], t2, 0.0, nullptr, ntot, st));
+                    t0 = t1;
+                    t1 = t2;
+                    nxt = (nxt + 1) % 3;
+                    if (tb[nxt] == t0) nxt = (nxt + 1) % 3;
+                }
+                CK(launch_dot_partials(q, w, n_vc, n_vc, nb, dotpart, npart, st));
+                ndot = npart;
+                dstride = npart;
+            }
+            CK(cudaEventRecord(e1, st));
+            CK(launch_lanczos_update1(w, q, qp, n_vc, nb, dotpart, ndot, dstride, S, k, normpart, npart, st));
+            if (reorth) {
+                for (int pass = 0; pass < 2; ++pass) {
+                    CK(launch_reorth_dots(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), npart,
+                                          st));
+                    CK(launch_reorth_apply(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), npart,
+                                           pass == 1 ? normpart : nullptr, st));
+                }
+            }
+            CK(launch_lanczos_update2(w, n_vc, nb, normpart, npart, S, k, ctx->xs.as<double>(), ldxs,
+                                      ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
+            CK(cudaEventRecord(e2, st));
+        }
+    }
+    ctx->run_chains = n_chains;
+    ctx->run_steps = L;
+    ctx->run_poly = poly ? 1 : 0;
+    if (n_chains > 0) {
+        const cudaMemcpyKind kind = ctx->device_ptrs ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+        if (alpha) CK(cudaMemcpyAsync(alpha, ctx->alpha.p, (size_t)n_chains * L * 8, kind, st));
+        if (beta) CK(cudaMemcpyAsync(beta, ctx->beta.p, (size_t)n_chains * L * 8, kind, st));
+        if (norm2) CK(cudaMemcpyAsync(norm2, ctx->norm2.p, (size_t)n_chains * 8, kind, st));
+        if (len) CK(cudaMemcpyAsync(len, ctx->len.p, (size_t)n_chains * 4, kind, st));
+    }
+    if (!ctx->device_ptrs) CK(cudaStreamSynchronize(st));
+    return GWL_OK;
+}
+
+gwl_status gwl_resolvent(gwl_ctx* ctx, const double* zeta, int64_t n_zeta, double* r) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (n_zeta < 0 || (n_zeta > 0 && (zeta == nullptr || r == nullptr)))
+        return ctx->fail(GWL_EINVAL, "gwl_resolvent: bad arguments");
+    if (ctx->run_steps == 0) return ctx->fail(GWL_ESTATE, "gwl_resolvent: run gwl_lanczos first");
+    if (n_zeta == 0 || ctx->run_chains == 0) return GWL_OK;
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const double* dz = zeta;
+    double* dr = r;
+    const size_t nr = (size_t)ctx->run_chains * n_zeta * 2 * 8;
+    if (!ctx->device_ptrs) {
+        CK(ctx->d_zeta.ensure((size_t)n_zeta * 16, st));
+        CK(ctx->d_sigma.ensure(nr, st));
+        CK(cudaMemcpyAsync(ctx->d_zeta.p, zeta, (size_t)n_zeta * 16, cudaMemcpyHostToDevice, st));
+        dz = ctx->d_zeta.as<double>();
+        dr = ctx->d_sigma.as<double>();
+    }
+    CK(launch_contfrac(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
+                       ctx->len.as<int32_t>(), ctx->run_steps, (int)ctx->run_chains, dz, (int)n_zeta, dr, st));
+    if (!ctx->device_ptrs) {
+        CK(cudaMemcpyAsync(r, dr, nr, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    return GWL_OK;
+}
+
+gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, double eta, double* sigma,
+                          double* sigma_sum) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (n_omega < 0 || (n_omega > 0 && omega == nullptr) || !(eta > 0.0))
+        return ctx->fail(GWL_EINVAL, "gwl_selfenergy: bad arguments (eta must be > 0)");
+    if (ctx->run_steps == 0) return ctx->fail(GWL_ESTATE, "gwl_selfenergy: run gwl_lanczos first");
+    if (n_omega == 0) return GWL_OK;
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int nch = (int)ctx->run_chains, L = ctx->run_steps;
+    const size_t nsig = (size_t)std::max(nch, 1) * n_omega * 16;
+    const double* dom = omega;
+    double* dsig = sigma;
+    double* dsum = sigma_sum;
+    if (!ctx->device_ptrs) {
+        CK(ctx->d_omega.ensure((size_t)n_omega * 8, st));
+        CK(cudaMemcpyAsync(ctx->d_omega.p, omega, (size_t)n_omega * 8, cudaMemcpyHostToDevice, st));
+        dom = ctx->d_omega.as<double>();
+    }
+    if (!ctx->device_ptrs || sigma == nullptr) {
+        CK(ctx->d_sigma.ensure(nsig, st));
+        dsig = ctx->d_sigma.as<double>();
+    }
+    if (sigma_sum != nullptr && !ctx->device_ptrs) {
+        CK(ctx->d_sigsum.ensure((size_t)n_omega * 16, st));
+        dsum = ctx->d_sigsum.as<double>();
+    }
+    if (nch > 0) {
+        if (ctx->run_poly) {
+            CK(launch_sigma_poly(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
+                                 ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
+                                 ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));
+        } else {
+            CK(ctx->theta.ensure((size_t)nch * L * 8, st));
+            CK(ctx->wgt.ensure((size_t)nch * L * 8, st));
+            CK(ctx->ritz_info.ensure((size_t)nch * 4, st));
+            CK(launch_ritz(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
+                           ctx->theta.as<double>(), ctx->wgt.as<double>(), nullptr, ctx->ritz_info.as<int32_t>(), st));
+            CK(launch_sigma_direct(ctx->theta.as<double>(), ctx->wgt.as<double>(), ctx->norm2.as<double>(),
+                                   ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
+                                   ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));
+        }
+    }
+    if (sigma_sum != nullptr) CK(launch_sigma_sum(dsig, nch, (int)n_omega, dsum, st));
+    if (!ctx->device_ptrs) {
+        if (sigma != nullptr && nch > 0)
+            CK(cudaMemcpyAsync(sigma, dsig, (size_t)nch * n_omega * 16, cudaMemcpyDeviceToHost, st));
+        if (sigma_sum != nullptr)
+            CK(cudaMemcpyAsync(sigma_sum, dsum, (size_t)n_omega * 16, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    return GWL_OK;
+}
+
+gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    double tm = 0.0, tv = 0.0;
+    for (size_t i = 0; i + 2 < ctx->ev_used; i += 3) {
+        float a = 0.f, b = 0.f;
+        CK(cudaEventElapsedTime(&a, ctx->ev[i], ctx->ev[i + 1]));
+        CK(cudaEventElapsedTime(&b, ctx->ev[i + 1], ctx->ev[i + 2]));
+        tm += a;
+        tv += b;
+    }
+    if (ms_matvec) *ms_matvec = tm;
+    if (ms_vecops) *ms_vecops = tv;
+    if (ms_total) *ms_total = tm + tv;
+    return GWL_OK;
+}
+
+gwl_status gwl_get_launch_count(gwl_ctx* ctx, int64_t* n_launches) {
+    if (ctx == nullptr || n_launches == nullptr) return GWL_EINVAL;
+    *n_launches = ctx->launches;
+    return GWL_OK;
+}
+
+gwl_status gwl_probe_fp64_peak(int kind, double* tflops) {
+    if (tflops == nullptr || (kind != 0 && kind != 1)) return GWL_EINVAL;
+    cudaError_t e = probe_fp64_peak(kind, tflops);
+    return e == cudaSuccess ? GWL_OK : GWL_ECUDA;
+}
+
+}  // extern "C"

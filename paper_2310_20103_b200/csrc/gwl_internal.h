@@ -1,0 +1,141 @@
+// Internal declarations shared by the translation units of libgwl.  No torch, no oracle code.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/gwl.h"
+
+namespace gwl {
+
+constexpr int BK = 16;  // doubles per k-tile row = one 128-byte swizzled shared-memory row
+
+static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+static inline int64_t ceil_div(int64_t x, int64_t m) { return (x + m - 1) / m; }
+
+// ---------------------------------------------------------------------------------------------
+// GEMM layer (kr_gemm.cu).  All three contractions of the Casida product are "TN" GEMMs
+//   out[n][m] = sum_k A[m][k] * B[n][k]      (both operands K-contiguous, output M-contiguous)
+// with A = the matrix (Phi_c, V, Phi_c^T) and B = the block of vectors.
+// ---------------------------------------------------------------------------------------------
+enum GemmMode { MODE_FWD = 0, MODE_PLAIN = 1, MODE_BWD = 2 };
+enum GemmEpi { EPI_STORE = 0, EPI_CASIDA = 1, EPI_START = 2 };
+
+struct GemmParams {
+    const double* A;      // [M][lda]
+    int64_t lda;
+    const double* B;      // [N][ldb]
+    int64_t ldb;
+    int M, N;             // valid rows of A / of B
+    int kt_total;         // k-tiles (of BK) in the whole reduction
+    int a_wrap;           // A column of k-tile kt is (kt % a_wrap) * BK   (FWD: k-tiles per v)
+    int kt_per_split;     // FWD/PLAIN: k-tiles handled by one blockIdx.z
+    const double* scale;  // Phi_v^T [n_v][lds]: FWD row scale (index m), BWD k scale (index k)
+    int64_t lds;
+    double* out;          // EPI_STORE: out[z*out_split_stride + n*ldo + m]; CASIDA/START: out[n*ldo + v*n_c + m]
+    int64_t ldo;
+    int64_t out_split_stride;
+    const double* X;      // EPI_CASIDA: x[n*ldx + v*n_c + m]
+    int64_t ldx;
+    const double* d2;     // Delta^2 [n_vc]
+    const double* s;      // sqrt(Delta) [n_vc]
+    double* dotpart;      // CASIDA: sum_m x*y, START: sum_m p*p ; dotpart[n*dot_stride + v*gridDim.x + blockIdx.x]
+    int dot_stride;
+    int n_c;
+    // TMA descriptors (kernel reads them from param space)
+};
+
+struct GemmPlan {
+    int bm, bn;       // CTA tile
+    int splits;       // grid.z for FWD/PLAIN
+    int kt_per_split;
+};
+
+// Chooses tile and split so that the grid is close to a multiple of the SM count.
+GemmPlan plan_gemm(int mode, int M, int N, int kt_total, int a_wrap, int n_sm);
+// Launches; returns cudaGetLastError().  `nz` = splits (FWD/PLAIN) or n_v (BWD).
+cudaError_t launch_gemm(int mode, int epi, const GemmPlan& plan, const GemmParams& p, int nz, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------
+// Vector kernels (vec_kernels.cu).  Block vectors are [nb][n_vc]; partial sums are [nb][npart].
+// ---------------------------------------------------------------------------------------------
+constexpr int VEC_THREADS = 256;
+int vec_parts(int64_t n_vc);  // number of partial-sum blocks per column used by the kernels below
+
+cudaError_t launch_build_delta(const double* eps_v, const double* eps_c, int n_v, int n_c, double* d2, double* s,
+                               cudaStream_t st);
+// xs[b][v][c_pad] = s[vc] * x[b][vc] * (colscale ? colscale[b] : 1)
+cudaError_t launch_prescale(const double* x, int64_t ldx, double* xs, int64_t ldxs, const double* s, int n_v, int n_c,
+                            int n_cp, int nb, cudaStream_t st);
+// t[b][m] = sum_z part[z][b][m]
+cudaError_t launch_splitk_reduce(const double* part, int64_t split_stride, int splits, double* t, int64_t ld, int m,
+                                 int nb, cudaStream_t st);
+// dst[r][c] = src[c][r]  (src [rows][cols] -> dst [cols][ld_dst]), for Phi^T copies
+cudaError_t launch_transpose(const double* src, int rows, int cols, double* dst, int64_t ld_dst, cudaStream_t st);
+cudaError_t launch_copy_pad(const double* src, int rows, int cols, double* dst, int64_t ld_dst, cudaStream_t st);
+// rho[b][mu] = phi_{n_b}(mu) * phi_{m_b}(mu), orbitals taken from PhiV^T / PhiC^T
+cudaError_t launch_rho(const double* phivT, const double* phicT, int64_t ldt, int n_v, int n_mu, const int32_t* n_idx,
+                       const int32_t* m_idx, double* rho, int64_t ld_rho, int nb, cudaStream_t st);
+// part[b][blk] = sum over the block's slice of x[b]*y[b]
+cudaError_t launch_dot_partials(const double* x, const double* y, int64_t ld, int64_t n, int nb, double* part,
+                                int npart, cudaStream_t st);
+
+struct LanczosState {       // device arrays, one entry per chain of the current block
+    double* alpha;          // [nb][steps]  (points into the context's per-chain arrays)
+    double* beta;           // [nb][steps]
+    double* norm2;          // [nb]
+    int32_t* len;           // [nb]
+    double* scale;          // [nb] running max(|a|+b)
+    int32_t* alive;         // [nb]
+    int steps;
+};
+// q0 = p/||p|| in place, xs = s o q0; norm2 from partials; dead if norm2 == 0.
+cudaError_t launch_lanczos_init(double* p, int64_t n_vc, int nb, const double* normpart, int npart, LanczosState st_,
+                                double* xs, int64_t ldxs, const double* s, int n_v, int n_c, int n_cp,
+                                cudaStream_t st);
+// alpha_k = sum(dotpart); w = w - alpha q - beta_{k} q_prev (in place in w); norm partials of the new w.
+cudaError_t launch_lanczos_update1(double* w, const double* q, const double* q_prev, int64_t n_vc, int nb,
+                                   const double* dotpart, int ndot, int dot_stride, LanczosState st_, int k,
+                                   double* normpart, int npart, cudaStream_t st);
+// beta_{k+1} = sqrt(sum normpart); breakdown test; q_next = w / beta in place; xs = s o q_next.
+cudaError_t launch_lanczos_update2(double* w, int64_t n_vc, int nb, const double* normpart, int npart,
+                                   LanczosState st_, int k, double* xs, int64_t ldxs, const double* s, int n_v,
+                                   int n_c, int n_cp, cudaStream_t st);
+// Full reorthogonalisation pass (classical Gram-Schmidt against basis vectors 0..k of each chain).
+// basis: [k+1 slots][nb][n_vc] with slot stride `slot_stride`; coef partials [nb][k+1][npart].
+cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nslots, const double* w, int64_t n_vc,
+                               int nb, double* coefpart, int npart, cudaStream_t st);
+cudaError_t launch_reorth_apply(const double* basis, int64_t slot_stride, int nslots, double* w, int64_t n_vc, int nb,
+                                const double* coefpart, int npart, double* normpart, cudaStream_t st);
+// out = a*x + b*y + c*z (any of y,z may be NULL), uniform scalars, n elements per column
+cudaError_t launch_axpby3(double* out, double a, const double* x, double b, const double* y, double c, const double* z,
+                          int64_t n_total, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------
+// Spectral kernels (spectral_kernels.cu): Eq. 14, Ritz pairs of T_L, Eq. 11 / Eq. 12, Eq. 10.
+// ---------------------------------------------------------------------------------------------
+cudaError_t launch_contfrac(const double* alpha, const double* beta, const double* norm2, const int32_t* len, int steps,
+                            int n_chains, const double* zeta, int n_zeta, double* r, cudaStream_t st);
+// theta[chain][steps], wgt[chain][steps] (first `len` entries valid); work: 3*n_chains*steps doubles
+cudaError_t launch_ritz(const double* alpha, const double* beta, const int32_t* len, int steps, int n_chains,
+                        double* theta, double* wgt, double* work, int32_t* info, cudaStream_t st);
+cudaError_t launch_sigma_direct(const double* theta, const double* wgt, const double* norm2, const int32_t* len,
+                                int steps, int n_chains, const double* eps_n, const int32_t* sgn_n,
+                                const double* omega, int n_omega, double eta, double* sigma, cudaStream_t st);
+cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const double* norm2, const int32_t* len,
+                              int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
+                              int n_omega, double eta, double* sigma, cudaStream_t st);
+cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, double* sigma_sum, cudaStream_t st);
+
+// probe.cu
+cudaError_t probe_fp64_peak(int kind, double* tflops);
+
+// Every launch_* bumps this counter once per kernel launched (read by gwl_get_launch_count).
+extern thread_local int64_t* g_launch_counter;
+inline void count_launch(int n = 1) {
+    if (g_launch_counter) *g_launch_counter += n;
+}
+
+}  // namespace gwl

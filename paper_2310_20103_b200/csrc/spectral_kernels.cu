@@ -1,0 +1,241 @@
+// Resolvent and self-energy kernels: Haydock continued fraction (Eq. 14), Ritz pairs of the
+// Lanczos tridiagonal T_L (Eq. 13), Sigma^corr(omega, n) by Eq. 11 (direct mode) or Eq. 12 + Eq. 14 (poly
+// mode), and the sum over chains (Eq. 10).  Complex FP64 on the plain FP64 ALUs; tiny next to the GEMMs.
+#include "gwl_internal.h"
+
+namespace gwl {
+
+namespace {
+
+struct cplx {
+    double re, im;
+};
+__device__ __forceinline__ cplx cdiv(cplx a, cplx b) {
+    const double d = b.re * b.re + b.im * b.im;
+    return cplx{(a.re * b.re + a.im * b.im) / d, (a.im * b.re - a.re * b.im) / d};
+}
+__device__ __forceinline__ cplx crecip_scaled(double num, cplx b) {  // num / b
+    const double d = b.re * b.re + b.im * b.im;
+    return cplx{num * b.re / d, -num * b.im / d};
+}
+
+// <P|(zeta - T)^{-1}|P> = norm2 / (zeta - a_0 - b_1^2/(zeta - a_1 - ... )), bottom-up, L levels.
+__device__ __forceinline__ cplx contfrac_eval(const double* __restrict__ a, const double* __restrict__ b, int L,
+                                              double norm2, cplx zeta) {
+    if (L <= 0) return cplx{0.0, 0.0};
+    cplx f{zeta.re - a[L - 1], zeta.im};
+    for (int k = L - 2; k >= 0; --k) {
+        const cplx t = crecip_scaled(b[k] * b[k], f);
+        f = cplx{zeta.re - a[k] - t.re, zeta.im - t.im};
+    }
+    return crecip_scaled(norm2, f);
+}
+
+__global__ void k_contfrac(const double* __restrict__ alpha, const double* __restrict__ beta,
+                           const double* __restrict__ norm2, const int32_t* __restrict__ len, int steps,
+                           const double* __restrict__ zeta, int n_zeta, double* __restrict__ r) {
+    const int j = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_zeta) return;
+    const cplx z{zeta[2 * i], zeta[2 * i + 1]};
+    const cplx v = contfrac_eval(alpha + (int64_t)j * steps, beta + (int64_t)j * steps, len[j], norm2[j], z);
+    r[((int64_t)j * n_zeta + i) * 2] = v.re;
+    r[((int64_t)j * n_zeta + i) * 2 + 1] = v.im;
+}
+
+// Golub-Welsch: eigenvalues of the symmetric tridiagonal T_L by the implicit QL iteration with Wilkinson
+// shifts; the same rotations are applied to e_1^T so that z_i = first component of eigenvector i.
+// One chain per block; lane 0 runs the (inherently sequential) sweeps on shared-memory copies.
+__global__ void k_ritz(const double* __restrict__ alpha, const double* __restrict__ beta,
+                       const int32_t* __restrict__ len, int steps, double* __restrict__ theta,
+                       double* __restrict__ wgt, int32_t* __restrict__ info) {
+    extern __shared__ double shm[];
+    double* d = shm;
+    double* e = shm + steps;
+    double* z = shm + 2 * steps;
+    const int j = blockIdx.x;
+    const int n = len[j];
+    for (int i = threadIdx.x; i < steps; i += blockDim.x) {
+        d[i] = (i < n) ? alpha[(int64_t)j * steps + i] : 0.0;
+        e[i] = (i + 1 < n) ? beta[(int64_t)j * steps + i] : 0.0;
+        z[i] = (i == 0) ? 1.0 : 0.0;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int fail = 0;
+        const double eps = 2.220446049250313e-16;
+        for (int l = 0; l < n && !fail; ++l) {
+            int iter = 0;
+            while (true) {
+                int m = l;
+                for (; m < n - 1; ++m) {
+                    const double dd = fabs(d[m]) + fabs(d[m + 1]);
+                    if (fabs(e[m]) <= eps * dd) break;
+                }
+                if (m == l) break;
+                if (++iter > 80) {
+                    fail = 1;
+                    break;
+                }
+                double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
+                double r = sqrt(g * g + 1.0);
+                g = d[m] - d[l] + e[l] / (g + copysign(r, g));
+                double s = 1.0, c = 1.0, p = 0.0;
+                int i = m - 1;
+                for (; i >= l; --i) {
+                    double f = s * e[i];
+                    const double bq = c * e[i];
+                    r = sqrt(f * f + g * g);
+                    e[i + 1] = r;
+                    if (r == 0.0) {
+                        d[i + 1] -= p;
+                        e[m] = 0.0;
+                        break;
+                    }
+                    const double rinv = 1.0 / r;
+                    s = f * rinv;
+                    c = g * rinv;
+                    g = d[i + 1] - p;
+                    r = (d[i] - g) * s + 2.0 * c * bq;
+                    p = s * r;
+                    d[i + 1] = g + p;
+                    g = c * r - bq;
+                    f = z[i + 1];
+                    z[i + 1] = s * z[i] + c * f;
+                    z[i] = c * z[i] - s * f;
+                }
+                if (r == 0.0 && i >= l) continue;
+                d[l] -= p;
+                e[l] = g;
+                e[m] = 0.0;
+            }
+        }
+        if (info != nullptr) info[j] = fail;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < steps; i += blockDim.x) {
+        theta[(int64_t)j * steps + i] = (i < n) ? d[i] : 0.0;
+        wgt[(int64_t)j * steps + i] = (i < n) ? z[i] * z[i] : 0.0;
+    }
+}
+
+// Eq. 11 on the Ritz pairs: Sigma_j(omega) = norm2 * sum_i w_i * sgn / (O_i (O_i + sgn z)), O_i = sqrt(theta_i),
+// z = omega - eps_n - i sgn eta.
+__global__ void k_sigma_direct(const double* __restrict__ theta, const double* __restrict__ wgt,
+                               const double* __restrict__ norm2, const int32_t* __restrict__ len, int steps,
+                               const double* __restrict__ eps_n, const int32_t* __restrict__ sgn_n,
+                               const double* __restrict__ omega, int n_omega, double eta,
+                               double* __restrict__ sigma) {
+    extern __shared__ double shm[];
+    double* O = shm;
+    double* wo = shm + steps;
+    const int j = blockIdx.y;
+    const int n = len[j];
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const double o = sqrt(fmax(theta[(int64_t)j * steps + i], 1e-300));
+        O[i] = o;
+        wo[i] = wgt[(int64_t)j * steps + i] / o;
+    }
+    __syncthreads();
+    const int iw = blockIdx.x * blockDim.x + threadIdx.x;
+    if (iw >= n_omega) return;
+    const double sg = (double)sgn_n[j];
+    const double zre = omega[iw] - eps_n[j], zim = -sg * eta;
+    double sre = 0.0, sim = 0.0;
+    for (int i = 0; i < n; ++i) {
+        const cplx den{O[i] + sg * zre, sg * zim};
+        const cplx t = crecip_scaled(wo[i], den);
+        sre += t.re;
+        sim += t.im;
+    }
+    const double f = norm2[j] * sg;
+    sigma[((int64_t)j * n_omega + iw) * 2] = f * sre;
+    sigma[((int64_t)j * n_omega + iw) * 2 + 1] = f * sim;
+}
+
+// Eq. 12 with Eq. 14: Sigma = (1/z) [ R(-sgn z) - R(0) ],  R(zeta) = <P|(zeta - D)^{-1}|P>.
+__global__ void k_sigma_poly(const double* __restrict__ alpha, const double* __restrict__ beta,
+                             const double* __restrict__ norm2, const int32_t* __restrict__ len, int steps,
+                             const double* __restrict__ eps_n, const int32_t* __restrict__ sgn_n,
+                             const double* __restrict__ omega, int n_omega, double eta, double* __restrict__ sigma) {
+    const int j = blockIdx.y;
+    const int iw = blockIdx.x * blockDim.x + threadIdx.x;
+    if (iw >= n_omega) return;
+    const double sg = (double)sgn_n[j];
+    const cplx z{omega[iw] - eps_n[j], -sg * eta};
+    const double* a = alpha + (int64_t)j * steps;
+    const double* b = beta + (int64_t)j * steps;
+    const cplx r0 = contfrac_eval(a, b, len[j], norm2[j], cplx{0.0, 0.0});
+    const cplx rz = contfrac_eval(a, b, len[j], norm2[j], cplx{-sg * z.re, -sg * z.im});
+    const cplx v = cdiv(cplx{rz.re - r0.re, rz.im - r0.im}, z);
+    sigma[((int64_t)j * n_omega + iw) * 2] = v.re;
+    sigma[((int64_t)j * n_omega + iw) * 2 + 1] = v.im;
+}
+
+__global__ void k_sigma_sum(const double* __restrict__ sigma, int n_chains, int n_omega,
+                            double* __restrict__ sigma_sum) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;  // over 2*n_omega reals
+    if (i >= 2 * n_omega) return;
+    double acc = 0.0;
+    for (int j = 0; j < n_chains; ++j) acc += sigma[(int64_t)j * n_omega * 2 + i];
+    sigma_sum[i] = acc;
+}
+
+}  // namespace
+
+cudaError_t launch_contfrac(const double* alpha, const double* beta, const double* norm2, const int32_t* len, int steps,
+                            int n_chains, const double* zeta, int n_zeta, double* r, cudaStream_t st) {
+    if (n_chains <= 0 || n_zeta <= 0) return cudaSuccess;
+    dim3 grid((unsigned)ceil_div(n_zeta, 128), (unsigned)n_chains);
+    k_contfrac<<<grid, 128, 0, st>>>(alpha, beta, norm2, len, steps, zeta, n_zeta, r);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ritz(const double* alpha, const double* beta, const int32_t* len, int steps, int n_chains,
+                        double* theta, double* wgt, double* work, int32_t* info, cudaStream_t st) {
+    (void)work;
+    if (n_chains <= 0) return cudaSuccess;
+    const size_t sm = (size_t)3 * steps * sizeof(double);
+    if (sm > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(k_ritz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e != cudaSuccess) return e;
+    }
+    k_ritz<<<(unsigned)n_chains, 32, sm, st>>>(alpha, beta, len, steps, theta, wgt, info);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sigma_direct(const double* theta, const double* wgt, const double* norm2, const int32_t* len,
+                                int steps, int n_chains, const double* eps_n, const int32_t* sgn_n,
+                                const double* omega, int n_omega, double eta, double* sigma, cudaStream_t st) {
+    if (n_chains <= 0 || n_omega <= 0) return cudaSuccess;
+    const size_t sm = (size_t)2 * steps * sizeof(double);
+    if (sm > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(k_sigma_direct, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e != cudaSuccess) return e;
+    }
+    dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)n_chains);
+    k_sigma_direct<<<grid, 128, sm, st>>>(theta, wgt, norm2, len, steps, eps_n, sgn_n, omega, n_omega, eta, sigma);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const double* norm2, const int32_t* len,
+                              int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
+                              int n_omega, double eta, double* sigma, cudaStream_t st) {
+    if (n_chains <= 0 || n_omega <= 0) return cudaSuccess;
+    dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)n_chains);
+    k_sigma_poly<<<grid, 128, 0, st>>>(alpha, beta, norm2, len, steps, eps_n, sgn_n, omega, n_omega, eta, sigma);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, double* sigma_sum, cudaStream_t st) {
+    if (n_omega <= 0) return cudaSuccess;
+    k_sigma_sum<<<(unsigned)ceil_div(2 * n_omega, 128), 128, 0, st>>>(sigma, n_chains, n_omega, sigma_sum);
+    count_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace gwl

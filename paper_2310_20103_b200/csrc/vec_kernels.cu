@@ -1,0 +1,398 @@
+// Streaming (HBM-bound) kernels of the path: Delta scaling, split-K reduction, and the batched Lanczos
+// three-term recurrence (Eq. 13) for nb independent chains, with optional two-pass full
+// reorthogonalisation.  All reductions are two-stage and deterministic: a fixed slice per block, a fixed
+// tree inside the block, and consumers re-reduce the per-block partials in a fixed order.
+#include "gwl_internal.h"
+
+namespace gwl {
+
+namespace {
+
+constexpr int NT = VEC_THREADS;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Sum over the block in a fixed order; result valid in every thread.
+__device__ __forceinline__ double block_sum(double v, double* sh /*[NT/32 + 1]*/) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    v = warp_sum(v);
+    __syncthreads();
+    if (lane == 0) sh[w] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int i = 0; i < NT / 32; ++i) t += sh[i];
+        sh[NT / 32] = t;
+    }
+    __syncthreads();
+    return sh[NT / 32];
+}
+
+// Fixed-order sum of a global array of `cnt` doubles, same result in every block that calls it.
+__device__ __forceinline__ double block_sum_array(const double* a, int cnt, double* sh) {
+    double t = 0.0;
+    for (int i = threadIdx.x; i < cnt; i += NT) t += a[i];
+    return block_sum(t, sh);
+}
+
+__device__ __forceinline__ void slice_of(int64_t n, int npart, int blk, int64_t& lo, int64_t& hi) {
+    const int64_t per = (n + npart - 1) / npart;
+    lo = (int64_t)blk * per;
+    hi = lo + per < n ? lo + per : n;
+    if (lo > n) lo = n;
+}
+
+__device__ __forceinline__ int64_t xs_index(int64_t vc, int n_c, int n_cp) {
+    if (n_c == n_cp) return vc;
+    const int64_t v = vc / n_c;
+    return v * n_cp + (vc - v * n_c);
+}
+
+__global__ void k_build_delta(const double* __restrict__ eps_v, const double* __restrict__ eps_c, int n_v, int n_c,
+                              double* __restrict__ d2, double* __restrict__ s) {
+    const int64_t n = (int64_t)n_v * n_c;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int v = (int)(i / n_c), c = (int)(i - (int64_t)v * n_c);
+        const double d = eps_c[c] - eps_v[v];
+        d2[i] = d * d;
+        s[i] = sqrt(d);
+    }
+}
+
+__global__ void k_prescale(const double* __restrict__ x, int64_t ldx, double* __restrict__ xs, int64_t ldxs,
+                           const double* __restrict__ s, int n_c, int n_cp, int64_t n_vc) {
+    const int b = blockIdx.y;
+    const double* xb = x + (int64_t)b * ldx;
+    double* xsb = xs + (int64_t)b * ldxs;
+    for (int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x; i < n_vc; i += (int64_t)gridDim.x * NT)
+        xsb[xs_index(i, n_c, n_cp)] = s[i] * xb[i];
+}
+
+__global__ void k_splitk_reduce(const double* __restrict__ part, int64_t split_stride, int splits,
+                                double* __restrict__ t, int64_t ld, int m) {
+    const int b = blockIdx.y;
+    for (int i = blockIdx.x * NT + threadIdx.x; i < m; i += gridDim.x * NT) {
+        const double* p = part + (int64_t)b * ld + i;
+        double acc = 0.0;
+        for (int z = 0; z < splits; ++z) acc += p[(int64_t)z * split_stride];
+        t[(int64_t)b * ld + i] = acc;
+    }
+}
+
+__global__ void k_transpose(const double* __restrict__ src, int rows, int cols, double* __restrict__ dst,
+                            int64_t ld_dst) {
+    __shared__ double tile[32][33];
+    const int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
+    for (int i = threadIdx.y; i < 32; i += blockDim.y) {
+        const int r = r0 + i, c = c0 + threadIdx.x;
+        if (r < rows && c < cols) tile[i][threadIdx.x] = src[(int64_t)r * cols + c];
+    }
+    __syncthreads();
+    for (int i = threadIdx.y; i < 32; i += blockDim.y) {
+        const int c = c0 + i, r = r0 + threadIdx.x;
+        if (r < rows && c < cols) dst[(int64_t)c * ld_dst + r] = tile[threadIdx.x][i];
+    }
+}
+
+__global__ void k_copy_pad(const double* __restrict__ src, int rows, int cols, double* __restrict__ dst,
+                           int64_t ld_dst) {
+    const int64_t n = (int64_t)rows * cols;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / cols, c = i - r * cols;
+        dst[r * ld_dst + c] = src[i];
+    }
+}
+
+__global__ void k_rho(const double* __restrict__ phivT, const double* __restrict__ phicT, int64_t ldt, int n_v,
+                      int n_mu, const int32_t* __restrict__ n_idx, const int32_t* __restrict__ m_idx,
+                      double* __restrict__ rho, int64_t ld_rho) {
+    const int b = blockIdx.y;
+    const int n = n_idx[b], m = m_idx[b];
+    const double* pn = n < n_v ? phivT + (int64_t)n * ldt : phicT + (int64_t)(n - n_v) * ldt;
+    const double* pm = m < n_v ? phivT + (int64_t)m * ldt : phicT + (int64_t)(m - n_v) * ldt;
+    for (int i = blockIdx.x * NT + threadIdx.x; i < n_mu; i += gridDim.x * NT)
+        rho[(int64_t)b * ld_rho + i] = pn[i] * pm[i];
+}
+
+__global__ void k_dot_partials(const double* __restrict__ x, const double* __restrict__ y, int64_t ld, int64_t n,
+                               double* __restrict__ part, int npart) {
+    __shared__ double sh[NT / 32 + 1];
+    const int b = blockIdx.y;
+    int64_t lo, hi;
+    slice_of(n, npart, blockIdx.x, lo, hi);
+    const double* xb = x + (int64_t)b * ld;
+    const double* yb = y + (int64_t)b * ld;
+    double acc = 0.0;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += NT) acc += xb[i] * yb[i];
+    acc = block_sum(acc, sh);
+    if (threadIdx.x == 0) part[(int64_t)b * npart + blockIdx.x] = acc;
+}
+
+// state parity: arrays scale/alive hold two copies [2][nb]; step k reads copy k&1 and writes copy (k+1)&1,
+// so that blocks of one launch never read what another block of the same launch writes.
+__global__ void k_lanczos_init(double* __restrict__ p, int64_t n_vc, int nb, const double* __restrict__ normpart,
+                               int npart, LanczosState st, double* __restrict__ xs, int64_t ldxs,
+                               const double* __restrict__ s, int n_c, int n_cp) {
+    __shared__ double sh[NT / 32 + 1];
+    const int b = blockIdx.y;
+    const double n2 = block_sum_array(normpart + (int64_t)b * npart, npart, sh);
+    const bool ok = n2 > 0.0;
+    const double nrm = sqrt(n2);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        st.norm2[b] = n2;
+        st.len[b] = ok ? st.steps : 0;
+        st.scale[b] = 0.0;
+        st.alive[b] = ok ? 1 : 0;
+    }
+    int64_t lo, hi;
+    slice_of(n_vc, gridDim.x, blockIdx.x, lo, hi);
+    double* pb = p + (int64_t)b * n_vc;
+    double* xsb = xs + (int64_t)b * ldxs;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += NT) {
+        const double qv = ok ? pb[i] / nrm : 0.0;
+        pb[i] = qv;
+        xsb[xs_index(i, n_c, n_cp)] = s[i] * qv;
+    }
+}
+
+__global__ void k_lanczos_update1(double* __restrict__ w, const double* __restrict__ q,
+                                  const double* __restrict__ q_prev, int64_t n_vc, int nb,
+                                  const double* __restrict__ dotpart, int ndot, int dot_stride, LanczosState st, int k,
+                                  double* __restrict__ normpart, int npart) {
+    __shared__ double sh[NT / 32 + 1];
+    const int b = blockIdx.y;
+    const int par = k & 1;
+    const bool alive = st.alive[par * nb + b] != 0;
+    double a = block_sum_array(dotpart + (int64_t)b * dot_stride, ndot, sh);
+    if (!alive) a = 0.0;
+    const double bprev = (k > 0) ? st.beta[(int64_t)b * st.steps + k - 1] : 0.0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) st.alpha[(int64_t)b * st.steps + k] = a;
+    int64_t lo, hi;
+    slice_of(n_vc, npart, blockIdx.x, lo, hi);
+    double* wb = w + (int64_t)b * n_vc;
+    const double* qb = q + (int64_t)b * n_vc;
+    double acc = 0.0;
+    if (k > 0) {
+        const double* qp = q_prev + (int64_t)b * n_vc;
+        for (int64_t i = lo + threadIdx.x; i < hi; i += NT) {
+            const double v = wb[i] - a * qb[i] - bprev * qp[i];
+            wb[i] = v;
+            acc += v * v;
+        }
+    } else {
+        for (int64_t i = lo + threadIdx.x; i < hi; i += NT) {
+            const double v = wb[i] - a * qb[i];
+            wb[i] = v;
+            acc += v * v;
+        }
+    }
+    acc = block_sum(acc, sh);
+    if (threadIdx.x == 0) normpart[(int64_t)b * npart + blockIdx.x] = acc;
+}
+
+__global__ void k_lanczos_update2(double* __restrict__ w, int64_t n_vc, int nb, const double* __restrict__ normpart,
+                                  int npart, LanczosState st, int k, double* __restrict__ xs, int64_t ldxs,
+                                  const double* __restrict__ s, int n_c, int n_cp) {
+    __shared__ double sh[NT / 32 + 1];
+    const int b = blockIdx.y;
+    const int par = k & 1;
+    const double n2 = block_sum_array(normpart + (int64_t)b * npart, npart, sh);
+    const double beta = sqrt(n2);
+    const bool alive = st.alive[par * nb + b] != 0;
+    const double a = st.alpha[(int64_t)b * st.steps + k];
+    const double sc_old = st.scale[par * nb + b];
+    const double sc_new = fmax(sc_old, fabs(a) + beta);
+    const bool broken = !alive || !(beta > 1e-12 * sc_new);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        st.beta[(int64_t)b * st.steps + k] = broken ? 0.0 : beta;
+        st.scale[(par ^ 1) * nb + b] = sc_new;
+        st.alive[(par ^ 1) * nb + b] = broken ? 0 : 1;
+        if (alive && broken) st.len[b] = k + 1;
+    }
+    int64_t lo, hi;
+    slice_of(n_vc, gridDim.x, blockIdx.x, lo, hi);
+    double* wb = w + (int64_t)b * n_vc;
+    double* xsb = xs + (int64_t)b * ldxs;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += NT) {
+        const double qv = broken ? 0.0 : wb[i] / beta;
+        wb[i] = qv;
+        xsb[xs_index(i, n_c, n_cp)] = s[i] * qv;
+    }
+}
+
+// coefpart[(b*nslots + i)*npart + blk] = sum over the slice of basis_i[b] * w[b]
+__global__ void k_reorth_dots(const double* __restrict__ basis, int64_t slot_stride, int nslots,
+                              const double* __restrict__ w, int64_t n_vc, double* __restrict__ coefpart, int npart) {
+    __shared__ double sh[NT / 32 + 1];
+    const int b = blockIdx.y;
+    int64_t lo, hi;
+    slice_of(n_vc, npart, blockIdx.x, lo, hi);
+    const double* wb = w + (int64_t)b * n_vc;
+    for (int i = 0; i < nslots; ++i) {
+        const double* qb = basis + (int64_t)i * slot_stride + (int64_t)b * n_vc;
+        double acc = 0.0;
+        for (int64_t j = lo + threadIdx.x; j < hi; j += NT) acc += qb[j] * wb[j];
+        acc = block_sum(acc, sh);
+        if (threadIdx.x == 0) coefpart[((int64_t)b * nslots + i) * npart + blockIdx.x] = acc;
+    }
+}
+
+__global__ void k_reorth_apply(const double* __restrict__ basis, int64_t slot_stride, int nslots,
+                               double* __restrict__ w, int64_t n_vc, const double* __restrict__ coefpart, int npart,
+                               double* __restrict__ normpart) {
+    extern __shared__ double coef[];  // [nslots] + block_sum scratch
+    double* sh = coef + nslots;
+    const int b = blockIdx.y;
+    for (int i = threadIdx.x; i < nslots; i += NT) {
+        const double* cp = coefpart + ((int64_t)b * nslots + i) * npart;
+        double t = 0.0;
+        for (int j = 0; j < npart; ++j) t += cp[j];
+        coef[i] = t;
+    }
+    __syncthreads();
+    int64_t lo, hi;
+    slice_of(n_vc, npart, blockIdx.x, lo, hi);
+    double* wb = w + (int64_t)b * n_vc;
+    double acc = 0.0;
+    for (int64_t j = lo + threadIdx.x; j < hi; j += NT) {
+        double v = wb[j];
+        for (int i = 0; i < nslots; ++i) v -= coef[i] * basis[(int64_t)i * slot_stride + (int64_t)b * n_vc + j];
+        wb[j] = v;
+        acc += v * v;
+    }
+    if (normpart != nullptr) {
+        acc = block_sum(acc, sh);
+        if (threadIdx.x == 0) normpart[(int64_t)b * npart + blockIdx.x] = acc;
+    }
+}
+
+__global__ void k_axpby3(double* __restrict__ out, double a, const double* __restrict__ x, double b,
+                         const double* __restrict__ y, double c, const double* __restrict__ z, int64_t n) {
+    for (int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x; i < n; i += (int64_t)gridDim.x * NT) {
+        double v = a * x[i];
+        if (y != nullptr) v += b * y[i];
+        if (z != nullptr) v += c * z[i];
+        out[i] = v;
+    }
+}
+
+inline unsigned grid1d(int64_t n, int per_thread = 4) {
+    int64_t g = ceil_div(n, (int64_t)NT * per_thread);
+    return (unsigned)std::max<int64_t>(1, std::min<int64_t>(g, 148 * 32));
+}
+
+}  // namespace
+
+int vec_parts(int64_t n_vc) { return (int)std::max<int64_t>(1, std::min<int64_t>(64, ceil_div(n_vc, 8192))); }
+
+cudaError_t launch_build_delta(const double* eps_v, const double* eps_c, int n_v, int n_c, double* d2, double* s,
+                               cudaStream_t st) {
+    k_build_delta<<<grid1d((int64_t)n_v * n_c, 1), NT, 0, st>>>(eps_v, eps_c, n_v, n_c, d2, s);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_prescale(const double* x, int64_t ldx, double* xs, int64_t ldxs, const double* s, int n_v, int n_c,
+                            int n_cp, int nb, cudaStream_t st) {
+    const int64_t n_vc = (int64_t)n_v * n_c;
+    dim3 grid(std::min<unsigned>(grid1d(n_vc), 1024u), (unsigned)nb);
+    k_prescale<<<grid, NT, 0, st>>>(x, ldx, xs, ldxs, s, n_c, n_cp, n_vc);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_splitk_reduce(const double* part, int64_t split_stride, int splits, double* t, int64_t ld, int m,
+                                 int nb, cudaStream_t st) {
+    dim3 grid((unsigned)ceil_div(m, NT), (unsigned)nb);
+    k_splitk_reduce<<<grid, NT, 0, st>>>(part, split_stride, splits, t, ld, m);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_transpose(const double* src, int rows, int cols, double* dst, int64_t ld_dst, cudaStream_t st) {
+    dim3 grid((unsigned)ceil_div(cols, 32), (unsigned)ceil_div(rows, 32));
+    k_transpose<<<grid, dim3(32, 8), 0, st>>>(src, rows, cols, dst, ld_dst);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_copy_pad(const double* src, int rows, int cols, double* dst, int64_t ld_dst, cudaStream_t st) {
+    k_copy_pad<<<grid1d((int64_t)rows * cols, 1), NT, 0, st>>>(src, rows, cols, dst, ld_dst);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rho(const double* phivT, const double* phicT, int64_t ldt, int n_v, int n_mu, const int32_t* n_idx,
+                       const int32_t* m_idx, double* rho, int64_t ld_rho, int nb, cudaStream_t st) {
+    dim3 grid((unsigned)ceil_div(n_mu, NT), (unsigned)nb);
+    k_rho<<<grid, NT, 0, st>>>(phivT, phicT, ldt, n_v, n_mu, n_idx, m_idx, rho, ld_rho);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_dot_partials(const double* x, const double* y, int64_t ld, int64_t n, int nb, double* part,
+                                int npart, cudaStream_t st) {
+    dim3 grid((unsigned)npart, (unsigned)nb);
+    k_dot_partials<<<grid, NT, 0, st>>>(x, y, ld, n, part, npart);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_lanczos_init(double* p, int64_t n_vc, int nb, const double* normpart, int npart, LanczosState st_,
+                                double* xs, int64_t ldxs, const double* s, int n_v, int n_c, int n_cp,
+                                cudaStream_t st) {
+    (void)n_v;
+    dim3 grid((unsigned)vec_parts(n_vc), (unsigned)nb);
+    k_lanczos_init<<<grid, NT, 0, st>>>(p, n_vc, nb, normpart, npart, st_, xs, ldxs, s, n_c, n_cp);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_lanczos_update1(double* w, const double* q, const double* q_prev, int64_t n_vc, int nb,
+                                   const double* dotpart, int ndot, int dot_stride, LanczosState st_, int k,
+                                   double* normpart, int npart, cudaStream_t st) {
+    dim3 grid((unsigned)npart, (unsigned)nb);
+    k_lanczos_update1<<<grid, NT, 0, st>>>(w, q, q_prev, n_vc, nb, dotpart, ndot, dot_stride, st_, k, normpart, npart);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_lanczos_update2(double* w, int64_t n_vc, int nb, const double* normpart, int npart,
+                                   LanczosState st_, int k, double* xs, int64_t ldxs, const double* s, int n_v,
+                                   int n_c, int n_cp, cudaStream_t st) {
+    (void)n_v;
+    dim3 grid((unsigned)vec_parts(n_vc), (unsigned)nb);
+    k_lanczos_update2<<<grid, NT, 0, st>>>(w, n_vc, nb, normpart, npart, st_, k, xs, ldxs, s, n_c, n_cp);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nslots, const double* w, int64_t n_vc,
+                               int nb, double* coefpart, int npart, cudaStream_t st) {
+    dim3 grid((unsigned)npart, (unsigned)nb);
+    k_reorth_dots<<<grid, NT, 0, st>>>(basis, slot_stride, nslots, w, n_vc, coefpart, npart);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_reorth_apply(const double* basis, int64_t slot_stride, int nslots, double* w, int64_t n_vc, int nb,
+                                const double* coefpart, int npart, double* normpart, cudaStream_t st) {
+    dim3 grid((unsigned)npart, (unsigned)nb);
+    const size_t sm = (size_t)(nslots + NT / 32 + 1) * sizeof(double);
+    k_reorth_apply<<<grid, NT, sm, st>>>(basis, slot_stride, nslots, w, n_vc, coefpart, npart, normpart);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_axpby3(double* out, double a, const double* x, double b, const double* y, double c, const double* z,
+                          int64_t n_total, cudaStream_t st) {
+    k_axpby3<<<grid1d(n_total), NT, 0, st>>>(out, a, x, b, y, c, z, n_total);
+    count_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace gwl

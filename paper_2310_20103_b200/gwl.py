@@ -1,0 +1,265 @@
+"""Thin ctypes binding over libgwl.so (include/gwl.h).  Argument marshalling only: every step of the path
+runs in the library's CUDA kernels.  There is no CPU fallback -- if libgwl.so is missing or the call
+fails, a GwlError is raised.
+
+Host mode (default): numpy float64 arrays in, numpy arrays out.
+Device mode (`ctx.set_pointer_mode(1)`): torch CUDA float64 tensors in/out, nothing is copied.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_char_p, c_double, c_int, c_int32, c_int64, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgwl.so")
+
+GWL_OK, GWL_EINVAL, GWL_ESTATE, GWL_ENOMEM, GWL_ECUDA = range(5)
+_STATUS = {0: "GWL_OK", 1: "GWL_EINVAL", 2: "GWL_ESTATE", 3: "GWL_ENOMEM", 4: "GWL_ECUDA"}
+
+# name -> (restype, argtypes); every symbol include/gwl.h declares
+SIGNATURES = {
+    "gwl_create": (c_int, [POINTER(c_void_p), c_int64, c_int64, c_int64]),
+    "gwl_destroy": (None, [c_void_p]),
+    "gwl_last_error": (c_char_p, [c_void_p]),
+    "gwl_set_pointer_mode": (c_int, [c_void_p, c_int]),
+    "gwl_set_stream": (c_int, [c_void_p, c_void_p]),
+    "gwl_set_orbitals": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "gwl_set_energies": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "gwl_set_kernel": (c_int, [c_void_p, c_void_p]),
+    "gwl_set_polynomial": (c_int, [c_void_p, c_int, c_void_p, c_double, c_double]),
+    "gwl_casida_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
+    "gwl_set_chains": (c_int, [c_void_p, c_int64, c_void_p, c_void_p]),
+    "gwl_set_start_vectors": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p]),
+    "gwl_lanczos": (c_int, [c_void_p, c_int64, c_int64, c_int64, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "gwl_resolvent": (c_int, [c_void_p, c_void_p, c_int64, c_void_p]),
+    "gwl_selfenergy": (c_int, [c_void_p, c_void_p, c_int64, c_double, c_void_p, c_void_p]),
+    "gwl_get_timing": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
+    "gwl_get_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
+    "gwl_probe_fp64_peak": (c_int, [c_int, POINTER(c_double)]),
+}
+
+
+class GwlError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library(path: str = LIB_PATH):
+    """Loads libgwl.so (built by `python -m paper_2310_20103_b200.build`); raises if it is absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(path):
+            raise GwlError(GWL_ESTATE, f"{path} not found: build it with `python -m paper_2310_20103_b200.build` "
+                                       "(there is no CPU fallback)")
+        lib = ctypes.CDLL(path)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def _is_torch(x):
+    return type(x).__module__.startswith("torch")
+
+
+def _host(a, dtype=np.float64):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _ptr(a):
+    if a is None:
+        return None
+    if _is_torch(a):
+        return c_void_p(a.data_ptr())
+    return c_void_p(a.ctypes.data)
+
+
+def probe_fp64_peak(kind: int = 0) -> float:
+    """TFLOP/s of a register-resident DMMA (kind 0) or DFMA (kind 1) loop on the current device."""
+    lib = load_library()
+    out = c_double(0.0)
+    st = lib.gwl_probe_fp64_peak(kind, byref(out))
+    if st != GWL_OK:
+        raise GwlError(st, "gwl_probe_fp64_peak failed")
+    return out.value
+
+
+class Context:
+    """gwl_ctx wrapper.  Method names follow the C ABI without the gwl_ prefix."""
+
+    def __init__(self, n_v: int, n_c: int, n_mu: int):
+        self._lib = load_library()
+        self._h = c_void_p()
+        self.n_v, self.n_c, self.n_mu = int(n_v), int(n_c), int(n_mu)
+        self.n_vc = self.n_v * self.n_c
+        self.device_ptrs = 0
+        st = self._lib.gwl_create(byref(self._h), n_v, n_c, n_mu)
+        if st != GWL_OK:
+            self._h = c_void_p()
+            raise GwlError(st, "gwl_create failed (no CUDA device, or bad sizes)")
+
+    # -- plumbing ---------------------------------------------------------------------------------
+    def _ck(self, st):
+        if st != GWL_OK:
+            msg = self._lib.gwl_last_error(self._h)
+            raise GwlError(st, msg.decode() if msg else "")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.gwl_destroy(self._h)
+            self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def last_error(self) -> str:
+        return self._lib.gwl_last_error(self._h).decode()
+
+    def set_pointer_mode(self, device_ptrs: int):
+        self._ck(self._lib.gwl_set_pointer_mode(self._h, int(device_ptrs)))
+        self.device_ptrs = int(device_ptrs)
+
+    def set_stream(self, cuda_stream: int | None):
+        self._ck(self._lib.gwl_set_stream(self._h, c_void_p(cuda_stream or 0)))
+
+    # -- inputs -----------------------------------------------------------------------------------
+    def set_orbitals(self, phi_v, phi_c):
+        pv, pc = _host(phi_v), _host(phi_c)
+        if pv.shape != (self.n_mu, self.n_v) or pc.shape != (self.n_mu, self.n_c):
+            raise GwlError(GWL_EINVAL, "set_orbitals: phi_v must be [n_mu, n_v], phi_c [n_mu, n_c]")
+        self._ck(self._lib.gwl_set_orbitals(self._h, _ptr(pv), _ptr(pc)))
+
+    def set_energies(self, eps_v, eps_c):
+        ev, ec = _host(eps_v), _host(eps_c)
+        if ev.shape != (self.n_v,) or ec.shape != (self.n_c,):
+            raise GwlError(GWL_EINVAL, "set_energies: eps_v must be [n_v], eps_c [n_c]")
+        self._ck(self._lib.gwl_set_energies(self._h, _ptr(ev), _ptr(ec)))
+
+    def set_kernel(self, V):
+        Vh = _host(V)
+        if Vh.shape != (self.n_mu, self.n_mu):
+            raise GwlError(GWL_EINVAL, "set_kernel: V must be [n_mu, n_mu]")
+        self._ck(self._lib.gwl_set_kernel(self._h, _ptr(Vh)))
+
+    def set_polynomial(self, g: int, cheb=None, lo: float = 0.0, hi: float = 0.0):
+        c = None if cheb is None else _host(cheb)
+        if g > 0 and (c is None or c.shape != (g + 1,)):
+            raise GwlError(GWL_EINVAL, "set_polynomial: cheb must have g+1 entries")
+        self._ck(self._lib.gwl_set_polynomial(self._h, int(g), _ptr(c), float(lo), float(hi)))
+
+    # -- the path ---------------------------------------------------------------------------------
+    def casida_matvec(self, x, y=None):
+        """y = C x.  Host mode: x numpy [nvec, n_v, n_c] (or [nvec, n_vc]) -> numpy of the same shape.
+        Device mode: x, y torch CUDA float64 tensors, contiguous; y is written in place and returned."""
+        if self.device_ptrs:
+            if y is None or not _is_torch(x) or not _is_torch(y):
+                raise GwlError(GWL_EINVAL, "casida_matvec (device mode): x and y must be torch CUDA tensors")
+            if not (x.is_contiguous() and y.is_contiguous()) or x.numel() != y.numel() or x.numel() % self.n_vc:
+                raise GwlError(GWL_EINVAL, "casida_matvec: x, y must be contiguous [nvec, n_v, n_c]")
+            nvec = x.numel() // self.n_vc
+            self._ck(self._lib.gwl_casida_matvec(self._h, _ptr(x), _ptr(y), nvec))
+            return y
+        xh = _host(x)
+        if xh.size % self.n_vc:
+            raise GwlError(GWL_EINVAL, "casida_matvec: x must be [nvec, n_v, n_c]")
+        nvec = xh.size // self.n_vc
+        yh = np.empty_like(xh)
+        self._ck(self._lib.gwl_casida_matvec(self._h, _ptr(xh), _ptr(yh), nvec))
+        return yh
+
+    def set_chains(self, n_idx, m_idx):
+        n, m = _host(n_idx, np.int32), _host(m_idx, np.int32)
+        if n.shape != m.shape or n.ndim != 1:
+            raise GwlError(GWL_EINVAL, "set_chains: n_idx and m_idx must be 1-d and of equal length")
+        self._ck(self._lib.gwl_set_chains(self._h, n.size, _ptr(n), _ptr(m)))
+
+    def set_start_vectors(self, p, eps_n, sgn_n):
+        e, s = _host(eps_n), _host(sgn_n, np.int32)
+        if self.device_ptrs:
+            n = p.numel() // self.n_vc
+            pp = p
+        else:
+            pp = _host(p)
+            n = pp.size // self.n_vc
+        if e.shape != (n,) or s.shape != (n,):
+            raise GwlError(GWL_EINVAL, "set_start_vectors: eps_n and sgn_n must have one entry per chain")
+        self._ck(self._lib.gwl_set_start_vectors(self._h, n, _ptr(pp), _ptr(e), _ptr(s)))
+
+    def lanczos(self, n_chains: int, steps: int, block: int, reorth: int = 0, out=None):
+        """Returns (alpha[n_chains, steps], beta[n_chains, steps], norm2[n_chains], len[n_chains]).
+        Device mode: pass out=(alpha, beta, norm2, len) torch CUDA tensors (or None to skip the copy-out)."""
+        if self.device_ptrs:
+            a = b = n2 = ln = None
+            if out is not None:
+                a, b, n2, ln = out
+            self._ck(self._lib.gwl_lanczos(self._h, n_chains, steps, block, reorth, _ptr(a), _ptr(b), _ptr(n2), _ptr(ln)))
+            return out
+        a = np.zeros((n_chains, steps))
+        b = np.zeros((n_chains, steps))
+        n2 = np.zeros(n_chains)
+        ln = np.zeros(n_chains, dtype=np.int32)
+        self._ck(self._lib.gwl_lanczos(self._h, n_chains, steps, block, reorth, _ptr(a), _ptr(b), _ptr(n2), _ptr(ln)))
+        return a, b, n2, ln
+
+    def resolvent(self, zeta, n_chains: int | None = None, out=None):
+        """r[chain, i] = <P|(zeta_i - Op)^-1|P> (complex).  Host mode: zeta complex numpy array."""
+        if self.device_ptrs:
+            n_zeta = zeta.numel() // 2
+            self._ck(self._lib.gwl_resolvent(self._h, _ptr(zeta), n_zeta, _ptr(out)))
+            return out
+        z = np.ascontiguousarray(zeta, dtype=np.complex128)
+        r = np.zeros((n_chains, z.size), dtype=np.complex128)
+        self._ck(self._lib.gwl_resolvent(self._h, _ptr(z), z.size, _ptr(r)))
+        return r
+
+    def selfenergy(self, omega, eta: float, n_chains: int | None = None, want_sum: bool = True, out=None):
+        """Host mode: returns (sigma[n_chains, n_omega] complex, sigma_sum[n_omega] complex or None).
+        Device mode: out=(sigma [n_chains, n_omega, 2] or None, sigma_sum [n_omega, 2] or None)."""
+        if self.device_ptrs:
+            sg, ss = out if out is not None else (None, None)
+            self._ck(self._lib.gwl_selfenergy(self._h, _ptr(omega), omega.numel(), float(eta), _ptr(sg), _ptr(ss)))
+            return out
+        om = _host(omega)
+        sg = np.zeros((n_chains, om.size), dtype=np.complex128)
+        ss = np.zeros(om.size, dtype=np.complex128) if want_sum else None
+        self._ck(self._lib.gwl_selfenergy(self._h, _ptr(om), om.size, float(eta), _ptr(sg), _ptr(ss)))
+        return sg, ss
+
+    def get_timing(self):
+        a, b, c = c_double(), c_double(), c_double()
+        self._ck(self._lib.gwl_get_timing(self._h, byref(a), byref(b), byref(c)))
+        return a.value, b.value, c.value
+
+    def get_launch_count(self) -> int:
+        n = c_int64()
+        self._ck(self._lib.gwl_get_launch_count(self._h, byref(n)))
+        return n.value
+
+
+def context_from_problem(prob) -> Context:
+    """Creates a context and uploads the inputs of a synth.Problem (orbitals, energies, kernel, chains)."""
+    cfg = prob.cfg
+    ctx = Context(cfg.n_v, cfg.n_c, cfg.n_mu)
+    ctx.set_orbitals(prob.phi_v, prob.phi_c)
+    ctx.set_energies(prob.eps_v, prob.eps_c)
+    ctx.set_kernel(prob.V)
+    ctx.set_chains(prob.n_idx, prob.m_idx)
+    return ctx

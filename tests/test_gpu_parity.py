@@ -1,0 +1,342 @@
+"""GPU parity: the CUDA path (through the C ABI of libgwl.so) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json:north_star, protocol of SURVEY.md §8(c)):
+  matvec            max|y_gpu - y_cpu| / max|y_cpu| <= 1e-12
+  alpha/beta[:30]   element-wise relative <= 1e-9, reorthogonalisation off
+  Sigma^c(omega)    absolute <= 1e-6 eV over the whole grid, reorthogonalisation on, on both sides
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import gw_oracle as orc
+from paper_2310_20103_b200 import gwl, synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_MATVEC = 1e-12
+TOL_AB = 1e-9
+TOL_SIGMA = 1e-6
+DLT = 0.1
+
+
+def _ctx(p, chains=True):
+    ctx = gwl.Context(p.cfg.n_v, p.cfg.n_c, p.cfg.n_mu)
+    ctx.set_orbitals(p.phi_v, p.phi_c)
+    ctx.set_energies(p.eps_v, p.eps_c)
+    ctx.set_kernel(p.V)
+    if chains:
+        ctx.set_chains(p.n_idx, p.m_idx)
+    return ctx
+
+
+def _relmax(a, b):
+    return np.abs(a - b).max() / np.abs(b).max()
+
+
+def _oracle_matvec(p, X):
+    return orc.casida_matvec_factored(p.phi_v, p.phi_c, p.V, orc.delta_vc(p.eps_v, p.eps_c), X)
+
+
+@pytest.fixture(scope="module")
+def p0():
+    p = synth.make_problem(0)
+    _ = p.V
+    return p
+
+
+@pytest.fixture(scope="module")
+def p1():
+    p = synth.make_problem(1)
+    _ = p.V
+    return p
+
+
+# ---- S2: Casida block product ------------------------------------------------------------------
+@pytest.mark.parametrize("nvec", [1, 4, 7])
+def test_matvec_config0(p0, nvec):
+    X = synth.random_block(p0.cfg, nvec)
+    with _ctx(p0, chains=False) as ctx:
+        Y = ctx.casida_matvec(X)
+    assert Y.shape == X.shape
+    assert _relmax(Y, _oracle_matvec(p0, X)) <= TOL_MATVEC
+
+
+@pytest.mark.parametrize("n_v,n_c,n_mu,nvec", [(1, 1, 1, 1), (3, 5, 37, 3), (5, 19, 130, 70), (2, 33, 257, 130),
+                                                (7, 16, 48, 300)])
+def test_matvec_ragged_sizes(n_v, n_c, n_mu, nvec):
+    """Odd N_c (unaligned rows), N_mu and N_c not multiples of the tiles, block wider than one N tile,
+    and nvec > 256 (two chunks)."""
+    p = synth.make_custom(n_v, n_c, n_mu, seed=n_mu)
+    X = synth.random_block(p.cfg, nvec, seed=2)
+    with _ctx(p, chains=False) as ctx:
+        Y = ctx.casida_matvec(X)
+    assert _relmax(Y, _oracle_matvec(p, X)) <= TOL_MATVEC
+
+
+def test_matvec_zero_kernel_is_exact(p0):
+    X = synth.random_block(p0.cfg, 3)
+    with gwl.Context(p0.cfg.n_v, p0.cfg.n_c, p0.cfg.n_mu) as ctx:
+        ctx.set_orbitals(p0.phi_v, p0.phi_c)
+        ctx.set_energies(p0.eps_v, p0.eps_c)
+        ctx.set_kernel(np.zeros_like(p0.V))
+        Y = ctx.casida_matvec(X)
+    d = orc.delta_vc(p0.eps_v, p0.eps_c).reshape(p0.cfg.n_v, p0.cfg.n_c)
+    assert np.array_equal(Y, d * d * X)
+
+
+def test_matvec_config1_full_block(p1):
+    X = synth.random_block(p1.cfg, p1.cfg.block)
+    with _ctx(p1, chains=False) as ctx:
+        Y = ctx.casida_matvec(X)
+        # columns do not depend on what else is in the block
+        Y1 = ctx.casida_matvec(X[5:6])
+    ref = _oracle_matvec(p1, X)
+    assert _relmax(Y, ref) <= TOL_MATVEC
+    assert _relmax(Y1, ref[5:6]) <= TOL_MATVEC
+    assert _relmax(Y1, Y[5:6]) <= 1e-13
+    # symmetry of C through the GPU path: x^T (C y) = y^T (C x)
+    a, b = X[0].ravel(), X[1].ravel()
+    assert abs(a @ Y[1].ravel() - b @ Y[0].ravel()) <= 1e-11 * abs(a @ Y[1].ravel())
+
+
+def test_matvec_device_pointer_mode(p0):
+    import torch
+    X = synth.random_block(p0.cfg, 4)
+    with _ctx(p0, chains=False) as ctx:
+        ctx.set_pointer_mode(1)
+        ctx.set_stream(torch.cuda.current_stream().cuda_stream)
+        xd = torch.from_numpy(X).cuda()
+        yd = torch.empty_like(xd)
+        ctx.casida_matvec(xd, yd)
+        torch.cuda.synchronize()
+        Y = yd.cpu().numpy()
+    assert _relmax(Y, _oracle_matvec(p0, X)) <= TOL_MATVEC
+
+
+def _sampled_matvec(cfg_id, cols):
+    p = synth.make_problem(cfg_id)
+    _ = p.V
+    X = synth.random_block(p.cfg, p.cfg.block)
+    with _ctx(p, chains=False) as ctx:
+        Y = ctx.casida_matvec(X)
+    ref = _oracle_matvec(p, X[cols])
+    assert _relmax(Y[cols], ref) <= TOL_MATVEC
+
+
+def test_matvec_config2_sampled_columns():
+    """Full block of 256 at the ~100-atom size; the oracle checks sampled columns one by one."""
+    _sampled_matvec(2, [0, 131, 255])
+
+
+@pytest.mark.skipif(os.environ.get("GWL_TEST_LARGE", "0") != "1", reason="set GWL_TEST_LARGE=1 (minutes of host time)")
+@pytest.mark.parametrize("cfg_id", [3, 4])
+def test_matvec_large_configs_sampled_columns(cfg_id):
+    _sampled_matvec(cfg_id, [1, synth.CONFIGS[cfg_id].block - 1])
+
+
+# ---- S1 + S4: start vectors and Lanczos --------------------------------------------------------------
+def _oracle_chains(p, idx, steps, reorth, poly=None):
+    return orc.run_chains(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, p.n_idx[idx], p.m_idx[idx], steps,
+                          p.omega, DLT, reorth=reorth, poly=poly)
+
+
+def _check_ab(a, b, ra, rb, upto):
+    assert np.abs(a[:, :upto] - ra[:, :upto]).max() <= TOL_AB * np.abs(ra[:, :upto]).max()
+    assert (np.abs(a[:, :upto] - ra[:, :upto]) <= TOL_AB * np.abs(ra[:, :upto])).all()
+    assert (np.abs(b[:, :upto] - rb[:, :upto]) <= TOL_AB * np.abs(rb[:, :upto])).all()
+
+
+def test_lanczos_config0_first30_no_reorth(p0):
+    cfg = p0.cfg
+    with _ctx(p0) as ctx:
+        a, b, n2, ln = ctx.lanczos(cfg.n_chains, cfg.steps, cfg.block, reorth=0)
+    ref = _oracle_chains(p0, slice(None), cfg.steps, False)
+    assert (np.abs(n2 - ref["norm2"]) <= 1e-12 * ref["norm2"]).all()
+    assert (ln == cfg.steps).all()
+    _check_ab(a, b, ref["alpha"], ref["beta"], 30)
+
+
+def test_lanczos_and_sigma_config0_reorth(p0):
+    cfg = p0.cfg
+    with _ctx(p0) as ctx:
+        a, b, n2, ln = ctx.lanczos(cfg.n_chains, cfg.steps, cfg.block, reorth=1)
+        sig, ssum = ctx.selfenergy(p0.omega, DLT, cfg.n_chains)
+    ref = _oracle_chains(p0, slice(None), cfg.steps, True)
+    _check_ab(a, b, ref["alpha"], ref["beta"], cfg.steps)
+    assert np.abs(sig - ref["sigma"]).max() <= TOL_SIGMA
+    assert np.abs(ssum - ref["sigma_sum"]).max() <= TOL_SIGMA
+
+
+def test_sigma_config0_30_steps_no_reorth(p0):
+    cfg = p0.cfg
+    with _ctx(p0) as ctx:
+        ctx.lanczos(cfg.n_chains, 30, cfg.block, reorth=0)
+        sig, _ = ctx.selfenergy(p0.omega, DLT, cfg.n_chains)
+    ref = _oracle_chains(p0, slice(None), 30, False)
+    assert np.abs(sig - ref["sigma"]).max() <= TOL_SIGMA
+
+
+def test_short_last_block_and_block_invariance(p0):
+    """n_chains not a multiple of block; chain j gives the same tridiagonal whatever block it runs in (Q10)."""
+    with _ctx(p0) as ctx:
+        a4, b4, n4, _ = ctx.lanczos(4, 25, 4, reorth=0)
+        a3, b3, n3, _ = ctx.lanczos(4, 25, 3, reorth=0)      # blocks of 3 + 1
+        a1, b1, n1, _ = ctx.lanczos(4, 25, 1, reorth=0)
+        a2, _, _, _ = ctx.lanczos(2, 25, 4, reorth=0)        # fewer chains than were set
+    for x, y in [(a3, a4), (b3, b4), (a1, a4), (b1, b4), (n3, n4), (n1, n4), (a2, a4[:2])]:
+        assert (np.abs(x - y) <= 1e-10 * np.abs(y)).all()
+
+
+def test_negative_sign_chains_and_eq10_sum(p0):
+    """m = highest valence, n over all N_v + N_c orbitals: exercises eta_n = -1 and the Eq. 10 sum."""
+    cfg = p0.cfg
+    n_idx = np.arange(cfg.n_v + cfg.n_c, dtype=np.int32)
+    m_idx = np.full_like(n_idx, cfg.n_v - 1)
+    L = 40
+    with _ctx(p0, chains=False) as ctx:
+        ctx.set_chains(n_idx, m_idx)
+        a, b, n2, ln = ctx.lanczos(len(n_idx), L, 12, reorth=1)
+        sig, ssum = ctx.selfenergy(p0.omega, DLT, len(n_idx))
+    ref = orc.run_chains(p0.phi_v, p0.phi_c, p0.eps_v, p0.eps_c, p0.V, n_idx, m_idx, L, p0.omega, DLT, reorth=True)
+    _check_ab(a, b, ref["alpha"], ref["beta"], L)
+    assert np.abs(sig - ref["sigma"]).max() <= TOL_SIGMA
+    assert np.abs(ssum - ref["sigma_sum"]).max() <= TOL_SIGMA
+    assert (sig[: cfg.n_v].imag > 0).all() and (sig[cfg.n_v:].imag < 0).all()        # Herglotz sign per eta_n
+
+
+def test_explicit_start_vectors_equal_index_chains(p0):
+    cfg = p0.cfg
+    delta = orc.delta_vc(p0.eps_v, p0.eps_c)
+    P = np.array([orc.start_vector(p0.phi_v, p0.phi_c, p0.V, delta, int(n), int(m))
+                  for n, m in zip(p0.n_idx, p0.m_idx)])
+    es = [orc.orbital_energy_sign(p0.eps_v, p0.eps_c, int(n)) for n in p0.n_idx]
+    with _ctx(p0) as ctx:
+        a, b, n2, _ = ctx.lanczos(4, 20, 4, 0)
+        s_idx, _ = ctx.selfenergy(p0.omega, DLT, 4)
+        ctx.set_start_vectors(P, [e for e, _ in es], [s for _, s in es])
+        a2, b2, n22, _ = ctx.lanczos(4, 20, 4, 0)
+        s_vec, _ = ctx.selfenergy(p0.omega, DLT, 4)
+    assert (np.abs(n2 - (P * P).sum(axis=1)) <= 1e-12 * n2).all()
+    assert (np.abs(a - a2) <= 1e-10 * np.abs(a)).all() and (np.abs(b - b2) <= 1e-10 * np.abs(b)).all()
+    assert np.abs(s_idx - s_vec).max() <= 1e-9
+
+
+def test_breakdown_and_zero_start_vector():
+    """Q9: with V = 0 the operator is diagonal; a start vector with 3 nonzeros spans a 3-dimensional invariant
+    subspace -> len = 3, zero-filled tail; a zero start vector gives len = 0 and Sigma = 0."""
+    p = synth.make_custom(2, 3, 16, seed=9)
+    delta = orc.delta_vc(p.eps_v, p.eps_c)
+    P = np.zeros((3, 6))
+    P[0, [0, 2, 5]] = [1.0, 2.0, -1.0]
+    P[2] = np.arange(1, 7)
+    with gwl.Context(2, 3, 16) as ctx:
+        ctx.set_orbitals(p.phi_v, p.phi_c)
+        ctx.set_energies(p.eps_v, p.eps_c)
+        ctx.set_kernel(np.zeros((16, 16)))
+        ctx.set_start_vectors(P, [-6.0, -6.0, 1.0], [1, 1, -1])
+        a, b, n2, ln = ctx.lanczos(3, 6, 3, 0)
+        sig, _ = ctx.selfenergy(p.omega, DLT, 3)
+        r = ctx.resolvent(np.array([1.0 + 1.0j, -5.0 + 0.2j]), 3)
+    assert list(ln) == [3, 0, 6]
+    assert (a[0, 3:] == 0).all() and (b[0, 2:] == 0).all() and (a[1] == 0).all() and n2[1] == 0
+    ra, rb, rn2, rl = orc.lanczos(lambda x: delta ** 2 * x, P[0], 6)
+    assert rl == 3 and np.abs(a[0] - ra).max() <= 1e-9 * np.abs(ra).max() and np.abs(b[0] - rb).max() <= 1e-9 * np.abs(ra).max()
+    assert (sig[1] == 0).all() and (r[1] == 0).all()
+    ref = orc.sigma_direct(ra, rb, rn2, rl, p.omega, -6.0, 1, DLT)
+    assert np.abs(sig[0] - ref).max() <= TOL_SIGMA
+    z = np.array([1.0 + 1.0j, -5.0 + 0.2j])
+    exact = (P[0] ** 2 / (z[:, None] - delta[None, :] ** 2)).sum(axis=1)        # P11 closed form
+    assert np.abs(r[0] - exact).max() <= 1e-10 * np.abs(exact).max()
+
+
+def test_resolvent_matches_oracle_continued_fraction(p0):
+    cfg = p0.cfg
+    zeta = (p0.omega[::10] + 1j * DLT) ** 2
+    with _ctx(p0) as ctx:
+        a, b, n2, ln = ctx.lanczos(4, 30, 4, 0)
+        r = ctx.resolvent(zeta, 4)
+    for j in range(4):
+        ref = orc.continued_fraction(a[j], b[j], n2[j], zeta, ln[j])
+        assert np.abs(r[j] - ref).max() <= 1e-11 * np.abs(ref).max()
+
+
+def test_poly_mode_config0(p0):
+    """The paper's route: Lanczos on p_g(C), Sigma by Eq. 12 + Eq. 14; g = 7 and 8, N_iter = 8."""
+    delta = orc.delta_vc(p0.eps_v, p0.eps_c)
+    lo, hi = 0.8 * (delta ** 2).min(), 1.25 * (delta ** 2).max()
+    for g in (7, 8):
+        c = orc.fit_sqrt_chebyshev(g, lo, hi)
+        with _ctx(p0) as ctx:
+            ctx.set_polynomial(g, c, lo, hi)
+            a, b, n2, ln = ctx.lanczos(4, 8, 4, 0)
+            sig, ssum = ctx.selfenergy(p0.omega, DLT, 4)
+            ctx.set_polynomial(0)
+            a_dir, _, _, _ = ctx.lanczos(4, 8, 4, 0)
+        ref = _oracle_chains(p0, slice(None), 8, False, poly=(c, lo, hi))
+        _check_ab(a, b, ref["alpha"], ref["beta"], 8)
+        assert np.abs(sig - ref["sigma"]).max() <= TOL_SIGMA
+        assert np.abs(ssum - ref["sigma_sum"]).max() <= TOL_SIGMA
+        assert np.abs(a_dir - a).max() > 1.0          # clearing the polynomial really switches back to Op = C
+
+
+def test_lanczos_config1_sampled(p1):
+    """Config 1, block of 64 as timed by bench.py: all 64 chains run on the GPU; the oracle checks sampled
+    chains (first 30 alpha/beta, reorth off) and Sigma of sampled chains at L = 60 with reorth on both sides."""
+    cfg = p1.cfg
+    idx = np.array([0, 21, 63])
+    with _ctx(p1) as ctx:
+        a, b, n2, ln = ctx.lanczos(cfg.n_chains, 30, cfg.block, 0)
+        sig30, _ = ctx.selfenergy(p1.omega, DLT, cfg.n_chains)
+    ref = _oracle_chains(p1, idx, 30, False)
+    _check_ab(a[idx], b[idx], ref["alpha"], ref["beta"], 30)
+    assert np.abs(sig30[idx] - ref["sigma"]).max() <= TOL_SIGMA
+    with _ctx(p1, chains=False) as ctx:
+        ctx.set_chains(p1.n_idx[idx], p1.m_idx[idx])
+        a, b, n2, ln = ctx.lanczos(3, 60, 3, 1)
+        sig, _ = ctx.selfenergy(p1.omega, DLT, 3)
+    ref = _oracle_chains(p1, idx, 60, True)
+    _check_ab(a, b, ref["alpha"], ref["beta"], 60)
+    assert np.abs(sig - ref["sigma"]).max() <= TOL_SIGMA
+
+
+# ---- API behaviour -------------------------------------------------------------------------------------
+def test_state_and_argument_errors(p0):
+    cfg = p0.cfg
+    with gwl.Context(cfg.n_v, cfg.n_c, cfg.n_mu) as ctx:
+        with pytest.raises(gwl.GwlError) as e:
+            ctx.casida_matvec(np.zeros((1, cfg.n_v, cfg.n_c)))
+        assert e.value.status == gwl.GWL_ESTATE
+        with pytest.raises(gwl.GwlError) as e:
+            ctx.set_energies(p0.eps_v, p0.eps_c - 100.0)              # eps_c below eps_v
+        assert e.value.status == gwl.GWL_EINVAL and "eps" in str(e.value)
+        ctx.set_orbitals(p0.phi_v, p0.phi_c)
+        ctx.set_energies(p0.eps_v, p0.eps_c)
+        ctx.set_kernel(p0.V)
+        with pytest.raises(gwl.GwlError) as e:
+            ctx.lanczos(1, 5, 1, 0)                                   # no chains set
+        assert e.value.status == gwl.GWL_ESTATE
+        with pytest.raises(gwl.GwlError) as e:
+            ctx.selfenergy(p0.omega, DLT, 1)                          # before lanczos
+        assert e.value.status == gwl.GWL_ESTATE
+        with pytest.raises(gwl.GwlError):
+            ctx.set_chains([0], [cfg.n_v + cfg.n_c])                  # index out of range
+        ctx.set_chains(p0.n_idx, p0.m_idx)
+        with pytest.raises(gwl.GwlError):
+            ctx.lanczos(5, 5, 1, 0)                                   # more chains than set
+        with pytest.raises(gwl.GwlError):
+            ctx.lanczos(1, 0, 1, 0)                                   # steps < 1
+        a, b, n2, ln = ctx.lanczos(0, 5, 4, 0)                        # empty run is fine
+        assert a.shape == (0, 5)
+        assert ctx.casida_matvec(np.zeros((0, cfg.n_v, cfg.n_c))).shape == (0, cfg.n_v, cfg.n_c)
+        assert ctx.get_launch_count() > 0
+
+
+def test_launches_and_timing_reported(p0):
+    with _ctx(p0) as ctx:
+        n0 = ctx.get_launch_count()
+        ctx.lanczos(4, 10, 4, 0)
+        assert ctx.get_launch_count() - n0 >= 10 * 5
+        tm, tv, tt = ctx.get_timing()
+        assert tm > 0 and tv > 0 and abs(tt - tm - tv) < 1e-9
