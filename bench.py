@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py -- times the whole hot path of the Lanczos full-frequency GW method on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--impl ours|reference]
+
+One "step" = one pass of the whole path over one synthetic problem of
+BASELINE.json:configs[i] (default configs[1]): start vectors, `steps` Lanczos steps of all chains in
+blocks (each step one Casida block product plus the recurrence), Ritz/continued-fraction evaluation of
+Sigma^c on the omega grid and the sum over chains.
+  value   = Lanczos chain-steps/s, whole job, inputs resident in HBM (device-pointer C-ABI calls)
+  e2e     = the same through the host-pointer C-ABI calls: every step uploads orbitals, energies, the
+            Coulomb kernel and the chain list from pinned host memory and reads alpha/beta/Sigma back
+  roofline= the dominant kernel (a Khatri-Rao GEMM) against the FP64 tensor (DMMA) peak
+  cpu_baseline = the NumPy oracle (oracle/gw_oracle.py), as it stands, on the host cores
+N > 1: independent replicas, one per GPU ("replicas only"); value sums their chain-steps over the max time.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "lanczos_chain_steps_per_s"
+UNIT = "chain-steps/s"
+L2_FLUSH_BYTES = 512 << 20
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json:configs (default 1)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--lanczos-steps", type=int, default=0, help="override L (for profiling runs only; marks the line)")
+    return ap.parse_args()
+
+
+def workload_config(cfg, n_gpus, L):
+    return {"workload": f"BASELINE.json:configs[{cfg_index(cfg)}] {cfg.name}", "n_v": cfg.n_v, "n_c": cfg.n_c,
+            "n_mu": cfg.n_mu, "n_vc": cfg.n_vc, "chains": cfg.n_chains, "block": cfg.block, "lanczos_steps": L,
+            "n_omega": cfg.n_omega, "eta_eV": cfg.eta, "mode": "direct (Op = C), reorth off",
+            "parallelism": "single GPU" if n_gpus == 1 else f"{n_gpus} independent replicas",
+            "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB write)", "seed": 0}
+
+
+def cfg_index(cfg):
+    from paper_2310_20103_b200 import synth
+    return synth.CONFIGS.index(cfg)
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(prob, n_chains, L):
+    """Runs the oracle, as it stands, on `n_chains` chains x `L` steps of the workload; returns seconds."""
+    from oracle import gw_oracle as orc
+    t0 = time.perf_counter()
+    orc.run_chains(prob.phi_v, prob.phi_c, prob.eps_v, prob.eps_c, prob.V, prob.n_idx[:n_chains],
+                   prob.m_idx[:n_chains], L, prob.omega, prob.cfg.eta, reorth=False)
+    return time.perf_counter() - t0
+
+
+def host_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [d.get("num_threads", 1) for d in threadpool_info() if d.get("user_api") == "blas"]
+        if n:
+            return int(max(n))
+    except Exception:
+        pass
+    return os.cpu_count() or 1
+
+
+def cpu_baseline(prob, budget_s=12.0):
+    """Oracle timed on a bounded sample of the same workload (about 10-30 s of host work)."""
+    cfg = prob.cfg
+    t1 = oracle_sample(prob, 1, 3)                 # calibration (also warms BLAS)
+    per = max(t1 / 3.0, 1e-6)
+    total = max(4, min(int(budget_s / per), cfg.n_chains * cfg.steps))
+    L = max(2, min(cfg.steps, 20, total))
+    nch = max(1, min(cfg.n_chains, total // L))
+    t = oracle_sample(prob, nch, L)
+    return {"value": nch * L / t, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
+            "sample": f"{nch} chains x {L} Lanczos steps of the same workload + Sigma on the full omega grid, "
+                      f"NumPy/SciPy FP64, {t:.1f} s", "host_cpus": os.cpu_count()}
+
+
+def run_reference(args):
+    """--impl reference: the oracle alone, on the host cores (this tier has no reference code to install)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2310_20103_b200 import synth
+    cfg = synth.CONFIGS[args.config]
+    prob = synth.make_problem(cfg)
+    _ = prob.V
+    t1 = oracle_sample(prob, 1, 2)
+    per = max(t1 / 2.0, 1e-6)
+    budget = 150.0 / max(args.steps + args.warmup, 1)        # whole run within a few minutes
+    total = max(2, int(budget / per))
+    L = max(2, min(cfg.steps, 20, total))
+    nch = max(1, min(cfg.n_chains, total // L))
+    for _ in range(args.warmup):
+        oracle_sample(prob, nch, L)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_sample(prob, nch, L)
+    el = time.perf_counter() - t0
+    val = args.steps * nch * L / el
+    sample = f"each step = {nch} chains x {L} Lanczos steps + Sigma on the omega grid (bounded sample of the workload)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg, args.gpus, cfg.steps),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": host_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    from paper_2310_20103_b200 import gwl, runtime, synth
+
+    rank, local_rank, world = runtime.dist_env()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if not os.path.exists(gwl.LIB_PATH):
+        if rank == 0:
+            from paper_2310_20103_b200 import build
+            build.build()
+        if world > 1:
+            dist.barrier()
+    gwl.load_library()
+
+    cfg = synth.CONFIGS[args.config]
+    L = args.lanczos_steps or cfg.steps
+    prob = synth.make_problem(cfg)
+    V = prob.V
+
+    def pin(a):
+        return torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+
+    h = {k: pin(v) for k, v in dict(phi_v=prob.phi_v, phi_c=prob.phi_c, eps_v=prob.eps_v, eps_c=prob.eps_c, V=V,
+                                    omega=prob.omega).items()}
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+
+    # ---- device-resident arm ----------------------------------------------------------------------
+    ctx = gwl.Context(cfg.n_v, cfg.n_c, cfg.n_mu)
+    ctx.set_stream(stream.cuda_stream)
+    ctx.set_orbitals(h["phi_v"], h["phi_c"])
+    ctx.set_energies(h["eps_v"], h["eps_c"])
+    ctx.set_kernel(h["V"])
+    ctx.set_chains(prob.n_idx, prob.m_idx)
+    ctx.set_pointer_mode(1)
+    ctx.set_profiling(2)
+    omega_d = torch.from_numpy(prob.omega).to(dev)
+    sig_d = torch.empty(cfg.n_chains, cfg.n_omega, 2, dtype=torch.float64, device=dev)
+    sum_d = torch.empty(cfg.n_omega, 2, dtype=torch.float64, device=dev)
+
+    def step_device():
+        ctx.lanczos(cfg.n_chains, L, cfg.block, 0, out=None)
+        ctx.selfenergy(omega_d, cfg.eta, out=(sig_d, sum_d))
+
+    dmma_peak = gwl.probe_fp64_peak(0)            # also warms the clocks
+    for _ in range(args.warmup):
+        step_device()
+    torch.cuda.synchronize()
+    sampler = runtime.ClockSampler(local_rank).start()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    pairs = []
+    ktimes = {k: [0.0, 0] for k in gwl.KERNEL_CLASSES}
+    n0 = ctx.get_launch_count()
+    for _ in range(args.steps):
+        flush.zero_()
+        e0, e1 = ev(), ev()
+        e0.record(stream)
+        step_device()
+        e1.record(stream)
+        pairs.append((e0, e1))
+        for k, (ms, cnt) in ctx.get_kernel_times().items():      # synchronises; outside the event pair
+            ktimes[k][0] += ms
+            ktimes[k][1] += cnt
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    launches = ctx.get_launch_count() - n0
+    clocks = sampler.stop()
+    elapsed_s = sum(a.elapsed_time(b) for a, b in pairs) * 1e-3
+    units = float(args.steps) * cfg.n_chains * L
+    tot_units, max_elapsed = runtime.aggregate_throughput(units, elapsed_s, dev)
+    value = tot_units / max_elapsed
+
+    # ---- the dominant kernel against the FP64 tensor roofline ----------------------------------------
+    gemm_keys = ("gemm_fwd_KX", "gemm_bwd_KtW", "gemm_V")
+    dom = max(gemm_keys, key=lambda k: ktimes[k][0])
+    blocks = -(-cfg.n_chains // cfg.block)
+    flop_launch = {"gemm_fwd_KX": 2.0 * cfg.n_mu * cfg.n_vc * cfg.block, "gemm_bwd_KtW": 2.0 * cfg.n_mu * cfg.n_vc * cfg.block,
+                   "gemm_V": 2.0 * cfg.n_mu * cfg.n_mu * cfg.block}
+    dom_ms = ktimes[dom][0] / max(ktimes[dom][1], 1)
+    achieved = flop_launch[dom] / (dom_ms * 1e-3) / 1e12
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"cfg{args.config}", {}).get(dom)
+    except Exception:
+        pass
+    roofline = {"bound": "tensor", "kernel": f"gemm_tn_dmma<{dom}>", "achieved": achieved, "peak": dmma_peak,
+                "unit": "TFLOP/s", "frac": achieved / dmma_peak, "traffic": traffic,
+                "peak_source": "live register-resident mma.sync.m8n8k4.f64 (DMMA) issue-rate probe on this GPU "
+                               "(gwl_probe_fp64_peak); MEASURED_PEAKS.json has no FP64 entry",
+                "peak_from_bf16_ratio": (peaks.get("bf16_tflops", 0) * 37.0 / 2250.0) or None,
+                "flop_per_launch": flop_launch[dom], "ms_per_launch": dom_ms, "launches_timed": ktimes[dom][1]}
+    step_ms = 1e3 * elapsed_s / args.steps
+    share = {k: round(v[0] / (1e3 * elapsed_s), 4) for k, v in ktimes.items() if v[1]}
+    mv_ms = sum(ktimes[k][0] for k in ("gemm_fwd_KX", "gemm_V", "gemm_bwd_KtW", "splitk_reduce")) / (args.steps * blocks * L)
+    matvec = {"tflops": cfg.flop_per_vector() * cfg.block / (mv_ms * 1e-3) / 1e12, "ms_per_block_matvec": mv_ms,
+              "frac_of_dmma_peak": cfg.flop_per_vector() * cfg.block / (mv_ms * 1e-3) / 1e12 / dmma_peak,
+              "flop_model": "(4 N_mu N_vc + 2 N_mu^2) B"}
+
+    # ---- end-to-end arm: host buffers through the C ABI --------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        hctx = gwl.Context(cfg.n_v, cfg.n_c, cfg.n_mu)
+        hctx.set_stream(stream.cuda_stream)
+        hctx.set_profiling(0)
+
+        def step_host():
+            hctx.set_orbitals(h["phi_v"], h["phi_c"])
+            hctx.set_energies(h["eps_v"], h["eps_c"])
+            hctx.set_kernel(h["V"])
+            hctx.set_chains(prob.n_idx, prob.m_idx)
+            out = hctx.lanczos(cfg.n_chains, L, cfg.block, 0)
+            sig = hctx.selfenergy(h["omega"], cfg.eta, cfg.n_chains)
+            return out, sig
+
+        for _ in range(min(args.warmup, 2)):
+            step_host()
+        ke = max(1, min(args.steps, 3))
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        hp = []
+        for _ in range(ke):
+            flush.zero_()
+            e0, e1 = ev(), ev()
+            e0.record(stream)
+            step_host()
+            e1.record(stream)
+            hp.append((e0, e1))
+        torch.cuda.synchronize()
+        he = sum(a.elapsed_time(b) for a, b in hp) * 1e-3
+        hu, ht = runtime.aggregate_throughput(float(ke) * cfg.n_chains * L, he, dev)
+        h2d = sum(h[k].nbytes for k in ("phi_v", "phi_c", "eps_v", "eps_c", "V", "omega")) + 2 * 4 * cfg.n_chains \
+            + 12 * cfg.n_chains
+        d2h = cfg.n_chains * L * 16 + cfg.n_chains * 12 + cfg.n_chains * cfg.n_omega * 16 + cfg.n_omega * 16
+        e2e = {"value": hu / ht, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "steps": ke, "ms_per_step": 1e3 * he / ke}
+        hctx.close()
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, world, L),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "matvec": matvec,
+                "kernel_time_share": share}
+        if args.lanczos_steps:
+            line["note"] = "lanczos_steps overridden: profiling run, not a bench value"
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(prob)
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

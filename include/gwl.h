@@ -116,6 +116,17 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
  * vector kernels (S4) and overall.  Any pointer may be NULL.  Synchronises the stream. */
 gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total);
 
+/* Profiling level: 0 no events; 1 (default) one CUDA-event triple per Lanczos step (feeds gwl_get_timing);
+ * 2 additionally an event pair around every kernel launch, tagged with its class (feeds gwl_get_kernel_times). */
+gwl_status gwl_set_profiling(gwl_ctx* ctx, int level);
+/* Per-class device time (ms) and launch count since the start of the last gwl_lanczos (including later
+ * gwl_resolvent / gwl_selfenergy calls); needs profiling level 2.  ms and count have GWL_N_KERNEL_CLASSES entries:
+ * 0 K.X GEMM, 1 V GEMM, 2 K^T.W GEMM (with the Delta epilogue), 3 split-K reduction, 4 scaling/axpy/dot
+ * helpers, 5 Lanczos recurrence kernels, 6 reorthogonalisation, 7 continued fraction / Ritz / Sigma.
+ * Synchronises the stream. */
+#define GWL_N_KERNEL_CLASSES 8
+gwl_status gwl_get_kernel_times(gwl_ctx* ctx, double* ms, int64_t* count);
+
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 gwl_status gwl_get_launch_count(gwl_ctx* ctx, int64_t* n_launches);
 

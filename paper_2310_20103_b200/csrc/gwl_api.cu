@@ -80,10 +80,14 @@ struct gwl_ctx {
     DevBuf xs, T, W, part, dotpart, normpart, basis, coefpart, tA, tB, tC, u;
     DevBuf theta, wgt, ritz_info, d_omega, d_zeta, d_sigma, d_sigsum, io_x, io_y;
 
-    // timing
+    // timing: per-step event triples (op start, op end, step end) and, at profiling level 2,
+    // an event pair around every kernel launch tagged with its class
     std::vector<cudaEvent_t> ev;
     size_t ev_used = 0;
-    std::vector<size_t> ev_marks;  // triples: op start, op end, step end
+    int prof_level = 1;
+    std::vector<cudaEvent_t> kev;
+    size_t kev_used = 0;
+    std::vector<int> kev_class;
 
     gwl_status fail(gwl_status st, const std::string& msg) {
         err = msg;
@@ -101,7 +105,36 @@ struct gwl_ctx {
         }
         return ev[ev_used++];
     }
+    cudaEvent_t next_kevent() {
+        if (kev_used == kev.size()) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            kev.push_back(e);
+        }
+        return kev[kev_used++];
+    }
 };
+
+// Event pair around one kernel launch when profiling level 2 is on (gwl_set_profiling).
+struct KernelTimer {
+    gwl_ctx* c;
+    bool on;
+    KernelTimer(gwl_ctx* ctx, int cls) : c(ctx), on(ctx->prof_level >= 2) {
+        if (on) {
+            c->kev_class.push_back(cls);
+            cudaEventRecord(c->next_kevent(), c->stream);
+        }
+    }
+    ~KernelTimer() {
+        if (on) cudaEventRecord(c->next_kevent(), c->stream);
+    }
+};
+#define CKL(cls, call)                                            \
+    do {                                                          \
+        KernelTimer kt__(ctx, cls);                               \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return ctx->cuda_fail(e__, #call); \
+    } while (0)
 
 #define CK(call)                                                  \
     do {                                                          \
@@ -160,9 +193,9 @@ gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double*
         p.out = pl.splits == 1 ? ctx->T.as<double>() : ctx->part.as<double>();
         p.ldo = ldm;
         p.out_split_stride = (int64_t)nb * ldm;
-        CK(launch_gemm(MODE_FWD, EPI_STORE, pl, p, pl.splits, st));
+        CKL(0, launch_gemm(MODE_FWD, EPI_STORE, pl, p, pl.splits, st));
         if (pl.splits > 1)
-            CK(launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->T.as<double>(), ldm,
+            CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->T.as<double>(), ldm,
                                     ctx->n_mu, nb, st));
     }
     {
@@ -181,9 +214,9 @@ gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double*
         p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
         p.ldo = ldm;
         p.out_split_stride = (int64_t)nb * ldm;
-        CK(launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
+        CKL(1, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
         if (pl.splits > 1)
-            CK(launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
+            CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
                                     ctx->n_mu, nb, st));
     }
     {
@@ -209,7 +242,7 @@ gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double*
         p.dotpart = dotpart;
         p.dot_stride = dot_stride;
         p.n_c = ctx->n_c;
-        CK(launch_gemm(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, pl, p, ctx->n_v, st));
+        CKL(2, launch_gemm(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, pl, p, ctx->n_v, st));
     }
     return GWL_OK;
 }
@@ -221,7 +254,7 @@ gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, doub
     cudaStream_t st = ctx->stream;
     const int64_t ldm = ctx->n_mup;
     const int kt_v = ctx->n_mup / BK;
-    CK(launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
+    CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
                   ctx->d_nidx.as<int32_t>() + j0, ctx->d_midx.as<int32_t>() + j0, ctx->T.as<double>(), ldm, nb, st));
     {
         GemmPlan pl = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
@@ -239,9 +272,9 @@ gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, doub
         p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
         p.ldo = ldm;
         p.out_split_stride = (int64_t)nb * ldm;
-        CK(launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
+        CKL(1, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
         if (pl.splits > 1)
-            CK(launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
+            CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
                                     ctx->n_mu, nb, st));
     }
     {
@@ -267,7 +300,7 @@ gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, doub
         p.dotpart = normpart;
         p.dot_stride = dot_stride;
         p.n_c = ctx->n_c;
-        CK(launch_gemm(MODE_BWD, EPI_START, pl, p, ctx->n_v, st));
+        CKL(2, launch_gemm(MODE_BWD, EPI_START, pl, p, ctx->n_v, st));
     }
     return GWL_OK;
 }
@@ -318,6 +351,7 @@ void gwl_destroy(gwl_ctx* ctx) {
                       &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y};
     for (DevBuf* b : bufs) b->release();
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->kev) cudaEventDestroy(e);
     delete ctx;
 }
 
@@ -351,11 +385,11 @@ gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi
     CK(cudaMemsetAsync(ctx->phi_cT.p, 0, ctx->phi_cT.bytes, st));
     CK(cudaMemsetAsync(ctx->phi_vT.p, 0, ctx->phi_vT.bytes, st));
     CK(cudaMemcpyAsync(tmp.p, phi_c, nc * 8, cudaMemcpyHostToDevice, st));
-    CK(launch_copy_pad(tmp.as<double>(), ctx->n_mu, ctx->n_c, ctx->phi_c.as<double>(), ctx->n_cp, st));
-    CK(launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_c, ctx->phi_cT.as<double>(), ctx->n_mup, st));
+    CKL(4, launch_copy_pad(tmp.as<double>(), ctx->n_mu, ctx->n_c, ctx->phi_c.as<double>(), ctx->n_cp, st));
+    CKL(4, launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_c, ctx->phi_cT.as<double>(), ctx->n_mup, st));
     CK(cudaStreamSynchronize(st));
     CK(cudaMemcpyAsync(tmp.p, phi_v, nv * 8, cudaMemcpyHostToDevice, st));
-    CK(launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_v, ctx->phi_vT.as<double>(), ctx->n_mup, st));
+    CKL(4, launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_v, ctx->phi_vT.as<double>(), ctx->n_mup, st));
     CK(cudaStreamSynchronize(st));
     tmp.release();
     ctx->have_orb = true;
@@ -385,7 +419,7 @@ gwl_status gwl_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps
     CK(ctx->s.ensure((size_t)ctx->n_vc * 8, st));
     CK(cudaMemcpyAsync(ctx->eps_v.p, eps_v, (size_t)ctx->n_v * 8, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ctx->eps_c.p, eps_c, (size_t)ctx->n_c * 8, cudaMemcpyHostToDevice, st));
-    CK(launch_build_delta(ctx->eps_v.as<double>(), ctx->eps_c.as<double>(), ctx->n_v, ctx->n_c, ctx->d2.as<double>(),
+    CKL(4, launch_build_delta(ctx->eps_v.as<double>(), ctx->eps_c.as<double>(), ctx->n_v, ctx->n_c, ctx->d2.as<double>(),
                           ctx->s.as<double>(), st));
     CK(cudaStreamSynchronize(st));
     ctx->have_eps = true;
@@ -450,7 +484,7 @@ gwl_status gwl_casida_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t n
             xd = ctx->io_x.as<double>();
             yd = ctx->io_y.as<double>();
         }
-        CK(launch_prescale(xd, ctx->n_vc, ctx->xs.as<double>(), ldxs, ctx->s.as<double>(), ctx->n_v, ctx->n_c,
+        CKL(4, launch_prescale(xd, ctx->n_vc, ctx->xs.as<double>(), ldxs, ctx->s.as<double>(), ctx->n_v, ctx->n_c,
                            ctx->n_cp, nb, st));
         rs = apply_casida_core(ctx, xd, ctx->n_vc, yd, ctx->n_vc, nb, nullptr, 0);
         if (rs != GWL_OK) return rs;
@@ -538,7 +572,8 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
 
     ctx->run_chains = 0;
     ctx->ev_used = 0;
-    ctx->ev_marks.clear();
+    ctx->kev_used = 0;
+    ctx->kev_class.clear();
     CK(ctx->alpha.ensure((size_t)std::max<int64_t>(n_chains, 1) * L * 8, st));
     CK(ctx->beta.ensure((size_t)std::max<int64_t>(n_chains, 1) * L * 8, st));
     CK(ctx->norm2.ensure((size_t)std::max<int64_t>(n_chains, 1) * 8, st));
@@ -582,13 +617,13 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
         if (ctx->chain_mode == 1) {
             gwl_status rs = build_start_vectors(ctx, j0, nb, slot(0), dotpart, ndot_c);
             if (rs != GWL_OK) return rs;
-            CK(launch_lanczos_init(slot(0), n_vc, nb, dotpart, ndot_c, S, ctx->xs.as<double>(), ldxs,
+            CKL(5, launch_lanczos_init(slot(0), n_vc, nb, dotpart, ndot_c, S, ctx->xs.as<double>(), ldxs,
                                    ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
         } else {
             CK(cudaMemcpyAsync(slot(0), ctx->d_start.as<double>() + j0 * n_vc, (size_t)nb * n_vc * 8,
                                cudaMemcpyDeviceToDevice, st));
-            CK(launch_dot_partials(slot(0), slot(0), n_vc, n_vc, nb, normpart, npart, st));
-            CK(launch_lanczos_init(slot(0), n_vc, nb, normpart, npart, S, ctx->xs.as<double>(), ldxs,
+            CKL(4, launch_dot_partials(slot(0), slot(0), n_vc, n_vc, nb, normpart, npart, st));
+            CKL(5, launch_lanczos_init(slot(0), n_vc, nb, normpart, npart, S, ctx->xs.as<double>(), ldxs,
                                    ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
         }
 
@@ -597,8 +632,14 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
             double* q = slot(k);
             double* w = slot(k + 1);
             const double* qp = k > 0 ? slot(k - 1) : nullptr;
-            cudaEvent_t e0 = ctx->next_event(), e1 = ctx->next_event(), e2 = ctx->next_event();
-            CK(cudaEventRecord(e0, st));
+            const bool tstep = ctx->prof_level >= 1;
+            cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
+            if (tstep) {
+                e0 = ctx->next_event();
+                e1 = ctx->next_event();
+                e2 = ctx->next_event();
+                CK(cudaEventRecord(e0, st));
+            }
             int ndot, dstride;
             if (!poly) {
                 gwl_status rs = apply_casida_core(ctx, q, n_vc, w, n_vc, nb, dotpart, ndot_c);
@@ -615,40 +656,40 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
                 if (rs != GWL_OK) return rs;
                 const double* t0 = q;
                 double* t1 = tb[0];
-                CK(launch_axpby3(t1, 2.0 / hl, u, -hs / hl, q, 0.0, nullptr, ntot, st));
-                CK(launch_axpby3(w, ctx->cheb[0], q, ctx->cheb[1], t1, 0.0, nullptr, ntot, st));
+                CKL(4, launch_axpby3(t1, 2.0 / hl, u, -hs / hl, q, 0.0, nullptr, ntot, st));
+                CKL(4, launch_axpby3(w, ctx->cheb[0], q, ctx->cheb[1], t1, 0.0, nullptr, ntot, st));
                 int nxt = 1;
                 for (int jj = 2; jj <= ctx->g; ++jj) {
-                    CK(launch_prescale(t1, n_vc, ctx->xs.as<double>(), ldxs, ctx->s.as<double>(), ctx->n_v, ctx->n_c,
+                    CKL(4, launch_prescale(t1, n_vc, ctx->xs.as<double>(), ldxs, ctx->s.as<double>(), ctx->n_v, ctx->n_c,
                                        ctx->n_cp, nb, st));
                     rs = apply_casida_core(ctx, t1, n_vc, u, n_vc, nb, nullptr, 0);
                     if (rs != GWL_OK) return rs;
                     double* t2 = tb[nxt];
                     // t2 may alias t0 (three rotating buffers, t0 is read element-wise before the write)
-                    CK(launch_axpby3(t2, 4.0 / hl, u, -2.0 * hs / hl, t1, -1.0, t0, ntot, st));
-                    CK(launch_axpby3(w, 1.0, w, ctx->cheb[jj], t2, 0.0, nullptr, ntot, st));
+                    CKL(4, launch_axpby3(t2, 4.0 / hl, u, -2.0 * hs / hl, t1, -1.0, t0, ntot, st));
+                    CKL(4, launch_axpby3(w, 1.0, w, ctx->cheb[jj], t2, 0.0, nullptr, ntot, st));
                     t0 = t1;
                     t1 = t2;
                     nxt = (nxt + 1) % 3;
                     if (tb[nxt] == t0) nxt = (nxt + 1) % 3;
                 }
-                CK(launch_dot_partials(q, w, n_vc, n_vc, nb, dotpart, npart, st));
+                CKL(4, launch_dot_partials(q, w, n_vc, n_vc, nb, dotpart, npart, st));
                 ndot = npart;
                 dstride = npart;
             }
-            CK(cudaEventRecord(e1, st));
-            CK(launch_lanczos_update1(w, q, qp, n_vc, nb, dotpart, ndot, dstride, S, k, normpart, npart, st));
+            if (tstep) CK(cudaEventRecord(e1, st));
+            CKL(5, launch_lanczos_update1(w, q, qp, n_vc, nb, dotpart, ndot, dstride, S, k, normpart, npart, st));
             if (reorth) {
                 for (int pass = 0; pass < 2; ++pass) {
-                    CK(launch_reorth_dots(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), npart,
+                    CKL(6, launch_reorth_dots(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), npart,
                                           st));
-                    CK(launch_reorth_apply(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), npart,
+                    CKL(6, launch_reorth_apply(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), npart,
                                            pass == 1 ? normpart : nullptr, st));
                 }
             }
-            CK(launch_lanczos_update2(w, n_vc, nb, normpart, npart, S, k, ctx->xs.as<double>(), ldxs,
+            CKL(5, launch_lanczos_update2(w, n_vc, nb, normpart, npart, S, k, ctx->xs.as<double>(), ldxs,
                                       ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
-            CK(cudaEventRecord(e2, st));
+            if (tstep) CK(cudaEventRecord(e2, st));
         }
     }
     ctx->run_chains = n_chains;
@@ -683,7 +724,7 @@ gwl_status gwl_resolvent(gwl_ctx* ctx, const double* zeta, int64_t n_zeta, doubl
         dz = ctx->d_zeta.as<double>();
         dr = ctx->d_sigma.as<double>();
     }
-    CK(launch_contfrac(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
+    CKL(7, launch_contfrac(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
                        ctx->len.as<int32_t>(), ctx->run_steps, (int)ctx->run_chains, dz, (int)n_zeta, dr, st));
     if (!ctx->device_ptrs) {
         CK(cudaMemcpyAsync(r, dr, nr, cudaMemcpyDeviceToHost, st));
@@ -721,21 +762,21 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
     }
     if (nch > 0) {
         if (ctx->run_poly) {
-            CK(launch_sigma_poly(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
+            CKL(7, launch_sigma_poly(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
                                  ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
                                  ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));
         } else {
             CK(ctx->theta.ensure((size_t)nch * L * 8, st));
             CK(ctx->wgt.ensure((size_t)nch * L * 8, st));
             CK(ctx->ritz_info.ensure((size_t)nch * 4, st));
-            CK(launch_ritz(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
+            CKL(7, launch_ritz(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
                            ctx->theta.as<double>(), ctx->wgt.as<double>(), nullptr, ctx->ritz_info.as<int32_t>(), st));
-            CK(launch_sigma_direct(ctx->theta.as<double>(), ctx->wgt.as<double>(), ctx->norm2.as<double>(),
+            CKL(7, launch_sigma_direct(ctx->theta.as<double>(), ctx->wgt.as<double>(), ctx->norm2.as<double>(),
                                    ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
                                    ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));
         }
     }
-    if (sigma_sum != nullptr) CK(launch_sigma_sum(dsig, nch, (int)n_omega, dsum, st));
+    if (sigma_sum != nullptr) CKL(7, launch_sigma_sum(dsig, nch, (int)n_omega, dsum, st));
     if (!ctx->device_ptrs) {
         if (sigma != nullptr && nch > 0)
             CK(cudaMemcpyAsync(sigma, dsig, (size_t)nch * n_omega * 16, cudaMemcpyDeviceToHost, st));
@@ -760,6 +801,28 @@ gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, do
     if (ms_matvec) *ms_matvec = tm;
     if (ms_vecops) *ms_vecops = tv;
     if (ms_total) *ms_total = tm + tv;
+    return GWL_OK;
+}
+
+gwl_status gwl_set_profiling(gwl_ctx* ctx, int level) {
+    if (ctx == nullptr || level < 0 || level > 2) return GWL_EINVAL;
+    ctx->prof_level = level;
+    return GWL_OK;
+}
+
+gwl_status gwl_get_kernel_times(gwl_ctx* ctx, double* ms, int64_t* count) {
+    if (ctx == nullptr || ms == nullptr || count == nullptr) return GWL_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < GWL_N_KERNEL_CLASSES; ++i) {
+        ms[i] = 0.0;
+        count[i] = 0;
+    }
+    for (size_t i = 0; i < ctx->kev_class.size() && 2 * i + 1 < ctx->kev_used; ++i) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, ctx->kev[2 * i], ctx->kev[2 * i + 1]));
+        ms[ctx->kev_class[i]] += t;
+        count[ctx->kev_class[i]] += 1;
+    }
     return GWL_OK;
 }
 

@@ -37,9 +37,15 @@ SIGNATURES = {
     "gwl_resolvent": (c_int, [c_void_p, c_void_p, c_int64, c_void_p]),
     "gwl_selfenergy": (c_int, [c_void_p, c_void_p, c_int64, c_double, c_void_p, c_void_p]),
     "gwl_get_timing": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
+    "gwl_set_profiling": (c_int, [c_void_p, c_int]),
+    "gwl_get_kernel_times": (c_int, [c_void_p, POINTER(c_double), POINTER(c_int64)]),
     "gwl_get_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
     "gwl_probe_fp64_peak": (c_int, [c_int, POINTER(c_double)]),
 }
+
+
+KERNEL_CLASSES = ("gemm_fwd_KX", "gemm_V", "gemm_bwd_KtW", "splitk_reduce", "scale_axpy_dot", "lanczos_update",
+                  "reorth", "spectral")
 
 
 class GwlError(RuntimeError):
@@ -247,6 +253,17 @@ class Context:
         a, b, c = c_double(), c_double(), c_double()
         self._ck(self._lib.gwl_get_timing(self._h, byref(a), byref(b), byref(c)))
         return a.value, b.value, c.value
+
+    def set_profiling(self, level: int):
+        self._ck(self._lib.gwl_set_profiling(self._h, int(level)))
+
+    def get_kernel_times(self):
+        """{class name: (ms, launches)} since the start of the last lanczos call (profiling level 2)."""
+        n = len(KERNEL_CLASSES)
+        ms = (c_double * n)()
+        cnt = (c_int64 * n)()
+        self._ck(self._lib.gwl_get_kernel_times(self._h, ms, cnt))
+        return {KERNEL_CLASSES[i]: (ms[i], cnt[i]) for i in range(n)}
 
     def get_launch_count(self) -> int:
         n = c_int64()

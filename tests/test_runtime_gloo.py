@@ -1,0 +1,56 @@
+"""N > 1 path on CPU: two gloo processes aggregate replica throughput exactly as bench.py does
+(sum of chain-steps over ranks / max of elapsed over ranks)."""
+import os
+import subprocess
+import sys
+import textwrap
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = textwrap.dedent("""
+    import os, sys
+    sys.path.insert(0, %r)
+    import torch.distributed as dist
+    from paper_2310_20103_b200 import runtime
+    rank, local_rank, world = runtime.dist_env()
+    dist.init_process_group("gloo")
+    units = 1000.0 * (rank + 1)           # replicas may differ only in the test
+    elapsed = 2.0 + rank                  # rank 1 is slower: the max must win
+    u, t = runtime.aggregate_throughput(units, elapsed)
+    v = runtime.whole_job_value(units, elapsed)
+    dist.barrier()
+    if rank == 0:
+        print("RESULT", world, u, t, v)
+    dist.destroy_process_group()
+""" % ROOT)
+
+
+def test_two_rank_gloo_aggregation(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+           "--master-addr", "127.0.0.1", "--master-port", "29511", str(script)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = [l for l in r.stdout.splitlines() if l.startswith("RESULT")][0].split()
+    assert int(line[1]) == 2
+    assert float(line[2]) == 3000.0 and float(line[3]) == 3.0 and abs(float(line[4]) - 1000.0) < 1e-9
+
+
+def test_single_process_passthrough():
+    from paper_2310_20103_b200 import runtime
+    assert runtime.aggregate_throughput(10.0, 2.0) == (10.0, 2.0)
+    assert runtime.whole_job_value(10.0, 2.0) == 5.0
+    assert runtime.dist_env()[2] >= 1
+
+
+def test_reference_arm_prints_contract_line():
+    """bench.py --impl reference runs the oracle on the host and prints the base-contract JSON line."""
+    import json
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "0",
+                        "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    d = json.loads(r.stdout.strip().splitlines()[-1])
+    assert d["impl"] == "reference" and d["metric"] == "lanczos_chain_steps_per_s" and d["value"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+    assert d["config"]["workload"].startswith("BASELINE.json:configs[0]")
