@@ -175,7 +175,7 @@ def main():
     ctx.set_kernel(h["V"])
     ctx.set_chains(prob.n_idx, prob.m_idx)
     ctx.set_pointer_mode(1)
-    ctx.set_profiling(2)
+    ctx.set_profiling(0)          # no events inside the timed region
     omega_d = torch.from_numpy(prob.omega).to(dev)
     sig_d = torch.empty(cfg.n_chains, cfg.n_omega, 2, dtype=torch.float64, device=dev)
     sum_d = torch.empty(cfg.n_omega, 2, dtype=torch.float64, device=dev)
@@ -193,7 +193,6 @@ def main():
         dist.barrier()
     torch.cuda.synchronize()
     pairs = []
-    ktimes = {k: [0.0, 0] for k in gwl.KERNEL_CLASSES}
     n0 = ctx.get_launch_count()
     for _ in range(args.steps):
         flush.zero_()
@@ -202,15 +201,31 @@ def main():
         step_device()
         e1.record(stream)
         pairs.append((e0, e1))
-        for k, (ms, cnt) in ctx.get_kernel_times().items():      # synchronises; outside the event pair
-            ktimes[k][0] += ms
-            ktimes[k][1] += cnt
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     launches = ctx.get_launch_count() - n0
-    clocks = sampler.stop()
     elapsed_s = sum(a.elapsed_time(b) for a, b in pairs) * 1e-3
+    # Per-kernel durations: the same steps again, immediately, with a CUDA-event pair around every launch
+    # (profiling level 2).  Kept out of the timed region above because ~7000 extra events per step cost a few %.
+    ctx.set_profiling(2)
+    ktimes = {k: [0.0, 0] for k in gwl.KERNEL_CLASSES}
+    prof_steps = max(1, min(args.steps, 3))
+    prof_pairs = []
+    for _ in range(prof_steps):
+        flush.zero_()
+        e0, e1 = ev(), ev()
+        e0.record(stream)
+        step_device()
+        e1.record(stream)
+        prof_pairs.append((e0, e1))
+        for k, (ms, cnt) in ctx.get_kernel_times().items():      # synchronises
+            ktimes[k][0] += ms
+            ktimes[k][1] += cnt
+    torch.cuda.synchronize()
+    prof_elapsed_s = sum(a.elapsed_time(b) for a, b in prof_pairs) * 1e-3
+    ctx.set_profiling(0)
+    clocks = sampler.stop()
     units = float(args.steps) * cfg.n_chains * L
     tot_units, max_elapsed = runtime.aggregate_throughput(units, elapsed_s, dev)
     value = tot_units / max_elapsed
@@ -238,10 +253,12 @@ def main():
                 "peak_source": "live register-resident mma.sync.m8n8k4.f64 (DMMA) issue-rate probe on this GPU "
                                "(gwl_probe_fp64_peak); MEASURED_PEAKS.json has no FP64 entry",
                 "peak_from_bf16_ratio": (peaks.get("bf16_tflops", 0) * 37.0 / 2250.0) or None,
-                "flop_per_launch": flop_launch[dom], "ms_per_launch": dom_ms, "launches_timed": ktimes[dom][1]}
+                "flop_per_launch": flop_launch[dom], "ms_per_launch": dom_ms, "launches_timed": ktimes[dom][1],
+                "timed_how": f"CUDA-event pair around every launch on the library's stream, {prof_steps} extra steps "
+                             "run right after the timed region (events inside it would perturb the step time)"}
     step_ms = 1e3 * elapsed_s / args.steps
-    share = {k: round(v[0] / (1e3 * elapsed_s), 4) for k, v in ktimes.items() if v[1]}
-    mv_ms = sum(ktimes[k][0] for k in ("gemm_fwd_KX", "gemm_V", "gemm_bwd_KtW", "splitk_reduce")) / (args.steps * blocks * L)
+    share = {k: round(v[0] / (1e3 * prof_elapsed_s), 4) for k, v in ktimes.items() if v[1]}
+    mv_ms = sum(ktimes[k][0] for k in ("gemm_fwd_KX", "gemm_V", "gemm_bwd_KtW", "splitk_reduce")) / (prof_steps * blocks * L)
     matvec = {"tflops": cfg.flop_per_vector() * cfg.block / (mv_ms * 1e-3) / 1e12, "ms_per_block_matvec": mv_ms,
               "frac_of_dmma_peak": cfg.flop_per_vector() * cfg.block / (mv_ms * 1e-3) / 1e12 / dmma_peak,
               "flop_model": "(4 N_mu N_vc + 2 N_mu^2) B"}

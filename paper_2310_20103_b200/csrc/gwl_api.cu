@@ -189,6 +189,7 @@ gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double*
         p.kt_per_split = pl.kt_per_split;
         p.scale = ctx->phi_vT.as<double>();
         p.lds = ldm;
+        p.scale_rows = ctx->n_v;
         if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
         p.out = pl.splits == 1 ? ctx->T.as<double>() : ctx->part.as<double>();
         p.ldo = ldm;
@@ -233,6 +234,7 @@ gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double*
         p.kt_per_split = kt_v;
         p.scale = ctx->phi_vT.as<double>();
         p.lds = ldm;
+        p.scale_rows = ctx->n_v;
         p.out = y;
         p.ldo = ldy;
         p.X = x;
@@ -291,6 +293,7 @@ gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, doub
         p.kt_per_split = kt_v;
         p.scale = ctx->phi_vT.as<double>();
         p.lds = ldm;
+        p.scale_rows = ctx->n_v;
         p.out = P;
         p.ldo = ctx->n_vc;
         p.X = nullptr;

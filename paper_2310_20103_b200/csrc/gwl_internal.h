@@ -34,6 +34,7 @@ struct GemmParams {
     int kt_per_split;     // FWD/PLAIN: k-tiles handled by one blockIdx.z
     const double* scale;  // Phi_v^T [n_v][lds]: FWD row scale (index m), BWD k scale (index k)
     int64_t lds;
+    int scale_rows;       // n_v
     double* out;          // EPI_STORE: out[z*out_split_stride + n*ldo + m]; CASIDA/START: out[n*ldo + v*n_c + m]
     int64_t ldo;
     int64_t out_split_stride;
@@ -44,7 +45,6 @@ struct GemmParams {
     double* dotpart;      // CASIDA: sum_m x*y, START: sum_m p*p ; dotpart[n*dot_stride + v*gridDim.x + blockIdx.x]
     int dot_stride;
     int n_c;
-    // TMA descriptors (kernel reads them from param space)
 };
 
 struct GemmPlan {

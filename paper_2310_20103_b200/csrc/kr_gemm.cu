@@ -10,6 +10,10 @@
 // Tiles are staged in shared memory as 128-byte rows (16 doubles) with the TMA SWIZZLE_128B pattern
 // (16-byte chunk index XOR (row & 7)); fragment rows are interleaved (row = 2*g + parity) so that every
 // LDS.64 of a half-warp touches 16 distinct 8-byte bank pairs.
+#include <cuda.h>
+
+#include <cstdlib>
+
 #include "gwl_internal.h"
 
 namespace gwl {
@@ -18,20 +22,41 @@ thread_local int64_t* g_launch_counter = nullptr;
 
 namespace {
 
+// ---- TMA / mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS) ---------------------------------
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n.reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n}\n"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+    asm volatile("prefetch.tensormap [%0];\n" ::"l"(map) : "memory");
+}
+
 __device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
         : "+d"(c0), "+d"(c1)
         : "d"(a), "d"(b));
-}
-
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool valid) {
-    int sz = valid ? 16 : 0;  // src-size 0 => the 16 destination bytes are zero-filled
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(sz) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
 }
 
 template <int BM, int BN, int MODE>
@@ -39,23 +64,36 @@ struct TileCfg {
     static constexpr int A_BYTES = BM * 128;
     static constexpr int B_BYTES = BN * 128;
     static constexpr int SC_BYTES = MODE == MODE_FWD ? BM * 8 : (MODE == MODE_BWD ? 128 : 0);
-    static constexpr int STAGE_BYTES = (A_BYTES + B_BYTES + SC_BYTES + 1023) / 1024 * 1024;
+    static constexpr int TX_BYTES = A_BYTES + B_BYTES + SC_BYTES;           // one k-tile (16 doubles deep)
+    static constexpr int KT_BYTES = (TX_BYTES + 1023) / 1024 * 1024;        // its shared-memory footprint
 };
 
-template <int BM, int BN, int WM, int WN, int STAGES, int MODE, int EPI, int MINB>
-__global__ void __launch_bounds__(256, MINB) gemm_tn_dmma(const GemmParams p) {
+// One CTA = NCW consumer warps (DMMA) + one producer warpgroup (TMA, a single elected lane; the warpgroup gives
+// its registers back with setmaxnreg.dec so that the consumers can take CREGS each with setmaxnreg.inc -- the
+// register file is per SMSP, so a ninth full-size warp would cap everybody at 168 registers).  A pipeline
+// stage holds one k-tile and has one "full" mbarrier (TMA complete_tx) and one "empty" mbarrier
+// (one arrive per consumer warp).  There is no CTA-wide barrier in the main loop: consumer warps drift up to
+// STAGES-1 stages apart and the producer blocks only on the empty barrier of the slot it refills.
+template <int BM, int BN, int WM, int WN, int STAGES, int MODE, int EPI, int CREGS>
+__global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
+    gemm_tn_dmma(const GemmParams p, const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                 const __grid_constant__ CUtensorMap tmS) {
     constexpr int WGM = BM / WM, WGN = BN / WN;
-    static_assert(WGM * WGN == 8, "8 warps per CTA");
+    constexpr int NCW = WGM * WGN;
     static_assert(WM % 16 == 0 && WN % 16 == 0, "warp tile must hold whole 16-row groups");
     constexpr int FM = WM / 8, FN = WN / 8;
     using TC = TileCfg<BM, BN, MODE>;
 
     extern __shared__ unsigned char smem_raw[];
+    __shared__ __align__(8) unsigned long long bars[2 * STAGES];
     const uint32_t smem_base = (static_cast<uint32_t>(__cvta_generic_to_shared(smem_raw)) + 1023u) & ~1023u;
     unsigned char* smem_gen = smem_raw + (smem_base - static_cast<uint32_t>(__cvta_generic_to_shared(smem_raw)));
+    const uint32_t bar_base = static_cast<uint32_t>(__cvta_generic_to_shared(bars));
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm = warp % WGM, wn = warp / WGM;
+    const int wm = warp % WGM, wn = (warp / WGM) % WGN;
     const int g = lane >> 2, q = lane & 3;
     const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN, z = blockIdx.z;
 
@@ -69,45 +107,53 @@ __global__ void __launch_bounds__(256, MINB) gemm_tn_dmma(const GemmParams p) {
     }
     const int nkt = max(kt1 - kt0, 0);
 
-    // ---- producer: one k-tile (A BMx16, B BNx16, scale slice) into stage `slot` -------------------
-    auto load_stage = [&](int kt, int slot) {
-        const uint32_t sA = smem_base + slot * TC::STAGE_BYTES;
-        const uint32_t sB = sA + TC::A_BYTES;
-        const uint32_t sS = sB + TC::B_BYTES;
-        const int64_t a_col = (MODE == MODE_FWD ? (kt % p.a_wrap) : kt) * (int64_t)BK;
-        const int64_t b_col = (int64_t)kt * BK;
+    if (tid == 0) {
+        tma_prefetch_desc(&tmA);
+        tma_prefetch_desc(&tmB);
+        if (MODE != MODE_PLAIN) tma_prefetch_desc(&tmS);
 #pragma unroll
-        for (int id = tid; id < BM * 8; id += 256) {
-            const int row = id >> 3, ch = id & 7;
-            const bool valid = (m0 + row) < p.M;
-            const double* src = p.A + (valid ? (int64_t)(m0 + row) * p.lda + a_col + ch * 2 : 0);
-            cp_async16(sA + row * 128 + ((ch ^ (row & 7)) << 4), src, valid);
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), NCW);
         }
-#pragma unroll
-        for (int id = tid; id < BN * 8; id += 256) {
-            const int row = id >> 3, ch = id & 7;
-            const bool valid = (n0 + row) < p.N;
-            const double* src = p.B + (valid ? (int64_t)(n0 + row) * p.ldb + b_col + ch * 2 : 0);
-            cp_async16(sB + row * 128 + ((ch ^ (row & 7)) << 4), src, valid);
-        }
-        if (MODE == MODE_FWD) {
-            const int v = kt / p.a_wrap;
-            if (tid < BM / 2) {
-                const bool valid = (m0 + 2 * tid) < p.M;
-                const double* src = p.scale + (valid ? (int64_t)v * p.lds + m0 + 2 * tid : 0);
-                cp_async16(sS + tid * 16, src, valid);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp >= NCW) {
+        // ---- producer warpgroup: TMA the k-tiles (A BMx16, B BNx16, scale slice) of each stage ---------------
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
+        if (warp == NCW && lane == 0) {
+            for (int it = 0; it < nkt; ++it) {
+                const int slot = it % STAGES;
+                const uint32_t par = ((it / STAGES) & 1) ^ 1;  // passes at once on a fresh barrier
+                while (!mbar_try_wait(empty_bar(slot), par)) {
+                }
+                const int kt = kt0 + it;
+                const uint32_t fb = full_bar(slot);
+                mbar_expect_tx(fb, TC::TX_BYTES);
+                const uint32_t sA = smem_base + slot * TC::KT_BYTES;
+                const uint32_t sB = sA + TC::A_BYTES;
+                const uint32_t sS = sB + TC::B_BYTES;
+                const int a_col = (MODE == MODE_FWD ? (kt % p.a_wrap) : kt) * BK;
+                tma_load_2d(sA, &tmA, a_col, m0, fb);
+                tma_load_2d(sB, &tmB, kt * BK, n0, fb);
+                if (MODE == MODE_FWD)
+                    tma_load_2d(sS, &tmS, m0, kt / p.a_wrap, fb);
+                else if (MODE == MODE_BWD)
+                    tma_load_2d(sS, &tmS, kt * BK, z, fb);
             }
-        } else if (MODE == MODE_BWD) {
-            if (tid < 8) cp_async16(sS + tid * 16, p.scale + (int64_t)z * p.lds + b_col + 2 * tid, true);
         }
-    };
+        return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(CREGS));
 
     double acc[FM][FN][2];
 #pragma unroll
     for (int i = 0; i < FM; ++i)
 #pragma unroll
         for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
+    // ---- consumer warps --------------------------------------------------------------------------------
     // fragment addressing (doubles): row*16 + (((chunk ^ (row&7)) << 1) | (q&1)), chunk = 2*ks + (q>>1)
     const int xr0 = (2 * (g & 3)), xr1 = xr0 | 1;  // (row & 7) for parity 0 / 1
     int rowA[FM], rowB[FN];
@@ -116,86 +162,103 @@ __global__ void __launch_bounds__(256, MINB) gemm_tn_dmma(const GemmParams p) {
 #pragma unroll
     for (int j = 0; j < FN; ++j) rowB[j] = wn * WN + 16 * (j >> 1) + 2 * g + (j & 1);
 
-#pragma unroll
-    for (int s = 0; s < STAGES - 1; ++s) {
-        if (s < nkt) load_stage(kt0 + s, s);
-        cp_async_commit();
-    }
+    // The k-steps of all k-tiles form one software pipeline: while the 32 (FM*FN) DMMAs of k-step s issue, the
+    // fragments of k-step s+1 are fetched from shared memory and scaled -- across k-tile boundaries too, where
+    // the wait on the next "full" barrier is issued one k-step early so that its latency is hidden as well.
+    double fa[2][FM], fb[2][FN];  // fragment double buffer, indexed by ks & 1 (all indices are compile-time)
+    double fv[FM];                // FWD: phi_v row scales of the k-tile being fetched
 
-    for (int it = 0; it < nkt; ++it) {
-        cp_async_wait<STAGES - 2>();
-        __syncthreads();
-        {
-            const int nx = it + STAGES - 1;
-            if (nx < nkt) load_stage(kt0 + nx, nx % STAGES);
-            cp_async_commit();
-        }
-        const int slot = it % STAGES;
-        const double* As = reinterpret_cast<const double*>(smem_gen + slot * TC::STAGE_BYTES);
-        const double* Bs = reinterpret_cast<const double*>(smem_gen + slot * TC::STAGE_BYTES + TC::A_BYTES);
-        const double* Sc =
-            reinterpret_cast<const double*>(smem_gen + slot * TC::STAGE_BYTES + TC::A_BYTES + TC::B_BYTES);
-
-        double fv[FM];
-        if (MODE == MODE_FWD) {
+    auto fetch = [&](int slot, int ks, double(&a)[FM], double(&b)[FN]) {
+        const unsigned char* base = smem_gen + slot * TC::KT_BYTES;
+        const double* As = reinterpret_cast<const double*>(base);
+        const double* Bs = reinterpret_cast<const double*>(base + TC::A_BYTES);
+        const double* Sc = reinterpret_cast<const double*>(base + TC::A_BYTES + TC::B_BYTES);
+        if (MODE == MODE_FWD && ks == 0) {
 #pragma unroll
             for (int i = 0; i < FM; ++i) fv[i] = Sc[rowA[i]];
         }
+        const int ch = 2 * ks + (q >> 1);
+        const int c0 = ((ch ^ xr0) << 1) | (q & 1);
+        const int c1 = ((ch ^ xr1) << 1) | (q & 1);
 #pragma unroll
-        for (int ks = 0; ks < 4; ++ks) {
-            const int ch = 2 * ks + (q >> 1);
-            const int c0 = ((ch ^ xr0) << 1) | (q & 1);
-            const int c1 = ((ch ^ xr1) << 1) | (q & 1);
-            double a[FM], b[FN];
+        for (int i = 0; i < FM; ++i) a[i] = As[rowA[i] * 16 + ((i & 1) ? c1 : c0)];
 #pragma unroll
-            for (int i = 0; i < FM; ++i) a[i] = As[rowA[i] * 16 + ((i & 1) ? c1 : c0)];
+        for (int j = 0; j < FN; ++j) b[j] = Bs[rowB[j] * 16 + ((j & 1) ? c1 : c0)];
+        if (MODE == MODE_FWD) {
 #pragma unroll
-            for (int j = 0; j < FN; ++j) b[j] = Bs[rowB[j] * 16 + ((j & 1) ? c1 : c0)];
-            if (MODE == MODE_FWD) {
+            for (int i = 0; i < FM; ++i) a[i] *= fv[i];
+        } else if (MODE == MODE_BWD) {
+            const double sk = Sc[4 * ks + q];
+            if (FM <= FN) {
 #pragma unroll
-                for (int i = 0; i < FM; ++i) a[i] *= fv[i];
-            } else if (MODE == MODE_BWD) {
-                const double sk = Sc[4 * ks + q];
-                if (FM <= FN) {
+                for (int i = 0; i < FM; ++i) a[i] *= sk;
+            } else {
 #pragma unroll
-                    for (int i = 0; i < FM; ++i) a[i] *= sk;
-                } else {
-#pragma unroll
-                    for (int j = 0; j < FN; ++j) b[j] *= sk;
-                }
+                for (int j = 0; j < FN; ++j) b[j] *= sk;
             }
-#pragma unroll
-            for (int i = 0; i < FM; ++i)
-#pragma unroll
-                for (int j = 0; j < FN; ++j) dmma_8x8x4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
+    };
+    auto mma_step = [&](const double(&a)[FM], const double(&b)[FN]) {
+#pragma unroll
+        for (int i = 0; i < FM; ++i)
+#pragma unroll
+            for (int j = 0; j < FN; ++j) dmma_8x8x4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+    };
+
+    if (nkt > 0) {
+        while (!mbar_try_wait(full_bar(0), 0)) {
+        }
+        fetch(0, 0, fa[0], fb[0]);
     }
-    cp_async_wait<0>();
-    __syncthreads();
+    for (int it = 0; it < nkt; ++it) {
+        const int slot = it % STAGES;
+        const int nslot = (it + 1) % STAGES;
+        const uint32_t npar = ((it + 1) / STAGES) & 1;
+        const bool has_next = (it + 1 < nkt);
+        fetch(slot, 1, fa[1], fb[1]);
+        mma_step(fa[0], fb[0]);
+        fetch(slot, 2, fa[0], fb[0]);
+        mma_step(fa[1], fb[1]);
+        bool ready = true;
+        if (has_next) ready = mbar_try_wait(full_bar(nslot), npar);  // result is needed one k-step later
+        fetch(slot, 3, fa[1], fb[1]);
+        mma_step(fa[0], fb[0]);
+        if (has_next) {
+            while (!ready) ready = mbar_try_wait(full_bar(nslot), npar);
+            fetch(nslot, 0, fa[0], fb[0]);
+        }
+        mma_step(fa[1], fb[1]);
+        // every fragment of this k-tile has been consumed by a DMMA: hand the slot back to the producer
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty_bar(slot));
+    }
 
     // ---- epilogue ------------------------------------------------------------------------------
     // acc[i][j][e]: row m = m0 + rowA[i] (i even/odd = adjacent rows), col n = n0 + wn*WN + 16*(j>>1) + 2*(2q+e) + (j&1)
+    constexpr bool consumer = true;  // the producer warpgroup has returned
     if (EPI == EPI_STORE) {
-        double* outb = p.out + (int64_t)z * p.out_split_stride;
-        const bool vec_ok = ((p.ldo & 1) == 0) && ((reinterpret_cast<uintptr_t>(outb) & 15) == 0);
+        if (consumer) {
+            double* outb = p.out + (int64_t)z * p.out_split_stride;
+            const bool vec_ok = ((p.ldo & 1) == 0) && ((reinterpret_cast<uintptr_t>(outb) & 15) == 0);
 #pragma unroll
-        for (int i2 = 0; i2 < FM / 2; ++i2) {
-            const int r0 = m0 + wm * WM + 16 * i2 + 2 * g;
+            for (int i2 = 0; i2 < FM / 2; ++i2) {
+                const int r0 = m0 + wm * WM + 16 * i2 + 2 * g;
 #pragma unroll
-            for (int j = 0; j < FN; ++j)
+                for (int j = 0; j < FN; ++j)
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
-                    if (n >= p.N) continue;
-                    double* ptr = outb + (int64_t)n * p.ldo + r0;
-                    const double v0 = acc[2 * i2][j][e], v1 = acc[2 * i2 + 1][j][e];
-                    if (vec_ok && r0 + 1 < p.M) {
-                        *reinterpret_cast<double2*>(ptr) = make_double2(v0, v1);
-                    } else {
-                        if (r0 < p.M) ptr[0] = v0;
-                        if (r0 + 1 < p.M) ptr[1] = v1;
+                    for (int e = 0; e < 2; ++e) {
+                        const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
+                        if (n >= p.N) continue;
+                        double* ptr = outb + (int64_t)n * p.ldo + r0;
+                        const double v0 = acc[2 * i2][j][e], v1 = acc[2 * i2 + 1][j][e];
+                        if (vec_ok && r0 + 1 < p.M) {
+                            *reinterpret_cast<double2*>(ptr) = make_double2(v0, v1);
+                        } else {
+                            if (r0 < p.M) ptr[0] = v0;
+                            if (r0 + 1 < p.M) ptr[1] = v1;
+                        }
                     }
-                }
+            }
         }
     } else {
         const int64_t voff = (int64_t)z * p.n_c;
@@ -205,66 +268,72 @@ __global__ void __launch_bounds__(256, MINB) gemm_tn_dmma(const GemmParams p) {
         double part[FN][2];
 #pragma unroll
         for (int j = 0; j < FN; ++j) part[j][0] = part[j][1] = 0.0;
+        if (consumer) {
 #pragma unroll
-        for (int i2 = 0; i2 < FM / 2; ++i2) {
-            const int r0 = m0 + wm * WM + 16 * i2 + 2 * g;
-            if (r0 >= p.M) continue;
-            const bool two = (r0 + 1 < p.M);
-            const double s0 = p.s[voff + r0], s1 = two ? p.s[voff + r0 + 1] : 0.0;
-            double d0 = 0.0, d1 = 0.0;
-            if (EPI == EPI_CASIDA) {
-                d0 = p.d2[voff + r0];
-                d1 = two ? p.d2[voff + r0 + 1] : 0.0;
-            }
-#pragma unroll
-            for (int j = 0; j < FN; ++j)
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
-                    if (n >= p.N) continue;
-                    const double u0 = acc[2 * i2][j][e], u1 = acc[2 * i2 + 1][j][e];
-                    double y0, y1;
-                    if (EPI == EPI_CASIDA) {
-                        const double* xp = p.X + (int64_t)n * p.ldx + voff + r0;
-                        double x0, x1 = 0.0;
-                        if (vec_ok && two) {
-                            const double2 xv = *reinterpret_cast<const double2*>(xp);
-                            x0 = xv.x;
-                            x1 = xv.y;
-                        } else {
-                            x0 = xp[0];
-                            if (two) x1 = xp[1];
-                        }
-                        y0 = d0 * x0 + 2.0 * (s0 * u0);
-                        y1 = d1 * x1 + 2.0 * (s1 * u1);
-                        part[j][e] += x0 * y0 + x1 * y1;
-                    } else {
-                        y0 = s0 * u0;
-                        y1 = s1 * u1;
-                        part[j][e] += y0 * y0 + y1 * y1;
-                    }
-                    double* yp = p.out + (int64_t)n * p.ldo + voff + r0;
-                    if (vec_ok && two) {
-                        *reinterpret_cast<double2*>(yp) = make_double2(y0, y1);
-                    } else {
-                        yp[0] = y0;
-                        if (two) yp[1] = y1;
-                    }
+            for (int i2 = 0; i2 < FM / 2; ++i2) {
+                const int r0 = m0 + wm * WM + 16 * i2 + 2 * g;
+                if (r0 >= p.M) continue;
+                const bool two = (r0 + 1 < p.M);
+                const double s0 = p.s[voff + r0], s1 = two ? p.s[voff + r0 + 1] : 0.0;
+                double d0 = 0.0, d1 = 0.0;
+                if (EPI == EPI_CASIDA) {
+                    d0 = p.d2[voff + r0];
+                    d1 = two ? p.d2[voff + r0 + 1] : 0.0;
                 }
+#pragma unroll
+                for (int j = 0; j < FN; ++j)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
+                        if (n >= p.N) continue;
+                        const double u0 = acc[2 * i2][j][e], u1 = acc[2 * i2 + 1][j][e];
+                        double y0, y1;
+                        if (EPI == EPI_CASIDA) {
+                            const double* xp = p.X + (int64_t)n * p.ldx + voff + r0;
+                            double x0, x1 = 0.0;
+                            if (vec_ok && two) {
+                                const double2 xv = *reinterpret_cast<const double2*>(xp);
+                                x0 = xv.x;
+                                x1 = xv.y;
+                            } else {
+                                x0 = xp[0];
+                                if (two) x1 = xp[1];
+                            }
+                            y0 = d0 * x0 + 2.0 * (s0 * u0);
+                            y1 = d1 * x1 + 2.0 * (s1 * u1);
+                            part[j][e] += x0 * y0 + x1 * y1;
+                        } else {
+                            y0 = s0 * u0;
+                            y1 = s1 * u1;
+                            part[j][e] += y0 * y0 + y1 * y1;
+                        }
+                        double* yp = p.out + (int64_t)n * p.ldo + voff + r0;
+                        if (vec_ok && two) {
+                            *reinterpret_cast<double2*>(yp) = make_double2(y0, y1);
+                        } else {
+                            yp[0] = y0;
+                            if (two) yp[1] = y1;
+                        }
+                    }
+            }
         }
         if (p.dotpart != nullptr) {
-            double* red = reinterpret_cast<double*>(smem_gen);  // [WGM][BN]; the stages are idle now
+            // every TMA write was consumed before the last empty-arrive; the stages can be reused as scratch
+            asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
+            double* red = reinterpret_cast<double*>(smem_gen);  // [WGM][BN]
+            if (consumer) {
 #pragma unroll
-            for (int j = 0; j < FN; ++j)
+                for (int j = 0; j < FN; ++j)
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    double vsum = part[j][e];
-                    vsum += __shfl_xor_sync(0xffffffffu, vsum, 4);
-                    vsum += __shfl_xor_sync(0xffffffffu, vsum, 8);
-                    vsum += __shfl_xor_sync(0xffffffffu, vsum, 16);
-                    if (g == 0) red[wm * BN + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1)] = vsum;
-                }
-            __syncthreads();
+                    for (int e = 0; e < 2; ++e) {
+                        double vsum = part[j][e];
+                        vsum += __shfl_xor_sync(0xffffffffu, vsum, 4);
+                        vsum += __shfl_xor_sync(0xffffffffu, vsum, 8);
+                        vsum += __shfl_xor_sync(0xffffffffu, vsum, 16);
+                        if (g == 0) red[wm * BN + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1)] = vsum;
+                    }
+            }
+            asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
             if (tid < BN && n0 + tid < p.N) {
                 double ssum = 0.0;
 #pragma unroll
@@ -275,29 +344,100 @@ __global__ void __launch_bounds__(256, MINB) gemm_tn_dmma(const GemmParams p) {
     }
 }
 
-constexpr int kStages = 4;
+using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                             const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                             CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-template <int BM, int BN, int WM, int WN, int MODE, int EPI, int MINB>
+// cuTensorMapEncodeTiled through the runtime's driver entry point: libgwl.so has no link-time dependency on libcuda.
+EncodeFn get_encode_fn() {
+    static EncodeFn fn = nullptr;
+    if (fn == nullptr) {
+        void* ptr = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeFn>(ptr);
+    }
+    return fn;
+}
+
+// 2-D FP64 tensor map over a row-major [rows][ld] array of which `cols` columns are valid; out-of-bounds
+// elements of a box read as zero.
+cudaError_t make_map(CUtensorMap* m, const double* base, uint64_t cols, uint64_t rows, uint64_t ld, uint32_t box_cols,
+                     uint32_t box_rows, bool swizzle) {
+    EncodeFn enc = get_encode_fn();
+    if (enc == nullptr) return cudaErrorNotSupported;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {ld * sizeof(double)};
+    cuuint32_t box[2] = {box_cols, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+template <int BM, int BN, int WM, int WN, int STAGES, int MODE, int EPI, int CREGS>
 cudaError_t launch_one(const GemmParams& p, dim3 grid, cudaStream_t st) {
     using TC = TileCfg<BM, BN, MODE>;
-    constexpr int SMEM = kStages * TC::STAGE_BYTES + 1024;
-    auto kern = gemm_tn_dmma<BM, BN, WM, WN, kStages, MODE, EPI, MINB>;
+    constexpr int SMEM = STAGES * TC::KT_BYTES + 1024;
+    constexpr int NTHREADS = ((BM / WM) * (BN / WN) + 4) * 32;
+    static_assert(SMEM <= 227 * 1024, "stage ring does not fit in shared memory");
+    auto kern = gemm_tn_dmma<BM, BN, WM, WN, STAGES, MODE, EPI, CREGS>;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    kern<<<grid, 256, SMEM, st>>>(p);
+    CUtensorMap tmA, tmB, tmS;
+    const uint64_t kcols = (uint64_t)p.kt_total * BK;
+    const uint64_t a_cols = MODE == MODE_FWD ? (uint64_t)p.a_wrap * BK : kcols;
+    cudaError_t e = make_map(&tmA, p.A, a_cols, (uint64_t)p.M, (uint64_t)p.lda, BK, BM, true);
+    if (e != cudaSuccess) return e;
+    e = make_map(&tmB, p.B, kcols, (uint64_t)p.N, (uint64_t)p.ldb, BK, BN, true);
+    if (e != cudaSuccess) return e;
+    if (MODE == MODE_FWD)  // Phi_v^T [n_v][lds]: box = BM row-scale values of one v
+        e = make_map(&tmS, p.scale, (uint64_t)p.lds, (uint64_t)p.scale_rows, (uint64_t)p.lds, BM, 1, false);
+    else if (MODE == MODE_BWD)  // box = the 16 k-scale values of one v
+        e = make_map(&tmS, p.scale, (uint64_t)p.lds, (uint64_t)p.scale_rows, (uint64_t)p.lds, BK, 1, false);
+    else
+        tmS = tmA;
+    if (e != cudaSuccess) return e;
+    kern<<<grid, NTHREADS, SMEM, st>>>(p, tmA, tmB, tmS);
     count_launch();
     return cudaGetLastError();
+}
+
+// Tile variants.  bn = 128: wide blocks (configs 2-4); bn = 64: narrow blocks (configs 0-1).
+// GWL_GEMM_VARIANT (development knob, read once) selects alternative instantiations for sweeps.
+int gemm_variant() {
+    static int v = -1;
+    if (v < 0) {
+        const char* e = getenv("GWL_GEMM_VARIANT");
+        v = e ? atoi(e) : 0;
+    }
+    return v;
 }
 
 template <int MODE, int EPI>
 cudaError_t launch_mode(const GemmPlan& plan, const GemmParams& p, int nz, cudaStream_t st) {
     dim3 grid((unsigned)ceil_div(p.M, plan.bm), (unsigned)ceil_div(p.N, plan.bn), (unsigned)nz);
-    if (plan.bn == 128) return launch_one<128, 128, 32, 64, MODE, EPI, 1>(p, grid, st);
-    return launch_one<128, 64, 32, 32, MODE, EPI, 2>(p, grid, st);
+    const int var = gemm_variant();
+    if (plan.bn == 128) {
+        switch (var) {
+            case 1: return launch_one<128, 128, 32, 32, 4, MODE, EPI, 104>(p, grid, st);  // 16 consumer warps
+            case 2: return launch_one<128, 128, 32, 64, 6, MODE, EPI, 232>(p, grid, st);
+            case 3: return launch_one<128, 128, 64, 32, 4, MODE, EPI, 232>(p, grid, st);
+            default: return launch_one<128, 128, 32, 64, 4, MODE, EPI, 232>(p, grid, st);
+        }
+    }
+    switch (var) {
+        case 1: return launch_one<128, 64, 32, 16, 4, MODE, EPI, 104>(p, grid, st);  // 16 consumer warps
+        case 2: return launch_one<128, 64, 32, 32, 8, MODE, EPI, 168>(p, grid, st);
+        case 3: return launch_one<128, 64, 16, 64, 4, MODE, EPI, 168>(p, grid, st);
+        default: return launch_one<128, 64, 32, 32, 4, MODE, EPI, 168>(p, grid, st);
+    }
 }
 
 }  // namespace
