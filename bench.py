@@ -87,8 +87,8 @@ def cpu_baseline(prob, budget_s=12.0):
     t1 = oracle_sample(prob, 1, 3)                 # calibration (also warms BLAS)
     per = max(t1 / 3.0, 1e-6)
     total = max(4, min(int(budget_s / per), cfg.n_chains * cfg.steps))
-    L = max(2, min(cfg.steps, 20, total))
-    nch = max(1, min(cfg.n_chains, total // L))
+    nch = max(1, min(cfg.n_chains, total // 20))              # at least 20 steps per sampled chain when affordable
+    L = max(2, min(cfg.steps, total // nch))
     t = oracle_sample(prob, nch, L)
     return {"value": nch * L / t, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
             "sample": f"{nch} chains x {L} Lanczos steps of the same workload + Sigma on the full omega grid, "
@@ -243,9 +243,12 @@ def main():
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
-    traffic = None
+    traffic = None   # dram bytes per launch of that kernel from the committed ncu --set full summary (profiles/traffic.csv)
     try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"cfg{args.config}", {}).get(dom)
+        import csv
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "traffic.csv"))):
+            if int(row["config"]) == args.config and row["kernel_class"] == dom:
+                traffic = float(row["dram_bytes_per_launch"])
     except Exception:
         pass
     roofline = {"bound": "tensor", "kernel": f"gemm_tn_dmma<{dom}>", "achieved": achieved, "peak": dmma_peak,
