@@ -681,6 +681,12 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
                 dstride = npart;
             }
             if (tstep) CK(cudaEventRecord(e1, st));
+            if (!reorth && lanczos_fused_fits(n_vc)) {
+                CKL(5, launch_lanczos_fused(w, q, qp, n_vc, nb, dotpart, ndot, dstride, S, k, ctx->xs.as<double>(), ldxs,
+                                        ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
+                if (tstep) CK(cudaEventRecord(e2, st));
+                continue;
+            }
             CKL(5, launch_lanczos_update1(w, q, qp, n_vc, nb, dotpart, ndot, dstride, S, k, normpart, npart, st));
             if (reorth) {
                 for (int pass = 0; pass < 2; ++pass) {

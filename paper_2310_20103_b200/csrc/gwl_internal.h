@@ -103,6 +103,11 @@ cudaError_t launch_lanczos_update1(double* w, const double* q, const double* q_p
 cudaError_t launch_lanczos_update2(double* w, int64_t n_vc, int nb, const double* normpart, int npart,
                                    LanczosState st_, int k, double* xs, int64_t ldxs, const double* s, int n_v,
                                    int n_c, int n_cp, cudaStream_t st);
+// update1 + update2 in one pass (reorth off) when one chain fits in the registers of a thread-block cluster.
+bool lanczos_fused_fits(int64_t n_vc);
+cudaError_t launch_lanczos_fused(double* w, const double* q, const double* q_prev, int64_t n_vc, int nb,
+                                 const double* dotpart, int ndot, int dot_stride, LanczosState st_, int k, double* xs,
+                                 int64_t ldxs, const double* s, int n_v, int n_c, int n_cp, cudaStream_t st);
 // Full reorthogonalisation pass (classical Gram-Schmidt against basis vectors 0..k of each chain).
 // basis: [k+1 slots][nb][n_vc] with slot stride `slot_stride`; coef partials [nb][k+1][npart].
 cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nslots, const double* w, int64_t n_vc,

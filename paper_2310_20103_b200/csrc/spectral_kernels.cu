@@ -55,9 +55,23 @@ __global__ void k_ritz(const double* __restrict__ alpha, const double* __restric
     double* z = shm + 2 * steps;
     const int j = blockIdx.x;
     const int n = len[j];
+    // Scale T by a power of two (exact) so that f^2 + g^2 below can neither overflow nor lose its small terms.
+    __shared__ double sh_max[32];
+    double mx = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        mx = fmax(mx, fabs(alpha[(int64_t)j * steps + i]));
+        if (i + 1 < n) mx = fmax(mx, fabs(beta[(int64_t)j * steps + i]));
+    }
+    sh_max[threadIdx.x] = mx;
+    __syncthreads();
+    mx = 0.0;
+    for (int i = 0; i < (int)blockDim.x; ++i) mx = fmax(mx, sh_max[i]);
+    int ex = 0;
+    if (mx > 0.0) frexp(mx, &ex);
+    const double sc = ldexp(1.0, -ex), unsc = ldexp(1.0, ex);
     for (int i = threadIdx.x; i < steps; i += blockDim.x) {
-        d[i] = (i < n) ? alpha[(int64_t)j * steps + i] : 0.0;
-        e[i] = (i + 1 < n) ? beta[(int64_t)j * steps + i] : 0.0;
+        d[i] = (i < n) ? sc * alpha[(int64_t)j * steps + i] : 0.0;
+        e[i] = (i + 1 < n) ? sc * beta[(int64_t)j * steps + i] : 0.0;
         z[i] = (i == 0) ? 1.0 : 0.0;
     }
     __syncthreads();
@@ -81,30 +95,43 @@ __global__ void k_ritz(const double* __restrict__ alpha, const double* __restric
                 double r = sqrt(g * g + 1.0);
                 g = d[m] - d[l] + e[l] / (g + copysign(r, g));
                 double s = 1.0, c = 1.0, p = 0.0;
-                int i = m - 1;
-                for (; i >= l; --i) {
-                    double f = s * e[i];
-                    const double bq = c * e[i];
-                    r = sqrt(f * f + g * g);
-                    e[i + 1] = r;
-                    if (r == 0.0) {
-                        d[i + 1] -= p;
+                bool underflow = false;
+                // The rotation chain is one long dependency; rsqrt (one MUFU + Newton steps) replaces the
+                // sqrt-then-divide pair on that critical path.  e[i], d[i] of the next rotation are fetched early.
+                double ei = e[m - 1], di = d[m - 1], dn = d[m];
+                double zf = z[m], zi = z[m - 1];  // zf: the (already rotated) entry i+1, carried in a register
+                for (int i = m - 1; i >= l; --i) {
+                    const double f = s * ei;
+                    const double bq = c * ei;
+                    const double h = f * f + g * g;
+                    const bool more = i > l;
+                    const double e_nx = more ? e[i - 1] : 0.0, d_nx = more ? d[i - 1] : 0.0, z_nx = more ? z[i - 1] : 0.0;
+                    if (h == 0.0) {
+                        e[i + 1] = 0.0;
+                        d[i + 1] = dn - p;
+                        z[i + 1] = zf;
                         e[m] = 0.0;
+                        underflow = true;
                         break;
                     }
-                    const double rinv = 1.0 / r;
+                    const double rinv = rsqrt(h);
+                    e[i + 1] = h * rinv;
                     s = f * rinv;
                     c = g * rinv;
-                    g = d[i + 1] - p;
-                    r = (d[i] - g) * s + 2.0 * c * bq;
+                    g = dn - p;
+                    r = (di - g) * s + 2.0 * c * bq;
                     p = s * r;
                     d[i + 1] = g + p;
                     g = c * r - bq;
-                    f = z[i + 1];
-                    z[i + 1] = s * z[i] + c * f;
-                    z[i] = c * z[i] - s * f;
+                    z[i + 1] = s * zi + c * zf;
+                    zf = c * zi - s * zf;
+                    ei = e_nx;
+                    dn = di;
+                    di = d_nx;
+                    zi = z_nx;
                 }
-                if (r == 0.0 && i >= l) continue;
+                if (underflow) continue;
+                z[l] = zf;
                 d[l] -= p;
                 e[l] = g;
                 e[m] = 0.0;
@@ -114,7 +141,7 @@ __global__ void k_ritz(const double* __restrict__ alpha, const double* __restric
     }
     __syncthreads();
     for (int i = threadIdx.x; i < steps; i += blockDim.x) {
-        theta[(int64_t)j * steps + i] = (i < n) ? d[i] : 0.0;
+        theta[(int64_t)j * steps + i] = (i < n) ? unsc * d[i] : 0.0;
         wgt[(int64_t)j * steps + i] = (i < n) ? z[i] * z[i] : 0.0;
     }
 }

@@ -2,7 +2,11 @@
 // three-term recurrence (Eq. 13) for nb independent chains, with optional two-pass full
 // reorthogonalisation.  All reductions are two-stage and deterministic: a fixed slice per block, a fixed
 // tree inside the block, and consumers re-reduce the per-block partials in a fixed order.
+#include <cooperative_groups.h>
+
 #include "gwl_internal.h"
+
+namespace cg = cooperative_groups;
 
 namespace gwl {
 
@@ -224,6 +228,81 @@ __global__ void k_lanczos_update2(double* __restrict__ w, int64_t n_vc, int nb, 
     }
 }
 
+// Single-pass Lanczos update for vectors that fit in the registers of one thread-block cluster (reorth off):
+//   alpha_k = sum(dotpart);  w <- w - alpha q - beta_k q_prev;  beta_{k+1} = ||w||;  q_next = w / beta_{k+1};  xs = s o q_next
+// One cluster of gridDim.x CTAs per chain; each CTA keeps its slice of w in registers between the two phases and
+// the norm is reduced across the cluster through distributed shared memory in a fixed order (rank 0..CS-1), so that
+// every CTA of the cluster sees the same beta bit for bit.  w, q, q_prev are read once and q_next, xs written once:
+// 40 N_vc bytes per chain-step instead of the 64 N_vc of the two-kernel path.
+template <int EPT>
+__global__ void __launch_bounds__(NT) k_lanczos_fused(double* __restrict__ w, const double* __restrict__ q,
+                                                      const double* __restrict__ q_prev, int64_t n_vc, int nb,
+                                                      const double* __restrict__ dotpart, int ndot, int dot_stride,
+                                                      LanczosState st, int k, double* __restrict__ xs, int64_t ldxs,
+                                                      const double* __restrict__ s, int n_c, int n_cp) {
+    __shared__ double sh[NT / 32 + 1];
+    __shared__ double cl_part;  // this CTA's partial of ||w||^2; read by the other CTAs of the cluster
+    __shared__ double cl_sum;
+    cg::cluster_group cluster = cg::this_cluster();
+    const unsigned rank = cluster.block_rank(), cs = cluster.num_blocks();
+    const int b = blockIdx.y;
+    const int par = k & 1;
+    const bool alive = st.alive[par * nb + b] != 0;
+    double a = block_sum_array(dotpart + (int64_t)b * dot_stride, ndot, sh);
+    if (!alive) a = 0.0;
+    const double bprev = (k > 0) ? st.beta[(int64_t)b * st.steps + k - 1] : 0.0;
+    int64_t lo, hi;
+    slice_of(n_vc, (int)cs, (int)rank, lo, hi);
+    double* wb = w + (int64_t)b * n_vc;
+    const double* qb = q + (int64_t)b * n_vc;
+    const double* qp = q_prev + (int64_t)b * n_vc;
+    double v[EPT];
+    double acc = 0.0;
+#pragma unroll
+    for (int j = 0; j < EPT; ++j) {
+        const int64_t i = lo + threadIdx.x + (int64_t)j * NT;
+        v[j] = 0.0;
+        if (i < hi) {
+            v[j] = (k > 0) ? wb[i] - a * qb[i] - bprev * qp[i] : wb[i] - a * qb[i];
+            acc += v[j] * v[j];
+        }
+    }
+    acc = block_sum(acc, sh);
+    if (threadIdx.x == 0) cl_part = acc;
+    cluster.sync();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (unsigned r = 0; r < cs; ++r) t += *cluster.map_shared_rank(&cl_part, r);
+        cl_sum = t;
+    }
+    __syncthreads();
+    // all remote reads of this cluster are done once every CTA has passed this arrive; the matching wait sits at the end
+    asm volatile("barrier.cluster.arrive.release.aligned;\n" ::: "memory");
+    const double n2 = cl_sum;
+    const double beta = sqrt(n2);
+    const double sc_old = st.scale[par * nb + b];
+    const double sc_new = fmax(sc_old, fabs(a) + beta);
+    const bool broken = !alive || !(beta > 1e-12 * sc_new);
+    if (rank == 0 && threadIdx.x == 0) {
+        st.alpha[(int64_t)b * st.steps + k] = a;
+        st.beta[(int64_t)b * st.steps + k] = broken ? 0.0 : beta;
+        st.scale[(par ^ 1) * nb + b] = sc_new;
+        st.alive[(par ^ 1) * nb + b] = broken ? 0 : 1;
+        if (alive && broken) st.len[b] = k + 1;
+    }
+    double* xsb = xs + (int64_t)b * ldxs;
+#pragma unroll
+    for (int j = 0; j < EPT; ++j) {
+        const int64_t i = lo + threadIdx.x + (int64_t)j * NT;
+        if (i < hi) {
+            const double qv = broken ? 0.0 : v[j] / beta;
+            wb[i] = qv;
+            xsb[xs_index(i, n_c, n_cp)] = s[i] * qv;
+        }
+    }
+    asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory");
+}
+
 // coefpart[(b*nslots + i)*npart + blk] = sum over the slice of basis_i[b] * w[b]
 __global__ void k_reorth_dots(const double* __restrict__ basis, int64_t slot_stride, int nslots,
                               const double* __restrict__ w, int64_t n_vc, double* __restrict__ coefpart, int npart) {
@@ -369,6 +448,41 @@ cudaError_t launch_lanczos_update2(double* w, int64_t n_vc, int nb, const double
     k_lanczos_update2<<<grid, NT, 0, st>>>(w, n_vc, nb, normpart, npart, st_, k, xs, ldxs, s, n_c, n_cp);
     count_launch();
     return cudaGetLastError();
+}
+
+bool lanczos_fused_fits(int64_t n_vc) { return n_vc <= (int64_t)8 * NT * 32; }
+
+cudaError_t launch_lanczos_fused(double* w, const double* q, const double* q_prev, int64_t n_vc, int nb,
+                                 const double* dotpart, int ndot, int dot_stride, LanczosState st_, int k, double* xs,
+                                 int64_t ldxs, const double* s, int n_v, int n_c, int n_cp, cudaStream_t st) {
+    (void)n_v;
+    if (!lanczos_fused_fits(n_vc)) return cudaErrorInvalidValue;
+    const int ept = n_vc <= (int64_t)8 * NT * 8 ? 8 : 32;
+    int cs = 1;
+    while ((int64_t)cs * NT * ept < n_vc) cs *= 2;  // 1, 2, 4 or 8: a function of n_vc alone (chain j does not
+                                                    // depend on what else is in its block)
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)cs, (unsigned)nb);
+    cfg.blockDim = dim3(NT);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cs;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (q_prev == nullptr) q_prev = q;  // never read at k = 0
+    cudaError_t e;
+    if (ept == 8)
+        e = cudaLaunchKernelEx(&cfg, k_lanczos_fused<8>, w, q, q_prev, n_vc, nb, dotpart, ndot, dot_stride, st_, k, xs,
+                               ldxs, s, n_c, n_cp);
+    else
+        e = cudaLaunchKernelEx(&cfg, k_lanczos_fused<32>, w, q, q_prev, n_vc, nb, dotpart, ndot, dot_stride, st_, k, xs,
+                               ldxs, s, n_c, n_cp);
+    count_launch();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nslots, const double* w, int64_t n_vc,
