@@ -45,6 +45,9 @@ struct GemmParams {
     double* dotpart;      // CASIDA: sum_m x*y, START: sum_m p*p ; dotpart[n*dot_stride + v*gridDim.x + blockIdx.x]
     int dot_stride;
     int n_c;
+#ifdef GWL_TRACE
+    unsigned long long* trace;  // development builds only
+#endif
 };
 
 struct GemmPlan {

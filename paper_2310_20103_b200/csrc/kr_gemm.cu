@@ -20,6 +20,25 @@ namespace gwl {
 
 thread_local int64_t* g_launch_counter = nullptr;
 
+#ifdef GWL_TRACE
+// Development builds only (-DGWL_TRACE): per-CTA %globaltimer stamps at entry / first tile landed / main loop done /
+// epilogue done, 4 x uint64 per CTA, written to a caller-provided device buffer.
+unsigned long long* g_trace_buf = nullptr;
+extern "C" void gwl_debug_set_trace(unsigned long long* dev_buf) { g_trace_buf = dev_buf; }
+#define GWL_STAMP(slot)                                                                            \
+    do {                                                                                           \
+        if (p.trace != nullptr && (tid & 31) == 0 && warp == 0) {                                  \
+            unsigned long long t__;                                                                \
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));                                \
+            p.trace[4 * ((blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) + slot] = t__; \
+        }                                                                                          \
+    } while (0)
+#else
+#define GWL_STAMP(slot) \
+    do {                \
+    } while (0)
+#endif
+
 namespace {
 
 // ---- TMA / mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS) ---------------------------------
@@ -106,6 +125,7 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
         kt1 = min(kt0 + p.kt_per_split, p.kt_total);
     }
     const int nkt = max(kt1 - kt0, 0);
+    GWL_STAMP(0);
 
     if (tid == 0) {
         tma_prefetch_desc(&tmA);
@@ -210,6 +230,7 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
         }
         fetch(0, 0, fa[0], fb[0]);
     }
+    GWL_STAMP(1);
     for (int it = 0; it < nkt; ++it) {
         const int slot = it % STAGES;
         const int nslot = (it + 1) % STAGES;
@@ -233,6 +254,7 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
         if (lane == 0) mbar_arrive(empty_bar(slot));
     }
 
+    GWL_STAMP(2);
     // ---- epilogue ------------------------------------------------------------------------------
     // acc[i][j][e]: row m = m0 + rowA[i] (i even/odd = adjacent rows), col n = n0 + wn*WN + 16*(j>>1) + 2*(2q+e) + (j&1)
     constexpr bool consumer = true;  // the producer warpgroup has returned
@@ -280,6 +302,28 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                     d0 = p.d2[voff + r0];
                     d1 = two ? p.d2[voff + r0 + 1] : 0.0;
                 }
+                // all x loads of this row pair are issued before the first store: one L2 round trip per i2 instead of
+                // one per element (x and out never alias, include/gwl.h, but the compiler cannot know)
+                double xr[FN][2][2];
+                if (EPI == EPI_CASIDA) {
+#pragma unroll
+                    for (int j = 0; j < FN; ++j)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
+                            xr[j][e][0] = xr[j][e][1] = 0.0;
+                            if (n >= p.N) continue;
+                            const double* xp = p.X + (int64_t)n * p.ldx + voff + r0;
+                            if (vec_ok && two) {
+                                const double2 xv = __ldg(reinterpret_cast<const double2*>(xp));
+                                xr[j][e][0] = xv.x;
+                                xr[j][e][1] = xv.y;
+                            } else {
+                                xr[j][e][0] = __ldg(xp);
+                                if (two) xr[j][e][1] = __ldg(xp + 1);
+                            }
+                        }
+                }
 #pragma unroll
                 for (int j = 0; j < FN; ++j)
 #pragma unroll
@@ -289,16 +333,7 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                         const double u0 = acc[2 * i2][j][e], u1 = acc[2 * i2 + 1][j][e];
                         double y0, y1;
                         if (EPI == EPI_CASIDA) {
-                            const double* xp = p.X + (int64_t)n * p.ldx + voff + r0;
-                            double x0, x1 = 0.0;
-                            if (vec_ok && two) {
-                                const double2 xv = *reinterpret_cast<const double2*>(xp);
-                                x0 = xv.x;
-                                x1 = xv.y;
-                            } else {
-                                x0 = xp[0];
-                                if (two) x1 = xp[1];
-                            }
+                            const double x0 = xr[j][e][0], x1 = xr[j][e][1];
                             y0 = d0 * x0 + 2.0 * (s0 * u0);
                             y1 = d1 * x1 + 2.0 * (s1 * u1);
                             part[j][e] += x0 * y0 + x1 * y1;
@@ -342,6 +377,7 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             }
         }
     }
+    GWL_STAMP(3);
 }
 
 using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -404,7 +440,14 @@ cudaError_t launch_one(const GemmParams& p, dim3 grid, cudaStream_t st) {
     else
         tmS = tmA;
     if (e != cudaSuccess) return e;
+#ifdef GWL_TRACE
+    GemmParams pt = p;
+    pt.trace = g_trace_buf;
+    if (g_trace_buf != nullptr) g_trace_buf += 4ull * grid.x * grid.y * grid.z;  // consecutive launches, consecutive records
+    kern<<<grid, NTHREADS, SMEM, st>>>(pt, tmA, tmB, tmS);
+#else
     kern<<<grid, NTHREADS, SMEM, st>>>(p, tmA, tmB, tmS);
+#endif
     count_launch();
     return cudaGetLastError();
 }
