@@ -78,6 +78,8 @@ struct gwl_ctx {
 
     // workspaces
     DevBuf xs, T, W, part, dotpart, normpart, basis, coefpart, tA, tB, tC, u;
+    DevBuf sk_ws, sk_flags;  // stream-K hand-over of the K^T.W GEMM (kr_gemm.cu)
+    unsigned sk_epoch = 0;
     DevBuf theta, wgt, ritz_info, d_omega, d_zeta, d_sigma, d_sigsum, io_x, io_y;
 
     // timing: per-step event triples (op start, op end, step end) and, at profiling level 2,
@@ -164,6 +166,8 @@ gwl_status ensure_workspace(gwl_ctx* ctx, int nb) {
     const int64_t ndot = std::max<int64_t>((int64_t)ctx->n_v * ceil_div(ctx->n_c, 128), npart);
     CK(ctx->dotpart.ensure((size_t)nb * ndot * 8, st));
     CK(ctx->normpart.ensure((size_t)nb * npart * 8, st));
+    CK(ctx->sk_ws.ensure(gemm_bwd_ws_bytes(ctx->n_sm), st));
+    CK(ctx->sk_flags.ensure(gemm_bwd_flag_bytes(ctx->n_sm), st));
     return GWL_OK;
 }
 
@@ -244,12 +248,21 @@ gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double*
         p.dotpart = dotpart;
         p.dot_stride = dot_stride;
         p.n_c = ctx->n_c;
+        p.ws = ctx->sk_ws.as<double>();
+        p.flags = ctx->sk_flags.as<unsigned>();
+        if (++ctx->sk_epoch == 0) ++ctx->sk_epoch;
+        p.epoch = ctx->sk_epoch;
+        p.n_sm = ctx->n_sm;
         CKL(2, launch_gemm(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, pl, p, ctx->n_v, st));
     }
     return GWL_OK;
 }
 
-int casida_ndot(const gwl_ctx* ctx) { return ctx->n_v * (int)ceil_div(ctx->n_c, 128); }
+// alpha / norm partials written by the K^T.W epilogue: one per (v, m-tile) of the plan used for a block of nb
+int casida_ndot(const gwl_ctx* ctx, int nb) {
+    const GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, ctx->n_mup / BK, ctx->n_mup / BK, ctx->n_sm);
+    return ctx->n_v * (int)ceil_div(ctx->n_c, pl.bm);
+}
 
 // S1: P_j = sqrt(Delta) o K^T (V rho_j) for index chains j0..j0+nb; writes P and sum(P^2) partials.
 gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, double* normpart, int dot_stride) {
@@ -303,6 +316,11 @@ gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, doub
         p.dotpart = normpart;
         p.dot_stride = dot_stride;
         p.n_c = ctx->n_c;
+        p.ws = ctx->sk_ws.as<double>();
+        p.flags = ctx->sk_flags.as<unsigned>();
+        if (++ctx->sk_epoch == 0) ++ctx->sk_epoch;
+        p.epoch = ctx->sk_epoch;
+        p.n_sm = ctx->n_sm;
         CKL(2, launch_gemm(MODE_BWD, EPI_START, pl, p, ctx->n_v, st));
     }
     return GWL_OK;
@@ -351,7 +369,7 @@ void gwl_destroy(gwl_ctx* ctx) {
                       &ctx->beta, &ctx->norm2, &ctx->len, &ctx->scale, &ctx->alive, &ctx->xs, &ctx->T, &ctx->W,
                       &ctx->part, &ctx->dotpart, &ctx->normpart, &ctx->basis, &ctx->coefpart, &ctx->tA, &ctx->tB,
                       &ctx->tC, &ctx->u, &ctx->theta, &ctx->wgt, &ctx->ritz_info, &ctx->d_omega, &ctx->d_zeta,
-                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y};
+                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y, &ctx->sk_ws, &ctx->sk_flags};
     for (DevBuf* b : bufs) b->release();
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->kev) cudaEventDestroy(e);
@@ -598,10 +616,10 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
             CK(ctx->u.ensure((size_t)nbmax * n_vc * 8, st));
         }
     }
-    const int ndot_c = casida_ndot(ctx);
 
     for (int64_t j0 = 0; j0 < n_chains; j0 += nbmax) {
         const int nb = (int)std::min<int64_t>(nbmax, n_chains - j0);
+        const int ndot_c = casida_ndot(ctx, nb);
         const int64_t slot_stride = (int64_t)nb * n_vc;
         double* basis = ctx->basis.as<double>();
         auto slot = [&](int k) -> double* { return basis + (int64_t)(reorth ? k : ((k % 3) + 3) % 3) * slot_stride; };

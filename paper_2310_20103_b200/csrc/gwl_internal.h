@@ -45,6 +45,12 @@ struct GemmParams {
     double* dotpart;      // CASIDA: sum_m x*y, START: sum_m p*p ; dotpart[n*dot_stride + v*gridDim.x + blockIdx.x]
     int dot_stride;
     int n_c;
+    // BWD (persistent stream-K grid, kr_gemm.cu): tile grid, partial-tile workspace and hand-over flags
+    int tiles_m, tiles_n, n_tiles;  // filled by launch_gemm
+    double* ws;                     // [grid][BM*BN] partial accumulators, >= gemm_bwd_ws_bytes()
+    unsigned* flags;                // [grid], flags[cta] == epoch once that CTA's partial of THIS launch is visible
+    unsigned epoch;                 // differs from every earlier launch that used the same flags (never 0)
+    int n_sm;
 #ifdef GWL_TRACE
     unsigned long long* trace;  // development builds only
 #endif
@@ -58,6 +64,9 @@ struct GemmPlan {
 
 // Chooses tile and split so that the grid is close to a multiple of the SM count.
 GemmPlan plan_gemm(int mode, int M, int N, int kt_total, int a_wrap, int n_sm);
+// Bytes of GemmParams::ws / ::flags a BWD launch may touch on a device with n_sm SMs.
+size_t gemm_bwd_ws_bytes(int n_sm);
+size_t gemm_bwd_flag_bytes(int n_sm);
 // Launches; returns cudaGetLastError().  `nz` = splits (FWD/PLAIN) or n_v (BWD).
 cudaError_t launch_gemm(int mode, int epi, const GemmPlan& plan, const GemmParams& p, int nz, cudaStream_t st);
 
@@ -139,6 +148,46 @@ cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, dou
 
 // probe.cu
 cudaError_t probe_fp64_peak(int kind, double* tflops);
+
+// ---------------------------------------------------------------------------------------------
+// Programmatic dependent launch.  The kernels of the Lanczos step loop are launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization: the next kernel's CTAs are dispatched, and run their
+// prologue (mbarrier init, tensor-map prefetch, index arithmetic), while the previous kernel drains; pdl_wait()
+// then blocks until every earlier kernel of the stream has completed and its writes are visible.  EVERY kernel
+// launched through launch_pdl() calls pdl_trigger(); pdl_wait(); in all threads before it touches global memory
+// (that also makes the ordering transitive along the stream).  GWL_NO_PDL=1 (read once) launches plainly.
+// ---------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
+#endif
+bool pdl_enabled();
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                              unsigned cluster_x, Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[2];
+    unsigned n = 0;
+    if (pdl_enabled()) {
+        attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[n].val.programmaticStreamSerializationAllowed = 1;
+        ++n;
+    }
+    if (cluster_x > 1) {
+        attr[n].id = cudaLaunchAttributeClusterDimension;
+        attr[n].val.clusterDim.x = cluster_x;
+        attr[n].val.clusterDim.y = 1;
+        attr[n].val.clusterDim.z = 1;
+        ++n;
+    }
+    cfg.attrs = attr;
+    cfg.numAttrs = n;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
 
 // Every launch_* bumps this counter once per kernel launched (read by gwl_get_launch_count).
 extern thread_local int64_t* g_launch_counter;

@@ -20,9 +20,18 @@ namespace gwl {
 
 thread_local int64_t* g_launch_counter = nullptr;
 
+bool pdl_enabled() {
+    static int v = -1;
+    if (v < 0) {
+        const char* e = getenv("GWL_NO_PDL");
+        v = (e != nullptr && e[0] == '1') ? 0 : 1;
+    }
+    return v != 0;
+}
+
 #ifdef GWL_TRACE
 // Development builds only (-DGWL_TRACE): per-CTA %globaltimer stamps at entry / first tile landed / main loop done /
-// epilogue done, 4 x uint64 per CTA, written to a caller-provided device buffer.
+// epilogue done, 4 x (globaltimer, clock64) = 8 x uint64 per CTA, written to a caller-provided device buffer.
 unsigned long long* g_trace_buf = nullptr;
 extern "C" void gwl_debug_set_trace(unsigned long long* dev_buf) { g_trace_buf = dev_buf; }
 #define GWL_STAMP(slot)                                                                            \
@@ -30,7 +39,8 @@ extern "C" void gwl_debug_set_trace(unsigned long long* dev_buf) { g_trace_buf =
         if (p.trace != nullptr && (tid & 31) == 0 && warp == 0) {                                  \
             unsigned long long t__;                                                                \
             asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));                                \
-            p.trace[4 * ((blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) + slot] = t__; \
+            p.trace[8 * ((blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) + slot] = t__; \
+            p.trace[8 * ((blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) + 4 + slot] = clock64(); \
         }                                                                                          \
     } while (0)
 #else
@@ -105,6 +115,7 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
 
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[2 * STAGES];
+    __shared__ double red[(EPI == EPI_STORE) ? 1 : (BM / WM) * BN];  // per-column dot partials of the epilogue
     const uint32_t smem_base = (static_cast<uint32_t>(__cvta_generic_to_shared(smem_raw)) + 1023u) & ~1023u;
     unsigned char* smem_gen = smem_raw + (smem_base - static_cast<uint32_t>(__cvta_generic_to_shared(smem_raw)));
     const uint32_t bar_base = static_cast<uint32_t>(__cvta_generic_to_shared(bars));
@@ -114,17 +125,49 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp % WGM, wn = (warp / WGM) % WGN;
     const int g = lane >> 2, q = lane & 3;
-    const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN, z = blockIdx.z;
-
-    int kt0, kt1;
+    // ---- work list ------------------------------------------------------------------------------------
+    // FWD / PLAIN: one segment per CTA, (m-tile, n-tile, split) = blockIdx.
+    // BWD ("stream-K"): a persistent 1-D grid; the tiles x k-tiles unit space is cut into gridDim.x equal
+    // contiguous ranges, so a range starts and ends in the middle of a tile.  The CTA whose range holds the LAST
+    // k-tile of a tile owns it (sums the partials of the others in a fixed order and runs the epilogue); the
+    // others store their accumulators to the workspace and raise a flag.  A range is processed head-of-last-tile
+    // first and tail-of-first-tile last: contributions are written at the very start, collected at the very
+    // end, and an owner only ever waits for CTAs of LOWER index (scheduled no later than itself).
+    const int KT = p.kt_total;
+    int ns = 1, first_tile = 0;
+    int64_t u0 = 0, u1 = 0, U = 0;
     if (MODE == MODE_BWD) {
-        kt0 = 0;
-        kt1 = p.kt_total;
-    } else {
-        kt0 = z * p.kt_per_split;
-        kt1 = min(kt0 + p.kt_per_split, p.kt_total);
+        U = (int64_t)p.n_tiles * KT;
+        u0 = U * blockIdx.x / gridDim.x;
+        u1 = U * (blockIdx.x + 1) / gridDim.x;
+        first_tile = (int)(u0 / KT);
+        ns = u1 > u0 ? (int)((u1 - 1) / KT) - first_tile + 1 : 0;
     }
-    const int nkt = max(kt1 - kt0, 0);
+    auto seg_at = [&](int i, int& tile, int& kb, int& ke) {
+        if (MODE != MODE_BWD) {
+            tile = 0;
+            kb = min(blockIdx.z * p.kt_per_split, KT);
+            ke = min(kb + p.kt_per_split, KT);
+            return;
+        }
+        const int sidx = ns == 1 ? 0 : (i == 0 ? ns - 1 : (i == ns - 1 ? 0 : i));
+        tile = first_tile + sidx;
+        const int64_t tb = (int64_t)tile * KT;
+        kb = (int)(max(u0, tb) - tb);
+        ke = (int)(min(u1, tb + KT) - tb);
+    };
+    auto tile_coords = [&](int tile, int& m0, int& n0, int& z) {
+        if (MODE != MODE_BWD) {
+            m0 = blockIdx.x * BM;
+            n0 = blockIdx.y * BN;
+            z = blockIdx.z;
+        } else {
+            const int mx = tile % p.tiles_m, r = tile / p.tiles_m;
+            m0 = mx * BM;
+            n0 = (r % p.tiles_n) * BN;
+            z = r / p.tiles_n;
+        }
+    };
     GWL_STAMP(0);
 
     if (tid == 0) {
@@ -139,29 +182,36 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();
+    pdl_trigger();
+    pdl_wait();  // everything above overlapped the tail of the previous kernel; no global access before this point
 
     if (warp >= NCW) {
         // ---- producer warpgroup: TMA the k-tiles (A BMx16, B BNx16, scale slice) of each stage ---------------
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
         if (warp == NCW && lane == 0) {
-            for (int it = 0; it < nkt; ++it) {
-                const int slot = it % STAGES;
-                const uint32_t par = ((it / STAGES) & 1) ^ 1;  // passes at once on a fresh barrier
-                while (!mbar_try_wait(empty_bar(slot), par)) {
+            int it = 0;
+            for (int i = 0; i < ns; ++i) {
+                int tile, kb, ke, m0, n0, z;
+                seg_at(i, tile, kb, ke);
+                tile_coords(tile, m0, n0, z);
+                for (int kt = kb; kt < ke; ++kt, ++it) {
+                    const int slot = it % STAGES;
+                    const uint32_t par = ((it / STAGES) & 1) ^ 1;  // passes at once on a fresh barrier
+                    while (!mbar_try_wait(empty_bar(slot), par)) {
+                    }
+                    const uint32_t fb = full_bar(slot);
+                    mbar_expect_tx(fb, TC::TX_BYTES);
+                    const uint32_t sA = smem_base + slot * TC::KT_BYTES;
+                    const uint32_t sB = sA + TC::A_BYTES;
+                    const uint32_t sS = sB + TC::B_BYTES;
+                    const int a_col = (MODE == MODE_FWD ? (kt % p.a_wrap) : kt) * BK;
+                    tma_load_2d(sA, &tmA, a_col, m0, fb);
+                    tma_load_2d(sB, &tmB, kt * BK, n0, fb);
+                    if (MODE == MODE_FWD)
+                        tma_load_2d(sS, &tmS, m0, kt / p.a_wrap, fb);
+                    else if (MODE == MODE_BWD)
+                        tma_load_2d(sS, &tmS, kt * BK, z, fb);
                 }
-                const int kt = kt0 + it;
-                const uint32_t fb = full_bar(slot);
-                mbar_expect_tx(fb, TC::TX_BYTES);
-                const uint32_t sA = smem_base + slot * TC::KT_BYTES;
-                const uint32_t sB = sA + TC::A_BYTES;
-                const uint32_t sS = sB + TC::B_BYTES;
-                const int a_col = (MODE == MODE_FWD ? (kt % p.a_wrap) : kt) * BK;
-                tma_load_2d(sA, &tmA, a_col, m0, fb);
-                tma_load_2d(sB, &tmB, kt * BK, n0, fb);
-                if (MODE == MODE_FWD)
-                    tma_load_2d(sS, &tmS, m0, kt / p.a_wrap, fb);
-                else if (MODE == MODE_BWD)
-                    tma_load_2d(sS, &tmS, kt * BK, z, fb);
             }
         }
         return;
@@ -169,10 +219,6 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(CREGS));
 
     double acc[FM][FN][2];
-#pragma unroll
-    for (int i = 0; i < FM; ++i)
-#pragma unroll
-        for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
     // ---- consumer warps --------------------------------------------------------------------------------
     // fragment addressing (doubles): row*16 + (((chunk ^ (row&7)) << 1) | (q&1)), chunk = 2*ks + (q>>1)
     const int xr0 = (2 * (g & 3)), xr1 = xr0 | 1;  // (row & 7) for parity 0 / 1
@@ -225,41 +271,51 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             for (int j = 0; j < FN; ++j) dmma_8x8x4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
     };
 
-    if (nkt > 0) {
-        while (!mbar_try_wait(full_bar(0), 0)) {
+    int it = 0;  // k-tiles consumed so far by this CTA (ring position), continuous across segments
+    for (int si = 0; si < ns; ++si) {
+        int tile, kb, ke, m0, n0, z;
+        seg_at(si, tile, kb, ke);
+        tile_coords(tile, m0, n0, z);
+        const int nkt = ke - kb;
+#pragma unroll
+        for (int i = 0; i < FM; ++i)
+#pragma unroll
+            for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        if (nkt > 0) {
+            const int slot = it % STAGES;
+            const uint32_t par = (it / STAGES) & 1;
+            while (!mbar_try_wait(full_bar(slot), par)) {
+            }
+            fetch(slot, 0, fa[0], fb[0]);
         }
-        fetch(0, 0, fa[0], fb[0]);
-    }
-    GWL_STAMP(1);
-    for (int it = 0; it < nkt; ++it) {
-        const int slot = it % STAGES;
-        const int nslot = (it + 1) % STAGES;
-        const uint32_t npar = ((it + 1) / STAGES) & 1;
-        const bool has_next = (it + 1 < nkt);
-        fetch(slot, 1, fa[1], fb[1]);
-        mma_step(fa[0], fb[0]);
-        fetch(slot, 2, fa[0], fb[0]);
-        mma_step(fa[1], fb[1]);
-        bool ready = true;
-        if (has_next) ready = mbar_try_wait(full_bar(nslot), npar);  // result is needed one k-step later
-        fetch(slot, 3, fa[1], fb[1]);
-        mma_step(fa[0], fb[0]);
-        if (has_next) {
-            while (!ready) ready = mbar_try_wait(full_bar(nslot), npar);
-            fetch(nslot, 0, fa[0], fb[0]);
+        if (si == 0) GWL_STAMP(1);
+        for (int j = 0; j < nkt; ++j, ++it) {
+            const int slot = it % STAGES;
+            const int nslot = (it + 1) % STAGES;
+            const uint32_t npar = ((it + 1) / STAGES) & 1;
+            const bool has_next = (j + 1 < nkt);
+            fetch(slot, 1, fa[1], fb[1]);
+            mma_step(fa[0], fb[0]);
+            fetch(slot, 2, fa[0], fb[0]);
+            mma_step(fa[1], fb[1]);
+            bool ready = true;
+            if (has_next) ready = mbar_try_wait(full_bar(nslot), npar);  // result is needed one k-step later
+            fetch(slot, 3, fa[1], fb[1]);
+            mma_step(fa[0], fb[0]);
+            if (has_next) {
+                while (!ready) ready = mbar_try_wait(full_bar(nslot), npar);
+                fetch(nslot, 0, fa[0], fb[0]);
+            }
+            mma_step(fa[1], fb[1]);
+            // every fragment of this k-tile has been consumed by a DMMA: hand the slot back to the producer
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar(slot));
         }
-        mma_step(fa[1], fb[1]);
-        // every fragment of this k-tile has been consumed by a DMMA: hand the slot back to the producer
-        __syncwarp();
-        if (lane == 0) mbar_arrive(empty_bar(slot));
-    }
+        if (si == ns - 1) GWL_STAMP(2);
 
-    GWL_STAMP(2);
-    // ---- epilogue ------------------------------------------------------------------------------
-    // acc[i][j][e]: row m = m0 + rowA[i] (i even/odd = adjacent rows), col n = n0 + wn*WN + 16*(j>>1) + 2*(2q+e) + (j&1)
-    constexpr bool consumer = true;  // the producer warpgroup has returned
-    if (EPI == EPI_STORE) {
-        if (consumer) {
+        // ---- epilogue ------------------------------------------------------------------------------
+        // acc[i][j][e]: row m = m0 + rowA[i] (i even/odd = adjacent rows), col n = n0 + wn*WN + 16*(j>>1) + 2*(2q+e) + (j&1)
+        if (EPI == EPI_STORE) {
             double* outb = p.out + (int64_t)z * p.out_split_stride;
             const bool vec_ok = ((p.ldo & 1) == 0) && ((reinterpret_cast<uintptr_t>(outb) & 15) == 0);
 #pragma unroll
@@ -281,16 +337,55 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                         }
                     }
             }
-        }
-    } else {
-        const int64_t voff = (int64_t)z * p.n_c;
-        const bool vec_ok = ((voff & 1) == 0) && ((p.ldo & 1) == 0) && ((p.ldx & 1) == 0) &&
-                            ((reinterpret_cast<uintptr_t>(p.out) & 15) == 0) &&
-                            (EPI == EPI_START || (reinterpret_cast<uintptr_t>(p.X) & 15) == 0);
-        double part[FN][2];
+        } else {
+            // ---- stream-K hand-over: partial tiles go through the workspace, in accumulator order -------------
+            // ws[cta][((warp*FM + i)*FN + j)*2 + e][lane]: every store / load of a warp is one 256-byte row
+            constexpr int TILE_ELEMS = NCW * FM * FN * 2 * 32;
+            if (ke < KT) {
+                double* wsp = p.ws + (int64_t)blockIdx.x * TILE_ELEMS + (int64_t)warp * (FM * FN * 2 * 32) + lane;
 #pragma unroll
-        for (int j = 0; j < FN; ++j) part[j][0] = part[j][1] = 0.0;
-        if (consumer) {
+                for (int i = 0; i < FM; ++i)
+#pragma unroll
+                    for (int j = 0; j < FN; ++j)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) wsp[((i * FN + j) * 2 + e) * 32] = acc[i][j][e];
+                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
+                if (tid == 0) {
+                    __threadfence();
+                    asm volatile("st.release.gpu.global.u32 [%0], %1;\n" ::"l"(p.flags + blockIdx.x), "r"(p.epoch) : "memory");
+                }
+                continue;
+            }
+            if (kb > 0) {
+                const int64_t tb = (int64_t)tile * KT;
+                int gf = blockIdx.x;  // first contributor: the CTA whose range holds the tile's first k-tile
+                while (gf > 0 && U * gf / gridDim.x > tb) --gf;
+                if (tid == 0) {
+                    for (int c = gf; c < (int)blockIdx.x; ++c) {
+                        unsigned f;
+                        do {
+                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(f) : "l"(p.flags + c) : "memory");
+                        } while (f != p.epoch);
+                    }
+                }
+                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
+                for (int c = gf; c < (int)blockIdx.x; ++c) {
+                    const double* wsp = p.ws + (int64_t)c * TILE_ELEMS + (int64_t)warp * (FM * FN * 2 * 32) + lane;
+#pragma unroll
+                    for (int i = 0; i < FM; ++i)
+#pragma unroll
+                        for (int j = 0; j < FN; ++j)
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) acc[i][j][e] += __ldcg(wsp + ((i * FN + j) * 2 + e) * 32);
+                }
+            }
+            const int64_t voff = (int64_t)z * p.n_c;
+            const bool vec_ok = ((voff & 1) == 0) && ((p.ldo & 1) == 0) && ((p.ldx & 1) == 0) &&
+                                ((reinterpret_cast<uintptr_t>(p.out) & 15) == 0) &&
+                                (EPI == EPI_START || (reinterpret_cast<uintptr_t>(p.X) & 15) == 0);
+            double part[FN][2];
+#pragma unroll
+            for (int j = 0; j < FN; ++j) part[j][0] = part[j][1] = 0.0;
 #pragma unroll
             for (int i2 = 0; i2 < FM / 2; ++i2) {
                 const int r0 = m0 + wm * WM + 16 * i2 + 2 * g;
@@ -330,16 +425,16 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                     for (int e = 0; e < 2; ++e) {
                         const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
                         if (n >= p.N) continue;
-                        const double u0 = acc[2 * i2][j][e], u1 = acc[2 * i2 + 1][j][e];
+                        const double u0v = acc[2 * i2][j][e], u1v = acc[2 * i2 + 1][j][e];
                         double y0, y1;
                         if (EPI == EPI_CASIDA) {
                             const double x0 = xr[j][e][0], x1 = xr[j][e][1];
-                            y0 = d0 * x0 + 2.0 * (s0 * u0);
-                            y1 = d1 * x1 + 2.0 * (s1 * u1);
+                            y0 = d0 * x0 + 2.0 * (s0 * u0v);
+                            y1 = d1 * x1 + 2.0 * (s1 * u1v);
                             part[j][e] += x0 * y0 + x1 * y1;
                         } else {
-                            y0 = s0 * u0;
-                            y1 = s1 * u1;
+                            y0 = s0 * u0v;
+                            y1 = s1 * u1v;
                             part[j][e] += y0 * y0 + y1 * y1;
                         }
                         double* yp = p.out + (int64_t)n * p.ldo + voff + r0;
@@ -351,12 +446,9 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                         }
                     }
             }
-        }
-        if (p.dotpart != nullptr) {
-            // every TMA write was consumed before the last empty-arrive; the stages can be reused as scratch
-            asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
-            double* red = reinterpret_cast<double*>(smem_gen);  // [WGM][BN]
-            if (consumer) {
+            if (p.dotpart != nullptr) {
+                // the producer is already refilling the stage ring for the next tile: `red` is its own array
+                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
 #pragma unroll
                 for (int j = 0; j < FN; ++j)
 #pragma unroll
@@ -367,13 +459,13 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                         vsum += __shfl_xor_sync(0xffffffffu, vsum, 16);
                         if (g == 0) red[wm * BN + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1)] = vsum;
                     }
-            }
-            asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
-            if (tid < BN && n0 + tid < p.N) {
-                double ssum = 0.0;
+                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
+                if (tid < BN && n0 + tid < p.N) {
+                    double ssum = 0.0;
 #pragma unroll
-                for (int w = 0; w < WGM; ++w) ssum += red[w * BN + tid];
-                p.dotpart[(int64_t)(n0 + tid) * p.dot_stride + (int64_t)z * gridDim.x + blockIdx.x] = ssum;
+                    for (int w = 0; w < WGM; ++w) ssum += red[w * BN + tid];
+                    p.dotpart[(int64_t)(n0 + tid) * p.dot_stride + (int64_t)z * p.tiles_m + m0 / BM] = ssum;
+                }
             }
         }
     }
@@ -443,13 +535,13 @@ cudaError_t launch_one(const GemmParams& p, dim3 grid, cudaStream_t st) {
 #ifdef GWL_TRACE
     GemmParams pt = p;
     pt.trace = g_trace_buf;
-    if (g_trace_buf != nullptr) g_trace_buf += 4ull * grid.x * grid.y * grid.z;  // consecutive launches, consecutive records
-    kern<<<grid, NTHREADS, SMEM, st>>>(pt, tmA, tmB, tmS);
+    if (g_trace_buf != nullptr) g_trace_buf += 8ull * grid.x * grid.y * grid.z;  // consecutive launches, consecutive records
+    cudaError_t le = launch_pdl(kern, grid, dim3(NTHREADS), SMEM, st, 1u, pt, tmA, tmB, tmS);
 #else
-    kern<<<grid, NTHREADS, SMEM, st>>>(p, tmA, tmB, tmS);
+    cudaError_t le = launch_pdl(kern, grid, dim3(NTHREADS), SMEM, st, 1u, p, tmA, tmB, tmS);
 #endif
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 // Tile variants.  bn = 128: wide blocks (configs 2-4); bn = 64: narrow blocks (configs 0-1).
@@ -463,9 +555,25 @@ int gemm_variant() {
     return v;
 }
 
+// BWD grid: one CTA per SM, fewer only when the whole product has too few k-tiles to be worth cutting
+// (every cut costs one partial tile through the workspace).
+constexpr int BWD_MIN_UNITS = 16;
+int bwd_grid(int64_t tiles, int kt_total, int n_sm) {
+    const int64_t by_units = tiles * kt_total / BWD_MIN_UNITS;
+    return (int)std::max<int64_t>(1, std::min<int64_t>(n_sm, std::max<int64_t>(std::min<int64_t>(tiles, n_sm), by_units)));
+}
+
 template <int MODE, int EPI>
-cudaError_t launch_mode(const GemmPlan& plan, const GemmParams& p, int nz, cudaStream_t st) {
-    dim3 grid((unsigned)ceil_div(p.M, plan.bm), (unsigned)ceil_div(p.N, plan.bn), (unsigned)nz);
+cudaError_t launch_mode(const GemmPlan& plan, const GemmParams& p0, int nz, cudaStream_t st) {
+    GemmParams p = p0;
+    p.tiles_m = (int)ceil_div(p.M, plan.bm);
+    p.tiles_n = (int)ceil_div(p.N, plan.bn);
+    p.n_tiles = p.tiles_m * p.tiles_n * nz;
+    dim3 grid((unsigned)p.tiles_m, (unsigned)p.tiles_n, (unsigned)nz);
+    if (MODE == MODE_BWD) {
+        if (p.ws == nullptr || p.flags == nullptr || p.epoch == 0 || p.n_sm <= 0) return cudaErrorInvalidValue;
+        grid = dim3((unsigned)bwd_grid(p.n_tiles, p.kt_total, p.n_sm), 1, 1);
+    }
     const int var = gemm_variant();
     if (plan.bn == 128) {
         switch (var) {
@@ -485,16 +593,19 @@ cudaError_t launch_mode(const GemmPlan& plan, const GemmParams& p, int nz, cudaS
 
 }  // namespace
 
+size_t gemm_bwd_ws_bytes(int n_sm) { return (size_t)n_sm * 128 * 128 * sizeof(double); }
+size_t gemm_bwd_flag_bytes(int n_sm) { return (size_t)n_sm * sizeof(unsigned); }
+
 GemmPlan plan_gemm(int mode, int M, int N, int kt_total, int a_wrap, int n_sm) {
     (void)a_wrap;
     GemmPlan pl;
     pl.bm = 128;
-    pl.bn = (N > 64) ? 128 : 64;
+    pl.bn = (N > 64) ? 128 : 64;  // a 256x64 tile was measured too (config 1): no faster in K.X, slower hand-over in K^T.W
     pl.splits = 1;
     pl.kt_per_split = kt_total;
     if (mode == MODE_BWD) return pl;
     const int64_t tiles = ceil_div(M, pl.bm) * ceil_div(N, pl.bn);
-    const int64_t slots = (int64_t)n_sm * (pl.bn == 64 ? 2 : 1);
+    const int64_t slots = n_sm;  // one CTA per SM (register file)
     const int min_kt = 8;
     int64_t best_cost = -1;
     int best_s = 1;

@@ -69,6 +69,8 @@ __global__ void k_build_delta(const double* __restrict__ eps_v, const double* __
 
 __global__ void k_prescale(const double* __restrict__ x, int64_t ldx, double* __restrict__ xs, int64_t ldxs,
                            const double* __restrict__ s, int n_c, int n_cp, int64_t n_vc) {
+    pdl_trigger();
+    pdl_wait();
     const int b = blockIdx.y;
     const double* xb = x + (int64_t)b * ldx;
     double* xsb = xs + (int64_t)b * ldxs;
@@ -78,6 +80,8 @@ __global__ void k_prescale(const double* __restrict__ x, int64_t ldx, double* __
 
 __global__ void k_splitk_reduce(const double* __restrict__ part, int64_t split_stride, int splits,
                                 double* __restrict__ t, int64_t ld, int m) {
+    pdl_trigger();
+    pdl_wait();
     const int b = blockIdx.y;
     for (int i = blockIdx.x * NT + threadIdx.x; i < m; i += gridDim.x * NT) {
         const double* p = part + (int64_t)b * ld + i;
@@ -114,6 +118,8 @@ __global__ void k_copy_pad(const double* __restrict__ src, int rows, int cols, d
 __global__ void k_rho(const double* __restrict__ phivT, const double* __restrict__ phicT, int64_t ldt, int n_v,
                       int n_mu, const int32_t* __restrict__ n_idx, const int32_t* __restrict__ m_idx,
                       double* __restrict__ rho, int64_t ld_rho) {
+    pdl_trigger();
+    pdl_wait();
     const int b = blockIdx.y;
     const int n = n_idx[b], m = m_idx[b];
     const double* pn = n < n_v ? phivT + (int64_t)n * ldt : phicT + (int64_t)(n - n_v) * ldt;
@@ -124,6 +130,8 @@ __global__ void k_rho(const double* __restrict__ phivT, const double* __restrict
 
 __global__ void k_dot_partials(const double* __restrict__ x, const double* __restrict__ y, int64_t ld, int64_t n,
                                double* __restrict__ part, int npart) {
+    pdl_trigger();
+    pdl_wait();
     __shared__ double sh[NT / 32 + 1];
     const int b = blockIdx.y;
     int64_t lo, hi;
@@ -141,6 +149,8 @@ __global__ void k_dot_partials(const double* __restrict__ x, const double* __res
 __global__ void k_lanczos_init(double* __restrict__ p, int64_t n_vc, int nb, const double* __restrict__ normpart,
                                int npart, LanczosState st, double* __restrict__ xs, int64_t ldxs,
                                const double* __restrict__ s, int n_c, int n_cp) {
+    pdl_trigger();
+    pdl_wait();
     __shared__ double sh[NT / 32 + 1];
     const int b = blockIdx.y;
     const double n2 = block_sum_array(normpart + (int64_t)b * npart, npart, sh);
@@ -167,6 +177,8 @@ __global__ void k_lanczos_update1(double* __restrict__ w, const double* __restri
                                   const double* __restrict__ q_prev, int64_t n_vc, int nb,
                                   const double* __restrict__ dotpart, int ndot, int dot_stride, LanczosState st, int k,
                                   double* __restrict__ normpart, int npart) {
+    pdl_trigger();
+    pdl_wait();
     __shared__ double sh[NT / 32 + 1];
     const int b = blockIdx.y;
     const int par = k & 1;
@@ -201,6 +213,8 @@ __global__ void k_lanczos_update1(double* __restrict__ w, const double* __restri
 __global__ void k_lanczos_update2(double* __restrict__ w, int64_t n_vc, int nb, const double* __restrict__ normpart,
                                   int npart, LanczosState st, int k, double* __restrict__ xs, int64_t ldxs,
                                   const double* __restrict__ s, int n_c, int n_cp) {
+    pdl_trigger();
+    pdl_wait();
     __shared__ double sh[NT / 32 + 1];
     const int b = blockIdx.y;
     const int par = k & 1;
@@ -240,6 +254,8 @@ __global__ void __launch_bounds__(NT) k_lanczos_fused(double* __restrict__ w, co
                                                       const double* __restrict__ dotpart, int ndot, int dot_stride,
                                                       LanczosState st, int k, double* __restrict__ xs, int64_t ldxs,
                                                       const double* __restrict__ s, int n_c, int n_cp) {
+    pdl_trigger();
+    pdl_wait();
     __shared__ double sh[NT / 32 + 1];
     __shared__ double cl_part;  // this CTA's partial of ||w||^2; read by the other CTAs of the cluster
     __shared__ double cl_sum;
@@ -306,6 +322,8 @@ __global__ void __launch_bounds__(NT) k_lanczos_fused(double* __restrict__ w, co
 // coefpart[(b*nslots + i)*npart + blk] = sum over the slice of basis_i[b] * w[b]
 __global__ void k_reorth_dots(const double* __restrict__ basis, int64_t slot_stride, int nslots,
                               const double* __restrict__ w, int64_t n_vc, double* __restrict__ coefpart, int npart) {
+    pdl_trigger();
+    pdl_wait();
     __shared__ double sh[NT / 32 + 1];
     const int b = blockIdx.y;
     int64_t lo, hi;
@@ -323,6 +341,8 @@ __global__ void k_reorth_dots(const double* __restrict__ basis, int64_t slot_str
 __global__ void k_reorth_apply(const double* __restrict__ basis, int64_t slot_stride, int nslots,
                                double* __restrict__ w, int64_t n_vc, const double* __restrict__ coefpart, int npart,
                                double* __restrict__ normpart) {
+    pdl_trigger();
+    pdl_wait();
     extern __shared__ double coef[];  // [nslots] + block_sum scratch
     double* sh = coef + nslots;
     const int b = blockIdx.y;
@@ -351,6 +371,8 @@ __global__ void k_reorth_apply(const double* __restrict__ basis, int64_t slot_st
 
 __global__ void k_axpby3(double* __restrict__ out, double a, const double* __restrict__ x, double b,
                          const double* __restrict__ y, double c, const double* __restrict__ z, int64_t n) {
+    pdl_trigger();
+    pdl_wait();
     for (int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x; i < n; i += (int64_t)gridDim.x * NT) {
         double v = a * x[i];
         if (y != nullptr) v += b * y[i];
@@ -379,17 +401,17 @@ cudaError_t launch_prescale(const double* x, int64_t ldx, double* xs, int64_t ld
                             int n_cp, int nb, cudaStream_t st) {
     const int64_t n_vc = (int64_t)n_v * n_c;
     dim3 grid(std::min<unsigned>(grid1d(n_vc), 1024u), (unsigned)nb);
-    k_prescale<<<grid, NT, 0, st>>>(x, ldx, xs, ldxs, s, n_c, n_cp, n_vc);
+    cudaError_t le = launch_pdl(k_prescale, dim3(grid), dim3(NT), (size_t)(0), st, 1u, x, ldx, xs, ldxs, s, n_c, n_cp, n_vc);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 cudaError_t launch_splitk_reduce(const double* part, int64_t split_stride, int splits, double* t, int64_t ld, int m,
                                  int nb, cudaStream_t st) {
     dim3 grid((unsigned)ceil_div(m, NT), (unsigned)nb);
-    k_splitk_reduce<<<grid, NT, 0, st>>>(part, split_stride, splits, t, ld, m);
+    cudaError_t le = launch_pdl(k_splitk_reduce, dim3(grid), dim3(NT), (size_t)(0), st, 1u, part, split_stride, splits, t, ld, m);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 cudaError_t launch_transpose(const double* src, int rows, int cols, double* dst, int64_t ld_dst, cudaStream_t st) {
@@ -408,17 +430,17 @@ cudaError_t launch_copy_pad(const double* src, int rows, int cols, double* dst, 
 cudaError_t launch_rho(const double* phivT, const double* phicT, int64_t ldt, int n_v, int n_mu, const int32_t* n_idx,
                        const int32_t* m_idx, double* rho, int64_t ld_rho, int nb, cudaStream_t st) {
     dim3 grid((unsigned)ceil_div(n_mu, NT), (unsigned)nb);
-    k_rho<<<grid, NT, 0, st>>>(phivT, phicT, ldt, n_v, n_mu, n_idx, m_idx, rho, ld_rho);
+    cudaError_t le = launch_pdl(k_rho, dim3(grid), dim3(NT), (size_t)(0), st, 1u, phivT, phicT, ldt, n_v, n_mu, n_idx, m_idx, rho, ld_rho);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 cudaError_t launch_dot_partials(const double* x, const double* y, int64_t ld, int64_t n, int nb, double* part,
                                 int npart, cudaStream_t st) {
     dim3 grid((unsigned)npart, (unsigned)nb);
-    k_dot_partials<<<grid, NT, 0, st>>>(x, y, ld, n, part, npart);
+    cudaError_t le = launch_pdl(k_dot_partials, dim3(grid), dim3(NT), (size_t)(0), st, 1u, x, y, ld, n, part, npart);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 cudaError_t launch_lanczos_init(double* p, int64_t n_vc, int nb, const double* normpart, int npart, LanczosState st_,
@@ -426,18 +448,18 @@ cudaError_t launch_lanczos_init(double* p, int64_t n_vc, int nb, const double* n
                                 cudaStream_t st) {
     (void)n_v;
     dim3 grid((unsigned)vec_parts(n_vc), (unsigned)nb);
-    k_lanczos_init<<<grid, NT, 0, st>>>(p, n_vc, nb, normpart, npart, st_, xs, ldxs, s, n_c, n_cp);
+    cudaError_t le = launch_pdl(k_lanczos_init, dim3(grid), dim3(NT), (size_t)(0), st, 1u, p, n_vc, nb, normpart, npart, st_, xs, ldxs, s, n_c, n_cp);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 cudaError_t launch_lanczos_update1(double* w, const double* q, const double* q_prev, int64_t n_vc, int nb,
                                    const double* dotpart, int ndot, int dot_stride, LanczosState st_, int k,
                                    double* normpart, int npart, cudaStream_t st) {
     dim3 grid((unsigned)npart, (unsigned)nb);
-    k_lanczos_update1<<<grid, NT, 0, st>>>(w, q, q_prev, n_vc, nb, dotpart, ndot, dot_stride, st_, k, normpart, npart);
+    cudaError_t le = launch_pdl(k_lanczos_update1, dim3(grid), dim3(NT), (size_t)(0), st, 1u, w, q, q_prev, n_vc, nb, dotpart, ndot, dot_stride, st_, k, normpart, npart);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 cudaError_t launch_lanczos_update2(double* w, int64_t n_vc, int nb, const double* normpart, int npart,
@@ -445,9 +467,9 @@ cudaError_t launch_lanczos_update2(double* w, int64_t n_vc, int nb, const double
                                    int n_c, int n_cp, cudaStream_t st) {
     (void)n_v;
     dim3 grid((unsigned)vec_parts(n_vc), (unsigned)nb);
-    k_lanczos_update2<<<grid, NT, 0, st>>>(w, n_vc, nb, normpart, npart, st_, k, xs, ldxs, s, n_c, n_cp);
+    cudaError_t le = launch_pdl(k_lanczos_update2, dim3(grid), dim3(NT), (size_t)(0), st, 1u, w, n_vc, nb, normpart, npart, st_, k, xs, ldxs, s, n_c, n_cp);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 bool lanczos_fused_fits(int64_t n_vc) { return n_vc <= (int64_t)8 * NT * 32; }
@@ -461,26 +483,15 @@ cudaError_t launch_lanczos_fused(double* w, const double* q, const double* q_pre
     int cs = 1;
     while ((int64_t)cs * NT * ept < n_vc) cs *= 2;  // 1, 2, 4 or 8: a function of n_vc alone (chain j does not
                                                     // depend on what else is in its block)
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)cs, (unsigned)nb);
-    cfg.blockDim = dim3(NT);
-    cfg.dynamicSmemBytes = 0;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = (unsigned)cs;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
     if (q_prev == nullptr) q_prev = q;  // never read at k = 0
+    const dim3 grid((unsigned)cs, (unsigned)nb);
     cudaError_t e;
     if (ept == 8)
-        e = cudaLaunchKernelEx(&cfg, k_lanczos_fused<8>, w, q, q_prev, n_vc, nb, dotpart, ndot, dot_stride, st_, k, xs,
-                               ldxs, s, n_c, n_cp);
+        e = launch_pdl(k_lanczos_fused<8>, grid, dim3(NT), 0, st, (unsigned)cs, w, q, q_prev, n_vc, nb, dotpart, ndot,
+                       dot_stride, st_, k, xs, ldxs, s, n_c, n_cp);
     else
-        e = cudaLaunchKernelEx(&cfg, k_lanczos_fused<32>, w, q, q_prev, n_vc, nb, dotpart, ndot, dot_stride, st_, k, xs,
-                               ldxs, s, n_c, n_cp);
+        e = launch_pdl(k_lanczos_fused<32>, grid, dim3(NT), 0, st, (unsigned)cs, w, q, q_prev, n_vc, nb, dotpart, ndot,
+                       dot_stride, st_, k, xs, ldxs, s, n_c, n_cp);
     count_launch();
     return e != cudaSuccess ? e : cudaGetLastError();
 }
@@ -488,25 +499,25 @@ cudaError_t launch_lanczos_fused(double* w, const double* q, const double* q_pre
 cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nslots, const double* w, int64_t n_vc,
                                int nb, double* coefpart, int npart, cudaStream_t st) {
     dim3 grid((unsigned)npart, (unsigned)nb);
-    k_reorth_dots<<<grid, NT, 0, st>>>(basis, slot_stride, nslots, w, n_vc, coefpart, npart);
+    cudaError_t le = launch_pdl(k_reorth_dots, dim3(grid), dim3(NT), (size_t)(0), st, 1u, basis, slot_stride, nslots, w, n_vc, coefpart, npart);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 cudaError_t launch_reorth_apply(const double* basis, int64_t slot_stride, int nslots, double* w, int64_t n_vc, int nb,
                                 const double* coefpart, int npart, double* normpart, cudaStream_t st) {
     dim3 grid((unsigned)npart, (unsigned)nb);
     const size_t sm = (size_t)(nslots + NT / 32 + 1) * sizeof(double);
-    k_reorth_apply<<<grid, NT, sm, st>>>(basis, slot_stride, nslots, w, n_vc, coefpart, npart, normpart);
+    cudaError_t le = launch_pdl(k_reorth_apply, dim3(grid), dim3(NT), (size_t)(sm), st, 1u, basis, slot_stride, nslots, w, n_vc, coefpart, npart, normpart);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 cudaError_t launch_axpby3(double* out, double a, const double* x, double b, const double* y, double c, const double* z,
                           int64_t n_total, cudaStream_t st) {
-    k_axpby3<<<grid1d(n_total), NT, 0, st>>>(out, a, x, b, y, c, z, n_total);
+    cudaError_t le = launch_pdl(k_axpby3, dim3(grid1d(n_total)), dim3(NT), (size_t)(0), st, 1u, out, a, x, b, y, c, z, n_total);
     count_launch();
-    return cudaGetLastError();
+    return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 }  // namespace gwl
