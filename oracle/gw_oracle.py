@@ -349,3 +349,62 @@ def run_chains(phi_v, phi_c, eps_v, eps_c, V, n_idx, m_idx, steps, omega, dlt,
         out["sigma"][j] = f(a, b, n2, ln, omega, eps_n, sgn, dlt)
     out["sigma_sum"] = sigma_sum(out["sigma"])
     return out
+
+
+# --------------------------------------------------------------------------- #
+# exchange part and the quasiparticle equation              #
+# --------------------------------------------------------------------------- #
+def exchange_eq6(phi_v, phi_c, V, m_idx):
+    """Sigma^ex_mm = - sum_v (vm|vm), PAPER.md:57 (Eq. 6; the printed summation index "m" is read as
+    the occupied orbital v, Q15), with (vm|vm) = rho_vm^T V rho_vm, rho_vm(mu) = phi_v(r_mu) phi_m(r_mu)
+    (Eq. 16 under Q4)."""
+    pm = orbital_column(phi_v, phi_c, m_idx)
+    tot = 0.0
+    for v in range(phi_v.shape[1]):
+        rho = phi_v[:, v] * pm
+        tot += rho @ (V @ rho)
+    return -tot
+
+
+def sigma_state(phi_v, phi_c, eps_v, eps_c, V, m_idx, steps, omega, dlt, reorth=False, poly=None):
+    """Sigma^corr_mm(omega) = sum over ALL n = 1..N_v+N_c of Sigma^corr_mm(omega, n), PAPER.md:73 (Eq. 10):
+    one Lanczos chain per n started from |P_nm>."""
+    n_orb = phi_v.shape[1] + phi_c.shape[1]
+    n_idx = np.arange(n_orb, dtype=np.int32)
+    r = run_chains(phi_v, phi_c, eps_v, eps_c, V, n_idx, np.full(n_orb, m_idx, dtype=np.int32), steps, omega, dlt,
+                   reorth=reorth, poly=poly)
+    return r["sigma_sum"]
+
+
+QP_MAX_ITER = 50
+QP_TOL = 1e-10   # eV
+
+
+def qp_solve(eps_m, vxc_m, sigma_x, sigma_c, omega):
+    """Quasiparticle equation of: E(omega) = eps_m + <m|Sigma(omega) - V_xc|m> is known on the
+    frequency grid; "the Newton-Raphson algorithm is used to get a graphical solution of E(omega) = omega".
+    Reading Q18 (the paper gives no more detail): F(w) = eps_m + Re[Sigma^ex + Sigma^corr(w)] - V_xc - w with
+    Re Sigma^corr interpolated linearly between grid points; Newton from w_0 = eps_m,
+    w <- w - F(w)/F'(w), F' = (slope of the grid interval holding w) - 1, w clamped to the grid range, until
+    |step| <= 1e-10 eV or 50 iterations.  Returns (E_qp, Z, iterations), Z = 1/(1 - dReSigma/dw) = -1/F'."""
+    omega = np.asarray(omega, dtype=np.float64)
+    re = np.real(np.asarray(sigma_c))
+    n = len(omega)
+    w = min(max(float(eps_m), omega[0]), omega[-1])
+    z = 1.0
+    it = 0
+    for it in range(1, QP_MAX_ITER + 1):
+        i = int(np.searchsorted(omega, w, side="right")) - 1      # largest i with omega[i] <= w
+        i = min(max(i, 0), n - 2)
+        slope = (re[i + 1] - re[i]) / (omega[i + 1] - omega[i])
+        s_w = re[i] + slope * (w - omega[i])
+        F = eps_m + sigma_x + s_w - vxc_m - w
+        dF = slope - 1.0
+        z = -1.0 / dF
+        step = -F / dF
+        w_new = min(max(w + step, omega[0]), omega[-1])
+        done = abs(w_new - w) <= QP_TOL
+        w = w_new
+        if done:
+            break
+    return w, z, it

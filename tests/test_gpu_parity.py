@@ -301,6 +301,32 @@ def test_lanczos_config1_sampled(p1):
     assert np.abs(sig - ref["sigma"]).max() <= TOL_SIGMA
 
 
+def _sampled_lanczos(cfg_id, idx, nb_gpu):
+    """Configs 2-4 (SURVEY.md §8(c) protocol items 2-3): a GPU block of nb_gpu chains in the bench launch
+    configuration; the oracle follows the sampled chains for 30 steps (reorth off): alpha/beta and Sigma."""
+    p = synth.make_problem(cfg_id)
+    _ = p.V
+    idx = np.asarray(idx)
+    with _ctx(p) as ctx:
+        a, b, n2, ln = ctx.lanczos(nb_gpu, 30, min(nb_gpu, p.cfg.block), 0)
+        sig, _ = ctx.selfenergy(p.omega, DLT, nb_gpu)
+    ref = _oracle_chains(p, idx, 30, False)
+    assert (np.abs(n2[idx] - ref["norm2"]) <= 1e-12 * ref["norm2"]).all()
+    _check_ab(a[idx], b[idx], ref["alpha"], ref["beta"], 30)
+    assert np.abs(sig[idx] - ref["sigma"]).max() <= TOL_SIGMA
+
+
+def test_lanczos_config2_sampled_chains():
+    """Full block of 256 chains at the ~100-atom size on the GPU; two chains followed by the oracle."""
+    _sampled_lanczos(2, [3, 200], synth.CONFIGS[2].block)
+
+
+@pytest.mark.skipif(os.environ.get("GWL_TEST_LARGE", "0") != "1", reason="set GWL_TEST_LARGE=1 (minutes of host time)")
+@pytest.mark.parametrize("cfg_id", [3, 4])
+def test_lanczos_large_configs_sampled_chains(cfg_id):
+    _sampled_lanczos(cfg_id, [1, synth.CONFIGS[cfg_id].block - 2], synth.CONFIGS[cfg_id].block)
+
+
 # ---- API behaviour -------------------------------------------------------------------------------------
 def test_state_and_argument_errors(p0):
     cfg = p0.cfg

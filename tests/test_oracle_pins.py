@@ -350,3 +350,63 @@ def test_run_chains_config0(cfg0, dense0):
         assert np.abs(out["beta"][j] - b).max() <= 1e-10 * np.abs(a).max()
         assert abs(out["norm2"][j] - n2) <= 1e-13 * n2
     assert np.abs(out["sigma_sum"] - out["sigma"].sum(axis=0)).max() == 0
+
+
+# ---- exchange part, Sigma_mm over all n, quasiparticle equation ------------------
+def test_exchange_eq6_bruteforce_and_hadamard_form():
+    """Eq. 6: -sum_v (vm|vm) by explicit loops over the fitting points, and the closed form
+    -p_m^T (V o (Phi_v Phi_v^T)) p_m (Hadamard product with the occupied density matrix)."""
+    p = _tiny(seed=5, n_v=3, n_c=4, n_mu=7)
+    for m in (0, 2, 3, 6):
+        pm = p.phi_v[:, m] if m < 3 else p.phi_c[:, m - 3]
+        brute = 0.0
+        for v in range(3):
+            for a in range(7):
+                for b in range(7):
+                    brute -= p.phi_v[a, v] * pm[a] * p.V[a, b] * p.phi_v[b, v] * pm[b]
+        had = -pm @ ((p.V * (p.phi_v @ p.phi_v.T)) @ pm)
+        got = orc.exchange_eq6(p.phi_v, p.phi_c, p.V, m)
+        assert abs(got - brute) <= 1e-13 * abs(brute) and abs(got - had) <= 1e-13 * abs(had)
+        assert got < 0                                  # V positive definite: every (vm|vm) > 0
+
+
+def test_sigma_state_full_length_equals_eq7_summed_over_n():
+    """Eq. 10 with one chain per n: at L = N_vc with reorthogonalisation the sum equals Eq. 7 (double sum
+    over n and s) evaluated on the exact eigenpairs of C."""
+    p = _tiny(seed=11, n_v=2, n_c=3, n_mu=9)
+    delta = orc.delta_vc(p.eps_v, p.eps_c)
+    C = orc.casida_dense(delta, orc.coupling_dense(orc.khatri_rao(p.phi_v, p.phi_c), p.V))
+    lam, Z = sla.eigh(C)
+    omega = np.linspace(-20, 20, 41)
+    for m in (1, 2):
+        exact = np.zeros(len(omega), dtype=np.complex128)
+        for n in range(5):
+            P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, n, m)
+            e_n, sg = orc.orbital_energy_sign(p.eps_v, p.eps_c, n)
+            exact += orc.sigma_exact_eq7(lam, Z, P, omega, e_n, sg, DLT)
+        got = orc.sigma_state(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, m, 6, omega, DLT, reorth=True)
+        assert np.abs(got - exact).max() <= 1e-11
+
+
+def test_qp_solve_linear_selfenergy_closed_form():
+    """Sigma(w) = a + b w (exactly representable by the linear interpolant): E = (eps + Sx + a - vxc)/(1 - b),
+    Z = 1/(1 - b); Newton on a linear function lands on the root in one step."""
+    omega = np.linspace(-20, 20, 201)
+    a, b, eps, sx, vxc = -0.7, -0.25, -6.3, -4.1, -5.2
+    e, z, it = orc.qp_solve(eps, vxc, sx, (a + b * omega) + 0.3j, omega)
+    assert abs(e - (eps + sx + a - vxc) / (1 - b)) <= 1e-12
+    assert abs(z - 1 / (1 - b)) <= 1e-12 and it <= 3
+
+
+def test_qp_solve_is_a_root_of_the_interpolated_equation():
+    import scipy.optimize as so
+    omega = np.linspace(-20, 20, 401)
+    re = 0.8 * np.tanh(0.3 * (omega + 5.0)) - 0.1 * omega
+    eps, sx, vxc = -6.0, -3.0, -3.5
+    F = lambda w: eps + sx + np.interp(w, omega, re) - vxc - w      # noqa: E731
+    root = so.brentq(F, -20, 20, xtol=1e-14)
+    e, z, it = orc.qp_solve(eps, vxc, sx, re.astype(np.complex128), omega)
+    assert abs(e - root) <= 1e-9 and 0 < z < 1.5 and it < orc.QP_MAX_ITER
+    # a root outside the grid is clamped to the grid edge
+    e2, _, _ = orc.qp_solve(100.0, 0.0, 0.0, np.zeros(401, dtype=np.complex128), omega)
+    assert e2 == omega[-1]
