@@ -112,6 +112,31 @@ gwl_status gwl_resolvent(gwl_ctx* ctx, const double* zeta, int64_t n_zeta, doubl
 gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, double eta,
                           double* sigma, double* sigma_sum);
 
+/* ---- the rest of one quasiparticle state ------------------------------------------------ */
+
+/* Sigma^corr_mm(omega) of ONE orbital m, summed over all n = 0 .. n_v+n_c-1 (Eq. 10; one Lanczos
+ * chain per n started from |P_nm>): equivalent to gwl_set_chains(all n, m) + gwl_lanczos(steps,
+ * block, reorth) + gwl_selfenergy(sum only), and it leaves the context in that state (gwl_resolvent etc. then
+ * refer to these n_v+n_c chains).  m_idx as in gwl_set_chains.  omega [n_omega], sigma_mm [n_omega][2]
+ * (pointer mode applies to both). */
+gwl_status gwl_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, int64_t block, int reorth,
+                                const double* omega, int64_t n_omega, double eta, double* sigma_mm);
+
+/* Exchange part Sigma^ex_mm = - sum_v (vm|vm) over the occupied orbitals, PAPER.md:57 (Eq. 6), with
+ * (vm|vm) = rho_vm^T V rho_vm, rho_vm(mu) = phi_v(r_mu) phi_m(r_mu) (Eq. 16).  m_idx [n_states] host, indices
+ * as in gwl_set_chains; sigma_x [n_states] (pointer mode applies).  Needs orbitals and kernel. */
+gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, double* sigma_x);
+
+/* Quasiparticle equation: E(omega) = eps_m + <m|Sigma(omega) - V_xc|m> on the frequency grid,
+ * solved for E(omega) = omega by Newton-Raphson on the piecewise-linear interpolant of Re Sigma^corr, started
+ * at eps_m, clamped to the grid, until |step| <= 1e-10 eV or 50 iterations (reading Q18).
+ * eps_m, vxc_m [n_states] host.  sigma_x [n_states], sigma_c [n_states][n_omega][2], omega [n_omega]
+ * (ascending, n_omega >= 2), and the outputs e_qp [n_states], z_qp [n_states] (renormalisation factor
+ * 1/(1 - dReSigma/domega) at the solution), iters [n_states] (may be NULL) follow the pointer mode. */
+gwl_status gwl_qp_solve(gwl_ctx* ctx, int64_t n_states, const double* eps_m, const double* vxc_m,
+                        const double* sigma_x, const double* sigma_c, const double* omega, int64_t n_omega,
+                        double* e_qp, double* z_qp, int32_t* iters);
+
 /* CUDA-event totals (ms) of the last gwl_lanczos: time inside Casida products (S2), inside the Lanczos
  * vector kernels (S4) and overall.  Any pointer may be NULL.  Synchronises the stream. */
 gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total);

@@ -78,6 +78,7 @@ struct gwl_ctx {
 
     // workspaces
     DevBuf xs, T, W, part, dotpart, normpart, basis, coefpart, tA, tB, tC, u;
+    DevBuf x_nidx, x_midx, x_part, x_sig, x_eps, x_vxc, x_sc, x_e, x_z, x_it;  // gwl_exchange / gwl_qp_solve staging
     DevBuf sk_ws, sk_flags;  // stream-K hand-over of the K^T.W GEMM (kr_gemm.cu)
     unsigned sk_epoch = 0;
     DevBuf theta, wgt, ritz_info, d_omega, d_zeta, d_sigma, d_sigsum, io_x, io_y;
@@ -369,7 +370,8 @@ void gwl_destroy(gwl_ctx* ctx) {
                       &ctx->beta, &ctx->norm2, &ctx->len, &ctx->scale, &ctx->alive, &ctx->xs, &ctx->T, &ctx->W,
                       &ctx->part, &ctx->dotpart, &ctx->normpart, &ctx->basis, &ctx->coefpart, &ctx->tA, &ctx->tB,
                       &ctx->tC, &ctx->u, &ctx->theta, &ctx->wgt, &ctx->ritz_info, &ctx->d_omega, &ctx->d_zeta,
-                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y, &ctx->sk_ws, &ctx->sk_flags};
+                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y, &ctx->sk_ws, &ctx->sk_flags, &ctx->x_nidx, &ctx->x_midx, &ctx->x_part, &ctx->x_sig,
+                      &ctx->x_eps, &ctx->x_vxc, &ctx->x_sc, &ctx->x_e, &ctx->x_z, &ctx->x_it};
     for (DevBuf* b : bufs) b->release();
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->kev) cudaEventDestroy(e);
@@ -809,6 +811,142 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
             CK(cudaMemcpyAsync(sigma, dsig, (size_t)nch * n_omega * 16, cudaMemcpyDeviceToHost, st));
         if (sigma_sum != nullptr)
             CK(cudaMemcpyAsync(sigma_sum, dsum, (size_t)n_omega * 16, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    return GWL_OK;
+}
+
+gwl_status gwl_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, int64_t block, int reorth,
+                                const double* omega, int64_t n_omega, double eta, double* sigma_mm) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (sigma_mm == nullptr || omega == nullptr || n_omega < 1)
+        return ctx->fail(GWL_EINVAL, "gwl_selfenergy_state: bad arguments");
+    const int n_orb = ctx->n_v + ctx->n_c;
+    std::vector<int32_t> n_idx(n_orb), m_rep(n_orb, m_idx);
+    for (int i = 0; i < n_orb; ++i) n_idx[i] = i;
+    gwl_status rs = gwl_set_chains(ctx, n_orb, n_idx.data(), m_rep.data());
+    if (rs != GWL_OK) return rs;
+    rs = gwl_lanczos(ctx, n_orb, steps, block, reorth, nullptr, nullptr, nullptr, nullptr);
+    if (rs != GWL_OK) return rs;
+    return gwl_selfenergy(ctx, omega, n_omega, eta, nullptr, sigma_mm);
+}
+
+gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, double* sigma_x) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (n_states < 0 || (n_states > 0 && (m_idx == nullptr || sigma_x == nullptr)))
+        return ctx->fail(GWL_EINVAL, "gwl_exchange: bad arguments");
+    if (!ctx->have_orb || !ctx->have_V) return ctx->fail(GWL_ESTATE, "gwl_exchange: orbitals and kernel must be set");
+    if (n_states == 0) return GWL_OK;
+    const int n_orb = ctx->n_v + ctx->n_c;
+    for (int64_t j = 0; j < n_states; ++j)
+        if (m_idx[j] < 0 || m_idx[j] >= n_orb) return ctx->fail(GWL_EINVAL, "gwl_exchange: orbital index out of range");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int chunk = std::min(ctx->n_v, 256);
+    gwl_status rs = ensure_workspace(ctx, chunk);
+    if (rs != GWL_OK) return rs;
+    const int64_t ldm = ctx->n_mup;
+    const int kt_v = ctx->n_mup / BK;
+    const int npart = vec_parts(ctx->n_mu);
+    // (v, m) index pairs of every rho_vm, state-major
+    std::vector<int32_t> hv((size_t)n_states * ctx->n_v), hm((size_t)n_states * ctx->n_v);
+    for (int64_t j = 0; j < n_states; ++j)
+        for (int v = 0; v < ctx->n_v; ++v) {
+            hv[(size_t)j * ctx->n_v + v] = v;
+            hm[(size_t)j * ctx->n_v + v] = m_idx[j];
+        }
+    CK(ctx->x_nidx.ensure(hv.size() * 4, st));
+    CK(ctx->x_midx.ensure(hm.size() * 4, st));
+    CK(ctx->x_part.ensure((size_t)chunk * npart * 8, st));
+    CK(cudaMemcpyAsync(ctx->x_nidx.p, hv.data(), hv.size() * 4, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctx->x_midx.p, hm.data(), hm.size() * 4, cudaMemcpyHostToDevice, st));
+    double* dout = sigma_x;
+    if (!ctx->device_ptrs) {
+        CK(ctx->x_sig.ensure((size_t)n_states * 8, st));
+        dout = ctx->x_sig.as<double>();
+    }
+    for (int64_t j = 0; j < n_states; ++j) {
+        for (int v0 = 0; v0 < ctx->n_v; v0 += chunk) {
+            const int nb = std::min(chunk, ctx->n_v - v0);
+            const int64_t off = j * ctx->n_v + v0;
+            // rho_vm -> T;  W = V T;  sum_v rho_vm . (V rho_vm)
+            CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
+                          ctx->x_nidx.as<int32_t>() + off, ctx->x_midx.as<int32_t>() + off, ctx->T.as<double>(), ldm, nb,
+                          st));
+            GemmPlan pl = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
+            GemmParams p{};
+            p.A = ctx->V.as<double>();
+            p.lda = ldm;
+            p.B = ctx->T.as<double>();
+            p.ldb = ldm;
+            p.M = ctx->n_mu;
+            p.N = nb;
+            p.kt_total = kt_v;
+            p.a_wrap = kt_v;
+            p.kt_per_split = pl.kt_per_split;
+            if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
+            p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
+            p.ldo = ldm;
+            p.out_split_stride = (int64_t)nb * ldm;
+            CKL(1, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
+            if (pl.splits > 1)
+                CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
+                                        ctx->n_mu, nb, st));
+            CKL(4, launch_dot_partials(ctx->T.as<double>(), ctx->W.as<double>(), ldm, ctx->n_mu, nb,
+                                   ctx->x_part.as<double>(), npart, st));
+            CKL(4, launch_accum_neg(ctx->x_part.as<double>(), nb * npart, dout + j, v0 == 0 ? 1 : 0, st));
+        }
+    }
+    if (!ctx->device_ptrs) {
+        CK(cudaMemcpyAsync(sigma_x, dout, (size_t)n_states * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    return GWL_OK;
+}
+
+gwl_status gwl_qp_solve(gwl_ctx* ctx, int64_t n_states, const double* eps_m, const double* vxc_m,
+                        const double* sigma_x, const double* sigma_c, const double* omega, int64_t n_omega,
+                        double* e_qp, double* z_qp, int32_t* iters) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (n_states < 0 || n_omega < 2 || n_omega > (1 << 28))
+        return ctx->fail(GWL_EINVAL, "gwl_qp_solve: need n_states >= 0 and n_omega >= 2");
+    if (n_states == 0) return GWL_OK;
+    if (eps_m == nullptr || vxc_m == nullptr || sigma_x == nullptr || sigma_c == nullptr || omega == nullptr ||
+        e_qp == nullptr || z_qp == nullptr)
+        return ctx->fail(GWL_EINVAL, "gwl_qp_solve: NULL argument");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    CK(ctx->x_eps.ensure((size_t)n_states * 8, st));
+    CK(ctx->x_vxc.ensure((size_t)n_states * 8, st));
+    CK(cudaMemcpyAsync(ctx->x_eps.p, eps_m, (size_t)n_states * 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctx->x_vxc.p, vxc_m, (size_t)n_states * 8, cudaMemcpyHostToDevice, st));
+    const double *dsx = sigma_x, *dsc = sigma_c, *dom = omega;
+    double *de = e_qp, *dz = z_qp;
+    int32_t* dit = iters;
+    if (!ctx->device_ptrs) {
+        const size_t nsc = (size_t)n_states * n_omega * 16;
+        CK(ctx->x_sig.ensure((size_t)n_states * 8, st));
+        CK(ctx->x_sc.ensure(nsc, st));
+        CK(ctx->d_omega.ensure((size_t)n_omega * 8, st));
+        CK(ctx->x_e.ensure((size_t)n_states * 8, st));
+        CK(ctx->x_z.ensure((size_t)n_states * 8, st));
+        CK(ctx->x_it.ensure((size_t)n_states * 4, st));
+        CK(cudaMemcpyAsync(ctx->x_sig.p, sigma_x, (size_t)n_states * 8, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->x_sc.p, sigma_c, nsc, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->d_omega.p, omega, (size_t)n_omega * 8, cudaMemcpyHostToDevice, st));
+        dsx = ctx->x_sig.as<double>();
+        dsc = ctx->x_sc.as<double>();
+        dom = ctx->d_omega.as<double>();
+        de = ctx->x_e.as<double>();
+        dz = ctx->x_z.as<double>();
+        dit = ctx->x_it.as<int32_t>();
+    }
+    CKL(7, launch_qp_solve((int)n_states, ctx->x_eps.as<double>(), ctx->x_vxc.as<double>(), dsx, dsc, dom, (int)n_omega,
+                           de, dz, dit, st));
+    if (!ctx->device_ptrs) {
+        CK(cudaMemcpyAsync(e_qp, de, (size_t)n_states * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(z_qp, dz, (size_t)n_states * 8, cudaMemcpyDeviceToHost, st));
+        if (iters != nullptr) CK(cudaMemcpyAsync(iters, dit, (size_t)n_states * 4, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
     }
     return GWL_OK;

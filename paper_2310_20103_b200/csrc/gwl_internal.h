@@ -145,6 +145,12 @@ cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const dou
                               int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
                               int n_omega, double eta, double* sigma, cudaStream_t st);
 cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, double* sigma_sum, cudaStream_t st);
+// out[0] = (first ? 0 : out[0]) - sum(part[0..count)) in a fixed order (Eq. 6 accumulation)
+cudaError_t launch_accum_neg(const double* part, int count, double* out, int first, cudaStream_t st);
+// Newton-Raphson solve of E(omega) = omega on the grid, one thread per state
+cudaError_t launch_qp_solve(int n_states, const double* eps_m, const double* vxc_m, const double* sigma_x,
+                            const double* sigma_c, const double* omega, int n_omega, double* e_qp, double* z_qp,
+                            int32_t* iters, cudaStream_t st);
 
 // probe.cu
 cudaError_t probe_fp64_peak(int kind, double* tflops);

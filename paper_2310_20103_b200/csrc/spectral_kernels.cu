@@ -208,6 +208,59 @@ __global__ void k_sigma_sum(const double* __restrict__ sigma, int n_chains, int 
     sigma_sum[i] = acc;
 }
 
+// Sigma^ex accumulation: one block, fixed-order tree.
+__global__ void k_accum_neg(const double* __restrict__ part, int count, double* __restrict__ out, int first) {
+    __shared__ double sh[256];
+    double t = 0.0;
+    for (int i = threadIdx.x; i < count; i += 256) t += part[i];
+    sh[threadIdx.x] = t;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[0] = (first ? 0.0 : out[0]) - sh[0];
+}
+
+// E(omega) = eps_m + Re[Sigma^ex + Sigma^corr(omega)] - V_xc = omega by Newton-Raphson on the piecewise-linear
+// interpolant of Re Sigma^corr (reading Q18): start at eps_m, clamp to the grid, stop at
+// |step| <= 1e-10 eV or after 50 iterations.
+__global__ void k_qp_solve(int n_states, const double* __restrict__ eps_m, const double* __restrict__ vxc_m,
+                           const double* __restrict__ sigma_x, const double* __restrict__ sigma_c,
+                           const double* __restrict__ omega, int n_omega, double* __restrict__ e_qp,
+                           double* __restrict__ z_qp, int32_t* __restrict__ iters) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_states) return;
+    const double* sc = sigma_c + (int64_t)j * n_omega * 2;
+    const double e0 = eps_m[j], vxc = vxc_m[j], sx = sigma_x[j];
+    const double wlo = omega[0], whi = omega[n_omega - 1];
+    double w = fmin(fmax(e0, wlo), whi);
+    double z = 1.0;
+    int it = 0;
+    for (it = 1; it <= 50; ++it) {
+        int lo = 0, hi = n_omega;  // first index with omega[idx] > w
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (omega[mid] <= w) lo = mid + 1; else hi = mid;
+        }
+        int i = lo - 1;
+        i = min(max(i, 0), n_omega - 2);
+        const double r0 = sc[2 * i], r1 = sc[2 * (i + 1)];
+        const double slope = (r1 - r0) / (omega[i + 1] - omega[i]);
+        const double s_w = r0 + slope * (w - omega[i]);
+        const double F = e0 + sx + s_w - vxc - w;
+        const double dF = slope - 1.0;
+        z = -1.0 / dF;
+        const double w_new = fmin(fmax(w + (-F / dF), wlo), whi);
+        const bool done = fabs(w_new - w) <= 1e-10;
+        w = w_new;
+        if (done) break;
+    }
+    e_qp[j] = w;
+    z_qp[j] = z;
+    if (iters != nullptr) iters[j] = it > 50 ? 50 : it;
+}
+
 }  // namespace
 
 cudaError_t launch_contfrac(const double* alpha, const double* beta, const double* norm2, const int32_t* len, int steps,
@@ -261,6 +314,22 @@ cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const dou
 cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, double* sigma_sum, cudaStream_t st) {
     if (n_omega <= 0) return cudaSuccess;
     k_sigma_sum<<<(unsigned)ceil_div(2 * n_omega, 128), 128, 0, st>>>(sigma, n_chains, n_omega, sigma_sum);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_accum_neg(const double* part, int count, double* out, int first, cudaStream_t st) {
+    k_accum_neg<<<1, 256, 0, st>>>(part, count, out, first);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_qp_solve(int n_states, const double* eps_m, const double* vxc_m, const double* sigma_x,
+                            const double* sigma_c, const double* omega, int n_omega, double* e_qp, double* z_qp,
+                            int32_t* iters, cudaStream_t st) {
+    if (n_states <= 0) return cudaSuccess;
+    k_qp_solve<<<(unsigned)ceil_div(n_states, 64), 64, 0, st>>>(n_states, eps_m, vxc_m, sigma_x, sigma_c, omega, n_omega,
+                                                               e_qp, z_qp, iters);
     count_launch();
     return cudaGetLastError();
 }

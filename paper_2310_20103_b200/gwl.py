@@ -36,6 +36,10 @@ SIGNATURES = {
     "gwl_lanczos": (c_int, [c_void_p, c_int64, c_int64, c_int64, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "gwl_resolvent": (c_int, [c_void_p, c_void_p, c_int64, c_void_p]),
     "gwl_selfenergy": (c_int, [c_void_p, c_void_p, c_int64, c_double, c_void_p, c_void_p]),
+    "gwl_selfenergy_state": (c_int, [c_void_p, c_int32, c_int64, c_int64, c_int, c_void_p, c_int64, c_double, c_void_p]),
+    "gwl_exchange": (c_int, [c_void_p, c_int64, c_void_p, c_void_p]),
+    "gwl_qp_solve": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int64, c_void_p,
+                             c_void_p, c_void_p]),
     "gwl_get_timing": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
     "gwl_set_profiling": (c_int, [c_void_p, c_int]),
     "gwl_get_kernel_times": (c_int, [c_void_p, POINTER(c_double), POINTER(c_int64)]),
@@ -248,6 +252,53 @@ class Context:
         ss = np.zeros(om.size, dtype=np.complex128) if want_sum else None
         self._ck(self._lib.gwl_selfenergy(self._h, _ptr(om), om.size, float(eta), _ptr(sg), _ptr(ss)))
         return sg, ss
+
+    def selfenergy_state(self, m_idx: int, steps: int, block: int, reorth: int, omega, eta: float, out=None):
+        """Sigma^corr_mm(omega) summed over all n (Eq. 10).  Host mode: returns complex numpy [n_omega].
+        Device mode: omega and out [n_omega, 2] are torch CUDA tensors; out is returned."""
+        if self.device_ptrs:
+            self._ck(self._lib.gwl_selfenergy_state(self._h, int(m_idx), steps, block, reorth, _ptr(omega),
+                                                    omega.numel(), float(eta), _ptr(out)))
+            return out
+        om = _host(omega)
+        ss = np.zeros(om.size, dtype=np.complex128)
+        self._ck(self._lib.gwl_selfenergy_state(self._h, int(m_idx), steps, block, reorth, _ptr(om), om.size,
+                                                float(eta), _ptr(ss)))
+        return ss
+
+    def exchange(self, m_idx, out=None):
+        """Sigma^ex_mm (Eq. 6) for the orbitals m_idx.  Host mode: numpy [n_states]; device mode: out torch tensor."""
+        m = _host(m_idx, np.int32)
+        if m.ndim != 1:
+            raise GwlError(GWL_EINVAL, "exchange: m_idx must be 1-d")
+        if self.device_ptrs:
+            self._ck(self._lib.gwl_exchange(self._h, m.size, _ptr(m), _ptr(out)))
+            return out
+        sx = np.zeros(m.size)
+        self._ck(self._lib.gwl_exchange(self._h, m.size, _ptr(m), _ptr(sx)))
+        return sx
+
+    def qp_solve(self, eps_m, vxc_m, sigma_x, sigma_c, omega, out=None):
+        """Newton-Raphson solution of E(omega) = omega (PAPER.md:317).  Host mode: sigma_c complex [n_states, n_omega];
+        returns (e_qp, z_qp, iters).  Device mode: sigma_x, sigma_c [n_states, n_omega, 2], omega and
+        out=(e_qp, z_qp, iters or None) are torch CUDA tensors."""
+        e, v = _host(eps_m), _host(vxc_m)
+        if e.ndim != 1 or e.shape != v.shape:
+            raise GwlError(GWL_EINVAL, "qp_solve: eps_m and vxc_m must be 1-d and of equal length")
+        n = e.size
+        if self.device_ptrs:
+            eq, zq, it = out
+            self._ck(self._lib.gwl_qp_solve(self._h, n, _ptr(e), _ptr(v), _ptr(sigma_x), _ptr(sigma_c), _ptr(omega),
+                                            omega.numel(), _ptr(eq), _ptr(zq), _ptr(it)))
+            return out
+        sx, om = _host(sigma_x), _host(omega)
+        sc = np.ascontiguousarray(sigma_c, dtype=np.complex128)
+        if sx.shape != (n,) or sc.shape != (n, om.size):
+            raise GwlError(GWL_EINVAL, "qp_solve: sigma_x must be [n_states], sigma_c [n_states, n_omega]")
+        eq, zq, it = np.zeros(n), np.zeros(n), np.zeros(n, dtype=np.int32)
+        self._ck(self._lib.gwl_qp_solve(self._h, n, _ptr(e), _ptr(v), _ptr(sx), _ptr(sc), _ptr(om), om.size, _ptr(eq),
+                                        _ptr(zq), _ptr(it)))
+        return eq, zq, it
 
     def get_timing(self):
         a, b, c = c_double(), c_double(), c_double()

@@ -1,8 +1,14 @@
-"""Host-side helpers for bench.py: replica aggregation over torch.distributed and clock sampling.
+"""Host-side helpers: replica aggregation over torch.distributed, clock sampling, and the chain-sharded
+evaluation of Sigma^corr_mm.
 
-The path does not shard inside one problem (BASELINE.json:north_star: one GPU, no collectives); with
-N > 1 GPUs bench.py runs N independent replicas ("replicas only").  The only communication is
-a barrier and a MAX/SUM reduction of the timing scalars, done here so that it can be tested with gloo."""
+bench.py: the timed path does not shard inside one problem (BASELINE.json:north_star: one GPU, no
+collectives); with N > 1 GPUs it runs N independent replicas ("replicas only"), and the only
+communication is a barrier and a MAX/SUM reduction of the timing scalars.
+
+Chain sharding (sharded_sigma_state): the N_v + N_c Lanczos chains of one state m are independent (one per n,
+PAPER.md:87, :155), so each rank takes a contiguous slice of n, runs them on its own GPU with its own replica
+of Phi and V, and ONE all-reduce (SUM) of n_omega complex numbers does the sum of Eq. 10.
+Nothing is exchanged inside the step loop.  Everything here works on gloo/CPU tensors too (tests)."""
 from __future__ import annotations
 
 import os
@@ -33,6 +39,45 @@ def whole_job_value(units_local: float, elapsed_s_local: float, device=None) -> 
     """Whole-job throughput = units all ranks processed / max-over-ranks time."""
     u, t = aggregate_throughput(units_local, elapsed_s_local, device)
     return u / t if t > 0 else 0.0
+
+
+def shard_range(n: int, rank: int, world: int):
+    """Contiguous, balanced slice [lo, hi) of n items for `rank` of `world` (first n % world ranks get one more)."""
+    base, rem = divmod(int(n), int(world))
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+def sharded_sigma_state(local_sigma_sum, n_orb: int):
+    """Sigma^corr_mm(omega) = sum over all n (Eq. 10) with the chains n partitioned over the ranks.
+    local_sigma_sum(lo, hi) -> float64 tensor [n_omega, 2] holding the sum over n in [lo, hi) (zeros if empty),
+    on the device of the process group's backend.  Returns the all-reduced tensor (same on every rank)."""
+    import torch.distributed as dist
+    on = dist.is_available() and dist.is_initialized()
+    rank = dist.get_rank() if on else 0
+    world = dist.get_world_size() if on else 1
+    lo, hi = shard_range(n_orb, rank, world)
+    part = local_sigma_sum(lo, hi)
+    if on and world > 1:
+        dist.all_reduce(part, op=dist.ReduceOp.SUM)
+    return part
+
+
+def gwl_local_sigma_sum(ctx, m_idx: int, steps: int, block: int, reorth: int, omega_d, eta: float):
+    """local_sigma_sum for sharded_sigma_state on a gwl.Context in device-pointer mode: chains (n, m) for n in
+    [lo, hi) through gwl_set_chains / gwl_lanczos / gwl_selfenergy (sum only), result left on the GPU."""
+    import numpy as np
+    import torch
+
+    def run(lo, hi):
+        out = torch.zeros(omega_d.numel(), 2, dtype=torch.float64, device=omega_d.device)
+        if hi > lo:
+            n = np.arange(lo, hi, dtype=np.int32)
+            ctx.set_chains(n, np.full_like(n, m_idx))
+            ctx.lanczos(hi - lo, steps, block, reorth, out=None)
+            ctx.selfenergy(omega_d, eta, out=(None, out))
+        return out
+    return run
 
 
 _REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",

@@ -366,3 +366,61 @@ def test_launches_and_timing_reported(p0):
         assert ctx.get_launch_count() - n0 >= 10 * 5
         tm, tv, tt = ctx.get_timing()
         assert tm > 0 and tv > 0 and abs(tt - tm - tv) < 1e-9
+
+
+# ---- one whole quasiparticle state ---------------------------------------------------
+def test_state_selfenergy_exchange_and_qp_solve_config0(p0):
+    """Sigma^corr_mm over all 32 chains (Eq. 10), Sigma^ex (Eq. 6) and the Newton-Raphson solve of
+    E(omega) = omega for the HOMO and the LUMO, reorthogonalisation on both sides."""
+    cfg = p0.cfg
+    L = 40
+    states = [cfg.n_v - 1, cfg.n_v]
+    vxc = np.array([-9.0, -7.5])
+    with _ctx(p0, chains=False) as ctx:
+        sx = ctx.exchange(states)
+        sc = np.array([ctx.selfenergy_state(m, L, 12, 1, p0.omega, DLT) for m in states])
+        eps_m = np.array([p0.eps_v[-1], p0.eps_c[0]])
+        eq, zq, it = ctx.qp_solve(eps_m, vxc, sx, sc, p0.omega)
+    for k, m in enumerate(states):
+        rx = orc.exchange_eq6(p0.phi_v, p0.phi_c, p0.V, m)
+        rc = orc.sigma_state(p0.phi_v, p0.phi_c, p0.eps_v, p0.eps_c, p0.V, m, L, p0.omega, DLT, reorth=True)
+        assert abs(sx[k] - rx) <= 1e-12 * abs(rx)
+        assert np.abs(sc[k] - rc).max() <= TOL_SIGMA
+        re, rz, rit = orc.qp_solve(eps_m[k], vxc[k], rx, rc, p0.omega)
+        assert abs(eq[k] - re) <= TOL_SIGMA and abs(zq[k] - rz) <= 1e-6 and it[k] == rit
+        # and on identical inputs (the oracle's Sigma) the solver agrees to rounding
+    with _ctx(p0, chains=False) as ctx:
+        rc = np.array([orc.sigma_state(p0.phi_v, p0.phi_c, p0.eps_v, p0.eps_c, p0.V, m, 10, p0.omega, DLT) for m in states])
+        rx = np.array([orc.exchange_eq6(p0.phi_v, p0.phi_c, p0.V, m) for m in states])
+        eq, zq, it = ctx.qp_solve(eps_m, vxc, rx, rc, p0.omega)
+    for k in range(2):
+        re, rz, rit = orc.qp_solve(eps_m[k], vxc[k], rx[k], rc[k], p0.omega)
+        assert abs(eq[k] - re) <= 1e-12 and abs(zq[k] - rz) <= 1e-12 and it[k] == rit
+
+
+def test_exchange_many_occupied_orbitals_two_chunks():
+    """N_v > 256: the sum over v runs in two GEMM chunks; N_mu not a multiple of the tile."""
+    p = synth.make_custom(300, 2, 70, seed=4)
+    m = [0, 299, 301]
+    with _ctx(p, chains=False) as ctx:
+        sx = ctx.exchange(m)
+    ref = np.array([orc.exchange_eq6(p.phi_v, p.phi_c, p.V, k) for k in m])
+    assert (np.abs(sx - ref) <= 1e-12 * np.abs(ref)).all()
+
+
+def test_qp_solve_device_pointer_mode_and_clamp(p0):
+    import torch
+    om = torch.linspace(-20, 20, 101, dtype=torch.float64, device="cuda")
+    sc = torch.zeros(2, 101, 2, dtype=torch.float64, device="cuda")
+    sc[0, :, 0] = -0.5 - 0.25 * om
+    sx = torch.tensor([-4.0, 0.0], dtype=torch.float64, device="cuda")
+    eq = torch.zeros(2, dtype=torch.float64, device="cuda")
+    zq = torch.zeros_like(eq)
+    it = torch.zeros(2, dtype=torch.int32, device="cuda")
+    with gwl.Context(2, 2, 8) as ctx:
+        ctx.set_pointer_mode(1)
+        ctx.set_stream(torch.cuda.current_stream().cuda_stream)
+        ctx.qp_solve([-6.0, 500.0], [-5.0, 0.0], sx, sc, om, out=(eq, zq, it))
+        torch.cuda.synchronize()
+    assert abs(eq[0].item() - (-6.0 - 4.0 - 0.5 + 5.0) / 1.25) <= 1e-12 and abs(zq[0].item() - 0.8) <= 1e-12
+    assert eq[1].item() == 20.0                                   # root outside the grid: clamped

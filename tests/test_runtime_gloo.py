@@ -54,3 +54,55 @@ def test_reference_arm_prints_contract_line():
     assert d["impl"] == "reference" and d["metric"] == "lanczos_chain_steps_per_s" and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
     assert d["config"]["workload"].startswith("BASELINE.json:configs[0]")
+
+
+SHARD_WORKER = textwrap.dedent("""
+    import os, sys
+    sys.path.insert(0, %r)
+    import numpy as np, torch
+    import torch.distributed as dist
+    from oracle import gw_oracle as orc
+    from paper_2310_20103_b200 import runtime, synth
+    dist.init_process_group("gloo")
+    rank = dist.get_rank()
+    p = synth.make_custom(3, 4, 12, seed=1)
+    omega = np.linspace(-20, 20, 21)
+    m, L = 2, 5
+    def local(lo, hi):       # stands in for the per-GPU run: the oracle on this rank's slice of n
+        out = torch.zeros(len(omega), 2, dtype=torch.float64)
+        if hi > lo:
+            n = np.arange(lo, hi, dtype=np.int32)
+            r = orc.run_chains(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, n, np.full_like(n, m), L, omega, 0.1)
+            out[:, 0] = torch.from_numpy(r["sigma_sum"].real.copy()); out[:, 1] = torch.from_numpy(r["sigma_sum"].imag.copy())
+        return out
+    tot = runtime.sharded_sigma_state(local, 7)
+    ref = orc.sigma_state(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, m, L, omega, 0.1)
+    err = max(np.abs(tot[:, 0].numpy() - ref.real).max(), np.abs(tot[:, 1].numpy() - ref.imag).max())
+    lo, hi = runtime.shard_range(7, rank, dist.get_world_size())
+    print("SHARD", rank, lo, hi, err)
+    dist.barrier()
+    dist.destroy_process_group()
+""" % ROOT)
+
+
+def test_chain_sharded_sigma_state_two_ranks(tmp_path):
+    """7 chains over 2 ranks (4 + 3), one all-reduce of the omega grid = Eq. 10."""
+    script = tmp_path / "shard_worker.py"
+    script.write_text(SHARD_WORKER)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+           "--master-addr", "127.0.0.1", "--master-port", "29513", str(script)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    rows = sorted(l.split() for l in r.stdout.splitlines() if l.startswith("SHARD"))
+    assert [(int(x[2]), int(x[3])) for x in rows] == [(0, 4), (4, 7)]
+    assert all(float(x[4]) <= 1e-12 for x in rows)
+
+
+def test_shard_range_covers_everything():
+    from paper_2310_20103_b200 import runtime
+    for n in (0, 1, 7, 32, 1280):
+        for w in (1, 2, 3, 8):
+            cuts = [runtime.shard_range(n, r, w) for r in range(w)]
+            assert cuts[0][0] == 0 and cuts[-1][1] == n
+            assert all(a[1] == b[0] for a, b in zip(cuts, cuts[1:]))
+            assert max(h - l for l, h in cuts) - min(h - l for l, h in cuts) <= 1
