@@ -408,3 +408,66 @@ def qp_solve(eps_m, vxc_m, sigma_x, sigma_c, omega):
         if done:
             break
     return w, z, it
+
+
+# --------------------------------------------------------------------------- #
+# SURVEY.md §8(f)-3, first step: Tamm-Dancoff approximation, real Gamma-only   #
+# --------------------------------------------------------------------------- #
+def tda_dense(delta, Ktilde):
+    """A = diag(Delta) + (vc|v'c'): "setting matrix B = 0 in the RPA Casida matrix ... only a Hermitian matrix A
+    remains" (PAPER.md:157; Eq. 2).  Real orbitals, one k-point: the Gamma-only restriction of A(q), PAPER.md:296."""
+    return np.diag(delta) + Ktilde
+
+
+def tda_matvec_factored(phi_v, phi_c, V, delta, X):
+    """y = A x = Delta o x + K^T (V (K x)) for a block X [nvec, N_vc], K never formed (same contraction order as
+    casida_matvec_factored)."""
+    n_v, n_c = phi_v.shape[1], phi_c.shape[1]
+    X = np.asarray(X, dtype=np.float64).reshape(-1, n_v * n_c)
+    X3 = X.reshape(-1, n_v, n_c)
+    T = np.einsum("mv,mc,bvc->mb", phi_v, phi_c, X3, optimize=True)
+    W = V @ T
+    U = np.einsum("mv,mc,mb->bvc", phi_v, phi_c, W, optimize=True).reshape(X.shape)
+    return delta[None, :] * X + U
+
+
+def tda_start_vector(phi_v, phi_c, V, n_idx, m_idx):
+    """P_vc = (nm|vc): the vector of PAPER.md:313 for one k-point (no (eps_c - eps_v)^{1/2} factor in the TDA)."""
+    rho = orbital_column(phi_v, phi_c, n_idx) * orbital_column(phi_v, phi_c, m_idx)
+    w = V @ rho
+    return np.einsum("mv,mc,m->vc", phi_v, phi_c, w, optimize=True).reshape(-1)
+
+
+def sigma_tda(alpha, beta, norm2, length, omega, eps_n, sgn_n, dlt):
+    """Sigma(omega, n) = <P| 1/(omega - eps_n + eta_n (A - i delta)) |P>  (one k-point, prefactor of
+    Eq. 7: reading Q19) = -eta_n R_A(-eta_n z_n), z_n = omega - eps_n - i eta_n delta, with the resolvent
+    R_A(zeta) = <P|(zeta - A)^{-1}|P> by the continued fraction of Eq. 14."""
+    z = z_n(omega, eps_n, sgn_n, dlt)
+    return -sgn_n * continued_fraction(alpha, beta, norm2, -sgn_n * z, length)
+
+
+def sigma_tda_exact(lam, X, P, omega, eps_n, sgn_n, dlt):
+    """Eq. 7 with B = 0: sum_s <P|X^s>^2 / (omega - eps_n + eta_n (Omega_s - i delta)), (Omega_s, X^s) = eig(A)."""
+    w2 = (X.T @ P) ** 2
+    den = np.asarray(omega)[:, None] - eps_n + sgn_n * (lam[None, :] - 1j * dlt)
+    return (w2[None, :] / den).sum(axis=1)
+
+
+def run_chains_tda(phi_v, phi_c, eps_v, eps_c, V, n_idx, m_idx, steps, omega, dlt, reorth=False):
+    """run_chains in the Tamm-Dancoff approximation: Lanczos on A started from (nm|vc), Sigma by sigma_tda."""
+    delta = delta_vc(eps_v, eps_c)
+
+    def op(x):
+        return tda_matvec_factored(phi_v, phi_c, V, delta, x[None])[0]
+
+    n = len(n_idx)
+    out = dict(alpha=np.zeros((n, steps)), beta=np.zeros((n, steps)), norm2=np.zeros(n),
+               len=np.zeros(n, dtype=np.int32), sigma=np.zeros((n, len(omega)), dtype=np.complex128))
+    for j in range(n):
+        P = tda_start_vector(phi_v, phi_c, V, int(n_idx[j]), int(m_idx[j]))
+        a, b, n2, ln = lanczos(op, P, steps, reorth=reorth)
+        eps_n, sgn = orbital_energy_sign(eps_v, eps_c, int(n_idx[j]))
+        out["alpha"][j], out["beta"][j], out["norm2"][j], out["len"][j] = a, b, n2, ln
+        out["sigma"][j] = sigma_tda(a, b, n2, ln, omega, eps_n, sgn, dlt)
+    out["sigma_sum"] = sigma_sum(out["sigma"])
+    return out

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -798,8 +799,18 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
             CK(ctx->theta.ensure((size_t)nch * L * 8, st));
             CK(ctx->wgt.ensure((size_t)nch * L * 8, st));
             CK(ctx->ritz_info.ensure((size_t)nch * 4, st));
-            CKL(7, launch_ritz(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
-                           ctx->theta.as<double>(), ctx->wgt.as<double>(), nullptr, ctx->ritz_info.as<int32_t>(), st));
+            // divide and conquer (parallel) when T_L fits one CTA's shared memory, else the sequential QL kernel;
+            // GWL_RITZ=ql forces the latter (A/B runs)
+            static const bool force_ql = [] {
+                const char* e = getenv("GWL_RITZ");
+                return e != nullptr && e[0] == 'q';
+            }();
+            if (ritz_dc_fits(L) && !force_ql)
+                CKL(7, launch_ritz_dc(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
+                                  ctx->theta.as<double>(), ctx->wgt.as<double>(), ctx->ritz_info.as<int32_t>(), st));
+            else
+                CKL(7, launch_ritz(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
+                               ctx->theta.as<double>(), ctx->wgt.as<double>(), nullptr, ctx->ritz_info.as<int32_t>(), st));
             CKL(7, launch_sigma_direct(ctx->theta.as<double>(), ctx->wgt.as<double>(), ctx->norm2.as<double>(),
                                    ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
                                    ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));

@@ -138,6 +138,10 @@ cudaError_t launch_contfrac(const double* alpha, const double* beta, const doubl
 // theta[chain][steps], wgt[chain][steps] (first `len` entries valid); work: 3*n_chains*steps doubles
 cudaError_t launch_ritz(const double* alpha, const double* beta, const int32_t* len, int steps, int n_chains,
                         double* theta, double* wgt, double* work, int32_t* info, cudaStream_t st);
+// Same outputs by divide and conquer, one CTA per chain (ritz_dc.cu); steps must satisfy ritz_dc_fits().
+bool ritz_dc_fits(int steps);
+cudaError_t launch_ritz_dc(const double* alpha, const double* beta, const int32_t* len, int steps, int n_chains,
+                           double* theta, double* wgt, int32_t* info, cudaStream_t st);
 cudaError_t launch_sigma_direct(const double* theta, const double* wgt, const double* norm2, const int32_t* len,
                                 int steps, int n_chains, const double* eps_n, const int32_t* sgn_n,
                                 const double* omega, int n_omega, double eta, double* sigma, cudaStream_t st);

@@ -410,3 +410,46 @@ def test_qp_solve_is_a_root_of_the_interpolated_equation():
     # a root outside the grid is clamped to the grid edge
     e2, _, _ = orc.qp_solve(100.0, 0.0, 0.0, np.zeros(401, dtype=np.complex128), omega)
     assert e2 == omega[-1]
+
+
+# ---- SURVEY.md §8(f)-3 (first step): Tamm-Dancoff, real Gamma-only ------------------------------------------
+def test_tda_operator_spectrum_and_selfenergy(cfg0, dense0):
+    """B = 0 in Eq. 1: the eigenvalues of the block matrix [[A, 0], [0, -A]] are +-eig(A); the
+    factored product equals the dense A x; Lanczos on A at full length with reorthogonalisation gives the exact
+    pole sum (Eq. 7 with B = 0)."""
+    p = cfg0
+    delta, Kt = dense0["delta"], dense0["Kt"]
+    A = orc.tda_dense(delta, Kt)
+    assert np.abs(A - A.T).max() <= 1e-14 * np.abs(A).max() and np.abs(np.diag(A) - delta - np.diag(Kt)).max() <= 1e-14 * np.abs(A).max()
+    lam, X = sla.eigh(A)
+    assert lam.min() >= delta.min()                               # Ktilde is positive semidefinite
+    x = np.random.default_rng(2).normal(size=(3, len(delta)))
+    y = orc.tda_matvec_factored(p.phi_v, p.phi_c, p.V, delta, x)
+    assert np.abs(y - x @ A).max() <= 1e-12 * np.abs(y).max()
+    n, m = 1, p.cfg.n_v + 2
+    P = orc.tda_start_vector(p.phi_v, p.phi_c, p.V, n, m)
+    K = dense0["K"]
+    rho = p.phi_v[:, n] * p.phi_c[:, 2]
+    assert np.abs(P - K.T @ (p.V @ rho)).max() <= 1e-13 * np.abs(P).max()
+    N = len(delta)
+    r = orc.run_chains_tda(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, [n, p.cfg.n_v], [m, m], N, p.omega, DLT, reorth=True)
+    for j, nn in enumerate([n, p.cfg.n_v]):
+        Pj = orc.tda_start_vector(p.phi_v, p.phi_c, p.V, nn, m)
+        e_n, sg = orc.orbital_energy_sign(p.eps_v, p.eps_c, nn)
+        exact = orc.sigma_tda_exact(lam, X, Pj, p.omega, e_n, sg, DLT)
+        assert np.abs(r["sigma"][j] - exact).max() <= 1e-10
+        assert (sg * r["sigma"][j].imag > 0).all()                # same Herglotz sign as the RPA case
+
+
+def test_tda_one_by_one_closed_form():
+    """N_v = N_c = 1: A = Delta + k, k = rho^T V rho; Sigma = P^2 / (omega - eps_n + eta (A - i delta))."""
+    p = synth.make_custom(1, 1, 6, seed=8)
+    delta = orc.delta_vc(p.eps_v, p.eps_c)
+    rho = p.phi_v[:, 0] * p.phi_c[:, 0]
+    k = rho @ p.V @ rho
+    om = np.linspace(-5, 5, 11)
+    r = orc.run_chains_tda(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, [0, 1], [1, 1], 1, om, DLT)
+    assert abs(r["alpha"][0, 0] - (delta[0] + k)) <= 1e-13 * (delta[0] + k)
+    for j, (e_n, sg, P2) in enumerate([(p.eps_v[0], 1, k * k), (p.eps_c[0], -1, ((p.phi_c[:, 0] ** 2) @ p.V @ rho) ** 2)]):
+        ref = P2 / (om - e_n + sg * (delta[0] + k - 1j * DLT))
+        assert np.abs(r["sigma"][j] - ref).max() <= 1e-12 * np.abs(ref).max()
