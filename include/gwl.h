@@ -73,6 +73,17 @@ gwl_status gwl_set_kernel(gwl_ctx* ctx, const double* V);
  * NULL) clears it: Op = C and gwl_selfenergy evaluates Eq. 11 on the Ritz pairs of T_L ("direct mode"). */
 gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo, double hi);
 
+/* SURVEY.md 8(f)-3, first step.  GWL_RPA (default): the operator is C of Eq. 4.  GWL_TDA: the Tamm-Dancoff
+ * approximation, "setting matrix B = 0 in the RPA Casida matrix ... only a Hermitian matrix A remains, and a standard
+ * Lanczos algorithm for Hermitian matrix can be used" (formulas PAPER.md:306-313), here for real
+ * orbitals and one k-point: the operator becomes A = diag(Delta) + K^T V K (Eq. 2), chains start from
+ * P_vc = (nm|vc) (no sqrt(Delta) factor), gwl_casida_matvec applies A, and gwl_selfenergy evaluates
+ * Sigma(omega, n) = <P| 1/(omega - eps_n + eta_n (A - i eta)) |P> = -eta_n R_A(-eta_n z_n) by Eq. 14.
+ * Switching invalidates the results of the last gwl_lanczos.  GWL_ESTATE if a polynomial is set (it fits sqrt(C)). */
+#define GWL_RPA 0
+#define GWL_TDA 1
+gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation);
+
 /* y = C x for nvec vectors, PAPER.md:52 with the factorisation of PAPER.md:128, :383-389:
  * y = Delta^2 o x + 2 sqrt(Delta) o K^T ( V ( K ( sqrt(Delta) o x ) ) ).  Always C, never p_g(C).
  * x, y [nvec][n_v][n_c]; x and y must not overlap.  nvec >= 0 (0 is a no-op). */

@@ -63,6 +63,7 @@ struct gwl_ctx {
     DevBuf phi_c, phi_cT, phi_vT, V, eps_v, eps_c, d2, s;
     std::vector<double> h_eps_v, h_eps_c;
 
+    int approx = 0;  // 0 RPA (operator C), 1 Tamm-Dancoff (operator A)
     int g = 0;
     std::vector<double> cheb;
     double lo = 0.0, hi = 0.0;
@@ -250,6 +251,7 @@ gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double*
         p.dotpart = dotpart;
         p.dot_stride = dot_stride;
         p.n_c = ctx->n_c;
+        p.coupling = ctx->approx ? 1.0 : 2.0;
         p.ws = ctx->sk_ws.as<double>();
         p.flags = ctx->sk_flags.as<unsigned>();
         if (++ctx->sk_epoch == 0) ++ctx->sk_epoch;
@@ -318,6 +320,7 @@ gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, doub
         p.dotpart = normpart;
         p.dot_stride = dot_stride;
         p.n_c = ctx->n_c;
+        p.coupling = ctx->approx ? 1.0 : 2.0;
         p.ws = ctx->sk_ws.as<double>();
         p.flags = ctx->sk_flags.as<unsigned>();
         if (++ctx->sk_epoch == 0) ++ctx->sk_epoch;
@@ -444,7 +447,7 @@ gwl_status gwl_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps
     CK(cudaMemcpyAsync(ctx->eps_v.p, eps_v, (size_t)ctx->n_v * 8, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ctx->eps_c.p, eps_c, (size_t)ctx->n_c * 8, cudaMemcpyHostToDevice, st));
     CKL(4, launch_build_delta(ctx->eps_v.as<double>(), ctx->eps_c.as<double>(), ctx->n_v, ctx->n_c, ctx->d2.as<double>(),
-                          ctx->s.as<double>(), st));
+                          ctx->s.as<double>(), ctx->approx, st));
     CK(cudaStreamSynchronize(st));
     ctx->have_eps = true;
     return GWL_OK;
@@ -473,10 +476,29 @@ gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo
     }
     if (cheb == nullptr || !(hi > lo) || !std::isfinite(lo) || !std::isfinite(hi))
         return ctx->fail(GWL_EINVAL, "gwl_set_polynomial: need cheb != NULL and hi > lo");
+    if (ctx->approx != GWL_RPA)
+        return ctx->fail(GWL_ESTATE, "gwl_set_polynomial: the polynomial square root applies to C (RPA) only");
     ctx->g = g;
     ctx->cheb.assign(cheb, cheb + g + 1);
     ctx->lo = lo;
     ctx->hi = hi;
+    return GWL_OK;
+}
+
+gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation) {
+    if (ctx == nullptr || (approximation != GWL_RPA && approximation != GWL_TDA)) return GWL_EINVAL;
+    if (approximation == GWL_TDA && ctx->g > 0)
+        return ctx->fail(GWL_ESTATE, "gwl_set_approximation: clear the polynomial first (it approximates sqrt(C), RPA only)");
+    ctx->approx = approximation;
+    ctx->run_chains = 0;
+    ctx->run_steps = 0;
+    if (ctx->have_eps) {  // rebuild the diagonal term and the scaling for the new operator
+        LaunchScope ls(ctx);
+        cudaStream_t st = ctx->stream;
+        CKL(4, launch_build_delta(ctx->eps_v.as<double>(), ctx->eps_c.as<double>(), ctx->n_v, ctx->n_c,
+                              ctx->d2.as<double>(), ctx->s.as<double>(), ctx->approx, st));
+        CK(cudaStreamSynchronize(st));
+    }
     return GWL_OK;
 }
 
@@ -724,7 +746,7 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
     }
     ctx->run_chains = n_chains;
     ctx->run_steps = L;
-    ctx->run_poly = poly ? 1 : 0;
+    ctx->run_poly = poly ? 1 : (ctx->approx == GWL_TDA ? 2 : 0);
     if (n_chains > 0) {
         const cudaMemcpyKind kind = ctx->device_ptrs ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
         if (alpha) CK(cudaMemcpyAsync(alpha, ctx->alpha.p, (size_t)n_chains * L * 8, kind, st));
@@ -791,7 +813,11 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
         dsum = ctx->d_sigsum.as<double>();
     }
     if (nch > 0) {
-        if (ctx->run_poly) {
+        if (ctx->run_poly == 2) {
+            CKL(7, launch_sigma_tda(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
+                                ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
+                                ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));
+        } else if (ctx->run_poly == 1) {
             CKL(7, launch_sigma_poly(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
                                  ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
                                  ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));

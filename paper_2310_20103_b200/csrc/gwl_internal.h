@@ -40,8 +40,9 @@ struct GemmParams {
     int64_t out_split_stride;
     const double* X;      // EPI_CASIDA: x[n*ldx + v*n_c + m]
     int64_t ldx;
-    const double* d2;     // Delta^2 [n_vc]
-    const double* s;      // sqrt(Delta) [n_vc]
+    const double* d2;     // diagonal term [n_vc]: Delta^2 (RPA, operator C) or Delta (TDA, operator A)
+    const double* s;      // scaling [n_vc]: sqrt(Delta) (RPA) or 1 (TDA)
+    double coupling;      // epilogue: y = d2 x + coupling * s * u; 2 (A+B, RPA) or 1 (A alone, TDA)
     double* dotpart;      // CASIDA: sum_m x*y, START: sum_m p*p ; dotpart[n*dot_stride + v*gridDim.x + blockIdx.x]
     int dot_stride;
     int n_c;
@@ -76,8 +77,9 @@ cudaError_t launch_gemm(int mode, int epi, const GemmPlan& plan, const GemmParam
 constexpr int VEC_THREADS = 256;
 int vec_parts(int64_t n_vc);  // number of partial-sum blocks per column used by the kernels below
 
+// tda = 0: d2 = Delta^2, s = sqrt(Delta);  tda = 1: d2 = Delta, s = 1
 cudaError_t launch_build_delta(const double* eps_v, const double* eps_c, int n_v, int n_c, double* d2, double* s,
-                               cudaStream_t st);
+                               int tda, cudaStream_t st);
 // xs[b][v][c_pad] = s[vc] * x[b][vc] * (colscale ? colscale[b] : 1)
 cudaError_t launch_prescale(const double* x, int64_t ldx, double* xs, int64_t ldxs, const double* s, int n_v, int n_c,
                             int n_cp, int nb, cudaStream_t st);
@@ -148,6 +150,10 @@ cudaError_t launch_sigma_direct(const double* theta, const double* wgt, const do
 cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const double* norm2, const int32_t* len,
                               int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
                               int n_omega, double eta, double* sigma, cudaStream_t st);
+// TDA: Sigma = -sgn R_A(-sgn z), R_A by Eq. 14
+cudaError_t launch_sigma_tda(const double* alpha, const double* beta, const double* norm2, const int32_t* len,
+                             int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
+                             int n_omega, double eta, double* sigma, cudaStream_t st);
 cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, double* sigma_sum, cudaStream_t st);
 // out[0] = (first ? 0 : out[0]) - sum(part[0..count)) in a fixed order (Eq. 6 accumulation)
 cudaError_t launch_accum_neg(const double* part, int count, double* out, int first, cudaStream_t st);

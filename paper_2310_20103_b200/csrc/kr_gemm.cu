@@ -383,6 +383,7 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             const bool vec_ok = ((voff & 1) == 0) && ((p.ldo & 1) == 0) && ((p.ldx & 1) == 0) &&
                                 ((reinterpret_cast<uintptr_t>(p.out) & 15) == 0) &&
                                 (EPI == EPI_START || (reinterpret_cast<uintptr_t>(p.X) & 15) == 0);
+            const double cpl = p.coupling;
             double part[FN][2];
 #pragma unroll
             for (int j = 0; j < FN; ++j) part[j][0] = part[j][1] = 0.0;
@@ -429,8 +430,8 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                         double y0, y1;
                         if (EPI == EPI_CASIDA) {
                             const double x0 = xr[j][e][0], x1 = xr[j][e][1];
-                            y0 = d0 * x0 + 2.0 * (s0 * u0v);
-                            y1 = d1 * x1 + 2.0 * (s1 * u1v);
+                            y0 = d0 * x0 + cpl * (s0 * u0v);
+                            y1 = d1 * x1 + cpl * (s1 * u1v);
                             part[j][e] += x0 * y0 + x1 * y1;
                         } else {
                             y0 = s0 * u0v;

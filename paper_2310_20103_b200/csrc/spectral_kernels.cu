@@ -199,6 +199,22 @@ __global__ void k_sigma_poly(const double* __restrict__ alpha, const double* __r
     sigma[((int64_t)j * n_omega + iw) * 2 + 1] = v.im;
 }
 
+// Tamm-Dancoff (B = 0): Sigma = <P| 1/(omega - eps_n + sgn (A - i eta)) |P> = -sgn R_A(-sgn z)  (Eq. 14).
+__global__ void k_sigma_tda(const double* __restrict__ alpha, const double* __restrict__ beta,
+                            const double* __restrict__ norm2, const int32_t* __restrict__ len, int steps,
+                            const double* __restrict__ eps_n, const int32_t* __restrict__ sgn_n,
+                            const double* __restrict__ omega, int n_omega, double eta, double* __restrict__ sigma) {
+    const int j = blockIdx.y;
+    const int iw = blockIdx.x * blockDim.x + threadIdx.x;
+    if (iw >= n_omega) return;
+    const double sg = (double)sgn_n[j];
+    const cplx z{omega[iw] - eps_n[j], -sg * eta};
+    const cplx r = contfrac_eval(alpha + (int64_t)j * steps, beta + (int64_t)j * steps, len[j], norm2[j],
+                                 cplx{-sg * z.re, -sg * z.im});
+    sigma[((int64_t)j * n_omega + iw) * 2] = -sg * r.re;
+    sigma[((int64_t)j * n_omega + iw) * 2 + 1] = -sg * r.im;
+}
+
 __global__ void k_sigma_sum(const double* __restrict__ sigma, int n_chains, int n_omega,
                             double* __restrict__ sigma_sum) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;  // over 2*n_omega reals
@@ -307,6 +323,16 @@ cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const dou
     if (n_chains <= 0 || n_omega <= 0) return cudaSuccess;
     dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)n_chains);
     k_sigma_poly<<<grid, 128, 0, st>>>(alpha, beta, norm2, len, steps, eps_n, sgn_n, omega, n_omega, eta, sigma);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sigma_tda(const double* alpha, const double* beta, const double* norm2, const int32_t* len,
+                             int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
+                             int n_omega, double eta, double* sigma, cudaStream_t st) {
+    if (n_chains <= 0 || n_omega <= 0) return cudaSuccess;
+    dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)n_chains);
+    k_sigma_tda<<<grid, 128, 0, st>>>(alpha, beta, norm2, len, steps, eps_n, sgn_n, omega, n_omega, eta, sigma);
     count_launch();
     return cudaGetLastError();
 }

@@ -57,13 +57,13 @@ __device__ __forceinline__ int64_t xs_index(int64_t vc, int n_c, int n_cp) {
 }
 
 __global__ void k_build_delta(const double* __restrict__ eps_v, const double* __restrict__ eps_c, int n_v, int n_c,
-                              double* __restrict__ d2, double* __restrict__ s) {
+                              double* __restrict__ d2, double* __restrict__ s, int tda) {
     const int64_t n = (int64_t)n_v * n_c;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         const int v = (int)(i / n_c), c = (int)(i - (int64_t)v * n_c);
         const double d = eps_c[c] - eps_v[v];
-        d2[i] = d * d;
-        s[i] = sqrt(d);
+        d2[i] = tda ? d : d * d;
+        s[i] = tda ? 1.0 : sqrt(d);
     }
 }
 
@@ -391,8 +391,8 @@ inline unsigned grid1d(int64_t n, int per_thread = 4) {
 int vec_parts(int64_t n_vc) { return (int)std::max<int64_t>(1, std::min<int64_t>(64, ceil_div(n_vc, 8192))); }
 
 cudaError_t launch_build_delta(const double* eps_v, const double* eps_c, int n_v, int n_c, double* d2, double* s,
-                               cudaStream_t st) {
-    k_build_delta<<<grid1d((int64_t)n_v * n_c, 1), NT, 0, st>>>(eps_v, eps_c, n_v, n_c, d2, s);
+                               int tda, cudaStream_t st) {
+    k_build_delta<<<grid1d((int64_t)n_v * n_c, 1), NT, 0, st>>>(eps_v, eps_c, n_v, n_c, d2, s, tda);
     count_launch();
     return cudaGetLastError();
 }

@@ -17,6 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgwl.so")
 
 GWL_OK, GWL_EINVAL, GWL_ESTATE, GWL_ENOMEM, GWL_ECUDA = range(5)
+GWL_RPA, GWL_TDA = 0, 1
 _STATUS = {0: "GWL_OK", 1: "GWL_EINVAL", 2: "GWL_ESTATE", 3: "GWL_ENOMEM", 4: "GWL_ECUDA"}
 
 # name -> (restype, argtypes); every symbol include/gwl.h declares
@@ -30,6 +31,7 @@ SIGNATURES = {
     "gwl_set_energies": (c_int, [c_void_p, c_void_p, c_void_p]),
     "gwl_set_kernel": (c_int, [c_void_p, c_void_p]),
     "gwl_set_polynomial": (c_int, [c_void_p, c_int, c_void_p, c_double, c_double]),
+    "gwl_set_approximation": (c_int, [c_void_p, c_int]),
     "gwl_casida_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
     "gwl_set_chains": (c_int, [c_void_p, c_int64, c_void_p, c_void_p]),
     "gwl_set_start_vectors": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p]),
@@ -174,6 +176,10 @@ class Context:
         if g > 0 and (c is None or c.shape != (g + 1,)):
             raise GwlError(GWL_EINVAL, "set_polynomial: cheb must have g+1 entries")
         self._ck(self._lib.gwl_set_polynomial(self._h, int(g), _ptr(c), float(lo), float(hi)))
+
+    def set_approximation(self, approximation: int):
+        """0 = RPA (operator C, default), 1 = Tamm-Dancoff (operator A)."""
+        self._ck(self._lib.gwl_set_approximation(self._h, int(approximation)))
 
     # -- the path ---------------------------------------------------------------------------------
     def casida_matvec(self, x, y=None):

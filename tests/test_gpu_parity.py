@@ -460,3 +460,37 @@ def test_ritz_quadrature_on_gpu_tridiagonals(p0, L):
         e_n, sg = orc.orbital_energy_sign(p0.eps_v, p0.eps_c, int(p0.n_idx[j]))
         ref = orc.sigma_direct(a[j], b[j], n2[j], int(ln[j]), p0.omega, e_n, sg, DLT)
         assert np.abs(sig[j] - ref).max() <= 1e-9
+
+
+# ---- SURVEY.md §8(f)-3, first step: Tamm-Dancoff approximation (operator A) ------------------------------
+def test_tda_mode_config0(p0):
+    cfg = p0.cfg
+    delta = orc.delta_vc(p0.eps_v, p0.eps_c)
+    X = synth.random_block(cfg, 5)
+    n_idx = np.array([0, 3, cfg.n_v, cfg.n_v + 5], dtype=np.int32)      # two occupied, two empty n
+    m_idx = np.full_like(n_idx, cfg.n_v - 1)
+    with _ctx(p0, chains=False) as ctx:
+        y_rpa = ctx.casida_matvec(X)
+        ctx.set_approximation(gwl.GWL_TDA)
+        y = ctx.casida_matvec(X)
+        ctx.set_chains(n_idx, m_idx)
+        a, b, n2, ln = ctx.lanczos(4, 50, 3, 1)
+        sig, ssum = ctx.selfenergy(p0.omega, DLT, 4)
+        r = ctx.resolvent(np.array([3.0 + 0.5j]), 4)
+        with pytest.raises(gwl.GwlError):
+            ctx.set_polynomial(2, np.ones(3), 1.0, 2.0)               # sqrt(C) fit has no meaning for A
+        ctx.set_approximation(gwl.GWL_RPA)
+        with pytest.raises(gwl.GwlError):
+            ctx.selfenergy(p0.omega, DLT, 4)                          # switching invalidates the last run
+        y_back = ctx.casida_matvec(X)
+    ref_y = orc.tda_matvec_factored(p0.phi_v, p0.phi_c, p0.V, delta, X.reshape(5, -1)).reshape(X.shape)
+    assert _relmax(y, ref_y) <= TOL_MATVEC
+    assert np.array_equal(y_back, y_rpa) and _relmax(y, y_rpa) > 1e-2
+    ref = orc.run_chains_tda(p0.phi_v, p0.phi_c, p0.eps_v, p0.eps_c, p0.V, n_idx, m_idx, 50, p0.omega, DLT, reorth=True)
+    assert (np.abs(n2 - ref["norm2"]) <= 1e-12 * ref["norm2"]).all()
+    _check_ab(a, b, ref["alpha"], ref["beta"], 50)
+    assert np.abs(sig - ref["sigma"]).max() <= TOL_SIGMA
+    assert np.abs(ssum - ref["sigma_sum"]).max() <= TOL_SIGMA
+    for j in range(4):
+        rr = orc.continued_fraction(a[j], b[j], n2[j], np.array([3.0 + 0.5j]), ln[j])
+        assert abs(r[j, 0] - rr[0]) <= 1e-11 * abs(rr[0])
