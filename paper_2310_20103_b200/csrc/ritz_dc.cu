@@ -27,6 +27,19 @@ namespace {
 constexpr int RT = 256;  // threads per CTA
 constexpr double DC_EPS = 2.220446049250313e-16;
 
+// 1/x to ~1 ulp: MUFU.RCP64H seed (about 2^-22) and two Newton steps.  The secular solver stops at
+// |w| <= 4 eps (1 + |psi| + |phi|) and every quotient below is one factor of a long product or sum, so correct
+// rounding (the ~30-instruction div.rn.f64 sequence, 60 % of this kernel's samples in the first profile) buys nothing.
+// x is finite and nonzero at every call site (distinct poles, offsets strictly inside a bracket).
+__device__ __forceinline__ double fast_rcp(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+
 struct DcShared {
     double *Ad, *Af, *Al;          // eigen-data of the current segments: value, first-row entry, last-row entry
     double *BD, *Bz, *BF, *BL;     // a merge's inputs in sorted order
@@ -159,7 +172,7 @@ __device__ void dc_secular_root(const double* __restrict__ CD, const double* __r
     if (r < K - 1) {
         const double mid = 0.5 * (CD[r + 1] - CD[r]);
         double g = 0.0;
-        for (int j = 0; j < K; ++j) g += Cz2[j] / ((CD[j] - CD[r]) - mid);
+        for (int j = 0; j < K; ++j) g += Cz2[j] * fast_rcp((CD[j] - CD[r]) - mid);
         g = 1.0 + rho * g;
         if (g >= 0.0) {
             o = r;
@@ -181,17 +194,43 @@ __device__ void dc_secular_root(const double* __restrict__ CD, const double* __r
     double t = 0.5 * (lo + hi);
     for (int it = 0; it < 80; ++it) {
         double psi = 0.0, dpsi = 0.0, phi = 0.0, dphi = 0.0;
-        for (int j = 0; j <= r; ++j) {
-            const double inv = 1.0 / ((CD[j] - dorg) - t);
-            const double q = Cz2[j] * inv;
-            psi += q;
-            dpsi += q * inv;
-        }
-        for (int j = r + 1; j < K; ++j) {
-            const double inv = 1.0 / ((CD[j] - dorg) - t);
-            const double q = Cz2[j] * inv;
-            phi += q;
-            dphi += q * inv;
+        {   // two independent accumulator sets per side: the sums are latency-bound (2 warps per scheduler)
+            double p1 = 0.0, d1 = 0.0;
+            int j = 0;
+            for (; j + 1 <= r; j += 2) {
+                const double i0 = fast_rcp((CD[j] - dorg) - t), i1 = fast_rcp((CD[j + 1] - dorg) - t);
+                const double q0 = Cz2[j] * i0, q1 = Cz2[j + 1] * i1;
+                psi += q0;
+                p1 += q1;
+                dpsi = fma(q0, i0, dpsi);
+                d1 = fma(q1, i1, d1);
+            }
+            if (j <= r) {
+                const double i0 = fast_rcp((CD[j] - dorg) - t);
+                const double q0 = Cz2[j] * i0;
+                psi += q0;
+                dpsi = fma(q0, i0, dpsi);
+            }
+            psi += p1;
+            dpsi += d1;
+            p1 = d1 = 0.0;
+            j = r + 1;
+            for (; j + 1 < K; j += 2) {
+                const double i0 = fast_rcp((CD[j] - dorg) - t), i1 = fast_rcp((CD[j + 1] - dorg) - t);
+                const double q0 = Cz2[j] * i0, q1 = Cz2[j + 1] * i1;
+                phi += q0;
+                p1 += q1;
+                dphi = fma(q0, i0, dphi);
+                d1 = fma(q1, i1, d1);
+            }
+            if (j < K) {
+                const double i0 = fast_rcp((CD[j] - dorg) - t);
+                const double q0 = Cz2[j] * i0;
+                phi += q0;
+                dphi = fma(q0, i0, dphi);
+            }
+            phi += p1;
+            dphi += d1;
         }
         psi *= rho;
         dpsi *= rho;
@@ -266,7 +305,7 @@ __device__ void dc_solve_and_update(const DcShared& s, int n, int t) {
         double prod = ((s.org[i] - dj) + s.tau[i]) / s.rho[lo];
         for (int k = 0; k < K; ++k) {
             if (k == j) continue;
-            prod *= ((s.org[lo + k] - dj) + s.tau[lo + k]) / (s.CD[lo + k] - dj);
+            prod *= ((s.org[lo + k] - dj) + s.tau[lo + k]) * fast_rcp(s.CD[lo + k] - dj);
         }
         s.zh[i] = copysign(sqrt(fabs(prod)), s.Cz[i]);
     }
@@ -285,7 +324,7 @@ __device__ void dc_solve_and_update(const DcShared& s, int n, int t) {
         const double o = s.org[i], tau = s.tau[i];
         double nrm = 0.0, sf = 0.0, sl = 0.0;
         for (int k = 0; k < K; ++k) {
-            const double v = s.zh[lo + k] / ((s.CD[lo + k] - o) - tau);
+            const double v = s.zh[lo + k] * fast_rcp((s.CD[lo + k] - o) - tau);
             nrm += v * v;
             sf += s.CF[lo + k] * v;
             sl += s.CL[lo + k] * v;

@@ -494,3 +494,21 @@ def test_tda_mode_config0(p0):
     for j in range(4):
         rr = orc.continued_fraction(a[j], b[j], n2[j], np.array([3.0 + 0.5j]), ln[j])
         assert abs(r[j, 0] - rr[0]) <= 1e-11 * abs(rr[0])
+
+
+def test_runs_are_bitwise_repeatable(p1):
+    """Every reduction has a fixed order (split-K, stream-K hand-over, cluster norm, dot partials): two runs of the
+    same problem give identical bits -- also a cheap detector of races in the flag/workspace hand-over."""
+    cfg = p1.cfg
+    outs = []
+    with _ctx(p1) as ctx:
+        for _ in range(3):
+            a, b, n2, ln = ctx.lanczos(cfg.n_chains, 25, cfg.block, 0)
+            sig, _ = ctx.selfenergy(p1.omega, DLT, cfg.n_chains)
+            outs.append((a, b, n2, sig))
+    X = synth.random_block(cfg, cfg.block)
+    with _ctx(p1, chains=False) as ctx:
+        ys = [ctx.casida_matvec(X) for _ in range(3)]
+    for o in outs[1:]:
+        assert all(np.array_equal(x, y) for x, y in zip(o, outs[0]))
+    assert np.array_equal(ys[0], ys[1]) and np.array_equal(ys[0], ys[2])
