@@ -88,6 +88,8 @@ __device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, dou
         : "d"(a), "d"(b));
 }
 
+constexpr int BWD_MIN_UNITS = 16;  // fewest k-tiles worth handing to one more CTA
+
 template <int BM, int BN, int MODE>
 struct TileCfg {
     static constexpr int A_BYTES = BM * 128;
@@ -127,21 +129,33 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
     const int g = lane >> 2, q = lane & 3;
     // ---- work list ------------------------------------------------------------------------------------
     // FWD / PLAIN: one segment per CTA, (m-tile, n-tile, split) = blockIdx.
-    // BWD ("stream-K"): a persistent 1-D grid; the tiles x k-tiles unit space is cut into gridDim.x equal
-    // contiguous ranges, so a range starts and ends in the middle of a tile.  The CTA whose range holds the LAST
-    // k-tile of a tile owns it (sums the partials of the others in a fixed order and runs the epilogue); the
-    // others store their accumulators to the workspace and raise a flag.  A range is processed head-of-last-tile
-    // first and tail-of-first-tile last: contributions are written at the very start, collected at the very
-    // end, and an owner only ever waits for CTAs of LOWER index (scheduled no later than itself).
+    // BWD: a persistent 1-D grid of G CTAs over the tiles, v fastest (tile = (m-tile, n-tile, v)), in two phases.
+    //  (1) R = floor(tiles / G) aligned rounds: CTA g takes tile i*G + g whole.  All CTAs walk the same k-range at the
+    //      same time and neighbouring CTAs differ only in v, so they read the SAME Phi_c^T and W k-tiles: each comes
+    //      from HBM once and is an L2 hit for the others.
+    //  (2) the remaining tiles ("stream-K"): their tiles x k-tiles unit space is cut into G equal contiguous ranges,
+    //      so a range starts and ends in the middle of a tile.  The CTA whose range holds the LAST k-tile of a tile
+    //      owns it (sums the partials of the others in a fixed order and runs the epilogue); the others store their
+    //      accumulators to the workspace and raise a flag.  A range is processed head-of-last-tile first and
+    //      tail-of-first-tile last: contributions are written at the start of the phase, collected at its end, and an
+    //      owner only ever waits for CTAs of LOWER index (dispatched no later than itself).
     const int KT = p.kt_total;
-    int ns = 1, first_tile = 0;
+    int ns = 1, nr = 0, ns_tail = 0, first_tile = 0, tile0 = 0, gt = 1;
     int64_t u0 = 0, u1 = 0, U = 0;
     if (MODE == MODE_BWD) {
-        U = (int64_t)p.n_tiles * KT;
-        u0 = U * blockIdx.x / gridDim.x;
-        u1 = U * (blockIdx.x + 1) / gridDim.x;
-        first_tile = (int)(u0 / KT);
-        ns = u1 > u0 ? (int)((u1 - 1) / KT) - first_tile + 1 : 0;
+        nr = p.n_tiles / (int)gridDim.x;
+        tile0 = nr * (int)gridDim.x;
+        U = (int64_t)(p.n_tiles - tile0) * KT;
+        // CTAs sharing phase 2: at least BWD_MIN_UNITS k-tiles each (every cut costs a partial tile through the
+        // workspace), never an empty range in front of a non-empty one (an owner waits for ALL lower CTAs of its tile)
+        gt = (int)min((int64_t)gridDim.x, max((int64_t)(p.n_tiles - tile0), U / BWD_MIN_UNITS));
+        if ((int)blockIdx.x < gt) {
+            u0 = U * blockIdx.x / gt;
+            u1 = U * (blockIdx.x + 1) / gt;
+            first_tile = tile0 + (int)(u0 / KT);
+            ns_tail = u1 > u0 ? tile0 + (int)((u1 - 1) / KT) - first_tile + 1 : 0;
+        }
+        ns = nr + ns_tail;
     }
     auto seg_at = [&](int i, int& tile, int& kb, int& ke) {
         if (MODE != MODE_BWD) {
@@ -150,9 +164,16 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             ke = min(kb + p.kt_per_split, KT);
             return;
         }
-        const int sidx = ns == 1 ? 0 : (i == 0 ? ns - 1 : (i == ns - 1 ? 0 : i));
+        if (i < nr) {
+            tile = i * (int)gridDim.x + (int)blockIdx.x;
+            kb = 0;
+            ke = KT;
+            return;
+        }
+        i -= nr;
+        const int sidx = ns_tail == 1 ? 0 : (i == 0 ? ns_tail - 1 : (i == ns_tail - 1 ? 0 : i));
         tile = first_tile + sidx;
-        const int64_t tb = (int64_t)tile * KT;
+        const int64_t tb = (int64_t)(tile - tile0) * KT;
         kb = (int)(max(u0, tb) - tb);
         ke = (int)(min(u1, tb + KT) - tb);
     };
@@ -162,10 +183,10 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             n0 = blockIdx.y * BN;
             z = blockIdx.z;
         } else {
-            const int mx = tile % p.tiles_m, r = tile / p.tiles_m;
-            m0 = mx * BM;
+            z = tile % p.scale_rows;  // v
+            const int r = tile / p.scale_rows;
             n0 = (r % p.tiles_n) * BN;
-            z = r / p.tiles_n;
+            m0 = (r / p.tiles_n) * BM;
         }
     };
     GWL_STAMP(0);
@@ -357,9 +378,9 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                 continue;
             }
             if (kb > 0) {
-                const int64_t tb = (int64_t)tile * KT;
+                const int64_t tb = (int64_t)(tile - tile0) * KT;
                 int gf = blockIdx.x;  // first contributor: the CTA whose range holds the tile's first k-tile
-                while (gf > 0 && U * gf / gridDim.x > tb) --gf;
+                while (gf > 0 && U * gf / gt > tb) --gf;
                 if (tid == 0) {
                     for (int c = gf; c < (int)blockIdx.x; ++c) {
                         unsigned f;
@@ -558,7 +579,6 @@ int gemm_variant() {
 
 // BWD grid: one CTA per SM, fewer only when the whole product has too few k-tiles to be worth cutting
 // (every cut costs one partial tile through the workspace).
-constexpr int BWD_MIN_UNITS = 16;
 int bwd_grid(int64_t tiles, int kt_total, int n_sm) {
     const int64_t by_units = tiles * kt_total / BWD_MIN_UNITS;
     return (int)std::max<int64_t>(1, std::min<int64_t>(n_sm, std::max<int64_t>(std::min<int64_t>(tiles, n_sm), by_units)));
