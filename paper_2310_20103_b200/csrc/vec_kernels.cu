@@ -155,7 +155,9 @@ __global__ void k_lanczos_init(double* __restrict__ p, int64_t n_vc, int nb, con
     const int b = blockIdx.y;
     const double n2 = block_sum_array(normpart + (int64_t)b * npart, npart, sh);
     const bool ok = n2 > 0.0;
-    const double nrm = sqrt(n2);
+    // one division per thread, then a multiply per element (the normalised vector differs from w / ||w|| by <= 1 ulp
+    // per element; a per-element div.rn.f64 costs ~30 FP64 instructions and made update2 ALU- rather than HBM-bound)
+    const double rnrm = ok ? 1.0 / sqrt(n2) : 0.0;
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         st.norm2[b] = n2;
         st.len[b] = ok ? st.steps : 0;
@@ -167,7 +169,7 @@ __global__ void k_lanczos_init(double* __restrict__ p, int64_t n_vc, int nb, con
     double* pb = p + (int64_t)b * n_vc;
     double* xsb = xs + (int64_t)b * ldxs;
     for (int64_t i = lo + threadIdx.x; i < hi; i += NT) {
-        const double qv = ok ? pb[i] / nrm : 0.0;
+        const double qv = ok ? pb[i] * rnrm : 0.0;
         pb[i] = qv;
         xsb[xs_index(i, n_c, n_cp)] = s[i] * qv;
     }
@@ -225,6 +227,7 @@ __global__ void k_lanczos_update2(double* __restrict__ w, int64_t n_vc, int nb, 
     const double sc_old = st.scale[par * nb + b];
     const double sc_new = fmax(sc_old, fabs(a) + beta);
     const bool broken = !alive || !(beta > 1e-12 * sc_new);
+    const double rbeta = broken ? 0.0 : 1.0 / beta;
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         st.beta[(int64_t)b * st.steps + k] = broken ? 0.0 : beta;
         st.scale[(par ^ 1) * nb + b] = sc_new;
@@ -236,7 +239,7 @@ __global__ void k_lanczos_update2(double* __restrict__ w, int64_t n_vc, int nb, 
     double* wb = w + (int64_t)b * n_vc;
     double* xsb = xs + (int64_t)b * ldxs;
     for (int64_t i = lo + threadIdx.x; i < hi; i += NT) {
-        const double qv = broken ? 0.0 : wb[i] / beta;
+        const double qv = broken ? 0.0 : wb[i] * rbeta;
         wb[i] = qv;
         xsb[xs_index(i, n_c, n_cp)] = s[i] * qv;
     }
@@ -299,6 +302,7 @@ __global__ void __launch_bounds__(NT) k_lanczos_fused(double* __restrict__ w, co
     const double sc_old = st.scale[par * nb + b];
     const double sc_new = fmax(sc_old, fabs(a) + beta);
     const bool broken = !alive || !(beta > 1e-12 * sc_new);
+    const double rbeta = broken ? 0.0 : 1.0 / beta;
     if (rank == 0 && threadIdx.x == 0) {
         st.alpha[(int64_t)b * st.steps + k] = a;
         st.beta[(int64_t)b * st.steps + k] = broken ? 0.0 : beta;
@@ -311,7 +315,7 @@ __global__ void __launch_bounds__(NT) k_lanczos_fused(double* __restrict__ w, co
     for (int j = 0; j < EPT; ++j) {
         const int64_t i = lo + threadIdx.x + (int64_t)j * NT;
         if (i < hi) {
-            const double qv = broken ? 0.0 : v[j] / beta;
+            const double qv = broken ? 0.0 : v[j] * rbeta;
             wb[i] = qv;
             xsb[xs_index(i, n_c, n_cp)] = s[i] * qv;
         }
