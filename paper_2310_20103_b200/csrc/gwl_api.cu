@@ -174,92 +174,110 @@ gwl_status ensure_workspace(gwl_ctx* ctx, int nb) {
     return GWL_OK;
 }
 
-// T[b][mu] <- K (xs);  W <- V T;  then the K^T product with the requested epilogue.
-// xs must already hold sqrt(Delta) o x in the padded [nb][n_v][n_cp] layout.
+// ---- the three contractions (kr_gemm.cu), each with its split-K reduction where the planner asks for one ---------
+// T[b][mu] = sum_vc K[mu, vc] xs[b][vc]   (xs = scaled input in the padded [nb][n_v][n_cp] layout)
+gwl_status gemm_kx(gwl_ctx* ctx, int nb) {
+    cudaStream_t st = ctx->stream;
+    const int kt_c = ctx->n_cp / BK, kt_f = ctx->n_v * kt_c;
+    const int64_t ldm = ctx->n_mup;
+    const GemmPlan pl = plan_gemm(MODE_FWD, ctx->n_mu, nb, kt_f, kt_c, ctx->n_sm);
+    GemmParams p{};
+    p.A = ctx->phi_c.as<double>();
+    p.lda = ctx->n_cp;
+    p.B = ctx->xs.as<double>();
+    p.ldb = (int64_t)ctx->n_v * ctx->n_cp;
+    p.M = ctx->n_mu;
+    p.N = nb;
+    p.kt_total = kt_f;
+    p.a_wrap = kt_c;
+    p.kt_per_split = pl.kt_per_split;
+    p.scale = ctx->phi_vT.as<double>();
+    p.lds = ldm;
+    p.scale_rows = ctx->n_v;
+    if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
+    p.out = pl.splits == 1 ? ctx->T.as<double>() : ctx->part.as<double>();
+    p.ldo = ldm;
+    p.out_split_stride = (int64_t)nb * ldm;
+    CKL(0, launch_gemm(MODE_FWD, EPI_STORE, pl, p, pl.splits, st));
+    if (pl.splits > 1)
+        CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->T.as<double>(), ldm, ctx->n_mu,
+                                nb, st));
+    return GWL_OK;
+}
+
+// W[b][mu] = sum_nu V[mu][nu] T[b][nu]
+gwl_status gemm_v(gwl_ctx* ctx, int nb) {
+    cudaStream_t st = ctx->stream;
+    const int kt_v = ctx->n_mup / BK;
+    const int64_t ldm = ctx->n_mup;
+    const GemmPlan pl = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
+    GemmParams p{};
+    p.A = ctx->V.as<double>();
+    p.lda = ldm;
+    p.B = ctx->T.as<double>();
+    p.ldb = ldm;
+    p.M = ctx->n_mu;
+    p.N = nb;
+    p.kt_total = kt_v;
+    p.a_wrap = kt_v;
+    p.kt_per_split = pl.kt_per_split;
+    if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
+    p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
+    p.ldo = ldm;
+    p.out_split_stride = (int64_t)nb * ldm;
+    CKL(1, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
+    if (pl.splits > 1)
+        CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm, ctx->n_mu,
+                                nb, st));
+    return GWL_OK;
+}
+
+// u = K^T W with the epilogue fused:  x != NULL: y = d2 o x + coupling s o u and the partial dots sum(x y);
+// x == NULL (start vectors): y = s o u and the partial dots sum(y y).
+gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64_t ldy, int nb, double* dotpart,
+                    int dot_stride) {
+    const int kt_v = ctx->n_mup / BK;
+    const int64_t ldm = ctx->n_mup;
+    const GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, kt_v, kt_v, ctx->n_sm);
+    GemmParams p{};
+    p.A = ctx->phi_cT.as<double>();
+    p.lda = ldm;
+    p.B = ctx->W.as<double>();
+    p.ldb = ldm;
+    p.M = ctx->n_c;
+    p.N = nb;
+    p.kt_total = kt_v;
+    p.a_wrap = kt_v;
+    p.kt_per_split = kt_v;
+    p.scale = ctx->phi_vT.as<double>();
+    p.lds = ldm;
+    p.scale_rows = ctx->n_v;
+    p.out = y;
+    p.ldo = ldy;
+    p.X = x;
+    p.ldx = ldx;
+    p.d2 = ctx->d2.as<double>();
+    p.s = ctx->s.as<double>();
+    p.dotpart = dotpart;
+    p.dot_stride = dot_stride;
+    p.n_c = ctx->n_c;
+    p.coupling = ctx->approx ? 1.0 : 2.0;
+    p.ws = ctx->sk_ws.as<double>();
+    p.flags = ctx->sk_flags.as<unsigned>();
+    if (++ctx->sk_epoch == 0) ++ctx->sk_epoch;
+    p.epoch = ctx->sk_epoch;
+    p.n_sm = ctx->n_sm;
+    CKL(2, launch_gemm(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, pl, p, ctx->n_v, ctx->stream));
+    return GWL_OK;
+}
+
+// y = Op x for a block whose scaled copy xs is ready: K, V, K^T with the Casida / TDA epilogue.
 gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64_t ldy, int nb,
                              double* dotpart, int dot_stride) {
-    cudaStream_t st = ctx->stream;
-    const int kt_c = ctx->n_cp / BK, kt_f = ctx->n_v * kt_c, kt_v = ctx->n_mup / BK;
-    const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
-    const int64_t ldm = ctx->n_mup;
-    {
-        GemmPlan pl = plan_gemm(MODE_FWD, ctx->n_mu, nb, kt_f, kt_c, ctx->n_sm);
-        GemmParams p{};
-        p.A = ctx->phi_c.as<double>();
-        p.lda = ctx->n_cp;
-        p.B = ctx->xs.as<double>();
-        p.ldb = ldxs;
-        p.M = ctx->n_mu;
-        p.N = nb;
-        p.kt_total = kt_f;
-        p.a_wrap = kt_c;
-        p.kt_per_split = pl.kt_per_split;
-        p.scale = ctx->phi_vT.as<double>();
-        p.lds = ldm;
-        p.scale_rows = ctx->n_v;
-        if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
-        p.out = pl.splits == 1 ? ctx->T.as<double>() : ctx->part.as<double>();
-        p.ldo = ldm;
-        p.out_split_stride = (int64_t)nb * ldm;
-        CKL(0, launch_gemm(MODE_FWD, EPI_STORE, pl, p, pl.splits, st));
-        if (pl.splits > 1)
-            CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->T.as<double>(), ldm,
-                                    ctx->n_mu, nb, st));
-    }
-    {
-        GemmPlan pl = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
-        GemmParams p{};
-        p.A = ctx->V.as<double>();
-        p.lda = ldm;
-        p.B = ctx->T.as<double>();
-        p.ldb = ldm;
-        p.M = ctx->n_mu;
-        p.N = nb;
-        p.kt_total = kt_v;
-        p.a_wrap = kt_v;
-        p.kt_per_split = pl.kt_per_split;
-        if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
-        p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
-        p.ldo = ldm;
-        p.out_split_stride = (int64_t)nb * ldm;
-        CKL(1, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
-        if (pl.splits > 1)
-            CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
-                                    ctx->n_mu, nb, st));
-    }
-    {
-        GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, kt_v, kt_v, ctx->n_sm);
-        GemmParams p{};
-        p.A = ctx->phi_cT.as<double>();
-        p.lda = ldm;
-        p.B = ctx->W.as<double>();
-        p.ldb = ldm;
-        p.M = ctx->n_c;
-        p.N = nb;
-        p.kt_total = kt_v;
-        p.a_wrap = kt_v;
-        p.kt_per_split = kt_v;
-        p.scale = ctx->phi_vT.as<double>();
-        p.lds = ldm;
-        p.scale_rows = ctx->n_v;
-        p.out = y;
-        p.ldo = ldy;
-        p.X = x;
-        p.ldx = ldx;
-        p.d2 = ctx->d2.as<double>();
-        p.s = ctx->s.as<double>();
-        p.dotpart = dotpart;
-        p.dot_stride = dot_stride;
-        p.n_c = ctx->n_c;
-        p.coupling = ctx->approx ? 1.0 : 2.0;
-        p.ws = ctx->sk_ws.as<double>();
-        p.flags = ctx->sk_flags.as<unsigned>();
-        if (++ctx->sk_epoch == 0) ++ctx->sk_epoch;
-        p.epoch = ctx->sk_epoch;
-        p.n_sm = ctx->n_sm;
-        CKL(2, launch_gemm(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, pl, p, ctx->n_v, st));
-    }
-    return GWL_OK;
+    gwl_status rs = gemm_kx(ctx, nb);
+    if (rs == GWL_OK) rs = gemm_v(ctx, nb);
+    if (rs == GWL_OK) rs = gemm_ktw(ctx, x, ldx, y, ldy, nb, dotpart, dot_stride);
+    return rs;
 }
 
 // alpha / norm partials written by the K^T.W epilogue: one per (v, m-tile) of the plan used for a block of nb
@@ -270,65 +288,13 @@ int casida_ndot(const gwl_ctx* ctx, int nb) {
 
 // S1: P_j = sqrt(Delta) o K^T (V rho_j) for index chains j0..j0+nb; writes P and sum(P^2) partials.
 gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, double* normpart, int dot_stride) {
-    cudaStream_t st = ctx->stream;
     const int64_t ldm = ctx->n_mup;
-    const int kt_v = ctx->n_mup / BK;
     CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
-                  ctx->d_nidx.as<int32_t>() + j0, ctx->d_midx.as<int32_t>() + j0, ctx->T.as<double>(), ldm, nb, st));
-    {
-        GemmPlan pl = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
-        GemmParams p{};
-        p.A = ctx->V.as<double>();
-        p.lda = ldm;
-        p.B = ctx->T.as<double>();
-        p.ldb = ldm;
-        p.M = ctx->n_mu;
-        p.N = nb;
-        p.kt_total = kt_v;
-        p.a_wrap = kt_v;
-        p.kt_per_split = pl.kt_per_split;
-        if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
-        p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
-        p.ldo = ldm;
-        p.out_split_stride = (int64_t)nb * ldm;
-        CKL(1, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
-        if (pl.splits > 1)
-            CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
-                                    ctx->n_mu, nb, st));
-    }
-    {
-        GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, kt_v, kt_v, ctx->n_sm);
-        GemmParams p{};
-        p.A = ctx->phi_cT.as<double>();
-        p.lda = ldm;
-        p.B = ctx->W.as<double>();
-        p.ldb = ldm;
-        p.M = ctx->n_c;
-        p.N = nb;
-        p.kt_total = kt_v;
-        p.a_wrap = kt_v;
-        p.kt_per_split = kt_v;
-        p.scale = ctx->phi_vT.as<double>();
-        p.lds = ldm;
-        p.scale_rows = ctx->n_v;
-        p.out = P;
-        p.ldo = ctx->n_vc;
-        p.X = nullptr;
-        p.ldx = ctx->n_vc;
-        p.d2 = ctx->d2.as<double>();
-        p.s = ctx->s.as<double>();
-        p.dotpart = normpart;
-        p.dot_stride = dot_stride;
-        p.n_c = ctx->n_c;
-        p.coupling = ctx->approx ? 1.0 : 2.0;
-        p.ws = ctx->sk_ws.as<double>();
-        p.flags = ctx->sk_flags.as<unsigned>();
-        if (++ctx->sk_epoch == 0) ++ctx->sk_epoch;
-        p.epoch = ctx->sk_epoch;
-        p.n_sm = ctx->n_sm;
-        CKL(2, launch_gemm(MODE_BWD, EPI_START, pl, p, ctx->n_v, st));
-    }
-    return GWL_OK;
+                  ctx->d_nidx.as<int32_t>() + j0, ctx->d_midx.as<int32_t>() + j0, ctx->T.as<double>(), ldm, nb,
+                  ctx->stream));
+    gwl_status rs = gemm_v(ctx, nb);
+    if (rs == GWL_OK) rs = gemm_ktw(ctx, nullptr, ctx->n_vc, P, ctx->n_vc, nb, normpart, dot_stride);
+    return rs;
 }
 
 bool ready(const gwl_ctx* ctx) { return ctx->have_orb && ctx->have_eps && ctx->have_V; }
@@ -883,7 +849,6 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
     gwl_status rs = ensure_workspace(ctx, chunk);
     if (rs != GWL_OK) return rs;
     const int64_t ldm = ctx->n_mup;
-    const int kt_v = ctx->n_mup / BK;
     const int npart = vec_parts(ctx->n_mu);
     // (v, m) index pairs of every rho_vm, state-major
     std::vector<int32_t> hv((size_t)n_states * ctx->n_v), hm((size_t)n_states * ctx->n_v);
@@ -910,25 +875,8 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
             CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
                           ctx->x_nidx.as<int32_t>() + off, ctx->x_midx.as<int32_t>() + off, ctx->T.as<double>(), ldm, nb,
                           st));
-            GemmPlan pl = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
-            GemmParams p{};
-            p.A = ctx->V.as<double>();
-            p.lda = ldm;
-            p.B = ctx->T.as<double>();
-            p.ldb = ldm;
-            p.M = ctx->n_mu;
-            p.N = nb;
-            p.kt_total = kt_v;
-            p.a_wrap = kt_v;
-            p.kt_per_split = pl.kt_per_split;
-            if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
-            p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
-            p.ldo = ldm;
-            p.out_split_stride = (int64_t)nb * ldm;
-            CKL(1, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
-            if (pl.splits > 1)
-                CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm,
-                                        ctx->n_mu, nb, st));
+            rs = gemm_v(ctx, nb);
+            if (rs != GWL_OK) return rs;
             CKL(4, launch_dot_partials(ctx->T.as<double>(), ctx->W.as<double>(), ldm, ctx->n_mu, nb,
                                    ctx->x_part.as<double>(), npart, st));
             CKL(4, launch_accum_neg(ctx->x_part.as<double>(), nb * npart, dout + j, v0 == 0 ? 1 : 0, st));
