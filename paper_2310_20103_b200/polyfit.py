@@ -1,0 +1,31 @@
+"""Host helper for the optional polynomial mode: coefficients of p_g(x) ~ sqrt(x) for
+gwl_set_polynomial.  PAPER.md:85, :284, :317: least-squares fit at the Chebyshev nodes of the fitting range,
+range [0.8 min(eps_c - eps_v)^2, 1.25 max(eps_c - eps_v)^2] (readings Q12, Q13).
+
+The fit is done in the Chebyshev basis, where it has a closed form: first-kind Chebyshev polynomials are orthogonal on
+the M first-kind nodes t_k = cos(pi (k + 1/2) / M), sum_k T_i(t_k) T_j(t_k) = M/2 delta_ij (M for i = j = 0), so the
+least-squares coefficients are c_j = (2 / M) sum_k f(x_k) T_j(t_k), c_0 halved.  No oracle code is used or imported.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def default_range(eps_v, eps_c):
+    """[0.8 min Delta^2, 1.25 max Delta^2], Delta = eps_c - eps_v (PAPER.md:284 with reading Q12)."""
+    d_min = float(np.min(eps_c) - np.max(eps_v))
+    d_max = float(np.max(eps_c) - np.min(eps_v))
+    return 0.8 * d_min * d_min, 1.25 * d_max * d_max
+
+
+def sqrt_chebyshev(g: int, lo: float, hi: float, nodes_per_coefficient: int = 4) -> np.ndarray:
+    """c[0..g] with p_g(x) = sum_j c_j T_j((2x - hi - lo)/(hi - lo)) the least-squares fit of sqrt(x) at
+    M = nodes_per_coefficient (g + 1) Chebyshev nodes of [lo, hi]."""
+    if g < 1 or not (hi > lo > 0.0):
+        raise ValueError("need g >= 1 and hi > lo > 0")
+    M = nodes_per_coefficient * (g + 1)
+    theta = np.pi * (np.arange(M) + 0.5) / M
+    f = np.sqrt(0.5 * (hi + lo) + 0.5 * (hi - lo) * np.cos(theta))
+    c = np.array([(2.0 / M) * np.sum(f * np.cos(j * theta)) for j in range(g + 1)])
+    c[0] *= 0.5
+    return c

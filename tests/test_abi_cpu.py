@@ -85,3 +85,20 @@ def test_synth_configs_match_baseline():
     s = synth.make_problem(synth.Config("s", 2, 2, 500, 40.0, True, (-12, -4), (-2, 25), 1, 1, 1, 1, 3))
     assert np.linalg.norm(s.r, axis=1).max() <= 20.0                               # diameter 40 (Q16)
     assert abs(synth.CONFIGS[2].flop_per_vector() - 6.52e9) < 0.01e9
+
+
+def test_polyfit_helper_closed_form_equals_least_squares():
+    """paper_2310_20103_b200/polyfit.py (discrete-orthogonality closed form) against the oracle's lstsq fit and
+    against sqrt itself on the range."""
+    import numpy as np
+    from oracle import gw_oracle as orc
+    from paper_2310_20103_b200 import polyfit
+    lo, hi = polyfit.default_range(np.array([-10.0, -5.5]), np.array([-3.0, 20.0]))
+    assert abs(lo - 0.8 * 2.5 ** 2) < 1e-12 and abs(hi - 1.25 * 30.0 ** 2) < 1e-9
+    for g in (1, 7, 8, 16):
+        c = polyfit.sqrt_chebyshev(g, lo, hi)
+        ref = orc.fit_sqrt_chebyshev(g, lo, hi)
+        assert np.abs(c - ref).max() <= 1e-12 * np.abs(ref).max()
+    x = np.linspace(lo, hi, 200)
+    err = np.abs(orc.poly_eval_scalar(polyfit.sqrt_chebyshev(8, lo, hi), lo, hi, x) - np.sqrt(x)) / np.sqrt(x)
+    assert err.max() < 0.2 and err[50:].max() < 0.01
