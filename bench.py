@@ -44,6 +44,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--lanczos-steps", type=int, default=0, help="override L (for profiling runs only; marks the line)")
+    ap.add_argument("--reorth", action="store_true",
+                    help="two-pass full reorthogonalisation on (not the bench workload; marks the line)")
     ap.add_argument("--paper-setting", default="", metavar="NV,NC,NMU",
                     help="context run, not the bench line: one whole quasiparticle state (all N_v+N_c chains, Sigma^x, "
                          "E(omega)=omega) with the paper's parameters N_iter = 8, g = 7 (PAPER.md:145) on a synthetic "
@@ -251,7 +253,7 @@ def main():
     sum_d = torch.empty(cfg.n_omega, 2, dtype=torch.float64, device=dev)
 
     def step_device():
-        ctx.lanczos(cfg.n_chains, L, cfg.block, 0, out=None)
+        ctx.lanczos(cfg.n_chains, L, cfg.block, 1 if args.reorth else 0, out=None)
         ctx.selfenergy(omega_d, cfg.eta, out=(sig_d, sum_d))
 
     dmma_peak = gwl.probe_fp64_peak(0)            # also warms the clocks
@@ -384,6 +386,13 @@ def main():
                 "kernel_time_share": share}
         if args.lanczos_steps:
             line["note"] = "lanczos_steps overridden: profiling run, not a bench value"
+        if args.reorth:
+            line["note"] = "full reorthogonalisation on: not the bench workload"
+            line["config"]["mode"] = "direct (Op = C), reorth on (CGS2)"
+            rt = ktimes["reorth"]
+            # CGS2 at step k reads the k+1 basis vectors twice per pass (dots, apply), two passes
+            nbytes = prof_steps * 4.0 * 8.0 * cfg.n_vc * cfg.n_chains * (L * (L + 1) / 2.0)
+            line["reorth"] = {"ms_per_pass_of_L_steps": rt[0] / prof_steps, "algorithmic_GBps": nbytes / (rt[0] * 1e-3) / 1e9}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(prob)
         print(json.dumps(line), flush=True)

@@ -168,7 +168,7 @@ gwl_status ensure_workspace(gwl_ctx* ctx, int nb) {
     const int npart = vec_parts(ctx->n_vc);
     const int64_t ndot = std::max<int64_t>((int64_t)ctx->n_v * ceil_div(ctx->n_c, 128), npart);
     CK(ctx->dotpart.ensure((size_t)nb * ndot * 8, st));
-    CK(ctx->normpart.ensure((size_t)nb * npart * 8, st));
+    CK(ctx->normpart.ensure((size_t)nb * std::max(npart, reorth_parts(ctx->n_vc)) * 8, st));
     CK(ctx->sk_ws.ensure(gemm_bwd_ws_bytes(ctx->n_sm), st));
     CK(ctx->sk_flags.ensure(gemm_bwd_flag_bytes(ctx->n_sm), st));
     return GWL_OK;
@@ -580,6 +580,7 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
     const int64_t n_vc = ctx->n_vc;
     const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
     const int npart = vec_parts(n_vc);
+    const int rparts = reorth_parts(n_vc);
     const bool poly = ctx->g > 0;
 
     ctx->run_chains = 0;
@@ -599,7 +600,7 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
         CK(ctx->alive.ensure((size_t)2 * nbmax * 4, st));
         const int nslots = reorth ? L + 1 : 3;
         CK(ctx->basis.ensure((size_t)nslots * nbmax * n_vc * 8, st));
-        if (reorth) CK(ctx->coefpart.ensure((size_t)nbmax * L * npart * 8, st));
+        if (reorth) CK(ctx->coefpart.ensure((size_t)nbmax * L * rparts * 8, st));
         if (poly) {
             CK(ctx->tA.ensure((size_t)nbmax * n_vc * 8, st));
             CK(ctx->tB.ensure((size_t)nbmax * n_vc * 8, st));
@@ -699,13 +700,13 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
             CKL(5, launch_lanczos_update1(w, q, qp, n_vc, nb, dotpart, ndot, dstride, S, k, normpart, npart, st));
             if (reorth) {
                 for (int pass = 0; pass < 2; ++pass) {
-                    CKL(6, launch_reorth_dots(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), npart,
+                    CKL(6, launch_reorth_dots(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), rparts,
                                           st));
-                    CKL(6, launch_reorth_apply(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), npart,
+                    CKL(6, launch_reorth_apply(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), rparts,
                                            pass == 1 ? normpart : nullptr, st));
                 }
             }
-            CKL(5, launch_lanczos_update2(w, n_vc, nb, normpart, npart, S, k, ctx->xs.as<double>(), ldxs,
+            CKL(5, launch_lanczos_update2(w, n_vc, nb, normpart, reorth ? rparts : npart, S, k, ctx->xs.as<double>(), ldxs,
                                       ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
             if (tstep) CK(cudaEventRecord(e2, st));
         }

@@ -122,6 +122,7 @@ bool lanczos_fused_fits(int64_t n_vc);
 cudaError_t launch_lanczos_fused(double* w, const double* q, const double* q_prev, int64_t n_vc, int nb,
                                  const double* dotpart, int ndot, int dot_stride, LanczosState st_, int k, double* xs,
                                  int64_t ldxs, const double* s, int n_v, int n_c, int n_cp, cudaStream_t st);
+int reorth_parts(int64_t n_vc);  // partial sums per chain of the two kernels below (their `npart`)
 // Full reorthogonalisation pass (classical Gram-Schmidt against basis vectors 0..k of each chain).
 // basis: [k+1 slots][nb][n_vc] with slot stride `slot_stride`; coef partials [nb][k+1][npart].
 cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nslots, const double* w, int64_t n_vc,

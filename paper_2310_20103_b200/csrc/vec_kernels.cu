@@ -323,28 +323,63 @@ __global__ void __launch_bounds__(NT) k_lanczos_fused(double* __restrict__ w, co
     asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory");
 }
 
+// ---- full reorthogonalisation (classical Gram-Schmidt, run twice): c = Q^T w, w -= Q c ---------------------------
+// HBM-bound: every pass streams the k+1 basis vectors of each chain twice (dots, apply).  Slices of RSLICE
+// elements per block (reorth_parts(n_vc) of them) so that a few blocks per SM keep enough loads in flight.
+// dots: the slice of w is staged in shared memory once; each WARP then takes basis vectors i = warp, warp + 8, ...
+// and reduces its dot by shuffles -- no block-wide barrier inside the loop over basis vectors.
 // coefpart[(b*nslots + i)*npart + blk] = sum over the slice of basis_i[b] * w[b]
-__global__ void k_reorth_dots(const double* __restrict__ basis, int64_t slot_stride, int nslots,
-                              const double* __restrict__ w, int64_t n_vc, double* __restrict__ coefpart, int npart) {
+constexpr int RSLICE = 2048;
+
+__global__ void __launch_bounds__(NT) k_reorth_dots(const double* __restrict__ basis, int64_t slot_stride, int nslots,
+                                                    const double* __restrict__ w, int64_t n_vc,
+                                                    double* __restrict__ coefpart, int npart, int64_t slice) {
     pdl_trigger();
     pdl_wait();
-    __shared__ double sh[NT / 32 + 1];
+    extern __shared__ double ws[];  // [slice]
     const int b = blockIdx.y;
-    int64_t lo, hi;
-    slice_of(n_vc, npart, blockIdx.x, lo, hi);
-    const double* wb = w + (int64_t)b * n_vc;
-    for (int i = 0; i < nslots; ++i) {
-        const double* qb = basis + (int64_t)i * slot_stride + (int64_t)b * n_vc;
-        double acc = 0.0;
-        for (int64_t j = lo + threadIdx.x; j < hi; j += NT) acc += qb[j] * wb[j];
-        acc = block_sum(acc, sh);
-        if (threadIdx.x == 0) coefpart[((int64_t)b * nslots + i) * npart + blockIdx.x] = acc;
+    const int64_t lo = (int64_t)blockIdx.x * slice;
+    const int len = (int)max((int64_t)0, min(slice, n_vc - lo));
+    const double* wb = w + (int64_t)b * n_vc + lo;
+    for (int j = threadIdx.x; j < len; j += NT) ws[j] = wb[j];
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool vec2 = ((n_vc | slot_stride | slice) & 1) == 0;  // 16-byte alignment of every (slot, chain, slice) start
+    for (int i = warp; i < nslots; i += NT / 32) {
+        const double* qb = basis + (int64_t)i * slot_stride + (int64_t)b * n_vc + lo;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        if (vec2) {
+            const double2* q2 = reinterpret_cast<const double2*>(qb);
+            const double2* w2 = reinterpret_cast<const double2*>(ws);
+            const int n2 = len >> 1;
+            int j = lane;
+            for (; j + 96 < n2; j += 128) {
+                const double2 x0 = __ldg(q2 + j), x1 = __ldg(q2 + j + 32), x2 = __ldg(q2 + j + 64), x3 = __ldg(q2 + j + 96);
+                const double2 y0 = w2[j], y1 = w2[j + 32], y2 = w2[j + 64], y3 = w2[j + 96];
+                a0 = fma(x0.x, y0.x, fma(x0.y, y0.y, a0));
+                a1 = fma(x1.x, y1.x, fma(x1.y, y1.y, a1));
+                a2 = fma(x2.x, y2.x, fma(x2.y, y2.y, a2));
+                a3 = fma(x3.x, y3.x, fma(x3.y, y3.y, a3));
+            }
+            for (; j < n2; j += 32) {
+                const double2 x0 = __ldg(q2 + j);
+                const double2 y0 = w2[j];
+                a0 = fma(x0.x, y0.x, fma(x0.y, y0.y, a0));
+            }
+            if ((len & 1) && lane == 0) a1 = fma(qb[len - 1], ws[len - 1], a1);
+        } else {
+            for (int j = lane; j < len; j += 32) a0 = fma(__ldg(qb + j), ws[j], a0);
+        }
+        const double acc = warp_sum((a0 + a1) + (a2 + a3));
+        if (lane == 0) coefpart[((int64_t)b * nslots + i) * npart + blockIdx.x] = acc;
     }
 }
 
-__global__ void k_reorth_apply(const double* __restrict__ basis, int64_t slot_stride, int nslots,
-                               double* __restrict__ w, int64_t n_vc, const double* __restrict__ coefpart, int npart,
-                               double* __restrict__ normpart) {
+// w -= sum_i c_i basis_i, c_i = fixed-order sum of the partials; optionally the partial norms of the new w.
+__global__ void __launch_bounds__(NT) k_reorth_apply(const double* __restrict__ basis, int64_t slot_stride, int nslots,
+                                                     double* __restrict__ w, int64_t n_vc,
+                                                     const double* __restrict__ coefpart, int npart,
+                                                     double* __restrict__ normpart, int64_t slice) {
     pdl_trigger();
     pdl_wait();
     extern __shared__ double coef[];  // [nslots] + block_sum scratch
@@ -357,15 +392,53 @@ __global__ void k_reorth_apply(const double* __restrict__ basis, int64_t slot_st
         coef[i] = t;
     }
     __syncthreads();
-    int64_t lo, hi;
-    slice_of(n_vc, npart, blockIdx.x, lo, hi);
-    double* wb = w + (int64_t)b * n_vc;
+    const int64_t lo = (int64_t)blockIdx.x * slice;
+    const int len = (int)max((int64_t)0, min(slice, n_vc - lo));
+    double* wb = w + (int64_t)b * n_vc + lo;
+    const double* q0 = basis + (int64_t)b * n_vc + lo;
+    const bool vec2 = ((n_vc | slot_stride | slice) & 1) == 0;
     double acc = 0.0;
-    for (int64_t j = lo + threadIdx.x; j < hi; j += NT) {
-        double v = wb[j];
-        for (int i = 0; i < nslots; ++i) v -= coef[i] * basis[(int64_t)i * slot_stride + (int64_t)b * n_vc + j];
-        wb[j] = v;
-        acc += v * v;
+    if (vec2) {
+        const int n2 = len >> 1;
+        for (int j = threadIdx.x; j < n2; j += NT) {
+            double2 v = reinterpret_cast<double2*>(wb)[j];
+            int i = 0;
+            for (; i + 3 < nslots; i += 4) {  // four independent 16-byte loads in flight per thread
+                const double2 x0 = __ldg(reinterpret_cast<const double2*>(q0 + (int64_t)i * slot_stride) + j);
+                const double2 x1 = __ldg(reinterpret_cast<const double2*>(q0 + (int64_t)(i + 1) * slot_stride) + j);
+                const double2 x2 = __ldg(reinterpret_cast<const double2*>(q0 + (int64_t)(i + 2) * slot_stride) + j);
+                const double2 x3 = __ldg(reinterpret_cast<const double2*>(q0 + (int64_t)(i + 3) * slot_stride) + j);
+                const double c0 = coef[i], c1 = coef[i + 1], c2 = coef[i + 2], c3 = coef[i + 3];
+                v.x -= c0 * x0.x;
+                v.y -= c0 * x0.y;
+                v.x -= c1 * x1.x;
+                v.y -= c1 * x1.y;
+                v.x -= c2 * x2.x;
+                v.y -= c2 * x2.y;
+                v.x -= c3 * x3.x;
+                v.y -= c3 * x3.y;
+            }
+            for (; i < nslots; ++i) {
+                const double2 x0 = __ldg(reinterpret_cast<const double2*>(q0 + (int64_t)i * slot_stride) + j);
+                v.x -= coef[i] * x0.x;
+                v.y -= coef[i] * x0.y;
+            }
+            reinterpret_cast<double2*>(wb)[j] = v;
+            acc += v.x * v.x + v.y * v.y;
+        }
+        if ((len & 1) && threadIdx.x == 0) {
+            double v = wb[len - 1];
+            for (int i = 0; i < nslots; ++i) v -= coef[i] * q0[(int64_t)i * slot_stride + len - 1];
+            wb[len - 1] = v;
+            acc += v * v;
+        }
+    } else {
+        for (int j = threadIdx.x; j < len; j += NT) {
+            double v = wb[j];
+            for (int i = 0; i < nslots; ++i) v -= coef[i] * __ldg(q0 + (int64_t)i * slot_stride + j);
+            wb[j] = v;
+            acc += v * v;
+        }
     }
     if (normpart != nullptr) {
         acc = block_sum(acc, sh);
@@ -500,19 +573,39 @@ cudaError_t launch_lanczos_fused(double* w, const double* q, const double* q_pre
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+// Slices of the reorthogonalisation kernels: RSLICE elements, at most 64 per chain (even length: 16-byte loads).
+int reorth_parts(int64_t n_vc) { return (int)std::max<int64_t>(1, std::min<int64_t>(64, ceil_div(n_vc, RSLICE))); }
+static int64_t reorth_slice(int64_t n_vc) { return round_up(ceil_div(n_vc, reorth_parts(n_vc)), 2); }
+
 cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nslots, const double* w, int64_t n_vc,
                                int nb, double* coefpart, int npart, cudaStream_t st) {
-    dim3 grid((unsigned)npart, (unsigned)nb);
-    cudaError_t le = launch_pdl(k_reorth_dots, dim3(grid), dim3(NT), (size_t)(0), st, 1u, basis, slot_stride, nslots, w, n_vc, coefpart, npart);
+    if (npart != reorth_parts(n_vc)) return cudaErrorInvalidValue;
+    const int64_t slice = reorth_slice(n_vc);
+    const size_t sm = (size_t)slice * sizeof(double);
+    static size_t configured = 0;
+    if (sm > 48 * 1024 && sm > configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_reorth_dots, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e != cudaSuccess) return e;
+        configured = sm;
+    }
+    cudaError_t le = launch_pdl(k_reorth_dots, dim3((unsigned)npart, (unsigned)nb), dim3(NT), sm, st, 1u, basis,
+                                slot_stride, nslots, w, n_vc, coefpart, npart, slice);
     count_launch();
     return le != cudaSuccess ? le : cudaGetLastError();
 }
 
 cudaError_t launch_reorth_apply(const double* basis, int64_t slot_stride, int nslots, double* w, int64_t n_vc, int nb,
                                 const double* coefpart, int npart, double* normpart, cudaStream_t st) {
-    dim3 grid((unsigned)npart, (unsigned)nb);
+    if (npart != reorth_parts(n_vc)) return cudaErrorInvalidValue;
     const size_t sm = (size_t)(nslots + NT / 32 + 1) * sizeof(double);
-    cudaError_t le = launch_pdl(k_reorth_apply, dim3(grid), dim3(NT), (size_t)(sm), st, 1u, basis, slot_stride, nslots, w, n_vc, coefpart, npart, normpart);
+    static size_t configured = 0;
+    if (sm > 48 * 1024 && sm > configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_reorth_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e != cudaSuccess) return e;
+        configured = sm;
+    }
+    cudaError_t le = launch_pdl(k_reorth_apply, dim3((unsigned)npart, (unsigned)nb), dim3(NT), sm, st, 1u, basis,
+                                slot_stride, nslots, w, n_vc, coefpart, npart, normpart, reorth_slice(n_vc));
     count_launch();
     return le != cudaSuccess ? le : cudaGetLastError();
 }
