@@ -81,6 +81,7 @@ struct gwl_ctx {
     // workspaces
     DevBuf xs, T, W, part, dotpart, normpart, basis, coefpart, tA, tB, tC, u;
     DevBuf x_nidx, x_midx, x_part, x_sig, x_eps, x_vxc, x_sc, x_e, x_z, x_it;  // gwl_exchange / gwl_qp_solve staging
+    DevBuf stage;            // gwl_set_orbitals staging
     DevBuf sk_ws, sk_flags;  // stream-K hand-over of the K^T.W GEMM (kr_gemm.cu)
     unsigned sk_epoch = 0;
     DevBuf theta, wgt, ritz_info, d_omega, d_zeta, d_sigma, d_sigsum, io_x, io_y;
@@ -340,7 +341,7 @@ void gwl_destroy(gwl_ctx* ctx) {
                       &ctx->beta, &ctx->norm2, &ctx->len, &ctx->scale, &ctx->alive, &ctx->xs, &ctx->T, &ctx->W,
                       &ctx->part, &ctx->dotpart, &ctx->normpart, &ctx->basis, &ctx->coefpart, &ctx->tA, &ctx->tB,
                       &ctx->tC, &ctx->u, &ctx->theta, &ctx->wgt, &ctx->ritz_info, &ctx->d_omega, &ctx->d_zeta,
-                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y, &ctx->sk_ws, &ctx->sk_flags, &ctx->x_nidx, &ctx->x_midx, &ctx->x_part, &ctx->x_sig,
+                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y, &ctx->sk_ws, &ctx->sk_flags, &ctx->stage, &ctx->x_nidx, &ctx->x_midx, &ctx->x_part, &ctx->x_sig,
                       &ctx->x_eps, &ctx->x_vxc, &ctx->x_sc, &ctx->x_e, &ctx->x_z, &ctx->x_it};
     for (DevBuf* b : bufs) b->release();
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
@@ -369,7 +370,7 @@ gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi
     LaunchScope ls(ctx);
     cudaStream_t st = ctx->stream;
     const size_t nv = (size_t)ctx->n_mu * ctx->n_v, nc = (size_t)ctx->n_mu * ctx->n_c;
-    DevBuf tmp;
+    DevBuf& tmp = ctx->stage;  // kept across calls: no cudaMalloc/cudaFree in a repeated set_orbitals
     CK(tmp.ensure(std::max(nv, nc) * 8, st));
     CK(ctx->phi_c.ensure((size_t)ctx->n_mu * ctx->n_cp * 8, st));
     CK(ctx->phi_cT.ensure((size_t)ctx->n_c * ctx->n_mup * 8, st));
@@ -384,7 +385,6 @@ gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi
     CK(cudaMemcpyAsync(tmp.p, phi_v, nv * 8, cudaMemcpyHostToDevice, st));
     CKL(4, launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_v, ctx->phi_vT.as<double>(), ctx->n_mup, st));
     CK(cudaStreamSynchronize(st));
-    tmp.release();
     ctx->have_orb = true;
     return GWL_OK;
 }

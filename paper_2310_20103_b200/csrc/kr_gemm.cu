@@ -253,17 +253,14 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
     // fragments of k-step s+1 are fetched from shared memory and scaled -- across k-tile boundaries too, where
     // the wait on the next "full" barrier is issued one k-step early so that its latency is hidden as well.
     double fa[2][FM], fb[2][FN];  // fragment double buffer, indexed by ks & 1 (all indices are compile-time)
-    double fv[FM];                // FWD: phi_v row scales of the k-tile being fetched
+    constexpr bool FV_REGS = (MODE == MODE_FWD) && FN <= 4;
+    double fv[FV_REGS ? FM : 1];  // FWD, narrow tiles: phi_v row scales of the k-tile being fetched
 
     auto fetch = [&](int slot, int ks, double(&a)[FM], double(&b)[FN]) {
         const unsigned char* base = smem_gen + slot * TC::KT_BYTES;
         const double* As = reinterpret_cast<const double*>(base);
         const double* Bs = reinterpret_cast<const double*>(base + TC::A_BYTES);
         const double* Sc = reinterpret_cast<const double*>(base + TC::A_BYTES + TC::B_BYTES);
-        if (MODE == MODE_FWD && ks == 0) {
-#pragma unroll
-            for (int i = 0; i < FM; ++i) fv[i] = Sc[rowA[i]];
-        }
         const int ch = 2 * ks + (q >> 1);
         const int c0 = ((ch ^ xr0) << 1) | (q & 1);
         const int c1 = ((ch ^ xr1) << 1) | (q & 1);
@@ -272,8 +269,20 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
 #pragma unroll
         for (int j = 0; j < FN; ++j) b[j] = Bs[rowB[j] * 16 + ((j & 1) ? c1 : c0)];
         if (MODE == MODE_FWD) {
+            // wide warp tiles (FN = 8, 232 registers): the row scales are re-read from shared memory at every k-step
+            // instead of living in FM registers for the whole k-tile (measured at config 2: K.X 24.0 -> 23.8 ms);
+            // narrow ones (FN = 4) have the registers and fewer DMMAs per k-step to hide the extra LDS behind.
+            if (FV_REGS) {
+                if (ks == 0) {
 #pragma unroll
-            for (int i = 0; i < FM; ++i) a[i] *= fv[i];
+                    for (int i = 0; i < FM; ++i) fv[i] = Sc[rowA[i]];
+                }
+#pragma unroll
+                for (int i = 0; i < FM; ++i) a[i] *= fv[i];
+            } else {
+#pragma unroll
+                for (int i = 0; i < FM; ++i) a[i] *= Sc[rowA[i]];
+            }
         } else if (MODE == MODE_BWD) {
             const double sk = Sc[4 * ks + q];
             if (FM <= FN) {

@@ -512,3 +512,28 @@ def test_runs_are_bitwise_repeatable(p1):
     for o in outs[1:]:
         assert all(np.array_equal(x, y) for x, y in zip(o, outs[0]))
     assert np.array_equal(ys[0], ys[1]) and np.array_equal(ys[0], ys[2])
+
+
+def test_chain_sharded_state_on_one_gpu(p0):
+    """SURVEY.md §8(f)-2 on the GPU path: the slices two ranks would take (runtime.shard_range), run one after the
+    other on this GPU through runtime.gwl_local_sigma_sum, add up to gwl_selfenergy_state; a single process
+    (no process group) passes through."""
+    import torch
+    from paper_2310_20103_b200 import runtime
+    cfg = p0.cfg
+    n_orb, m, L = cfg.n_v + cfg.n_c, cfg.n_v - 1, 20
+    with _ctx(p0, chains=False) as ctx:
+        full_host = ctx.selfenergy_state(m, L, 12, 0, p0.omega, DLT)
+        ctx.set_pointer_mode(1)
+        ctx.set_stream(torch.cuda.current_stream().cuda_stream)
+        om = torch.from_numpy(p0.omega).cuda()
+        local = runtime.gwl_local_sigma_sum(ctx, m, L, 12, 0, om, DLT)
+        parts = [local(*runtime.shard_range(n_orb, r, 2)) for r in range(2)]
+        single = runtime.sharded_sigma_state(local, n_orb)
+        torch.cuda.synchronize()
+    tot = (parts[0] + parts[1]).cpu().numpy()
+    assert np.abs(tot[:, 0] + 1j * tot[:, 1] - full_host).max() <= 1e-11 * np.abs(full_host).max()
+    one = single.cpu().numpy()
+    assert np.abs(one[:, 0] + 1j * one[:, 1] - full_host).max() <= 1e-11 * np.abs(full_host).max()
+    ref = orc.sigma_state(p0.phi_v, p0.phi_c, p0.eps_v, p0.eps_c, p0.V, m, L, p0.omega, DLT)
+    assert np.abs(full_host - ref).max() <= TOL_SIGMA
