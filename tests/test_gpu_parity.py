@@ -537,3 +537,18 @@ def test_chain_sharded_state_on_one_gpu(p0):
     assert np.abs(one[:, 0] + 1j * one[:, 1] - full_host).max() <= 1e-11 * np.abs(full_host).max()
     ref = orc.sigma_state(p0.phi_v, p0.phi_c, p0.eps_v, p0.eps_c, p0.V, m, L, p0.omega, DLT)
     assert np.abs(full_host - ref).max() <= TOL_SIGMA
+
+
+@pytest.mark.parametrize("n_v,n_c,n_mu,L", [(3, 5, 37, 12), (7, 331, 64, 25), (4, 600, 48, 30)])
+def test_reorthogonalised_lanczos_ragged_sizes(n_v, n_c, n_mu, L):
+    """Full reorthogonalisation kernels on odd N_vc (scalar loads), on N_vc spanning several 2048-element slices with a
+    ragged last slice, and on an even N_vc (16-byte loads): alpha/beta and Sigma against the oracle, both sides
+    reorthogonalised."""
+    p = synth.make_custom(n_v, n_c, n_mu, seed=n_c, chains_a=2, chains_b=3)
+    with _ctx(p) as ctx:
+        a, b, n2, ln = ctx.lanczos(6, L, 4, 1)
+        sig, _ = ctx.selfenergy(p.omega, DLT, 6)
+    ref = orc.run_chains(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, p.n_idx, p.m_idx, L, p.omega, DLT, reorth=True)
+    assert (ln == ref["len"]).all()
+    _check_ab(a, b, ref["alpha"], ref["beta"], L)
+    assert np.abs(sig - ref["sigma"]).max() <= TOL_SIGMA
