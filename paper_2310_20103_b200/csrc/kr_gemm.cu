@@ -82,8 +82,10 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];\n" ::"l"(map) : "memory");
 }
 
+// volatile: keeps the DMMAs of a k-step in program order (A fragment outer, B inner).  Without it ptxas scrambled the
+// order in the K.X kernel (no operand reuse, accumulators out of sequence); in order, K.X runs as fast as K^T.W.
 __device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, double b) {
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
         : "+d"(c0), "+d"(c1)
         : "d"(a), "d"(b));
 }
