@@ -453,3 +453,24 @@ def test_tda_one_by_one_closed_form():
     for j, (e_n, sg, P2) in enumerate([(p.eps_v[0], 1, k * k), (p.eps_c[0], -1, ((p.phi_c[:, 0] ** 2) @ p.V @ rho) ** 2)]):
         ref = P2 / (om - e_n + sg * (delta[0] + k - 1j * DLT))
         assert np.abs(r["sigma"][j] - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+def test_oracle_matches_its_golden_file():
+    """Regression pin: tests/golden/cfg0_oracle.txt (written by tests/golden/make_golden.py from the oracle alone; the paper
+    prints no worked example).  A deliberate change of the oracle's arithmetic regenerates the file in the same commit."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    got = {(n, j, k): v for n, j, k, v in mod.compute()}
+    stored = {}
+    for line in open(os.path.join(here, "cfg0_oracle.txt")):
+        if line.startswith("#"):
+            continue
+        n, j, k, v = line.split()
+        stored[(n, int(j), int(k))] = float(v)
+    assert set(got) == set(stored)
+    for key, v in stored.items():
+        assert abs(got[key] - v) <= 1e-9 * max(1.0, abs(v)), key
