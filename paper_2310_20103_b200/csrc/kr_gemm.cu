@@ -430,54 +430,61 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                     d0 = p.d2[voff + r0];
                     d1 = two ? p.d2[voff + r0 + 1] : 0.0;
                 }
-                // all x loads of this row pair are issued before the first store: one L2 round trip per i2 instead of
-                // one per element (x and out never alias, include/gwl.h, but the compiler cannot know)
-                double xr[FN][2][2];
-                if (EPI == EPI_CASIDA) {
+                // the x loads of a batch of JB columns are issued before its first store: one L2 round trip per batch
+                // instead of one per element (x and out never alias, include/gwl.h, but the compiler cannot know);
+                // wide warp tiles take two batches so that the batch fits beside the 128 accumulator registers
+                constexpr int JB = FN > 4 ? FN / 2 : FN;
 #pragma unroll
-                    for (int j = 0; j < FN; ++j)
+                for (int j0 = 0; j0 < FN; j0 += JB) {
+                    double xr[JB][2][2];
+                    if (EPI == EPI_CASIDA) {
+#pragma unroll
+                        for (int jj = 0; jj < JB; ++jj)
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                const int j = j0 + jj;
+                                const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
+                                xr[jj][e][0] = xr[jj][e][1] = 0.0;
+                                if (n >= p.N) continue;
+                                const double* xp = p.X + (int64_t)n * p.ldx + voff + r0;
+                                if (vec_ok && two) {
+                                    const double2 xv = __ldg(reinterpret_cast<const double2*>(xp));
+                                    xr[jj][e][0] = xv.x;
+                                    xr[jj][e][1] = xv.y;
+                                } else {
+                                    xr[jj][e][0] = __ldg(xp);
+                                    if (two) xr[jj][e][1] = __ldg(xp + 1);
+                                }
+                            }
+                    }
+#pragma unroll
+                    for (int jj = 0; jj < JB; ++jj)
 #pragma unroll
                         for (int e = 0; e < 2; ++e) {
+                            const int j = j0 + jj;
                             const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
-                            xr[j][e][0] = xr[j][e][1] = 0.0;
                             if (n >= p.N) continue;
-                            const double* xp = p.X + (int64_t)n * p.ldx + voff + r0;
-                            if (vec_ok && two) {
-                                const double2 xv = __ldg(reinterpret_cast<const double2*>(xp));
-                                xr[j][e][0] = xv.x;
-                                xr[j][e][1] = xv.y;
+                            const double u0v = acc[2 * i2][j][e], u1v = acc[2 * i2 + 1][j][e];
+                            double y0, y1;
+                            if (EPI == EPI_CASIDA) {
+                                const double x0 = xr[jj][e][0], x1 = xr[jj][e][1];
+                                y0 = d0 * x0 + cpl * (s0 * u0v);
+                                y1 = d1 * x1 + cpl * (s1 * u1v);
+                                part[j][e] += x0 * y0 + x1 * y1;
                             } else {
-                                xr[j][e][0] = __ldg(xp);
-                                if (two) xr[j][e][1] = __ldg(xp + 1);
+                                y0 = s0 * u0v;
+                                y1 = s1 * u1v;
+                                part[j][e] += y0 * y0 + y1 * y1;
+                            }
+                            double* yp = p.out + (int64_t)n * p.ldo + voff + r0;
+                            if (vec_ok && two) {
+                                *reinterpret_cast<double2*>(yp) = make_double2(y0, y1);
+                            } else {
+                                yp[0] = y0;
+                                if (two) yp[1] = y1;
                             }
                         }
                 }
-#pragma unroll
-                for (int j = 0; j < FN; ++j)
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
-                        if (n >= p.N) continue;
-                        const double u0v = acc[2 * i2][j][e], u1v = acc[2 * i2 + 1][j][e];
-                        double y0, y1;
-                        if (EPI == EPI_CASIDA) {
-                            const double x0 = xr[j][e][0], x1 = xr[j][e][1];
-                            y0 = d0 * x0 + cpl * (s0 * u0v);
-                            y1 = d1 * x1 + cpl * (s1 * u1v);
-                            part[j][e] += x0 * y0 + x1 * y1;
-                        } else {
-                            y0 = s0 * u0v;
-                            y1 = s1 * u1v;
-                            part[j][e] += y0 * y0 + y1 * y1;
-                        }
-                        double* yp = p.out + (int64_t)n * p.ldo + voff + r0;
-                        if (vec_ok && two) {
-                            *reinterpret_cast<double2*>(yp) = make_double2(y0, y1);
-                        } else {
-                            yp[0] = y0;
-                            if (two) yp[1] = y1;
-                        }
-                    }
             }
             if (p.dotpart != nullptr) {
                 // the producer is already refilling the stage ring for the next tile: `red` is its own array

@@ -44,7 +44,7 @@ __device__ __forceinline__ double block_sum_array(const double* a, int cnt, doub
 }
 
 __device__ __forceinline__ void slice_of(int64_t n, int npart, int blk, int64_t& lo, int64_t& hi) {
-    const int64_t per = (n + npart - 1) / npart;
+    const int64_t per = ((n + npart - 1) / npart + 1) & ~(int64_t)1;  // even: slices start 16-byte aligned
     lo = (int64_t)blk * per;
     hi = lo + per < n ? lo + per : n;
     if (lo > n) lo = n;
@@ -238,6 +238,20 @@ __global__ void k_lanczos_update2(double* __restrict__ w, int64_t n_vc, int nb, 
     slice_of(n_vc, gridDim.x, blockIdx.x, lo, hi);
     double* wb = w + (int64_t)b * n_vc;
     double* xsb = xs + (int64_t)b * ldxs;
+    if (n_c == n_cp && ((n_vc | ldxs) & 1) == 0) {  // no padding inside xs, every chain 16-byte aligned: 16-byte accesses
+        double2* w2 = reinterpret_cast<double2*>(wb);
+        double2* x2 = reinterpret_cast<double2*>(xsb);
+        const double2* s2 = reinterpret_cast<const double2*>(s);
+        for (int64_t i = (lo >> 1) + threadIdx.x; i < ((hi + 1) >> 1); i += NT) {
+            double2 v = w2[i];
+            const double2 sv = __ldg(s2 + i);
+            v.x = broken ? 0.0 : v.x * rbeta;
+            v.y = broken ? 0.0 : v.y * rbeta;
+            w2[i] = v;
+            x2[i] = make_double2(sv.x * v.x, sv.y * v.y);
+        }
+        return;
+    }
     for (int64_t i = lo + threadIdx.x; i < hi; i += NT) {
         const double qv = broken ? 0.0 : wb[i] * rbeta;
         wb[i] = qv;
