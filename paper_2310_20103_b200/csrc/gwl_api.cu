@@ -30,6 +30,7 @@ struct DevBuf {
         cudaError_t e = cudaMalloc(&p, need);
         if (e != cudaSuccess) {
             p = nullptr;
+            cudaGetLastError();  // clear it: the caller reports GWL_ENOMEM and the context stays usable
             return e;
         }
         bytes = need;

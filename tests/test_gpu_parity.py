@@ -552,3 +552,34 @@ def test_reorthogonalised_lanczos_ragged_sizes(n_v, n_c, n_mu, L):
     assert (ln == ref["len"]).all()
     _check_ab(a, b, ref["alpha"], ref["beta"], L)
     assert np.abs(sig - ref["sigma"]).max() <= TOL_SIGMA
+
+
+def test_poly_mode_config1_paper_parameters(p1):
+    """The paper's own parameters (g = 7, N_iter = 8) at config 1: full block of 64 chains on the GPU with
+    the product-side Chebyshev fit (polyfit.py); the oracle follows sampled chains with ITS fit."""
+    from paper_2310_20103_b200 import polyfit
+    cfg = p1.cfg
+    lo, hi = polyfit.default_range(p1.eps_v, p1.eps_c)
+    idx = np.array([0, 37, 63])
+    with _ctx(p1) as ctx:
+        ctx.set_polynomial(7, polyfit.sqrt_chebyshev(7, lo, hi), lo, hi)
+        a, b, n2, ln = ctx.lanczos(cfg.n_chains, 8, cfg.block, 0)
+        sig, _ = ctx.selfenergy(p1.omega, DLT, cfg.n_chains)
+    delta = orc.delta_vc(p1.eps_v, p1.eps_c)
+    rlo, rhi = 0.8 * (delta ** 2).min(), 1.25 * (delta ** 2).max()
+    assert abs(lo - rlo) <= 1e-12 * rlo and abs(hi - rhi) <= 1e-12 * rhi
+    ref = _oracle_chains(p1, idx, 8, False, poly=(orc.fit_sqrt_chebyshev(7, rlo, rhi), rlo, rhi))
+    _check_ab(a[idx], b[idx], ref["alpha"], ref["beta"], 8)
+    assert np.abs(sig[idx] - ref["sigma"]).max() <= TOL_SIGMA
+
+
+def test_out_of_memory_is_reported_and_context_survives():
+    """A reorthogonalised run whose basis (100 001 x 4 x 65 536 doubles = 210 GB) cannot be allocated returns
+    GWL_ENOMEM from a single failed cudaMalloc; the context keeps working afterwards."""
+    p = synth.make_custom(8, 8192, 32, seed=2)
+    with _ctx(p) as ctx:
+        with pytest.raises(gwl.GwlError) as e:
+            ctx._ck(ctx._lib.gwl_lanczos(ctx._h, 4, 100000, 4, 1, None, None, None, None))
+        assert e.value.status == gwl.GWL_ENOMEM
+        a, b, n2, ln = ctx.lanczos(4, 10, 4, 1)
+        assert (ln == 10).all() and np.isfinite(a).all() and (b > 0).all()
