@@ -350,43 +350,51 @@ __global__ void __launch_bounds__(NT) k_reorth_dots(const double* __restrict__ b
                                                     double* __restrict__ coefpart, int npart, int64_t slice) {
     pdl_trigger();
     pdl_wait();
-    extern __shared__ double ws[];  // [slice]
+    extern __shared__ double ws[];  // [RSLICE] chunk of w, then [nslots] running sums (one owner warp per basis vector)
+    double* accs = ws + RSLICE;
     const int b = blockIdx.y;
     const int64_t lo = (int64_t)blockIdx.x * slice;
-    const int len = (int)max((int64_t)0, min(slice, n_vc - lo));
-    const double* wb = w + (int64_t)b * n_vc + lo;
-    for (int j = threadIdx.x; j < len; j += NT) ws[j] = wb[j];
-    __syncthreads();
+    const int64_t len = max((int64_t)0, min(slice, n_vc - lo));
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool vec2 = ((n_vc | slot_stride | slice) & 1) == 0;  // 16-byte alignment of every (slot, chain, slice) start
-    for (int i = warp; i < nslots; i += NT / 32) {
-        const double* qb = basis + (int64_t)i * slot_stride + (int64_t)b * n_vc + lo;
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        if (vec2) {
-            const double2* q2 = reinterpret_cast<const double2*>(qb);
-            const double2* w2 = reinterpret_cast<const double2*>(ws);
-            const int n2 = len >> 1;
-            int j = lane;
-            for (; j + 96 < n2; j += 128) {
-                const double2 x0 = __ldg(q2 + j), x1 = __ldg(q2 + j + 32), x2 = __ldg(q2 + j + 64), x3 = __ldg(q2 + j + 96);
-                const double2 y0 = w2[j], y1 = w2[j + 32], y2 = w2[j + 64], y3 = w2[j + 96];
-                a0 = fma(x0.x, y0.x, fma(x0.y, y0.y, a0));
-                a1 = fma(x1.x, y1.x, fma(x1.y, y1.y, a1));
-                a2 = fma(x2.x, y2.x, fma(x2.y, y2.y, a2));
-                a3 = fma(x3.x, y3.x, fma(x3.y, y3.y, a3));
+    for (int i = threadIdx.x; i < nslots; i += NT) accs[i] = 0.0;
+    // a slice longer than RSLICE (N_vc > 64 * RSLICE) is walked in chunks; the chunk order is fixed
+    for (int64_t c0 = 0; c0 < len; c0 += RSLICE) {
+        const int clen = (int)min((int64_t)RSLICE, len - c0);
+        const double* wb = w + (int64_t)b * n_vc + lo + c0;
+        __syncthreads();  // the previous chunk has been consumed (and accs is initialised)
+        for (int j = threadIdx.x; j < clen; j += NT) ws[j] = wb[j];
+        __syncthreads();
+        for (int i = warp; i < nslots; i += NT / 32) {
+            const double* qb = basis + (int64_t)i * slot_stride + (int64_t)b * n_vc + lo + c0;
+            double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+            if (vec2) {
+                const double2* q2 = reinterpret_cast<const double2*>(qb);
+                const double2* w2 = reinterpret_cast<const double2*>(ws);
+                const int n2 = clen >> 1;
+                int j = lane;
+                for (; j + 96 < n2; j += 128) {
+                    const double2 x0 = __ldg(q2 + j), x1 = __ldg(q2 + j + 32), x2 = __ldg(q2 + j + 64), x3 = __ldg(q2 + j + 96);
+                    const double2 y0 = w2[j], y1 = w2[j + 32], y2 = w2[j + 64], y3 = w2[j + 96];
+                    a0 = fma(x0.x, y0.x, fma(x0.y, y0.y, a0));
+                    a1 = fma(x1.x, y1.x, fma(x1.y, y1.y, a1));
+                    a2 = fma(x2.x, y2.x, fma(x2.y, y2.y, a2));
+                    a3 = fma(x3.x, y3.x, fma(x3.y, y3.y, a3));
+                }
+                for (; j < n2; j += 32) {
+                    const double2 x0 = __ldg(q2 + j);
+                    const double2 y0 = w2[j];
+                    a0 = fma(x0.x, y0.x, fma(x0.y, y0.y, a0));
+                }
+            } else {
+                for (int j = lane; j < clen; j += 32) a0 = fma(__ldg(qb + j), ws[j], a0);
             }
-            for (; j < n2; j += 32) {
-                const double2 x0 = __ldg(q2 + j);
-                const double2 y0 = w2[j];
-                a0 = fma(x0.x, y0.x, fma(x0.y, y0.y, a0));
-            }
-            if ((len & 1) && lane == 0) a1 = fma(qb[len - 1], ws[len - 1], a1);
-        } else {
-            for (int j = lane; j < len; j += 32) a0 = fma(__ldg(qb + j), ws[j], a0);
+            const double acc = warp_sum((a0 + a1) + (a2 + a3));
+            if (lane == 0) accs[i] += acc;  // basis vector i always belongs to this warp
         }
-        const double acc = warp_sum((a0 + a1) + (a2 + a3));
-        if (lane == 0) coefpart[((int64_t)b * nslots + i) * npart + blockIdx.x] = acc;
     }
+    __syncthreads();
+    for (int i = threadIdx.x; i < nslots; i += NT) coefpart[((int64_t)b * nslots + i) * npart + blockIdx.x] = accs[i];
 }
 
 // w -= sum_i c_i basis_i, c_i = fixed-order sum of the partials; optionally the partial norms of the new w.
@@ -595,7 +603,7 @@ cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nsl
                                int nb, double* coefpart, int npart, cudaStream_t st) {
     if (npart != reorth_parts(n_vc)) return cudaErrorInvalidValue;
     const int64_t slice = reorth_slice(n_vc);
-    const size_t sm = (size_t)slice * sizeof(double);
+    const size_t sm = (size_t)(RSLICE + nslots) * sizeof(double);
     static size_t configured = 0;
     if (sm > 48 * 1024 && sm > configured) {
         cudaError_t e = cudaFuncSetAttribute(k_reorth_dots, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);

@@ -539,11 +539,11 @@ def test_chain_sharded_state_on_one_gpu(p0):
     assert np.abs(full_host - ref).max() <= TOL_SIGMA
 
 
-@pytest.mark.parametrize("n_v,n_c,n_mu,L", [(3, 5, 37, 12), (7, 331, 64, 25), (4, 600, 48, 30)])
+@pytest.mark.parametrize("n_v,n_c,n_mu,L", [(3, 5, 37, 12), (7, 331, 64, 25), (4, 600, 48, 30), (16, 8200, 32, 8)])
 def test_reorthogonalised_lanczos_ragged_sizes(n_v, n_c, n_mu, L):
     """Full reorthogonalisation kernels on odd N_vc (scalar loads), on N_vc spanning several 2048-element slices with a
-    ragged last slice, and on an even N_vc (16-byte loads): alpha/beta and Sigma against the oracle, both sides
-    reorthogonalised."""
+    ragged last slice, on an even N_vc (16-byte loads), and on N_vc = 131 200 > 64 x 2048 (slices longer than the
+    shared-memory chunk, as at configs 3-4): alpha/beta and Sigma against the oracle, both sides reorthogonalised."""
     p = synth.make_custom(n_v, n_c, n_mu, seed=n_c, chains_a=2, chains_b=3)
     with _ctx(p) as ctx:
         a, b, n2, ln = ctx.lanczos(6, L, 4, 1)
