@@ -1,12 +1,15 @@
 #!/usr/bin/env python
 """bench.py -- times the whole hot path of the Lanczos full-frequency GW method on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--full] [--impl ours|reference]
 
 One "step" = one pass of the whole path over one synthetic problem of
-BASELINE.json:configs[i] (default configs[1]): start vectors, `steps` Lanczos steps of all chains in
-blocks (each step one Casida block product plus the recurrence), Ritz/continued-fraction evaluation of
-Sigma^c on the omega grid and the sum over chains.
+BASELINE.json:configs[i] (default configs[4], the largest single-GPU configuration): start vectors, Lanczos
+steps of the chains in blocks (each step one Casida block product plus the recurrence), Ritz/continued-fraction
+evaluation of Sigma^c on the omega grid and the sum over chains.  For configs 2-4 a pass is BOUNDED so that the
+default run ends within minutes: one block of B chains x L_bench Lanczos steps (PASS below; named in
+config.workload / chains / lanczos_steps); chain-steps/s does not depend on L in steady state (every step is the same
+block product) and the S1/S6 overhead of the short pass is inside the timed region.  --full runs all chains x full L.
   value   = Lanczos chain-steps/s, whole job, inputs resident in HBM (device-pointer C-ABI calls)
   e2e     = the same through the host-pointer C-ABI calls: every step uploads orbitals, energies, the
             Coulomb kernel and the chain list from pinned host memory and reads alpha/beta/Sigma back
@@ -32,6 +35,8 @@ import numpy as np  # noqa: E402
 METRIC = "lanczos_chain_steps_per_s"
 UNIT = "chain-steps/s"
 L2_FLUSH_BYTES = 512 << 20
+# bounded pass per config: (chains, Lanczos steps); None = the whole config (all chains x full L)
+PASS = {0: None, 1: None, 2: (256, 60), 3: (256, 20), 4: (128, 10)}
 
 
 def parse():
@@ -39,7 +44,13 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json:configs (default 1)")
+    ap.add_argument("--config", type=int, default=None,
+                    help="index into BASELINE.json:configs (default 4, the largest; 2 with --sharded-state)")
+    ap.add_argument("--full", action="store_true", help="all chains x full L of the config instead of the bounded pass")
+    ap.add_argument("--chains", type=int, default=0, help="override the number of chains of a pass (marks the line)")
+    ap.add_argument("--sharded-state", action="store_true",
+                    help="SURVEY 8(f)-2 arm, its own line: the N_v+N_c chains of ONE state partitioned over the ranks "
+                         "(runtime.shard_range), one NCCL all-reduce of the omega grid; strong scaling")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -53,9 +64,26 @@ def parse():
     return ap.parse_args()
 
 
-def workload_config(cfg, n_gpus, L):
-    return {"workload": f"BASELINE.json:configs[{cfg_index(cfg)}] {cfg.name}", "n_v": cfg.n_v, "n_c": cfg.n_c,
-            "n_mu": cfg.n_mu, "n_vc": cfg.n_vc, "chains": cfg.n_chains, "block": cfg.block, "lanczos_steps": L,
+def pass_shape(args, cfg):
+    """(chains, L) of one timed pass."""
+    i = cfg_index(cfg)
+    nch, L = (cfg.n_chains, cfg.steps) if (args.full or PASS[i] is None) else PASS[i]
+    if args.lanczos_steps:
+        L = args.lanczos_steps
+    if args.chains:
+        nch = min(args.chains, cfg.n_chains)
+    return nch, L
+
+
+def workload_config(cfg, n_gpus, L, nch=None):
+    nch = cfg.n_chains if nch is None else nch
+    i = cfg_index(cfg)
+    what = f"BASELINE.json:configs[{i}] {cfg.name}"
+    if (nch, L) != (cfg.n_chains, cfg.steps):
+        what += (f"; bounded pass: {nch} chains (blocks of {cfg.block}) x {L} Lanczos steps of the config's "
+                 f"{cfg.n_chains} x {cfg.steps}, S1 + S2-S4 + S5-S7 on the full omega grid")
+    return {"workload": what, "n_v": cfg.n_v, "n_c": cfg.n_c,
+            "n_mu": cfg.n_mu, "n_vc": cfg.n_vc, "chains": nch, "block": cfg.block, "lanczos_steps": L,
             "n_omega": cfg.n_omega, "eta_eV": cfg.eta, "mode": "direct (Op = C), reorth off",
             "parallelism": "single GPU" if n_gpus == 1 else f"{n_gpus} independent replicas",
             "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB write)", "seed": 0}
@@ -87,14 +115,13 @@ def host_threads():
     return os.cpu_count() or 1
 
 
-def cpu_baseline(prob, budget_s=12.0):
+def cpu_baseline(prob, nch_pass, L_pass, budget_s=12.0):
     """Oracle timed on a bounded sample of the same workload (about 10-30 s of host work)."""
-    cfg = prob.cfg
-    t1 = oracle_sample(prob, 1, 3)                 # calibration (also warms BLAS)
-    per = max(t1 / 3.0, 1e-6)
-    total = max(4, min(int(budget_s / per), cfg.n_chains * cfg.steps))
-    nch = max(1, min(cfg.n_chains, total // 20))              # at least 20 steps per sampled chain when affordable
-    L = max(2, min(cfg.steps, total // nch))
+    t1 = oracle_sample(prob, 1, 2)                 # calibration (also warms BLAS)
+    per = max(t1 / 2.0, 1e-6)
+    total = max(4, min(int(budget_s / per), nch_pass * L_pass))
+    L = max(2, min(L_pass, 20, total))
+    nch = max(1, min(nch_pass, total // L))
     t = oracle_sample(prob, nch, L)
     return {"value": nch * L / t, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
             "sample": f"{nch} chains x {L} Lanczos steps of the same workload + Sigma on the full omega grid, "
@@ -108,14 +135,15 @@ def run_reference(args):
         return
     from paper_2310_20103_b200 import synth
     cfg = synth.CONFIGS[args.config]
+    nch_pass, L_pass = pass_shape(args, cfg)
     prob = synth.make_problem(cfg)
     _ = prob.V
     t1 = oracle_sample(prob, 1, 2)
     per = max(t1 / 2.0, 1e-6)
     budget = 150.0 / max(args.steps + args.warmup, 1)        # whole run within a few minutes
     total = max(2, int(budget / per))
-    L = max(2, min(cfg.steps, 20, total))
-    nch = max(1, min(cfg.n_chains, total // L))
+    L = max(2, min(L_pass, 20, total))
+    nch = max(1, min(nch_pass, total // L))
     for _ in range(args.warmup):
         oracle_sample(prob, nch, L)
     t0 = time.perf_counter()
@@ -127,7 +155,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(cfg, args.gpus, cfg.steps),
+            "config": workload_config(cfg, args.gpus, L_pass, nch_pass),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": host_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -138,7 +166,8 @@ def run_paper_setting(args):
     """One quasiparticle state the way the paper runs it: Lanczos on p_g(C), g = 7,
     N_iter = 8, one chain per n = 1..N_v+N_c, then Sigma^x and the Newton-Raphson solve.  Context for BASELINE.md's
     Table I quotes (the paper's wall times include the CPU-only ISDF step and real data; this is the hot path only, on
-    synthetic inputs of the same shape)."""
+    synthetic inputs of the same shape).  The fitting range comes from a 40-step Lanczos estimate of the top of the
+    spectrum (polyfit.range_from_spectrum), inside the timed state."""
     import torch
 
     from paper_2310_20103_b200 import gwl, polyfit, synth
@@ -151,14 +180,12 @@ def run_paper_setting(args):
     prob = synth.make_custom(n_v, n_c, n_mu, box=25.0, seed=0, n_omega=401)
     n_orb = n_v + n_c
     m = n_v - 1                                                   # the HOMO
-    lo, hi = polyfit.default_range(prob.eps_v, prob.eps_c)
     ctx = gwl.Context(n_v, n_c, n_mu)
     stream = torch.cuda.current_stream()
     ctx.set_stream(stream.cuda_stream)
     ctx.set_orbitals(prob.phi_v, prob.phi_c)
     ctx.set_energies(prob.eps_v, prob.eps_c)
     ctx.set_kernel(prob.V)
-    ctx.set_polynomial(g, polyfit.sqrt_chebyshev(g, lo, hi), lo, hi)
     ctx.set_pointer_mode(1)
     ctx.set_profiling(0)
     om = torch.from_numpy(prob.omega).to(dev)
@@ -166,8 +193,13 @@ def run_paper_setting(args):
     sx = torch.empty(1, dtype=torch.float64, device=dev)
     out = (torch.empty(1, dtype=torch.float64, device=dev), torch.empty(1, dtype=torch.float64, device=dev),
            torch.empty(1, dtype=torch.int32, device=dev))
+    rng = [0.0, 0.0]
 
     def state():
+        ctx.set_polynomial(0)
+        lo, hi = polyfit.range_from_spectrum(ctx, prob.eps_v, prob.eps_c, steps=40)
+        rng[:] = [lo, hi]
+        ctx.set_polynomial(g, polyfit.sqrt_chebyshev(g, lo, hi), lo, hi)
         ctx.selfenergy_state(m, n_iter, block, 0, om, 0.68, out=sc[0])        # delta = 0.05 Ry
         ctx.exchange([m], out=sx)
         ctx.qp_solve([prob.eps_v[m]], [-9.0], sx, sc, om, out=out)
@@ -183,13 +215,14 @@ def run_paper_setting(args):
         b.record(stream)
     torch.cuda.synchronize()
     sec = sum(a.elapsed_time(b) for a, b in ev) * 1e-3 / args.steps
-    flop = n_orb * n_iter * g * (4.0 * n_mu * n_v * n_c + 2.0 * n_mu * n_mu)
+    flop = (n_orb * n_iter * g + 40) * (4.0 * n_mu * n_v * n_c + 2.0 * n_mu * n_mu)
     line = {"metric": "seconds_per_quasiparticle_state", "value": sec, "unit": "s", "higher_is_better": False,
             "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "paper setting: N_iter = 8, g = 7 (PAPER.md:145), all N_v+N_c chains of one state, "
-                                   "Sigma^x, Newton-Raphson", "n_v": n_v, "n_c": n_c, "n_mu": n_mu, "chains": n_orb,
-                       "block": block},
-            "c_applies": n_orb * n_iter * g, "tflops_flop_model": flop / sec / 1e12,
+                                   "Sigma^x, Newton-Raphson; fitting range from a 40-step Lanczos bound (PAPER.md:284)",
+                       "n_v": n_v, "n_c": n_c, "n_mu": n_mu, "chains": n_orb, "block": block,
+                       "fit_range_eV2": rng},
+            "c_applies": n_orb * n_iter * g + 40, "tflops_flop_model": flop / sec / 1e12,
             "gpu_launches": int((ctx.get_launch_count() - n0) / args.steps),
             "e_qp_eV": float(out[0].item()), "z": float(out[1].item()),
             "note": "context only: hot path on synthetic inputs; the paper's Table I wall times include ISDF on CPUs"}
@@ -197,14 +230,115 @@ def run_paper_setting(args):
     ctx.close()
 
 
+def cublas_dgemm_tflops(dev, n=8192, reps=3):
+    """torch.matmul FP64 n^3 (cuBLAS DGEMM), best of `reps`: printed beside the DMMA probe as context."""
+    import torch
+    a = torch.randn(n, n, dtype=torch.float64, device=dev)
+    b = torch.randn(n, n, dtype=torch.float64, device=dev)
+    c = torch.matmul(a, b)
+    torch.cuda.synchronize()
+    best = None
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        torch.matmul(a, b, out=c)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    del a, b, c
+    torch.cuda.empty_cache()
+    return 2.0 * n ** 3 / (best * 1e-3) / 1e12
+
+
+def run_sharded_state(args):
+    """Sigma^corr_mm(omega) of ONE state with its N_v+N_c chains partitioned over the ranks
+    (runtime.shard_range), direct mode, L steps each, ONE all-reduce (NCCL) of the omega grid.  Strong scaling:
+    the total work is fixed as N grows.  Prints its own JSON line (not the headline bench line)."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2310_20103_b200 import gwl, runtime, synth
+
+    rank, local_rank, world = runtime.dist_env()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    gwl.load_library()
+    cfg = synth.CONFIGS[args.config]
+    L = args.lanczos_steps or 8
+    prob = synth.make_problem(cfg)
+    n_orb = cfg.n_v + cfg.n_c
+    m = cfg.n_v - 1
+    stream = torch.cuda.current_stream()
+    ctx = gwl.Context(cfg.n_v, cfg.n_c, cfg.n_mu)
+    ctx.set_stream(stream.cuda_stream)
+    ctx.set_orbitals(prob.phi_v, prob.phi_c)
+    ctx.set_energies(prob.eps_v, prob.eps_c)
+    ctx.set_kernel(prob.V)
+    ctx.set_pointer_mode(1)
+    ctx.set_profiling(0)
+    om = torch.from_numpy(prob.omega).to(dev)
+    local = runtime.gwl_local_sigma_sum(ctx, m, L, cfg.block, 0, om, cfg.eta)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    for _ in range(args.warmup):
+        runtime.sharded_sigma_state(local, n_orb)
+    torch.cuda.synchronize()
+    sampler = runtime.ClockSampler(local_rank).start()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    pairs = []
+    n0 = ctx.get_launch_count()
+    for _ in range(args.steps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        sig = runtime.sharded_sigma_state(local, n_orb)
+        e1.record(stream)
+        pairs.append((e0, e1))
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop()
+    elapsed = sum(a.elapsed_time(b) for a, b in pairs) * 1e-3
+    lo, hi = runtime.shard_range(n_orb, rank, world)
+    units, tmax = runtime.aggregate_throughput(float(args.steps) * (hi - lo) * L, elapsed, dev)
+    if rank == 0:
+        line = {"metric": METRIC, "value": units / tmax, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": 1e3 * tmax / args.steps, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "arm": "sharded-state (SURVEY 8(f)-2): not the headline bench line",
+                "config": {"workload": f"BASELINE.json:configs[{args.config}] {cfg.name}: Sigma^corr_mm of one state (HOMO), "
+                                       f"all {n_orb} chains x {L} Lanczos steps, chains partitioned over {world} rank(s), "
+                                       "one all-reduce of the omega grid", "n_v": cfg.n_v, "n_c": cfg.n_c,
+                           "n_mu": cfg.n_mu, "chains": n_orb, "block": cfg.block, "lanczos_steps": L,
+                           "n_omega": cfg.n_omega, "parallelism": f"chain-sharded x{world}",
+                           "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB write)"},
+                "clocks": clocks, "gpu_launches": int(ctx.get_launch_count() - n0),
+                "allreduce_bytes_per_step": int(cfg.n_omega * 16) if world > 1 else 0,
+                "sigma_checksum": float(sig.abs().sum().item())}
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 # ------------------------------------------------------------------------------------------------
 def main():
     args = parse()
+    if args.config is None:
+        args.config = 2 if args.sharded_state else 4
     if args.impl == "reference":
         run_reference(args)
         return
     if args.paper_setting:
         run_paper_setting(args)
+        return
+    if args.sharded_state:
+        run_sharded_state(args)
         return
 
     import torch
@@ -226,7 +360,7 @@ def main():
     gwl.load_library()
 
     cfg = synth.CONFIGS[args.config]
-    L = args.lanczos_steps or cfg.steps
+    nch, L = pass_shape(args, cfg)
     prob = synth.make_problem(cfg)
     V = prob.V
 
@@ -235,6 +369,7 @@ def main():
 
     h = {k: pin(v) for k, v in dict(phi_v=prob.phi_v, phi_c=prob.phi_c, eps_v=prob.eps_v, eps_c=prob.eps_c, V=V,
                                     omega=prob.omega).items()}
+    n_idx, m_idx = prob.n_idx[:nch], prob.m_idx[:nch]
     stream = torch.cuda.current_stream()
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
     ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
@@ -245,18 +380,19 @@ def main():
     ctx.set_orbitals(h["phi_v"], h["phi_c"])
     ctx.set_energies(h["eps_v"], h["eps_c"])
     ctx.set_kernel(h["V"])
-    ctx.set_chains(prob.n_idx, prob.m_idx)
+    ctx.set_chains(n_idx, m_idx)
     ctx.set_pointer_mode(1)
     ctx.set_profiling(0)          # no events inside the timed region
     omega_d = torch.from_numpy(prob.omega).to(dev)
-    sig_d = torch.empty(cfg.n_chains, cfg.n_omega, 2, dtype=torch.float64, device=dev)
+    sig_d = torch.empty(nch, cfg.n_omega, 2, dtype=torch.float64, device=dev)
     sum_d = torch.empty(cfg.n_omega, 2, dtype=torch.float64, device=dev)
 
     def step_device():
-        ctx.lanczos(cfg.n_chains, L, cfg.block, 1 if args.reorth else 0, out=None)
+        ctx.lanczos(nch, L, cfg.block, 1 if args.reorth else 0, out=None)
         ctx.selfenergy(omega_d, cfg.eta, out=(sig_d, sum_d))
 
     dmma_peak = gwl.probe_fp64_peak(0)            # also warms the clocks
+    dgemm_peak = cublas_dgemm_tflops(dev) if rank == 0 else None
     for _ in range(args.warmup):
         step_device()
     torch.cuda.synchronize()
@@ -298,16 +434,17 @@ def main():
     prof_elapsed_s = sum(a.elapsed_time(b) for a, b in prof_pairs) * 1e-3
     ctx.set_profiling(0)
     clocks = sampler.stop()
-    units = float(args.steps) * cfg.n_chains * L
+    units = float(args.steps) * nch * L
     tot_units, max_elapsed = runtime.aggregate_throughput(units, elapsed_s, dev)
     value = tot_units / max_elapsed
 
     # ---- the dominant kernel against the FP64 tensor roofline ----------------------------------------
     gemm_keys = ("gemm_fwd_KX", "gemm_bwd_KtW", "gemm_V")
     dom = max(gemm_keys, key=lambda k: ktimes[k][0])
-    blocks = -(-cfg.n_chains // cfg.block)
-    flop_launch = {"gemm_fwd_KX": 2.0 * cfg.n_mu * cfg.n_vc * cfg.block, "gemm_bwd_KtW": 2.0 * cfg.n_mu * cfg.n_vc * cfg.block,
-                   "gemm_V": 2.0 * cfg.n_mu * cfg.n_mu * cfg.block}
+    nbl = min(cfg.block, nch)
+    blocks = -(-nch // cfg.block)
+    flop_launch = {"gemm_fwd_KX": 2.0 * cfg.n_mu * cfg.n_vc * nbl, "gemm_bwd_KtW": 2.0 * cfg.n_mu * cfg.n_vc * nbl,
+                   "gemm_V": 2.0 * cfg.n_mu * cfg.n_mu * nbl}
     dom_ms = ktimes[dom][0] / max(ktimes[dom][1], 1)
     achieved = flop_launch[dom] / (dom_ms * 1e-3) / 1e12
     peaks = {}
@@ -327,16 +464,26 @@ def main():
                 "unit": "TFLOP/s", "frac": achieved / dmma_peak, "traffic": traffic,
                 "peak_source": "live register-resident mma.sync.m8n8k4.f64 (DMMA) issue-rate probe on this GPU "
                                "(gwl_probe_fp64_peak); MEASURED_PEAKS.json has no FP64 entry",
+                "peak_cublas_dgemm": dgemm_peak,
+                "peak_cublas_dgemm_how": "torch.matmul float64 8192^3, best of 3, same process (context: what the "
+                                         "vendor library reaches on the same pipe)",
                 "peak_from_bf16_ratio": (peaks.get("bf16_tflops", 0) * 37.0 / 2250.0) or None,
                 "flop_per_launch": flop_launch[dom], "ms_per_launch": dom_ms, "launches_timed": ktimes[dom][1],
                 "timed_how": f"CUDA-event pair around every launch on the library's stream, {prof_steps} extra steps "
                              "run right after the timed region (events inside it would perturb the step time)"}
     step_ms = 1e3 * elapsed_s / args.steps
     share = {k: round(v[0] / (1e3 * prof_elapsed_s), 4) for k, v in ktimes.items() if v[1]}
-    mv_ms = sum(ktimes[k][0] for k in ("gemm_fwd_KX", "gemm_V", "gemm_bwd_KtW", "splitk_reduce")) / (prof_steps * blocks * L)
-    matvec = {"tflops": cfg.flop_per_vector() * cfg.block / (mv_ms * 1e-3) / 1e12, "ms_per_block_matvec": mv_ms,
-              "frac_of_dmma_peak": cfg.flop_per_vector() * cfg.block / (mv_ms * 1e-3) / 1e12 / dmma_peak,
-              "flop_model": "(4 N_mu N_vc + 2 N_mu^2) B"}
+    # block products inside the Lanczos loop only: S1 launches one V.T and one K^T.W per block on top of the L steps
+    n_mv = prof_steps * blocks * L
+    per = {k: ktimes[k][0] / max(ktimes[k][1], 1) for k in ("gemm_fwd_KX", "gemm_V", "gemm_bwd_KtW")}
+    # split-K reductions: two per product inside the loop (K.X, V.T), one per block in S1 (V.T)
+    red_ms = 2.0 * ktimes["splitk_reduce"][0] / (prof_steps * blocks * (2 * L + 1))
+    mv_ms = per["gemm_fwd_KX"] + per["gemm_V"] + per["gemm_bwd_KtW"] + red_ms
+    fpv = cfg.flop_per_vector() * nbl
+    matvec = {"tflops": fpv / (mv_ms * 1e-3) / 1e12, "ms_per_block_matvec": mv_ms,
+              "frac_of_dmma_peak": fpv / (mv_ms * 1e-3) / 1e12 / dmma_peak,
+              "flop_model": "(4 N_mu N_vc + 2 N_mu^2) B", "block_products_timed": n_mv,
+              "how": "mean launch duration of K.X + V.T + K^T.W (+ split-K reductions per product)"}
 
     # ---- end-to-end arm: host buffers through the C ABI --------------------------------------------------
     e2e = None
@@ -349,9 +496,9 @@ def main():
             hctx.set_orbitals(h["phi_v"], h["phi_c"])
             hctx.set_energies(h["eps_v"], h["eps_c"])
             hctx.set_kernel(h["V"])
-            hctx.set_chains(prob.n_idx, prob.m_idx)
-            out = hctx.lanczos(cfg.n_chains, L, cfg.block, 0)
-            sig = hctx.selfenergy(h["omega"], cfg.eta, cfg.n_chains)
+            hctx.set_chains(n_idx, m_idx)
+            out = hctx.lanczos(nch, L, cfg.block, 0)
+            sig = hctx.selfenergy(h["omega"], cfg.eta, nch)
             return out, sig
 
         for _ in range(min(args.warmup, 2)):
@@ -370,10 +517,9 @@ def main():
             hp.append((e0, e1))
         torch.cuda.synchronize()
         he = sum(a.elapsed_time(b) for a, b in hp) * 1e-3
-        hu, ht = runtime.aggregate_throughput(float(ke) * cfg.n_chains * L, he, dev)
-        h2d = sum(h[k].nbytes for k in ("phi_v", "phi_c", "eps_v", "eps_c", "V", "omega")) + 2 * 4 * cfg.n_chains \
-            + 12 * cfg.n_chains
-        d2h = cfg.n_chains * L * 16 + cfg.n_chains * 12 + cfg.n_chains * cfg.n_omega * 16 + cfg.n_omega * 16
+        hu, ht = runtime.aggregate_throughput(float(ke) * nch * L, he, dev)
+        h2d = sum(h[k].nbytes for k in ("phi_v", "phi_c", "eps_v", "eps_c", "V", "omega")) + 2 * 4 * nch + 12 * nch
+        d2h = nch * L * 16 + nch * 12 + nch * cfg.n_omega * 16 + cfg.n_omega * 16
         e2e = {"value": hu / ht, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "steps": ke, "ms_per_step": 1e3 * he / ke, "ms_each": [round(a.elapsed_time(b), 3) for a, b in hp]}
         hctx.close()
@@ -381,20 +527,20 @@ def main():
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, world, L),
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, world, L, nch),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "matvec": matvec,
                 "kernel_time_share": share}
-        if args.lanczos_steps:
-            line["note"] = "lanczos_steps overridden: profiling run, not a bench value"
+        if args.lanczos_steps or args.chains:
+            line["note"] = "chains / lanczos_steps overridden: profiling run, not a bench value"
         if args.reorth:
             line["note"] = "full reorthogonalisation on: not the bench workload"
             line["config"]["mode"] = "direct (Op = C), reorth on (CGS2)"
             rt = ktimes["reorth"]
             # CGS2 at step k reads the k+1 basis vectors twice per pass (dots, apply), two passes
-            nbytes = prof_steps * 4.0 * 8.0 * cfg.n_vc * cfg.n_chains * (L * (L + 1) / 2.0)
+            nbytes = prof_steps * 4.0 * 8.0 * cfg.n_vc * nch * (L * (L + 1) / 2.0)
             line["reorth"] = {"ms_per_pass_of_L_steps": rt[0] / prof_steps, "algorithmic_GBps": nbytes / (rt[0] * 1e-3) / 1e9}
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(prob)
+            line["cpu_baseline"] = cpu_baseline(prob, nch, L)
         print(json.dumps(line), flush=True)
     ctx.close()
     if world > 1:

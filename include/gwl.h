@@ -73,6 +73,16 @@ gwl_status gwl_set_kernel(gwl_ctx* ctx, const double* V);
  * NULL) clears it: Op = C and gwl_selfenergy evaluates Eq. 11 on the Ritz pairs of T_L ("direct mode"). */
 gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo, double hi);
 
+/* Extremal eigenvalues of the operator for the fitting range of p_g: "One can use standard Lanczos algorithm to
+ * determine the extremal eigenvalues min(Omega_s^2) and max(Omega_s^2) of C".  Runs `steps`
+ * (2..512; 30-60 is plenty) Lanczos steps on the operator itself (C, or A in the TDA; never p_g(C)) from a generic
+ * pseudo-random start vector and returns lam_max = theta_max + r_max and lam_min = theta_min - r_min, where theta are
+ * the extreme Ritz values and r = b_L |s_L| their residual norms (an eigenvalue lies within r of each; the top of a
+ * spectrum with a separated upper edge converges in a few steps, the dense lower edge slowly -- lam_min is a lower
+ * ESTIMATE that can undershoot; with V positive semidefinite min(Delta)^2 is a rigorous lower bound of C).
+ * Host outputs.  Replaces the chain list (call it before gwl_set_chains / gwl_set_start_vectors), synchronises. */
+gwl_status gwl_spectrum_bounds(gwl_ctx* ctx, int64_t steps, double* lam_min, double* lam_max);
+
 /* SURVEY.md 8(f)-3, first step.  GWL_RPA (default): the operator is C of Eq. 4.  GWL_TDA: the Tamm-Dancoff
  * approximation, "setting matrix B = 0 in the RPA Casida matrix ... only a Hermitian matrix A remains, and a standard
  * Lanczos algorithm for Hermitian matrix can be used" (formulas PAPER.md:306-313), here for real

@@ -138,6 +138,20 @@ def fit_sqrt_chebyshev(g, lo, hi):
     return c
 
 
+def spectrum_bounds_lanczos(apply_op, n, steps, seed=0):
+    """Extremal eigenvalues of the operator for the fitting range: "One can use standard Lanczos algorithm to determine
+    the extremal eigenvalues min(Omega_s^2) and max(Omega_s^2) of C".  `steps` Lanczos steps from a
+    generic random vector; returns (theta_min - r_min, theta_max + r_max) with theta the extreme eigenvalues of T and
+    r_i = b_L |s_L,i| the residual norm of that Ritz pair (an eigenvalue of the operator lies within r_i of theta_i)."""
+    p = np.random.default_rng(seed).uniform(-1.0, 1.0, n)
+    a, b, _, ln = lanczos(apply_op, p, min(int(steps), n))
+    if ln == 1:
+        return float(a[0] - b[0]), float(a[0] + b[0])
+    theta, S = sla.eigh_tridiagonal(a[:ln], b[:ln - 1])
+    r = b[ln - 1] * np.abs(S[-1, :])
+    return float(theta[0] - r[0]), float(theta[-1] + r[-1])
+
+
 def poly_eval_scalar(c, lo, hi, x):
     """p_g(x) for scalars/arrays, by the same three-term recurrence as poly_apply."""
     t = (2.0 * np.asarray(x, dtype=np.float64) - (hi + lo)) / (hi - lo)

@@ -80,7 +80,7 @@ struct gwl_ctx {
     DevBuf alpha, beta, norm2, len, scale, alive;
 
     // workspaces
-    DevBuf xs, T, W, part, dotpart, normpart, basis, coefpart, tA, tB, tC, u;
+    DevBuf xs, T, W, part, dotpart, normpart, basis, coefpart, tA, tB;
     DevBuf x_nidx, x_midx, x_part, x_sig, x_eps, x_vxc, x_sc, x_e, x_z, x_it;  // gwl_exchange / gwl_qp_solve staging
     DevBuf stage;            // gwl_set_orbitals staging
     DevBuf sk_ws, sk_flags;  // stream-K hand-over of the K^T.W GEMM (kr_gemm.cu)
@@ -150,6 +150,25 @@ struct KernelTimer {
     } while (0)
 
 namespace {
+
+// Makes the context's device current for the duration of an entry point and restores the caller's device after.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const gwl_ctx* c) {
+        if (c != nullptr && cudaGetDevice(&prev) == cudaSuccess && prev != c->device)
+            switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+
+// A new operator or chain list makes the tridiagonals of the last gwl_lanczos meaningless.
+void invalidate_run(gwl_ctx* ctx) {
+    ctx->run_chains = 0;
+    ctx->run_steps = 0;
+}
 
 struct LaunchScope {
     explicit LaunchScope(gwl_ctx* c) { g_launch_counter = &c->launches; }
@@ -236,8 +255,18 @@ gwl_status gemm_v(gwl_ctx* ctx, int nb) {
 
 // u = K^T W with the epilogue fused:  x != NULL: y = d2 o x + coupling s o u and the partial dots sum(x y);
 // x == NULL (start vectors): y = s o u and the partial dots sum(y y).
+// One term of the Chebyshev recurrence fused into the K^T.W epilogue (EPI_CHEB, kr_gemm.cu)
+struct ChebTerm {
+    const double* t0;  // t_{j-2} or NULL
+    double* w;         // running sum
+    const double* q;   // NULL except on the last term (alpha dots)
+    double* xs_out;    // NULL on the last term
+    double ca, cb, cc, cw, c0;
+    int first;
+};
+
 gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64_t ldy, int nb, double* dotpart,
-                    int dot_stride) {
+                    int dot_stride, const ChebTerm* cheb = nullptr) {
     const int kt_v = ctx->n_mup / BK;
     const int64_t ldm = ctx->n_mup;
     const GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, kt_v, kt_v, ctx->n_sm);
@@ -269,7 +298,24 @@ gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64
     if (++ctx->sk_epoch == 0) ++ctx->sk_epoch;
     p.epoch = ctx->sk_epoch;
     p.n_sm = ctx->n_sm;
-    CKL(2, launch_gemm(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, pl, p, ctx->n_v, ctx->stream));
+    int epi = x != nullptr ? EPI_CASIDA : EPI_START;
+    if (cheb != nullptr) {
+        if (x == nullptr || ldx != ldy) return ctx->fail(GWL_EINVAL, "internal: EPI_CHEB needs x and a common leading dimension");
+        epi = EPI_CHEB;
+        p.T0 = cheb->t0;
+        p.Wacc = cheb->w;
+        p.Q = cheb->q;
+        p.xs_out = cheb->xs_out;
+        p.ldxs = (int64_t)ctx->n_v * ctx->n_cp;
+        p.n_cp = ctx->n_cp;
+        p.ca = cheb->ca;
+        p.cb = cheb->cb;
+        p.cc = cheb->cc;
+        p.cw = cheb->cw;
+        p.c0 = cheb->c0;
+        p.first = cheb->first;
+    }
+    CKL(2, launch_gemm(MODE_BWD, epi, pl, p, ctx->n_v, ctx->stream));
     return GWL_OK;
 }
 
@@ -320,6 +366,7 @@ gwl_status gwl_create(gwl_ctx** out, int64_t n_v, int64_t n_c, int64_t n_mu) {
         cudaGetLastError();
         return GWL_ECUDA;
     }
+    if (prop.major != 10) return GWL_ECUDA;  // the kernels are sm_100a code (TMA, DMMA, clusters, PDL): B200 only
     gwl_ctx* ctx = new (std::nothrow) gwl_ctx();
     if (ctx == nullptr) return GWL_ENOMEM;
     ctx->n_v = (int)n_v;
@@ -336,12 +383,13 @@ gwl_status gwl_create(gwl_ctx** out, int64_t n_v, int64_t n_c, int64_t n_mu) {
 
 void gwl_destroy(gwl_ctx* ctx) {
     if (ctx == nullptr) return;
+    DeviceGuard dg(ctx);
     cudaStreamSynchronize(ctx->stream);
     DevBuf* bufs[] = {&ctx->phi_c, &ctx->phi_cT, &ctx->phi_vT, &ctx->V, &ctx->eps_v, &ctx->eps_c, &ctx->d2, &ctx->s,
                       &ctx->d_nidx, &ctx->d_midx, &ctx->d_start, &ctx->d_eps_n, &ctx->d_sgn_n, &ctx->alpha,
                       &ctx->beta, &ctx->norm2, &ctx->len, &ctx->scale, &ctx->alive, &ctx->xs, &ctx->T, &ctx->W,
                       &ctx->part, &ctx->dotpart, &ctx->normpart, &ctx->basis, &ctx->coefpart, &ctx->tA, &ctx->tB,
-                      &ctx->tC, &ctx->u, &ctx->theta, &ctx->wgt, &ctx->ritz_info, &ctx->d_omega, &ctx->d_zeta,
+                      &ctx->theta, &ctx->wgt, &ctx->ritz_info, &ctx->d_omega, &ctx->d_zeta,
                       &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y, &ctx->sk_ws, &ctx->sk_flags, &ctx->stage, &ctx->x_nidx, &ctx->x_midx, &ctx->x_part, &ctx->x_sig,
                       &ctx->x_eps, &ctx->x_vxc, &ctx->x_sc, &ctx->x_e, &ctx->x_z, &ctx->x_it};
     for (DevBuf* b : bufs) b->release();
@@ -354,12 +402,14 @@ const char* gwl_last_error(const gwl_ctx* ctx) { return ctx ? ctx->err.c_str() :
 
 gwl_status gwl_set_pointer_mode(gwl_ctx* ctx, int device_ptrs) {
     if (ctx == nullptr || (device_ptrs != 0 && device_ptrs != 1)) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     ctx->device_ptrs = device_ptrs;
     return GWL_OK;
 }
 
 gwl_status gwl_set_stream(gwl_ctx* ctx, void* cuda_stream) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->stream = static_cast<cudaStream_t>(cuda_stream);
     return GWL_OK;
@@ -367,6 +417,7 @@ gwl_status gwl_set_stream(gwl_ctx* ctx, void* cuda_stream) {
 
 gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi_c) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (phi_v == nullptr || phi_c == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_orbitals: NULL input");
     LaunchScope ls(ctx);
     cudaStream_t st = ctx->stream;
@@ -387,11 +438,13 @@ gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi
     CKL(4, launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_v, ctx->phi_vT.as<double>(), ctx->n_mup, st));
     CK(cudaStreamSynchronize(st));
     ctx->have_orb = true;
+    invalidate_run(ctx);
     return GWL_OK;
 }
 
 gwl_status gwl_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps_c) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (eps_v == nullptr || eps_c == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_energies: NULL input");
     double vmax = -INFINITY, cmin = INFINITY;
     for (int i = 0; i < ctx->n_v; ++i) {
@@ -417,11 +470,17 @@ gwl_status gwl_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps
                           ctx->s.as<double>(), ctx->approx, st));
     CK(cudaStreamSynchronize(st));
     ctx->have_eps = true;
+    invalidate_run(ctx);
+    if (ctx->chain_mode == 1) {  // eps_n / eta_n of index chains were taken from the old energies
+        ctx->chain_mode = 0;
+        ctx->n_chains_set = 0;
+    }
     return GWL_OK;
 }
 
 gwl_status gwl_set_kernel(gwl_ctx* ctx, const double* V) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (V == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_kernel: NULL input");
     cudaStream_t st = ctx->stream;
     CK(ctx->V.ensure((size_t)ctx->n_mu * ctx->n_mup * 8, st));
@@ -430,15 +489,18 @@ gwl_status gwl_set_kernel(gwl_ctx* ctx, const double* V) {
                          (size_t)ctx->n_mu, cudaMemcpyHostToDevice, st));
     CK(cudaStreamSynchronize(st));
     ctx->have_V = true;
+    invalidate_run(ctx);
     return GWL_OK;
 }
 
 gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo, double hi) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (g < 0 || g > 64) return ctx->fail(GWL_EINVAL, "gwl_set_polynomial: g out of range [0, 64]");
     if (g == 0) {
         ctx->g = 0;
         ctx->cheb.clear();
+        invalidate_run(ctx);
         return GWL_OK;
     }
     if (cheb == nullptr || !(hi > lo) || !std::isfinite(lo) || !std::isfinite(hi))
@@ -449,16 +511,17 @@ gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo
     ctx->cheb.assign(cheb, cheb + g + 1);
     ctx->lo = lo;
     ctx->hi = hi;
+    invalidate_run(ctx);
     return GWL_OK;
 }
 
 gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation) {
     if (ctx == nullptr || (approximation != GWL_RPA && approximation != GWL_TDA)) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (approximation == GWL_TDA && ctx->g > 0)
         return ctx->fail(GWL_ESTATE, "gwl_set_approximation: clear the polynomial first (it approximates sqrt(C), RPA only)");
     ctx->approx = approximation;
-    ctx->run_chains = 0;
-    ctx->run_steps = 0;
+    invalidate_run(ctx);
     if (ctx->have_eps) {  // rebuild the diagonal term and the scaling for the new operator
         LaunchScope ls(ctx);
         cudaStream_t st = ctx->stream;
@@ -471,6 +534,7 @@ gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation) {
 
 gwl_status gwl_casida_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (nvec < 0) return ctx->fail(GWL_EINVAL, "gwl_casida_matvec: nvec < 0");
     if (nvec == 0) return GWL_OK;
     if (x == nullptr || y == nullptr) return ctx->fail(GWL_EINVAL, "gwl_casida_matvec: NULL vector");
@@ -511,6 +575,7 @@ gwl_status gwl_casida_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t n
 
 gwl_status gwl_set_chains(gwl_ctx* ctx, int64_t n_chains, const int32_t* n_idx, const int32_t* m_idx) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (n_chains < 0 || (n_chains > 0 && (n_idx == nullptr || m_idx == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_set_chains: bad arguments");
     if (!ctx->have_eps) return ctx->fail(GWL_ESTATE, "gwl_set_chains: energies must be set first");
@@ -538,13 +603,14 @@ gwl_status gwl_set_chains(gwl_ctx* ctx, int64_t n_chains, const int32_t* n_idx, 
     CK(cudaStreamSynchronize(st));
     ctx->chain_mode = 1;
     ctx->n_chains_set = n_chains;
-    ctx->run_chains = 0;
+    invalidate_run(ctx);
     return GWL_OK;
 }
 
 gwl_status gwl_set_start_vectors(gwl_ctx* ctx, int64_t n_chains, const double* p, const double* eps_n,
                                  const int32_t* sgn_n) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (n_chains < 0 || (n_chains > 0 && (p == nullptr || eps_n == nullptr || sgn_n == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_set_start_vectors: bad arguments");
     for (int64_t j = 0; j < n_chains; ++j)
@@ -562,13 +628,14 @@ gwl_status gwl_set_start_vectors(gwl_ctx* ctx, int64_t n_chains, const double* p
     CK(cudaStreamSynchronize(st));
     ctx->chain_mode = 2;
     ctx->n_chains_set = n_chains;
-    ctx->run_chains = 0;
+    invalidate_run(ctx);
     return GWL_OK;
 }
 
 gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t block, int reorth, double* alpha,
                        double* beta, double* norm2, int32_t* len) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (n_chains < 0 || steps < 1 || steps > 100000 || block < 1 || (reorth != 0 && reorth != 1))
         return ctx->fail(GWL_EINVAL, "gwl_lanczos: bad arguments");
     if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_lanczos: orbitals, energies and kernel must be set");
@@ -577,14 +644,15 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
     LaunchScope ls(ctx);
     cudaStream_t st = ctx->stream;
     const int L = (int)steps;
-    const int nbmax = (int)std::min<int64_t>(block, std::max<int64_t>(n_chains, 1));
+    // `block` is a batching hint: chains per launch are capped by grid.y of the vector kernels
+    const int nbmax = (int)std::min<int64_t>(std::min<int64_t>(block, 65535), std::max<int64_t>(n_chains, 1));
     const int64_t n_vc = ctx->n_vc;
     const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
     const int npart = vec_parts(n_vc);
     const int rparts = reorth_parts(n_vc);
     const bool poly = ctx->g > 0;
 
-    ctx->run_chains = 0;
+    invalidate_run(ctx);  // stays invalid if this call fails part-way
     ctx->ev_used = 0;
     ctx->kev_used = 0;
     ctx->kev_class.clear();
@@ -605,8 +673,6 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
         if (poly) {
             CK(ctx->tA.ensure((size_t)nbmax * n_vc * 8, st));
             CK(ctx->tB.ensure((size_t)nbmax * n_vc * 8, st));
-            CK(ctx->tC.ensure((size_t)nbmax * n_vc * 8, st));
-            CK(ctx->u.ensure((size_t)nbmax * n_vc * 8, st));
         }
     }
 
@@ -661,35 +727,38 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
                 ndot = ndot_c;
                 dstride = ndot_c;
             } else {
-                // w = p_g(C) q by the Chebyshev three-term recurrence on Ct = (2C - (hi+lo))/(hi-lo)
+                // w = p_g(C) q by the Chebyshev three-term recurrence on Ct = (2C - (hi+lo))/(hi-lo):
+                //   t_1 = Ct q,  t_j = 2 Ct t_{j-1} - t_{j-2},  w = sum_j c_j t_j.
+                // Every term is ONE Casida product whose K^T.W epilogue (EPI_CHEB) forms t_j from the accumulators, adds
+                // c_j t_j to w, writes the scaled copy s o t_j that the next K.X reads and, on the last term, the
+                // partial dots q.w of alpha: no streaming kernel between the GEMMs.
                 const double hl = ctx->hi - ctx->lo, hs = ctx->hi + ctx->lo;
-                const int64_t ntot = (int64_t)nb * n_vc;
-                double* u = ctx->u.as<double>();
-                double* tb[3] = {ctx->tA.as<double>(), ctx->tB.as<double>(), ctx->tC.as<double>()};
-                gwl_status rs = apply_casida_core(ctx, q, n_vc, u, n_vc, nb, nullptr, 0);  // xs = s o q is ready
-                if (rs != GWL_OK) return rs;
-                const double* t0 = q;
-                double* t1 = tb[0];
-                CKL(4, launch_axpby3(t1, 2.0 / hl, u, -hs / hl, q, 0.0, nullptr, ntot, st));
-                CKL(4, launch_axpby3(w, ctx->cheb[0], q, ctx->cheb[1], t1, 0.0, nullptr, ntot, st));
-                int nxt = 1;
-                for (int jj = 2; jj <= ctx->g; ++jj) {
-                    CKL(4, launch_prescale(t1, n_vc, ctx->xs.as<double>(), ldxs, ctx->s.as<double>(), ctx->n_v, ctx->n_c,
-                                       ctx->n_cp, nb, st));
-                    rs = apply_casida_core(ctx, t1, n_vc, u, n_vc, nb, nullptr, 0);
+                double* tb[2] = {ctx->tA.as<double>(), ctx->tB.as<double>()};
+                const double* x = q;         // t_{j-1}
+                const double* t0 = nullptr;  // t_{j-2}
+                for (int jj = 1; jj <= ctx->g; ++jj) {
+                    const bool last = jj == ctx->g;
+                    double* out = tb[(jj - 1) & 1];  // j >= 3: aliases t_{j-2} (read and written by the same thread)
+                    ChebTerm ct;
+                    ct.t0 = t0;
+                    ct.w = w;
+                    ct.q = last ? q : nullptr;
+                    ct.xs_out = last ? nullptr : ctx->xs.as<double>();
+                    ct.ca = (jj == 1 ? 2.0 : 4.0) / hl;
+                    ct.cb = (jj == 1 ? -1.0 : -2.0) * hs / hl;
+                    ct.cc = -1.0;
+                    ct.cw = ctx->cheb[jj];
+                    ct.c0 = ctx->cheb[0];
+                    ct.first = jj == 1;
+                    gwl_status rs = gemm_kx(ctx, nb);
+                    if (rs == GWL_OK) rs = gemm_v(ctx, nb);
+                    if (rs == GWL_OK) rs = gemm_ktw(ctx, x, n_vc, out, n_vc, nb, last ? dotpart : nullptr, ndot_c, &ct);
                     if (rs != GWL_OK) return rs;
-                    double* t2 = tb[nxt];
-                    // t2 may alias t0 (three rotating buffers, t0 is read element-wise before the write)
-                    CKL(4, launch_axpby3(t2, 4.0 / hl, u, -2.0 * hs / hl, t1, -1.0, t0, ntot, st));
-                    CKL(4, launch_axpby3(w, 1.0, w, ctx->cheb[jj], t2, 0.0, nullptr, ntot, st));
-                    t0 = t1;
-                    t1 = t2;
-                    nxt = (nxt + 1) % 3;
-                    if (tb[nxt] == t0) nxt = (nxt + 1) % 3;
+                    t0 = x;
+                    x = out;
                 }
-                CKL(4, launch_dot_partials(q, w, n_vc, n_vc, nb, dotpart, npart, st));
-                ndot = npart;
-                dstride = npart;
+                ndot = ndot_c;
+                dstride = ndot_c;
             }
             if (tstep) CK(cudaEventRecord(e1, st));
             if (!reorth && lanczos_fused_fits(n_vc)) {
@@ -728,6 +797,7 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
 
 gwl_status gwl_resolvent(gwl_ctx* ctx, const double* zeta, int64_t n_zeta, double* r) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (n_zeta < 0 || (n_zeta > 0 && (zeta == nullptr || r == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_resolvent: bad arguments");
     if (ctx->run_steps == 0) return ctx->fail(GWL_ESTATE, "gwl_resolvent: run gwl_lanczos first");
@@ -756,6 +826,7 @@ gwl_status gwl_resolvent(gwl_ctx* ctx, const double* zeta, int64_t n_zeta, doubl
 gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, double eta, double* sigma,
                           double* sigma_sum) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (n_omega < 0 || (n_omega > 0 && omega == nullptr) || !(eta > 0.0))
         return ctx->fail(GWL_EINVAL, "gwl_selfenergy: bad arguments (eta must be > 0)");
     if (ctx->run_steps == 0) return ctx->fail(GWL_ESTATE, "gwl_selfenergy: run gwl_lanczos first");
@@ -793,13 +864,8 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
             CK(ctx->theta.ensure((size_t)nch * L * 8, st));
             CK(ctx->wgt.ensure((size_t)nch * L * 8, st));
             CK(ctx->ritz_info.ensure((size_t)nch * 4, st));
-            // divide and conquer (parallel) when T_L fits one CTA's shared memory, else the sequential QL kernel;
-            // GWL_RITZ=ql forces the latter (A/B runs)
-            static const bool force_ql = [] {
-                const char* e = getenv("GWL_RITZ");
-                return e != nullptr && e[0] == 'q';
-            }();
-            if (ritz_dc_fits(L) && !force_ql)
+            // divide and conquer (parallel) when T_L fits one CTA's shared memory, else the sequential QL kernel
+            if (ritz_dc_fits(L))
                 CKL(7, launch_ritz_dc(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
                                   ctx->theta.as<double>(), ctx->wgt.as<double>(), ctx->ritz_info.as<int32_t>(), st));
             else
@@ -824,6 +890,7 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
 gwl_status gwl_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, int64_t block, int reorth,
                                 const double* omega, int64_t n_omega, double eta, double* sigma_mm) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (sigma_mm == nullptr || omega == nullptr || n_omega < 1)
         return ctx->fail(GWL_EINVAL, "gwl_selfenergy_state: bad arguments");
     const int n_orb = ctx->n_v + ctx->n_c;
@@ -838,6 +905,7 @@ gwl_status gwl_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, int6
 
 gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, double* sigma_x) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (n_states < 0 || (n_states > 0 && (m_idx == nullptr || sigma_x == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_exchange: bad arguments");
     if (!ctx->have_orb || !ctx->have_V) return ctx->fail(GWL_ESTATE, "gwl_exchange: orbitals and kernel must be set");
@@ -848,10 +916,12 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
     LaunchScope ls(ctx);
     cudaStream_t st = ctx->stream;
     const int chunk = std::min(ctx->n_v, 256);
-    gwl_status rs = ensure_workspace(ctx, chunk);
-    if (rs != GWL_OK) return rs;
     const int64_t ldm = ctx->n_mup;
     const int npart = vec_parts(ctx->n_mu);
+    // only what rho -> V rho -> dot touches: T, W and the V.T split-K partials (none of the N_vc-sized Casida buffers)
+    CK(ctx->T.ensure((size_t)chunk * ldm * 8, st));
+    CK(ctx->W.ensure((size_t)chunk * ldm * 8, st));
+    gwl_status rs = GWL_OK;
     // (v, m) index pairs of every rho_vm, state-major
     std::vector<int32_t> hv((size_t)n_states * ctx->n_v), hm((size_t)n_states * ctx->n_v);
     for (int64_t j = 0; j < n_states; ++j)
@@ -895,6 +965,7 @@ gwl_status gwl_qp_solve(gwl_ctx* ctx, int64_t n_states, const double* eps_m, con
                         const double* sigma_x, const double* sigma_c, const double* omega, int64_t n_omega,
                         double* e_qp, double* z_qp, int32_t* iters) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     if (n_states < 0 || n_omega < 2 || n_omega > (1 << 28))
         return ctx->fail(GWL_EINVAL, "gwl_qp_solve: need n_states >= 0 and n_omega >= 2");
     if (n_states == 0) return GWL_OK;
@@ -939,8 +1010,85 @@ gwl_status gwl_qp_solve(gwl_ctx* ctx, int64_t n_states, const double* eps_m, con
     return GWL_OK;
 }
 
+gwl_status gwl_spectrum_bounds(gwl_ctx* ctx, int64_t steps, double* lam_min, double* lam_max) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (steps < 2 || steps > 512 || lam_min == nullptr || lam_max == nullptr)
+        return ctx->fail(GWL_EINVAL, "gwl_spectrum_bounds: need 2 <= steps <= 512 and non-NULL outputs");
+    if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: orbitals, energies and kernel must be set");
+    cudaStream_t st = ctx->stream;
+    const int L = (int)std::min<int64_t>(steps, ctx->n_vc);
+    // one chain from a generic (counter-based pseudo-random) start vector, on the operator itself (never p_g)
+    {
+        LaunchScope ls(ctx);
+        CK(ctx->d_start.ensure((size_t)ctx->n_vc * 8, st));
+        CK(ctx->d_eps_n.ensure(8, st));
+        CK(ctx->d_sgn_n.ensure(4, st));
+        CKL(4, launch_fill_hash(ctx->d_start.as<double>(), ctx->n_vc, 0x9E3779B97F4A7C15ull, st));
+        const double e0 = 0.0;
+        const int32_t s0 = 1;
+        CK(cudaMemcpyAsync(ctx->d_eps_n.p, &e0, 8, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->d_sgn_n.p, &s0, 4, cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    ctx->chain_mode = 2;
+    ctx->n_chains_set = 1;
+    const int g_saved = ctx->g, ptr_saved = ctx->device_ptrs;
+    ctx->g = 0;
+    ctx->device_ptrs = 0;
+    std::vector<double> a(L), b(L);
+    double n2 = 0.0;
+    int32_t len = 0;
+    gwl_status rs = gwl_lanczos(ctx, 1, L, 1, 0, a.data(), b.data(), &n2, &len);
+    ctx->g = g_saved;
+    ctx->device_ptrs = ptr_saved;
+    ctx->chain_mode = 0;  // the probe chain is not the caller's chain list
+    ctx->n_chains_set = 0;
+    invalidate_run(ctx);
+    if (rs != GWL_OK) return rs;
+    if (len < 1) return ctx->fail(GWL_ECUDA, "gwl_spectrum_bounds: Lanczos broke down at the first step");
+    // Ritz values of T_len and, for the residual bound beta_len |s_len,i|, the LAST eigenvector components:
+    // those are the first components of the reversed tridiagonal (same QL kernel, second launch).
+    const int n = len;
+    std::vector<double> h(4 * (size_t)n, 0.0);  // a, b, reversed a, reversed b
+    for (int i = 0; i < n; ++i) {
+        h[i] = a[i];
+        h[n + i] = (i + 1 < n) ? b[i] : 0.0;
+        h[2 * n + i] = a[n - 1 - i];
+        h[3 * n + i] = (i + 1 < n) ? b[n - 2 - i] : 0.0;
+    }
+    LaunchScope ls(ctx);
+    CK(ctx->theta.ensure((size_t)4 * n * 8, st));
+    CK(ctx->wgt.ensure((size_t)4 * n * 8, st));
+    CK(ctx->ritz_info.ensure(16, st));
+    double* dT = ctx->theta.as<double>();  // [a | b | ra | rb]
+    double* dO = ctx->wgt.as<double>();    // [theta | w_first | theta_r | w_last]
+    const int32_t lens[2] = {n, n};
+    CK(cudaMemcpyAsync(dT, h.data(), (size_t)4 * n * 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctx->ritz_info.as<int32_t>() + 2, lens, 8, cudaMemcpyHostToDevice, st));
+    CKL(7, launch_ritz(dT, dT + n, ctx->ritz_info.as<int32_t>() + 2, n, 1, dO, dO + n, nullptr,
+                       ctx->ritz_info.as<int32_t>(), st));
+    CKL(7, launch_ritz(dT + 2 * n, dT + 3 * n, ctx->ritz_info.as<int32_t>() + 3, n, 1, dO + 2 * n, dO + 3 * n, nullptr,
+                       ctx->ritz_info.as<int32_t>() + 1, st));
+    std::vector<double> o(4 * (size_t)n);
+    CK(cudaMemcpyAsync(o.data(), dO, (size_t)4 * n * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    int imax = 0, imin = 0, rmax = 0, rmin = 0;
+    for (int i = 1; i < n; ++i) {
+        if (o[i] > o[imax]) imax = i;
+        if (o[i] < o[imin]) imin = i;
+        if (o[2 * n + i] > o[2 * n + rmax]) rmax = i;
+        if (o[2 * n + i] < o[2 * n + rmin]) rmin = i;
+    }
+    const double b_last = (len == L) ? b[n - 1] : 0.0;  // after a breakdown the Krylov space is invariant: exact
+    *lam_max = o[imax] + b_last * std::sqrt(std::max(o[3 * n + rmax], 0.0));
+    *lam_min = o[imin] - b_last * std::sqrt(std::max(o[3 * n + rmin], 0.0));
+    return GWL_OK;
+}
+
 gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total) {
     if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     CK(cudaStreamSynchronize(ctx->stream));
     double tm = 0.0, tv = 0.0;
     for (size_t i = 0; i + 2 < ctx->ev_used; i += 3) {
@@ -958,12 +1106,14 @@ gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, do
 
 gwl_status gwl_set_profiling(gwl_ctx* ctx, int level) {
     if (ctx == nullptr || level < 0 || level > 2) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     ctx->prof_level = level;
     return GWL_OK;
 }
 
 gwl_status gwl_get_kernel_times(gwl_ctx* ctx, double* ms, int64_t* count) {
     if (ctx == nullptr || ms == nullptr || count == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     CK(cudaStreamSynchronize(ctx->stream));
     for (int i = 0; i < GWL_N_KERNEL_CLASSES; ++i) {
         ms[i] = 0.0;
@@ -980,6 +1130,7 @@ gwl_status gwl_get_kernel_times(gwl_ctx* ctx, double* ms, int64_t* count) {
 
 gwl_status gwl_get_launch_count(gwl_ctx* ctx, int64_t* n_launches) {
     if (ctx == nullptr || n_launches == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
     *n_launches = ctx->launches;
     return GWL_OK;
 }

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <string>
 #include <vector>
 
@@ -21,7 +22,7 @@ static inline int64_t ceil_div(int64_t x, int64_t m) { return (x + m - 1) / m; }
 // with A = the matrix (Phi_c, V, Phi_c^T) and B = the block of vectors.
 // ---------------------------------------------------------------------------------------------
 enum GemmMode { MODE_FWD = 0, MODE_PLAIN = 1, MODE_BWD = 2 };
-enum GemmEpi { EPI_STORE = 0, EPI_CASIDA = 1, EPI_START = 2 };
+enum GemmEpi { EPI_STORE = 0, EPI_CASIDA = 1, EPI_START = 2, EPI_CHEB = 3 };
 
 struct GemmParams {
     const double* A;      // [M][lda]
@@ -46,15 +47,24 @@ struct GemmParams {
     double* dotpart;      // CASIDA: sum_m x*y, START: sum_m p*p ; dotpart[n*dot_stride + v*gridDim.x + blockIdx.x]
     int dot_stride;
     int n_c;
+    // EPI_CHEB: one term of the Chebyshev recurrence of p_g(C) fused behind the Casida epilogue:
+    //   y = d2 x + coupling s u;  t = ca y + cb x + cc t0;  w = first ? c0 x + cw t : w + cw t;
+    //   out = t, xs_out = s o t (padded layout, the next K.X operand), dotpart = sum q w (last term only).
+    // x, t0, w, q and out share ldx; t0 may alias out (every element is read and written by the same thread).
+    const double* T0;     // t_{j-2} or NULL (then cc is ignored)
+    double* Wacc;         // running sum p_g(C) q
+    const double* Q;      // Lanczos vector for the alpha dots, or NULL
+    double* xs_out;       // [N][n_v][n_cp] or NULL
+    int64_t ldxs;
+    int n_cp;
+    double ca, cb, cc, cw, c0;
+    int first;
     // BWD (persistent stream-K grid, kr_gemm.cu): tile grid, partial-tile workspace and hand-over flags
     int tiles_m, tiles_n, n_tiles;  // filled by launch_gemm
     double* ws;                     // [grid][BM*BN] partial accumulators, >= gemm_bwd_ws_bytes()
     unsigned* flags;                // [grid], flags[cta] == epoch once that CTA's partial of THIS launch is visible
     unsigned epoch;                 // differs from every earlier launch that used the same flags (never 0)
     int n_sm;
-#ifdef GWL_TRACE
-    unsigned long long* trace;  // development builds only
-#endif
 };
 
 struct GemmPlan {
@@ -80,6 +90,8 @@ int vec_parts(int64_t n_vc);  // number of partial-sum blocks per column used by
 // tda = 0: d2 = Delta^2, s = sqrt(Delta);  tda = 1: d2 = Delta, s = 1
 cudaError_t launch_build_delta(const double* eps_v, const double* eps_c, int n_v, int n_c, double* d2, double* s,
                                int tda, cudaStream_t st);
+// x[i] = pseudo-random uniform in [-1, 1), a function of (seed, i) only
+cudaError_t launch_fill_hash(double* x, int64_t n, unsigned long long seed, cudaStream_t st);
 // xs[b][v][c_pad] = s[vc] * x[b][vc] * (colscale ? colscale[b] : 1)
 cudaError_t launch_prescale(const double* x, int64_t ldx, double* xs, int64_t ldxs, const double* s, int n_v, int n_c,
                             int n_cp, int nb, cudaStream_t st);
@@ -129,9 +141,6 @@ cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nsl
                                int nb, double* coefpart, int npart, cudaStream_t st);
 cudaError_t launch_reorth_apply(const double* basis, int64_t slot_stride, int nslots, double* w, int64_t n_vc, int nb,
                                 const double* coefpart, int npart, double* normpart, cudaStream_t st);
-// out = a*x + b*y + c*z (any of y,z may be NULL), uniform scalars, n elements per column
-cudaError_t launch_axpby3(double* out, double a, const double* x, double b, const double* y, double c, const double* z,
-                          int64_t n_total, cudaStream_t st);
 
 // ---------------------------------------------------------------------------------------------
 // Spectral kernels (spectral_kernels.cu): Eq. 14, Ritz pairs of T_L, Eq. 11 / Eq. 12, Eq. 10.
@@ -172,13 +181,12 @@ cudaError_t probe_fp64_peak(int kind, double* tflops);
 // prologue (mbarrier init, tensor-map prefetch, index arithmetic), while the previous kernel drains; pdl_wait()
 // then blocks until every earlier kernel of the stream has completed and its writes are visible.  EVERY kernel
 // launched through launch_pdl() calls pdl_trigger(); pdl_wait(); in all threads before it touches global memory
-// (that also makes the ordering transitive along the stream).  GWL_NO_PDL=1 (read once) launches plainly.
+// (that also makes the ordering transitive along the stream).
 // ---------------------------------------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
 #endif
-bool pdl_enabled();
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
                               unsigned cluster_x, Args... args) {
@@ -189,11 +197,9 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
     cfg.stream = st;
     cudaLaunchAttribute attr[2];
     unsigned n = 0;
-    if (pdl_enabled()) {
-        attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[n].val.programmaticStreamSerializationAllowed = 1;
-        ++n;
-    }
+    attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[n].val.programmaticStreamSerializationAllowed = 1;
+    ++n;
     if (cluster_x > 1) {
         attr[n].id = cudaLaunchAttributeClusterDimension;
         attr[n].val.clusterDim.x = cluster_x;
@@ -204,6 +210,37 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
     cfg.attrs = attr;
     cfg.numAttrs = n;
     return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of a function ON a device: one instance of this per
+// kernel remembers, per device, the largest size already configured (contexts on several GPUs in one process).
+struct SmemAttr {
+    std::atomic<size_t> configured[64] = {};
+    template <class K>
+    cudaError_t ensure(K kern, size_t bytes) {
+        if (bytes <= 48 * 1024) return cudaSuccess;
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        if (dev < 0 || dev >= 64) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (configured[dev].load(std::memory_order_relaxed) >= bytes) return cudaSuccess;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e == cudaSuccess) configured[dev].store(bytes, std::memory_order_relaxed);
+        return e;
+    }
+};
+
+// SM count of the current device (cached per device); grids of the streaming kernels are sized from it.
+inline int device_sm_count() {
+    static std::atomic<int> cached[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    int n = cached[dev].load(std::memory_order_relaxed);
+    if (n == 0) {
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        cached[dev].store(n, std::memory_order_relaxed);
+    }
+    return n;
 }
 
 // Every launch_* bumps this counter once per kernel launched (read by gwl_get_launch_count).

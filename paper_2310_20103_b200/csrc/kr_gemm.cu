@@ -20,35 +20,6 @@ namespace gwl {
 
 thread_local int64_t* g_launch_counter = nullptr;
 
-bool pdl_enabled() {
-    static int v = -1;
-    if (v < 0) {
-        const char* e = getenv("GWL_NO_PDL");
-        v = (e != nullptr && e[0] == '1') ? 0 : 1;
-    }
-    return v != 0;
-}
-
-#ifdef GWL_TRACE
-// Development builds only (-DGWL_TRACE): per-CTA %globaltimer stamps at entry / first tile landed / main loop done /
-// epilogue done, 4 x (globaltimer, clock64) = 8 x uint64 per CTA, written to a caller-provided device buffer.
-unsigned long long* g_trace_buf = nullptr;
-extern "C" void gwl_debug_set_trace(unsigned long long* dev_buf) { g_trace_buf = dev_buf; }
-#define GWL_STAMP(slot)                                                                            \
-    do {                                                                                           \
-        if (p.trace != nullptr && (tid & 31) == 0 && warp == 0) {                                  \
-            unsigned long long t__;                                                                \
-            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));                                \
-            p.trace[8 * ((blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) + slot] = t__; \
-            p.trace[8 * ((blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) + 4 + slot] = clock64(); \
-        }                                                                                          \
-    } while (0)
-#else
-#define GWL_STAMP(slot) \
-    do {                \
-    } while (0)
-#endif
-
 namespace {
 
 // ---- TMA / mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS) ---------------------------------
@@ -191,7 +162,6 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             m0 = (r / p.tiles_n) * BM;
         }
     };
-    GWL_STAMP(0);
 
     if (tid == 0) {
         tma_prefetch_desc(&tmA);
@@ -320,7 +290,6 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             }
             fetch(slot, 0, fa[0], fb[0]);
         }
-        if (si == 0) GWL_STAMP(1);
         for (int j = 0; j < nkt; ++j, ++it) {
             const int slot = it % STAGES;
             const int nslot = (it + 1) % STAGES;
@@ -343,7 +312,6 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_bar(slot));
         }
-        if (si == ns - 1) GWL_STAMP(2);
 
         // ---- epilogue ------------------------------------------------------------------------------
         // acc[i][j][e]: row m = m0 + rowA[i] (i even/odd = adjacent rows), col n = n0 + wn*WN + 16*(j>>1) + 2*(2q+e) + (j&1)
@@ -412,6 +380,116 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                 }
             }
             const int64_t voff = (int64_t)z * p.n_c;
+            if (EPI == EPI_CHEB) {
+                // ---- one Chebyshev term of p_g(C): t = ca (C x) + cb x + cc t0, w += cw t, xs = s o t, dots q.w -------
+                const bool vec2 = ((voff & 1) == 0) && ((p.ldx & 1) == 0) &&
+                                  (((reinterpret_cast<uintptr_t>(p.X) | reinterpret_cast<uintptr_t>(p.out) |
+                                     reinterpret_cast<uintptr_t>(p.Wacc) | reinterpret_cast<uintptr_t>(p.T0) |
+                                     reinterpret_cast<uintptr_t>(p.Q)) & 15) == 0);
+                const bool has_t0 = p.T0 != nullptr, has_q = p.Q != nullptr, first = p.first != 0;
+                const double cpl = p.coupling, ca = p.ca, cb = p.cb, cc = p.cc, cw = p.cw, c0 = p.c0;
+                double part[FN][2];
+#pragma unroll
+                for (int j = 0; j < FN; ++j) part[j][0] = part[j][1] = 0.0;
+                auto ld2 = [&](const double* ptr, bool two, double& a, double& b) {
+                    if (vec2 && two) {
+                        const double2 v2 = *reinterpret_cast<const double2*>(ptr);
+                        a = v2.x;
+                        b = v2.y;
+                    } else {
+                        a = ptr[0];
+                        b = two ? ptr[1] : 0.0;
+                    }
+                };
+                auto st2 = [&](double* ptr, bool two, double a, double b) {
+                    if (vec2 && two) {
+                        *reinterpret_cast<double2*>(ptr) = make_double2(a, b);
+                    } else {
+                        ptr[0] = a;
+                        if (two) ptr[1] = b;
+                    }
+                };
+#pragma unroll
+                for (int i2 = 0; i2 < FM / 2; ++i2) {
+                    const int r0 = m0 + wm * WM + 16 * i2 + 2 * g;
+                    if (r0 >= p.M) continue;
+                    const bool two = (r0 + 1 < p.M);
+                    const double s0 = p.s[voff + r0], s1 = two ? p.s[voff + r0 + 1] : 0.0;
+                    const double d0 = p.d2[voff + r0], d1 = two ? p.d2[voff + r0 + 1] : 0.0;
+                    constexpr int JB = 2;  // columns whose loads are in flight together (3-4 streams of 16 bytes each)
+#pragma unroll
+                    for (int j0 = 0; j0 < FN; j0 += JB) {
+                        double xr[JB][2][2], tr[JB][2][2], wr[JB][2][2], qr[JB][2][2];
+#pragma unroll
+                        for (int jj = 0; jj < JB; ++jj)
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                const int j = j0 + jj;
+                                const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
+                                xr[jj][e][0] = xr[jj][e][1] = tr[jj][e][0] = tr[jj][e][1] = 0.0;
+                                wr[jj][e][0] = wr[jj][e][1] = qr[jj][e][0] = qr[jj][e][1] = 0.0;
+                                if (n >= p.N) continue;
+                                const int64_t off = (int64_t)n * p.ldx + voff + r0;
+                                ld2(p.X + off, two, xr[jj][e][0], xr[jj][e][1]);
+                                if (has_t0) ld2(p.T0 + off, two, tr[jj][e][0], tr[jj][e][1]);
+                                if (!first) ld2(p.Wacc + off, two, wr[jj][e][0], wr[jj][e][1]);
+                                if (has_q) ld2(p.Q + off, two, qr[jj][e][0], qr[jj][e][1]);
+                            }
+#pragma unroll
+                        for (int jj = 0; jj < JB; ++jj)
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                const int j = j0 + jj;
+                                const int n = n0 + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1);
+                                if (n >= p.N) continue;
+                                const double x0 = xr[jj][e][0], x1 = xr[jj][e][1];
+                                const double y0 = d0 * x0 + cpl * (s0 * acc[2 * i2][j][e]);
+                                const double y1 = d1 * x1 + cpl * (s1 * acc[2 * i2 + 1][j][e]);
+                                double t0v = ca * y0 + cb * x0, t1v = ca * y1 + cb * x1;
+                                if (has_t0) {
+                                    t0v += cc * tr[jj][e][0];
+                                    t1v += cc * tr[jj][e][1];
+                                }
+                                const double w0 = first ? c0 * x0 + cw * t0v : wr[jj][e][0] + cw * t0v;
+                                const double w1 = first ? c0 * x1 + cw * t1v : wr[jj][e][1] + cw * t1v;
+                                const int64_t off = (int64_t)n * p.ldx + voff + r0;
+                                st2(p.Wacc + off, two, w0, w1);
+                                if (p.xs_out != nullptr) {  // not the last term: t and its scaled copy feed the next one
+                                    st2(p.out + off, two, t0v, t1v);
+                                    // n_cp is a multiple of 16 and r0 is even: always 16-byte aligned
+                                    double* xp = p.xs_out + (int64_t)n * p.ldxs + (int64_t)z * p.n_cp + r0;
+                                    if (two) {
+                                        *reinterpret_cast<double2*>(xp) = make_double2(s0 * t0v, s1 * t1v);
+                                    } else {
+                                        xp[0] = s0 * t0v;
+                                    }
+                                }
+                                if (has_q) part[j][e] += qr[jj][e][0] * w0 + qr[jj][e][1] * w1;
+                            }
+                    }
+                }
+                if (p.dotpart != nullptr && has_q) {
+                    asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
+#pragma unroll
+                    for (int j = 0; j < FN; ++j)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            double vsum = part[j][e];
+                            vsum += __shfl_xor_sync(0xffffffffu, vsum, 4);
+                            vsum += __shfl_xor_sync(0xffffffffu, vsum, 8);
+                            vsum += __shfl_xor_sync(0xffffffffu, vsum, 16);
+                            if (g == 0) red[wm * BN + wn * WN + 16 * (j >> 1) + 2 * (2 * q + e) + (j & 1)] = vsum;
+                        }
+                    asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
+                    if (tid < BN && n0 + tid < p.N) {
+                        double ssum = 0.0;
+#pragma unroll
+                        for (int w = 0; w < WGM; ++w) ssum += red[w * BN + tid];
+                        p.dotpart[(int64_t)(n0 + tid) * p.dot_stride + (int64_t)z * p.tiles_m + m0 / BM] = ssum;
+                    }
+                }
+                continue;
+            }
             const bool vec_ok = ((voff & 1) == 0) && ((p.ldo & 1) == 0) && ((p.ldx & 1) == 0) &&
                                 ((reinterpret_cast<uintptr_t>(p.out) & 15) == 0) &&
                                 (EPI == EPI_START || (reinterpret_cast<uintptr_t>(p.X) & 15) == 0);
@@ -509,7 +587,6 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             }
         }
     }
-    GWL_STAMP(3);
 }
 
 using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -552,12 +629,9 @@ cudaError_t launch_one(const GemmParams& p, dim3 grid, cudaStream_t st) {
     constexpr int NTHREADS = ((BM / WM) * (BN / WN) + 4) * 32;
     static_assert(SMEM <= 227 * 1024, "stage ring does not fit in shared memory");
     auto kern = gemm_tn_dmma<BM, BN, WM, WN, STAGES, MODE, EPI, CREGS>;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static SmemAttr attr;  // per device (the attribute is a property of the function ON a device)
+    cudaError_t ea = attr.ensure(kern, SMEM);
+    if (ea != cudaSuccess) return ea;
     CUtensorMap tmA, tmB, tmS;
     const uint64_t kcols = (uint64_t)p.kt_total * BK;
     const uint64_t a_cols = MODE == MODE_FWD ? (uint64_t)p.a_wrap * BK : kcols;
@@ -572,27 +646,9 @@ cudaError_t launch_one(const GemmParams& p, dim3 grid, cudaStream_t st) {
     else
         tmS = tmA;
     if (e != cudaSuccess) return e;
-#ifdef GWL_TRACE
-    GemmParams pt = p;
-    pt.trace = g_trace_buf;
-    if (g_trace_buf != nullptr) g_trace_buf += 8ull * grid.x * grid.y * grid.z;  // consecutive launches, consecutive records
-    cudaError_t le = launch_pdl(kern, grid, dim3(NTHREADS), SMEM, st, 1u, pt, tmA, tmB, tmS);
-#else
     cudaError_t le = launch_pdl(kern, grid, dim3(NTHREADS), SMEM, st, 1u, p, tmA, tmB, tmS);
-#endif
     count_launch();
     return le != cudaSuccess ? le : cudaGetLastError();
-}
-
-// Tile variants.  bn = 128: wide blocks (configs 2-4); bn = 64: narrow blocks (configs 0-1).
-// GWL_GEMM_VARIANT (development knob, read once) selects alternative instantiations for sweeps.
-int gemm_variant() {
-    static int v = -1;
-    if (v < 0) {
-        const char* e = getenv("GWL_GEMM_VARIANT");
-        v = e ? atoi(e) : 0;
-    }
-    return v;
 }
 
 // BWD grid: one CTA per SM, fewer only when the whole product has too few k-tiles to be worth cutting
@@ -613,21 +669,10 @@ cudaError_t launch_mode(const GemmPlan& plan, const GemmParams& p0, int nz, cuda
         if (p.ws == nullptr || p.flags == nullptr || p.epoch == 0 || p.n_sm <= 0) return cudaErrorInvalidValue;
         grid = dim3((unsigned)bwd_grid(p.n_tiles, p.kt_total, p.n_sm), 1, 1);
     }
-    const int var = gemm_variant();
-    if (plan.bn == 128) {
-        switch (var) {
-            case 1: return launch_one<128, 128, 32, 32, 4, MODE, EPI, 104>(p, grid, st);  // 16 consumer warps
-            case 2: return launch_one<128, 128, 32, 64, 6, MODE, EPI, 232>(p, grid, st);
-            case 3: return launch_one<128, 128, 64, 32, 4, MODE, EPI, 232>(p, grid, st);
-            default: return launch_one<128, 128, 32, 64, 4, MODE, EPI, 232>(p, grid, st);
-        }
-    }
-    switch (var) {
-        case 1: return launch_one<128, 64, 32, 16, 4, MODE, EPI, 104>(p, grid, st);  // 16 consumer warps
-        case 2: return launch_one<128, 64, 32, 32, 8, MODE, EPI, 168>(p, grid, st);
-        case 3: return launch_one<128, 64, 16, 64, 4, MODE, EPI, 168>(p, grid, st);
-        default: return launch_one<128, 64, 32, 32, 4, MODE, EPI, 168>(p, grid, st);
-    }
+    // bn = 128: wide blocks (configs 2-4); bn = 64: narrow blocks (configs 0-1).  Other warp tilings were measured in
+    // round 1 (16 consumer warps of 32x32 / 32x16, 64x32 warp tiles, 6- and 8-stage rings) and were slower.
+    if (plan.bn == 128) return launch_one<128, 128, 32, 64, 4, MODE, EPI, 232>(p, grid, st);
+    return launch_one<128, 64, 32, 32, 4, MODE, EPI, 168>(p, grid, st);
 }
 
 }  // namespace
@@ -670,6 +715,7 @@ cudaError_t launch_gemm(int mode, int epi, const GemmPlan& plan, const GemmParam
     if (mode == MODE_PLAIN && epi == EPI_STORE) return launch_mode<MODE_PLAIN, EPI_STORE>(plan, p, nz, st);
     if (mode == MODE_BWD && epi == EPI_CASIDA) return launch_mode<MODE_BWD, EPI_CASIDA>(plan, p, nz, st);
     if (mode == MODE_BWD && epi == EPI_START) return launch_mode<MODE_BWD, EPI_START>(plan, p, nz, st);
+    if (mode == MODE_BWD && epi == EPI_CHEB) return launch_mode<MODE_BWD, EPI_CHEB>(plan, p, nz, st);
     return cudaErrorInvalidValue;
 }
 

@@ -385,12 +385,9 @@ cudaError_t launch_ritz_dc(const double* alpha, const double* beta, const int32_
                            double* theta, double* wgt, int32_t* info, cudaStream_t st) {
     if (n_chains <= 0) return cudaSuccess;
     const size_t sm = ritz_dc_smem_bytes(steps);
-    static size_t configured = 0;
-    if (sm > 48 * 1024 && sm > configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_ritz_dc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        if (e != cudaSuccess) return e;
-        configured = sm;
-    }
+    static SmemAttr attr;
+    cudaError_t ea = attr.ensure(k_ritz_dc, sm);
+    if (ea != cudaSuccess) return ea;
     k_ritz_dc<<<(unsigned)n_chains, RT, sm, st>>>(alpha, beta, len, steps, theta, wgt, info);
     count_launch();
     return cudaGetLastError();

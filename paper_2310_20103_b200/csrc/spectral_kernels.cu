@@ -1,6 +1,8 @@
 // Resolvent and self-energy kernels: Haydock continued fraction (Eq. 14), Ritz pairs of the
 // Lanczos tridiagonal T_L (Eq. 13), Sigma^corr(omega, n) by Eq. 11 (direct mode) or Eq. 12 + Eq. 14 (poly
 // mode), and the sum over chains (Eq. 10).  Complex FP64 on the plain FP64 ALUs; tiny next to the GEMMs.
+#include <algorithm>
+
 #include "gwl_internal.h"
 
 namespace gwl {
@@ -279,12 +281,18 @@ __global__ void k_qp_solve(int n_states, const double* __restrict__ eps_m, const
 
 }  // namespace
 
+constexpr int MAX_GRID_Y = 65535;  // chains go to grid.y: longer lists are cut into launches of at most this many
+
 cudaError_t launch_contfrac(const double* alpha, const double* beta, const double* norm2, const int32_t* len, int steps,
                             int n_chains, const double* zeta, int n_zeta, double* r, cudaStream_t st) {
     if (n_chains <= 0 || n_zeta <= 0) return cudaSuccess;
-    dim3 grid((unsigned)ceil_div(n_zeta, 128), (unsigned)n_chains);
-    k_contfrac<<<grid, 128, 0, st>>>(alpha, beta, norm2, len, steps, zeta, n_zeta, r);
-    count_launch();
+    for (int j0 = 0; j0 < n_chains; j0 += MAX_GRID_Y) {
+        const int nc = std::min(MAX_GRID_Y, n_chains - j0);
+        dim3 grid((unsigned)ceil_div(n_zeta, 128), (unsigned)nc);
+        k_contfrac<<<grid, 128, 0, st>>>(alpha + (int64_t)j0 * steps, beta + (int64_t)j0 * steps, norm2 + j0, len + j0, steps,
+                                         zeta, n_zeta, r + (int64_t)j0 * n_zeta * 2);
+        count_launch();
+    }
     return cudaGetLastError();
 }
 
@@ -293,10 +301,9 @@ cudaError_t launch_ritz(const double* alpha, const double* beta, const int32_t* 
     (void)work;
     if (n_chains <= 0) return cudaSuccess;
     const size_t sm = (size_t)3 * steps * sizeof(double);
-    if (sm > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(k_ritz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        if (e != cudaSuccess) return e;
-    }
+    static SmemAttr attr;
+    cudaError_t ea = attr.ensure(k_ritz, sm);
+    if (ea != cudaSuccess) return ea;
     k_ritz<<<(unsigned)n_chains, 32, sm, st>>>(alpha, beta, len, steps, theta, wgt, info);
     count_launch();
     return cudaGetLastError();
@@ -307,13 +314,16 @@ cudaError_t launch_sigma_direct(const double* theta, const double* wgt, const do
                                 const double* omega, int n_omega, double eta, double* sigma, cudaStream_t st) {
     if (n_chains <= 0 || n_omega <= 0) return cudaSuccess;
     const size_t sm = (size_t)2 * steps * sizeof(double);
-    if (sm > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(k_sigma_direct, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        if (e != cudaSuccess) return e;
+    static SmemAttr attr;
+    cudaError_t ea = attr.ensure(k_sigma_direct, sm);
+    if (ea != cudaSuccess) return ea;
+    for (int j0 = 0; j0 < n_chains; j0 += MAX_GRID_Y) {
+        const int nc = std::min(MAX_GRID_Y, n_chains - j0);
+        dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)nc);
+        k_sigma_direct<<<grid, 128, sm, st>>>(theta + (int64_t)j0 * steps, wgt + (int64_t)j0 * steps, norm2 + j0, len + j0, steps,
+                                              eps_n + j0, sgn_n + j0, omega, n_omega, eta, sigma + (int64_t)j0 * n_omega * 2);
+        count_launch();
     }
-    dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)n_chains);
-    k_sigma_direct<<<grid, 128, sm, st>>>(theta, wgt, norm2, len, steps, eps_n, sgn_n, omega, n_omega, eta, sigma);
-    count_launch();
     return cudaGetLastError();
 }
 
@@ -321,9 +331,13 @@ cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const dou
                               int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
                               int n_omega, double eta, double* sigma, cudaStream_t st) {
     if (n_chains <= 0 || n_omega <= 0) return cudaSuccess;
-    dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)n_chains);
-    k_sigma_poly<<<grid, 128, 0, st>>>(alpha, beta, norm2, len, steps, eps_n, sgn_n, omega, n_omega, eta, sigma);
-    count_launch();
+    for (int j0 = 0; j0 < n_chains; j0 += MAX_GRID_Y) {
+        const int nc = std::min(MAX_GRID_Y, n_chains - j0);
+        dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)nc);
+        k_sigma_poly<<<grid, 128, 0, st>>>(alpha + (int64_t)j0 * steps, beta + (int64_t)j0 * steps, norm2 + j0, len + j0, steps,
+                                  eps_n + j0, sgn_n + j0, omega, n_omega, eta, sigma + (int64_t)j0 * n_omega * 2);
+        count_launch();
+    }
     return cudaGetLastError();
 }
 
@@ -331,9 +345,13 @@ cudaError_t launch_sigma_tda(const double* alpha, const double* beta, const doub
                              int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
                              int n_omega, double eta, double* sigma, cudaStream_t st) {
     if (n_chains <= 0 || n_omega <= 0) return cudaSuccess;
-    dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)n_chains);
-    k_sigma_tda<<<grid, 128, 0, st>>>(alpha, beta, norm2, len, steps, eps_n, sgn_n, omega, n_omega, eta, sigma);
-    count_launch();
+    for (int j0 = 0; j0 < n_chains; j0 += MAX_GRID_Y) {
+        const int nc = std::min(MAX_GRID_Y, n_chains - j0);
+        dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)nc);
+        k_sigma_tda<<<grid, 128, 0, st>>>(alpha + (int64_t)j0 * steps, beta + (int64_t)j0 * steps, norm2 + j0, len + j0, steps,
+                                  eps_n + j0, sgn_n + j0, omega, n_omega, eta, sigma + (int64_t)j0 * n_omega * 2);
+        count_launch();
+    }
     return cudaGetLastError();
 }
 

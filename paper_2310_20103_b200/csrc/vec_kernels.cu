@@ -468,21 +468,20 @@ __global__ void __launch_bounds__(NT) k_reorth_apply(const double* __restrict__ 
     }
 }
 
-__global__ void k_axpby3(double* __restrict__ out, double a, const double* __restrict__ x, double b,
-                         const double* __restrict__ y, double c, const double* __restrict__ z, int64_t n) {
-    pdl_trigger();
-    pdl_wait();
+// x[i] = uniform in [-1, 1) from a counter-based hash (splitmix64 finaliser) of (seed, i): a generic start vector
+__global__ void k_fill_hash(double* __restrict__ x, int64_t n, unsigned long long seed) {
     for (int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x; i < n; i += (int64_t)gridDim.x * NT) {
-        double v = a * x[i];
-        if (y != nullptr) v += b * y[i];
-        if (z != nullptr) v += c * z[i];
-        out[i] = v;
+        unsigned long long z = seed + 0x9E3779B97F4A7C15ull * (unsigned long long)(i + 1);
+        z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+        z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+        z ^= z >> 31;
+        x[i] = (double)(z >> 11) * (2.0 / 9007199254740992.0) - 1.0;
     }
 }
 
 inline unsigned grid1d(int64_t n, int per_thread = 4) {
     int64_t g = ceil_div(n, (int64_t)NT * per_thread);
-    return (unsigned)std::max<int64_t>(1, std::min<int64_t>(g, 148 * 32));
+    return (unsigned)std::max<int64_t>(1, std::min<int64_t>(g, (int64_t)device_sm_count() * 32));
 }
 
 }  // namespace
@@ -492,6 +491,12 @@ int vec_parts(int64_t n_vc) { return (int)std::max<int64_t>(1, std::min<int64_t>
 cudaError_t launch_build_delta(const double* eps_v, const double* eps_c, int n_v, int n_c, double* d2, double* s,
                                int tda, cudaStream_t st) {
     k_build_delta<<<grid1d((int64_t)n_v * n_c, 1), NT, 0, st>>>(eps_v, eps_c, n_v, n_c, d2, s, tda);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fill_hash(double* x, int64_t n, unsigned long long seed, cudaStream_t st) {
+    k_fill_hash<<<grid1d(n), NT, 0, st>>>(x, n, seed);
     count_launch();
     return cudaGetLastError();
 }
@@ -604,12 +609,9 @@ cudaError_t launch_reorth_dots(const double* basis, int64_t slot_stride, int nsl
     if (npart != reorth_parts(n_vc)) return cudaErrorInvalidValue;
     const int64_t slice = reorth_slice(n_vc);
     const size_t sm = (size_t)(RSLICE + nslots) * sizeof(double);
-    static size_t configured = 0;
-    if (sm > 48 * 1024 && sm > configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_reorth_dots, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        if (e != cudaSuccess) return e;
-        configured = sm;
-    }
+    static SmemAttr attr;
+    cudaError_t ea = attr.ensure(k_reorth_dots, sm);
+    if (ea != cudaSuccess) return ea;
     cudaError_t le = launch_pdl(k_reorth_dots, dim3((unsigned)npart, (unsigned)nb), dim3(NT), sm, st, 1u, basis,
                                 slot_stride, nslots, w, n_vc, coefpart, npart, slice);
     count_launch();
@@ -620,21 +622,11 @@ cudaError_t launch_reorth_apply(const double* basis, int64_t slot_stride, int ns
                                 const double* coefpart, int npart, double* normpart, cudaStream_t st) {
     if (npart != reorth_parts(n_vc)) return cudaErrorInvalidValue;
     const size_t sm = (size_t)(nslots + NT / 32 + 1) * sizeof(double);
-    static size_t configured = 0;
-    if (sm > 48 * 1024 && sm > configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_reorth_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        if (e != cudaSuccess) return e;
-        configured = sm;
-    }
+    static SmemAttr attr;
+    cudaError_t ea = attr.ensure(k_reorth_apply, sm);
+    if (ea != cudaSuccess) return ea;
     cudaError_t le = launch_pdl(k_reorth_apply, dim3((unsigned)npart, (unsigned)nb), dim3(NT), sm, st, 1u, basis,
                                 slot_stride, nslots, w, n_vc, coefpart, npart, normpart, reorth_slice(n_vc));
-    count_launch();
-    return le != cudaSuccess ? le : cudaGetLastError();
-}
-
-cudaError_t launch_axpby3(double* out, double a, const double* x, double b, const double* y, double c, const double* z,
-                          int64_t n_total, cudaStream_t st) {
-    cudaError_t le = launch_pdl(k_axpby3, dim3(grid1d(n_total)), dim3(NT), (size_t)(0), st, 1u, out, a, x, b, y, c, z, n_total);
     count_launch();
     return le != cudaSuccess ? le : cudaGetLastError();
 }

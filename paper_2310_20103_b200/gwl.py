@@ -32,6 +32,7 @@ SIGNATURES = {
     "gwl_set_kernel": (c_int, [c_void_p, c_void_p]),
     "gwl_set_polynomial": (c_int, [c_void_p, c_int, c_void_p, c_double, c_double]),
     "gwl_set_approximation": (c_int, [c_void_p, c_int]),
+    "gwl_spectrum_bounds": (c_int, [c_void_p, c_int64, POINTER(c_double), POINTER(c_double)]),
     "gwl_casida_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
     "gwl_set_chains": (c_int, [c_void_p, c_int64, c_void_p, c_void_p]),
     "gwl_set_start_vectors": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p]),
@@ -180,6 +181,12 @@ class Context:
     def set_approximation(self, approximation: int):
         """0 = RPA (operator C, default), 1 = Tamm-Dancoff (operator A)."""
         self._ck(self._lib.gwl_set_approximation(self._h, int(approximation)))
+
+    def spectrum_bounds(self, steps: int = 40):
+        """(lam_min, lam_max) estimates of the operator's spectrum from a short Lanczos run."""
+        lo, hi = c_double(), c_double()
+        self._ck(self._lib.gwl_spectrum_bounds(self._h, int(steps), byref(lo), byref(hi)))
+        return lo.value, hi.value
 
     # -- the path ---------------------------------------------------------------------------------
     def casida_matvec(self, x, y=None):

@@ -12,10 +12,26 @@ import numpy as np
 
 
 def default_range(eps_v, eps_c):
-    """[0.8 min Delta^2, 1.25 max Delta^2], Delta = eps_c - eps_v (PAPER.md:284 with reading Q12)."""
+    """The paper's heuristic [0.8 min Delta^2, 1.25 max Delta^2], Delta = eps_c - eps_v (PAPER.md:284 with reading
+    Q12).  Its upper end is NOT a bound on lambda_max(C) once the coupling 2 sqrt(Delta) K^T V K sqrt(Delta) is
+    strong (config 2: lambda_max ~ 2321 eV^2 against 1.25 max Delta^2 = 1125): outside [lo, hi] a Chebyshev fit
+    diverges.  Use range_from_spectrum unless the spectrum is known to lie inside."""
     d_min = float(np.min(eps_c) - np.max(eps_v))
     d_max = float(np.max(eps_c) - np.min(eps_v))
     return 0.8 * d_min * d_min, 1.25 * d_max * d_max
+
+
+def range_from_spectrum(ctx, eps_v, eps_c, steps: int = 40, margin: float = 0.02):
+    """Fitting range from the operator itself, "One can use standard Lanczos algorithm to determine the extremal
+    eigenvalues min(Omega_s^2) and max(Omega_s^2) of C": hi = (1 + margin) x the Lanczos upper bound of
+    gwl_spectrum_bounds (top Ritz value + its residual), never below the heuristic 1.25 max Delta^2 ... no: never
+    below max Delta^2 (a diagonal entry of C - its coupling part is positive semidefinite - bounds lambda_max from
+    below); lo = the paper's 0.8 min Delta^2, which IS a lower bound of C whenever V is positive semidefinite
+    (C - diag(Delta^2) is then positive semidefinite).  Call before the chain list is set (the probe replaces it)."""
+    d_min = float(np.min(eps_c) - np.max(eps_v))
+    d_max = float(np.max(eps_c) - np.min(eps_v))
+    _, lam_max = ctx.spectrum_bounds(steps)
+    return 0.8 * d_min * d_min, (1.0 + margin) * max(lam_max, d_max * d_max)
 
 
 def sqrt_chebyshev(g: int, lo: float, hi: float, nodes_per_coefficient: int = 4) -> np.ndarray:

@@ -137,3 +137,67 @@ def random_block(cfg: Config, nvec: int, seed: int = 1) -> np.ndarray:
     """A seeded block of test vectors X[nvec][n_v][n_c] ~ N(0,1)."""
     rng = np.random.default_rng(seed)
     return rng.standard_normal((nvec, cfg.n_v, cfg.n_c))
+
+
+# ---------------------------------------------------------------------------------------------
+# SURVEY.md §8(f)-3: complex-orbital (periodic) Tamm-Dancoff variant, PAPER.md:157, :286-313.
+# Stand-ins for Bloch orbitals at N_k k-points and ONE transferred momentum q: complex Gaussians of the same
+# normalisation as the real configs; the conduction set is the one already shifted by q (psi_{c k+q}).
+# ---------------------------------------------------------------------------------------------
+@dataclass
+class PeriodicProblem:
+    n_k: int
+    n_v: int
+    n_c: int
+    n_mu: int
+    r: np.ndarray          # [n_mu, 3]
+    psi_v: np.ndarray      # [n_k, n_mu, n_v] complex128   psi_{v k}(r_mu)
+    psi_cq: np.ndarray     # [n_k, n_mu, n_c] complex128   psi_{c k+q}(r_mu)
+    eps_v: np.ndarray      # [n_k, n_v]
+    eps_cq: np.ndarray     # [n_k, n_c]
+    omega: np.ndarray      # [n_omega]
+    chains: np.ndarray     # [n_chains, 4] int32: (k slot of n, n index, k slot of m, m index)
+    eta: float = 0.1
+    _V: np.ndarray | None = field(default=None, repr=False)
+
+    @property
+    def V(self) -> np.ndarray:
+        if self._V is None:
+            self._V = coulomb_kernel(self.r)
+        return self._V
+
+    @property
+    def n_kvc(self) -> int:
+        return self.n_k * self.n_v * self.n_c
+
+
+def make_periodic(n_k: int, n_v: int, n_c: int, n_mu: int, box: float = 10.0, seed: int = 0, n_omega: int = 101,
+                  n_chains: int = 4, real_orbitals: bool = False) -> PeriodicProblem:
+    """Draw order r, Re/Im psi_v, Re/Im psi_cq, eps_v, eps_cq.  Chains: n runs over the first orbitals of slot
+    (j mod n_k), alternating occupied / empty, m = the highest occupied orbital of slot 0."""
+    rng = np.random.default_rng(seed)
+    r = rng.random((n_mu, 3)) * box
+
+    def orbitals(n):
+        re = rng.standard_normal((n_k, n_mu, n))
+        im = rng.standard_normal((n_k, n_mu, n))
+        if real_orbitals:
+            return (re / np.sqrt(n_mu)).astype(np.complex128)
+        return (re + 1j * im) / np.sqrt(2.0 * n_mu)
+
+    psi_v = orbitals(n_v)
+    psi_cq = orbitals(n_c)
+    eps_v = np.sort(rng.uniform(-10.0, -5.0, (n_k, n_v)), axis=1)
+    eps_cq = np.sort(rng.uniform(-3.0, 20.0, (n_k, n_c)), axis=1)
+    omega = np.linspace(-20.0, 20.0, n_omega)
+    n_orb = n_v + n_c
+    chains = np.zeros((n_chains, 4), dtype=np.int32)
+    for j in range(n_chains):
+        idx = (j // 2) % n_v if j % 2 == 0 else n_v + (j // 2) % n_c
+        chains[j] = (j % n_k, min(idx, n_orb - 1), 0, n_v - 1)
+    return PeriodicProblem(n_k, n_v, n_c, n_mu, r, psi_v, psi_cq, eps_v, eps_cq, omega, chains)
+
+
+def random_complex_block(n: int, nvec: int, seed: int = 1) -> np.ndarray:
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((nvec, n)) + 1j * rng.standard_normal((nvec, n))

@@ -474,3 +474,103 @@ def test_oracle_matches_its_golden_file():
     assert set(got) == set(stored)
     for key, v in stored.items():
         assert abs(got[key] - v) <= 1e-9 * max(1.0, abs(v)), key
+
+
+# ---- thin spots named by the round-1 review ------------------------------------------------------
+def test_fit_sqrt_chebyshev_least_squares_optimality():
+    """The fit is THE least-squares solution on M = 4(g+1) first-kind Chebyshev nodes of [lo, hi] (PAPER.md:85, :284,
+    :317; reading Q13): the residual is orthogonal to T_0..T_g on those nodes (normal equations), rebuilt here from the
+    textbook node formula x_k = mid + half cos(pi (2k+1) / (2M)).  A wrong node set, node count or basis fails this."""
+    for g, lo, hi in [(1, 2.0, 3.0), (7, 9.4, 997.0), (8, 0.1, 10.0), (12, 7.0, 2600.0)]:
+        c = orc.fit_sqrt_chebyshev(g, lo, hi)
+        M = 4 * (g + 1)
+        k = np.arange(M)
+        t = np.cos(np.pi * (2 * k + 1) / (2 * M))
+        x = 0.5 * (hi + lo) + 0.5 * (hi - lo) * t
+        T = np.cos(np.arange(g + 1)[None, :] * np.arccos(t)[:, None])         # T_j(t_k) = cos(j arccos t_k)
+        resid = T @ c - np.sqrt(x)
+        assert np.abs(T.T @ resid).max() <= 1e-11 * np.sqrt(hi) * M
+        # and it beats any perturbed coefficient vector in the discrete 2-norm
+        rng = np.random.default_rng(g)
+        for _ in range(5):
+            d = 1e-3 * rng.standard_normal(g + 1)
+            assert np.linalg.norm(T @ (c + d) - np.sqrt(x)) > np.linalg.norm(resid)
+        # discrete orthogonality gives the same coefficients in closed form: c_j = (2/M) sum_k f(x_k) T_j(t_k), c_0 halved
+        cf = (2.0 / M) * (T.T @ np.sqrt(x))
+        cf[0] *= 0.5
+        assert np.abs(c - cf).max() <= 1e-12 * np.abs(cf).max()
+
+
+def _strongly_coupled_tiny():
+    """N_vc = 96 on 16 fitting points in a 3 A box: the coupling dominates, lambda_max(C) ~ 2138 eV^2."""
+    p = synth.make_custom(6, 16, 16, box=3.0, seed=3, chains_a=2, chains_b=2)
+    delta = orc.delta_vc(p.eps_v, p.eps_c)
+    C = orc.casida_dense(delta, orc.coupling_dense(orc.khatri_rao(p.phi_v, p.phi_c), p.V))
+    lam, Z = sla.eigh(C)
+    return p, delta, C, lam, Z
+
+
+def test_heuristic_fit_range_misses_a_strongly_coupled_spectrum():
+    """PAPER.md:284's heuristic range (reading Q12) is not a bound on the spectrum of C: its lower end is
+    (lambda_min(C) >= min Delta^2 for V >= 0, pin P1), its upper end is not once 2 sqrt(Delta) K^T V K sqrt(Delta) is
+    large, and a Chebyshev fit evaluated outside its interval diverges."""
+    p, delta, C, lam, Z = _strongly_coupled_tiny()
+    lo, hi = 0.8 * (delta ** 2).min(), 1.25 * (delta ** 2).max()
+    assert lo < lam[0] and lam[-1] > 2.0 * hi
+    c = orc.fit_sqrt_chebyshev(7, lo, hi)
+    assert abs(orc.poly_eval_scalar(c, lo, hi, lam[-1])) > 100.0 * np.sqrt(lam[-1])
+
+
+def test_spectrum_bounds_lanczos():
+    """extremal eigenvalues by Lanczos.  Full length: exact extremes.  Short runs: the upper estimate
+    theta_max + r_max has converged from above after a few steps (separated top eigenvalue), the Ritz values stay inside
+    the spectrum, and the intervals shrink with the number of steps."""
+    p, delta, C, lam, Z = _strongly_coupled_tiny()
+    n = delta.size
+    lo_f, hi_f = orc.spectrum_bounds_lanczos(lambda x: C @ x, n, n)
+    assert abs(hi_f - lam[-1]) <= 1e-9 * lam[-1] and abs(lo_f - lam[0]) <= 1e-7 * lam[-1]
+    prev = None
+    for steps in (5, 10, 20, 40):
+        lo_s, hi_s = orc.spectrum_bounds_lanczos(lambda x: C @ x, n, steps)
+        assert hi_s >= lam[-1] * (1 - 1e-12) and lo_s <= lam[0] * (1 + 1e-12)
+        if prev is not None:
+            assert hi_s <= prev[1] * (1 + 1e-12) and lo_s >= prev[0] - 1e-9
+        prev = (lo_s, hi_s)
+    assert prev[1] <= lam[-1] * (1 + 1e-9)
+    # the factored product gives the same estimate as the dense matrix
+    lo_x, hi_x = orc.spectrum_bounds_lanczos(
+        lambda x: orc.casida_matvec_factored(p.phi_v, p.phi_c, p.V, delta, x[None])[0], n, 20)
+    lo_d, hi_d = orc.spectrum_bounds_lanczos(lambda x: C @ x, n, 20)
+    # (the lower estimate is rounding-sensitive once the top Ritz value has converged and the basis loses orthogonality)
+    assert abs(hi_x - hi_d) <= 1e-9 * hi_d and abs(lo_x - lo_d) <= 1e-2 * hi_d
+
+
+def test_run_chains_poly_branch_end_to_end_against_eq7():
+    """The poly= branch of run_chains (start vector -> Lanczos on p_g(C) -> sigma_poly dispatch -> Eq. 10 sum) as one
+    piece against Eq. 7 by full diagonalisation, on the strongly coupled problem with the range taken from its
+    spectrum.  At L = N_vc with reorthogonalisation the only error left is the fit error
+    eps = max_s |p_g(Omega_s^2) - Omega_s|, which moves every pole of Eq. 12 by at most eps:
+    |dSigma| <= <P|P> eps (1/(Omega_min (Omega_min - eps)) + 1/delta^2) / delta.  The error must also fall with g."""
+    p, delta, C, lam, Z = _strongly_coupled_tiny()
+    n, dl = delta.size, 0.68
+    lo, hi = 0.8 * (delta ** 2).min(), 1.02 * lam[-1]
+    o_min = np.sqrt(lam[0])
+    worst = []
+    for g in (7, 12, 24):
+        c = orc.fit_sqrt_chebyshev(g, lo, hi)
+        eps = np.abs(orc.poly_eval_scalar(c, lo, hi, lam) - np.sqrt(lam)).max()
+        r = orc.run_chains(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, p.n_idx, p.m_idx, n, p.omega, dl, reorth=True,
+                           poly=(c, lo, hi))
+        errs, tot = [], 0.0
+        for j in range(len(p.n_idx)):
+            P = orc.start_vector(p.phi_v, p.phi_c, p.V, delta, int(p.n_idx[j]), int(p.m_idx[j]))
+            e_n, sg = orc.orbital_energy_sign(p.eps_v, p.eps_c, int(p.n_idx[j]))
+            exact = orc.sigma_exact_eq7(lam, Z, P, p.omega, e_n, sg, dl)
+            bound = (P @ P) * eps * (1.0 / (o_min * (o_min - eps)) + 1.0 / dl ** 2) / dl
+            err = np.abs(r["sigma"][j] - exact).max()
+            assert err <= bound, (g, j, err, bound)
+            errs.append(err / np.abs(exact).max())
+            tot = tot + exact
+        assert np.abs(r["sigma_sum"] - tot).max() <= sum(errs) * np.abs(tot).max() + 1e-12
+        worst.append(max(errs))
+    assert worst[0] > worst[1] > worst[2] and worst[2] < 0.01
