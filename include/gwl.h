@@ -158,6 +158,51 @@ gwl_status gwl_qp_solve(gwl_ctx* ctx, int64_t n_states, const double* eps_m, con
                         const double* sigma_x, const double* sigma_c, const double* omega, int64_t n_omega,
                         double* e_qp, double* z_qp, int32_t* iters);
 
+/* ---- complex orbitals and k-points in the Tamm-Dancoff approximation -------------------------------
+ * PAPER.md:157 and Supplemental Material section 1: for periodic systems the orbitals are complex and
+ * "if the Tamm-Dancoff approximation is used ... only a Hermitian matrix A remains, and a standard Lanczos algorithm for
+ * Hermitian matrix can be used".  One context serves ONE transferred momentum q:
+ *   A(q)_{vck,v'c'k'} = (eps_{ck+q} - eps_{vk}) delta + (vk, ck+q | v'k', c'k'+q)
+ *                     = diag(Delta) + K^H V K,  K[mu, (k,v,c)] = conj(psi_{vk}(r_mu)) psi_{ck+q}(r_mu),
+ *   Sigma^corr_{mk,mk}(omega) = 2/(N_q N_k) sum_n sum_q <P_nmk(q)| 1/(omega - eps_{nk-q} + eta (A(q) - i delta)) |P_nmk(q)>
+ * with V = (alpha|beta) real symmetric as set by gwl_set_kernel (A Hermitian and B symmetric, need that).
+ * Pair index (k, v, c), c fastest.  Complex arrays are interleaved (re, im) doubles.
+ * A context made by gwl_tdc_create accepts gwl_tdc_set_orbitals / gwl_tdc_set_energies / gwl_set_kernel /
+ * gwl_tdc_set_chains / gwl_tdc_matvec and then gwl_lanczos, gwl_resolvent, gwl_selfenergy, gwl_get_* exactly as above
+ * (alpha, beta are real: A is Hermitian; gwl_selfenergy includes the prefactor 2/(N_q N_k) in every chain and evaluates
+ * Eq. 14 at -eta_n z_n as in GWL_TDA); the real-orbital set_* calls, gwl_set_polynomial, gwl_exchange return GWL_ESTATE.
+ * The pseudo-Hermitian Lanczos for the full RPA matrix with complex orbitals is not part of this library. */
+gwl_status gwl_tdc_create(gwl_ctx** out, int64_t n_k, int64_t n_v, int64_t n_c, int64_t n_mu, int64_t n_q);
+/* psi_v [n_k][n_mu][n_v][2] = psi_{v k}(r_mu); psi_cq [n_k][n_mu][n_c][2] = psi_{c k+q}(r_mu) (slot k holds the conduction
+ * orbitals of momentum k+q: the caller does the momentum bookkeeping).  Host. */
+gwl_status gwl_tdc_set_orbitals(gwl_ctx* ctx, const double* psi_v, const double* psi_cq);
+/* eps_v [n_k][n_v], eps_cq [n_k][n_c] (eps_{c k+q} in slot k), host; GWL_EINVAL unless min(eps_cq) > max(eps_v). */
+gwl_status gwl_tdc_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps_cq);
+/* Chain j starts from the ket of PAPER.md:310-313 for (n k-q, m k): chains [n_chains][4] = (slot of n, n index,
+ * slot of m, m index), host; an orbital (slot s, index i) is psi_v[s][:, i] for i < n_v (eta = +1), else the conduction
+ * orbital psi_cq[s][:, i - n_v] (eta = -1).  The printed elements P_{v'c'k'} = (nk-q, mk | v'k', c'k'+q) enter the pole
+ * strengths bilinearly (W^s = sum P X^s), so the Lanczos start vector is their complex conjugate
+ * K^H (V rho~), rho~ = psi_m conj(psi_n) (reading Q20; identical for real orbitals). */
+gwl_status gwl_tdc_set_chains(gwl_ctx* ctx, int64_t n_chains, const int32_t* chains);
+/* y = A(q) x for nvec complex vectors x, y [nvec][n_k][n_v][n_c][2] (pointer mode applies); x and y must not overlap. */
+gwl_status gwl_tdc_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec);
+
+/* ---- interpolative separable density fitting front end -------------------------------------------
+ * PAPER.md:115-128 (Eq. 15-17): phi_n(r) phi_m(r) ~ sum_mu zeta_mu(r) C^mu_nm with C^mu_nm = phi_n(r_mu) phi_m(r_mu) at given
+ * interpolation points r_mu = r[idx[mu]] (ISDF, refs. [62, 63]); zeta is the least-squares solution
+ * zeta = Z C^T (C C^T)^{-1} over the pairs of ALL n_v + n_c orbitals, computed from the separable normal equations
+ * Z C^T = (Phi Phi_mu^T) o (Phi Phi_mu^T) (Cholesky; GWL_EINVAL if C C^T is not positive definite); then
+ * (alpha|beta) = int int zeta_alpha(r) zeta_beta(r') / |r - r'| (Eq. 17) as the grid quadrature
+ * sum_ij zeta_alpha(r_i) G_ij zeta_beta(r_j), G_ij = weight^2 14.4 / sqrt(|r_i - r_j|^2 + soft^2) eV (softened at short range:
+ * the stand-in for the real-space Poisson solve).  The paper's code runs this part on CPUs.
+ * Inputs (host): phi_v_grid [n_r][n_v], phi_c_grid [n_r][n_c] orbitals on the real-space grid, r [n_r][3] grid points
+ * (Angstrom), weight = h^3, soft > 0, idx [n_mu] distinct grid indices.  n_mu <= n_r <= 65535.
+ * Effect: the context's orbitals become the grid orbitals at the interpolation points and its kernel becomes (alpha|beta),
+ * exactly as after gwl_set_orbitals + gwl_set_kernel (gwl_set_energies is still needed).  Optional host outputs:
+ * zeta_t [n_mu][n_r] (zeta transposed) and V_out [n_mu][n_mu]; either may be NULL. */
+gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, const double* phi_c_grid, const double* r,
+                          double weight, double soft, const int32_t* idx, double* zeta_t, double* V_out);
+
 /* CUDA-event totals (ms) of the last gwl_lanczos: time inside Casida products (S2), inside the Lanczos
  * vector kernels (S4) and overall.  Any pointer may be NULL.  Synchronises the stream. */
 gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total);

@@ -55,6 +55,10 @@ struct gwl_ctx {
     int n_cp = 0, n_mup = 0;
     int n_sm = 148;
     int device = 0;
+    // complex-orbital (periodic Tamm-Dancoff) contexts, gwl_tdc_create: Lanczos vectors are planar [re | im], so the
+    // vector layout has n_v = 2 * n_kv "rows" of n_c and n_vc = 2 * n_k * nv_k * n_c real entries
+    bool cplx = false;
+    int n_k = 1, nv_k = 0, n_kv = 0, n_q = 1;
     cudaStream_t stream = nullptr;
     int device_ptrs = 0;
     std::string err;
@@ -84,6 +88,8 @@ struct gwl_ctx {
     DevBuf x_nidx, x_midx, x_part, x_sig, x_eps, x_vxc, x_sc, x_e, x_z, x_it;  // gwl_exchange / gwl_qp_solve staging
     DevBuf stage;            // gwl_set_orbitals staging
     DevBuf sk_ws, sk_flags;  // stream-K hand-over of the K^T.W GEMM (kr_gemm.cu)
+    DevBuf isdf_phi, isdf_phimu, isdf_y, isdf_s, isdf_g, isdf_u;  // gwl_isdf_build
+    DevBuf red_cnt;          // arrive / done counters of the in-kernel split-K reduction (K.X, V.T), zero between launches
     unsigned sk_epoch = 0;
     DevBuf theta, wgt, ritz_info, d_omega, d_zeta, d_sigma, d_sigsum, io_x, io_y;
 
@@ -179,25 +185,65 @@ gwl_status ensure_workspace(gwl_ctx* ctx, int nb) {
     cudaStream_t st = ctx->stream;
     const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
     CK(ctx->xs.ensure((size_t)nb * ldxs * 8, st));
-    CK(ctx->T.ensure((size_t)nb * ctx->n_mup * 8, st));
-    CK(ctx->W.ensure((size_t)nb * ctx->n_mup * 8, st));
+    const int rows = ctx->cplx ? 2 * nb : nb;  // complex: T and W hold a real and an imaginary plane of nb rows each
+    CK(ctx->T.ensure((size_t)rows * ctx->n_mup * 8, st));
+    CK(ctx->W.ensure((size_t)rows * ctx->n_mup * 8, st));
     const int kt_f = ctx->n_v * (ctx->n_cp / BK), kt_v = ctx->n_mup / BK;
-    const GemmPlan pf = plan_gemm(MODE_FWD, ctx->n_mu, nb, kt_f, ctx->n_cp / BK, ctx->n_sm);
-    const GemmPlan pv = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
+    const GemmPlan pf = ctx->cplx ? plan_gemm_c(ctx->n_mu, nb, ctx->n_kv * (ctx->n_cp / BK), ctx->n_sm)
+                                  : plan_gemm(MODE_FWD, ctx->n_mu, nb, kt_f, ctx->n_cp / BK, ctx->n_sm);
+    const GemmPlan pv = plan_gemm(MODE_PLAIN, ctx->n_mu, rows, kt_v, kt_v, ctx->n_sm);
     const int smax = std::max(pf.splits, pv.splits);
-    CK(ctx->part.ensure((size_t)smax * nb * ctx->n_mup * 8, st));
+    CK(ctx->part.ensure((size_t)smax * rows * ctx->n_mup * 8, st));
     const int npart = vec_parts(ctx->n_vc);
     const int64_t ndot = std::max<int64_t>((int64_t)ctx->n_v * ceil_div(ctx->n_c, 128), npart);
     CK(ctx->dotpart.ensure((size_t)nb * ndot * 8, st));
     CK(ctx->normpart.ensure((size_t)nb * std::max(npart, reorth_parts(ctx->n_vc)) * 8, st));
     CK(ctx->sk_ws.ensure(gemm_bwd_ws_bytes(ctx->n_sm), st));
     CK(ctx->sk_flags.ensure(gemm_bwd_flag_bytes(ctx->n_sm), st));
+    CK(ctx->red_cnt.ensure(gemm_red_cnt_bytes(ctx->n_sm), st));
     return GWL_OK;
 }
 
 // ---- the three contractions (kr_gemm.cu), each with its split-K reduction where the planner asks for one ---------
 // T[b][mu] = sum_vc K[mu, vc] xs[b][vc]   (xs = scaled input in the padded [nb][n_v][n_cp] layout)
+// complex (planar) K.x of the periodic Tamm-Dancoff operator: T[2][nb][n_mup] (kr_gemm_c.cu)
+gwl_status gemm_kx_c(gwl_ctx* ctx, int nb) {
+    cudaStream_t st = ctx->stream;
+    const int kt_c = ctx->n_cp / BK, kt_f = ctx->n_kv * kt_c;
+    const int64_t ldm = ctx->n_mup;
+    const GemmPlan pl = plan_gemm_c(ctx->n_mu, nb, kt_f, ctx->n_sm);
+    GemmParamsC p{};
+    p.A = ctx->phi_c.as<double>();
+    p.lda = (int64_t)ctx->n_k * ctx->n_cp;
+    p.a_plane = (int64_t)ctx->n_mu * p.lda;
+    p.B = ctx->xs.as<double>();
+    p.ldb = (int64_t)ctx->n_v * ctx->n_cp;
+    p.b_plane_cols = ctx->n_kv * ctx->n_cp;
+    p.M = ctx->n_mu;
+    p.N = nb;
+    p.kt_total = kt_f;
+    p.a_wrap = kt_c;
+    p.kt_per_split = pl.kt_per_split;
+    p.n_v = ctx->nv_k;
+    p.n_c = ctx->n_c;
+    p.scale = ctx->phi_vT.as<double>();
+    p.lds = ldm;
+    p.s_plane = (int64_t)ctx->n_kv * ldm;
+    p.scale_rows = ctx->n_kv;
+    if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * 2 * nb * ldm * 8, st));
+    p.out = pl.splits == 1 ? ctx->T.as<double>() : ctx->part.as<double>();
+    p.ldo = ldm;
+    p.o_plane = (int64_t)nb * ldm;
+    p.out_split_stride = (int64_t)2 * nb * ldm;
+    CKL(0, launch_gemm_c(MODE_FWD, EPI_STORE, p, pl.splits, st));
+    if (pl.splits > 1)
+        CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)2 * nb * ldm, pl.splits, ctx->T.as<double>(), ldm,
+                                    ctx->n_mu, 2 * nb, st));
+    return GWL_OK;
+}
+
 gwl_status gemm_kx(gwl_ctx* ctx, int nb) {
+    if (ctx->cplx) return gemm_kx_c(ctx, nb);
     cudaStream_t st = ctx->stream;
     const int kt_c = ctx->n_cp / BK, kt_f = ctx->n_v * kt_c;
     const int64_t ldm = ctx->n_mup;
@@ -219,38 +265,55 @@ gwl_status gemm_kx(gwl_ctx* ctx, int nb) {
     p.out = pl.splits == 1 ? ctx->T.as<double>() : ctx->part.as<double>();
     p.ldo = ldm;
     p.out_split_stride = (int64_t)nb * ldm;
+    const bool fused = gemm_reduces_in_kernel(pl, ctx->n_mu, nb, ctx->n_sm);
+    if (fused) {
+        p.red_cnt = ctx->red_cnt.as<unsigned>();
+        p.out_final = ctx->T.as<double>();
+    }
     CKL(0, launch_gemm(MODE_FWD, EPI_STORE, pl, p, pl.splits, st));
-    if (pl.splits > 1)
+    if (pl.splits > 1 && !fused)
         CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->T.as<double>(), ldm, ctx->n_mu,
                                 nb, st));
     return GWL_OK;
 }
 
+// out[n][m] = sum_k A[m][k] B[n][k] on the DMMA GEMM (MODE_PLAIN): A [M][lda], B [N][ldb], both K-contiguous with k_tiles
+// tiles of 16 valid (zero-padded) columns; split-K reduced in the kernel when the grid is co-resident, else by k_splitk_reduce
+gwl_status plain_gemm(gwl_ctx* ctx, const double* A, int64_t lda, const double* B, int64_t ldb, int M, int N, int k_tiles,
+                      double* out, int64_t ldo, int cls) {
+    cudaStream_t st = ctx->stream;
+    const GemmPlan pl = plan_gemm(MODE_PLAIN, M, N, k_tiles, k_tiles, ctx->n_sm);
+    GemmParams p{};
+    p.A = A;
+    p.lda = lda;
+    p.B = B;
+    p.ldb = ldb;
+    p.M = M;
+    p.N = N;
+    p.kt_total = k_tiles;
+    p.a_wrap = k_tiles;
+    p.kt_per_split = pl.kt_per_split;
+    if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * N * ldo * 8, st));
+    p.out = pl.splits == 1 ? out : ctx->part.as<double>();
+    p.ldo = ldo;
+    p.out_split_stride = (int64_t)N * ldo;
+    const bool fused = gemm_reduces_in_kernel(pl, M, N, ctx->n_sm);
+    if (fused) {
+        CK(ctx->red_cnt.ensure(gemm_red_cnt_bytes(ctx->n_sm), st));
+        p.red_cnt = ctx->red_cnt.as<unsigned>();
+        p.out_final = out;
+    }
+    CKL(cls, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
+    if (pl.splits > 1 && !fused)
+        CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)N * ldo, pl.splits, out, ldo, M, N, st));
+    return GWL_OK;
+}
+
 // W[b][mu] = sum_nu V[mu][nu] T[b][nu]
 gwl_status gemm_v(gwl_ctx* ctx, int nb) {
-    cudaStream_t st = ctx->stream;
-    const int kt_v = ctx->n_mup / BK;
-    const int64_t ldm = ctx->n_mup;
-    const GemmPlan pl = plan_gemm(MODE_PLAIN, ctx->n_mu, nb, kt_v, kt_v, ctx->n_sm);
-    GemmParams p{};
-    p.A = ctx->V.as<double>();
-    p.lda = ldm;
-    p.B = ctx->T.as<double>();
-    p.ldb = ldm;
-    p.M = ctx->n_mu;
-    p.N = nb;
-    p.kt_total = kt_v;
-    p.a_wrap = kt_v;
-    p.kt_per_split = pl.kt_per_split;
-    if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
-    p.out = pl.splits == 1 ? ctx->W.as<double>() : ctx->part.as<double>();
-    p.ldo = ldm;
-    p.out_split_stride = (int64_t)nb * ldm;
-    CKL(1, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
-    if (pl.splits > 1)
-        CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->W.as<double>(), ldm, ctx->n_mu,
-                                nb, st));
-    return GWL_OK;
+    if (ctx->cplx) nb *= 2;  // V is real: the two planes of T are 2 nb independent columns
+    return plain_gemm(ctx, ctx->V.as<double>(), ctx->n_mup, ctx->T.as<double>(), ctx->n_mup, ctx->n_mu, nb, ctx->n_mup / BK,
+                      ctx->W.as<double>(), ctx->n_mup, 1);
 }
 
 // u = K^T W with the epilogue fused:  x != NULL: y = d2 o x + coupling s o u and the partial dots sum(x y);
@@ -265,8 +328,48 @@ struct ChebTerm {
     int first;
 };
 
+// complex (planar) K^H.W with the epilogue y = Delta o x + u (or y = u for start vectors), kr_gemm_c.cu
+gwl_status gemm_ktw_c(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64_t ldy, int nb, double* dotpart,
+                      int dot_stride) {
+    const int64_t ldm = ctx->n_mup;
+    const int64_t n_kvc = (int64_t)ctx->n_kv * ctx->n_c;
+    GemmParamsC p{};
+    p.A = ctx->phi_cT.as<double>();
+    p.lda = ldm;
+    p.a_rows = ctx->n_k * ctx->n_c;
+    p.a_plane = (int64_t)p.a_rows * ldm;
+    p.B = ctx->W.as<double>();
+    p.ldb = ldm;
+    p.b_plane = (int64_t)nb * ldm;
+    p.M = ctx->n_c;
+    p.N = nb;
+    p.kt_total = ctx->n_mup / BK;
+    p.n_v = ctx->nv_k;
+    p.n_c = ctx->n_c;
+    p.scale = ctx->phi_vT.as<double>();
+    p.lds = ldm;
+    p.s_plane = (int64_t)ctx->n_kv * ldm;
+    p.scale_rows = ctx->n_kv;
+    p.out = y;
+    p.ldo = ldy;
+    p.o_plane = n_kvc;
+    p.X = x;
+    p.ldx = ldx;
+    p.x_plane = n_kvc;
+    p.d2 = ctx->d2.as<double>();
+    p.coupling = 1.0;
+    p.dotpart = dotpart;
+    p.dot_stride = dot_stride;
+    CKL(2, launch_gemm_c(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, p, ctx->n_kv, ctx->stream));
+    return GWL_OK;
+}
+
 gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64_t ldy, int nb, double* dotpart,
                     int dot_stride, const ChebTerm* cheb = nullptr) {
+    if (ctx->cplx) {
+        if (cheb != nullptr) return ctx->fail(GWL_EINVAL, "internal: no polynomial mode for complex orbitals");
+        return gemm_ktw_c(ctx, x, ldx, y, ldy, nb, dotpart, dot_stride);
+    }
     const int kt_v = ctx->n_mup / BK;
     const int64_t ldm = ctx->n_mup;
     const GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, kt_v, kt_v, ctx->n_sm);
@@ -330,6 +433,7 @@ gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double*
 
 // alpha / norm partials written by the K^T.W epilogue: one per (v, m-tile) of the plan used for a block of nb
 int casida_ndot(const gwl_ctx* ctx, int nb) {
+    if (ctx->cplx) return ctx->n_kv * gemm_c_tiles_m(ctx->n_c);
     const GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, ctx->n_mup / BK, ctx->n_mup / BK, ctx->n_sm);
     return ctx->n_v * (int)ceil_div(ctx->n_c, pl.bm);
 }
@@ -337,9 +441,14 @@ int casida_ndot(const gwl_ctx* ctx, int nb) {
 // S1: P_j = sqrt(Delta) o K^T (V rho_j) for index chains j0..j0+nb; writes P and sum(P^2) partials.
 gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, double* normpart, int dot_stride) {
     const int64_t ldm = ctx->n_mup;
-    CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
-                  ctx->d_nidx.as<int32_t>() + j0, ctx->d_midx.as<int32_t>() + j0, ctx->T.as<double>(), ldm, nb,
-                  ctx->stream));
+    if (ctx->cplx)  // rho~ = psi_m conj(psi_n): the ket of PAPER.md:310 is the conjugate of the printed elements (Q20)
+        CKL(4, launch_rho_c(ctx->phi_vT.as<double>(), (int64_t)ctx->n_kv * ldm, ctx->phi_cT.as<double>(),
+                            (int64_t)ctx->n_k * ctx->n_c * ldm, ldm, ctx->nv_k, ctx->n_c, ctx->n_mu,
+                            ctx->d_nidx.as<int32_t>() + 4 * j0, ctx->T.as<double>(), ldm, nb, ctx->stream));
+    else
+        CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
+                      ctx->d_nidx.as<int32_t>() + j0, ctx->d_midx.as<int32_t>() + j0, ctx->T.as<double>(), ldm, nb,
+                      ctx->stream));
     gwl_status rs = gemm_v(ctx, nb);
     if (rs == GWL_OK) rs = gemm_ktw(ctx, nullptr, ctx->n_vc, P, ctx->n_vc, nb, normpart, dot_stride);
     return rs;
@@ -352,10 +461,12 @@ bool ready(const gwl_ctx* ctx) { return ctx->have_orb && ctx->have_eps && ctx->h
 // ------------------------------------------------------------------------------------------------
 extern "C" {
 
-gwl_status gwl_create(gwl_ctx** out, int64_t n_v, int64_t n_c, int64_t n_mu) {
+static gwl_status create_common(gwl_ctx** out, int64_t n_k, int64_t n_v, int64_t n_c, int64_t n_mu, bool cplx, int64_t n_q) {
     if (out == nullptr) return GWL_EINVAL;
     *out = nullptr;
-    if (n_v < 1 || n_c < 1 || n_mu < 1 || n_v > (1 << 20) || n_c > (1 << 20) || n_mu > (1 << 24)) return GWL_EINVAL;
+    if (n_v < 1 || n_c < 1 || n_mu < 1 || n_k < 1 || n_q < 1 || n_k > 4096 || n_k * n_v > (1 << 20) || n_c > (1 << 20) ||
+        n_mu > (1 << 24))
+        return GWL_EINVAL;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) {
         cudaGetLastError();
@@ -369,16 +480,30 @@ gwl_status gwl_create(gwl_ctx** out, int64_t n_v, int64_t n_c, int64_t n_mu) {
     if (prop.major != 10) return GWL_ECUDA;  // the kernels are sm_100a code (TMA, DMMA, clusters, PDL): B200 only
     gwl_ctx* ctx = new (std::nothrow) gwl_ctx();
     if (ctx == nullptr) return GWL_ENOMEM;
-    ctx->n_v = (int)n_v;
+    ctx->cplx = cplx;
+    ctx->n_k = (int)n_k;
+    ctx->nv_k = (int)n_v;
+    ctx->n_kv = (int)(n_k * n_v);
+    ctx->n_q = (int)n_q;
+    ctx->n_v = cplx ? 2 * ctx->n_kv : (int)n_v;
     ctx->n_c = (int)n_c;
     ctx->n_mu = (int)n_mu;
-    ctx->n_vc = n_v * n_c;
+    ctx->n_vc = (int64_t)ctx->n_v * n_c;
     ctx->n_cp = (int)round_up(n_c, BK);
     ctx->n_mup = (int)round_up(n_mu, BK);
     ctx->n_sm = prop.multiProcessorCount;
     ctx->device = dev;
+    if (cplx) ctx->approx = GWL_TDA;  // Lanczos on the Hermitian A(q)
     *out = ctx;
     return GWL_OK;
+}
+
+gwl_status gwl_create(gwl_ctx** out, int64_t n_v, int64_t n_c, int64_t n_mu) {
+    return create_common(out, 1, n_v, n_c, n_mu, false, 1);
+}
+
+gwl_status gwl_tdc_create(gwl_ctx** out, int64_t n_k, int64_t n_v, int64_t n_c, int64_t n_mu, int64_t n_q) {
+    return create_common(out, n_k, n_v, n_c, n_mu, true, n_q);
 }
 
 void gwl_destroy(gwl_ctx* ctx) {
@@ -390,7 +515,7 @@ void gwl_destroy(gwl_ctx* ctx) {
                       &ctx->beta, &ctx->norm2, &ctx->len, &ctx->scale, &ctx->alive, &ctx->xs, &ctx->T, &ctx->W,
                       &ctx->part, &ctx->dotpart, &ctx->normpart, &ctx->basis, &ctx->coefpart, &ctx->tA, &ctx->tB,
                       &ctx->theta, &ctx->wgt, &ctx->ritz_info, &ctx->d_omega, &ctx->d_zeta,
-                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y, &ctx->sk_ws, &ctx->sk_flags, &ctx->stage, &ctx->x_nidx, &ctx->x_midx, &ctx->x_part, &ctx->x_sig,
+                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y, &ctx->sk_ws, &ctx->sk_flags, &ctx->red_cnt, &ctx->isdf_phi, &ctx->isdf_phimu, &ctx->isdf_y, &ctx->isdf_s, &ctx->isdf_g, &ctx->isdf_u, &ctx->stage, &ctx->x_nidx, &ctx->x_midx, &ctx->x_part, &ctx->x_sig,
                       &ctx->x_eps, &ctx->x_vxc, &ctx->x_sc, &ctx->x_e, &ctx->x_z, &ctx->x_it};
     for (DevBuf* b : bufs) b->release();
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
@@ -415,27 +540,38 @@ gwl_status gwl_set_stream(gwl_ctx* ctx, void* cuda_stream) {
     return GWL_OK;
 }
 
-gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi_c) {
-    if (ctx == nullptr) return GWL_EINVAL;
-    DeviceGuard dg(ctx);
-    if (phi_v == nullptr || phi_c == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_orbitals: NULL input");
-    LaunchScope ls(ctx);
+// Orbitals at the fitting points from compact DEVICE arrays d_phi_v [n_mu][n_v], d_phi_c [n_mu][n_c]: the padded and
+// transposed copies the GEMMs read
+static gwl_status install_orbitals(gwl_ctx* ctx, const double* d_phi_v, const double* d_phi_c) {
     cudaStream_t st = ctx->stream;
-    const size_t nv = (size_t)ctx->n_mu * ctx->n_v, nc = (size_t)ctx->n_mu * ctx->n_c;
-    DevBuf& tmp = ctx->stage;  // kept across calls: no cudaMalloc/cudaFree in a repeated set_orbitals
-    CK(tmp.ensure(std::max(nv, nc) * 8, st));
     CK(ctx->phi_c.ensure((size_t)ctx->n_mu * ctx->n_cp * 8, st));
     CK(ctx->phi_cT.ensure((size_t)ctx->n_c * ctx->n_mup * 8, st));
     CK(ctx->phi_vT.ensure((size_t)ctx->n_v * ctx->n_mup * 8, st));
     CK(cudaMemsetAsync(ctx->phi_c.p, 0, ctx->phi_c.bytes, st));
     CK(cudaMemsetAsync(ctx->phi_cT.p, 0, ctx->phi_cT.bytes, st));
     CK(cudaMemsetAsync(ctx->phi_vT.p, 0, ctx->phi_vT.bytes, st));
-    CK(cudaMemcpyAsync(tmp.p, phi_c, nc * 8, cudaMemcpyHostToDevice, st));
-    CKL(4, launch_copy_pad(tmp.as<double>(), ctx->n_mu, ctx->n_c, ctx->phi_c.as<double>(), ctx->n_cp, st));
-    CKL(4, launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_c, ctx->phi_cT.as<double>(), ctx->n_mup, st));
-    CK(cudaStreamSynchronize(st));
-    CK(cudaMemcpyAsync(tmp.p, phi_v, nv * 8, cudaMemcpyHostToDevice, st));
-    CKL(4, launch_transpose(tmp.as<double>(), ctx->n_mu, ctx->n_v, ctx->phi_vT.as<double>(), ctx->n_mup, st));
+    CKL(4, launch_copy_pad(d_phi_c, ctx->n_mu, ctx->n_c, ctx->phi_c.as<double>(), ctx->n_cp, st));
+    CKL(4, launch_transpose(d_phi_c, ctx->n_mu, ctx->n_c, ctx->phi_cT.as<double>(), ctx->n_mup, st));
+    CKL(4, launch_transpose(d_phi_v, ctx->n_mu, ctx->n_v, ctx->phi_vT.as<double>(), ctx->n_mup, st));
+    return GWL_OK;
+}
+
+gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi_c) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_orbitals: real-orbital call on a complex (gwl_tdc_create) context");
+    if (phi_v == nullptr || phi_c == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_orbitals: NULL input");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const size_t nv = (size_t)ctx->n_mu * ctx->n_v, nc = (size_t)ctx->n_mu * ctx->n_c;
+    DevBuf& tmp = ctx->stage;  // kept across calls: no cudaMalloc/cudaFree in a repeated set_orbitals
+    CK(tmp.ensure((nv + nc) * 8, st));
+    double* dv = tmp.as<double>();
+    double* dc = dv + nv;
+    CK(cudaMemcpyAsync(dc, phi_c, nc * 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(dv, phi_v, nv * 8, cudaMemcpyHostToDevice, st));
+    gwl_status rs = install_orbitals(ctx, dv, dc);
+    if (rs != GWL_OK) return rs;
     CK(cudaStreamSynchronize(st));
     ctx->have_orb = true;
     invalidate_run(ctx);
@@ -445,6 +581,7 @@ gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi
 gwl_status gwl_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps_c) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_energies: real-orbital call on a complex (gwl_tdc_create) context");
     if (eps_v == nullptr || eps_c == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_energies: NULL input");
     double vmax = -INFINITY, cmin = INFINITY;
     for (int i = 0; i < ctx->n_v; ++i) {
@@ -496,6 +633,7 @@ gwl_status gwl_set_kernel(gwl_ctx* ctx, const double* V) {
 gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo, double hi) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_polynomial: real-orbital call on a complex (gwl_tdc_create) context");
     if (g < 0 || g > 64) return ctx->fail(GWL_EINVAL, "gwl_set_polynomial: g out of range [0, 64]");
     if (g == 0) {
         ctx->g = 0;
@@ -518,6 +656,7 @@ gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo
 gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation) {
     if (ctx == nullptr || (approximation != GWL_RPA && approximation != GWL_TDA)) return GWL_EINVAL;
     DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_approximation: real-orbital call on a complex (gwl_tdc_create) context");
     if (approximation == GWL_TDA && ctx->g > 0)
         return ctx->fail(GWL_ESTATE, "gwl_set_approximation: clear the polynomial first (it approximates sqrt(C), RPA only)");
     ctx->approx = approximation;
@@ -535,6 +674,7 @@ gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation) {
 gwl_status gwl_casida_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_casida_matvec: real-orbital call on a complex (gwl_tdc_create) context");
     if (nvec < 0) return ctx->fail(GWL_EINVAL, "gwl_casida_matvec: nvec < 0");
     if (nvec == 0) return GWL_OK;
     if (x == nullptr || y == nullptr) return ctx->fail(GWL_EINVAL, "gwl_casida_matvec: NULL vector");
@@ -576,6 +716,7 @@ gwl_status gwl_casida_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t n
 gwl_status gwl_set_chains(gwl_ctx* ctx, int64_t n_chains, const int32_t* n_idx, const int32_t* m_idx) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_chains: real-orbital call on a complex (gwl_tdc_create) context");
     if (n_chains < 0 || (n_chains > 0 && (n_idx == nullptr || m_idx == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_set_chains: bad arguments");
     if (!ctx->have_eps) return ctx->fail(GWL_ESTATE, "gwl_set_chains: energies must be set first");
@@ -611,6 +752,7 @@ gwl_status gwl_set_start_vectors(gwl_ctx* ctx, int64_t n_chains, const double* p
                                  const int32_t* sgn_n) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_start_vectors: real-orbital call on a complex (gwl_tdc_create) context");
     if (n_chains < 0 || (n_chains > 0 && (p == nullptr || eps_n == nullptr || sgn_n == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_set_start_vectors: bad arguments");
     for (int64_t j = 0; j < n_chains; ++j)
@@ -834,7 +976,11 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
     LaunchScope ls(ctx);
     cudaStream_t st = ctx->stream;
     const int nch = (int)ctx->run_chains, L = ctx->run_steps;
-    const size_t nsig = (size_t)std::max(nch, 1) * n_omega * 16;
+    // Only the sum is wanted (gwl_selfenergy_state): Sigma[chain][omega] is never materialised -- the chains go through a
+    // small buffer in chunks and Eq. 10 is accumulated chunk by chunk on the device, in a fixed order.
+    const bool sum_only = sigma == nullptr && sigma_sum != nullptr;
+    const int chunk = sum_only ? std::min(std::max(nch, 1), 256) : std::max(nch, 1);
+    const size_t nsig = (size_t)chunk * n_omega * 16;
     const double* dom = omega;
     double* dsig = sigma;
     double* dsum = sigma_sum;
@@ -851,32 +997,38 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
         CK(ctx->d_sigsum.ensure((size_t)n_omega * 16, st));
         dsum = ctx->d_sigsum.as<double>();
     }
-    if (nch > 0) {
-        if (ctx->run_poly == 2) {
-            CKL(7, launch_sigma_tda(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
-                                ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
-                                ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));
-        } else if (ctx->run_poly == 1) {
-            CKL(7, launch_sigma_poly(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->norm2.as<double>(),
-                                 ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
-                                 ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));
-        } else {
-            CK(ctx->theta.ensure((size_t)nch * L * 8, st));
-            CK(ctx->wgt.ensure((size_t)nch * L * 8, st));
-            CK(ctx->ritz_info.ensure((size_t)nch * 4, st));
-            // divide and conquer (parallel) when T_L fits one CTA's shared memory, else the sequential QL kernel
-            if (ritz_dc_fits(L))
-                CKL(7, launch_ritz_dc(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
-                                  ctx->theta.as<double>(), ctx->wgt.as<double>(), ctx->ritz_info.as<int32_t>(), st));
-            else
-                CKL(7, launch_ritz(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
-                               ctx->theta.as<double>(), ctx->wgt.as<double>(), nullptr, ctx->ritz_info.as<int32_t>(), st));
-            CKL(7, launch_sigma_direct(ctx->theta.as<double>(), ctx->wgt.as<double>(), ctx->norm2.as<double>(),
-                                   ctx->len.as<int32_t>(), L, nch, ctx->d_eps_n.as<double>(),
-                                   ctx->d_sgn_n.as<int32_t>(), dom, (int)n_omega, eta, dsig, st));
-        }
+    if (nch > 0 && ctx->run_poly == 0) {
+        CK(ctx->theta.ensure((size_t)nch * L * 8, st));
+        CK(ctx->wgt.ensure((size_t)nch * L * 8, st));
+        CK(ctx->ritz_info.ensure((size_t)nch * 4, st));
+        // divide and conquer (parallel) when T_L fits one CTA's shared memory, else the sequential QL kernel
+        if (ritz_dc_fits(L))
+            CKL(7, launch_ritz_dc(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
+                              ctx->theta.as<double>(), ctx->wgt.as<double>(), ctx->ritz_info.as<int32_t>(), st));
+        else
+            CKL(7, launch_ritz(ctx->alpha.as<double>(), ctx->beta.as<double>(), ctx->len.as<int32_t>(), L, nch,
+                           ctx->theta.as<double>(), ctx->wgt.as<double>(), nullptr, ctx->ritz_info.as<int32_t>(), st));
     }
-    if (sigma_sum != nullptr) CKL(7, launch_sigma_sum(dsig, nch, (int)n_omega, dsum, st));
+    for (int c0 = 0; c0 < nch; c0 += chunk) {
+        const int nc = std::min(chunk, nch - c0);
+        double* out = sum_only ? dsig : dsig + (size_t)c0 * n_omega * 2;
+        const double* al = ctx->alpha.as<double>() + (size_t)c0 * L;
+        const double* be = ctx->beta.as<double>() + (size_t)c0 * L;
+        const double* n2 = ctx->norm2.as<double>() + c0;
+        const int32_t* ln = ctx->len.as<int32_t>() + c0;
+        const double* en = ctx->d_eps_n.as<double>() + c0;
+        const int32_t* sg = ctx->d_sgn_n.as<int32_t>() + c0;
+        if (ctx->run_poly == 2)
+            CKL(7, launch_sigma_tda(al, be, n2, ln, L, nc, en, sg, dom, (int)n_omega, eta,
+                                    ctx->cplx ? 2.0 / ((double)ctx->n_q * ctx->n_k) : 1.0, out, st));
+        else if (ctx->run_poly == 1)
+            CKL(7, launch_sigma_poly(al, be, n2, ln, L, nc, en, sg, dom, (int)n_omega, eta, out, st));
+        else
+            CKL(7, launch_sigma_direct(ctx->theta.as<double>() + (size_t)c0 * L, ctx->wgt.as<double>() + (size_t)c0 * L, n2, ln,
+                                       L, nc, en, sg, dom, (int)n_omega, eta, out, st));
+        if (sigma_sum != nullptr) CKL(7, launch_sigma_sum(out, nc, (int)n_omega, dsum, c0 > 0 ? 1 : 0, st));
+    }
+    if (sigma_sum != nullptr && nch == 0) CKL(7, launch_sigma_sum(dsig, 0, (int)n_omega, dsum, 0, st));
     if (!ctx->device_ptrs) {
         if (sigma != nullptr && nch > 0)
             CK(cudaMemcpyAsync(sigma, dsig, (size_t)nch * n_omega * 16, cudaMemcpyDeviceToHost, st));
@@ -891,6 +1043,7 @@ gwl_status gwl_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, int6
                                 const double* omega, int64_t n_omega, double eta, double* sigma_mm) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_selfenergy_state: real-orbital call on a complex (gwl_tdc_create) context");
     if (sigma_mm == nullptr || omega == nullptr || n_omega < 1)
         return ctx->fail(GWL_EINVAL, "gwl_selfenergy_state: bad arguments");
     const int n_orb = ctx->n_v + ctx->n_c;
@@ -906,6 +1059,7 @@ gwl_status gwl_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, int6
 gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, double* sigma_x) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_exchange: real-orbital call on a complex (gwl_tdc_create) context");
     if (n_states < 0 || (n_states > 0 && (m_idx == nullptr || sigma_x == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_exchange: bad arguments");
     if (!ctx->have_orb || !ctx->have_V) return ctx->fail(GWL_ESTATE, "gwl_exchange: orbitals and kernel must be set");
@@ -921,6 +1075,7 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
     // only what rho -> V rho -> dot touches: T, W and the V.T split-K partials (none of the N_vc-sized Casida buffers)
     CK(ctx->T.ensure((size_t)chunk * ldm * 8, st));
     CK(ctx->W.ensure((size_t)chunk * ldm * 8, st));
+    CK(ctx->red_cnt.ensure(gemm_red_cnt_bytes(ctx->n_sm), st));
     gwl_status rs = GWL_OK;
     // (v, m) index pairs of every rho_vm, state-major
     std::vector<int32_t> hv((size_t)n_states * ctx->n_v), hm((size_t)n_states * ctx->n_v);
@@ -1013,6 +1168,7 @@ gwl_status gwl_qp_solve(gwl_ctx* ctx, int64_t n_states, const double* eps_m, con
 gwl_status gwl_spectrum_bounds(gwl_ctx* ctx, int64_t steps, double* lam_min, double* lam_max) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: real-orbital call on a complex (gwl_tdc_create) context");
     if (steps < 2 || steps > 512 || lam_min == nullptr || lam_max == nullptr)
         return ctx->fail(GWL_EINVAL, "gwl_spectrum_bounds: need 2 <= steps <= 512 and non-NULL outputs");
     if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: orbitals, energies and kernel must be set");
@@ -1083,6 +1239,242 @@ gwl_status gwl_spectrum_bounds(gwl_ctx* ctx, int64_t steps, double* lam_min, dou
     const double b_last = (len == L) ? b[n - 1] : 0.0;  // after a breakdown the Krylov space is invariant: exact
     *lam_max = o[imax] + b_last * std::sqrt(std::max(o[3 * n + rmax], 0.0));
     *lam_min = o[imin] - b_last * std::sqrt(std::max(o[3 * n + rmin], 0.0));
+    return GWL_OK;
+}
+
+// ---- complex orbitals, k-points, Tamm-Dancoff ---------------------------------
+gwl_status gwl_tdc_set_orbitals(gwl_ctx* ctx, const double* psi_v, const double* psi_cq) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_tdc_set_orbitals: not a gwl_tdc_create context");
+    if (psi_v == nullptr || psi_cq == nullptr) return ctx->fail(GWL_EINVAL, "gwl_tdc_set_orbitals: NULL input");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const size_t nv = (size_t)ctx->n_k * ctx->n_mu * ctx->nv_k, nc = (size_t)ctx->n_k * ctx->n_mu * ctx->n_c;
+    const int64_t ldm = ctx->n_mup, lda = (int64_t)ctx->n_k * ctx->n_cp;
+    DevBuf& tmp = ctx->stage;
+    CK(tmp.ensure(std::max(nv, nc) * 16, st));
+    CK(ctx->phi_c.ensure((size_t)2 * ctx->n_mu * lda * 8, st));                       // psi_cq planar [2][n_mu][n_k n_cp]
+    CK(ctx->phi_cT.ensure((size_t)2 * ctx->n_k * ctx->n_c * ldm * 8, st));            // psi_cq^T planar [2][n_k n_c][n_mup]
+    CK(ctx->phi_vT.ensure((size_t)2 * ctx->n_kv * ldm * 8, st));                      // psi_v^T planar [2][n_kv][n_mup]
+    CK(cudaMemsetAsync(ctx->phi_c.p, 0, ctx->phi_c.bytes, st));
+    CK(cudaMemsetAsync(ctx->phi_cT.p, 0, ctx->phi_cT.bytes, st));
+    CK(cudaMemsetAsync(ctx->phi_vT.p, 0, ctx->phi_vT.bytes, st));
+    CK(cudaMemcpyAsync(tmp.p, psi_cq, nc * 16, cudaMemcpyHostToDevice, st));
+    CKL(4, launch_scatter_complex(tmp.as<double>(), ctx->n_k, ctx->n_mu, ctx->n_c, ctx->phi_c.as<double>(),
+                                  ctx->phi_c.as<double>() + (int64_t)ctx->n_mu * lda, ctx->n_cp, lda, 1, st));
+    CKL(4, launch_scatter_complex(tmp.as<double>(), ctx->n_k, ctx->n_mu, ctx->n_c, ctx->phi_cT.as<double>(),
+                                  ctx->phi_cT.as<double>() + (int64_t)ctx->n_k * ctx->n_c * ldm, (int64_t)ctx->n_c * ldm, 1,
+                                  ldm, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaMemcpyAsync(tmp.p, psi_v, nv * 16, cudaMemcpyHostToDevice, st));
+    CKL(4, launch_scatter_complex(tmp.as<double>(), ctx->n_k, ctx->n_mu, ctx->nv_k, ctx->phi_vT.as<double>(),
+                                  ctx->phi_vT.as<double>() + (int64_t)ctx->n_kv * ldm, (int64_t)ctx->nv_k * ldm, 1, ldm, st));
+    CK(cudaStreamSynchronize(st));
+    ctx->have_orb = true;
+    invalidate_run(ctx);
+    return GWL_OK;
+}
+
+gwl_status gwl_tdc_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps_cq) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_tdc_set_energies: not a gwl_tdc_create context");
+    if (eps_v == nullptr || eps_cq == nullptr) return ctx->fail(GWL_EINVAL, "gwl_tdc_set_energies: NULL input");
+    const size_t nv = (size_t)ctx->n_kv, nc = (size_t)ctx->n_k * ctx->n_c;
+    double vmax = -INFINITY, cmin = INFINITY;
+    for (size_t i = 0; i < nv; ++i) {
+        if (!std::isfinite(eps_v[i])) return ctx->fail(GWL_EINVAL, "gwl_tdc_set_energies: non-finite eps_v");
+        vmax = std::max(vmax, eps_v[i]);
+    }
+    for (size_t i = 0; i < nc; ++i) {
+        if (!std::isfinite(eps_cq[i])) return ctx->fail(GWL_EINVAL, "gwl_tdc_set_energies: non-finite eps_cq");
+        cmin = std::min(cmin, eps_cq[i]);
+    }
+    if (!(cmin > vmax)) return ctx->fail(GWL_EINVAL, "gwl_tdc_set_energies: need min(eps_cq) > max(eps_v)");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    ctx->h_eps_v.assign(eps_v, eps_v + nv);
+    ctx->h_eps_c.assign(eps_cq, eps_cq + nc);
+    CK(ctx->eps_v.ensure(nv * 8, st));
+    CK(ctx->eps_c.ensure(nc * 8, st));
+    CK(ctx->d2.ensure((size_t)ctx->n_vc * 8, st));
+    CK(ctx->s.ensure((size_t)ctx->n_vc * 8, st));
+    CK(cudaMemcpyAsync(ctx->eps_v.p, eps_v, nv * 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctx->eps_c.p, eps_cq, nc * 8, cudaMemcpyHostToDevice, st));
+    CKL(4, launch_build_delta_c(ctx->eps_v.as<double>(), ctx->eps_c.as<double>(), ctx->n_k, ctx->nv_k, ctx->n_c,
+                                ctx->d2.as<double>(), ctx->s.as<double>(), st));
+    CK(cudaStreamSynchronize(st));
+    ctx->have_eps = true;
+    invalidate_run(ctx);
+    ctx->chain_mode = 0;
+    ctx->n_chains_set = 0;
+    return GWL_OK;
+}
+
+gwl_status gwl_tdc_set_chains(gwl_ctx* ctx, int64_t n_chains, const int32_t* chains) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_tdc_set_chains: not a gwl_tdc_create context");
+    if (n_chains < 0 || (n_chains > 0 && chains == nullptr)) return ctx->fail(GWL_EINVAL, "gwl_tdc_set_chains: bad arguments");
+    if (!ctx->have_eps) return ctx->fail(GWL_ESTATE, "gwl_tdc_set_chains: energies must be set first");
+    const int n_orb = ctx->nv_k + ctx->n_c;
+    std::vector<double> eps(n_chains);
+    std::vector<int32_t> sgn(n_chains);
+    for (int64_t j = 0; j < n_chains; ++j) {
+        const int32_t kn = chains[4 * j], n = chains[4 * j + 1], km = chains[4 * j + 2], m = chains[4 * j + 3];
+        if (kn < 0 || kn >= ctx->n_k || km < 0 || km >= ctx->n_k || n < 0 || n >= n_orb || m < 0 || m >= n_orb)
+            return ctx->fail(GWL_EINVAL, "gwl_tdc_set_chains: k slot or orbital index out of range");
+        const bool occ = n < ctx->nv_k;
+        eps[j] = occ ? ctx->h_eps_v[(size_t)kn * ctx->nv_k + n] : ctx->h_eps_c[(size_t)kn * ctx->n_c + (n - ctx->nv_k)];
+        sgn[j] = occ ? 1 : -1;
+    }
+    cudaStream_t st = ctx->stream;
+    CK(ctx->d_nidx.ensure((size_t)n_chains * 16, st));
+    CK(ctx->d_eps_n.ensure((size_t)n_chains * 8, st));
+    CK(ctx->d_sgn_n.ensure((size_t)n_chains * 4, st));
+    if (n_chains > 0) {
+        CK(cudaMemcpyAsync(ctx->d_nidx.p, chains, (size_t)n_chains * 16, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->d_eps_n.p, eps.data(), (size_t)n_chains * 8, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->d_sgn_n.p, sgn.data(), (size_t)n_chains * 4, cudaMemcpyHostToDevice, st));
+    }
+    CK(cudaStreamSynchronize(st));
+    ctx->chain_mode = 1;
+    ctx->n_chains_set = n_chains;
+    invalidate_run(ctx);
+    return GWL_OK;
+}
+
+gwl_status gwl_tdc_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_tdc_matvec: not a gwl_tdc_create context");
+    if (nvec < 0) return ctx->fail(GWL_EINVAL, "gwl_tdc_matvec: nvec < 0");
+    if (nvec == 0) return GWL_OK;
+    if (x == nullptr || y == nullptr) return ctx->fail(GWL_EINVAL, "gwl_tdc_matvec: NULL vector");
+    if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_tdc_matvec: orbitals, energies and kernel must be set");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int chunk = (int)std::min<int64_t>(nvec, 128);
+    gwl_status rs = ensure_workspace(ctx, chunk);
+    if (rs != GWL_OK) return rs;
+    const int64_t n_vc = ctx->n_vc, n_kvc = n_vc / 2;  // n_vc real entries = n_kvc complex ones
+    const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
+    CK(ctx->io_x.ensure((size_t)chunk * n_vc * 8, st));  // planar copies
+    CK(ctx->io_y.ensure((size_t)chunk * n_vc * 8, st));
+    if (!ctx->device_ptrs) CK(ctx->stage.ensure((size_t)chunk * n_vc * 8, st));
+    for (int64_t j0 = 0; j0 < nvec; j0 += chunk) {
+        const int nb = (int)std::min<int64_t>(chunk, nvec - j0);
+        const double* xin = x + j0 * n_vc;
+        if (!ctx->device_ptrs) {
+            CK(cudaMemcpyAsync(ctx->stage.p, xin, (size_t)nb * n_vc * 8, cudaMemcpyHostToDevice, st));
+            xin = ctx->stage.as<double>();
+        }
+        CKL(4, launch_deinterleave(xin, n_kvc, nb, ctx->io_x.as<double>(), st));
+        CKL(4, launch_prescale(ctx->io_x.as<double>(), n_vc, ctx->xs.as<double>(), ldxs, ctx->s.as<double>(), ctx->n_v,
+                               ctx->n_c, ctx->n_cp, nb, st));
+        rs = apply_casida_core(ctx, ctx->io_x.as<double>(), n_vc, ctx->io_y.as<double>(), n_vc, nb, nullptr, 0);
+        if (rs != GWL_OK) return rs;
+        if (ctx->device_ptrs) {
+            CKL(4, launch_interleave(ctx->io_y.as<double>(), n_kvc, nb, y + j0 * n_vc, st));
+        } else {
+            CKL(4, launch_interleave(ctx->io_y.as<double>(), n_kvc, nb, ctx->stage.as<double>(), st));
+            CK(cudaMemcpyAsync(y + j0 * n_vc, ctx->stage.p, (size_t)nb * n_vc * 8, cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+        }
+    }
+    return GWL_OK;
+}
+
+// ---- ISDF front end (PAPER.md:115-128, Eq. 15-17; :319) ---------------------------------------------
+gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, const double* phi_c_grid, const double* r,
+                          double weight, double soft, const int32_t* idx, double* zeta_t, double* V_out) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_isdf_build: real-orbital call on a complex (gwl_tdc_create) context");
+    if (phi_v_grid == nullptr || phi_c_grid == nullptr || r == nullptr || idx == nullptr)
+        return ctx->fail(GWL_EINVAL, "gwl_isdf_build: NULL input");
+    if (n_r < ctx->n_mu || n_r > 65535 || !(weight > 0.0) || !(soft > 0.0))
+        return ctx->fail(GWL_EINVAL, "gwl_isdf_build: need n_mu <= n_r <= 65535, weight > 0, soft > 0");
+    const int n_mu = ctx->n_mu, n_orb = ctx->n_v + ctx->n_c, nr = (int)n_r;
+    {
+        std::vector<char> seen((size_t)n_r, 0);
+        for (int m = 0; m < n_mu; ++m) {
+            if (idx[m] < 0 || idx[m] >= n_r || seen[idx[m]])
+                return ctx->fail(GWL_EINVAL, "gwl_isdf_build: interpolation point index out of range or repeated");
+            seen[idx[m]] = 1;
+        }
+    }
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int64_t nop = round_up(n_orb, BK), nrp = round_up(n_r, BK), ldm = ctx->n_mup;
+    DevBuf &Phi = ctx->isdf_phi, &PhiMu = ctx->isdf_phimu, &Y = ctx->isdf_y, &S = ctx->isdf_s, &G = ctx->isdf_g, &U = ctx->isdf_u;
+    CK(Phi.ensure((size_t)n_r * nop * 8, st));
+    CK(PhiMu.ensure((size_t)n_mu * nop * 8 + (size_t)n_mu * n_orb * 8, st));
+    CK(Y.ensure((size_t)n_mu * nrp * 8, st));
+    CK(S.ensure((size_t)n_mu * ldm * 8 + (size_t)n_r * 24 + 8 + (size_t)n_mu * 4 + 16, st));
+    CK(G.ensure((size_t)n_r * nrp * 8, st));
+    CK(U.ensure((size_t)n_mu * nrp * 8, st));
+    CK(ctx->V.ensure((size_t)n_mu * ldm * 8, st));
+    CK(cudaMemsetAsync(Phi.p, 0, Phi.bytes, st));
+    CK(cudaMemsetAsync(PhiMu.p, 0, PhiMu.bytes, st));
+    CK(cudaMemsetAsync(Y.p, 0, Y.bytes, st));
+    CK(cudaMemsetAsync(S.p, 0, S.bytes, st));
+    CK(cudaMemsetAsync(G.p, 0, G.bytes, st));
+    CK(cudaMemsetAsync(U.p, 0, U.bytes, st));
+    CK(cudaMemsetAsync(ctx->V.p, 0, ctx->V.bytes, st));
+    double* dS = S.as<double>();
+    double* d_r = dS + (size_t)n_mu * ldm;
+    double* d_scale = d_r + (size_t)n_r * 3;
+    int32_t* d_idx = reinterpret_cast<int32_t*>(d_scale + 1);
+    int* d_info = d_idx + n_mu;
+    // all orbitals side by side, [n_r][v | c], zero-padded to a multiple of 16 columns
+    CK(cudaMemcpy2DAsync(Phi.p, (size_t)nop * 8, phi_v_grid, (size_t)ctx->n_v * 8, (size_t)ctx->n_v * 8, (size_t)n_r,
+                         cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpy2DAsync(Phi.as<double>() + ctx->n_v, (size_t)nop * 8, phi_c_grid, (size_t)ctx->n_c * 8, (size_t)ctx->n_c * 8,
+                         (size_t)n_r, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(d_r, r, (size_t)n_r * 24, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(d_idx, idx, (size_t)n_mu * 4, cudaMemcpyHostToDevice, st));
+    CKL(4, launch_gather_rows(Phi.as<double>(), nop, (int)nop, d_idx, n_mu, PhiMu.as<double>(), nop, st));
+    // P[mu][r] = sum_n phi_n(r_mu) phi_n(r);  Z C^T = P o P (pairs of ALL orbitals);  C C^T = its columns at the points
+    gwl_status rs = plain_gemm(ctx, Phi.as<double>(), nop, PhiMu.as<double>(), nop, nr, n_mu, (int)(nop / BK), Y.as<double>(),
+                               nrp, 1);
+    if (rs != GWL_OK) return rs;
+    CKL(4, launch_hadamard(Y.as<double>(), Y.as<double>(), (int64_t)n_mu * nrp, st));
+    CKL(4, launch_gather_cols(Y.as<double>(), nrp, d_idx, n_mu, dS, ldm, st));
+    // zeta^T = (C C^T)^{-1} (Z C^T)^T by Cholesky
+    CKL(4, launch_cholesky(dS, ldm, n_mu, d_scale, d_info, st));
+    int h_info = 0;
+    CK(cudaMemcpyAsync(&h_info, d_info, 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (h_info != 0)
+        return ctx->fail(GWL_EINVAL, "gwl_isdf_build: C C^T is not positive definite (pivot " + std::to_string(h_info) +
+                                         "): the interpolation points do not resolve the pair products");
+    CKL(4, launch_cholesky_solve(dS, ldm, n_mu, Y.as<double>(), nrp, nr, st));
+    // (alpha|beta) = zeta^T G zeta with the Coulomb quadrature matrix of the grid
+    CKL(4, launch_coulomb_grid(d_r, nr, weight, soft, G.as<double>(), nrp, st));
+    rs = plain_gemm(ctx, G.as<double>(), nrp, Y.as<double>(), nrp, nr, n_mu, (int)(nrp / BK), U.as<double>(), nrp, 1);
+    if (rs != GWL_OK) return rs;
+    rs = plain_gemm(ctx, Y.as<double>(), nrp, U.as<double>(), nrp, n_mu, n_mu, (int)(nrp / BK), ctx->V.as<double>(), ldm, 1);
+    if (rs != GWL_OK) return rs;
+    // the orbitals at the interpolation points become the context's orbitals
+    double* compact = PhiMu.as<double>() + (size_t)n_mu * nop;  // [n_mu][n_v] then [n_mu][n_c]
+    CK(cudaMemcpy2DAsync(compact, (size_t)ctx->n_v * 8, PhiMu.p, (size_t)nop * 8, (size_t)ctx->n_v * 8, (size_t)n_mu,
+                         cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpy2DAsync(compact + (size_t)n_mu * ctx->n_v, (size_t)ctx->n_c * 8, PhiMu.as<double>() + ctx->n_v, (size_t)nop * 8,
+                         (size_t)ctx->n_c * 8, (size_t)n_mu, cudaMemcpyDeviceToDevice, st));
+    rs = install_orbitals(ctx, compact, compact + (size_t)n_mu * ctx->n_v);
+    if (rs != GWL_OK) return rs;
+    if (zeta_t != nullptr)
+        CK(cudaMemcpy2DAsync(zeta_t, (size_t)n_r * 8, Y.p, (size_t)nrp * 8, (size_t)n_r * 8, (size_t)n_mu, cudaMemcpyDeviceToHost,
+                             st));
+    if (V_out != nullptr)
+        CK(cudaMemcpy2DAsync(V_out, (size_t)n_mu * 8, ctx->V.p, (size_t)ldm * 8, (size_t)n_mu * 8, (size_t)n_mu,
+                             cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    ctx->have_orb = true;
+    ctx->have_V = true;
+    invalidate_run(ctx);
     return GWL_OK;
 }
 

@@ -31,7 +31,7 @@ struct GemmParams {
     int64_t ldb;
     int M, N;             // valid rows of A / of B
     int kt_total;         // k-tiles (of BK) in the whole reduction
-    int a_wrap;           // A column of k-tile kt is (kt % a_wrap) * BK   (FWD: k-tiles per v)
+    int a_wrap;           // FWD: k-tiles per v (n_cp / BK); k-tile kt = (c-tile kt / n_v, v = kt % n_v)
     int kt_per_split;     // FWD/PLAIN: k-tiles handled by one blockIdx.z
     const double* scale;  // Phi_v^T [n_v][lds]: FWD row scale (index m), BWD k scale (index k)
     int64_t lds;
@@ -39,6 +39,9 @@ struct GemmParams {
     double* out;          // EPI_STORE: out[z*out_split_stride + n*ldo + m]; CASIDA/START: out[n*ldo + v*n_c + m]
     int64_t ldo;
     int64_t out_split_stride;
+    // FWD / PLAIN with splits > 1 and a co-resident grid: in-kernel reduction of the split-K partials (kr_gemm.cu)
+    unsigned* red_cnt;    // [tiles][2] arrive / done counters, zero between launches; NULL = separate reduction kernel
+    double* out_final;    // [N][ldo] the reduced result
     const double* X;      // EPI_CASIDA: x[n*ldx + v*n_c + m]
     int64_t ldx;
     const double* d2;     // diagonal term [n_vc]: Delta^2 (RPA, operator C) or Delta (TDA, operator A)
@@ -78,8 +81,44 @@ GemmPlan plan_gemm(int mode, int M, int N, int kt_total, int a_wrap, int n_sm);
 // Bytes of GemmParams::ws / ::flags a BWD launch may touch on a device with n_sm SMs.
 size_t gemm_bwd_ws_bytes(int n_sm);
 size_t gemm_bwd_flag_bytes(int n_sm);
+// True when a FWD / PLAIN launch of this plan reduces its split-K partials itself (GemmParams::red_cnt / out_final must
+// then be set; red_cnt holds 2 * tiles counters): more than one split and the whole grid resident at once.
+bool gemm_reduces_in_kernel(const GemmPlan& plan, int M, int N, int n_sm);
+size_t gemm_red_cnt_bytes(int n_sm);
 // Launches; returns cudaGetLastError().  `nz` = splits (FWD/PLAIN) or n_v (BWD).
 cudaError_t launch_gemm(int mode, int epi, const GemmPlan& plan, const GemmParams& p, int nz, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------
+// Complex GEMM layer (kr_gemm_c.cu): the two Khatri-Rao contractions of the periodic Tamm-Dancoff operator
+// A(q) = diag(Delta) + K^H V K, K[mu, (k,v,c)] = conj(psi_vk(mu)) psi_ck+q(mu).  All arrays planar.
+// ---------------------------------------------------------------------------------------------
+struct GemmParamsC {
+    const double* A;       // FWD: psi_cq planar [2][n_mu][lda = n_k*n_cp]; BWD: psi_cq^T planar [2][a_rows = n_k*n_c][lda = n_mup]
+    int64_t lda, a_plane;  // a_plane: elements between the real and the imaginary plane
+    int a_rows;
+    const double* B;       // FWD: x [N][ldb = 2*n_kv*n_cp], planes side by side; BWD: W planar [2][N][ldb]
+    int64_t ldb, b_plane;
+    int b_plane_cols;      // FWD: column offset of the imaginary plane (n_kv * n_cp)
+    int M, N;              // FWD: M = n_mu; BWD: M = n_c (rows of one k-point's conduction block)
+    int kt_total;          // FWD: n_kv * (n_cp / 16); BWD: n_mup / 16
+    int a_wrap;            // FWD: k-tiles per (k, v) = n_cp / 16
+    int kt_per_split;      // FWD: k-tiles per blockIdx.z
+    int n_v, n_c;          // occupied orbitals per k-point; conduction orbitals per k-point
+    const double* scale;   // psi_v^T planar [2][scale_rows = n_kv][lds]
+    int64_t lds, s_plane;
+    int scale_rows;
+    double* out;           // STORE: out[z*out_split_stride + n*ldo + m] (+ o_plane: imaginary); BWD: out[n*ldo + kv*n_c + m]
+    int64_t ldo, o_plane, out_split_stride;
+    const double* X;       // CASIDA: x[n*ldx + kv*n_c + m] (+ x_plane)
+    int64_t ldx, x_plane;
+    const double* d2;      // diagonal term [n_kv*n_c]
+    double coupling;
+    double* dotpart;       // [n*dot_stride + kv*tiles_m + m-tile]
+    int dot_stride;
+};
+int gemm_c_tiles_m(int M);  // m-tiles of a BWD launch (dot partials per kv)
+GemmPlan plan_gemm_c(int M, int N, int kt_total, int n_sm);  // split-K plan of the FWD product
+cudaError_t launch_gemm_c(int mode, int epi, const GemmParamsC& p, int nz, cudaStream_t st);
 
 // ---------------------------------------------------------------------------------------------
 // Vector kernels (vec_kernels.cu).  Block vectors are [nb][n_vc]; partial sums are [nb][npart].
@@ -104,6 +143,19 @@ cudaError_t launch_copy_pad(const double* src, int rows, int cols, double* dst, 
 // rho[b][mu] = phi_{n_b}(mu) * phi_{m_b}(mu), orbitals taken from PhiV^T / PhiC^T
 cudaError_t launch_rho(const double* phivT, const double* phicT, int64_t ldt, int n_v, int n_mu, const int32_t* n_idx,
                        const int32_t* m_idx, double* rho, int64_t ld_rho, int nb, cudaStream_t st);
+// Planar copies of complex (interleaved re, im) input: dst_{r,i}[k*stride_k + m*stride_m + o*stride_o] = src[k][m][o]
+cudaError_t launch_scatter_complex(const double* src, int n_k, int n_m, int n_o, double* dst_r, double* dst_i,
+                                   int64_t stride_k, int64_t stride_m, int64_t stride_o, cudaStream_t st);
+// x interleaved [nvec][n][2] <-> planar [nvec][2][n]
+cudaError_t launch_deinterleave(const double* src, int64_t n, int nvec, double* dst, cudaStream_t st);
+cudaError_t launch_interleave(const double* src, int64_t n, int nvec, double* dst, cudaStream_t st);
+// rho~_j(mu) = psi_m(mu) conj(psi_n(mu)) (planar, rows j and nb + j of rho), orbitals from the planar psi_v^T / psi_cq^T;
+// chains[j] = (k slot of n, n index, k slot of m, m index)
+cudaError_t launch_rho_c(const double* psivT, int64_t pv_plane, const double* psicT, int64_t pc_plane, int64_t ldt, int n_v,
+                         int n_c, int n_mu, const int32_t* chains, double* rho, int64_t ld_rho, int nb, cudaStream_t st);
+// d2[(part, k, v, c)] = eps_cq[k][c] - eps_v[k][v], s = 1, both planes
+cudaError_t launch_build_delta_c(const double* eps_v, const double* eps_cq, int n_k, int n_v, int n_c, double* d2,
+                                 double* s, cudaStream_t st);
 // part[b][blk] = sum over the block's slice of x[b]*y[b]
 cudaError_t launch_dot_partials(const double* x, const double* y, int64_t ld, int64_t n, int nb, double* part,
                                 int npart, cudaStream_t st);
@@ -163,14 +215,31 @@ cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const dou
 // TDA: Sigma = -sgn R_A(-sgn z), R_A by Eq. 14
 cudaError_t launch_sigma_tda(const double* alpha, const double* beta, const double* norm2, const int32_t* len,
                              int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
-                             int n_omega, double eta, double* sigma, cudaStream_t st);
-cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, double* sigma_sum, cudaStream_t st);
+                             int n_omega, double eta, double prefactor, double* sigma, cudaStream_t st);
+// sigma_sum[w] (+)= sum over the chains (Eq. 10), fixed order; accumulate = 1 adds to what sigma_sum holds
+cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, double* sigma_sum, int accumulate,
+                             cudaStream_t st);
 // out[0] = (first ? 0 : out[0]) - sum(part[0..count)) in a fixed order (Eq. 6 accumulation)
 cudaError_t launch_accum_neg(const double* part, int count, double* out, int first, cudaStream_t st);
 // Newton-Raphson solve of E(omega) = omega on the grid, one thread per state
 cudaError_t launch_qp_solve(int n_states, const double* eps_m, const double* vxc_m, const double* sigma_x,
                             const double* sigma_c, const double* omega, int n_omega, double* e_qp, double* z_qp,
                             int32_t* iters, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------
+// ISDF front end (isdf.cu): gathers, Hadamard product, Coulomb quadrature matrix, Cholesky factorisation and solves.
+// ---------------------------------------------------------------------------------------------
+cudaError_t launch_gather_rows(const double* src, int64_t ld_src, int n_cols, const int32_t* idx, int n_mu, double* dst,
+                               int64_t ld_dst, cudaStream_t st);
+cudaError_t launch_hadamard(double* y, const double* x, int64_t n, cudaStream_t st);
+cudaError_t launch_gather_cols(const double* Y, int64_t ld_y, const int32_t* idx, int n_mu, double* S, int64_t ld_s,
+                               cudaStream_t st);
+cudaError_t launch_coulomb_grid(const double* r, int n_r, double weight, double soft, double* G, int64_t ld, cudaStream_t st);
+// S = L L^T in place (lower triangle, upper zeroed inside the diagonal blocks); *info (zero on entry) = 1-based index of the
+// first pivot that is not above 1e-13 max_i S_ii (scale: one device double of scratch)
+cudaError_t launch_cholesky(double* S, int64_t ld, int n, double* scale, int* info, cudaStream_t st);
+// X <- (L L^T)^{-1} X for X [n][ldx] with n_r columns
+cudaError_t launch_cholesky_solve(const double* L, int64_t ldl, int n, double* X, int64_t ldx, int n_r, cudaStream_t st);
 
 // probe.cu
 cudaError_t probe_fp64_peak(int kind, double* tflops);

@@ -1,0 +1,293 @@
+// Interpolative separable density fitting front end, PAPER.md:115-128 (Eq. 15-17) and :319:
+//   phi_n(r) phi_m(r) ~ sum_mu zeta_mu(r) C^mu_nm,  C^mu_nm = phi_n(r_mu) phi_m(r_mu)                         (Eq. 15)
+//   zeta = Z C^T (C C^T)^{-1}  (least squares at given interpolation points r_mu = r[idx[mu]], refs. [62, 63]) with the
+//   separable normal equations  Z C^T = (Phi Phi_mu^T) o (Phi Phi_mu^T),  C C^T = the same at the interpolation points,
+//   (alpha|beta) = int int zeta_alpha(r) zeta_beta(r') / |r - r'|  -> zeta^T G zeta on the grid quadrature        (Eq. 17)
+// The dense contractions (Gram products, G zeta, zeta^T (G zeta)) run on the DMMA GEMM of kr_gemm.cu (MODE_PLAIN); this
+// file holds what is left: gathers, the Hadamard product, the Coulomb quadrature matrix, and a blocked Cholesky
+// factorisation with its two triangular solves for N_r right-hand sides.  Everything FP64; zeta is kept transposed,
+// zeta_t[mu][r], which is both the GEMM operand layout and the row-block layout of the solves.
+#include <algorithm>
+
+#include "gwl_internal.h"
+
+namespace gwl {
+
+namespace {
+
+constexpr int NB = 32;  // Cholesky / solve block size
+
+__global__ void k_gather_rows(const double* __restrict__ src, int64_t ld_src, int n_cols, const int32_t* __restrict__ idx,
+                              double* __restrict__ dst, int64_t ld_dst) {
+    const int mu = blockIdx.x;
+    const double* s = src + (int64_t)idx[mu] * ld_src;
+    for (int j = threadIdx.x; j < n_cols; j += blockDim.x) dst[(int64_t)mu * ld_dst + j] = s[j];
+}
+
+// y[mu][r] *= x[mu][r]
+__global__ void k_hadamard(double* __restrict__ y, const double* __restrict__ x, int64_t n) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] *= x[i];
+}
+
+// S[mu][nu] = Y[mu][idx[nu]]   (C C^T = Z C^T sampled at the interpolation points)
+__global__ void k_gather_cols(const double* __restrict__ Y, int64_t ld_y, const int32_t* __restrict__ idx, int n_mu,
+                              double* __restrict__ S, int64_t ld_s) {
+    const int mu = blockIdx.x;
+    for (int nu = threadIdx.x; nu < n_mu; nu += blockDim.x) S[(int64_t)mu * ld_s + nu] = Y[(int64_t)mu * ld_y + idx[nu]];
+}
+
+// G[i][j] = w^2 * 14.4 / sqrt(|r_i - r_j|^2 + soft^2): the grid quadrature of 1/|r - r'| (eV Angstrom)
+__global__ void k_coulomb_grid(const double* __restrict__ r, int n_r, double w2, double soft2, double* __restrict__ G,
+                               int64_t ld) {
+    const int i = blockIdx.y;
+    const double xi = r[3 * i], yi = r[3 * i + 1], zi = r[3 * i + 2];
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n_r; j += gridDim.x * blockDim.x) {
+        const double dx = xi - r[3 * j], dy = yi - r[3 * j + 1], dz = zi - r[3 * j + 2];
+        G[(int64_t)i * ld + j] = w2 * 14.4 / sqrt(dx * dx + dy * dy + dz * dz + soft2);
+    }
+}
+
+// ---- blocked right-looking Cholesky, lower triangle in place: S = L L^T ---------------------------------------------
+// (a) diagonal block: one CTA of NB x NB threads, column by column in shared memory
+// scale[0] = max_i S[i][i]: pivots below 1e-13 of it count as "not positive definite" (an exactly singular C C^T
+// leaves pivots of either sign at rounding level)
+__global__ void k_max_diag(const double* __restrict__ S, int64_t ld, int n, double* __restrict__ scale) {
+    __shared__ double sh[256];
+    double m = 0.0;
+    for (int i = threadIdx.x; i < n; i += 256) m = fmax(m, S[(int64_t)i * ld + i]);
+    sh[threadIdx.x] = m;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] = fmax(sh[threadIdx.x], sh[threadIdx.x + o]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) scale[0] = sh[0];
+}
+
+__global__ void k_chol_diag(double* __restrict__ S, int64_t ld, int n, int k0, const double* __restrict__ scale,
+                            int* __restrict__ info) {
+    __shared__ double a[NB][NB + 1];
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int nb = min(NB, n - k0);
+    a[ty][tx] = (ty < nb && tx < nb) ? S[(int64_t)(k0 + ty) * ld + k0 + tx] : (ty == tx ? 1.0 : 0.0);
+    __syncthreads();
+    for (int j = 0; j < nb; ++j) {
+        if (tx == 0 && ty == 0) {
+            const double d = a[j][j];
+            if (!(d > 1e-13 * scale[0])) {
+                if (*info == 0) *info = k0 + j + 1;
+                a[j][j] = 1.0;
+            } else {
+                a[j][j] = sqrt(d);
+            }
+        }
+        __syncthreads();
+        if (tx == 0 && ty > j) a[ty][j] /= a[j][j];
+        __syncthreads();
+        if (tx > j && ty >= tx) a[ty][tx] -= a[ty][j] * a[tx][j];
+        __syncthreads();
+    }
+    if (ty < nb && tx < nb) S[(int64_t)(k0 + ty) * ld + k0 + tx] = (tx <= ty) ? a[ty][tx] : 0.0;
+}
+
+// (b) panel below the diagonal block: L_ik = A_ik L_kk^{-T}, one row per thread
+__global__ void k_chol_panel(double* __restrict__ S, int64_t ld, int n, int k0) {
+    __shared__ double l[NB][NB + 1];
+    const int nb = min(NB, n - k0);
+    for (int t = threadIdx.x; t < NB * NB; t += blockDim.x) {
+        const int i = t / NB, j = t % NB;
+        l[i][j] = (i < nb && j < nb) ? S[(int64_t)(k0 + i) * ld + k0 + j] : (i == j ? 1.0 : 0.0);
+    }
+    __syncthreads();
+    const int row = k0 + nb + blockIdx.x * blockDim.x + threadIdx.x;
+    if (row >= n) return;
+    double x[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) x[j] = j < nb ? S[(int64_t)row * ld + k0 + j] : 0.0;
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+        double v = x[j];
+#pragma unroll
+        for (int t = 0; t < NB; ++t)
+            if (t < j) v -= x[t] * l[j][t];
+        x[j] = v / l[j][j];
+    }
+#pragma unroll
+    for (int j = 0; j < NB; ++j)
+        if (j < nb) S[(int64_t)row * ld + k0 + j] = x[j];
+}
+
+// (c) trailing update of the lower triangle: A_ij -= sum_t L_it L_jt, 32 x 32 tile per CTA
+__global__ void k_chol_update(double* __restrict__ S, int64_t ld, int n, int k0) {
+    const int nb = min(NB, n - k0);
+    const int bi = blockIdx.y, bj = blockIdx.x;
+    if (bj > bi) return;
+    const int base = k0 + nb;
+    __shared__ double li[NB][NB + 1], lj[NB][NB + 1];
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int ri = base + bi * NB + ty, rj = base + bj * NB + ty;
+    li[ty][tx] = (ri < n && tx < nb) ? S[(int64_t)ri * ld + k0 + tx] : 0.0;
+    lj[ty][tx] = (rj < n && tx < nb) ? S[(int64_t)rj * ld + k0 + tx] : 0.0;
+    __syncthreads();
+    const int i = base + bi * NB + ty, j = base + bj * NB + tx;
+    if (i >= n || j >= n || j > i) return;
+    double acc = 0.0;
+#pragma unroll
+    for (int t = 0; t < NB; ++t) acc += li[ty][t] * lj[tx][t];
+    S[(int64_t)i * ld + j] -= acc;
+}
+
+// ---- triangular solves with n_r right-hand sides, X[mu][r] in place -------------------------------------------------
+// forward (L Z = Y), block row k: Z_k = L_kk^{-1} (Y_k - sum_{j<k} L_kj Z_j); one column r per thread, NB accumulators
+__global__ void k_trsm_fwd(const double* __restrict__ L, int64_t ldl, int n, double* __restrict__ X, int64_t ldx, int n_r,
+                           int k0) {
+    __shared__ double l[NB][NB + 1];
+    const int nb = min(NB, n - k0);
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    double acc[NB];
+#pragma unroll
+    for (int i = 0; i < NB; ++i) acc[i] = (i < nb && c < n_r) ? X[(int64_t)(k0 + i) * ldx + c] : 0.0;
+    for (int j0 = 0; j0 < k0; j0 += NB) {
+        __syncthreads();
+        for (int t = threadIdx.x; t < NB * NB; t += blockDim.x) {
+            const int i = t / NB, j = t % NB;
+            l[i][j] = i < nb ? L[(int64_t)(k0 + i) * ldl + j0 + j] : 0.0;
+        }
+        __syncthreads();
+        if (c < n_r) {
+#pragma unroll 4
+            for (int j = 0; j < NB; ++j) {
+                const double xj = X[(int64_t)(j0 + j) * ldx + c];
+#pragma unroll
+                for (int i = 0; i < NB; ++i) acc[i] -= l[i][j] * xj;
+            }
+        }
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < NB * NB; t += blockDim.x) {
+        const int i = t / NB, j = t % NB;
+        l[i][j] = (i < nb && j < nb) ? L[(int64_t)(k0 + i) * ldl + k0 + j] : (i == j ? 1.0 : 0.0);
+    }
+    __syncthreads();
+    if (c >= n_r) return;
+#pragma unroll
+    for (int i = 0; i < NB; ++i) {
+        double v = acc[i];
+#pragma unroll
+        for (int t = 0; t < NB; ++t)
+            if (t < i) v -= l[i][t] * acc[t];
+        acc[i] = v / l[i][i];
+    }
+#pragma unroll
+    for (int i = 0; i < NB; ++i)
+        if (i < nb) X[(int64_t)(k0 + i) * ldx + c] = acc[i];
+}
+
+// backward (L^T X = Z), block row k from the bottom: X_k = L_kk^{-T} (Z_k - sum_{j>k} L_jk^T X_j)
+__global__ void k_trsm_bwd(const double* __restrict__ L, int64_t ldl, int n, double* __restrict__ X, int64_t ldx, int n_r,
+                           int k0) {
+    __shared__ double l[NB][NB + 1];
+    const int nb = min(NB, n - k0);
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    double acc[NB];
+#pragma unroll
+    for (int i = 0; i < NB; ++i) acc[i] = (i < nb && c < n_r) ? X[(int64_t)(k0 + i) * ldx + c] : 0.0;
+    for (int j0 = k0 + nb; j0 < n; j0 += NB) {
+        const int njb = min(NB, n - j0);
+        __syncthreads();
+        for (int t = threadIdx.x; t < NB * NB; t += blockDim.x) {
+            const int j = t / NB, i = t % NB;  // l[j][i] = L[j0 + j][k0 + i]
+            l[j][i] = (j < njb && i < nb) ? L[(int64_t)(j0 + j) * ldl + k0 + i] : 0.0;
+        }
+        __syncthreads();
+        if (c < n_r) {
+            for (int j = 0; j < njb; ++j) {
+                const double xj = X[(int64_t)(j0 + j) * ldx + c];
+#pragma unroll
+                for (int i = 0; i < NB; ++i) acc[i] -= l[j][i] * xj;
+            }
+        }
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < NB * NB; t += blockDim.x) {
+        const int i = t / NB, j = t % NB;
+        l[i][j] = (i < nb && j < nb) ? L[(int64_t)(k0 + i) * ldl + k0 + j] : (i == j ? 1.0 : 0.0);
+    }
+    __syncthreads();
+    if (c >= n_r) return;
+#pragma unroll
+    for (int i = NB - 1; i >= 0; --i) {
+        double v = acc[i];
+#pragma unroll
+        for (int t = 0; t < NB; ++t)
+            if (t > i) v -= l[t][i] * acc[t];
+        acc[i] = v / l[i][i];
+    }
+#pragma unroll
+    for (int i = 0; i < NB; ++i)
+        if (i < nb) X[(int64_t)(k0 + i) * ldx + c] = acc[i];
+}
+
+}  // namespace
+
+cudaError_t launch_gather_rows(const double* src, int64_t ld_src, int n_cols, const int32_t* idx, int n_mu, double* dst,
+                               int64_t ld_dst, cudaStream_t st) {
+    k_gather_rows<<<(unsigned)n_mu, 128, 0, st>>>(src, ld_src, n_cols, idx, dst, ld_dst);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hadamard(double* y, const double* x, int64_t n, cudaStream_t st) {
+    const unsigned g = (unsigned)std::max<int64_t>(1, std::min<int64_t>(ceil_div(n, 1024), (int64_t)device_sm_count() * 16));
+    k_hadamard<<<g, 256, 0, st>>>(y, x, n);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gather_cols(const double* Y, int64_t ld_y, const int32_t* idx, int n_mu, double* S, int64_t ld_s,
+                               cudaStream_t st) {
+    k_gather_cols<<<(unsigned)n_mu, 128, 0, st>>>(Y, ld_y, idx, n_mu, S, ld_s);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_coulomb_grid(const double* r, int n_r, double weight, double soft, double* G, int64_t ld, cudaStream_t st) {
+    dim3 grid((unsigned)std::min<int64_t>(ceil_div(n_r, 256), 64), (unsigned)n_r);
+    if (n_r > 65535) return cudaErrorInvalidValue;
+    k_coulomb_grid<<<grid, 256, 0, st>>>(r, n_r, weight * weight, soft * soft, G, ld);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cholesky(double* S, int64_t ld, int n, double* scale, int* info, cudaStream_t st) {
+    k_max_diag<<<1, 256, 0, st>>>(S, ld, n, scale);
+    count_launch();
+    for (int k0 = 0; k0 < n; k0 += NB) {
+        const int nb = std::min(NB, n - k0);
+        k_chol_diag<<<1, dim3(NB, NB), 0, st>>>(S, ld, n, k0, scale, info);
+        const int rest = n - k0 - nb;
+        if (rest > 0) {
+            k_chol_panel<<<(unsigned)ceil_div(rest, 128), 128, 0, st>>>(S, ld, n, k0);
+            const unsigned nt = (unsigned)ceil_div(rest, NB);
+            k_chol_update<<<dim3(nt, nt), dim3(NB, NB), 0, st>>>(S, ld, n, k0);
+            count_launch(2);
+        }
+        count_launch();
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cholesky_solve(const double* L, int64_t ldl, int n, double* X, int64_t ldx, int n_r, cudaStream_t st) {
+    const unsigned g = (unsigned)ceil_div(n_r, 128);
+    for (int k0 = 0; k0 < n; k0 += NB) {
+        k_trsm_fwd<<<g, 128, 0, st>>>(L, ldl, n, X, ldx, n_r, k0);
+        count_launch();
+    }
+    for (int k0 = (n - 1) / NB * NB; k0 >= 0; k0 -= NB) {
+        k_trsm_bwd<<<g, 128, 0, st>>>(L, ldl, n, X, ldx, n_r, k0);
+        count_launch();
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace gwl

@@ -10,11 +10,7 @@
 // Tiles are staged in shared memory as 128-byte rows (16 doubles) with the TMA SWIZZLE_128B pattern
 // (16-byte chunk index XOR (row & 7)); fragment rows are interleaved (row = 2*g + parity) so that every
 // LDS.64 of a half-warp touches 16 distinct 8-byte bank pairs.
-#include <cuda.h>
-
-#include <cstdlib>
-
-#include "gwl_internal.h"
+#include "kr_gemm_common.cuh"
 
 namespace gwl {
 
@@ -22,45 +18,7 @@ thread_local int64_t* g_launch_counter = nullptr;
 
 namespace {
 
-// ---- TMA / mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS) ---------------------------------
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
-    uint32_t ok;
-    asm volatile(
-        "{\n.reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, p;\n}\n"
-        : "=r"(ok)
-        : "r"(bar), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(dst),
-        "l"(map), "r"(c0), "r"(c1), "r"(bar)
-        : "memory");
-}
-__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
-    asm volatile("prefetch.tensormap [%0];\n" ::"l"(map) : "memory");
-}
-
-// volatile: keeps the DMMAs of a k-step in program order (A fragment outer, B inner).  Without it ptxas scrambled the
-// order in the K.X kernel (no operand reuse, accumulators out of sequence); in order, K.X runs as fast as K^T.W.
-__device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-        : "+d"(c0), "+d"(c1)
-        : "d"(a), "d"(b));
-}
-
+constexpr int FWD_VCHUNK = 64;   // K.X k-tile order: occupied orbitals per chunk (see the producer loop)
 constexpr int BWD_MIN_UNITS = 16;  // fewest k-tiles worth handing to one more CTA
 
 template <int BM, int BN, int MODE>
@@ -197,13 +155,25 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                     const uint32_t sA = smem_base + slot * TC::KT_BYTES;
                     const uint32_t sB = sA + TC::A_BYTES;
                     const uint32_t sS = sB + TC::B_BYTES;
-                    const int a_col = (MODE == MODE_FWD ? (kt % p.a_wrap) : kt) * BK;
-                    tma_load_2d(sA, &tmA, a_col, m0, fb);
-                    tma_load_2d(sB, &tmB, kt * BK, n0, fb);
-                    if (MODE == MODE_FWD)
-                        tma_load_2d(sS, &tmS, m0, kt / p.a_wrap, fb);
-                    else if (MODE == MODE_BWD)
-                        tma_load_2d(sS, &tmS, kt * BK, z, fb);
+                    if (MODE == MODE_FWD) {
+                        // k-tile order (chunk of FWD_VCHUNK occupied orbitals, c-tile, v in chunk).  The A tile (Phi_c rows of
+                        // this m-tile, 16 columns) is the same for a whole run of v and is an L2 hit, one chunk's row scales
+                        // (FWD_VCHUNK x BM doubles = 64 KB) stay in L2 over all c-tiles, and Phi_c is streamed once per chunk.
+                        // DRAM reads of one launch at config 4 (ncu): v outermost (round 1) 703 GB -- every CTA re-streamed
+                        // its slice of Phi_c once per v --, v innermost 58.7 GB (the row scales once per c-tile), against
+                        // about 5 GB algorithmic.  The B tile is xs[:, v, c-tile]: a strided walk over xs, read once either way.
+                        const int per_chunk = p.a_wrap * FWD_VCHUNK;
+                        const int chunk = kt / per_chunk, rem = kt - chunk * per_chunk;
+                        const int vlen = min(FWD_VCHUNK, p.scale_rows - chunk * FWD_VCHUNK);
+                        const int ct = rem / vlen, v = chunk * FWD_VCHUNK + (rem - ct * vlen);
+                        tma_load_2d(sA, &tmA, ct * BK, m0, fb);
+                        tma_load_2d(sB, &tmB, (v * p.a_wrap + ct) * BK, n0, fb);
+                        tma_load_2d(sS, &tmS, m0, v, fb);
+                    } else {
+                        tma_load_2d(sA, &tmA, kt * BK, m0, fb);
+                        tma_load_2d(sB, &tmB, kt * BK, n0, fb);
+                        if (MODE == MODE_BWD) tma_load_2d(sS, &tmS, kt * BK, z, fb);
+                    }
                 }
             }
         }
@@ -336,6 +306,63 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                             if (r0 + 1 < p.M) ptr[1] = v1;
                         }
                     }
+            }
+            if (p.red_cnt != nullptr) {
+                // ---- in-kernel split-K reduction (whole grid co-resident: grid <= SM count, checked by the launcher) ----
+                // Every split of a tile stores its partial, raises the tile's counter and waits until all S splits have
+                // arrived; split z then sums ITS share of the tile over the partials in the fixed order 0..S-1 and writes
+                // the result: deterministic, and the separate reduction launch (and its two kernel boundaries) is gone.
+                // The last split to finish resets both counters, so that they are zero again at the next launch.
+                const int S = (int)gridDim.z;
+                const int tile = (int)(blockIdx.y * gridDim.x + blockIdx.x);
+                unsigned* arrive = p.red_cnt + 2 * tile;
+                unsigned* done = arrive + 1;
+                __threadfence();
+                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
+                if (tid == 0) {
+                    asm volatile("red.release.gpu.global.add.u32 [%0], 1;\n" ::"l"(arrive) : "memory");
+                    unsigned c;
+                    do {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(c) : "l"(arrive) : "memory");
+                    } while (c < (unsigned)S);
+                }
+                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
+                const int rows_m = min(BM, p.M - m0), cols_n = min(BN, p.N - n0);
+                const int half = (rows_m + 1) >> 1;  // items of two adjacent m (16-byte accesses; ldo and M tiles are even)
+                const int items = half * cols_n;
+                const bool v2 = ((p.ldo & 1) == 0) && ((p.out_split_stride & 1) == 0) &&
+                                (((reinterpret_cast<uintptr_t>(p.out) | reinterpret_cast<uintptr_t>(p.out_final)) & 15) == 0);
+                for (int idx = z * (NCW * 32) + tid; idx < items; idx += S * (NCW * 32)) {
+                    const int n = idx / half, m = 2 * (idx - n * half);
+                    const int64_t off = (int64_t)(n0 + n) * p.ldo + m0 + m;
+                    const bool two = (m + 1 < rows_m);
+                    double a0 = 0.0, a1 = 0.0;
+                    if (v2 && two) {
+                        for (int zz = 0; zz < S; ++zz) {
+                            const double2 t2 = __ldcg(reinterpret_cast<const double2*>(p.out + (int64_t)zz * p.out_split_stride + off));
+                            a0 += t2.x;
+                            a1 += t2.y;
+                        }
+                        *reinterpret_cast<double2*>(p.out_final + off) = make_double2(a0, a1);
+                    } else {
+                        for (int zz = 0; zz < S; ++zz) {
+                            const double* pp = p.out + (int64_t)zz * p.out_split_stride + off;
+                            a0 += __ldcg(pp);
+                            if (two) a1 += __ldcg(pp + 1);
+                        }
+                        p.out_final[off] = a0;
+                        if (two) p.out_final[off + 1] = a1;
+                    }
+                }
+                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");  // all reads of the partials are done
+                if (tid == 0) {
+                    const unsigned d = atomicAdd(done, 1u);
+                    if (d == (unsigned)S - 1) {  // everybody of this tile has read its share: reset for the next launch
+                        *done = 0u;
+                        __threadfence();
+                        *arrive = 0u;
+                    }
+                }
             }
         } else {
             // ---- stream-K hand-over: partial tiles go through the workspace, in accumulator order -------------
@@ -589,39 +616,6 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
     }
 }
 
-using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                             const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                             CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-// cuTensorMapEncodeTiled through the runtime's driver entry point: libgwl.so has no link-time dependency on libcuda.
-EncodeFn get_encode_fn() {
-    static EncodeFn fn = nullptr;
-    if (fn == nullptr) {
-        void* ptr = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
-            qres == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeFn>(ptr);
-    }
-    return fn;
-}
-
-// 2-D FP64 tensor map over a row-major [rows][ld] array of which `cols` columns are valid; out-of-bounds
-// elements of a box read as zero.
-cudaError_t make_map(CUtensorMap* m, const double* base, uint64_t cols, uint64_t rows, uint64_t ld, uint32_t box_cols,
-                     uint32_t box_rows, bool swizzle) {
-    EncodeFn enc = get_encode_fn();
-    if (enc == nullptr) return cudaErrorNotSupported;
-    cuuint64_t dims[2] = {cols, rows};
-    cuuint64_t strides[1] = {ld * sizeof(double)};
-    cuuint32_t box[2] = {box_cols, box_rows};
-    cuuint32_t estr[2] = {1, 1};
-    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base), dims, strides, box, estr,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
-                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
-}
-
 template <int BM, int BN, int WM, int WN, int STAGES, int MODE, int EPI, int CREGS>
 cudaError_t launch_one(const GemmParams& p, dim3 grid, cudaStream_t st) {
     using TC = TileCfg<BM, BN, MODE>;
@@ -676,6 +670,12 @@ cudaError_t launch_mode(const GemmPlan& plan, const GemmParams& p0, int nz, cuda
 }
 
 }  // namespace
+
+bool gemm_reduces_in_kernel(const GemmPlan& plan, int M, int N, int n_sm) {
+    const int64_t tiles = ceil_div(M, plan.bm) * ceil_div(N, plan.bn);
+    return plan.splits > 1 && tiles * plan.splits <= n_sm;
+}
+size_t gemm_red_cnt_bytes(int n_sm) { return (size_t)2 * n_sm * sizeof(unsigned); }
 
 size_t gemm_bwd_ws_bytes(int n_sm) { return (size_t)n_sm * 128 * 128 * sizeof(double); }
 size_t gemm_bwd_flag_bytes(int n_sm) { return (size_t)n_sm * sizeof(unsigned); }

@@ -205,7 +205,8 @@ __global__ void k_sigma_poly(const double* __restrict__ alpha, const double* __r
 __global__ void k_sigma_tda(const double* __restrict__ alpha, const double* __restrict__ beta,
                             const double* __restrict__ norm2, const int32_t* __restrict__ len, int steps,
                             const double* __restrict__ eps_n, const int32_t* __restrict__ sgn_n,
-                            const double* __restrict__ omega, int n_omega, double eta, double* __restrict__ sigma) {
+                            const double* __restrict__ omega, int n_omega, double eta, double prefactor,
+                            double* __restrict__ sigma) {
     const int j = blockIdx.y;
     const int iw = blockIdx.x * blockDim.x + threadIdx.x;
     if (iw >= n_omega) return;
@@ -213,15 +214,15 @@ __global__ void k_sigma_tda(const double* __restrict__ alpha, const double* __re
     const cplx z{omega[iw] - eps_n[j], -sg * eta};
     const cplx r = contfrac_eval(alpha + (int64_t)j * steps, beta + (int64_t)j * steps, len[j], norm2[j],
                                  cplx{-sg * z.re, -sg * z.im});
-    sigma[((int64_t)j * n_omega + iw) * 2] = -sg * r.re;
-    sigma[((int64_t)j * n_omega + iw) * 2 + 1] = -sg * r.im;
+    sigma[((int64_t)j * n_omega + iw) * 2] = -sg * prefactor * r.re;
+    sigma[((int64_t)j * n_omega + iw) * 2 + 1] = -sg * prefactor * r.im;
 }
 
 __global__ void k_sigma_sum(const double* __restrict__ sigma, int n_chains, int n_omega,
-                            double* __restrict__ sigma_sum) {
+                            double* __restrict__ sigma_sum, int accumulate) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;  // over 2*n_omega reals
     if (i >= 2 * n_omega) return;
-    double acc = 0.0;
+    double acc = accumulate ? sigma_sum[i] : 0.0;
     for (int j = 0; j < n_chains; ++j) acc += sigma[(int64_t)j * n_omega * 2 + i];
     sigma_sum[i] = acc;
 }
@@ -343,21 +344,22 @@ cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const dou
 
 cudaError_t launch_sigma_tda(const double* alpha, const double* beta, const double* norm2, const int32_t* len,
                              int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
-                             int n_omega, double eta, double* sigma, cudaStream_t st) {
+                             int n_omega, double eta, double prefactor, double* sigma, cudaStream_t st) {
     if (n_chains <= 0 || n_omega <= 0) return cudaSuccess;
     for (int j0 = 0; j0 < n_chains; j0 += MAX_GRID_Y) {
         const int nc = std::min(MAX_GRID_Y, n_chains - j0);
         dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)nc);
         k_sigma_tda<<<grid, 128, 0, st>>>(alpha + (int64_t)j0 * steps, beta + (int64_t)j0 * steps, norm2 + j0, len + j0, steps,
-                                  eps_n + j0, sgn_n + j0, omega, n_omega, eta, sigma + (int64_t)j0 * n_omega * 2);
+                                  eps_n + j0, sgn_n + j0, omega, n_omega, eta, prefactor, sigma + (int64_t)j0 * n_omega * 2);
         count_launch();
     }
     return cudaGetLastError();
 }
 
-cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, double* sigma_sum, cudaStream_t st) {
+cudaError_t launch_sigma_sum(const double* sigma, int n_chains, int n_omega, double* sigma_sum, int accumulate,
+                             cudaStream_t st) {
     if (n_omega <= 0) return cudaSuccess;
-    k_sigma_sum<<<(unsigned)ceil_div(2 * n_omega, 128), 128, 0, st>>>(sigma, n_chains, n_omega, sigma_sum);
+    k_sigma_sum<<<(unsigned)ceil_div(2 * n_omega, 128), 128, 0, st>>>(sigma, n_chains, n_omega, sigma_sum, accumulate);
     count_launch();
     return cudaGetLastError();
 }

@@ -468,6 +468,68 @@ __global__ void __launch_bounds__(NT) k_reorth_apply(const double* __restrict__ 
     }
 }
 
+// ---- complex (planar) helpers of the periodic Tamm-Dancoff variant -------------------------------------------------
+__global__ void k_scatter_complex(const double* __restrict__ src, int n_k, int n_m, int n_o, double* __restrict__ dst_r,
+                                  double* __restrict__ dst_i, int64_t stride_k, int64_t stride_m, int64_t stride_o) {
+    const int64_t n = (int64_t)n_k * n_m * n_o;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t o = i % n_o, m = (i / n_o) % n_m, k = i / ((int64_t)n_o * n_m);
+        const int64_t d = k * stride_k + m * stride_m + o * stride_o;
+        dst_r[d] = src[2 * i];
+        dst_i[d] = src[2 * i + 1];
+    }
+}
+
+__global__ void k_deinterleave(const double* __restrict__ src, int64_t n, double* __restrict__ dst) {
+    const int b = blockIdx.y;
+    const double2* s2 = reinterpret_cast<const double2*>(src) + (int64_t)b * n;
+    double* d = dst + (int64_t)b * 2 * n;
+    for (int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x; i < n; i += (int64_t)gridDim.x * NT) {
+        const double2 v = s2[i];
+        d[i] = v.x;
+        d[n + i] = v.y;
+    }
+}
+
+__global__ void k_interleave(const double* __restrict__ src, int64_t n, double* __restrict__ dst) {
+    const int b = blockIdx.y;
+    const double* s = src + (int64_t)b * 2 * n;
+    double2* d2 = reinterpret_cast<double2*>(dst) + (int64_t)b * n;
+    for (int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x; i < n; i += (int64_t)gridDim.x * NT)
+        d2[i] = make_double2(s[i], s[n + i]);
+}
+
+__global__ void k_rho_c(const double* __restrict__ psivT, int64_t pv_plane, const double* __restrict__ psicT,
+                        int64_t pc_plane, int64_t ldt, int n_v, int n_c, int n_mu, const int32_t* __restrict__ chains,
+                        double* __restrict__ rho, int64_t ld_rho, int nb) {
+    pdl_trigger();
+    pdl_wait();
+    const int b = blockIdx.y;
+    const int kn = chains[4 * b], n = chains[4 * b + 1], km = chains[4 * b + 2], m = chains[4 * b + 3];
+    const double* pn = n < n_v ? psivT + ((int64_t)kn * n_v + n) * ldt : psicT + ((int64_t)kn * n_c + (n - n_v)) * ldt;
+    const double* pm = m < n_v ? psivT + ((int64_t)km * n_v + m) * ldt : psicT + ((int64_t)km * n_c + (m - n_v)) * ldt;
+    const int64_t pln = n < n_v ? pv_plane : pc_plane, plm = m < n_v ? pv_plane : pc_plane;
+    for (int i = blockIdx.x * NT + threadIdx.x; i < n_mu; i += gridDim.x * NT) {
+        const double nr = pn[i], ni = pn[pln + i], mr = pm[i], mi = pm[plm + i];
+        // psi_m conj(psi_n)
+        rho[(int64_t)b * ld_rho + i] = mr * nr + mi * ni;
+        rho[(int64_t)(nb + b) * ld_rho + i] = mi * nr - mr * ni;
+    }
+}
+
+__global__ void k_build_delta_c(const double* __restrict__ eps_v, const double* __restrict__ eps_cq, int n_k, int n_v,
+                                int n_c, double* __restrict__ d2, double* __restrict__ s) {
+    const int64_t n = (int64_t)n_k * n_v * n_c;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int c = (int)(i % n_c), v = (int)((i / n_c) % n_v), k = (int)(i / ((int64_t)n_c * n_v));
+        const double d = eps_cq[(int64_t)k * n_c + c] - eps_v[(int64_t)k * n_v + v];
+        d2[i] = d;
+        d2[n + i] = d;
+        s[i] = 1.0;
+        s[n + i] = 1.0;
+    }
+}
+
 // x[i] = uniform in [-1, 1) from a counter-based hash (splitmix64 finaliser) of (seed, i): a generic start vector
 __global__ void k_fill_hash(double* __restrict__ x, int64_t n, unsigned long long seed) {
     for (int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x; i < n; i += (int64_t)gridDim.x * NT) {
@@ -491,6 +553,44 @@ int vec_parts(int64_t n_vc) { return (int)std::max<int64_t>(1, std::min<int64_t>
 cudaError_t launch_build_delta(const double* eps_v, const double* eps_c, int n_v, int n_c, double* d2, double* s,
                                int tda, cudaStream_t st) {
     k_build_delta<<<grid1d((int64_t)n_v * n_c, 1), NT, 0, st>>>(eps_v, eps_c, n_v, n_c, d2, s, tda);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scatter_complex(const double* src, int n_k, int n_m, int n_o, double* dst_r, double* dst_i,
+                                   int64_t stride_k, int64_t stride_m, int64_t stride_o, cudaStream_t st) {
+    k_scatter_complex<<<grid1d((int64_t)n_k * n_m * n_o, 1), NT, 0, st>>>(src, n_k, n_m, n_o, dst_r, dst_i, stride_k, stride_m,
+                                                                          stride_o);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_deinterleave(const double* src, int64_t n, int nvec, double* dst, cudaStream_t st) {
+    dim3 grid(std::min<unsigned>(grid1d(n), 1024u), (unsigned)nvec);
+    k_deinterleave<<<grid, NT, 0, st>>>(src, n, dst);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_interleave(const double* src, int64_t n, int nvec, double* dst, cudaStream_t st) {
+    dim3 grid(std::min<unsigned>(grid1d(n), 1024u), (unsigned)nvec);
+    k_interleave<<<grid, NT, 0, st>>>(src, n, dst);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rho_c(const double* psivT, int64_t pv_plane, const double* psicT, int64_t pc_plane, int64_t ldt, int n_v,
+                         int n_c, int n_mu, const int32_t* chains, double* rho, int64_t ld_rho, int nb, cudaStream_t st) {
+    dim3 grid((unsigned)ceil_div(n_mu, NT), (unsigned)nb);
+    cudaError_t le = launch_pdl(k_rho_c, grid, dim3(NT), (size_t)0, st, 1u, psivT, pv_plane, psicT, pc_plane, ldt, n_v, n_c,
+                                n_mu, chains, rho, ld_rho, nb);
+    count_launch();
+    return le != cudaSuccess ? le : cudaGetLastError();
+}
+
+cudaError_t launch_build_delta_c(const double* eps_v, const double* eps_cq, int n_k, int n_v, int n_c, double* d2,
+                                 double* s, cudaStream_t st) {
+    k_build_delta_c<<<grid1d((int64_t)n_k * n_v * n_c, 1), NT, 0, st>>>(eps_v, eps_cq, n_k, n_v, n_c, d2, s);
     count_launch();
     return cudaGetLastError();
 }

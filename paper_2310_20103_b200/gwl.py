@@ -43,6 +43,13 @@ SIGNATURES = {
     "gwl_exchange": (c_int, [c_void_p, c_int64, c_void_p, c_void_p]),
     "gwl_qp_solve": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int64, c_void_p,
                              c_void_p, c_void_p]),
+    "gwl_tdc_create": (c_int, [POINTER(c_void_p), c_int64, c_int64, c_int64, c_int64, c_int64]),
+    "gwl_tdc_set_orbitals": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "gwl_tdc_set_energies": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "gwl_tdc_set_chains": (c_int, [c_void_p, c_int64, c_void_p]),
+    "gwl_tdc_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
+    "gwl_isdf_build": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_double, c_double, c_void_p, c_void_p,
+                               c_void_p]),
     "gwl_get_timing": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
     "gwl_set_profiling": (c_int, [c_void_p, c_int]),
     "gwl_get_kernel_times": (c_int, [c_void_p, POINTER(c_double), POINTER(c_int64)]),
@@ -187,6 +194,19 @@ class Context:
         lo, hi = c_double(), c_double()
         self._ck(self._lib.gwl_spectrum_bounds(self._h, int(steps), byref(lo), byref(hi)))
         return lo.value, hi.value
+
+    def isdf_build(self, phi_v_grid, phi_c_grid, r, weight: float, soft: float, idx, want_zeta: bool = True):
+        """ISDF front end: fits zeta at the interpolation points idx, builds (alpha|beta) and installs
+        the orbitals at those points and the kernel in this context.  Returns (zeta_t [n_mu, n_r] or None, V [n_mu, n_mu])."""
+        pv, pc, rr, ix = _host(phi_v_grid), _host(phi_c_grid), _host(r), _host(idx, np.int32)
+        n_r = rr.shape[0]
+        if pv.shape != (n_r, self.n_v) or pc.shape != (n_r, self.n_c) or rr.shape != (n_r, 3) or ix.shape != (self.n_mu,):
+            raise GwlError(GWL_EINVAL, "isdf_build: phi_v_grid [n_r, n_v], phi_c_grid [n_r, n_c], r [n_r, 3], idx [n_mu]")
+        zt = np.zeros((self.n_mu, n_r)) if want_zeta else None
+        V = np.zeros((self.n_mu, self.n_mu))
+        self._ck(self._lib.gwl_isdf_build(self._h, n_r, _ptr(pv), _ptr(pc), _ptr(rr), float(weight), float(soft), _ptr(ix),
+                                          _ptr(zt), _ptr(V)))
+        return zt, V
 
     # -- the path ---------------------------------------------------------------------------------
     def casida_matvec(self, x, y=None):
@@ -333,6 +353,56 @@ class Context:
         n = c_int64()
         self._ck(self._lib.gwl_get_launch_count(self._h, byref(n)))
         return n.value
+
+
+class TdcContext(Context):
+    """Complex-orbital (periodic Tamm-Dancoff) context, gwl_tdc_* (SURVEY.md 8(f)-3).
+    lanczos / resolvent / selfenergy / timing calls are the inherited ones."""
+
+    def __init__(self, n_k: int, n_v: int, n_c: int, n_mu: int, n_q: int = 1):
+        self._lib = load_library()
+        self._h = c_void_p()
+        self.n_k, self.n_v, self.n_c, self.n_mu, self.n_q = int(n_k), int(n_v), int(n_c), int(n_mu), int(n_q)
+        self.n_kvc = self.n_k * self.n_v * self.n_c
+        self.n_vc = 2 * self.n_kvc                        # real entries of one (planar) Lanczos vector
+        self.device_ptrs = 0
+        st = self._lib.gwl_tdc_create(byref(self._h), n_k, n_v, n_c, n_mu, n_q)
+        if st != GWL_OK:
+            self._h = c_void_p()
+            raise GwlError(st, "gwl_tdc_create failed (no CUDA device, or bad sizes)")
+
+    def set_orbitals(self, psi_v, psi_cq):
+        pv = np.ascontiguousarray(psi_v, dtype=np.complex128)
+        pc = np.ascontiguousarray(psi_cq, dtype=np.complex128)
+        if pv.shape != (self.n_k, self.n_mu, self.n_v) or pc.shape != (self.n_k, self.n_mu, self.n_c):
+            raise GwlError(GWL_EINVAL, "set_orbitals: psi_v must be [n_k, n_mu, n_v], psi_cq [n_k, n_mu, n_c] complex")
+        self._ck(self._lib.gwl_tdc_set_orbitals(self._h, _ptr(pv), _ptr(pc)))
+
+    def set_energies(self, eps_v, eps_cq):
+        ev, ec = _host(eps_v), _host(eps_cq)
+        if ev.shape != (self.n_k, self.n_v) or ec.shape != (self.n_k, self.n_c):
+            raise GwlError(GWL_EINVAL, "set_energies: eps_v must be [n_k, n_v], eps_cq [n_k, n_c]")
+        self._ck(self._lib.gwl_tdc_set_energies(self._h, _ptr(ev), _ptr(ec)))
+
+    def set_chains(self, chains):
+        ch = _host(chains, np.int32)
+        if ch.ndim != 2 or ch.shape[1] != 4:
+            raise GwlError(GWL_EINVAL, "set_chains: chains must be [n_chains, 4] = (k slot of n, n, k slot of m, m)")
+        self._ck(self._lib.gwl_tdc_set_chains(self._h, ch.shape[0], _ptr(ch)))
+
+    def matvec(self, x, y=None):
+        """y = A(q) x.  Host mode: x complex numpy [nvec, n_k, n_v, n_c] (or [nvec, n_kvc]).  Device mode: x, y torch
+        CUDA complex128 tensors, contiguous."""
+        if self.device_ptrs:
+            nvec = x.numel() // self.n_kvc
+            self._ck(self._lib.gwl_tdc_matvec(self._h, _ptr(x), _ptr(y), nvec))
+            return y
+        xh = np.ascontiguousarray(x, dtype=np.complex128)
+        if xh.size % self.n_kvc:
+            raise GwlError(GWL_EINVAL, "matvec: x must be [nvec, n_k, n_v, n_c]")
+        yh = np.empty_like(xh)
+        self._ck(self._lib.gwl_tdc_matvec(self._h, _ptr(xh), _ptr(yh), xh.size // self.n_kvc))
+        return yh
 
 
 def context_from_problem(prob) -> Context:

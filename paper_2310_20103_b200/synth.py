@@ -201,3 +201,31 @@ def make_periodic(n_k: int, n_v: int, n_c: int, n_mu: int, box: float = 10.0, se
 def random_complex_block(n: int, nvec: int, seed: int = 1) -> np.ndarray:
     rng = np.random.default_rng(seed)
     return rng.standard_normal((nvec, n)) + 1j * rng.standard_normal((nvec, n))
+
+
+# ---------------------------------------------------------------------------------------------
+# smooth synthetic orbitals on a real-space grid for the ISDF front end.
+# Particle-in-a-box eigenfunctions on a uniform n^3 grid (the paper's orbitals live on a uniform real-space grid,
+# PAPER.md:317): smooth, orthonormal under the grid quadrature, and their pair products have low numerical rank.
+# ---------------------------------------------------------------------------------------------
+def box_orbitals(n_grid: int, n_orb: int, box: float = 8.0):
+    """Returns (r [n^3, 3], phi [n^3, n_orb], weight h^3): the n_orb lowest states sin(a pi x / L) sin(b pi y / L)
+    sin(c pi z / L), (a, b, c) ordered by a^2 + b^2 + c^2 then lexicographically, on the interior points of a cube."""
+    h = box / (n_grid + 1)
+    x = h * np.arange(1, n_grid + 1)
+    X, Y, Z = np.meshgrid(x, x, x, indexing="ij")
+    r = np.stack([X.ravel(), Y.ravel(), Z.ravel()], axis=1)
+    q = [(a * a + b * b + c * c, a, b, c) for a in range(1, 12) for b in range(1, 12) for c in range(1, 12)]
+    q.sort()
+    s = {k: np.sqrt(2.0 / box) * np.sin(k * np.pi * x / box) for k in range(1, 12)}
+    phi = np.empty((n_grid ** 3, n_orb))
+    for j, (_, a, b, c) in enumerate(q[:n_orb]):
+        phi[:, j] = (s[a][:, None, None] * s[b][None, :, None] * s[c][None, None, :]).ravel()
+    return r, phi, h ** 3
+
+
+def stride_points(n_r: int, n_mu: int, seed: int = 0) -> np.ndarray:
+    """n_mu distinct grid indices, seeded: the interpolation points handed to both sides (their selection, by pivoted QR
+    or k-means in the ISDF literature, is not part of the parity tests)."""
+    rng = np.random.default_rng(seed)
+    return np.sort(rng.choice(n_r, size=n_mu, replace=False)).astype(np.int32)

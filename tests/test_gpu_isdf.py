@@ -1,0 +1,85 @@
+"""GPU parity of the ISDF front end (gwl_isdf_build; Eq. 15-17) against oracle/isdf.py on
+smooth synthetic orbitals (particle-in-a-box states on a uniform real-space grid), and of the hot path run on what it built.
+Tolerances: zeta and (alpha|beta) to 1e-8 relative (max-norm): the normal equations square the condition number of the
+fit, the oracle solves the same least squares by SVD (lstsq); reconstruction of the pair products to the oracle's own level."""
+import numpy as np
+import pytest
+
+from oracle import gw_oracle as orc
+from oracle import isdf
+from paper_2310_20103_b200 import gwl, synth
+
+pytestmark = pytest.mark.gpu
+
+
+def _problem(n_grid, n_v, n_c, n_mu, seed=1):
+    """Products of box states are linearly dependent (numerical rank 18 / 31 / 51 of the 21 / 45 / 91 pairs of 6 / 9 / 13
+    orbitals): N_mu stays below that rank, where C C^T is positive definite (condition number 1e4-1e5 for these seeds)."""
+    r, phi, w = synth.box_orbitals(n_grid, n_v + n_c)
+    idx = synth.stride_points(r.shape[0], n_mu, seed)
+    return r, phi, w, idx
+
+
+@pytest.mark.parametrize("n_grid,n_v,n_c,n_mu,seed", [(8, 2, 4, 14, 1), (10, 3, 6, 24, 5), (12, 4, 9, 40, 0)])
+def test_isdf_fit_and_two_center_integrals(n_grid, n_v, n_c, n_mu, seed):
+    r, phi, w, idx = _problem(n_grid, n_v, n_c, n_mu, seed)
+    soft = 0.5
+    with gwl.Context(n_v, n_c, n_mu) as ctx:
+        zt, V = ctx.isdf_build(phi[:, :n_v], phi[:, n_v:], r, w, soft, idx)
+    zeta = isdf.fit(phi, phi, idx)
+    Vref = isdf.two_center(zeta, isdf.coulomb_grid(r, w, soft))
+    assert np.abs(zt.T - zeta).max() <= 1e-8 * np.abs(zeta).max()
+    assert np.abs(V - Vref).max() <= 1e-8 * np.abs(Vref).max()
+    assert np.abs(V - V.T).max() <= 1e-10 * np.abs(V).max()
+    # Eq. 15: the fitted pair products reproduce the exact ones as well as the oracle's fit does
+    Z = isdf.pair_products(phi, phi)
+    e_gpu = np.linalg.norm(Z - zt.T @ Z[idx]) / np.linalg.norm(Z)
+    e_ref = np.linalg.norm(Z - zeta @ Z[idx]) / np.linalg.norm(Z)
+    assert e_gpu <= 2.0 * e_ref + 1e-9
+    # interpolation property: zeta_mu(r_nu) = delta_mu,nu
+    assert np.abs(zt[:, idx] - np.eye(n_mu)).max() <= 1e-7
+
+
+def test_isdf_built_context_runs_the_hot_path():
+    """gwl_isdf_build installs Phi(r_mu) and (alpha|beta): the Casida product, Lanczos and Sigma on that context against
+    the oracle fed with the ORACLE's own fit."""
+    n_v, n_c, n_mu = 3, 6, 24
+    r, phi, w, idx = _problem(10, n_v, n_c, n_mu, seed=5)
+    rng = np.random.default_rng(0)
+    eps_v = np.sort(rng.uniform(-10, -5, n_v))
+    eps_c = np.sort(rng.uniform(-3, 20, n_c))
+    omega = np.linspace(-20, 20, 101)
+    n_idx = np.array([0, 1, n_v, n_v + 2], dtype=np.int32)
+    m_idx = np.full_like(n_idx, n_v - 1)
+    X = synth.random_block(synth.make_custom(n_v, n_c, n_mu).cfg, 3)
+    with gwl.Context(n_v, n_c, n_mu) as ctx:
+        ctx.isdf_build(phi[:, :n_v], phi[:, n_v:], r, w, 0.5, idx, want_zeta=False)
+        ctx.set_energies(eps_v, eps_c)
+        Y = ctx.casida_matvec(X)
+        ctx.set_chains(n_idx, m_idx)
+        a, b, n2, ln = ctx.lanczos(4, n_v * n_c, 4, 1)
+        sig, _ = ctx.selfenergy(omega, 0.1, 4)
+    zeta = isdf.fit(phi, phi, idx)
+    V = isdf.two_center(zeta, isdf.coulomb_grid(r, w, 0.5))
+    pv, pc = phi[idx][:, :n_v], phi[idx][:, n_v:]
+    ref_y = orc.casida_matvec_factored(pv, pc, V, orc.delta_vc(eps_v, eps_c), X)
+    assert np.abs(Y - ref_y).max() <= 1e-8 * np.abs(ref_y).max()
+    ref = orc.run_chains(pv, pc, eps_v, eps_c, V, n_idx, m_idx, n_v * n_c, omega, 0.1, reorth=True)
+    assert (np.abs(n2 - ref["norm2"]) <= 1e-7 * ref["norm2"]).all()
+    assert np.abs(sig - ref["sigma"]).max() <= 1e-6 * max(1.0, np.abs(ref["sigma"]).max())
+
+
+def test_isdf_rejects_bad_points_and_rank_deficient_fits():
+    r, phi, w, idx = _problem(8, 2, 3, 20)
+    with gwl.Context(2, 3, 20) as ctx:
+        bad = idx.copy()
+        bad[1] = bad[0]
+        with pytest.raises(gwl.GwlError) as e:
+            ctx.isdf_build(phi[:, :2], phi[:, 2:], r, w, 0.5, bad)
+        assert e.value.status == gwl.GWL_EINVAL
+        # the 15 pair products of 5 orbitals cannot be resolved at 20 points: C C^T is singular
+        with pytest.raises(gwl.GwlError) as e:
+            ctx.isdf_build(phi[:, :2], phi[:, 2:], r, w, 0.5, idx)
+        assert e.value.status == gwl.GWL_EINVAL and "positive definite" in str(e.value)
+        with pytest.raises(gwl.GwlError):
+            ctx.casida_matvec(np.zeros((1, 2, 3)))                        # nothing was installed
