@@ -215,6 +215,15 @@ def run_paper_setting(args):
         b.record(stream)
     torch.cuda.synchronize()
     sec = sum(a.elapsed_time(b) for a, b in ev) * 1e-3 / args.steps
+    launches = int((ctx.get_launch_count() - n0) / args.steps)
+    # one more state with an event pair around every launch: where the time goes (not part of the timed value)
+    ctx.set_profiling(2)
+    state()
+    kt = ctx.get_kernel_times()
+    ctx.set_profiling(0)
+    tot = sum(v[0] for v in kt.values())
+    share = {k: round(v[0] / tot, 4) for k, v in kt.items() if v[1]}
+    per_launch_ms = {k: round(v[0] / v[1], 4) for k, v in kt.items() if v[1]}
     flop = (n_orb * n_iter * g + 40) * (4.0 * n_mu * n_v * n_c + 2.0 * n_mu * n_mu)
     line = {"metric": "seconds_per_quasiparticle_state", "value": sec, "unit": "s", "higher_is_better": False,
             "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
@@ -223,7 +232,7 @@ def run_paper_setting(args):
                        "n_v": n_v, "n_c": n_c, "n_mu": n_mu, "chains": n_orb, "block": block,
                        "fit_range_eV2": rng},
             "c_applies": n_orb * n_iter * g + 40, "tflops_flop_model": flop / sec / 1e12,
-            "gpu_launches": int((ctx.get_launch_count() - n0) / args.steps),
+            "gpu_launches": launches, "kernel_time_share": share, "kernel_ms_per_launch": per_launch_ms,
             "e_qp_eV": float(out[0].item()), "z": float(out[1].item()),
             "note": "context only: hot path on synthetic inputs; the paper's Table I wall times include ISDF on CPUs"}
     print(json.dumps(line), flush=True)

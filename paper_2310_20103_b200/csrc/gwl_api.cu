@@ -83,14 +83,22 @@ struct gwl_ctx {
     int run_poly = 0;
     DevBuf alpha, beta, norm2, len, scale, alive;
 
-    // workspaces
-    DevBuf xs, T, W, part, dotpart, normpart, basis, coefpart, tA, tB;
+    // workspaces.  The GEMM scratch (T, W, split-K partials, stream-K hand-over) exists twice: set 0 serves the context's
+    // stream, set 1 the side stream on which gwl_lanczos builds the start vectors of the NEXT block (S1) under the step
+    // loop of the current one.
+    struct WorkSet {
+        DevBuf T, W, part, sk_ws, sk_flags;
+        unsigned sk_epoch = 0;
+    } wset[2];
+    int cur = 0;
+    cudaStream_t stream2 = nullptr;
+    cudaEvent_t ev_consumed = nullptr, ev_s1 = nullptr;
+    WorkSet& ws() { return wset[cur]; }
+    cudaStream_t lstream() const { return cur ? stream2 : stream; }
+    DevBuf xs, dotpart, normpart, basis, coefpart, tA, tB, pnext, pnext_part;
     DevBuf x_nidx, x_midx, x_part, x_sig, x_eps, x_vxc, x_sc, x_e, x_z, x_it;  // gwl_exchange / gwl_qp_solve staging
     DevBuf stage;            // gwl_set_orbitals staging
-    DevBuf sk_ws, sk_flags;  // stream-K hand-over of the K^T.W GEMM (kr_gemm.cu)
     DevBuf isdf_phi, isdf_phimu, isdf_y, isdf_s, isdf_g, isdf_u;  // gwl_isdf_build
-    DevBuf red_cnt;          // arrive / done counters of the in-kernel split-K reduction (K.X, V.T), zero between launches
-    unsigned sk_epoch = 0;
     DevBuf theta, wgt, ritz_info, d_omega, d_zeta, d_sigma, d_sigsum, io_x, io_y;
 
     // timing: per-step event triples (op start, op end, step end) and, at profiling level 2,
@@ -135,11 +143,11 @@ struct KernelTimer {
     KernelTimer(gwl_ctx* ctx, int cls) : c(ctx), on(ctx->prof_level >= 2) {
         if (on) {
             c->kev_class.push_back(cls);
-            cudaEventRecord(c->next_kevent(), c->stream);
+            cudaEventRecord(c->next_kevent(), c->lstream());
         }
     }
     ~KernelTimer() {
-        if (on) cudaEventRecord(c->next_kevent(), c->stream);
+        if (on) cudaEventRecord(c->next_kevent(), c->lstream());
     }
 };
 #define CKL(cls, call)                                            \
@@ -184,23 +192,22 @@ struct LaunchScope {
 gwl_status ensure_workspace(gwl_ctx* ctx, int nb) {
     cudaStream_t st = ctx->stream;
     const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
-    CK(ctx->xs.ensure((size_t)nb * ldxs * 8, st));
+    if (ctx->cur == 0) CK(ctx->xs.ensure((size_t)nb * ldxs * 8, st));
     const int rows = ctx->cplx ? 2 * nb : nb;  // complex: T and W hold a real and an imaginary plane of nb rows each
-    CK(ctx->T.ensure((size_t)rows * ctx->n_mup * 8, st));
-    CK(ctx->W.ensure((size_t)rows * ctx->n_mup * 8, st));
+    CK(ctx->ws().T.ensure((size_t)rows * ctx->n_mup * 8, st));
+    CK(ctx->ws().W.ensure((size_t)rows * ctx->n_mup * 8, st));
     const int kt_f = ctx->n_v * (ctx->n_cp / BK), kt_v = ctx->n_mup / BK;
     const GemmPlan pf = ctx->cplx ? plan_gemm_c(ctx->n_mu, nb, ctx->n_kv * (ctx->n_cp / BK), ctx->n_sm)
                                   : plan_gemm(MODE_FWD, ctx->n_mu, nb, kt_f, ctx->n_cp / BK, ctx->n_sm);
     const GemmPlan pv = plan_gemm(MODE_PLAIN, ctx->n_mu, rows, kt_v, kt_v, ctx->n_sm);
     const int smax = std::max(pf.splits, pv.splits);
-    CK(ctx->part.ensure((size_t)smax * rows * ctx->n_mup * 8, st));
+    CK(ctx->ws().part.ensure((size_t)smax * rows * ctx->n_mup * 8, st));
     const int npart = vec_parts(ctx->n_vc);
     const int64_t ndot = std::max<int64_t>((int64_t)ctx->n_v * ceil_div(ctx->n_c, 128), npart);
     CK(ctx->dotpart.ensure((size_t)nb * ndot * 8, st));
     CK(ctx->normpart.ensure((size_t)nb * std::max(npart, reorth_parts(ctx->n_vc)) * 8, st));
-    CK(ctx->sk_ws.ensure(gemm_bwd_ws_bytes(ctx->n_sm), st));
-    CK(ctx->sk_flags.ensure(gemm_bwd_flag_bytes(ctx->n_sm), st));
-    CK(ctx->red_cnt.ensure(gemm_red_cnt_bytes(ctx->n_sm), st));
+    CK(ctx->ws().sk_ws.ensure(gemm_bwd_ws_bytes(ctx->n_sm), st));
+    CK(ctx->ws().sk_flags.ensure(gemm_bwd_flag_bytes(ctx->n_sm), st));
     return GWL_OK;
 }
 
@@ -208,7 +215,7 @@ gwl_status ensure_workspace(gwl_ctx* ctx, int nb) {
 // T[b][mu] = sum_vc K[mu, vc] xs[b][vc]   (xs = scaled input in the padded [nb][n_v][n_cp] layout)
 // complex (planar) K.x of the periodic Tamm-Dancoff operator: T[2][nb][n_mup] (kr_gemm_c.cu)
 gwl_status gemm_kx_c(gwl_ctx* ctx, int nb) {
-    cudaStream_t st = ctx->stream;
+    cudaStream_t st = ctx->lstream();
     const int kt_c = ctx->n_cp / BK, kt_f = ctx->n_kv * kt_c;
     const int64_t ldm = ctx->n_mup;
     const GemmPlan pl = plan_gemm_c(ctx->n_mu, nb, kt_f, ctx->n_sm);
@@ -230,21 +237,21 @@ gwl_status gemm_kx_c(gwl_ctx* ctx, int nb) {
     p.lds = ldm;
     p.s_plane = (int64_t)ctx->n_kv * ldm;
     p.scale_rows = ctx->n_kv;
-    if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * 2 * nb * ldm * 8, st));
-    p.out = pl.splits == 1 ? ctx->T.as<double>() : ctx->part.as<double>();
+    if (pl.splits > 1) CK(ctx->ws().part.ensure((size_t)pl.splits * 2 * nb * ldm * 8, st));
+    p.out = pl.splits == 1 ? ctx->ws().T.as<double>() : ctx->ws().part.as<double>();
     p.ldo = ldm;
     p.o_plane = (int64_t)nb * ldm;
     p.out_split_stride = (int64_t)2 * nb * ldm;
     CKL(0, launch_gemm_c(MODE_FWD, EPI_STORE, p, pl.splits, st));
     if (pl.splits > 1)
-        CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)2 * nb * ldm, pl.splits, ctx->T.as<double>(), ldm,
+        CKL(3, launch_splitk_reduce(ctx->ws().part.as<double>(), (int64_t)2 * nb * ldm, pl.splits, ctx->ws().T.as<double>(), ldm,
                                     ctx->n_mu, 2 * nb, st));
     return GWL_OK;
 }
 
 gwl_status gemm_kx(gwl_ctx* ctx, int nb) {
     if (ctx->cplx) return gemm_kx_c(ctx, nb);
-    cudaStream_t st = ctx->stream;
+    cudaStream_t st = ctx->lstream();
     const int kt_c = ctx->n_cp / BK, kt_f = ctx->n_v * kt_c;
     const int64_t ldm = ctx->n_mup;
     const GemmPlan pl = plan_gemm(MODE_FWD, ctx->n_mu, nb, kt_f, kt_c, ctx->n_sm);
@@ -261,27 +268,22 @@ gwl_status gemm_kx(gwl_ctx* ctx, int nb) {
     p.scale = ctx->phi_vT.as<double>();
     p.lds = ldm;
     p.scale_rows = ctx->n_v;
-    if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * nb * ldm * 8, st));
-    p.out = pl.splits == 1 ? ctx->T.as<double>() : ctx->part.as<double>();
+    if (pl.splits > 1) CK(ctx->ws().part.ensure((size_t)pl.splits * nb * ldm * 8, st));
+    p.out = pl.splits == 1 ? ctx->ws().T.as<double>() : ctx->ws().part.as<double>();
     p.ldo = ldm;
     p.out_split_stride = (int64_t)nb * ldm;
-    const bool fused = gemm_reduces_in_kernel(pl, ctx->n_mu, nb, ctx->n_sm);
-    if (fused) {
-        p.red_cnt = ctx->red_cnt.as<unsigned>();
-        p.out_final = ctx->T.as<double>();
-    }
     CKL(0, launch_gemm(MODE_FWD, EPI_STORE, pl, p, pl.splits, st));
-    if (pl.splits > 1 && !fused)
-        CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->T.as<double>(), ldm, ctx->n_mu,
+    if (pl.splits > 1)
+        CKL(3, launch_splitk_reduce(ctx->ws().part.as<double>(), (int64_t)nb * ldm, pl.splits, ctx->ws().T.as<double>(), ldm, ctx->n_mu,
                                 nb, st));
     return GWL_OK;
 }
 
 // out[n][m] = sum_k A[m][k] B[n][k] on the DMMA GEMM (MODE_PLAIN): A [M][lda], B [N][ldb], both K-contiguous with k_tiles
-// tiles of 16 valid (zero-padded) columns; split-K reduced in the kernel when the grid is co-resident, else by k_splitk_reduce
+// tiles of 16 valid (zero-padded) columns; split-K partials reduced in a fixed order by k_splitk_reduce
 gwl_status plain_gemm(gwl_ctx* ctx, const double* A, int64_t lda, const double* B, int64_t ldb, int M, int N, int k_tiles,
                       double* out, int64_t ldo, int cls) {
-    cudaStream_t st = ctx->stream;
+    cudaStream_t st = ctx->lstream();
     const GemmPlan pl = plan_gemm(MODE_PLAIN, M, N, k_tiles, k_tiles, ctx->n_sm);
     GemmParams p{};
     p.A = A;
@@ -293,27 +295,21 @@ gwl_status plain_gemm(gwl_ctx* ctx, const double* A, int64_t lda, const double* 
     p.kt_total = k_tiles;
     p.a_wrap = k_tiles;
     p.kt_per_split = pl.kt_per_split;
-    if (pl.splits > 1) CK(ctx->part.ensure((size_t)pl.splits * N * ldo * 8, st));
-    p.out = pl.splits == 1 ? out : ctx->part.as<double>();
+    if (pl.splits > 1) CK(ctx->ws().part.ensure((size_t)pl.splits * N * ldo * 8, st));
+    p.out = pl.splits == 1 ? out : ctx->ws().part.as<double>();
     p.ldo = ldo;
     p.out_split_stride = (int64_t)N * ldo;
-    const bool fused = gemm_reduces_in_kernel(pl, M, N, ctx->n_sm);
-    if (fused) {
-        CK(ctx->red_cnt.ensure(gemm_red_cnt_bytes(ctx->n_sm), st));
-        p.red_cnt = ctx->red_cnt.as<unsigned>();
-        p.out_final = out;
-    }
     CKL(cls, launch_gemm(MODE_PLAIN, EPI_STORE, pl, p, pl.splits, st));
-    if (pl.splits > 1 && !fused)
-        CKL(3, launch_splitk_reduce(ctx->part.as<double>(), (int64_t)N * ldo, pl.splits, out, ldo, M, N, st));
+    if (pl.splits > 1)
+        CKL(3, launch_splitk_reduce(ctx->ws().part.as<double>(), (int64_t)N * ldo, pl.splits, out, ldo, M, N, st));
     return GWL_OK;
 }
 
 // W[b][mu] = sum_nu V[mu][nu] T[b][nu]
 gwl_status gemm_v(gwl_ctx* ctx, int nb) {
     if (ctx->cplx) nb *= 2;  // V is real: the two planes of T are 2 nb independent columns
-    return plain_gemm(ctx, ctx->V.as<double>(), ctx->n_mup, ctx->T.as<double>(), ctx->n_mup, ctx->n_mu, nb, ctx->n_mup / BK,
-                      ctx->W.as<double>(), ctx->n_mup, 1);
+    return plain_gemm(ctx, ctx->V.as<double>(), ctx->n_mup, ctx->ws().T.as<double>(), ctx->n_mup, ctx->n_mu, nb, ctx->n_mup / BK,
+                      ctx->ws().W.as<double>(), ctx->n_mup, 1);
 }
 
 // u = K^T W with the epilogue fused:  x != NULL: y = d2 o x + coupling s o u and the partial dots sum(x y);
@@ -338,7 +334,7 @@ gwl_status gemm_ktw_c(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int
     p.lda = ldm;
     p.a_rows = ctx->n_k * ctx->n_c;
     p.a_plane = (int64_t)p.a_rows * ldm;
-    p.B = ctx->W.as<double>();
+    p.B = ctx->ws().W.as<double>();
     p.ldb = ldm;
     p.b_plane = (int64_t)nb * ldm;
     p.M = ctx->n_c;
@@ -360,7 +356,7 @@ gwl_status gemm_ktw_c(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int
     p.coupling = 1.0;
     p.dotpart = dotpart;
     p.dot_stride = dot_stride;
-    CKL(2, launch_gemm_c(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, p, ctx->n_kv, ctx->stream));
+    CKL(2, launch_gemm_c(MODE_BWD, x != nullptr ? EPI_CASIDA : EPI_START, p, ctx->n_kv, ctx->lstream()));
     return GWL_OK;
 }
 
@@ -376,7 +372,7 @@ gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64
     GemmParams p{};
     p.A = ctx->phi_cT.as<double>();
     p.lda = ldm;
-    p.B = ctx->W.as<double>();
+    p.B = ctx->ws().W.as<double>();
     p.ldb = ldm;
     p.M = ctx->n_c;
     p.N = nb;
@@ -396,10 +392,10 @@ gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64
     p.dot_stride = dot_stride;
     p.n_c = ctx->n_c;
     p.coupling = ctx->approx ? 1.0 : 2.0;
-    p.ws = ctx->sk_ws.as<double>();
-    p.flags = ctx->sk_flags.as<unsigned>();
-    if (++ctx->sk_epoch == 0) ++ctx->sk_epoch;
-    p.epoch = ctx->sk_epoch;
+    p.ws = ctx->ws().sk_ws.as<double>();
+    p.flags = ctx->ws().sk_flags.as<unsigned>();
+    if (++ctx->ws().sk_epoch == 0) ++ctx->ws().sk_epoch;
+    p.epoch = ctx->ws().sk_epoch;
     p.n_sm = ctx->n_sm;
     int epi = x != nullptr ? EPI_CASIDA : EPI_START;
     if (cheb != nullptr) {
@@ -418,7 +414,7 @@ gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64
         p.c0 = cheb->c0;
         p.first = cheb->first;
     }
-    CKL(2, launch_gemm(MODE_BWD, epi, pl, p, ctx->n_v, ctx->stream));
+    CKL(2, launch_gemm(MODE_BWD, epi, pl, p, ctx->n_v, ctx->lstream()));
     return GWL_OK;
 }
 
@@ -444,11 +440,11 @@ gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, doub
     if (ctx->cplx)  // rho~ = psi_m conj(psi_n): the ket of PAPER.md:310 is the conjugate of the printed elements (Q20)
         CKL(4, launch_rho_c(ctx->phi_vT.as<double>(), (int64_t)ctx->n_kv * ldm, ctx->phi_cT.as<double>(),
                             (int64_t)ctx->n_k * ctx->n_c * ldm, ldm, ctx->nv_k, ctx->n_c, ctx->n_mu,
-                            ctx->d_nidx.as<int32_t>() + 4 * j0, ctx->T.as<double>(), ldm, nb, ctx->stream));
+                            ctx->d_nidx.as<int32_t>() + 4 * j0, ctx->ws().T.as<double>(), ldm, nb, ctx->lstream()));
     else
         CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
-                      ctx->d_nidx.as<int32_t>() + j0, ctx->d_midx.as<int32_t>() + j0, ctx->T.as<double>(), ldm, nb,
-                      ctx->stream));
+                      ctx->d_nidx.as<int32_t>() + j0, ctx->d_midx.as<int32_t>() + j0, ctx->ws().T.as<double>(), ldm, nb,
+                      ctx->lstream()));
     gwl_status rs = gemm_v(ctx, nb);
     if (rs == GWL_OK) rs = gemm_ktw(ctx, nullptr, ctx->n_vc, P, ctx->n_vc, nb, normpart, dot_stride);
     return rs;
@@ -510,16 +506,25 @@ void gwl_destroy(gwl_ctx* ctx) {
     if (ctx == nullptr) return;
     DeviceGuard dg(ctx);
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->stream2 != nullptr) cudaStreamSynchronize(ctx->stream2);
     DevBuf* bufs[] = {&ctx->phi_c, &ctx->phi_cT, &ctx->phi_vT, &ctx->V, &ctx->eps_v, &ctx->eps_c, &ctx->d2, &ctx->s,
                       &ctx->d_nidx, &ctx->d_midx, &ctx->d_start, &ctx->d_eps_n, &ctx->d_sgn_n, &ctx->alpha,
-                      &ctx->beta, &ctx->norm2, &ctx->len, &ctx->scale, &ctx->alive, &ctx->xs, &ctx->T, &ctx->W,
-                      &ctx->part, &ctx->dotpart, &ctx->normpart, &ctx->basis, &ctx->coefpart, &ctx->tA, &ctx->tB,
-                      &ctx->theta, &ctx->wgt, &ctx->ritz_info, &ctx->d_omega, &ctx->d_zeta,
-                      &ctx->d_sigma, &ctx->d_sigsum, &ctx->io_x, &ctx->io_y, &ctx->sk_ws, &ctx->sk_flags, &ctx->red_cnt, &ctx->isdf_phi, &ctx->isdf_phimu, &ctx->isdf_y, &ctx->isdf_s, &ctx->isdf_g, &ctx->isdf_u, &ctx->stage, &ctx->x_nidx, &ctx->x_midx, &ctx->x_part, &ctx->x_sig,
-                      &ctx->x_eps, &ctx->x_vxc, &ctx->x_sc, &ctx->x_e, &ctx->x_z, &ctx->x_it};
+                      &ctx->beta, &ctx->norm2, &ctx->len, &ctx->scale, &ctx->alive, &ctx->xs, &ctx->dotpart,
+                      &ctx->normpart, &ctx->basis, &ctx->coefpart, &ctx->tA, &ctx->tB, &ctx->pnext, &ctx->pnext_part,
+                      &ctx->theta, &ctx->wgt, &ctx->ritz_info, &ctx->d_omega, &ctx->d_zeta, &ctx->d_sigma, &ctx->d_sigsum,
+                      &ctx->io_x, &ctx->io_y, &ctx->isdf_phi, &ctx->isdf_phimu, &ctx->isdf_y, &ctx->isdf_s, &ctx->isdf_g,
+                      &ctx->isdf_u, &ctx->stage, &ctx->x_nidx, &ctx->x_midx, &ctx->x_part, &ctx->x_sig, &ctx->x_eps,
+                      &ctx->x_vxc, &ctx->x_sc, &ctx->x_e, &ctx->x_z, &ctx->x_it};
     for (DevBuf* b : bufs) b->release();
+    for (gwl_ctx::WorkSet& w : ctx->wset) {
+        DevBuf* wb[] = {&w.T, &w.W, &w.part, &w.sk_ws, &w.sk_flags};
+        for (DevBuf* b : wb) b->release();
+    }
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->kev) cudaEventDestroy(e);
+    if (ctx->ev_consumed != nullptr) cudaEventDestroy(ctx->ev_consumed);
+    if (ctx->ev_s1 != nullptr) cudaEventDestroy(ctx->ev_s1);
+    if (ctx->stream2 != nullptr) cudaStreamDestroy(ctx->stream2);
     delete ctx;
 }
 
@@ -791,7 +796,7 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
     const int64_t n_vc = ctx->n_vc;
     const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
     const int npart = vec_parts(n_vc);
-    const int rparts = reorth_parts(n_vc);
+    const int rparts = ctx->cplx ? reorth_parts(n_vc / 2) : reorth_parts(n_vc);
     const bool poly = ctx->g > 0;
 
     invalidate_run(ctx);  // stays invalid if this call fails part-way
@@ -811,11 +816,27 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
         CK(ctx->alive.ensure((size_t)2 * nbmax * 4, st));
         const int nslots = reorth ? L + 1 : 3;
         CK(ctx->basis.ensure((size_t)nslots * nbmax * n_vc * 8, st));
-        if (reorth) CK(ctx->coefpart.ensure((size_t)nbmax * L * rparts * 8, st));
+        if (reorth) CK(ctx->coefpart.ensure((size_t)nbmax * L * rparts * 8 * (ctx->cplx ? 2 : 1), st));
         if (poly) {
             CK(ctx->tA.ensure((size_t)nbmax * n_vc * 8, st));
             CK(ctx->tB.ensure((size_t)nbmax * n_vc * 8, st));
         }
+    }
+    // with more than one block of index chains, S1 of block i+1 (rho, V rho, K^T: 1.5 GEMMs) runs on a side
+    // stream with its own GEMM scratch under the step loop of block i, into `pnext`; block i+1 then starts with a copy.
+    const bool overlap = ctx->chain_mode == 1 && n_chains > nbmax;
+    if (overlap) {
+        if (ctx->stream2 == nullptr) {
+            CK(cudaStreamCreateWithFlags(&ctx->stream2, cudaStreamNonBlocking));
+            CK(cudaEventCreateWithFlags(&ctx->ev_consumed, cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&ctx->ev_s1, cudaEventDisableTiming));
+        }
+        ctx->cur = 1;
+        gwl_status rs = ensure_workspace(ctx, nbmax);
+        ctx->cur = 0;
+        if (rs != GWL_OK) return rs;
+        CK(ctx->pnext.ensure((size_t)nbmax * n_vc * 8, st));
+        CK(ctx->pnext_part.ensure((size_t)nbmax * casida_ndot(ctx, nbmax) * 8, st));
     }
 
     for (int64_t j0 = 0; j0 < n_chains; j0 += nbmax) {
@@ -837,10 +858,27 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
 
         // ---- S1: start vectors into slot 0 ----
         if (ctx->chain_mode == 1) {
-            gwl_status rs = build_start_vectors(ctx, j0, nb, slot(0), dotpart, ndot_c);
-            if (rs != GWL_OK) return rs;
+            if (overlap && j0 > 0) {  // built on the side stream while the previous block was stepping
+                CK(cudaStreamWaitEvent(st, ctx->ev_s1, 0));
+                CK(cudaMemcpyAsync(slot(0), ctx->pnext.p, (size_t)nb * n_vc * 8, cudaMemcpyDeviceToDevice, st));
+                CK(cudaMemcpyAsync(dotpart, ctx->pnext_part.p, (size_t)nb * ndot_c * 8, cudaMemcpyDeviceToDevice, st));
+            } else {
+                gwl_status rs = build_start_vectors(ctx, j0, nb, slot(0), dotpart, ndot_c);
+                if (rs != GWL_OK) return rs;
+            }
             CKL(5, launch_lanczos_init(slot(0), n_vc, nb, dotpart, ndot_c, S, ctx->xs.as<double>(), ldxs,
                                    ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
+            if (overlap && j0 + nbmax < n_chains) {
+                const int nb_next = (int)std::min<int64_t>(nbmax, n_chains - j0 - nbmax);
+                CK(cudaEventRecord(ctx->ev_consumed, st));  // pnext / pnext_part of this block have been copied out
+                CK(cudaStreamWaitEvent(ctx->stream2, ctx->ev_consumed, 0));
+                ctx->cur = 1;
+                gwl_status rs = build_start_vectors(ctx, j0 + nbmax, nb_next, ctx->pnext.as<double>(),
+                                                    ctx->pnext_part.as<double>(), casida_ndot(ctx, nb_next));
+                ctx->cur = 0;
+                if (rs != GWL_OK) return rs;
+                CK(cudaEventRecord(ctx->ev_s1, ctx->stream2));
+            }
         } else {
             CK(cudaMemcpyAsync(slot(0), ctx->d_start.as<double>() + j0 * n_vc, (size_t)nb * n_vc * 8,
                                cudaMemcpyDeviceToDevice, st));
@@ -912,6 +950,13 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
             CKL(5, launch_lanczos_update1(w, q, qp, n_vc, nb, dotpart, ndot, dstride, S, k, normpart, npart, st));
             if (reorth) {
                 for (int pass = 0; pass < 2; ++pass) {
+                    if (ctx->cplx) {  // complex projection coefficients <q_j, w>
+                        CKL(6, launch_reorth_dots_c(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), rparts,
+                                                    st));
+                        CKL(6, launch_reorth_apply_c(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(),
+                                                     rparts, pass == 1 ? normpart : nullptr, st));
+                        continue;
+                    }
                     CKL(6, launch_reorth_dots(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), rparts,
                                           st));
                     CKL(6, launch_reorth_apply(basis, slot_stride, k + 1, w, n_vc, nb, ctx->coefpart.as<double>(), rparts,
@@ -1073,9 +1118,8 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
     const int64_t ldm = ctx->n_mup;
     const int npart = vec_parts(ctx->n_mu);
     // only what rho -> V rho -> dot touches: T, W and the V.T split-K partials (none of the N_vc-sized Casida buffers)
-    CK(ctx->T.ensure((size_t)chunk * ldm * 8, st));
-    CK(ctx->W.ensure((size_t)chunk * ldm * 8, st));
-    CK(ctx->red_cnt.ensure(gemm_red_cnt_bytes(ctx->n_sm), st));
+    CK(ctx->ws().T.ensure((size_t)chunk * ldm * 8, st));
+    CK(ctx->ws().W.ensure((size_t)chunk * ldm * 8, st));
     gwl_status rs = GWL_OK;
     // (v, m) index pairs of every rho_vm, state-major
     std::vector<int32_t> hv((size_t)n_states * ctx->n_v), hm((size_t)n_states * ctx->n_v);
@@ -1100,11 +1144,11 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
             const int64_t off = j * ctx->n_v + v0;
             // rho_vm -> T;  W = V T;  sum_v rho_vm . (V rho_vm)
             CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
-                          ctx->x_nidx.as<int32_t>() + off, ctx->x_midx.as<int32_t>() + off, ctx->T.as<double>(), ldm, nb,
+                          ctx->x_nidx.as<int32_t>() + off, ctx->x_midx.as<int32_t>() + off, ctx->ws().T.as<double>(), ldm, nb,
                           st));
             rs = gemm_v(ctx, nb);
             if (rs != GWL_OK) return rs;
-            CKL(4, launch_dot_partials(ctx->T.as<double>(), ctx->W.as<double>(), ldm, ctx->n_mu, nb,
+            CKL(4, launch_dot_partials(ctx->ws().T.as<double>(), ctx->ws().W.as<double>(), ldm, ctx->n_mu, nb,
                                    ctx->x_part.as<double>(), npart, st));
             CKL(4, launch_accum_neg(ctx->x_part.as<double>(), nb * npart, dout + j, v0 == 0 ? 1 : 0, st));
         }

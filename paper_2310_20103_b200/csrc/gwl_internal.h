@@ -39,9 +39,6 @@ struct GemmParams {
     double* out;          // EPI_STORE: out[z*out_split_stride + n*ldo + m]; CASIDA/START: out[n*ldo + v*n_c + m]
     int64_t ldo;
     int64_t out_split_stride;
-    // FWD / PLAIN with splits > 1 and a co-resident grid: in-kernel reduction of the split-K partials (kr_gemm.cu)
-    unsigned* red_cnt;    // [tiles][2] arrive / done counters, zero between launches; NULL = separate reduction kernel
-    double* out_final;    // [N][ldo] the reduced result
     const double* X;      // EPI_CASIDA: x[n*ldx + v*n_c + m]
     int64_t ldx;
     const double* d2;     // diagonal term [n_vc]: Delta^2 (RPA, operator C) or Delta (TDA, operator A)
@@ -81,10 +78,6 @@ GemmPlan plan_gemm(int mode, int M, int N, int kt_total, int a_wrap, int n_sm);
 // Bytes of GemmParams::ws / ::flags a BWD launch may touch on a device with n_sm SMs.
 size_t gemm_bwd_ws_bytes(int n_sm);
 size_t gemm_bwd_flag_bytes(int n_sm);
-// True when a FWD / PLAIN launch of this plan reduces its split-K partials itself (GemmParams::red_cnt / out_final must
-// then be set; red_cnt holds 2 * tiles counters): more than one split and the whole grid resident at once.
-bool gemm_reduces_in_kernel(const GemmPlan& plan, int M, int N, int n_sm);
-size_t gemm_red_cnt_bytes(int n_sm);
 // Launches; returns cudaGetLastError().  `nz` = splits (FWD/PLAIN) or n_v (BWD).
 cudaError_t launch_gemm(int mode, int epi, const GemmPlan& plan, const GemmParams& p, int nz, cudaStream_t st);
 
@@ -143,6 +136,12 @@ cudaError_t launch_copy_pad(const double* src, int rows, int cols, double* dst, 
 // rho[b][mu] = phi_{n_b}(mu) * phi_{m_b}(mu), orbitals taken from PhiV^T / PhiC^T
 cudaError_t launch_rho(const double* phivT, const double* phicT, int64_t ldt, int n_v, int n_mu, const int32_t* n_idx,
                        const int32_t* m_idx, double* rho, int64_t ld_rho, int nb, cudaStream_t st);
+// The same two passes for complex planar vectors [re (n_vc/2) | im (n_vc/2)] with COMPLEX projection coefficients;
+// npart = reorth_parts(n_vc / 2), coef partials [nb][nslots][2][npart]
+cudaError_t launch_reorth_dots_c(const double* basis, int64_t slot_stride, int nslots, const double* w, int64_t n_vc,
+                                 int nb, double* coefpart, int npart, cudaStream_t st);
+cudaError_t launch_reorth_apply_c(const double* basis, int64_t slot_stride, int nslots, double* w, int64_t n_vc, int nb,
+                                  const double* coefpart, int npart, double* normpart, cudaStream_t st);
 // Planar copies of complex (interleaved re, im) input: dst_{r,i}[k*stride_k + m*stride_m + o*stride_o] = src[k][m][o]
 cudaError_t launch_scatter_complex(const double* src, int n_k, int n_m, int n_o, double* dst_r, double* dst_i,
                                    int64_t stride_k, int64_t stride_m, int64_t stride_o, cudaStream_t st);

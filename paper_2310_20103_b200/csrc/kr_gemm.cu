@@ -307,63 +307,6 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
                         }
                     }
             }
-            if (p.red_cnt != nullptr) {
-                // ---- in-kernel split-K reduction (whole grid co-resident: grid <= SM count, checked by the launcher) ----
-                // Every split of a tile stores its partial, raises the tile's counter and waits until all S splits have
-                // arrived; split z then sums ITS share of the tile over the partials in the fixed order 0..S-1 and writes
-                // the result: deterministic, and the separate reduction launch (and its two kernel boundaries) is gone.
-                // The last split to finish resets both counters, so that they are zero again at the next launch.
-                const int S = (int)gridDim.z;
-                const int tile = (int)(blockIdx.y * gridDim.x + blockIdx.x);
-                unsigned* arrive = p.red_cnt + 2 * tile;
-                unsigned* done = arrive + 1;
-                __threadfence();
-                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
-                if (tid == 0) {
-                    asm volatile("red.release.gpu.global.add.u32 [%0], 1;\n" ::"l"(arrive) : "memory");
-                    unsigned c;
-                    do {
-                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(c) : "l"(arrive) : "memory");
-                    } while (c < (unsigned)S);
-                }
-                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");
-                const int rows_m = min(BM, p.M - m0), cols_n = min(BN, p.N - n0);
-                const int half = (rows_m + 1) >> 1;  // items of two adjacent m (16-byte accesses; ldo and M tiles are even)
-                const int items = half * cols_n;
-                const bool v2 = ((p.ldo & 1) == 0) && ((p.out_split_stride & 1) == 0) &&
-                                (((reinterpret_cast<uintptr_t>(p.out) | reinterpret_cast<uintptr_t>(p.out_final)) & 15) == 0);
-                for (int idx = z * (NCW * 32) + tid; idx < items; idx += S * (NCW * 32)) {
-                    const int n = idx / half, m = 2 * (idx - n * half);
-                    const int64_t off = (int64_t)(n0 + n) * p.ldo + m0 + m;
-                    const bool two = (m + 1 < rows_m);
-                    double a0 = 0.0, a1 = 0.0;
-                    if (v2 && two) {
-                        for (int zz = 0; zz < S; ++zz) {
-                            const double2 t2 = __ldcg(reinterpret_cast<const double2*>(p.out + (int64_t)zz * p.out_split_stride + off));
-                            a0 += t2.x;
-                            a1 += t2.y;
-                        }
-                        *reinterpret_cast<double2*>(p.out_final + off) = make_double2(a0, a1);
-                    } else {
-                        for (int zz = 0; zz < S; ++zz) {
-                            const double* pp = p.out + (int64_t)zz * p.out_split_stride + off;
-                            a0 += __ldcg(pp);
-                            if (two) a1 += __ldcg(pp + 1);
-                        }
-                        p.out_final[off] = a0;
-                        if (two) p.out_final[off + 1] = a1;
-                    }
-                }
-                asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");  // all reads of the partials are done
-                if (tid == 0) {
-                    const unsigned d = atomicAdd(done, 1u);
-                    if (d == (unsigned)S - 1) {  // everybody of this tile has read its share: reset for the next launch
-                        *done = 0u;
-                        __threadfence();
-                        *arrive = 0u;
-                    }
-                }
-            }
         } else {
             // ---- stream-K hand-over: partial tiles go through the workspace, in accumulator order -------------
             // ws[cta][((warp*FM + i)*FN + j)*2 + e][lane]: every store / load of a warp is one 256-byte row
@@ -670,12 +613,6 @@ cudaError_t launch_mode(const GemmPlan& plan, const GemmParams& p0, int nz, cuda
 }
 
 }  // namespace
-
-bool gemm_reduces_in_kernel(const GemmPlan& plan, int M, int N, int n_sm) {
-    const int64_t tiles = ceil_div(M, plan.bm) * ceil_div(N, plan.bn);
-    return plan.splits > 1 && tiles * plan.splits <= n_sm;
-}
-size_t gemm_red_cnt_bytes(int n_sm) { return (size_t)2 * n_sm * sizeof(unsigned); }
 
 size_t gemm_bwd_ws_bytes(int n_sm) { return (size_t)n_sm * 128 * 128 * sizeof(double); }
 size_t gemm_bwd_flag_bytes(int n_sm) { return (size_t)n_sm * sizeof(unsigned); }

@@ -468,6 +468,101 @@ __global__ void __launch_bounds__(NT) k_reorth_apply(const double* __restrict__ 
     }
 }
 
+// ---- the same for complex (planar) Lanczos vectors of the periodic Tamm-Dancoff variant ------------------------------
+// w = [w_r (N) | w_i (N)], N = n_vc / 2.  The projection coefficient on q_j is the COMPLEX <q_j, w> =
+// (q_r.w_r + q_i.w_i) + i (q_r.w_i - q_i.w_r): the real dot of the stacked vectors is only its real part, and rounding
+// feeds the imaginary part just as much (without it the basis lost orthogonality after ~30 steps at 16 384 pairs).
+// coefpart[((b*nslots + i)*2 + part)*npart + blk]; slices run over the N complex elements.
+__global__ void __launch_bounds__(NT) k_reorth_dots_c(const double* __restrict__ basis, int64_t slot_stride, int nslots,
+                                                      const double* __restrict__ w, int64_t n_vc,
+                                                      double* __restrict__ coefpart, int npart, int64_t slice) {
+    pdl_trigger();
+    pdl_wait();
+    extern __shared__ double ws[];  // [RSLICE] w_r chunk, [RSLICE] w_i chunk, [2 nslots] running sums
+    double* wi_s = ws + RSLICE;
+    double* accs = ws + 2 * RSLICE;
+    const int b = blockIdx.y;
+    const int64_t N = n_vc >> 1;
+    const int64_t lo = (int64_t)blockIdx.x * slice;
+    const int64_t len = max((int64_t)0, min(slice, N - lo));
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < 2 * nslots; i += NT) accs[i] = 0.0;
+    for (int64_t c0 = 0; c0 < len; c0 += RSLICE) {
+        const int clen = (int)min((int64_t)RSLICE, len - c0);
+        const double* wb = w + (int64_t)b * n_vc + lo + c0;
+        __syncthreads();
+        for (int j = threadIdx.x; j < clen; j += NT) {
+            ws[j] = wb[j];
+            wi_s[j] = wb[N + j];
+        }
+        __syncthreads();
+        for (int i = warp; i < nslots; i += NT / 32) {
+            const double* qb = basis + (int64_t)i * slot_stride + (int64_t)b * n_vc + lo + c0;
+            double ar0 = 0.0, ar1 = 0.0, ai0 = 0.0, ai1 = 0.0;
+            int j = lane;
+            for (; j + 32 < clen; j += 64) {
+                const double qr0 = __ldg(qb + j), qi0 = __ldg(qb + N + j), qr1 = __ldg(qb + j + 32), qi1 = __ldg(qb + N + j + 32);
+                ar0 = fma(qr0, ws[j], fma(qi0, wi_s[j], ar0));
+                ai0 = fma(qr0, wi_s[j], fma(-qi0, ws[j], ai0));
+                ar1 = fma(qr1, ws[j + 32], fma(qi1, wi_s[j + 32], ar1));
+                ai1 = fma(qr1, wi_s[j + 32], fma(-qi1, ws[j + 32], ai1));
+            }
+            for (; j < clen; j += 32) {
+                const double qr0 = __ldg(qb + j), qi0 = __ldg(qb + N + j);
+                ar0 = fma(qr0, ws[j], fma(qi0, wi_s[j], ar0));
+                ai0 = fma(qr0, wi_s[j], fma(-qi0, ws[j], ai0));
+            }
+            const double sr = warp_sum(ar0 + ar1), si = warp_sum(ai0 + ai1);
+            if (lane == 0) {
+                accs[2 * i] += sr;
+                accs[2 * i + 1] += si;
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 2 * nslots; i += NT) coefpart[((int64_t)b * 2 * nslots + i) * npart + blockIdx.x] = accs[i];
+}
+
+__global__ void __launch_bounds__(NT) k_reorth_apply_c(const double* __restrict__ basis, int64_t slot_stride, int nslots,
+                                                       double* __restrict__ w, int64_t n_vc,
+                                                       const double* __restrict__ coefpart, int npart,
+                                                       double* __restrict__ normpart, int64_t slice) {
+    pdl_trigger();
+    pdl_wait();
+    extern __shared__ double coef[];  // [2 nslots] (re, im) + block_sum scratch
+    double* sh = coef + 2 * nslots;
+    const int b = blockIdx.y;
+    const int64_t N = n_vc >> 1;
+    for (int i = threadIdx.x; i < 2 * nslots; i += NT) {
+        const double* cp = coefpart + ((int64_t)b * 2 * nslots + i) * npart;
+        double t = 0.0;
+        for (int j = 0; j < npart; ++j) t += cp[j];
+        coef[i] = t;
+    }
+    __syncthreads();
+    const int64_t lo = (int64_t)blockIdx.x * slice;
+    const int len = (int)max((int64_t)0, min(slice, N - lo));
+    double* wb = w + (int64_t)b * n_vc + lo;
+    const double* q0 = basis + (int64_t)b * n_vc + lo;
+    double acc = 0.0;
+    for (int j = threadIdx.x; j < len; j += NT) {
+        double vr = wb[j], vi = wb[N + j];
+        for (int i = 0; i < nslots; ++i) {
+            const double qr = __ldg(q0 + (int64_t)i * slot_stride + j), qi = __ldg(q0 + (int64_t)i * slot_stride + N + j);
+            const double cr = coef[2 * i], ci = coef[2 * i + 1];
+            vr -= cr * qr - ci * qi;
+            vi -= cr * qi + ci * qr;
+        }
+        wb[j] = vr;
+        wb[N + j] = vi;
+        acc += vr * vr + vi * vi;
+    }
+    if (normpart != nullptr) {
+        acc = block_sum(acc, sh);
+        if (threadIdx.x == 0) normpart[(int64_t)b * npart + blockIdx.x] = acc;
+    }
+}
+
 // ---- complex (planar) helpers of the periodic Tamm-Dancoff variant -------------------------------------------------
 __global__ void k_scatter_complex(const double* __restrict__ src, int n_k, int n_m, int n_o, double* __restrict__ dst_r,
                                   double* __restrict__ dst_i, int64_t stride_k, int64_t stride_m, int64_t stride_o) {
@@ -727,6 +822,34 @@ cudaError_t launch_reorth_apply(const double* basis, int64_t slot_stride, int ns
     if (ea != cudaSuccess) return ea;
     cudaError_t le = launch_pdl(k_reorth_apply, dim3((unsigned)npart, (unsigned)nb), dim3(NT), sm, st, 1u, basis,
                                 slot_stride, nslots, w, n_vc, coefpart, npart, normpart, reorth_slice(n_vc));
+    count_launch();
+    return le != cudaSuccess ? le : cudaGetLastError();
+}
+
+cudaError_t launch_reorth_dots_c(const double* basis, int64_t slot_stride, int nslots, const double* w, int64_t n_vc,
+                                 int nb, double* coefpart, int npart, cudaStream_t st) {
+    const int64_t N = n_vc / 2;
+    if (npart != reorth_parts(N)) return cudaErrorInvalidValue;
+    const size_t sm = (size_t)(2 * RSLICE + 2 * nslots) * sizeof(double);
+    static SmemAttr attr;
+    cudaError_t ea = attr.ensure(k_reorth_dots_c, sm);
+    if (ea != cudaSuccess) return ea;
+    cudaError_t le = launch_pdl(k_reorth_dots_c, dim3((unsigned)npart, (unsigned)nb), dim3(NT), sm, st, 1u, basis,
+                                slot_stride, nslots, w, n_vc, coefpart, npart, reorth_slice(N));
+    count_launch();
+    return le != cudaSuccess ? le : cudaGetLastError();
+}
+
+cudaError_t launch_reorth_apply_c(const double* basis, int64_t slot_stride, int nslots, double* w, int64_t n_vc, int nb,
+                                  const double* coefpart, int npart, double* normpart, cudaStream_t st) {
+    const int64_t N = n_vc / 2;
+    if (npart != reorth_parts(N)) return cudaErrorInvalidValue;
+    const size_t sm = (size_t)(2 * nslots + NT / 32 + 1) * sizeof(double);
+    static SmemAttr attr;
+    cudaError_t ea = attr.ensure(k_reorth_apply_c, sm);
+    if (ea != cudaSuccess) return ea;
+    cudaError_t le = launch_pdl(k_reorth_apply_c, dim3((unsigned)npart, (unsigned)nb), dim3(NT), sm, st, 1u, basis,
+                                slot_stride, nslots, w, n_vc, coefpart, npart, normpart, reorth_slice(N));
     count_launch();
     return le != cudaSuccess ? le : cudaGetLastError();
 }
