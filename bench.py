@@ -48,6 +48,10 @@ def parse():
                     help="index into BASELINE.json:configs (default 4, the largest; 2 with --sharded-state)")
     ap.add_argument("--full", action="store_true", help="all chains x full L of the config instead of the bounded pass")
     ap.add_argument("--chains", type=int, default=0, help="override the number of chains of a pass (marks the line)")
+    ap.add_argument("--tdc", default="", metavar="NK,NV,NC,NMU",
+                    help="context run, not the bench line: the complex-orbital Tamm-Dancoff variant (SURVEY 8(f)-3) on a "
+                         "synthetic periodic problem of that shape, e.g. 4,64,1024,6144; block = --chains (default 128), "
+                         "L = --lanczos-steps (default 10)")
     ap.add_argument("--sharded-state", action="store_true",
                     help="SURVEY 8(f)-2 arm, its own line: the N_v+N_c chains of ONE state partitioned over the ranks "
                          "(runtime.shard_range), one NCCL all-reduce of the omega grid; strong scaling")
@@ -166,7 +170,7 @@ def run_paper_setting(args):
     """One quasiparticle state the way the paper runs it: Lanczos on p_g(C), g = 7,
     N_iter = 8, one chain per n = 1..N_v+N_c, then Sigma^x and the Newton-Raphson solve.  Context for BASELINE.md's
     Table I quotes (the paper's wall times include the CPU-only ISDF step and real data; this is the hot path only, on
-    synthetic inputs of the same shape).  The fitting range comes from a 40-step Lanczos estimate of the top of the
+    synthetic inputs of the same shape).  The fitting range comes from a 24-step Lanczos estimate of the top of the
     spectrum (polyfit.range_from_spectrum), inside the timed state."""
     import torch
 
@@ -197,7 +201,7 @@ def run_paper_setting(args):
 
     def state():
         ctx.set_polynomial(0)
-        lo, hi = polyfit.range_from_spectrum(ctx, prob.eps_v, prob.eps_c, steps=40)
+        lo, hi = polyfit.range_from_spectrum(ctx, prob.eps_v, prob.eps_c, steps=24)
         rng[:] = [lo, hi]
         ctx.set_polynomial(g, polyfit.sqrt_chebyshev(g, lo, hi), lo, hi)
         ctx.selfenergy_state(m, n_iter, block, 0, om, 0.68, out=sc[0])        # delta = 0.05 Ry
@@ -224,17 +228,82 @@ def run_paper_setting(args):
     tot = sum(v[0] for v in kt.values())
     share = {k: round(v[0] / tot, 4) for k, v in kt.items() if v[1]}
     per_launch_ms = {k: round(v[0] / v[1], 4) for k, v in kt.items() if v[1]}
-    flop = (n_orb * n_iter * g + 40) * (4.0 * n_mu * n_v * n_c + 2.0 * n_mu * n_mu)
+    flop = (n_orb * n_iter * g + 24) * (4.0 * n_mu * n_v * n_c + 2.0 * n_mu * n_mu)
     line = {"metric": "seconds_per_quasiparticle_state", "value": sec, "unit": "s", "higher_is_better": False,
             "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "paper setting: N_iter = 8, g = 7 (PAPER.md:145), all N_v+N_c chains of one state, "
-                                   "Sigma^x, Newton-Raphson; fitting range from a 40-step Lanczos bound (PAPER.md:284)",
+                                   "Sigma^x, Newton-Raphson; fitting range from a 24-step Lanczos bound (PAPER.md:284)",
                        "n_v": n_v, "n_c": n_c, "n_mu": n_mu, "chains": n_orb, "block": block,
                        "fit_range_eV2": rng},
-            "c_applies": n_orb * n_iter * g + 40, "tflops_flop_model": flop / sec / 1e12,
+            "c_applies": n_orb * n_iter * g + 24, "tflops_flop_model": flop / sec / 1e12,
             "gpu_launches": launches, "kernel_time_share": share, "kernel_ms_per_launch": per_launch_ms,
             "e_qp_eV": float(out[0].item()), "z": float(out[1].item()),
             "note": "context only: hot path on synthetic inputs; the paper's Table I wall times include ISDF on CPUs"}
+    print(json.dumps(line), flush=True)
+    ctx.close()
+
+
+def run_tdc(args):
+    """Complex-orbital Tamm-Dancoff variant (gwl_tdc_*): one block of chains x L Lanczos steps on the Hermitian A(q) + Sigma,
+    with the complex Khatri-Rao GEMMs against the DMMA roofline (8 N_mu N_kvc B real flop per launch: 4 real multiply-adds
+    per complex one)."""
+    import torch
+
+    from paper_2310_20103_b200 import gwl, synth
+
+    n_k, n_v, n_c, n_mu = (int(x) for x in args.tdc.split(","))
+    nch = args.chains or 128
+    L = args.lanczos_steps or 10
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    gwl.load_library()
+    p = synth.make_periodic(n_k, n_v, n_c, n_mu, box=20.0, seed=0, n_omega=401, n_chains=nch)
+    ctx = gwl.TdcContext(n_k, n_v, n_c, n_mu, 1)
+    stream = torch.cuda.current_stream()
+    ctx.set_stream(stream.cuda_stream)
+    ctx.set_orbitals(p.psi_v, p.psi_cq)
+    ctx.set_energies(p.eps_v, p.eps_cq)
+    ctx.set_kernel(p.V)
+    ctx.set_chains(p.chains)
+    ctx.set_pointer_mode(1)
+    ctx.set_profiling(0)
+    om = torch.from_numpy(p.omega).to(dev)
+    ssum = torch.empty(len(p.omega), 2, dtype=torch.float64, device=dev)
+    peak = gwl.probe_fp64_peak(0)
+
+    def step():
+        ctx.lanczos(nch, L, nch, 0, out=None)
+        ctx.selfenergy(om, 0.1, out=(None, ssum))
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        a.record(stream)
+        step()
+        b.record(stream)
+    torch.cuda.synchronize()
+    sec = sum(a.elapsed_time(b) for a, b in ev) * 1e-3 / args.steps
+    ctx.set_profiling(2)
+    step()
+    kt = ctx.get_kernel_times()
+    ctx.set_profiling(0)
+    n_kvc = n_k * n_v * n_c
+    fl = 8.0 * n_mu * n_kvc * nch
+    per = {k: v[0] / v[1] for k, v in kt.items() if v[1]}
+    line = {"metric": METRIC, "value": nch * L / sec, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * sec, "higher_is_better": True, "dtype": "complex f64 (planar)", "data": "synthetic",
+            "arm": "tdc (SURVEY 8(f)-3): context run, not the headline bench line",
+            "config": {"workload": "periodic Tamm-Dancoff: Lanczos on the Hermitian A(q), one block of chains", "n_k": n_k,
+                       "n_v": n_v, "n_c": n_c, "n_mu": n_mu, "n_kvc": n_kvc, "chains": nch, "lanczos_steps": L},
+            "roofline": {"bound": "tensor", "peak": peak, "unit": "TFLOP/s",
+                         "Kx": {"achieved": fl / (per["gemm_fwd_KX"] * 1e-3) / 1e12, "ms_per_launch": per["gemm_fwd_KX"]},
+                         "KhW": {"achieved": fl / (per["gemm_bwd_KtW"] * 1e-3) / 1e12, "ms_per_launch": per["gemm_bwd_KtW"]},
+                         "flop_per_launch": fl, "flop_model": "8 N_mu N_kvc B real flop (4 real multiply-adds per complex one)"},
+            "kernel_time_share": {k: round(v[0] / sum(x[0] for x in kt.values()), 4) for k, v in kt.items() if v[1]}}
+    line["roofline"]["Kx"]["frac"] = line["roofline"]["Kx"]["achieved"] / peak
+    line["roofline"]["KhW"]["frac"] = line["roofline"]["KhW"]["achieved"] / peak
     print(json.dumps(line), flush=True)
     ctx.close()
 
@@ -348,6 +417,9 @@ def main():
         return
     if args.sharded_state:
         run_sharded_state(args)
+        return
+    if args.tdc:
+        run_tdc(args)
         return
 
     import torch

@@ -203,6 +203,17 @@ gwl_status gwl_tdc_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec
 gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, const double* phi_c_grid, const double* r,
                           double weight, double soft, const int32_t* idx, double* zeta_t, double* V_out);
 
+/* Interpolation points for gwl_isdf_build by centroidal Voronoi tessellation (weighted k-means).  PAPER.md:128 names the
+ * ISDF method of its refs. [13, 62, 63] and is silent on how the points are chosen; this is the k-means choice of that
+ * literature (reading Q22).  Lloyd iterations on the grid points r [n_r][3] with weights weight [n_r] >= 0 (e.g.
+ * sum_n phi_n(r)^2): assign every point to its nearest centroid (ties: the lowest centroid index), move every centroid to
+ * the weighted mean of its points (an empty cluster keeps its centroid), starting from the grid points init_idx [n_mu],
+ * at most max_iters times or until no assignment changes; finally every centroid is replaced by the nearest grid point of
+ * its own cluster (ties: the lowest index), so the n_mu = ctx's N_mu points are distinct.  Host arrays; idx [n_mu] receives
+ * the grid indices (-1 for a cluster that ended empty), *iters_done (may be NULL) the number of centroid updates. */
+gwl_status gwl_isdf_select_points(gwl_ctx* ctx, int64_t n_r, const double* r, const double* weight, const int32_t* init_idx,
+                                  int64_t max_iters, int32_t* idx, int32_t* iters_done);
+
 /* CUDA-event totals (ms) of the last gwl_lanczos: time inside Casida products (S2), inside the Lanczos
  * vector kernels (S4) and overall.  Any pointer may be NULL.  Synchronises the stream. */
 gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total);

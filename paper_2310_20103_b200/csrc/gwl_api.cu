@@ -1522,6 +1522,56 @@ gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, c
     return GWL_OK;
 }
 
+gwl_status gwl_isdf_select_points(gwl_ctx* ctx, int64_t n_r, const double* r, const double* weight, const int32_t* init_idx,
+                                  int64_t max_iters, int32_t* idx, int32_t* iters_done) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (r == nullptr || weight == nullptr || init_idx == nullptr || idx == nullptr)
+        return ctx->fail(GWL_EINVAL, "gwl_isdf_select_points: NULL argument");
+    const int n_mu = ctx->n_mu;
+    if (n_r < n_mu || n_r > (1 << 30) || max_iters < 0 || max_iters > 100000)
+        return ctx->fail(GWL_EINVAL, "gwl_isdf_select_points: need n_mu <= n_r and 0 <= max_iters <= 100000");
+    for (int m = 0; m < n_mu; ++m)
+        if (init_idx[m] < 0 || init_idx[m] >= n_r) return ctx->fail(GWL_EINVAL, "gwl_isdf_select_points: init_idx out of range");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int nr = (int)n_r;
+    // scratch in isdf_s: r [n_r][3], w [n_r], c [n_mu][3], assign [n_r], idx [n_mu], changed
+    DevBuf& buf = ctx->isdf_s;
+    CK(buf.ensure((size_t)n_r * 32 + (size_t)n_mu * 24 + (size_t)n_r * 4 + (size_t)n_mu * 4 + 16, st));
+    double* d_r = buf.as<double>();
+    double* d_w = d_r + (size_t)n_r * 3;
+    double* d_c = d_w + n_r;
+    int32_t* d_assign = reinterpret_cast<int32_t*>(d_c + (size_t)n_mu * 3);
+    int32_t* d_idx = d_assign + n_r;
+    int* d_changed = d_idx + n_mu;
+    std::vector<double> c0((size_t)n_mu * 3);
+    for (int m = 0; m < n_mu; ++m)
+        for (int q = 0; q < 3; ++q) c0[3 * (size_t)m + q] = r[3 * (size_t)init_idx[m] + q];
+    CK(cudaMemcpyAsync(d_r, r, (size_t)n_r * 24, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(d_w, weight, (size_t)n_r * 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(d_c, c0.data(), (size_t)n_mu * 24, cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(d_assign, 0xff, (size_t)n_r * 4, st));  // -1: the first assignment always counts as a change
+    int done = 0;
+    for (int it = 0; it < max_iters; ++it) {
+        int changed = 0;
+        CK(cudaMemsetAsync(d_changed, 0, 4, st));
+        CKL(4, launch_cvt_assign(d_r, nr, d_c, n_mu, d_assign, d_changed, st));
+        CK(cudaMemcpyAsync(&changed, d_changed, 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));  // a set-up step: the host decides whether Lloyd has converged
+        if (!changed) break;
+        CKL(4, launch_cvt_update(d_r, d_w, nr, d_assign, n_mu, d_c, st));
+        done = it + 1;
+    }
+    CK(cudaMemsetAsync(d_changed, 0, 4, st));
+    CKL(4, launch_cvt_assign(d_r, nr, d_c, n_mu, d_assign, d_changed, st));
+    CKL(4, launch_cvt_snap(d_r, nr, d_assign, d_c, n_mu, d_idx, st));
+    CK(cudaMemcpyAsync(idx, d_idx, (size_t)n_mu * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (iters_done != nullptr) *iters_done = done;
+    return GWL_OK;
+}
+
 gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);

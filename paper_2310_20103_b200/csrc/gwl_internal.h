@@ -240,6 +240,15 @@ cudaError_t launch_cholesky(double* S, int64_t ld, int n, double* scale, int* in
 // X <- (L L^T)^{-1} X for X [n][ldx] with n_r columns
 cudaError_t launch_cholesky_solve(const double* L, int64_t ldl, int n, double* X, int64_t ldx, int n_r, cudaStream_t st);
 
+// Weighted k-means (centroidal Voronoi) selection of the interpolation points: nearest-centroid assignment (sets *changed
+// when an assignment differs from the stored one), deterministic centroid update, snap to the nearest member grid point
+cudaError_t launch_cvt_assign(const double* r, int n_r, const double* c, int n_mu, int32_t* assign, int* changed,
+                              cudaStream_t st);
+cudaError_t launch_cvt_update(const double* r, const double* w, int n_r, const int32_t* assign, int n_mu, double* c,
+                              cudaStream_t st);
+cudaError_t launch_cvt_snap(const double* r, int n_r, const int32_t* assign, const double* c, int n_mu, int32_t* idx,
+                            cudaStream_t st);
+
 // probe.cu
 cudaError_t probe_fp64_peak(int kind, double* tflops);
 

@@ -228,6 +228,110 @@ __global__ void k_trsm_bwd(const double* __restrict__ L, int64_t ldl, int n, dou
         if (i < nb) X[(int64_t)(k0 + i) * ldx + c] = acc[i];
 }
 
+
+// ---- interpolation points by centroidal Voronoi tessellation (weighted k-means, Lloyd) -------------------------------
+// assign: a_i = argmin_mu |r_i - c_mu|^2, ties to the lowest mu; d2 = (dx dx + dy dy) + dz dz in that order
+__global__ void k_cvt_assign(const double* __restrict__ r, int n_r, const double* __restrict__ c, int n_mu,
+                             int32_t* __restrict__ assign, int* __restrict__ changed) {
+    extern __shared__ double cs[];  // centroids, chunk of up to 1024
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double x = 0.0, y = 0.0, z = 0.0;
+    if (i < n_r) {
+        x = r[3 * i];
+        y = r[3 * i + 1];
+        z = r[3 * i + 2];
+    }
+    double best = INFINITY;
+    int arg = 0;
+    for (int m0 = 0; m0 < n_mu; m0 += 1024) {
+        const int nm = min(1024, n_mu - m0);
+        __syncthreads();
+        for (int t = threadIdx.x; t < 3 * nm; t += blockDim.x) cs[t] = c[3 * m0 + t];
+        __syncthreads();
+        for (int m = 0; m < nm; ++m) {
+            const double dx = x - cs[3 * m], dy = y - cs[3 * m + 1], dz = z - cs[3 * m + 2];
+            const double d2 = (dx * dx + dy * dy) + dz * dz;
+            if (d2 < best) {
+                best = d2;
+                arg = m0 + m;
+            }
+        }
+    }
+    if (i < n_r) {
+        if (assign[i] != arg) *changed = 1;
+        assign[i] = arg;
+    }
+}
+
+// update: one CTA per cluster walks all points in index order (fixed slices, fixed tree: deterministic);
+// c_mu = sum w r / sum w over its members, unchanged if the cluster is empty
+__global__ void k_cvt_update(const double* __restrict__ r, const double* __restrict__ w, int n_r,
+                             const int32_t* __restrict__ assign, double* __restrict__ c) {
+    __shared__ double sh[4][256];
+    const int mu = blockIdx.x;
+    double sw = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int i = threadIdx.x; i < n_r; i += 256) {
+        if (assign[i] == mu) {
+            const double wi = w[i];
+            sw += wi;
+            sx += wi * r[3 * i];
+            sy += wi * r[3 * i + 1];
+            sz += wi * r[3 * i + 2];
+        }
+    }
+    sh[0][threadIdx.x] = sw;
+    sh[1][threadIdx.x] = sx;
+    sh[2][threadIdx.x] = sy;
+    sh[3][threadIdx.x] = sz;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o)
+            for (int q = 0; q < 4; ++q) sh[q][threadIdx.x] += sh[q][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0 && sh[0][0] > 0.0) {
+        c[3 * mu] = sh[1][0] / sh[0][0];
+        c[3 * mu + 1] = sh[2][0] / sh[0][0];
+        c[3 * mu + 2] = sh[3][0] / sh[0][0];
+    }
+}
+
+// snap: idx_mu = the member grid point nearest to c_mu (ties: the lowest i); -1 for an empty cluster
+__global__ void k_cvt_snap(const double* __restrict__ r, int n_r, const int32_t* __restrict__ assign,
+                           const double* __restrict__ c, int32_t* __restrict__ idx) {
+    __shared__ double bd[256];
+    __shared__ int bi[256];
+    const int mu = blockIdx.x;
+    const double cx = c[3 * mu], cy = c[3 * mu + 1], cz = c[3 * mu + 2];
+    double best = INFINITY;
+    int arg = -1;
+    for (int i = threadIdx.x; i < n_r; i += 256) {
+        if (assign[i] == mu) {
+            const double dx = r[3 * i] - cx, dy = r[3 * i + 1] - cy, dz = r[3 * i + 2] - cz;
+            const double d2 = (dx * dx + dy * dy) + dz * dz;
+            if (d2 < best) {  // i ascends within a thread: the first minimum is the lowest index
+                best = d2;
+                arg = i;
+            }
+        }
+    }
+    bd[threadIdx.x] = best;
+    bi[threadIdx.x] = arg;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            const double d = bd[threadIdx.x + o];
+            const int j = bi[threadIdx.x + o];
+            if (j >= 0 && (bi[threadIdx.x] < 0 || d < bd[threadIdx.x] || (d == bd[threadIdx.x] && j < bi[threadIdx.x]))) {
+                bd[threadIdx.x] = d;
+                bi[threadIdx.x] = j;
+            }
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) idx[mu] = bi[0];
+}
+
 }  // namespace
 
 cudaError_t launch_gather_rows(const double* src, int64_t ld_src, int n_cols, const int32_t* idx, int n_mu, double* dst,
@@ -287,6 +391,27 @@ cudaError_t launch_cholesky_solve(const double* L, int64_t ldl, int n, double* X
         k_trsm_bwd<<<g, 128, 0, st>>>(L, ldl, n, X, ldx, n_r, k0);
         count_launch();
     }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cvt_assign(const double* r, int n_r, const double* c, int n_mu, int32_t* assign, int* changed,
+                              cudaStream_t st) {
+    k_cvt_assign<<<(unsigned)ceil_div(n_r, 256), 256, 3 * 1024 * sizeof(double), st>>>(r, n_r, c, n_mu, assign, changed);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cvt_update(const double* r, const double* w, int n_r, const int32_t* assign, int n_mu, double* c,
+                              cudaStream_t st) {
+    k_cvt_update<<<(unsigned)n_mu, 256, 0, st>>>(r, w, n_r, assign, c);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cvt_snap(const double* r, int n_r, const int32_t* assign, const double* c, int n_mu, int32_t* idx,
+                            cudaStream_t st) {
+    k_cvt_snap<<<(unsigned)n_mu, 256, 0, st>>>(r, n_r, assign, c, idx);
+    count_launch();
     return cudaGetLastError();
 }
 

@@ -18,7 +18,7 @@ thread_local int64_t* g_launch_counter = nullptr;
 
 namespace {
 
-constexpr int FWD_VCHUNK = 64;   // K.X k-tile order: occupied orbitals per chunk (see the producer loop)
+constexpr int FWD_VCHUNK = 256;  // K.X k-tile order: occupied orbitals per chunk (see the producer loop)
 constexpr int BWD_MIN_UNITS = 16;  // fewest k-tiles worth handing to one more CTA
 
 template <int BM, int BN, int MODE>

@@ -50,6 +50,7 @@ SIGNATURES = {
     "gwl_tdc_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
     "gwl_isdf_build": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_double, c_double, c_void_p, c_void_p,
                                c_void_p]),
+    "gwl_isdf_select_points": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_int64, c_void_p, POINTER(c_int32)]),
     "gwl_get_timing": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
     "gwl_set_profiling": (c_int, [c_void_p, c_int]),
     "gwl_get_kernel_times": (c_int, [c_void_p, POINTER(c_double), POINTER(c_int64)]),
@@ -207,6 +208,18 @@ class Context:
         self._ck(self._lib.gwl_isdf_build(self._h, n_r, _ptr(pv), _ptr(pc), _ptr(rr), float(weight), float(soft), _ptr(ix),
                                           _ptr(zt), _ptr(V)))
         return zt, V
+
+    def isdf_select_points(self, r, weight, init_idx, max_iters: int = 50):
+        """Weighted k-means (CVT) interpolation points; returns (idx [n_mu] int32, iterations done)."""
+        rr, w, ii = _host(r), _host(weight), _host(init_idx, np.int32)
+        n_r = rr.shape[0]
+        if rr.shape != (n_r, 3) or w.shape != (n_r,) or ii.shape != (self.n_mu,):
+            raise GwlError(GWL_EINVAL, "isdf_select_points: r [n_r, 3], weight [n_r], init_idx [n_mu]")
+        idx = np.zeros(self.n_mu, dtype=np.int32)
+        done = c_int32(0)
+        self._ck(self._lib.gwl_isdf_select_points(self._h, n_r, _ptr(rr), _ptr(w), _ptr(ii), int(max_iters), _ptr(idx),
+                                                  byref(done)))
+        return idx, done.value
 
     # -- the path ---------------------------------------------------------------------------------
     def casida_matvec(self, x, y=None):

@@ -83,3 +83,32 @@ def test_isdf_rejects_bad_points_and_rank_deficient_fits():
         assert e.value.status == gwl.GWL_EINVAL and "positive definite" in str(e.value)
         with pytest.raises(gwl.GwlError):
             ctx.casida_matvec(np.zeros((1, 2, 3)))                        # nothing was installed
+
+
+def test_cvt_point_selection_matches_oracle_and_feeds_the_fit():
+    """gwl_isdf_select_points (weighted k-means) against the oracle: the same integer grid indices and iteration count
+    (both sides decide nearest-centroid in FP64 with the same expression and tie rule), on the uniform box grid with the
+    density as weight and on a random cloud with random weights; the selected points then go through gwl_isdf_build."""
+    n_v, n_c, n_mu = 3, 6, 24
+    r, phi, w, _ = _problem(10, n_v, n_c, n_mu)
+    dens = (phi ** 2).sum(axis=1)
+    init = synth.stride_points(r.shape[0], n_mu, 5)
+    ref_idx, ref_done, _ = isdf.select_points_cvt(r, dens, init, 50)
+    with gwl.Context(n_v, n_c, n_mu) as ctx:
+        idx, done = ctx.isdf_select_points(r, dens, init, 50)
+        assert np.array_equal(idx, ref_idx) and done == ref_done
+        idx1, done1 = ctx.isdf_select_points(r, dens, init, 1)                  # stopped by max_iters
+        ref1, rdone1, _ = isdf.select_points_cvt(r, dens, init, 1)
+        assert np.array_equal(idx1, ref1) and done1 == rdone1 == 1
+        zt, V = ctx.isdf_build(phi[:, :n_v], phi[:, n_v:], r, w, 0.5, idx)
+    zeta = isdf.fit(phi, phi, ref_idx)
+    assert np.abs(zt.T - zeta).max() <= 1e-9 * np.abs(zeta).max()
+    rng = np.random.default_rng(7)
+    cloud = rng.random((3000, 3)) * 12.0
+    wts = rng.random(3000) + 0.1
+    init = synth.stride_points(3000, 50, 2)
+    ref_idx, ref_done, _ = isdf.select_points_cvt(cloud, wts, init, 100)
+    with gwl.Context(2, 2, 50) as ctx:
+        idx, done = ctx.isdf_select_points(cloud, wts, init, 100)
+    assert np.array_equal(idx, ref_idx) and done == ref_done
+    assert len(set(idx.tolist())) == 50

@@ -69,3 +69,36 @@ def test_two_orbital_sets_fit_only_their_cross_pairs():
     assert np.linalg.norm(Z - zeta @ Z[idx]) <= 1e-8 * np.linalg.norm(Z)       # 12 pairs, 12 points
     Pv, Pc = pv @ pv[idx].T, pc @ pc[idx].T
     assert np.abs(zeta @ (Pv[idx] * Pc[idx]) - Pv * Pc).max() <= 1e-9 * np.abs(Pv * Pc).max()
+
+
+# ---- interpolation points by weighted k-means (reading Q22) ------------------------------------------------------
+def test_cvt_two_cluster_closed_form():
+    """Six collinear points in two groups, unit weights, both initial centroids in the left group: Lloyd must end with the
+    groups {0,1,2} and {10,11,12}, centroids 1 and 11, i.e. the grid points 1 and 4."""
+    x = np.array([0.0, 1.0, 2.0, 10.0, 11.0, 12.0])
+    r = np.stack([x, np.zeros(6), np.zeros(6)], axis=1)
+    idx, done, obj = isdf.select_points_cvt(r, np.ones(6), np.array([0, 1]), 20)
+    assert list(idx) == [1, 4]
+    assert abs(obj[-1] - 4.0) <= 1e-12                      # 2 x (1 + 0 + 1)
+    # weights move the centroid: heavy point 12 pulls the right centroid to 11.5 -> nearest member is 11 (index 4) or 12 (5): tie -> lowest
+    idx_w, _, _ = isdf.select_points_cvt(r, np.array([1, 1, 1, 1, 1, 3.0]), np.array([0, 1]), 20)
+    c_right = (10 + 11 + 3 * 12) / 5.0
+    assert idx_w[0] == 1 and idx_w[1] == (4 if abs(11 - c_right) <= abs(12 - c_right) else 5)
+
+
+def test_cvt_objective_decreases_and_points_are_valid():
+    r, phi, w, _ = _setup(n_grid=10, n_orb=9)
+    dens = (phi ** 2).sum(axis=1)
+    init = synth.stride_points(r.shape[0], 24, 5)
+    idx, done, obj = isdf.select_points_cvt(r, dens, init, 50)
+    assert all(b <= a * (1 + 1e-14) for a, b in zip(obj, obj[1:]))          # Lloyd never increases the weighted objective
+    assert done < 50 and len(set(idx.tolist())) == 24 and idx.min() >= 0 and idx.max() < r.shape[0]
+    # a converged tessellation is a fixed point: restarting from the selected points' centroids changes nothing further
+    idx2, done2, _ = isdf.select_points_cvt(r, dens, init, done + 5)
+    assert np.array_equal(idx, idx2) and done2 == done
+    # and it serves its purpose: C C^T at these points is far better conditioned than at the seeded random points
+    def cond(ix):
+        P = phi @ phi[ix].T
+        ev = np.linalg.eigvalsh(P[ix] * P[ix])
+        return ev[-1] / ev[0]
+    assert cond(idx) < 1e-2 * cond(init)
