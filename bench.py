@@ -566,6 +566,28 @@ def main():
               "flop_model": "(4 N_mu N_vc + 2 N_mu^2) B", "block_products_timed": n_mv,
               "how": "mean launch duration of K.X + V.T + K^T.W (+ split-K reductions per product)"}
 
+    # ---- the block product alone, through its own C-ABI call (gwl_casida_matvec, device pointers), back to back ----------
+    # (the per-launch sum above is taken with an event pair around every launch, which breaks the overlap of a kernel's
+    # prologue with its predecessor's tail; this is the same product as a user calls it, launch gaps included)
+    xb = torch.randn(nbl, cfg.n_v, cfg.n_c, dtype=torch.float64, device=dev)
+    yb = torch.empty_like(xb)
+    mv_reps = max(3, min(200, int(0.5 / max(mv_ms * 1e-3, 1e-6))))
+    for _ in range(2):
+        ctx.casida_matvec(xb, yb)
+    torch.cuda.synchronize()
+    m0, m1 = ev(), ev()
+    m0.record(stream)
+    for _ in range(mv_reps):
+        ctx.casida_matvec(xb, yb)
+    m1.record(stream)
+    torch.cuda.synchronize()
+    abi_ms = m0.elapsed_time(m1) / mv_reps
+    matvec["abi_call"] = {"ms_per_block_matvec": abi_ms, "tflops": fpv / (abi_ms * 1e-3) / 1e12,
+                          "frac_of_dmma_peak": fpv / (abi_ms * 1e-3) / 1e12 / dmma_peak, "reps": mv_reps,
+                          "how": "gwl_casida_matvec(block) in device-pointer mode, back-to-back calls between two CUDA "
+                                 "events; includes the sqrt(Delta) prescale kernel and every launch gap"}
+    del xb, yb
+
     # ---- end-to-end arm: host buffers through the C ABI --------------------------------------------------
     e2e = None
     if not args.no_e2e:
