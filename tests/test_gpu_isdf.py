@@ -87,10 +87,14 @@ def test_isdf_rejects_bad_points_and_rank_deficient_fits():
 
 def test_cvt_point_selection_matches_oracle_and_feeds_the_fit():
     """gwl_isdf_select_points (weighted k-means) against the oracle: the same integer grid indices and iteration count
-    (both sides decide nearest-centroid in FP64 with the same expression and tie rule), on the uniform box grid with the
-    density as weight and on a random cloud with random weights; the selected points then go through gwl_isdf_build."""
+    (both sides decide nearest-centroid in FP64 with the same expression and tie rule), on the box grid with the
+    density as weight and on a random cloud with random weights; the selected points then go through gwl_isdf_build.
+    The box grid is jittered by 1e-3 A: on the exact uniform grid with its symmetric density many points are equidistant from
+    two centroids up to the rounding of the centroid sums, whose summation order (NumPy pairwise, CUDA tree) is not part of the
+    method, so the integer result would hinge on the last bit; exact ties still follow the lowest-index rule on both sides."""
     n_v, n_c, n_mu = 3, 6, 24
     r, phi, w, _ = _problem(10, n_v, n_c, n_mu)
+    r = r + 1e-3 * np.random.default_rng(11).standard_normal(r.shape)
     dens = (phi ** 2).sum(axis=1)
     init = synth.stride_points(r.shape[0], n_mu, 5)
     ref_idx, ref_done, _ = isdf.select_points_cvt(r, dens, init, 50)
