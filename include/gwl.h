@@ -89,7 +89,9 @@ gwl_status gwl_spectrum_bounds(gwl_ctx* ctx, int64_t steps, double* lam_min, dou
  * orbitals and one k-point: the operator becomes A = diag(Delta) + K^T V K (Eq. 2), chains start from
  * P_vc = (nm|vc) (no sqrt(Delta) factor), gwl_casida_matvec applies A, and gwl_selfenergy evaluates
  * Sigma(omega, n) = <P| 1/(omega - eps_n + eta_n (A - i eta)) |P> = -eta_n R_A(-eta_n z_n) by Eq. 14.
- * Switching invalidates the results of the last gwl_lanczos.  GWL_ESTATE if a polynomial is set (it fits sqrt(C)). */
+ * Switching invalidates the results of the last gwl_lanczos.  GWL_ESTATE if a polynomial is set (it fits sqrt(C)).
+ * On a complex-orbital context (gwl_tdc_create, below) GWL_TDA is the default and GWL_RPA selects the pseudo-Hermitian
+ * Lanczos for the full C^RPA(q) described there. */
 #define GWL_RPA 0
 #define GWL_TDA 1
 gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation);
@@ -171,7 +173,19 @@ gwl_status gwl_qp_solve(gwl_ctx* ctx, int64_t n_states, const double* eps_m, con
  * gwl_tdc_set_chains / gwl_tdc_matvec and then gwl_lanczos, gwl_resolvent, gwl_selfenergy, gwl_get_* exactly as above
  * (alpha, beta are real: A is Hermitian; gwl_selfenergy includes the prefactor 2/(N_q N_k) in every chain and evaluates
  * Eq. 14 at -eta_n z_n as in GWL_TDA); the real-orbital set_* calls, gwl_set_polynomial, gwl_exchange return GWL_ESTATE.
- * The pseudo-Hermitian Lanczos for the full RPA matrix with complex orbitals is not part of this library. */
+ *
+ * Full RPA with complex orbitals (gwl_set_approximation(ctx, GWL_RPA) on such a context): "if RPA is used, then a Lanczos-based
+ * method designed for pseudo-Hermitian matrices can be adopted".  The paper fixes the target,
+ *   Sigma^corr_{mk,mk}(omega) = 2/(N_q N_k) sum_n sum_q sum_s |W^s|^2 / (omega - eps_{nk-q} + eta (Omega_s(q) - i delta)),
+ *   W^s = sum_j [ (nk-q, mk | v'k', c'k'+q) X^s_j + (nk-q, mk | c'k'+q, v'k') Y^s_j ],
+ * over the positive eigenvalues of C^RPA(q) = [[A, B], [-B^*, -A^*]], B = K^H V conj(K), and leaves the
+ * Lanczos scheme to its refs. [34, 36, 74]; the one built here (reading Q24): C^RPA = F Omega^ with F = diag(1, -1) and
+ * Omega^ = [[A, B], [B^*, A^*]] Hermitian positive definite is self-adjoint in <a, b>_O = a^H Omega^ b, so a three-term Lanczos
+ * in that inner product, started from u = F conj([P1; P2]) (the printed integrals), gives a real symmetric T_L with
+ *   sum_{s: Omega_s > 0} |W^s|^2 g(Omega_s) ~ <u,u>_O sum_{i: theta_i > 0} w_i g(theta_i) / theta_i     (Ritz pairs of T_L),
+ * exact at L = 2 N_k N_v N_c.  One step costs one product with Omega^ (2 K, 1 V, 2 K^H contractions: twice a TDA step).
+ * gwl_lanczos then returns the alpha, beta of that T_L and norm2 = <u,u>_O; gwl_selfenergy evaluates the sum above (with the
+ * prefactor); gwl_resolvent gives <u|(zeta - C^RPA)^{-1}|u>_O by Eq. 14 (both branches). */
 gwl_status gwl_tdc_create(gwl_ctx** out, int64_t n_k, int64_t n_v, int64_t n_c, int64_t n_mu, int64_t n_q);
 /* psi_v [n_k][n_mu][n_v][2] = psi_{v k}(r_mu); psi_cq [n_k][n_mu][n_c][2] = psi_{c k+q}(r_mu) (slot k holds the conduction
  * orbitals of momentum k+q: the caller does the momentum bookkeeping).  Host. */
@@ -186,6 +200,9 @@ gwl_status gwl_tdc_set_energies(gwl_ctx* ctx, const double* eps_v, const double*
 gwl_status gwl_tdc_set_chains(gwl_ctx* ctx, int64_t n_chains, const int32_t* chains);
 /* y = A(q) x for nvec complex vectors x, y [nvec][n_k][n_v][n_c][2] (pointer mode applies); x and y must not overlap. */
 gwl_status gwl_tdc_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec);
+/* [ox; oy] = Omega^ [x; y] = [A x + B y; B^* x + A^* y] (C^RPA [x; y] = [ox; -oy]) for nvec pairs of complex
+ * vectors, each [nvec][n_k][n_v][n_c][2] (pointer mode applies); inputs and outputs must not overlap.  Either approximation. */
+gwl_status gwl_tdc_matvec_rpa(gwl_ctx* ctx, const double* x, const double* y, double* ox, double* oy, int64_t nvec);
 
 /* ---- interpolative separable density fitting front end -------------------------------------------
  * PAPER.md:115-128 (Eq. 15-17): phi_n(r) phi_m(r) ~ sum_mu zeta_mu(r) C^mu_nm with C^mu_nm = phi_n(r_mu) phi_m(r_mu) at given

@@ -96,6 +96,7 @@ struct gwl_ctx {
     WorkSet& ws() { return wset[cur]; }
     cudaStream_t lstream() const { return cur ? stream2 : stream; }
     DevBuf xs, dotpart, normpart, basis, coefpart, tA, tB, pnext, pnext_part;
+    DevBuf sbasis, prpa_tc, prpa_wc, prpa_apart;  // pseudo-Hermitian RPA Lanczos (complex contexts, GWL_RPA)
     DevBuf x_nidx, x_midx, x_part, x_sig, x_eps, x_vxc, x_sc, x_e, x_z, x_it;  // gwl_exchange / gwl_qp_solve staging
     DevBuf stage;            // gwl_set_orbitals staging
     DevBuf isdf_phi, isdf_phimu, isdf_y, isdf_s, isdf_g, isdf_u;  // gwl_isdf_build
@@ -452,6 +453,123 @@ gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, doub
 
 bool ready(const gwl_ctx* ctx) { return ctx->have_orb && ctx->have_eps && ctx->have_V; }
 
+// ---- pseudo-Hermitian RPA for complex orbitals (Q24; prpa_kernels.cu) ------------------
+bool prpa(const gwl_ctx* ctx) { return ctx->cplx && ctx->approx == GWL_RPA; }
+
+gwl_status prpa_workspace(gwl_ctx* ctx, int nb) {
+    cudaStream_t st = ctx->stream;
+    gwl_status rs = ensure_workspace(ctx, 2 * nb);  // 2 nb GEMM columns: x_0, z_0, x_1, z_1, ...
+    if (rs != GWL_OK) return rs;
+    CK(ctx->prpa_tc.ensure((size_t)2 * nb * ctx->n_mup * 8, st));
+    CK(ctx->prpa_wc.ensure((size_t)2 * nb * ctx->n_mup * 8, st));
+    const int np = prpa_parts(2 * ctx->n_vc);
+    CK(ctx->prpa_apart.ensure((size_t)nb * np * 8, st));
+    CK(ctx->normpart.ensure((size_t)2 * nb * std::max(np, vec_parts(2 * ctx->n_vc)) * 8, st));
+    return GWL_OK;
+}
+
+// Coupling part of Omega^ on nb pairs whose padded copy is in xs:  out (x, z) = ( K^H W, K^H conj(W) ),  W = V ( K x + conj(K z) );
+// with h != NULL the diagonal term is added in the epilogue: out = Delta o h + coupling part (h = the unpadded vectors in xs).
+gwl_status prpa_apply(gwl_ctx* ctx, const double* h, double* out, int nb) {
+    const int64_t ldm = ctx->n_mup;
+    gwl_status rs = gemm_kx_c(ctx, 2 * nb);
+    if (rs != GWL_OK) return rs;
+    CKL(4, launch_prpa_combine(ctx->ws().T.as<double>(), ldm, nb, ctx->n_mu, ctx->prpa_tc.as<double>(), ctx->lstream()));
+    rs = plain_gemm(ctx, ctx->V.as<double>(), ldm, ctx->prpa_tc.as<double>(), ldm, ctx->n_mu, 2 * nb, ctx->n_mup / BK,
+                    ctx->prpa_wc.as<double>(), ldm, 1);
+    if (rs != GWL_OK) return rs;
+    CKL(4, launch_prpa_expand(ctx->prpa_wc.as<double>(), ldm, nb, ctx->n_mu, 1.0, ctx->ws().W.as<double>(), ctx->lstream()));
+    return gemm_ktw_c(ctx, h, ctx->n_vc, out, ctx->n_vc, 2 * nb, nullptr, 0);
+}
+
+// S1 in the RPA: u = F conj([P1; P2]) of PAPER.md:290 = ( K^H g~, -K^H conj(g~) ) in the stored variables, g~ = V (psi_m conj(psi_n))
+gwl_status prpa_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* u) {
+    const int64_t ldm = ctx->n_mup;
+    CKL(4, launch_rho_c(ctx->phi_vT.as<double>(), (int64_t)ctx->n_kv * ldm, ctx->phi_cT.as<double>(),
+                        (int64_t)ctx->n_k * ctx->n_c * ldm, ldm, ctx->nv_k, ctx->n_c, ctx->n_mu,
+                        ctx->d_nidx.as<int32_t>() + 4 * j0, ctx->prpa_tc.as<double>(), ldm, nb, ctx->lstream()));
+    gwl_status rs = plain_gemm(ctx, ctx->V.as<double>(), ldm, ctx->prpa_tc.as<double>(), ldm, ctx->n_mu, 2 * nb, ctx->n_mup / BK,
+                               ctx->prpa_wc.as<double>(), ldm, 1);
+    if (rs != GWL_OK) return rs;
+    CKL(4, launch_prpa_expand(ctx->prpa_wc.as<double>(), ldm, nb, ctx->n_mu, -1.0, ctx->ws().W.as<double>(), ctx->lstream()));
+    return gemm_ktw_c(ctx, nullptr, ctx->n_vc, u, ctx->n_vc, 2 * nb, nullptr, 0);
+}
+
+// gwl_lanczos for complex contexts in the RPA: three-term Lanczos of H = F Omega^ in the Omega^ inner product.
+gwl_status lanczos_prpa(gwl_ctx* ctx, int64_t n_chains, int L, int nbmax, int reorth) {
+    cudaStream_t st = ctx->stream;
+    const int64_t n_vc = ctx->n_vc, n4 = 2 * n_vc;
+    const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
+    const int np = prpa_parts(n4);
+    gwl_status rs = prpa_workspace(ctx, nbmax);
+    if (rs != GWL_OK) return rs;
+    CK(ctx->scale.ensure((size_t)2 * nbmax * 8, st));
+    CK(ctx->alive.ensure((size_t)2 * nbmax * 4, st));
+    const int nslots = reorth ? L + 1 : 3;
+    CK(ctx->basis.ensure((size_t)nslots * nbmax * n4 * 8, st));
+    CK(ctx->sbasis.ensure((size_t)nslots * nbmax * n4 * 8, st));
+    if (reorth) CK(ctx->coefpart.ensure((size_t)nbmax * L * 2 * np * 8, st));
+    for (int64_t j0 = 0; j0 < n_chains; j0 += nbmax) {
+        const int nb = (int)std::min<int64_t>(nbmax, n_chains - j0);
+        const int64_t slot_stride = (int64_t)nb * n4;
+        auto slot_of = [&](int k) { return (int64_t)(reorth ? k : ((k % 3) + 3) % 3) * slot_stride; };
+        double* qb = ctx->basis.as<double>();
+        double* sb = ctx->sbasis.as<double>();
+        LanczosState S;
+        S.alpha = ctx->alpha.as<double>() + j0 * L;
+        S.beta = ctx->beta.as<double>() + j0 * L;
+        S.norm2 = ctx->norm2.as<double>() + j0;
+        S.len = ctx->len.as<int32_t>() + j0;
+        S.scale = ctx->scale.as<double>();
+        S.alive = ctx->alive.as<int32_t>();
+        S.steps = L;
+        double* normpart = ctx->normpart.as<double>();
+        double* apart = ctx->prpa_apart.as<double>();
+        double* xs = ctx->xs.as<double>();
+        // ---- S1: u, Omega^ u, <u,u>_O ----
+        double* u = qb + slot_of(0);
+        double* su = sb + slot_of(0);
+        rs = prpa_start_vectors(ctx, j0, nb, u);
+        if (rs != GWL_OK) return rs;
+        CKL(4, launch_prescale(u, n_vc, xs, ldxs, ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, 2 * nb, st));
+        rs = prpa_apply(ctx, u, su, nb);
+        if (rs != GWL_OK) return rs;
+        CKL(4, launch_dot_partials(u, su, n4, n4, nb, normpart, np, st));
+        CKL(5, launch_prpa_init(u, su, n4, nb, normpart, np, S, xs, ldxs, ctx->n_c, ctx->n_cp, apart, st));
+        // ---- the step loop: one product with Omega^ per step, nothing touches the host ----
+        for (int k = 0; k < L; ++k) {
+            const double* q = qb + slot_of(k);
+            const double* s = sb + slot_of(k);
+            double* wq = qb + slot_of(k + 1);
+            double* t = sb + slot_of(k + 1);
+            const double* qp = k > 0 ? qb + slot_of(k - 1) : nullptr;
+            const double* sp = k > 0 ? sb + slot_of(k - 1) : nullptr;
+            const bool tstep = ctx->prof_level >= 1;
+            cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
+            if (tstep) {
+                e0 = ctx->next_event();
+                e1 = ctx->next_event();
+                e2 = ctx->next_event();
+                CK(cudaEventRecord(e0, st));
+            }
+            rs = prpa_apply(ctx, nullptr, t, nb);  // coupling part of Omega^ (F s_k); the diagonal term is added in update1
+            if (rs != GWL_OK) return rs;
+            if (tstep) CK(cudaEventRecord(e1, st));
+            CKL(5, launch_prpa_update1(t, wq, q, qp, s, sp, ctx->d2.as<double>(), n4, nb, apart, S, k, normpart, st));
+            if (reorth) {
+                for (int pass = 0; pass < 2; ++pass) {
+                    CKL(6, launch_prpa_reorth_dots(sb, slot_stride, k + 1, wq, n4, nb, ctx->coefpart.as<double>(), st));
+                    CKL(6, launch_prpa_reorth_apply(qb, sb, slot_stride, k + 1, wq, t, n4, nb, ctx->coefpart.as<double>(),
+                                                    pass == 1 ? normpart : nullptr, st));
+                }
+            }
+            CKL(5, launch_prpa_update2(wq, t, n4, nb, normpart, S, k, xs, ldxs, ctx->n_c, ctx->n_cp, apart, st));
+            if (tstep) CK(cudaEventRecord(e2, st));
+        }
+    }
+    return GWL_OK;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------
@@ -661,7 +779,11 @@ gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo
 gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation) {
     if (ctx == nullptr || (approximation != GWL_RPA && approximation != GWL_TDA)) return GWL_EINVAL;
     DeviceGuard dg(ctx);
-    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_approximation: real-orbital call on a complex (gwl_tdc_create) context");
+    if (ctx->cplx) {  // GWL_TDA (default): Lanczos on A(q); GWL_RPA: pseudo-Hermitian Lanczos on C^RPA(q); Delta and s are shared
+        ctx->approx = approximation;
+        invalidate_run(ctx);
+        return GWL_OK;
+    }
     if (approximation == GWL_TDA && ctx->g > 0)
         return ctx->fail(GWL_ESTATE, "gwl_set_approximation: clear the polynomial first (it approximates sqrt(C), RPA only)");
     ctx->approx = approximation;
@@ -809,6 +931,25 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
     CK(ctx->len.ensure((size_t)std::max<int64_t>(n_chains, 1) * 4, st));
     CK(cudaMemsetAsync(ctx->alpha.p, 0, ctx->alpha.bytes, st));
     CK(cudaMemsetAsync(ctx->beta.p, 0, ctx->beta.bytes, st));
+    if (prpa(ctx)) {
+        if (ctx->chain_mode != 1) return ctx->fail(GWL_ESTATE, "gwl_lanczos: the complex RPA needs gwl_tdc_set_chains");
+        if (n_chains > 0) {
+            gwl_status rs = lanczos_prpa(ctx, n_chains, L, nbmax, reorth);
+            if (rs != GWL_OK) return rs;
+        }
+        ctx->run_chains = n_chains;
+        ctx->run_steps = L;
+        ctx->run_poly = 3;
+        if (n_chains > 0) {
+            const cudaMemcpyKind kind = ctx->device_ptrs ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+            if (alpha) CK(cudaMemcpyAsync(alpha, ctx->alpha.p, (size_t)n_chains * L * 8, kind, st));
+            if (beta) CK(cudaMemcpyAsync(beta, ctx->beta.p, (size_t)n_chains * L * 8, kind, st));
+            if (norm2) CK(cudaMemcpyAsync(norm2, ctx->norm2.p, (size_t)n_chains * 8, kind, st));
+            if (len) CK(cudaMemcpyAsync(len, ctx->len.p, (size_t)n_chains * 4, kind, st));
+        }
+        if (!ctx->device_ptrs) CK(cudaStreamSynchronize(st));
+        return GWL_OK;
+    }
     if (n_chains > 0) {
         gwl_status rs = ensure_workspace(ctx, nbmax);
         if (rs != GWL_OK) return rs;
@@ -1042,7 +1183,7 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
         CK(ctx->d_sigsum.ensure((size_t)n_omega * 16, st));
         dsum = ctx->d_sigsum.as<double>();
     }
-    if (nch > 0 && ctx->run_poly == 0) {
+    if (nch > 0 && (ctx->run_poly == 0 || ctx->run_poly == 3)) {
         CK(ctx->theta.ensure((size_t)nch * L * 8, st));
         CK(ctx->wgt.ensure((size_t)nch * L * 8, st));
         CK(ctx->ritz_info.ensure((size_t)nch * 4, st));
@@ -1068,9 +1209,12 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
                                     ctx->cplx ? 2.0 / ((double)ctx->n_q * ctx->n_k) : 1.0, out, st));
         else if (ctx->run_poly == 1)
             CKL(7, launch_sigma_poly(al, be, n2, ln, L, nc, en, sg, dom, (int)n_omega, eta, out, st));
+        else if (ctx->run_poly == 3)  // complex RPA: positive Ritz branch of T, prefactor 2/(N_q N_k)
+            CKL(7, launch_sigma_direct(ctx->theta.as<double>() + (size_t)c0 * L, ctx->wgt.as<double>() + (size_t)c0 * L, n2, ln,
+                                       L, nc, en, sg, dom, (int)n_omega, eta, 1, 2.0 / ((double)ctx->n_q * ctx->n_k), out, st));
         else
             CKL(7, launch_sigma_direct(ctx->theta.as<double>() + (size_t)c0 * L, ctx->wgt.as<double>() + (size_t)c0 * L, n2, ln,
-                                       L, nc, en, sg, dom, (int)n_omega, eta, out, st));
+                                       L, nc, en, sg, dom, (int)n_omega, eta, 0, 1.0, out, st));
         if (sigma_sum != nullptr) CKL(7, launch_sigma_sum(out, nc, (int)n_omega, dsum, c0 > 0 ? 1 : 0, st));
     }
     if (sigma_sum != nullptr && nch == 0) CKL(7, launch_sigma_sum(dsig, 0, (int)n_omega, dsum, 0, st));
@@ -1424,6 +1568,52 @@ gwl_status gwl_tdc_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec
         } else {
             CKL(4, launch_interleave(ctx->io_y.as<double>(), n_kvc, nb, ctx->stage.as<double>(), st));
             CK(cudaMemcpyAsync(y + j0 * n_vc, ctx->stage.p, (size_t)nb * n_vc * 8, cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+        }
+    }
+    return GWL_OK;
+}
+
+gwl_status gwl_tdc_matvec_rpa(gwl_ctx* ctx, const double* x, const double* y, double* ox, double* oy, int64_t nvec) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_tdc_matvec_rpa: not a gwl_tdc_create context");
+    if (nvec < 0) return ctx->fail(GWL_EINVAL, "gwl_tdc_matvec_rpa: nvec < 0");
+    if (nvec == 0) return GWL_OK;
+    if (x == nullptr || y == nullptr || ox == nullptr || oy == nullptr) return ctx->fail(GWL_EINVAL, "gwl_tdc_matvec_rpa: NULL vector");
+    if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_tdc_matvec_rpa: orbitals, energies and kernel must be set");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int chunk = (int)std::min<int64_t>(nvec, 64);
+    gwl_status rs = prpa_workspace(ctx, chunk);
+    if (rs != GWL_OK) return rs;
+    const int64_t n_vc = ctx->n_vc, n_kvc = n_vc / 2, n4 = 2 * n_vc;
+    const int64_t ldxs = (int64_t)ctx->n_v * ctx->n_cp;
+    CK(ctx->io_x.ensure((size_t)chunk * n4 * 8, st));
+    CK(ctx->io_y.ensure((size_t)chunk * n4 * 8, st));
+    if (!ctx->device_ptrs) CK(ctx->stage.ensure((size_t)2 * chunk * n_vc * 8, st));
+    for (int64_t j0 = 0; j0 < nvec; j0 += chunk) {
+        const int nb = (int)std::min<int64_t>(chunk, nvec - j0);
+        const double* xin = x + j0 * n_vc;
+        const double* yin = y + j0 * n_vc;
+        double* stage = ctx->stage.as<double>();
+        if (!ctx->device_ptrs) {
+            CK(cudaMemcpyAsync(stage, xin, (size_t)nb * n_vc * 8, cudaMemcpyHostToDevice, st));
+            CK(cudaMemcpyAsync(stage + (int64_t)chunk * n_vc, yin, (size_t)nb * n_vc * 8, cudaMemcpyHostToDevice, st));
+            xin = stage;
+            yin = stage + (int64_t)chunk * n_vc;
+        }
+        CKL(4, launch_prpa_pack(xin, yin, n_kvc, nb, ctx->io_x.as<double>(), st));
+        CKL(4, launch_prescale(ctx->io_x.as<double>(), n_vc, ctx->xs.as<double>(), ldxs, ctx->s.as<double>(), ctx->n_v, ctx->n_c,
+                               ctx->n_cp, 2 * nb, st));
+        rs = prpa_apply(ctx, ctx->io_x.as<double>(), ctx->io_y.as<double>(), nb);
+        if (rs != GWL_OK) return rs;
+        if (ctx->device_ptrs) {
+            CKL(4, launch_prpa_unpack(ctx->io_y.as<double>(), n_kvc, nb, ox + j0 * n_vc, oy + j0 * n_vc, st));
+        } else {
+            CKL(4, launch_prpa_unpack(ctx->io_y.as<double>(), n_kvc, nb, stage, stage + (int64_t)chunk * n_vc, st));
+            CK(cudaMemcpyAsync(ox + j0 * n_vc, stage, (size_t)nb * n_vc * 8, cudaMemcpyDeviceToHost, st));
+            CK(cudaMemcpyAsync(oy + j0 * n_vc, stage + (int64_t)chunk * n_vc, (size_t)nb * n_vc * 8, cudaMemcpyDeviceToHost, st));
             CK(cudaStreamSynchronize(st));
         }
     }

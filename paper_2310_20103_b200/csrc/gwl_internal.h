@@ -194,6 +194,37 @@ cudaError_t launch_reorth_apply(const double* basis, int64_t slot_stride, int ns
                                 const double* coefpart, int npart, double* normpart, cudaStream_t st);
 
 // ---------------------------------------------------------------------------------------------
+// Pseudo-Hermitian RPA Lanczos for complex orbitals (prpa_kernels.cu, reading Q24).
+// A chain is the real vector [x_re | x_im | z_re | z_im] of n4 = 4 n_kvc doubles, z = conj(y) of the pair [x; y].
+// ---------------------------------------------------------------------------------------------
+int prpa_parts(int64_t n4);  // partial sums per chain of the kernels below
+// Tc[j] = T[2j] + conj(T[2j+1]); T planar [2][2 nb][ld], Tc planar [2][nb][ld]
+cudaError_t launch_prpa_combine(const double* T, int64_t ld, int nb, int n_mu, double* Tc, cudaStream_t st);
+// W[2j] = Wc[j], W[2j+1] = sign conj(Wc[j]); Wc planar [2][nb][ld], W planar [2][2 nb][ld]
+cudaError_t launch_prpa_expand(const double* Wc, int64_t ld, int nb, int n_mu, double sign, double* W, cudaStream_t st);
+// q_0 = u / sqrt(u . su), s_0 = su / sqrt(u . su) in place (normpart: partials of u . su); xs = F s_0; apart [nb][prpa_parts]
+cudaError_t launch_prpa_init(double* u, double* su, int64_t n4, int nb, const double* normpart, int npart_in, LanczosState st_,
+                             double* xs, int64_t ldxs, int n_c, int n_cp, double* apart, cudaStream_t st);
+// a_k = sum(apart); h = F s; w = h - a q - b_k q_prev -> wq; t (= K^H W part of Omega^ h on entry) <- t + d2 o h - a s - b_k s_prev;
+// normpart [nb][prpa_parts] = partials of w . t
+cudaError_t launch_prpa_update1(double* t, double* wq, const double* q, const double* q_prev, const double* s,
+                                const double* s_prev, const double* d2, int64_t n4, int nb, const double* apart, LanczosState st_,
+                                int k, double* normpart, cudaStream_t st);
+// b_{k+1}, breakdown, q_{k+1} = wq / b, s_{k+1} = sw / b in place, xs = F s_{k+1}, apart for the next a
+cudaError_t launch_prpa_update2(double* wq, double* sw, int64_t n4, int nb, const double* normpart, LanczosState st_, int k,
+                                double* xs, int64_t ldxs, int n_c, int n_cp, double* apart, cudaStream_t st);
+// complex coefficients c_j = s_j^H w, j < nslots: coefpart [nb][nslots][2][prpa_parts]
+cudaError_t launch_prpa_reorth_dots(const double* sbasis, int64_t slot_stride, int nslots, const double* w, int64_t n4, int nb,
+                                    double* coefpart, cudaStream_t st);
+// w -= sum c_j q_j, sw -= sum c_j s_j; normpart (may be NULL) = partials of w . sw
+cudaError_t launch_prpa_reorth_apply(const double* qbasis, const double* sbasis, int64_t slot_stride, int nslots, double* w,
+                                     double* sw, int64_t n4, int nb, const double* coefpart, double* normpart, cudaStream_t st);
+
+// interleaved pairs x, y [nvec][n][2] <-> stored chains [nvec][x_re | x_im | Re y | -Im y]
+cudaError_t launch_prpa_pack(const double* x, const double* y, int64_t n, int nvec, double* out, cudaStream_t st);
+cudaError_t launch_prpa_unpack(const double* in, int64_t n, int nvec, double* x, double* y, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------
 // Spectral kernels (spectral_kernels.cu): Eq. 14, Ritz pairs of T_L, Eq. 11 / Eq. 12, Eq. 10.
 // ---------------------------------------------------------------------------------------------
 cudaError_t launch_contfrac(const double* alpha, const double* beta, const double* norm2, const int32_t* len, int steps,
@@ -205,9 +236,12 @@ cudaError_t launch_ritz(const double* alpha, const double* beta, const int32_t* 
 bool ritz_dc_fits(int steps);
 cudaError_t launch_ritz_dc(const double* alpha, const double* beta, const int32_t* len, int steps, int n_chains,
                            double* theta, double* wgt, int32_t* info, cudaStream_t st);
+// linear = 0: Eq. 11 on the Ritz pairs of C (Omega_i = sqrt(theta_i)); linear = 1: pseudo-Hermitian RPA (Omega_i = theta_i,
+// Ritz values theta_i <= 0 -- the negative branch of C^RPA -- are left out); Sigma is multiplied by prefactor
 cudaError_t launch_sigma_direct(const double* theta, const double* wgt, const double* norm2, const int32_t* len,
                                 int steps, int n_chains, const double* eps_n, const int32_t* sgn_n,
-                                const double* omega, int n_omega, double eta, double* sigma, cudaStream_t st);
+                                const double* omega, int n_omega, double eta, int linear, double prefactor, double* sigma,
+                                cudaStream_t st);
 cudaError_t launch_sigma_poly(const double* alpha, const double* beta, const double* norm2, const int32_t* len,
                               int steps, int n_chains, const double* eps_n, const int32_t* sgn_n, const double* omega,
                               int n_omega, double eta, double* sigma, cudaStream_t st);

@@ -153,17 +153,23 @@ __global__ void k_ritz(const double* __restrict__ alpha, const double* __restric
 __global__ void k_sigma_direct(const double* __restrict__ theta, const double* __restrict__ wgt,
                                const double* __restrict__ norm2, const int32_t* __restrict__ len, int steps,
                                const double* __restrict__ eps_n, const int32_t* __restrict__ sgn_n,
-                               const double* __restrict__ omega, int n_omega, double eta,
-                               double* __restrict__ sigma) {
+                               const double* __restrict__ omega, int n_omega, double eta, int linear,
+                               double prefactor, double* __restrict__ sigma) {
     extern __shared__ double shm[];
     double* O = shm;
     double* wo = shm + steps;
     const int j = blockIdx.y;
     const int n = len[j];
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
-        const double o = sqrt(fmax(theta[(int64_t)j * steps + i], 1e-300));
-        O[i] = o;
-        wo[i] = wgt[(int64_t)j * steps + i] / o;
+        const double th = theta[(int64_t)j * steps + i];
+        if (linear) {  // pseudo-Hermitian RPA: the Ritz values approximate +-Omega_s; only the positive branch enters
+            O[i] = th > 0.0 ? th : 1.0;
+            wo[i] = th > 0.0 ? wgt[(int64_t)j * steps + i] / th : 0.0;
+        } else {
+            const double o = sqrt(fmax(th, 1e-300));
+            O[i] = o;
+            wo[i] = wgt[(int64_t)j * steps + i] / o;
+        }
     }
     __syncthreads();
     const int iw = blockIdx.x * blockDim.x + threadIdx.x;
@@ -177,7 +183,7 @@ __global__ void k_sigma_direct(const double* __restrict__ theta, const double* _
         sre += t.re;
         sim += t.im;
     }
-    const double f = norm2[j] * sg;
+    const double f = prefactor * norm2[j] * sg;
     sigma[((int64_t)j * n_omega + iw) * 2] = f * sre;
     sigma[((int64_t)j * n_omega + iw) * 2 + 1] = f * sim;
 }
@@ -312,7 +318,8 @@ cudaError_t launch_ritz(const double* alpha, const double* beta, const int32_t* 
 
 cudaError_t launch_sigma_direct(const double* theta, const double* wgt, const double* norm2, const int32_t* len,
                                 int steps, int n_chains, const double* eps_n, const int32_t* sgn_n,
-                                const double* omega, int n_omega, double eta, double* sigma, cudaStream_t st) {
+                                const double* omega, int n_omega, double eta, int linear, double prefactor, double* sigma,
+                                cudaStream_t st) {
     if (n_chains <= 0 || n_omega <= 0) return cudaSuccess;
     const size_t sm = (size_t)2 * steps * sizeof(double);
     static SmemAttr attr;
@@ -322,7 +329,8 @@ cudaError_t launch_sigma_direct(const double* theta, const double* wgt, const do
         const int nc = std::min(MAX_GRID_Y, n_chains - j0);
         dim3 grid((unsigned)ceil_div(n_omega, 128), (unsigned)nc);
         k_sigma_direct<<<grid, 128, sm, st>>>(theta + (int64_t)j0 * steps, wgt + (int64_t)j0 * steps, norm2 + j0, len + j0, steps,
-                                              eps_n + j0, sgn_n + j0, omega, n_omega, eta, sigma + (int64_t)j0 * n_omega * 2);
+                                              eps_n + j0, sgn_n + j0, omega, n_omega, eta, linear, prefactor,
+                                              sigma + (int64_t)j0 * n_omega * 2);
         count_launch();
     }
     return cudaGetLastError();

@@ -48,6 +48,7 @@ SIGNATURES = {
     "gwl_tdc_set_energies": (c_int, [c_void_p, c_void_p, c_void_p]),
     "gwl_tdc_set_chains": (c_int, [c_void_p, c_int64, c_void_p]),
     "gwl_tdc_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
+    "gwl_tdc_matvec_rpa": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int64]),
     "gwl_isdf_build": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_double, c_double, c_void_p, c_void_p,
                                c_void_p]),
     "gwl_isdf_select_points": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_int64, c_void_p, POINTER(c_int32)]),
@@ -416,6 +417,21 @@ class TdcContext(Context):
         yh = np.empty_like(xh)
         self._ck(self._lib.gwl_tdc_matvec(self._h, _ptr(xh), _ptr(yh), xh.size // self.n_kvc))
         return yh
+
+    def matvec_rpa(self, x, y, ox=None, oy=None):
+        """[ox; oy] = Omega^ [x; y] = [A x + B y; B^* x + A^* y].  Host mode: complex numpy arrays
+        [nvec, n_kvc]; device mode: torch CUDA complex128 tensors (ox, oy given)."""
+        if self.device_ptrs:
+            nvec = x.numel() // self.n_kvc
+            self._ck(self._lib.gwl_tdc_matvec_rpa(self._h, _ptr(x), _ptr(y), _ptr(ox), _ptr(oy), nvec))
+            return ox, oy
+        xh = np.ascontiguousarray(x, dtype=np.complex128)
+        yh = np.ascontiguousarray(y, dtype=np.complex128)
+        if xh.size % self.n_kvc or xh.shape != yh.shape:
+            raise GwlError(GWL_EINVAL, "matvec_rpa: x and y must both be [nvec, n_k, n_v, n_c]")
+        oxh, oyh = np.empty_like(xh), np.empty_like(yh)
+        self._ck(self._lib.gwl_tdc_matvec_rpa(self._h, _ptr(xh), _ptr(yh), _ptr(oxh), _ptr(oyh), xh.size // self.n_kvc))
+        return oxh, oyh
 
 
 def context_from_problem(prob) -> Context:
