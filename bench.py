@@ -52,6 +52,9 @@ def parse():
                     help="context run, not the bench line: the complex-orbital Tamm-Dancoff variant (SURVEY 8(f)-3) on a "
                          "synthetic periodic problem of that shape, e.g. 4,64,1024,6144; block = --chains (default 128), "
                          "L = --lanczos-steps (default 10)")
+    ap.add_argument("--rpa", action="store_true",
+                    help="with --tdc: the full RPA for complex orbitals (pseudo-Hermitian Lanczos on C^RPA(q), PAPER.md:159): every "
+                         "chain is a pair [x; y] = two GEMM columns, one product with Omega^ per step")
     ap.add_argument("--sharded-state", action="store_true",
                     help="SURVEY 8(f)-2 arm, its own line: the N_v+N_c chains of ONE state partitioned over the ranks "
                          "(runtime.shard_range), one NCCL all-reduce of the omega grid; strong scaling")
@@ -264,12 +267,15 @@ def run_tdc(args):
     ctx.set_orbitals(p.psi_v, p.psi_cq)
     ctx.set_energies(p.eps_v, p.eps_cq)
     ctx.set_kernel(p.V)
+    if args.rpa:
+        ctx.set_approximation(gwl.GWL_RPA)
     ctx.set_chains(p.chains)
     ctx.set_pointer_mode(1)
     ctx.set_profiling(0)
     om = torch.from_numpy(p.omega).to(dev)
     ssum = torch.empty(len(p.omega), 2, dtype=torch.float64, device=dev)
     peak = gwl.probe_fp64_peak(0)
+    cols = 2 * nch if args.rpa else nch      # GEMM columns per block: a pair [x; y] is two columns
 
     def step():
         ctx.lanczos(nch, L, nch, 0, out=None)
@@ -290,17 +296,19 @@ def run_tdc(args):
     kt = ctx.get_kernel_times()
     ctx.set_profiling(0)
     n_kvc = n_k * n_v * n_c
-    fl = 8.0 * n_mu * n_kvc * nch
+    fl = 8.0 * n_mu * n_kvc * cols
     per = {k: v[0] / v[1] for k, v in kt.items() if v[1]}
     line = {"metric": METRIC, "value": nch * L / sec, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * sec, "higher_is_better": True, "dtype": "complex f64 (planar)", "data": "synthetic",
-            "arm": "tdc (SURVEY 8(f)-3): context run, not the headline bench line",
-            "config": {"workload": "periodic Tamm-Dancoff: Lanczos on the Hermitian A(q), one block of chains", "n_k": n_k,
+            "arm": ("complex RPA" if args.rpa else "tdc") + " (SURVEY 8(f)-3): context run, not the headline bench line",
+            "config": {"workload": ("periodic RPA: pseudo-Hermitian Lanczos on C^RPA(q) in the Omega^ inner product, one block of "
+                                    "chain pairs (2 GEMM columns per chain)" if args.rpa else
+                                    "periodic Tamm-Dancoff: Lanczos on the Hermitian A(q), one block of chains"), "n_k": n_k,
                        "n_v": n_v, "n_c": n_c, "n_mu": n_mu, "n_kvc": n_kvc, "chains": nch, "lanczos_steps": L},
             "roofline": {"bound": "tensor", "peak": peak, "unit": "TFLOP/s",
                          "Kx": {"achieved": fl / (per["gemm_fwd_KX"] * 1e-3) / 1e12, "ms_per_launch": per["gemm_fwd_KX"]},
                          "KhW": {"achieved": fl / (per["gemm_bwd_KtW"] * 1e-3) / 1e12, "ms_per_launch": per["gemm_bwd_KtW"]},
-                         "flop_per_launch": fl, "flop_model": "8 N_mu N_kvc B real flop (4 real multiply-adds per complex one)"},
+                         "flop_per_launch": fl, "flop_model": "8 N_mu N_kvc B real flop (4 real multiply-adds per complex one), B = GEMM columns"},
             "kernel_time_share": {k: round(v[0] / sum(x[0] for x in kt.values()), 4) for k, v in kt.items() if v[1]}}
     line["roofline"]["Kx"]["frac"] = line["roofline"]["Kx"]["achieved"] / peak
     line["roofline"]["KhW"]["frac"] = line["roofline"]["KhW"]["achieved"] / peak
