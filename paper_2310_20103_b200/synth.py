@@ -229,3 +229,80 @@ def stride_points(n_r: int, n_mu: int, seed: int = 0) -> np.ndarray:
     or k-means in the ISDF literature, is not part of the parity tests)."""
     rng = np.random.default_rng(seed)
     return np.sort(rng.choice(n_r, size=n_mu, replace=False)).astype(np.int32)
+
+
+# ---------------------------------------------------------------------------------------------
+# SURVEY.md §8(f)-4, second part: inputs with an abelian point group for the symmetry blocks of C (PAPER.md:128).
+# The group is generated by n_refl mirror planes (x -> -x, y -> -y, z -> -z: C_s, C_2v-like, D_2h-like; order g = 2^n_refl);
+# element h in [0, g) reflects the axes whose bit is set in h.  Only the data are made here: fitting points in the
+# irreducible wedge and all their images, orbital values on the wedge, an irreducible-representation label per orbital
+# (a bit mask: bit i set = odd under mirror i).  What the labels MEAN (characters, unfolding, block structure) is the
+# method's arithmetic and lives in oracle/symmetry.py and in the library separately.
+# ---------------------------------------------------------------------------------------------
+@dataclass
+class SymmetricProblem:
+    n_refl: int
+    nv_irrep: np.ndarray   # [g] occupied orbitals per irrep (orbitals are sorted by irrep)
+    nc_irrep: np.ndarray   # [g] empty orbitals per irrep
+    r_w: np.ndarray        # [n_w, 3] fitting points of the wedge
+    r_full: np.ndarray     # [g * n_w, 3]: r_full[h * n_w + mu] = image of r_w[mu] under element h
+    phi_v_w: np.ndarray    # [n_w, N_v] orbital values on the wedge
+    phi_c_w: np.ndarray    # [n_w, N_c]
+    irrep_v: np.ndarray    # [N_v] int32 labels, ascending
+    irrep_c: np.ndarray    # [N_c]
+    eps_v: np.ndarray      # [N_v]
+    eps_c: np.ndarray      # [N_c]
+    omega: np.ndarray
+    eta: float = 0.1
+    _V: np.ndarray | None = field(default=None, repr=False)
+
+    @property
+    def g(self) -> int:
+        return 1 << self.n_refl
+
+    @property
+    def n_w(self) -> int:
+        return self.r_w.shape[0]
+
+    @property
+    def V_full(self) -> np.ndarray:
+        """Coulomb kernel of ALL points (invariant under the group because reflections are isometries)."""
+        if self._V is None:
+            self._V = coulomb_kernel(self.r_full)
+        return self._V
+
+    @property
+    def V_wf(self) -> np.ndarray:
+        """[n_w][g][n_w]: rows of V_full for the wedge points against every image, V(r_mu, h r_nu) (a slice, no arithmetic)."""
+        return np.ascontiguousarray(self.V_full[:self.n_w].reshape(self.n_w, self.g, self.n_w))
+
+
+def make_symmetric(n_refl: int, nv_irrep, nc_irrep, n_w: int, box: float = 12.0, seed: int = 0,
+                   n_omega: int = 101) -> SymmetricProblem:
+    """Draw order r_w, Phi_v, Phi_c, eps_v, eps_c.  Wedge points: coordinates along mirrored axes uniform in
+    [0.3, box/2] (off the mirror planes, so the g images are distinct), the others uniform in [-box/2, box/2]."""
+    g = 1 << n_refl
+    nv_irrep = np.asarray(nv_irrep, dtype=np.int32)
+    nc_irrep = np.asarray(nc_irrep, dtype=np.int32)
+    if nv_irrep.shape != (g,) or nc_irrep.shape != (g,):
+        raise ValueError("nv_irrep and nc_irrep need one entry per irrep (2^n_refl)")
+    rng = np.random.default_rng(seed)
+    r_w = np.empty((n_w, 3))
+    for ax in range(3):
+        if ax < n_refl:
+            r_w[:, ax] = rng.uniform(0.3, 0.5 * box, n_w)
+        else:
+            r_w[:, ax] = rng.uniform(-0.5 * box, 0.5 * box, n_w)
+    r_full = np.empty((g * n_w, 3))
+    for h in range(g):
+        sign = np.array([-1.0 if (h >> ax) & 1 else 1.0 for ax in range(3)])
+        r_full[h * n_w:(h + 1) * n_w] = r_w * sign[None, :]
+    n_v, n_c = int(nv_irrep.sum()), int(nc_irrep.sum())
+    phi_v_w = rng.standard_normal((n_w, n_v)) / np.sqrt(g * n_w)
+    phi_c_w = rng.standard_normal((n_w, n_c)) / np.sqrt(g * n_w)
+    eps_v = rng.uniform(-10.0, -5.0, n_v)
+    eps_c = rng.uniform(-3.0, 20.0, n_c)
+    irrep_v = np.repeat(np.arange(g, dtype=np.int32), nv_irrep)
+    irrep_c = np.repeat(np.arange(g, dtype=np.int32), nc_irrep)
+    omega = np.linspace(-20.0, 20.0, n_omega)
+    return SymmetricProblem(n_refl, nv_irrep, nc_irrep, r_w, r_full, phi_v_w, phi_c_w, irrep_v, irrep_c, eps_v, eps_c, omega)
