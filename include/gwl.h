@@ -231,6 +231,39 @@ gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, c
 gwl_status gwl_isdf_select_points(gwl_ctx* ctx, int64_t n_r, const double* r, const double* weight, const int32_t* init_idx,
                                   int64_t max_iters, int32_t* idx, int32_t* iters_done);
 
+/* ---- SURVEY.md 8(f)-4, second part: point-group symmetry blocks of the Casida matrix ---------------------------------------
+ * "One can further exploit the point-group symmetries to make the Casida matrix C block diagonal and simplify the calculation
+ * of matrix-vector products [64]".  Reading (Q25): an abelian group of order g = 2^n_gen (n_gen <= 3
+ * commuting generators, e.g. mirror planes: C_s, C_2v, D_2h, ...) with one-dimensional real irreducible representations.  An
+ * irrep is a bit mask in [0, g), its character at the element h is (-1)^popcount(irrep & h), the product of two irreps is their
+ * XOR.  Orbitals are sorted by irrep (nv_irrep[a] occupied, nc_irrep[a] empty orbitals of irrep a).  The pair (v, c) belongs to
+ * block gamma = irrep(v) ^ irrep(c); C does not couple different blocks and |P_nm> lies in block irrep(n) ^ irrep(m).  With
+ * fitting points closed under the group (n_mu_w points r_mu of the irreducible wedge and their images h r_mu), within block gamma
+ *   K^T V K = Kw^T Vg Kw,  Kw = K on the wedge,  Vg[mu][nu] = g sum_h chi_gamma(h) V(r_mu, h r_nu),
+ * so one chain-step costs 4 n_mu_w N_pairs(gamma) + 2 n_mu_w^2 flop: about g^2 fewer than without the symmetry.
+ * A context made by gwl_sym_create takes gwl_sym_set_orbitals / gwl_set_energies / gwl_sym_set_kernel once, then
+ * gwl_sym_select(gamma) makes block gamma the operator: gwl_sym_matvec, gwl_set_chains (pairs (n, m) of that block only, else
+ * GWL_EINVAL), gwl_lanczos, gwl_resolvent, gwl_selfenergy, gwl_set_polynomial and the gwl_get_* calls then work as on a plain
+ * context; gwl_sym_selfenergy_state walks all blocks for one orbital m.  Block vectors hold the pairs of block gamma ordered by
+ * the irrep a of v (ascending), then v, then c over the irrep a ^ gamma.  The other real-orbital calls return GWL_ESTATE. */
+gwl_status gwl_sym_create(gwl_ctx** out, int n_gen, const int32_t* nv_irrep /*[2^n_gen]*/, const int32_t* nc_irrep /*[2^n_gen]*/,
+                          int64_t n_mu_w);
+/* Orbital values at the wedge points: phi_v_w [n_mu_w][N_v], phi_c_w [n_mu_w][N_c] (N_v = sum nv_irrep, N_c = sum nc_irrep), host. */
+gwl_status gwl_sym_set_orbitals(gwl_ctx* ctx, const double* phi_v_w, const double* phi_c_w);
+/* Rows of (alpha|beta) for the wedge points against every image: V_wf [n_mu_w][g][n_mu_w] = V(r_mu, h r_nu), host; element h is
+ * the bit mask of the generators applied.  The g reduced kernels Vg are formed on the device. */
+gwl_status gwl_sym_set_kernel(gwl_ctx* ctx, const double* V_wf);
+/* Makes block gamma the operator (needs the energies); *n_pairs (may be NULL) receives its dimension.  GWL_EINVAL if the block
+ * has no pairs.  Invalidates chains and results. */
+gwl_status gwl_sym_select(gwl_ctx* ctx, int gamma, int64_t* n_pairs);
+/* y = C_gamma x for nvec vectors of the selected block, x, y [nvec][n_pairs] (pointer mode applies); must not overlap. */
+gwl_status gwl_sym_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec);
+/* Sigma^corr_mm(omega) = sum over ALL n (Eq. 10) for one orbital m, block by block: for every gamma the chains
+ * n with irrep(n) ^ irrep(m) = gamma run inside block gamma and Eq. 10 is accumulated on the device.  Arguments as
+ * gwl_selfenergy_state; leaves the last non-empty block selected. */
+gwl_status gwl_sym_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, int64_t block, int reorth, const double* omega,
+                                    int64_t n_omega, double eta, double* sigma_mm);
+
 /* CUDA-event totals (ms) of the last gwl_lanczos: time inside Casida products (S2), inside the Lanczos
  * vector kernels (S4) and overall.  Any pointer may be NULL.  Synchronises the stream. */
 gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total);

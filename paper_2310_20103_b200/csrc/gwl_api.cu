@@ -59,6 +59,16 @@ struct gwl_ctx {
     // vector layout has n_v = 2 * n_kv "rows" of n_c and n_vc = 2 * n_k * nv_k * n_c real entries
     bool cplx = false;
     int n_k = 1, nv_k = 0, n_kv = 0, n_q = 1;
+    // symmetry-block contexts (gwl_sym_create, Q25): irreps are bit masks, products are XORs.  After
+    // gwl_sym_select(gamma) the vector kernels see one padded block vector (n_c = n_cp = 16, n_v = n_vc / 16) and the GEMM
+    // drivers walk the rectangles (v in irrep a) x (c in irrep a ^ gamma), every irrep's conduction count padded to 16 columns
+    bool sym = false;
+    int sym_g = 1, sym_gamma = -1;
+    int sym_nv[8] = {}, sym_nc[8] = {}, sym_ncp[8] = {}, sym_voff[8] = {}, sym_coff[8] = {}, sym_cpoff[8] = {};
+    int sym_nv_tot = 0, sym_nc_tot = 0, sym_ncp_tot = 0;
+    int64_t sym_vecoff[8] = {}, sym_apioff[8] = {}, sym_npairs = 0;
+    int64_t v_sel = 0;          // element offset of the selected kernel inside V (V holds the g reduced kernels)
+    bool sig_accumulate = false;  // gwl_selfenergy adds to sigma_sum instead of overwriting it (gwl_sym_selfenergy_state)
     cudaStream_t stream = nullptr;
     int device_ptrs = 0;
     std::string err;
@@ -250,8 +260,10 @@ gwl_status gemm_kx_c(gwl_ctx* ctx, int nb) {
     return GWL_OK;
 }
 
+gwl_status gemm_kx_sym(gwl_ctx* ctx, int nb);
 gwl_status gemm_kx(gwl_ctx* ctx, int nb) {
     if (ctx->cplx) return gemm_kx_c(ctx, nb);
+    if (ctx->sym) return gemm_kx_sym(ctx, nb);
     cudaStream_t st = ctx->lstream();
     const int kt_c = ctx->n_cp / BK, kt_f = ctx->n_v * kt_c;
     const int64_t ldm = ctx->n_mup;
@@ -309,8 +321,8 @@ gwl_status plain_gemm(gwl_ctx* ctx, const double* A, int64_t lda, const double* 
 // W[b][mu] = sum_nu V[mu][nu] T[b][nu]
 gwl_status gemm_v(gwl_ctx* ctx, int nb) {
     if (ctx->cplx) nb *= 2;  // V is real: the two planes of T are 2 nb independent columns
-    return plain_gemm(ctx, ctx->V.as<double>(), ctx->n_mup, ctx->ws().T.as<double>(), ctx->n_mup, ctx->n_mu, nb, ctx->n_mup / BK,
-                      ctx->ws().W.as<double>(), ctx->n_mup, 1);
+    return plain_gemm(ctx, ctx->V.as<double>() + ctx->v_sel, ctx->n_mup, ctx->ws().T.as<double>(), ctx->n_mup, ctx->n_mu, nb,
+                      ctx->n_mup / BK, ctx->ws().W.as<double>(), ctx->n_mup, 1);
 }
 
 // u = K^T W with the epilogue fused:  x != NULL: y = d2 o x + coupling s o u and the partial dots sum(x y);
@@ -361,37 +373,66 @@ gwl_status gemm_ktw_c(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int
     return GWL_OK;
 }
 
+// One rectangle of the K^T.W product: conduction rows [c_row0, c_row0 + n_c_rows) of Phi_c^T, occupied orbitals
+// [v0, v0 + n_v_rows), output / x / Delta / Chebyshev vectors shifted by vec_off inside every chain.  The whole product of an
+// ordinary context is the rectangle (0, N_c, 0, N_v, 0); a symmetry block is one rectangle per irrep of v.
+struct KtwRect {
+    int c_row0, n_c_rows, v0, n_v_rows;
+    int64_t vec_off;
+};
+
+gwl_status gemm_ktw_rect(gwl_ctx* ctx, const KtwRect& r, const double* x, int64_t ldx, double* y, int64_t ldy, int nb,
+                         double* dotpart, int dot_stride, const ChebTerm* cheb);
+
 gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64_t ldy, int nb, double* dotpart,
                     int dot_stride, const ChebTerm* cheb = nullptr) {
     if (ctx->cplx) {
         if (cheb != nullptr) return ctx->fail(GWL_EINVAL, "internal: no polynomial mode for complex orbitals");
         return gemm_ktw_c(ctx, x, ldx, y, ldy, nb, dotpart, dot_stride);
     }
+    if (ctx->sym) {  // block gamma: rectangles (v in irrep a) x (c in irrep a ^ gamma), dot partials one after the other
+        int dbase = 0;
+        for (int a = 0; a < ctx->sym_g; ++a) {
+            const int b = a ^ ctx->sym_gamma;
+            if (ctx->sym_nv[a] == 0 || ctx->sym_nc[b] == 0) continue;
+            const KtwRect r{ctx->sym_cpoff[b], ctx->sym_ncp[b], ctx->sym_voff[a], ctx->sym_nv[a], ctx->sym_vecoff[a]};
+            gwl_status rs = gemm_ktw_rect(ctx, r, x, ldx, y, ldy, nb, dotpart != nullptr ? dotpart + dbase : nullptr, dot_stride, cheb);
+            if (rs != GWL_OK) return rs;
+            dbase += ctx->sym_nv[a] * (int)ceil_div(ctx->sym_ncp[b], 128);
+        }
+        return GWL_OK;
+    }
+    const KtwRect r{0, ctx->n_c, 0, ctx->n_v, 0};
+    return gemm_ktw_rect(ctx, r, x, ldx, y, ldy, nb, dotpart, dot_stride, cheb);
+}
+
+gwl_status gemm_ktw_rect(gwl_ctx* ctx, const KtwRect& r, const double* x, int64_t ldx, double* y, int64_t ldy, int nb,
+                         double* dotpart, int dot_stride, const ChebTerm* cheb) {
     const int kt_v = ctx->n_mup / BK;
     const int64_t ldm = ctx->n_mup;
-    const GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, kt_v, kt_v, ctx->n_sm);
+    const GemmPlan pl = plan_gemm(MODE_BWD, r.n_c_rows, nb, kt_v, kt_v, ctx->n_sm);
     GemmParams p{};
-    p.A = ctx->phi_cT.as<double>();
+    p.A = ctx->phi_cT.as<double>() + (int64_t)r.c_row0 * ldm;
     p.lda = ldm;
     p.B = ctx->ws().W.as<double>();
     p.ldb = ldm;
-    p.M = ctx->n_c;
+    p.M = r.n_c_rows;
     p.N = nb;
     p.kt_total = kt_v;
     p.a_wrap = kt_v;
     p.kt_per_split = kt_v;
-    p.scale = ctx->phi_vT.as<double>();
+    p.scale = ctx->phi_vT.as<double>() + (int64_t)r.v0 * ldm;
     p.lds = ldm;
-    p.scale_rows = ctx->n_v;
-    p.out = y;
+    p.scale_rows = r.n_v_rows;
+    p.out = y + r.vec_off;
     p.ldo = ldy;
-    p.X = x;
+    p.X = x != nullptr ? x + r.vec_off : nullptr;
     p.ldx = ldx;
-    p.d2 = ctx->d2.as<double>();
-    p.s = ctx->s.as<double>();
+    p.d2 = ctx->d2.as<double>() + r.vec_off;
+    p.s = ctx->s.as<double>() + r.vec_off;
     p.dotpart = dotpart;
     p.dot_stride = dot_stride;
-    p.n_c = ctx->n_c;
+    p.n_c = r.n_c_rows;
     p.coupling = ctx->approx ? 1.0 : 2.0;
     p.ws = ctx->ws().sk_ws.as<double>();
     p.flags = ctx->ws().sk_flags.as<unsigned>();
@@ -402,12 +443,12 @@ gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64
     if (cheb != nullptr) {
         if (x == nullptr || ldx != ldy) return ctx->fail(GWL_EINVAL, "internal: EPI_CHEB needs x and a common leading dimension");
         epi = EPI_CHEB;
-        p.T0 = cheb->t0;
-        p.Wacc = cheb->w;
-        p.Q = cheb->q;
-        p.xs_out = cheb->xs_out;
+        p.T0 = cheb->t0 != nullptr ? cheb->t0 + r.vec_off : nullptr;
+        p.Wacc = cheb->w + r.vec_off;
+        p.Q = cheb->q != nullptr ? cheb->q + r.vec_off : nullptr;
+        p.xs_out = cheb->xs_out != nullptr ? cheb->xs_out + r.vec_off : nullptr;  // sym: padded layout = vector layout
         p.ldxs = (int64_t)ctx->n_v * ctx->n_cp;
-        p.n_cp = ctx->n_cp;
+        p.n_cp = ctx->sym ? r.n_c_rows : ctx->n_cp;
         p.ca = cheb->ca;
         p.cb = cheb->cb;
         p.cc = cheb->cc;
@@ -415,7 +456,49 @@ gwl_status gemm_ktw(gwl_ctx* ctx, const double* x, int64_t ldx, double* y, int64
         p.c0 = cheb->c0;
         p.first = cheb->first;
     }
-    CKL(2, launch_gemm(MODE_BWD, epi, pl, p, ctx->n_v, ctx->lstream()));
+    CKL(2, launch_gemm(MODE_BWD, epi, pl, p, r.n_v_rows, ctx->lstream()));
+    return GWL_OK;
+}
+
+// K.X of a symmetry block: one launch per rectangle, all partials (rectangles x their split-K) reduced together
+gwl_status gemm_kx_sym(gwl_ctx* ctx, int nb) {
+    cudaStream_t st = ctx->lstream();
+    const int64_t ldm = ctx->n_mup;
+    GemmPlan plans[8];
+    int total = 0;
+    for (int a = 0; a < ctx->sym_g; ++a) {
+        const int b = a ^ ctx->sym_gamma;
+        if (ctx->sym_nv[a] == 0 || ctx->sym_nc[b] == 0) continue;
+        const int kt_c = ctx->sym_ncp[b] / BK;
+        plans[a] = plan_gemm(MODE_FWD, ctx->n_mu, nb, ctx->sym_nv[a] * kt_c, kt_c, ctx->n_sm);
+        total += plans[a].splits;
+    }
+    CK(ctx->ws().part.ensure((size_t)std::max(total, 1) * nb * ldm * 8, st));
+    int zbase = 0;
+    for (int a = 0; a < ctx->sym_g; ++a) {
+        const int b = a ^ ctx->sym_gamma;
+        if (ctx->sym_nv[a] == 0 || ctx->sym_nc[b] == 0) continue;
+        const int kt_c = ctx->sym_ncp[b] / BK;
+        GemmParams p{};
+        p.A = ctx->phi_c.as<double>() + ctx->sym_cpoff[b];
+        p.lda = ctx->sym_ncp_tot;
+        p.B = ctx->xs.as<double>() + ctx->sym_vecoff[a];
+        p.ldb = ctx->n_vc;
+        p.M = ctx->n_mu;
+        p.N = nb;
+        p.kt_total = ctx->sym_nv[a] * kt_c;
+        p.a_wrap = kt_c;
+        p.kt_per_split = plans[a].kt_per_split;
+        p.scale = ctx->phi_vT.as<double>() + (int64_t)ctx->sym_voff[a] * ldm;
+        p.lds = ldm;
+        p.scale_rows = ctx->sym_nv[a];
+        p.out = ctx->ws().part.as<double>() + (int64_t)zbase * nb * ldm;
+        p.ldo = ldm;
+        p.out_split_stride = (int64_t)nb * ldm;
+        CKL(0, launch_gemm(MODE_FWD, EPI_STORE, plans[a], p, plans[a].splits, st));
+        zbase += plans[a].splits;
+    }
+    CKL(3, launch_splitk_reduce(ctx->ws().part.as<double>(), (int64_t)nb * ldm, zbase, ctx->ws().T.as<double>(), ldm, ctx->n_mu, nb, st));
     return GWL_OK;
 }
 
@@ -431,6 +514,13 @@ gwl_status apply_casida_core(gwl_ctx* ctx, const double* x, int64_t ldx, double*
 // alpha / norm partials written by the K^T.W epilogue: one per (v, m-tile) of the plan used for a block of nb
 int casida_ndot(const gwl_ctx* ctx, int nb) {
     if (ctx->cplx) return ctx->n_kv * gemm_c_tiles_m(ctx->n_c);
+    if (ctx->sym) {
+        int n = 0;
+        for (int a = 0; a < ctx->sym_g; ++a)
+            if (ctx->sym_nv[a] > 0 && ctx->sym_nc[a ^ ctx->sym_gamma] > 0)
+                n += ctx->sym_nv[a] * (int)ceil_div(ctx->sym_ncp[a ^ ctx->sym_gamma], 128);
+        return std::max(n, 1);
+    }
     const GemmPlan pl = plan_gemm(MODE_BWD, ctx->n_c, nb, ctx->n_mup / BK, ctx->n_mup / BK, ctx->n_sm);
     return ctx->n_v * (int)ceil_div(ctx->n_c, pl.bm);
 }
@@ -443,7 +533,7 @@ gwl_status build_start_vectors(gwl_ctx* ctx, int64_t j0, int nb, double* P, doub
                             (int64_t)ctx->n_k * ctx->n_c * ldm, ldm, ctx->nv_k, ctx->n_c, ctx->n_mu,
                             ctx->d_nidx.as<int32_t>() + 4 * j0, ctx->ws().T.as<double>(), ldm, nb, ctx->lstream()));
     else
-        CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
+        CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->sym ? ctx->sym_nv_tot : ctx->n_v, ctx->n_mu,
                       ctx->d_nidx.as<int32_t>() + j0, ctx->d_midx.as<int32_t>() + j0, ctx->ws().T.as<double>(), ldm, nb,
                       ctx->lstream()));
     gwl_status rs = gemm_v(ctx, nb);
@@ -683,6 +773,7 @@ gwl_status gwl_set_orbitals(gwl_ctx* ctx, const double* phi_v, const double* phi
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_orbitals: real-orbital call on a complex (gwl_tdc_create) context");
+    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_set_orbitals: symmetry-block (gwl_sym_create) context: use gwl_sym_set_orbitals");
     if (phi_v == nullptr || phi_c == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_orbitals: NULL input");
     LaunchScope ls(ctx);
     cudaStream_t st = ctx->stream;
@@ -706,22 +797,34 @@ gwl_status gwl_set_energies(gwl_ctx* ctx, const double* eps_v, const double* eps
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_energies: real-orbital call on a complex (gwl_tdc_create) context");
     if (eps_v == nullptr || eps_c == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_energies: NULL input");
+    const int nv_orb = ctx->sym ? ctx->sym_nv_tot : ctx->n_v, nc_orb = ctx->sym ? ctx->sym_nc_tot : ctx->n_c;
     double vmax = -INFINITY, cmin = INFINITY;
-    for (int i = 0; i < ctx->n_v; ++i) {
+    for (int i = 0; i < nv_orb; ++i) {
         if (!std::isfinite(eps_v[i])) return ctx->fail(GWL_EINVAL, "gwl_set_energies: non-finite eps_v");
         vmax = std::max(vmax, eps_v[i]);
     }
-    for (int i = 0; i < ctx->n_c; ++i) {
+    for (int i = 0; i < nc_orb; ++i) {
         if (!std::isfinite(eps_c[i])) return ctx->fail(GWL_EINVAL, "gwl_set_energies: non-finite eps_c");
         cmin = std::min(cmin, eps_c[i]);
     }
     if (!(cmin > vmax)) return ctx->fail(GWL_EINVAL, "gwl_set_energies: need min(eps_c) > max(eps_v)");
     LaunchScope ls(ctx);
     cudaStream_t st = ctx->stream;
-    ctx->h_eps_v.assign(eps_v, eps_v + ctx->n_v);
-    ctx->h_eps_c.assign(eps_c, eps_c + ctx->n_c);
-    CK(ctx->eps_v.ensure((size_t)ctx->n_v * 8, st));
-    CK(ctx->eps_c.ensure((size_t)ctx->n_c * 8, st));
+    ctx->h_eps_v.assign(eps_v, eps_v + nv_orb);
+    ctx->h_eps_c.assign(eps_c, eps_c + nc_orb);
+    CK(ctx->eps_v.ensure((size_t)nv_orb * 8, st));
+    CK(ctx->eps_c.ensure((size_t)nc_orb * 8, st));
+    if (ctx->sym) {  // the diagonal term of a block is built by gwl_sym_select
+        CK(cudaMemcpyAsync(ctx->eps_v.p, eps_v, (size_t)nv_orb * 8, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(ctx->eps_c.p, eps_c, (size_t)nc_orb * 8, cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+        ctx->have_eps = true;
+        ctx->sym_gamma = -1;
+        invalidate_run(ctx);
+        ctx->chain_mode = 0;
+        ctx->n_chains_set = 0;
+        return GWL_OK;
+    }
     CK(ctx->d2.ensure((size_t)ctx->n_vc * 8, st));
     CK(ctx->s.ensure((size_t)ctx->n_vc * 8, st));
     CK(cudaMemcpyAsync(ctx->eps_v.p, eps_v, (size_t)ctx->n_v * 8, cudaMemcpyHostToDevice, st));
@@ -742,6 +845,7 @@ gwl_status gwl_set_kernel(gwl_ctx* ctx, const double* V) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (V == nullptr) return ctx->fail(GWL_EINVAL, "gwl_set_kernel: NULL input");
+    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_set_kernel: symmetry-block (gwl_sym_create) context: use gwl_sym_set_kernel");
     cudaStream_t st = ctx->stream;
     CK(ctx->V.ensure((size_t)ctx->n_mu * ctx->n_mup * 8, st));
     CK(cudaMemsetAsync(ctx->V.p, 0, ctx->V.bytes, st));
@@ -784,6 +888,7 @@ gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation) {
         invalidate_run(ctx);
         return GWL_OK;
     }
+    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_set_approximation: symmetry-block (gwl_sym_create) contexts run the RPA operator C only");
     if (approximation == GWL_TDA && ctx->g > 0)
         return ctx->fail(GWL_ESTATE, "gwl_set_approximation: clear the polynomial first (it approximates sqrt(C), RPA only)");
     ctx->approx = approximation;
@@ -802,6 +907,7 @@ gwl_status gwl_casida_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t n
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_casida_matvec: real-orbital call on a complex (gwl_tdc_create) context");
+    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_casida_matvec: symmetry-block (gwl_sym_create) context: use gwl_sym_matvec");
     if (nvec < 0) return ctx->fail(GWL_EINVAL, "gwl_casida_matvec: nvec < 0");
     if (nvec == 0) return GWL_OK;
     if (x == nullptr || y == nullptr) return ctx->fail(GWL_EINVAL, "gwl_casida_matvec: NULL vector");
@@ -847,15 +953,39 @@ gwl_status gwl_set_chains(gwl_ctx* ctx, int64_t n_chains, const int32_t* n_idx, 
     if (n_chains < 0 || (n_chains > 0 && (n_idx == nullptr || m_idx == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_set_chains: bad arguments");
     if (!ctx->have_eps) return ctx->fail(GWL_ESTATE, "gwl_set_chains: energies must be set first");
-    const int n_orb = ctx->n_v + ctx->n_c;
+    if (ctx->sym && ctx->sym_gamma < 0) return ctx->fail(GWL_ESTATE, "gwl_set_chains: select a symmetry block first (gwl_sym_select)");
+    const int nv_orb = ctx->sym ? ctx->sym_nv_tot : ctx->n_v;
+    const int n_orb = nv_orb + (ctx->sym ? ctx->sym_nc_tot : ctx->n_c);
     std::vector<double> eps(n_chains);
-    std::vector<int32_t> sgn(n_chains);
+    std::vector<int32_t> sgn(n_chains), n_pos, m_pos;
     for (int64_t j = 0; j < n_chains; ++j) {
         if (n_idx[j] < 0 || n_idx[j] >= n_orb || m_idx[j] < 0 || m_idx[j] >= n_orb)
             return ctx->fail(GWL_EINVAL, "gwl_set_chains: orbital index out of range");
-        const bool occ = n_idx[j] < ctx->n_v;
-        eps[j] = occ ? ctx->h_eps_v[n_idx[j]] : ctx->h_eps_c[n_idx[j] - ctx->n_v];
+        const bool occ = n_idx[j] < nv_orb;
+        eps[j] = occ ? ctx->h_eps_v[n_idx[j]] : ctx->h_eps_c[n_idx[j] - nv_orb];
         sgn[j] = occ ? 1 : -1;
+    }
+    if (ctx->sym) {  // |P_nm> lives in block Gamma_n ^ Gamma_m; conduction indices become rows of the padded Phi_c^T
+        auto locate = [&](int idx, int& irrep, int& pos) {
+            const bool occ = idx < nv_orb;
+            const int loc = occ ? idx : idx - nv_orb;
+            const int* off = occ ? ctx->sym_voff : ctx->sym_coff;
+            const int* cnt = occ ? ctx->sym_nv : ctx->sym_nc;
+            irrep = 0;
+            while (irrep + 1 < ctx->sym_g && loc >= off[irrep] + cnt[irrep]) ++irrep;
+            pos = occ ? idx : nv_orb + ctx->sym_cpoff[irrep] + (loc - off[irrep]);
+        };
+        n_pos.resize(n_chains);
+        m_pos.resize(n_chains);
+        for (int64_t j = 0; j < n_chains; ++j) {
+            int gn, gm;
+            locate(n_idx[j], gn, n_pos[j]);
+            locate(m_idx[j], gm, m_pos[j]);
+            if ((gn ^ gm) != ctx->sym_gamma)
+                return ctx->fail(GWL_EINVAL, "gwl_set_chains: the pair (n, m) does not belong to the selected symmetry block");
+        }
+        n_idx = n_pos.data();
+        m_idx = m_pos.data();
     }
     cudaStream_t st = ctx->stream;
     CK(ctx->d_nidx.ensure((size_t)n_chains * 4, st));
@@ -880,6 +1010,7 @@ gwl_status gwl_set_start_vectors(gwl_ctx* ctx, int64_t n_chains, const double* p
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_set_start_vectors: real-orbital call on a complex (gwl_tdc_create) context");
+    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_set_start_vectors: symmetry-block (gwl_sym_create) context: chains are set by orbital indices");
     if (n_chains < 0 || (n_chains > 0 && (p == nullptr || eps_n == nullptr || sgn_n == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_set_start_vectors: bad arguments");
     for (int64_t j = 0; j < n_chains; ++j)
@@ -1215,7 +1346,7 @@ gwl_status gwl_selfenergy(gwl_ctx* ctx, const double* omega, int64_t n_omega, do
         else
             CKL(7, launch_sigma_direct(ctx->theta.as<double>() + (size_t)c0 * L, ctx->wgt.as<double>() + (size_t)c0 * L, n2, ln,
                                        L, nc, en, sg, dom, (int)n_omega, eta, 0, 1.0, out, st));
-        if (sigma_sum != nullptr) CKL(7, launch_sigma_sum(out, nc, (int)n_omega, dsum, c0 > 0 ? 1 : 0, st));
+        if (sigma_sum != nullptr) CKL(7, launch_sigma_sum(out, nc, (int)n_omega, dsum, (c0 > 0 || ctx->sig_accumulate) ? 1 : 0, st));
     }
     if (sigma_sum != nullptr && nch == 0) CKL(7, launch_sigma_sum(dsig, 0, (int)n_omega, dsum, 0, st));
     if (!ctx->device_ptrs) {
@@ -1233,6 +1364,7 @@ gwl_status gwl_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, int6
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_selfenergy_state: real-orbital call on a complex (gwl_tdc_create) context");
+    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_selfenergy_state: symmetry-block (gwl_sym_create) context: use gwl_sym_selfenergy_state");
     if (sigma_mm == nullptr || omega == nullptr || n_omega < 1)
         return ctx->fail(GWL_EINVAL, "gwl_selfenergy_state: bad arguments");
     const int n_orb = ctx->n_v + ctx->n_c;
@@ -1249,6 +1381,7 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_exchange: real-orbital call on a complex (gwl_tdc_create) context");
+    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_exchange: symmetry-block (gwl_sym_create) context: not available on a symmetry-block context");
     if (n_states < 0 || (n_states > 0 && (m_idx == nullptr || sigma_x == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_exchange: bad arguments");
     if (!ctx->have_orb || !ctx->have_V) return ctx->fail(GWL_ESTATE, "gwl_exchange: orbitals and kernel must be set");
@@ -1287,7 +1420,7 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
             const int nb = std::min(chunk, ctx->n_v - v0);
             const int64_t off = j * ctx->n_v + v0;
             // rho_vm -> T;  W = V T;  sum_v rho_vm . (V rho_vm)
-            CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->n_v, ctx->n_mu,
+            CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->sym ? ctx->sym_nv_tot : ctx->n_v, ctx->n_mu,
                           ctx->x_nidx.as<int32_t>() + off, ctx->x_midx.as<int32_t>() + off, ctx->ws().T.as<double>(), ldm, nb,
                           st));
             rs = gemm_v(ctx, nb);
@@ -1357,6 +1490,7 @@ gwl_status gwl_spectrum_bounds(gwl_ctx* ctx, int64_t steps, double* lam_min, dou
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: real-orbital call on a complex (gwl_tdc_create) context");
+    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: symmetry-block (gwl_sym_create) context: not available on a symmetry-block context");
     if (steps < 2 || steps > 512 || lam_min == nullptr || lam_max == nullptr)
         return ctx->fail(GWL_EINVAL, "gwl_spectrum_bounds: need 2 <= steps <= 512 and non-NULL outputs");
     if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: orbitals, energies and kernel must be set");
@@ -1620,12 +1754,243 @@ gwl_status gwl_tdc_matvec_rpa(gwl_ctx* ctx, const double* x, const double* y, do
     return GWL_OK;
 }
 
+// ---- SURVEY.md 8(f)-4, second part: point-group symmetry blocks of C (reading Q25) -----------------
+gwl_status gwl_sym_create(gwl_ctx** out, int n_gen, const int32_t* nv_irrep, const int32_t* nc_irrep, int64_t n_mu_w) {
+    if (out == nullptr) return GWL_EINVAL;
+    *out = nullptr;
+    if (n_gen < 0 || n_gen > 3 || nv_irrep == nullptr || nc_irrep == nullptr || n_mu_w < 1) return GWL_EINVAL;
+    const int g = 1 << n_gen;
+    int64_t nv = 0, nc = 0, ncp = 0;
+    for (int a = 0; a < g; ++a) {
+        if (nv_irrep[a] < 0 || nc_irrep[a] < 0) return GWL_EINVAL;
+        nv += nv_irrep[a];
+        nc += nc_irrep[a];
+        ncp += round_up(nc_irrep[a], BK);
+    }
+    if (nv < 1 || nc < 1) return GWL_EINVAL;
+    gwl_status rs = create_common(out, 1, nv, ncp, n_mu_w, false, 1);
+    if (rs != GWL_OK) return rs;
+    gwl_ctx* ctx = *out;
+    ctx->sym = true;
+    ctx->sym_g = g;
+    ctx->sym_nv_tot = (int)nv;
+    ctx->sym_nc_tot = (int)nc;
+    ctx->sym_ncp_tot = (int)ncp;
+    int vo = 0, co = 0, cpo = 0;
+    for (int a = 0; a < g; ++a) {
+        ctx->sym_nv[a] = nv_irrep[a];
+        ctx->sym_nc[a] = nc_irrep[a];
+        ctx->sym_ncp[a] = (int)round_up(nc_irrep[a], BK);
+        ctx->sym_voff[a] = vo;
+        ctx->sym_coff[a] = co;
+        ctx->sym_cpoff[a] = cpo;
+        vo += nv_irrep[a];
+        co += nc_irrep[a];
+        cpo += ctx->sym_ncp[a];
+    }
+    return GWL_OK;
+}
+
+gwl_status gwl_sym_set_orbitals(gwl_ctx* ctx, const double* phi_v_w, const double* phi_c_w) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_sym_set_orbitals: not a gwl_sym_create context");
+    if (phi_v_w == nullptr || phi_c_w == nullptr) return ctx->fail(GWL_EINVAL, "gwl_sym_set_orbitals: NULL input");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int n_w = ctx->n_mu, nv = ctx->sym_nv_tot, nc = ctx->sym_nc_tot, ncp = ctx->sym_ncp_tot;
+    const int64_t ldm = ctx->n_mup;
+    DevBuf& tmp = ctx->stage;
+    CK(tmp.ensure(((size_t)n_w * nv + (size_t)n_w * nc) * 8, st));
+    double* dv = tmp.as<double>();
+    double* dc = dv + (size_t)n_w * nv;
+    CK(cudaMemcpyAsync(dv, phi_v_w, (size_t)n_w * nv * 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(dc, phi_c_w, (size_t)n_w * nc * 8, cudaMemcpyHostToDevice, st));
+    CK(ctx->phi_c.ensure((size_t)n_w * ncp * 8, st));    // [n_w][ncp_tot]: every irrep's columns padded to 16 with zero orbitals
+    CK(ctx->phi_cT.ensure((size_t)ncp * ldm * 8, st));   // [ncp_tot][n_mup]
+    CK(ctx->phi_vT.ensure((size_t)nv * ldm * 8, st));
+    CK(cudaMemsetAsync(ctx->phi_c.p, 0, ctx->phi_c.bytes, st));
+    CK(cudaMemsetAsync(ctx->phi_cT.p, 0, ctx->phi_cT.bytes, st));
+    CK(cudaMemsetAsync(ctx->phi_vT.p, 0, ctx->phi_vT.bytes, st));
+    for (int b = 0; b < ctx->sym_g; ++b) {
+        if (ctx->sym_nc[b] == 0) continue;
+        CK(cudaMemcpy2DAsync(ctx->phi_c.as<double>() + ctx->sym_cpoff[b], (size_t)ncp * 8, dc + ctx->sym_coff[b], (size_t)nc * 8,
+                             (size_t)ctx->sym_nc[b] * 8, (size_t)n_w, cudaMemcpyDeviceToDevice, st));
+    }
+    CKL(4, launch_transpose(ctx->phi_c.as<double>(), n_w, ncp, ctx->phi_cT.as<double>(), ldm, st));
+    CKL(4, launch_transpose(dv, n_w, nv, ctx->phi_vT.as<double>(), ldm, st));
+    CK(cudaStreamSynchronize(st));
+    ctx->have_orb = true;
+    invalidate_run(ctx);
+    return GWL_OK;
+}
+
+gwl_status gwl_sym_set_kernel(gwl_ctx* ctx, const double* V_wf) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_sym_set_kernel: not a gwl_sym_create context");
+    if (V_wf == nullptr) return ctx->fail(GWL_EINVAL, "gwl_sym_set_kernel: NULL input");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int n_w = ctx->n_mu, g = ctx->sym_g;
+    const size_t n_in = (size_t)n_w * g * n_w;
+    CK(ctx->stage.ensure(n_in * 8, st));
+    CK(cudaMemcpyAsync(ctx->stage.p, V_wf, n_in * 8, cudaMemcpyHostToDevice, st));
+    CK(ctx->V.ensure((size_t)g * n_w * ctx->n_mup * 8, st));
+    CK(cudaMemsetAsync(ctx->V.p, 0, ctx->V.bytes, st));
+    CKL(4, launch_sym_reduce_kernel(ctx->stage.as<double>(), n_w, g, ctx->V.as<double>(), ctx->n_mup, st));
+    CK(cudaStreamSynchronize(st));
+    ctx->have_V = true;
+    invalidate_run(ctx);
+    return GWL_OK;
+}
+
+gwl_status gwl_sym_select(gwl_ctx* ctx, int gamma, int64_t* n_pairs) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_sym_select: not a gwl_sym_create context");
+    if (gamma < 0 || gamma >= ctx->sym_g) return ctx->fail(GWL_EINVAL, "gwl_sym_select: no such irreducible representation");
+    if (!ctx->have_eps) return ctx->fail(GWL_ESTATE, "gwl_sym_select: energies must be set first");
+    int64_t npad = 0, napi = 0;
+    int64_t vecoff[8], apioff[8];
+    for (int a = 0; a < ctx->sym_g; ++a) {
+        const int b = a ^ gamma;
+        vecoff[a] = npad;
+        apioff[a] = napi;
+        npad += (int64_t)ctx->sym_nv[a] * ctx->sym_ncp[b];
+        napi += (int64_t)ctx->sym_nv[a] * ctx->sym_nc[b];
+    }
+    if (n_pairs != nullptr) *n_pairs = napi;
+    if (napi == 0) return ctx->fail(GWL_EINVAL, "gwl_sym_select: this block has no pairs");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    CK(cudaStreamSynchronize(st));
+    ctx->sym_gamma = gamma;
+    ctx->sym_npairs = napi;
+    for (int a = 0; a < ctx->sym_g; ++a) {
+        ctx->sym_vecoff[a] = vecoff[a];
+        ctx->sym_apioff[a] = apioff[a];
+    }
+    ctx->n_c = ctx->n_cp = BK;  // the vector kernels see ONE padded block vector whose K.X copy has the same layout
+    ctx->n_v = (int)(npad / BK);
+    ctx->n_vc = npad;
+    ctx->v_sel = (int64_t)gamma * ctx->n_mu * ctx->n_mup;
+    CK(ctx->d2.ensure((size_t)npad * 8, st));
+    CK(ctx->s.ensure((size_t)npad * 8, st));
+    for (int a = 0; a < ctx->sym_g; ++a) {
+        const int b = a ^ gamma;
+        CKL(4, launch_sym_build_delta(ctx->eps_v.as<double>() + ctx->sym_voff[a], ctx->eps_c.as<double>() + ctx->sym_coff[b],
+                                      ctx->sym_nv[a], ctx->sym_nc[b], ctx->sym_ncp[b], ctx->d2.as<double>() + vecoff[a],
+                                      ctx->s.as<double>() + vecoff[a], st));
+    }
+    CK(cudaStreamSynchronize(st));
+    invalidate_run(ctx);
+    ctx->chain_mode = 0;
+    ctx->n_chains_set = 0;
+    return GWL_OK;
+}
+
+gwl_status gwl_sym_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_sym_matvec: not a gwl_sym_create context");
+    if (nvec < 0) return ctx->fail(GWL_EINVAL, "gwl_sym_matvec: nvec < 0");
+    if (nvec == 0) return GWL_OK;
+    if (x == nullptr || y == nullptr) return ctx->fail(GWL_EINVAL, "gwl_sym_matvec: NULL vector");
+    if (!ready(ctx) || ctx->sym_gamma < 0) return ctx->fail(GWL_ESTATE, "gwl_sym_matvec: orbitals, energies, kernel and a selected block are needed");
+    LaunchScope ls(ctx);
+    cudaStream_t st = ctx->stream;
+    const int chunk = (int)std::min<int64_t>(nvec, 256);
+    gwl_status rs = ensure_workspace(ctx, chunk);
+    if (rs != GWL_OK) return rs;
+    const int64_t npad = ctx->n_vc, napi = ctx->sym_npairs;
+    CK(ctx->io_x.ensure((size_t)chunk * npad * 8, st));
+    CK(ctx->io_y.ensure((size_t)chunk * npad * 8, st));
+    if (!ctx->device_ptrs) CK(ctx->stage.ensure((size_t)chunk * napi * 8, st));
+    for (int64_t j0 = 0; j0 < nvec; j0 += chunk) {
+        const int nb = (int)std::min<int64_t>(chunk, nvec - j0);
+        double* api = const_cast<double*>(x) + j0 * napi;
+        if (!ctx->device_ptrs) {
+            CK(cudaMemcpyAsync(ctx->stage.p, x + j0 * napi, (size_t)nb * napi * 8, cudaMemcpyHostToDevice, st));
+            api = ctx->stage.as<double>();
+        }
+        for (int a = 0; a < ctx->sym_g; ++a) {
+            const int b = a ^ ctx->sym_gamma;
+            CKL(4, launch_sym_copy_rect(api + ctx->sym_apioff[a], napi, ctx->io_x.as<double>() + ctx->sym_vecoff[a], npad,
+                                        ctx->sym_nv[a], ctx->sym_nc[b], ctx->sym_ncp[b], nb, 0, st));
+        }
+        CKL(4, launch_prescale(ctx->io_x.as<double>(), npad, ctx->xs.as<double>(), npad, ctx->s.as<double>(), ctx->n_v, ctx->n_c,
+                               ctx->n_cp, nb, st));
+        rs = apply_casida_core(ctx, ctx->io_x.as<double>(), npad, ctx->io_y.as<double>(), npad, nb, nullptr, 0);
+        if (rs != GWL_OK) return rs;
+        double* out = ctx->device_ptrs ? y + j0 * napi : ctx->stage.as<double>();
+        for (int a = 0; a < ctx->sym_g; ++a) {
+            const int b = a ^ ctx->sym_gamma;
+            CKL(4, launch_sym_copy_rect(out + ctx->sym_apioff[a], napi, ctx->io_y.as<double>() + ctx->sym_vecoff[a], npad,
+                                        ctx->sym_nv[a], ctx->sym_nc[b], ctx->sym_ncp[b], nb, 1, st));
+        }
+        if (!ctx->device_ptrs) {
+            CK(cudaMemcpyAsync(y + j0 * napi, ctx->stage.p, (size_t)nb * napi * 8, cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+        }
+    }
+    return GWL_OK;
+}
+
+gwl_status gwl_sym_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, int64_t block, int reorth, const double* omega,
+                                    int64_t n_omega, double eta, double* sigma_mm) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_sym_selfenergy_state: not a gwl_sym_create context");
+    if (sigma_mm == nullptr || omega == nullptr || n_omega < 1) return ctx->fail(GWL_EINVAL, "gwl_sym_selfenergy_state: bad arguments");
+    const int nv = ctx->sym_nv_tot, n_orb = nv + ctx->sym_nc_tot;
+    if (m_idx < 0 || m_idx >= n_orb) return ctx->fail(GWL_EINVAL, "gwl_sym_selfenergy_state: orbital index out of range");
+    auto irrep_of = [&](int idx) {
+        const bool occ = idx < nv;
+        const int loc = occ ? idx : idx - nv;
+        const int* off = occ ? ctx->sym_voff : ctx->sym_coff;
+        const int* cnt = occ ? ctx->sym_nv : ctx->sym_nc;
+        int a = 0;
+        while (a + 1 < ctx->sym_g && loc >= off[a] + cnt[a]) ++a;
+        return a;
+    };
+    const int gm = irrep_of(m_idx);
+    bool first = true;
+    gwl_status rs = GWL_OK;
+    for (int gamma = 0; gamma < ctx->sym_g && rs == GWL_OK; ++gamma) {
+        std::vector<int32_t> n_idx;
+        for (int n = 0; n < n_orb; ++n)
+            if ((irrep_of(n) ^ gm) == gamma) n_idx.push_back(n);
+        if (n_idx.empty()) continue;
+        int64_t npairs = -1;
+        rs = gwl_sym_select(ctx, gamma, &npairs);
+        if (rs != GWL_OK) {
+            if (npairs == 0) {  // no excitation carries this symmetry: these chains contribute nothing
+                rs = GWL_OK;
+                continue;
+            }
+            break;
+        }
+        std::vector<int32_t> m_rep(n_idx.size(), m_idx);
+        rs = gwl_set_chains(ctx, (int64_t)n_idx.size(), n_idx.data(), m_rep.data());
+        if (rs == GWL_OK) rs = gwl_lanczos(ctx, (int64_t)n_idx.size(), steps, block, reorth, nullptr, nullptr, nullptr, nullptr);
+        if (rs != GWL_OK) break;
+        ctx->sig_accumulate = !first;
+        rs = gwl_selfenergy(ctx, omega, n_omega, eta, nullptr, sigma_mm);
+        ctx->sig_accumulate = false;
+        first = false;
+    }
+    if (rs == GWL_OK && first) return ctx->fail(GWL_EINVAL, "gwl_sym_selfenergy_state: no symmetry block has pairs");
+    return rs;
+}
+
 // ---- ISDF front end (PAPER.md:115-128, Eq. 15-17; :319) ---------------------------------------------
 gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, const double* phi_c_grid, const double* r,
                           double weight, double soft, const int32_t* idx, double* zeta_t, double* V_out) {
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_isdf_build: real-orbital call on a complex (gwl_tdc_create) context");
+    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_isdf_build: symmetry-block (gwl_sym_create) context: not available on a symmetry-block context");
     if (phi_v_grid == nullptr || phi_c_grid == nullptr || r == nullptr || idx == nullptr)
         return ctx->fail(GWL_EINVAL, "gwl_isdf_build: NULL input");
     if (n_r < ctx->n_mu || n_r > 65535 || !(weight > 0.0) || !(soft > 0.0))

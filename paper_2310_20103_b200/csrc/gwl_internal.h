@@ -283,6 +283,18 @@ cudaError_t launch_cvt_update(const double* r, const double* w, int n_r, const i
 cudaError_t launch_cvt_snap(const double* r, int n_r, const int32_t* assign, const double* c, int n_mu, int32_t* idx,
                             cudaStream_t st);
 
+// ---------------------------------------------------------------------------------------------
+// Point-group symmetry blocks (sym_kernels.cu, reading Q25)
+// ---------------------------------------------------------------------------------------------
+// vg[gamma][mu][nu] (row stride ld) = g sum_h chi_gamma(h) vwf[mu][h][nu], all gamma < g <= 8
+cudaError_t launch_sym_reduce_kernel(const double* vwf, int n_w, int g, double* vg, int64_t ld, cudaStream_t st);
+// d2 = Delta^2, s = sqrt(Delta) of one [nv][ncp] rectangle (columns >= nc are padding: d2 = s = 1)
+cudaError_t launch_sym_build_delta(const double* eps_v, const double* eps_c, int nv, int nc, int ncp, double* d2, double* s,
+                                   cudaStream_t st);
+// one rectangle of nvec block vectors: dir 0 api [nv][nc] -> padded [nv][ncp] (zero fill), dir 1 back
+cudaError_t launch_sym_copy_rect(double* api, int64_t ld_api, double* padded, int64_t ld_pad, int nv, int nc, int ncp, int nvec,
+                                 int dir, cudaStream_t st);
+
 // probe.cu
 cudaError_t probe_fp64_peak(int kind, double* tflops);
 

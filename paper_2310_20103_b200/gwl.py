@@ -49,6 +49,12 @@ SIGNATURES = {
     "gwl_tdc_set_chains": (c_int, [c_void_p, c_int64, c_void_p]),
     "gwl_tdc_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
     "gwl_tdc_matvec_rpa": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int64]),
+    "gwl_sym_create": (c_int, [POINTER(c_void_p), c_int, c_void_p, c_void_p, c_int64]),
+    "gwl_sym_set_orbitals": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "gwl_sym_set_kernel": (c_int, [c_void_p, c_void_p]),
+    "gwl_sym_select": (c_int, [c_void_p, c_int, POINTER(c_int64)]),
+    "gwl_sym_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
+    "gwl_sym_selfenergy_state": (c_int, [c_void_p, c_int32, c_int64, c_int64, c_int, c_void_p, c_int64, c_double, c_void_p]),
     "gwl_isdf_build": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_double, c_double, c_void_p, c_void_p,
                                c_void_p]),
     "gwl_isdf_select_points": (c_int, [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_int64, c_void_p, POINTER(c_int32)]),
@@ -432,6 +438,68 @@ class TdcContext(Context):
         oxh, oyh = np.empty_like(xh), np.empty_like(yh)
         self._ck(self._lib.gwl_tdc_matvec_rpa(self._h, _ptr(xh), _ptr(yh), _ptr(oxh), _ptr(oyh), xh.size // self.n_kvc))
         return oxh, oyh
+
+
+class SymContext(Context):
+    """Symmetry-block context, gwl_sym_* (reading Q25): an abelian point group of
+    order 2^n_gen, orbitals sorted by irrep.  After select(gamma) the inherited set_chains / lanczos / resolvent /
+    selfenergy / set_polynomial calls act on block gamma."""
+
+    def __init__(self, n_gen: int, nv_irrep, nc_irrep, n_mu_w: int):
+        self._lib = load_library()
+        self._h = c_void_p()
+        self.nv_irrep, self.nc_irrep = _host(nv_irrep, np.int32), _host(nc_irrep, np.int32)
+        self.g = 1 << int(n_gen)
+        if self.nv_irrep.shape != (self.g,) or self.nc_irrep.shape != (self.g,):
+            raise GwlError(GWL_EINVAL, "SymContext: nv_irrep and nc_irrep need 2^n_gen entries")
+        self.n_v, self.n_c, self.n_mu = int(self.nv_irrep.sum()), int(self.nc_irrep.sum()), int(n_mu_w)
+        self.n_vc = 0                                      # pairs of the selected block
+        self.device_ptrs = 0
+        st = self._lib.gwl_sym_create(byref(self._h), int(n_gen), _ptr(self.nv_irrep), _ptr(self.nc_irrep), int(n_mu_w))
+        if st != GWL_OK:
+            self._h = c_void_p()
+            raise GwlError(st, "gwl_sym_create failed (no CUDA device, or bad sizes)")
+
+    def set_orbitals(self, phi_v_w, phi_c_w):
+        pv, pc = _host(phi_v_w), _host(phi_c_w)
+        if pv.shape != (self.n_mu, self.n_v) or pc.shape != (self.n_mu, self.n_c):
+            raise GwlError(GWL_EINVAL, "set_orbitals: phi_v_w must be [n_mu_w, N_v], phi_c_w [n_mu_w, N_c]")
+        self._ck(self._lib.gwl_sym_set_orbitals(self._h, _ptr(pv), _ptr(pc)))
+
+    def set_kernel(self, V_wf):
+        Vh = _host(V_wf)
+        if Vh.shape != (self.n_mu, self.g, self.n_mu):
+            raise GwlError(GWL_EINVAL, "set_kernel: V_wf must be [n_mu_w, g, n_mu_w]")
+        self._ck(self._lib.gwl_sym_set_kernel(self._h, _ptr(Vh)))
+
+    def select(self, gamma: int) -> int:
+        n = c_int64(0)
+        self._ck(self._lib.gwl_sym_select(self._h, int(gamma), byref(n)))
+        self.n_vc = n.value
+        return n.value
+
+    def matvec(self, x, y=None):
+        """y = C_gamma x on the selected block.  Host mode: numpy [nvec, n_pairs]; device mode: torch CUDA tensors."""
+        if self.device_ptrs:
+            self._ck(self._lib.gwl_sym_matvec(self._h, _ptr(x), _ptr(y), x.numel() // self.n_vc))
+            return y
+        xh = _host(x)
+        if self.n_vc == 0 or xh.size % self.n_vc:
+            raise GwlError(GWL_EINVAL, "matvec: x must be [nvec, n_pairs of the selected block]")
+        yh = np.empty_like(xh)
+        self._ck(self._lib.gwl_sym_matvec(self._h, _ptr(xh), _ptr(yh), xh.size // self.n_vc))
+        return yh
+
+    def selfenergy_state(self, m_idx: int, steps: int, block: int, reorth: int, omega, eta: float, out=None):
+        if self.device_ptrs:
+            self._ck(self._lib.gwl_sym_selfenergy_state(self._h, int(m_idx), steps, block, reorth, _ptr(omega), omega.numel(),
+                                                        float(eta), _ptr(out)))
+            return out
+        om = _host(omega)
+        ss = np.zeros(om.size, dtype=np.complex128)
+        self._ck(self._lib.gwl_sym_selfenergy_state(self._h, int(m_idx), steps, block, reorth, _ptr(om), om.size, float(eta),
+                                                    _ptr(ss)))
+        return ss
 
 
 def context_from_problem(prob) -> Context:
