@@ -55,6 +55,10 @@ def parse():
     ap.add_argument("--rpa", action="store_true",
                     help="with --tdc: the full RPA for complex orbitals (pseudo-Hermitian Lanczos on C^RPA(q), PAPER.md:159): every "
                          "chain is a pair [x; y] = two GEMM columns, one product with Omega^ per step")
+    ap.add_argument("--sym", type=int, default=-1, metavar="NGEN",
+                    help="context run, not the bench line: the point-group symmetry blocks of C (SURVEY 8(f)-4, PAPER.md:128) for an "
+                         "abelian group of order 2^NGEN on a synthetic system with the sizes of --config (default 4): one block "
+                         "of chains x L Lanczos steps inside the pair-irrep block gamma = 1")
     ap.add_argument("--sharded-state", action="store_true",
                     help="SURVEY 8(f)-2 arm, its own line: the N_v+N_c chains of ONE state partitioned over the ranks "
                          "(runtime.shard_range), one NCCL all-reduce of the omega grid; strong scaling")
@@ -316,6 +320,82 @@ def run_tdc(args):
     ctx.close()
 
 
+def run_sym(args):
+    """Symmetry blocks (gwl_sym_*): one block of chains x L steps inside one pair-irrep block of a system with the sizes of a
+    BASELINE config and an abelian point group of order g; flop model of the REDUCED operator, (4 n_w N_pairs + 2 n_w^2) B per
+    block product, next to what the same chains cost without the symmetry."""
+    import numpy as np
+    import torch
+
+    from paper_2310_20103_b200 import gwl, synth
+
+    cfg = synth.CONFIGS[2 if args.config is None else args.config]
+    g = 1 << args.sym
+    if cfg.n_v % g or cfg.n_c % g or cfg.n_mu % g:
+        raise SystemExit("--sym: the config's N_v, N_c, N_mu must be divisible by the group order")
+    nch = args.chains or min(cfg.block, cfg.n_v // g + cfg.n_c // g)
+    L = args.lanczos_steps or 10
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    gwl.load_library()
+    p = synth.make_symmetric(args.sym, [cfg.n_v // g] * g, [cfg.n_c // g] * g, cfg.n_mu // g, box=cfg.box, seed=0,
+                             n_omega=cfg.n_omega)
+    gamma = 1 if g > 1 else 0
+    irr = np.concatenate([p.irrep_v, p.irrep_c])
+    m = 0
+    n_idx = np.array([n for n in range(irr.size) if irr[n] ^ irr[m] == gamma][:nch], dtype=np.int32)
+    nch = n_idx.size
+    ctx = gwl.SymContext(args.sym, p.nv_irrep, p.nc_irrep, p.n_w)
+    stream = torch.cuda.current_stream()
+    ctx.set_stream(stream.cuda_stream)
+    ctx.set_orbitals(p.phi_v_w, p.phi_c_w)
+    ctx.set_energies(p.eps_v, p.eps_c)
+    ctx.set_kernel(p.V_wf)
+    n_pairs = ctx.select(gamma)
+    ctx.set_chains(n_idx, np.full(nch, m, dtype=np.int32))
+    ctx.set_pointer_mode(1)
+    ctx.set_profiling(0)
+    om = torch.from_numpy(p.omega).to(dev)
+    ssum = torch.empty(len(p.omega), 2, dtype=torch.float64, device=dev)
+    peak = gwl.probe_fp64_peak(0)
+
+    def step():
+        ctx.lanczos(nch, L, nch, 0, out=None)
+        ctx.selfenergy(om, cfg.eta, out=(None, ssum))
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        a.record(stream)
+        step()
+        b.record(stream)
+    torch.cuda.synchronize()
+    sec = sum(a.elapsed_time(b) for a, b in ev) * 1e-3 / args.steps
+    ctx.set_profiling(2)
+    step()
+    kt = ctx.get_kernel_times()
+    ctx.set_profiling(0)
+    fl_block = (4.0 * p.n_w * n_pairs + 2.0 * p.n_w * p.n_w) * nch
+    ms_mv = sum(kt[k][0] for k in ("gemm_fwd_KX", "gemm_V", "gemm_bwd_KtW", "splitk_reduce")) / (L + 0.5)
+    line = {"metric": METRIC, "value": nch * L / sec, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * sec, "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+            "arm": "sym (SURVEY 8(f)-4, PAPER.md:128): context run, not the headline bench line",
+            "config": {"workload": f"symmetry block gamma = {gamma} of a system with the sizes of {cfg.name} and an abelian point "
+                                   f"group of order {g}: one block of chains x L steps inside the block",
+                       "group_order": g, "n_v": cfg.n_v, "n_c": cfg.n_c, "n_mu_full": cfg.n_mu, "n_mu_wedge": p.n_w,
+                       "n_pairs_block": int(n_pairs), "n_vc_full": cfg.n_vc, "chains": int(nch), "lanczos_steps": L},
+            "matvec": {"tflops": fl_block / (ms_mv * 1e-3) / 1e12, "frac_of_dmma_peak": fl_block / (ms_mv * 1e-3) / 1e12 / peak,
+                       "ms_per_block_matvec": ms_mv, "flop_model": "(4 n_w N_pairs + 2 n_w^2) B (reduced operator)",
+                       "flop_without_symmetry": cfg.flop_per_vector() * nch,
+                       "flop_ratio": cfg.flop_per_vector() * nch / fl_block},
+            "roofline": {"bound": "tensor", "peak": peak, "unit": "TFLOP/s"},
+            "kernel_time_share": {k: round(v[0] / sum(x[0] for x in kt.values()), 4) for k, v in kt.items() if v[1]}}
+    print(json.dumps(line), flush=True)
+    ctx.close()
+
+
 def cublas_dgemm_tflops(dev, n=8192, reps=3):
     """torch.matmul FP64 n^3 (cuBLAS DGEMM), best of `reps`: printed beside the DMMA probe as context."""
     import torch
@@ -425,6 +505,9 @@ def main():
         return
     if args.sharded_state:
         run_sharded_state(args)
+        return
+    if args.sym >= 0:
+        run_sym(args)
         return
     if args.tdc:
         run_tdc(args)
