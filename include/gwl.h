@@ -244,8 +244,11 @@ gwl_status gwl_isdf_select_points(gwl_ctx* ctx, int64_t n_r, const double* r, co
  * A context made by gwl_sym_create takes gwl_sym_set_orbitals / gwl_set_energies / gwl_sym_set_kernel once, then
  * gwl_sym_select(gamma) makes block gamma the operator: gwl_sym_matvec, gwl_set_chains (pairs (n, m) of that block only, else
  * GWL_EINVAL), gwl_lanczos, gwl_resolvent, gwl_selfenergy, gwl_set_polynomial and the gwl_get_* calls then work as on a plain
- * context; gwl_sym_selfenergy_state walks all blocks for one orbital m.  Block vectors hold the pairs of block gamma ordered by
- * the irrep a of v (ascending), then v, then c over the irrep a ^ gamma.  The other real-orbital calls return GWL_ESTATE. */
+ * context, and so does gwl_spectrum_bounds (bounds of the selected block); gwl_sym_selfenergy_state walks all blocks for one
+ * orbital m; gwl_exchange works on any orbital (rho_vm transforms as irrep(v) ^ irrep(m): every irrep of v goes against its own
+ * reduced kernel) and gwl_qp_solve is unchanged.  Block vectors hold the pairs of block gamma ordered by the irrep a of v
+ * (ascending), then v, then c over the irrep a ^ gamma.  gwl_set_orbitals, gwl_set_kernel, gwl_casida_matvec,
+ * gwl_set_start_vectors, gwl_selfenergy_state, gwl_set_approximation and gwl_isdf_build return GWL_ESTATE on such a context. */
 gwl_status gwl_sym_create(gwl_ctx** out, int n_gen, const int32_t* nv_irrep /*[2^n_gen]*/, const int32_t* nc_irrep /*[2^n_gen]*/,
                           int64_t n_mu_w);
 /* Orbital values at the wedge points: phi_v_w [n_mu_w][N_v], phi_c_w [n_mu_w][N_c] (N_v = sum nv_irrep, N_c = sum nc_irrep), host. */

@@ -1381,30 +1381,47 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_exchange: real-orbital call on a complex (gwl_tdc_create) context");
-    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_exchange: symmetry-block (gwl_sym_create) context: not available on a symmetry-block context");
     if (n_states < 0 || (n_states > 0 && (m_idx == nullptr || sigma_x == nullptr)))
         return ctx->fail(GWL_EINVAL, "gwl_exchange: bad arguments");
     if (!ctx->have_orb || !ctx->have_V) return ctx->fail(GWL_ESTATE, "gwl_exchange: orbitals and kernel must be set");
     if (n_states == 0) return GWL_OK;
-    const int n_orb = ctx->n_v + ctx->n_c;
+    const int nv_orb = ctx->sym ? ctx->sym_nv_tot : ctx->n_v;
+    const int n_orb = nv_orb + (ctx->sym ? ctx->sym_nc_tot : ctx->n_c);
     for (int64_t j = 0; j < n_states; ++j)
         if (m_idx[j] < 0 || m_idx[j] >= n_orb) return ctx->fail(GWL_EINVAL, "gwl_exchange: orbital index out of range");
     LaunchScope ls(ctx);
     cudaStream_t st = ctx->stream;
-    const int chunk = std::min(ctx->n_v, 256);
+    const int chunk = std::min(nv_orb, 256);
     const int64_t ldm = ctx->n_mup;
     const int npart = vec_parts(ctx->n_mu);
     // only what rho -> V rho -> dot touches: T, W and the V.T split-K partials (none of the N_vc-sized Casida buffers)
     CK(ctx->ws().T.ensure((size_t)chunk * ldm * 8, st));
     CK(ctx->ws().W.ensure((size_t)chunk * ldm * 8, st));
     gwl_status rs = GWL_OK;
+    // Symmetry-block contexts (reading Q25): rho_vm transforms as gamma = irrep(v) ^ irrep(m), so (vm|vm) over all points is
+    // rho_w^T V^gamma rho_w on the wedge; the occupied orbitals go irrep by irrep, each against its own reduced kernel.
+    auto irrep_pos = [&](int idx, int& irrep, int& pos) {
+        irrep = 0;
+        pos = idx;
+        if (!ctx->sym) return;
+        const bool occ = idx < nv_orb;
+        const int loc = occ ? idx : idx - nv_orb;
+        const int* off = occ ? ctx->sym_voff : ctx->sym_coff;
+        const int* cnt = occ ? ctx->sym_nv : ctx->sym_nc;
+        while (irrep + 1 < ctx->sym_g && loc >= off[irrep] + cnt[irrep]) ++irrep;
+        pos = occ ? idx : nv_orb + ctx->sym_cpoff[irrep] + (loc - off[irrep]);  // row of the padded Phi_c^T
+    };
     // (v, m) index pairs of every rho_vm, state-major
-    std::vector<int32_t> hv((size_t)n_states * ctx->n_v), hm((size_t)n_states * ctx->n_v);
-    for (int64_t j = 0; j < n_states; ++j)
-        for (int v = 0; v < ctx->n_v; ++v) {
-            hv[(size_t)j * ctx->n_v + v] = v;
-            hm[(size_t)j * ctx->n_v + v] = m_idx[j];
+    std::vector<int32_t> hv((size_t)n_states * nv_orb), hm((size_t)n_states * nv_orb), gm(n_states);
+    for (int64_t j = 0; j < n_states; ++j) {
+        int irr, pos;
+        irrep_pos(m_idx[j], irr, pos);
+        gm[j] = irr;
+        for (int v = 0; v < nv_orb; ++v) {
+            hv[(size_t)j * nv_orb + v] = v;
+            hm[(size_t)j * nv_orb + v] = pos;
         }
+    }
     CK(ctx->x_nidx.ensure(hv.size() * 4, st));
     CK(ctx->x_midx.ensure(hm.size() * 4, st));
     CK(ctx->x_part.ensure((size_t)chunk * npart * 8, st));
@@ -1415,21 +1432,33 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
         CK(ctx->x_sig.ensure((size_t)n_states * 8, st));
         dout = ctx->x_sig.as<double>();
     }
+    const int64_t v_sel_saved = ctx->v_sel;
+    const int n_seg = ctx->sym ? ctx->sym_g : 1;
     for (int64_t j = 0; j < n_states; ++j) {
-        for (int v0 = 0; v0 < ctx->n_v; v0 += chunk) {
-            const int nb = std::min(chunk, ctx->n_v - v0);
-            const int64_t off = j * ctx->n_v + v0;
-            // rho_vm -> T;  W = V T;  sum_v rho_vm . (V rho_vm)
-            CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, ctx->sym ? ctx->sym_nv_tot : ctx->n_v, ctx->n_mu,
-                          ctx->x_nidx.as<int32_t>() + off, ctx->x_midx.as<int32_t>() + off, ctx->ws().T.as<double>(), ldm, nb,
-                          st));
-            rs = gemm_v(ctx, nb);
-            if (rs != GWL_OK) return rs;
-            CKL(4, launch_dot_partials(ctx->ws().T.as<double>(), ctx->ws().W.as<double>(), ldm, ctx->n_mu, nb,
-                                   ctx->x_part.as<double>(), npart, st));
-            CKL(4, launch_accum_neg(ctx->x_part.as<double>(), nb * npart, dout + j, v0 == 0 ? 1 : 0, st));
+        bool first = true;
+        for (int a = 0; a < n_seg; ++a) {
+            const int seg0 = ctx->sym ? ctx->sym_voff[a] : 0, seg1 = ctx->sym ? seg0 + ctx->sym_nv[a] : nv_orb;
+            if (ctx->sym) ctx->v_sel = (int64_t)(a ^ gm[j]) * ctx->n_mu * ctx->n_mup;
+            for (int v0 = seg0; v0 < seg1; v0 += chunk) {
+                const int nb = std::min(chunk, seg1 - v0);
+                const int64_t off = j * nv_orb + v0;
+                // rho_vm -> T;  W = V T;  sum_v rho_vm . (V rho_vm)
+                CKL(4, launch_rho(ctx->phi_vT.as<double>(), ctx->phi_cT.as<double>(), ldm, nv_orb, ctx->n_mu,
+                                  ctx->x_nidx.as<int32_t>() + off, ctx->x_midx.as<int32_t>() + off, ctx->ws().T.as<double>(), ldm, nb,
+                                  st));
+                rs = gemm_v(ctx, nb);
+                if (rs != GWL_OK) {
+                    ctx->v_sel = v_sel_saved;
+                    return rs;
+                }
+                CKL(4, launch_dot_partials(ctx->ws().T.as<double>(), ctx->ws().W.as<double>(), ldm, ctx->n_mu, nb,
+                                           ctx->x_part.as<double>(), npart, st));
+                CKL(4, launch_accum_neg(ctx->x_part.as<double>(), nb * npart, dout + j, first ? 1 : 0, st));
+                first = false;
+            }
         }
     }
+    ctx->v_sel = v_sel_saved;
     if (!ctx->device_ptrs) {
         CK(cudaMemcpyAsync(sigma_x, dout, (size_t)n_states * 8, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
@@ -1490,12 +1519,12 @@ gwl_status gwl_spectrum_bounds(gwl_ctx* ctx, int64_t steps, double* lam_min, dou
     if (ctx == nullptr) return GWL_EINVAL;
     DeviceGuard dg(ctx);
     if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: real-orbital call on a complex (gwl_tdc_create) context");
-    if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: symmetry-block (gwl_sym_create) context: not available on a symmetry-block context");
     if (steps < 2 || steps > 512 || lam_min == nullptr || lam_max == nullptr)
         return ctx->fail(GWL_EINVAL, "gwl_spectrum_bounds: need 2 <= steps <= 512 and non-NULL outputs");
     if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: orbitals, energies and kernel must be set");
+    if (ctx->sym && ctx->sym_gamma < 0) return ctx->fail(GWL_ESTATE, "gwl_spectrum_bounds: select a symmetry block first (gwl_sym_select)");
     cudaStream_t st = ctx->stream;
-    const int L = (int)std::min<int64_t>(steps, ctx->n_vc);
+    const int L = (int)std::min<int64_t>(steps, ctx->sym ? ctx->sym_npairs : ctx->n_vc);
     // one chain from a generic (counter-based pseudo-random) start vector, on the operator itself (never p_g)
     {
         LaunchScope ls(ctx);
@@ -1503,6 +1532,12 @@ gwl_status gwl_spectrum_bounds(gwl_ctx* ctx, int64_t steps, double* lam_min, dou
         CK(ctx->d_eps_n.ensure(8, st));
         CK(ctx->d_sgn_n.ensure(4, st));
         CKL(4, launch_fill_hash(ctx->d_start.as<double>(), ctx->n_vc, 0x9E3779B97F4A7C15ull, st));
+        if (ctx->sym)  // the padding pairs are not part of the block: keep the probe vector off them
+            for (int a = 0; a < ctx->sym_g; ++a) {
+                const int b = a ^ ctx->sym_gamma;
+                CKL(4, launch_sym_zero_pad(ctx->d_start.as<double>() + ctx->sym_vecoff[a], ctx->n_vc, ctx->sym_nv[a], ctx->sym_nc[b],
+                                           ctx->sym_ncp[b], 1, st));
+            }
         const double e0 = 0.0;
         const int32_t s0 = 1;
         CK(cudaMemcpyAsync(ctx->d_eps_n.p, &e0, 8, cudaMemcpyHostToDevice, st));

@@ -295,6 +295,9 @@ cudaError_t launch_sym_build_delta(const double* eps_v, const double* eps_c, int
 cudaError_t launch_sym_copy_rect(double* api, int64_t ld_api, double* padded, int64_t ld_pad, int nv, int nc, int ncp, int nvec,
                                  int dir, cudaStream_t st);
 
+// zero the padding columns c >= nc of one [nv][ncp] rectangle of nvec block vectors (row stride ld)
+cudaError_t launch_sym_zero_pad(double* x, int64_t ld, int nv, int nc, int ncp, int nvec, cudaStream_t st);
+
 // probe.cu
 cudaError_t probe_fp64_peak(int kind, double* tflops);
 

@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
     const int g = lane >> 2, q = lane & 3;
     // ---- work list ------------------------------------------------------------------------------------
     // FWD / PLAIN: one segment per CTA, (m-tile, n-tile, split) = blockIdx.
-    // BWD: a persistent 1-D grid of G CTAs over the tiles (order: n-tile, group of G v's, m-tile, v in group), in two phases.
+    // BWD: a persistent 1-D grid of G CTAs over the tiles, v fastest (tile = (m-tile, n-tile, v)), in two phases.
     //  (1) R = floor(tiles / G) aligned rounds: CTA g takes tile i*G + g whole.  All CTAs walk the same k-range at the
     //      same time and neighbouring CTAs differ only in v, so they read the SAME Phi_c^T and W k-tiles: each comes
     //      from HBM once and is an L2 hit for the others.
@@ -114,20 +114,13 @@ __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 4) * 32, 1)
             n0 = blockIdx.y * BN;
             z = blockIdx.z;
         } else {
-            // n-tile outermost, then groups of G = gridDim.x consecutive v, inside a group m-tile then v (v fastest): one aligned
-            // round still shares one Phi_c^T m-tile and one W n-tile among CTAs that differ only in v, AND the group's G rows of
-            // Phi_v^T stay in L2 over all m-tiles instead of being re-streamed once per m-tile (config 4: 5.4 GB per launch)
-            const int per_n = p.scale_rows * p.tiles_m;
-            const int nt = tile / per_n, r = tile - nt * per_n;
-            const int G = (int)gridDim.x;
-            const int sg = r / (G * p.tiles_m);
-            const int v_start = sg * G;
-            const int len = min(G, p.scale_rows - v_start);
-            const int r_sg = r - sg * G * p.tiles_m;
-            const int mi = r_sg / len;
-            z = v_start + (r_sg - mi * len);  // v
-            n0 = nt * BN;
-            m0 = mi * BM;
+            // v fastest.  Tried in round 2 and dropped: groups of G v's with the m-tile inside a group (to keep a group's rows of
+            // Phi_v^T in L2): 25.8 GB instead of 18.3 GB of DRAM reads per launch at config 4 and 0.6 % slower -- a new 21 MB
+            // Phi_c^T slice every round costs more than the Phi_v^T rows it saves.
+            z = tile % p.scale_rows;  // v
+            const int r = tile / p.scale_rows;
+            n0 = (r % p.tiles_n) * BN;
+            m0 = (r / p.tiles_n) * BM;
         }
     };
 

@@ -55,7 +55,26 @@ __global__ void k_sym_copy_rect(double* __restrict__ api, int64_t ld_api, double
     }
 }
 
+// x[b][v][c] = 0 on the padding columns c >= nc of one rectangle
+__global__ void k_sym_zero_pad(double* __restrict__ x, int64_t ld, int nv, int nc, int ncp) {
+    const int b = blockIdx.y;
+    const int npad = ncp - nc;
+    const int64_t n = (int64_t)nv * npad;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int v = (int)(i / npad), c = nc + (int)(i - (int64_t)v * npad);
+        x[(int64_t)b * ld + (int64_t)v * ncp + c] = 0.0;
+    }
+}
+
 }  // namespace
+
+cudaError_t launch_sym_zero_pad(double* x, int64_t ld, int nv, int nc, int ncp, int nvec, cudaStream_t st) {
+    if (nv <= 0 || ncp <= nc || nvec <= 0) return cudaSuccess;
+    dim3 grid((unsigned)std::min<int64_t>(ceil_div((int64_t)nv * (ncp - nc), 256), 1024), (unsigned)nvec);
+    k_sym_zero_pad<<<grid, 256, 0, st>>>(x, ld, nv, nc, ncp);
+    count_launch();
+    return cudaGetLastError();
+}
 
 cudaError_t launch_sym_reduce_kernel(const double* vwf, int n_w, int g, double* vg, int64_t ld, cudaStream_t st) {
     dim3 grid((unsigned)std::min<int64_t>(ceil_div(n_w, 128), 64), (unsigned)n_w);

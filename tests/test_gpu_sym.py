@@ -158,7 +158,8 @@ def test_sym_poly_mode_and_state_errors():
         a, b, n2, ln = ctx.lanczos(n_idx.size, 10, 4, 1)
         sig, _ = ctx.selfenergy(p.omega, DLT, n_idx.size)
         for bad in (lambda: ctx.casida_matvec(np.zeros((1, vs.size))), lambda: ctx.set_approximation(gwl.GWL_TDA),
-                    lambda: ctx.spectrum_bounds(10), lambda: ctx.exchange(np.array([0], dtype=np.int32))):
+                    lambda: gwl.Context.selfenergy_state(ctx, 0, 4, 4, 0, p.omega, DLT),     # the plain-context entry point
+                    lambda: gwl.Context.set_kernel(ctx, np.zeros((p.n_w, p.n_w)))):
             with pytest.raises(gwl.GwlError) as e:
                 bad()
             assert e.value.status == gwl.GWL_ESTATE
@@ -214,3 +215,42 @@ def test_sym_cluster_scale_sampled():
     # well-separated top of those blocks' spectra (1.4e-3 eV of Sigma at L = 60); inside a block it cannot arise.
     full = orc.run_chains(phi_v, phi_c, p.eps_v, p.eps_c, p.V_full, n_idx[idx[:1]], m_idx[idx[:1]], 10, p.omega, DLT, reorth=True)
     assert np.abs(sig10[0] - full["sigma"][0]).max() <= 1e-6
+
+
+def test_sym_exchange_spectrum_bounds_and_quasiparticle_state():
+    """Sigma^x (Eq. 6) through the reduced kernels against gw_oracle.exchange_eq6 on the unfolded problem; the Lanczos bounds
+    of every block against its dense spectrum (the probe vector stays off the padding pairs); then one whole quasiparticle
+    state the paper's way inside the blocks (fitting range over all blocks, p_g(C), Eq. 10 over all n, Sigma^x, E(omega) = omega)
+    against the unreduced oracle."""
+    p = synth.make_symmetric(2, [2, 2, 1, 2], [5, 4, 6, 3], 36, seed=66, n_omega=161)
+    phi_v = sym.unfold_orbitals(p.phi_v_w, p.irrep_v, p.g)
+    phi_c = sym.unfold_orbitals(p.phi_c_w, p.irrep_c, p.g)
+    n_v = phi_v.shape[1]
+    ms = np.array([0, n_v - 1, n_v + 2, n_v + 9], dtype=np.int32)
+    g_poly, L = 8, 10
+    m = n_v - 1
+    with _ctx(p) as ctx:
+        sx = ctx.exchange(ms)
+        lam_hi = 0.0
+        for gamma in range(p.g):
+            ctx.select(gamma)
+            lo_g, hi_g = ctx.spectrum_bounds(40)
+            lam = np.linalg.eigvalsh(sym.casida_block_dense(p.phi_v_w, p.phi_c_w, p.eps_v, p.eps_c, p.irrep_v, p.irrep_c, p.V_wf,
+                                                            gamma))
+            assert lam[-1] * (1 - 1e-10) <= hi_g <= 1.02 * lam[-1]
+            assert lo_g <= lam[0] * (1 + 1e-10) and lo_g >= 0.5 * lam[0]
+            lam_hi = max(lam_hi, hi_g)
+        d_min = p.eps_c.min() - p.eps_v.max()
+        lo, hi = 0.8 * d_min * d_min, 1.02 * lam_hi
+        c = polyfit.sqrt_chebyshev(g_poly, lo, hi)
+        ctx.set_polynomial(g_poly, c, lo, hi)
+        sc = ctx.selfenergy_state(m, L, 8, 1, p.omega, 0.68)
+        sxm = ctx.exchange([m])
+        e_qp, z_qp, it = ctx.qp_solve([p.eps_v[m]], [-9.0], sxm, sc[None, :], p.omega)
+    for j, mm in enumerate(ms):
+        ref = orc.exchange_eq6(phi_v, phi_c, p.V_full, int(mm))
+        assert abs(sx[j] - ref) <= 1e-12 * abs(ref)
+    ref_c = orc.sigma_state(phi_v, phi_c, p.eps_v, p.eps_c, p.V_full, m, L, p.omega, 0.68, reorth=True, poly=(c, lo, hi))
+    assert np.abs(sc - ref_c).max() <= 1e-6
+    e_ref, z_ref, _ = orc.qp_solve(p.eps_v[m], -9.0, orc.exchange_eq6(phi_v, phi_c, p.V_full, m), ref_c, p.omega)
+    assert abs(e_qp[0] - e_ref) <= 1e-6 and abs(z_qp[0] - z_ref) <= 1e-6
