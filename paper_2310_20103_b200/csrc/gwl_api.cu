@@ -69,6 +69,22 @@ struct gwl_ctx {
     int64_t sym_vecoff[8] = {}, sym_apioff[8] = {}, sym_npairs = 0;
     int64_t v_sel = 0;          // element offset of the selected kernel inside V (V holds the g reduced kernels)
     bool sig_accumulate = false;  // gwl_selfenergy adds to sigma_sum instead of overwriting it (gwl_sym_selfenergy_state)
+    // CUDA graphs of the step loop for small problems (launch-bound: the fused-update path, N_vc <= 65 536): six consecutive
+    // Lanczos steps are captured once (slot rotation has period 3, state parity period 2) and replayed; the step number comes
+    // from a device counter.  Runs on an internal stream (the caller's may be the legacy default stream, which cannot capture).
+    struct StepGraph {
+        uint64_t key = 0;
+        cudaGraphExec_t exec = nullptr;
+        int launches = 0;
+        unsigned max_epoch = 0;
+        uint64_t stamp = 0;
+    };
+    std::vector<StepGraph> graphs;
+    uint64_t graph_stamp = 0;
+    bool graph_off = false;       // set after a failed capture: plain launches from then on
+    cudaStream_t gstream = nullptr;
+    cudaEvent_t ev_gin = nullptr, ev_gout = nullptr;
+    DevBuf kbase;
     cudaStream_t stream = nullptr;
     int device_ptrs = 0;
     std::string err;
@@ -733,6 +749,16 @@ void gwl_destroy(gwl_ctx* ctx) {
     if (ctx->ev_consumed != nullptr) cudaEventDestroy(ctx->ev_consumed);
     if (ctx->ev_s1 != nullptr) cudaEventDestroy(ctx->ev_s1);
     if (ctx->stream2 != nullptr) cudaStreamDestroy(ctx->stream2);
+    for (gwl_ctx::StepGraph& g : ctx->graphs)
+        if (g.exec != nullptr) cudaGraphExecDestroy(g.exec);
+    if (ctx->ev_gin != nullptr) cudaEventDestroy(ctx->ev_gin);
+    if (ctx->ev_gout != nullptr) cudaEventDestroy(ctx->ev_gout);
+    if (ctx->gstream != nullptr) cudaStreamDestroy(ctx->gstream);
+    ctx->kbase.release();
+    ctx->sbasis.release();
+    ctx->prpa_tc.release();
+    ctx->prpa_wc.release();
+    ctx->prpa_apart.release();
     delete ctx;
 }
 
@@ -1032,15 +1058,8 @@ gwl_status gwl_set_start_vectors(gwl_ctx* ctx, int64_t n_chains, const double* p
     return GWL_OK;
 }
 
-gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t block, int reorth, double* alpha,
-                       double* beta, double* norm2, int32_t* len) {
-    if (ctx == nullptr) return GWL_EINVAL;
-    DeviceGuard dg(ctx);
-    if (n_chains < 0 || steps < 1 || steps > 100000 || block < 1 || (reorth != 0 && reorth != 1))
-        return ctx->fail(GWL_EINVAL, "gwl_lanczos: bad arguments");
-    if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_lanczos: orbitals, energies and kernel must be set");
-    if (ctx->chain_mode == 0) return ctx->fail(GWL_ESTATE, "gwl_lanczos: no chains set");
-    if (n_chains > ctx->n_chains_set) return ctx->fail(GWL_EINVAL, "gwl_lanczos: more chains than were set");
+static gwl_status lanczos_impl(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t block, int reorth, double* alpha,
+                               double* beta, double* norm2, int32_t* len, bool graph_active) {
     LaunchScope ls(ctx);
     cudaStream_t st = ctx->stream;
     const int L = (int)steps;
@@ -1160,7 +1179,9 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
         }
 
         // ---- S2-S4: the step loop; nothing below touches the host ----
-        for (int k = 0; k < L; ++k) {
+        // One Lanczos step.  k selects the vector slots (period 3) and the state parity (period 2); the fused update gets
+        // k_arg and adds the device step counter Sk.kbase when that is set (graph replay, below).
+        auto enqueue_step = [&](int k, int k_arg, const LanczosState& Sk) -> gwl_status {
             double* q = slot(k);
             double* w = slot(k + 1);
             const double* qp = k > 0 ? slot(k - 1) : nullptr;
@@ -1214,12 +1235,12 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
             }
             if (tstep) CK(cudaEventRecord(e1, st));
             if (!reorth && lanczos_fused_fits(n_vc)) {
-                CKL(5, launch_lanczos_fused(w, q, qp, n_vc, nb, dotpart, ndot, dstride, S, k, ctx->xs.as<double>(), ldxs,
+                CKL(5, launch_lanczos_fused(w, q, qp, n_vc, nb, dotpart, ndot, dstride, Sk, k_arg, ctx->xs.as<double>(), ldxs,
                                         ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
                 if (tstep) CK(cudaEventRecord(e2, st));
-                continue;
+                return GWL_OK;
             }
-            CKL(5, launch_lanczos_update1(w, q, qp, n_vc, nb, dotpart, ndot, dstride, S, k, normpart, npart, st));
+            CKL(5, launch_lanczos_update1(w, q, qp, n_vc, nb, dotpart, ndot, dstride, Sk, k, normpart, npart, st));
             if (reorth) {
                 for (int pass = 0; pass < 2; ++pass) {
                     if (ctx->cplx) {  // complex projection coefficients <q_j, w>
@@ -1235,9 +1256,99 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
                                            pass == 1 ? normpart : nullptr, st));
                 }
             }
-            CKL(5, launch_lanczos_update2(w, n_vc, nb, normpart, reorth ? rparts : npart, S, k, ctx->xs.as<double>(), ldxs,
+            CKL(5, launch_lanczos_update2(w, n_vc, nb, normpart, reorth ? rparts : npart, Sk, k, ctx->xs.as<double>(), ldxs,
                                       ctx->s.as<double>(), ctx->n_v, ctx->n_c, ctx->n_cp, st));
             if (tstep) CK(cudaEventRecord(e2, st));
+            return GWL_OK;
+        };
+
+        int k = 0;
+        // Launch-bound sizes (fused-update path): after a few plain steps, which also size every workspace, the rest of the
+        // chain is replayed from a CUDA graph of six steps.
+        if (graph_active && !ctx->graph_off && ctx->prof_level == 0 && !reorth && !ctx->cplx && lanczos_fused_fits(n_vc) &&
+            L >= 16) {
+            const int pfx = ((L - 2) % 6) + 2;  // 2..7, (L - pfx) % 6 == 0
+            for (; k < pfx; ++k) {
+                gwl_status rs = enqueue_step(k, k, S);
+                if (rs != GWL_OK) return rs;
+            }
+            // everything a replay depends on that is not reached through one of the hashed pointers
+            uint64_t key = 1469598103934665603ull;
+            auto mix = [&key](uint64_t v) {
+                key ^= v;
+                key *= 1099511628211ull;
+            };
+            const void* ptrs[] = {basis, ctx->xs.p, dotpart, S.alpha, S.beta, S.norm2, S.len, S.scale, S.alive, ctx->ws().T.p,
+                                  ctx->ws().W.p, ctx->ws().part.p, ctx->ws().sk_ws.p, ctx->ws().sk_flags.p, ctx->phi_c.p,
+                                  ctx->phi_cT.p, ctx->phi_vT.p, ctx->V.p, ctx->d2.p, ctx->s.p, ctx->tA.p, ctx->tB.p};
+            for (const void* q : ptrs) mix((uint64_t)(uintptr_t)q);
+            const int64_t ints[] = {nb, L, pfx, ctx->g, ctx->approx, n_vc, ctx->n_v, ctx->n_c, ctx->n_mu, ctx->v_sel,
+                                    ctx->sym ? ctx->sym_gamma : -1};
+            for (int64_t v : ints) mix((uint64_t)v);
+            auto mixd = [&mix](double d) {
+                uint64_t u;
+                std::memcpy(&u, &d, 8);
+                mix(u);
+            };
+            mixd(ctx->lo);
+            mixd(ctx->hi);
+            for (double c : ctx->cheb) mixd(c);
+            gwl_ctx::StepGraph* sg = nullptr;
+            for (gwl_ctx::StepGraph& g : ctx->graphs)
+                if (g.key == key && g.exec != nullptr) sg = &g;
+            if (sg == nullptr) {
+                CK(ctx->kbase.ensure(4, st));
+                gwl_ctx::StepGraph ng;
+                ng.key = key;
+                const unsigned epoch_saved = ctx->ws().sk_epoch;
+                const int64_t launches_before = ctx->launches;
+                cudaGraph_t graph = nullptr;
+                bool ok = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+                if (ok) {
+                    // the stream-K hand-over flags start from zero in every replay, the epochs of the captured launches from 1
+                    ok = cudaMemsetAsync(ctx->ws().sk_flags.p, 0, ctx->ws().sk_flags.bytes, st) == cudaSuccess;
+                    ctx->ws().sk_epoch = 0;
+                    LanczosState Sg = S;
+                    Sg.kbase = ctx->kbase.as<int>();
+                    for (int i = 0; i < 6 && ok; ++i) ok = enqueue_step(pfx + i, i, Sg) == GWL_OK;
+                    if (ok) ok = launch_add_int(ctx->kbase.as<int>(), 6, st) == cudaSuccess;
+                    const cudaError_t ee = cudaStreamEndCapture(st, &graph);
+                    ok = ok && ee == cudaSuccess && graph != nullptr;
+                    ng.max_epoch = ctx->ws().sk_epoch;
+                    ctx->ws().sk_epoch = std::max(epoch_saved, ng.max_epoch);
+                }
+                if (ok) ok = cudaGraphInstantiate(&ng.exec, graph, 0) == cudaSuccess;
+                if (graph != nullptr) cudaGraphDestroy(graph);
+                ng.launches = (int)(ctx->launches - launches_before);
+                ctx->launches = launches_before;  // captured, not launched
+                if (!ok) {  // no graphs on this stream / driver: plain launches from here on
+                    cudaGetLastError();
+                    ctx->graph_off = true;
+                } else {
+                    if (ctx->graphs.size() >= 8) {  // evict the least recently used
+                        size_t old = 0;
+                        for (size_t i = 1; i < ctx->graphs.size(); ++i)
+                            if (ctx->graphs[i].stamp < ctx->graphs[old].stamp) old = i;
+                        cudaGraphExecDestroy(ctx->graphs[old].exec);
+                        ctx->graphs.erase(ctx->graphs.begin() + old);
+                    }
+                    ctx->graphs.push_back(ng);
+                    sg = &ctx->graphs.back();
+                }
+            }
+            if (sg != nullptr) {
+                sg->stamp = ++ctx->graph_stamp;
+                ctx->ws().sk_epoch = std::max(ctx->ws().sk_epoch, sg->max_epoch);  // later plain launches: epochs the flags cannot hold
+                CK(launch_set_int(ctx->kbase.as<int>(), pfx, st));
+                for (; k < L; k += 6) {
+                    CK(cudaGraphLaunch(sg->exec, st));
+                    ctx->launches += sg->launches;
+                }
+            }
+        }
+        for (; k < L; ++k) {
+            gwl_status rs = enqueue_step(k, k, S);
+            if (rs != GWL_OK) return rs;
         }
     }
     ctx->run_chains = n_chains;
@@ -1252,6 +1363,36 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
     }
     if (!ctx->device_ptrs) CK(cudaStreamSynchronize(st));
     return GWL_OK;
+}
+
+gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t block, int reorth, double* alpha,
+                       double* beta, double* norm2, int32_t* len) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (n_chains < 0 || steps < 1 || steps > 100000 || block < 1 || (reorth != 0 && reorth != 1))
+        return ctx->fail(GWL_EINVAL, "gwl_lanczos: bad arguments");
+    if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_lanczos: orbitals, energies and kernel must be set");
+    if (ctx->chain_mode == 0) return ctx->fail(GWL_ESTATE, "gwl_lanczos: no chains set");
+    if (n_chains > ctx->n_chains_set) return ctx->fail(GWL_EINVAL, "gwl_lanczos: more chains than were set");
+    // Step graphs (small problems, no profiling events, no reorthogonalisation): the whole call runs on an internal stream
+    // fenced against the caller's stream on both sides, because the caller's stream may be the legacy default stream.
+    static const bool graphs_allowed = std::getenv("GWL_NO_GRAPH") == nullptr;
+    const bool want_graph = graphs_allowed && !ctx->graph_off && ctx->prof_level == 0 && reorth == 0 && !ctx->cplx && steps >= 16 &&
+                            n_chains > 0 && lanczos_fused_fits(ctx->n_vc);
+    if (!want_graph) return lanczos_impl(ctx, n_chains, steps, block, reorth, alpha, beta, norm2, len, false);
+    if (ctx->gstream == nullptr) {
+        CK(cudaStreamCreateWithFlags(&ctx->gstream, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&ctx->ev_gin, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&ctx->ev_gout, cudaEventDisableTiming));
+    }
+    cudaStream_t user = ctx->stream;
+    CK(cudaEventRecord(ctx->ev_gin, user));
+    CK(cudaStreamWaitEvent(ctx->gstream, ctx->ev_gin, 0));
+    ctx->stream = ctx->gstream;
+    const gwl_status rs = lanczos_impl(ctx, n_chains, steps, block, reorth, alpha, beta, norm2, len, true);
+    ctx->stream = user;
+    if (cudaEventRecord(ctx->ev_gout, ctx->gstream) == cudaSuccess) cudaStreamWaitEvent(user, ctx->ev_gout, 0);
+    return rs;
 }
 
 gwl_status gwl_resolvent(gwl_ctx* ctx, const double* zeta, int64_t n_zeta, double* r) {
@@ -1432,7 +1573,11 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
         CK(ctx->x_sig.ensure((size_t)n_states * 8, st));
         dout = ctx->x_sig.as<double>();
     }
-    const int64_t v_sel_saved = ctx->v_sel;
+    struct RestoreKernel {  // whatever path leaves this function, the V GEMM points at the selected block's kernel again
+        gwl_ctx* c;
+        int64_t saved;
+        ~RestoreKernel() { c->v_sel = saved; }
+    } restore_kernel{ctx, ctx->v_sel};
     const int n_seg = ctx->sym ? ctx->sym_g : 1;
     for (int64_t j = 0; j < n_states; ++j) {
         bool first = true;
@@ -1447,10 +1592,7 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
                                   ctx->x_nidx.as<int32_t>() + off, ctx->x_midx.as<int32_t>() + off, ctx->ws().T.as<double>(), ldm, nb,
                                   st));
                 rs = gemm_v(ctx, nb);
-                if (rs != GWL_OK) {
-                    ctx->v_sel = v_sel_saved;
-                    return rs;
-                }
+                if (rs != GWL_OK) return rs;
                 CKL(4, launch_dot_partials(ctx->ws().T.as<double>(), ctx->ws().W.as<double>(), ldm, ctx->n_mu, nb,
                                            ctx->x_part.as<double>(), npart, st));
                 CKL(4, launch_accum_neg(ctx->x_part.as<double>(), nb * npart, dout + j, first ? 1 : 0, st));
@@ -1458,7 +1600,6 @@ gwl_status gwl_exchange(gwl_ctx* ctx, int64_t n_states, const int32_t* m_idx, do
             }
         }
     }
-    ctx->v_sel = v_sel_saved;
     if (!ctx->device_ptrs) {
         CK(cudaMemcpyAsync(sigma_x, dout, (size_t)n_states * 8, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));

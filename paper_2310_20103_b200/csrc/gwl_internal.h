@@ -167,7 +167,11 @@ struct LanczosState {       // device arrays, one entry per chain of the current
     double* scale;          // [nb] running max(|a|+b)
     int32_t* alive;         // [nb]
     int steps;
+    const int* kbase = nullptr;  // device step counter added to the kernel's step argument (CUDA-graph replay), or NULL
 };
+// *p = v / *p += d (one thread): the step counter of the graph replay
+cudaError_t launch_set_int(int* p, int v, cudaStream_t st);
+cudaError_t launch_add_int(int* p, int d, cudaStream_t st);
 // q0 = p/||p|| in place, xs = s o q0; norm2 from partials; dead if norm2 == 0.
 cudaError_t launch_lanczos_init(double* p, int64_t n_vc, int nb, const double* normpart, int npart, LanczosState st_,
                                 double* xs, int64_t ldxs, const double* s, int n_v, int n_c, int n_cp,

@@ -269,10 +269,11 @@ template <int EPT>
 __global__ void __launch_bounds__(NT) k_lanczos_fused(double* __restrict__ w, const double* __restrict__ q,
                                                       const double* __restrict__ q_prev, int64_t n_vc, int nb,
                                                       const double* __restrict__ dotpart, int ndot, int dot_stride,
-                                                      LanczosState st, int k, double* __restrict__ xs, int64_t ldxs,
+                                                      LanczosState st, int k_arg, double* __restrict__ xs, int64_t ldxs,
                                                       const double* __restrict__ s, int n_c, int n_cp) {
     pdl_trigger();
     pdl_wait();
+    const int k = k_arg + (st.kbase != nullptr ? *st.kbase : 0);  // graph replay: the step number lives on the device
     __shared__ double sh[NT / 32 + 1];
     __shared__ double cl_part;  // this CTA's partial of ||w||^2; read by the other CTAs of the cluster
     __shared__ double cl_sum;
@@ -626,6 +627,18 @@ __global__ void k_build_delta_c(const double* __restrict__ eps_v, const double* 
 }
 
 // x[i] = uniform in [-1, 1) from a counter-based hash (splitmix64 finaliser) of (seed, i): a generic start vector
+__global__ void k_set_int(int* p, int v) {
+    pdl_trigger();
+    pdl_wait();
+    *p = v;
+}
+
+__global__ void k_add_int(int* p, int d) {
+    pdl_trigger();
+    pdl_wait();
+    *p += d;
+}
+
 __global__ void k_fill_hash(double* __restrict__ x, int64_t n, unsigned long long seed) {
     for (int64_t i = blockIdx.x * (int64_t)NT + threadIdx.x; i < n; i += (int64_t)gridDim.x * NT) {
         unsigned long long z = seed + 0x9E3779B97F4A7C15ull * (unsigned long long)(i + 1);
@@ -688,6 +701,18 @@ cudaError_t launch_build_delta_c(const double* eps_v, const double* eps_cq, int 
     k_build_delta_c<<<grid1d((int64_t)n_k * n_v * n_c, 1), NT, 0, st>>>(eps_v, eps_cq, n_k, n_v, n_c, d2, s);
     count_launch();
     return cudaGetLastError();
+}
+
+cudaError_t launch_set_int(int* p, int v, cudaStream_t st) {
+    cudaError_t e = launch_pdl(k_set_int, dim3(1), dim3(1), 0, st, 1u, p, v);
+    count_launch();
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+cudaError_t launch_add_int(int* p, int d, cudaStream_t st) {
+    cudaError_t e = launch_pdl(k_add_int, dim3(1), dim3(1), 0, st, 1u, p, d);
+    count_launch();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t launch_fill_hash(double* x, int64_t n, unsigned long long seed, cudaStream_t st) {

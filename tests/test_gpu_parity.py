@@ -549,6 +549,44 @@ def test_runs_are_bitwise_repeatable(p1):
     assert np.array_equal(ys[0], ys[1]) and np.array_equal(ys[0], ys[2])
 
 
+def test_step_graph_replay_is_bitwise_identical(p0, p1):
+    """Small problems (fused-update path) replay the step loop from a CUDA graph of six steps when no per-step events are
+    recorded (profiling level 0): same kernels, same order, same arguments apart from the device-resident step counter, so
+    alpha, beta, <P|P>, len and Sigma are IDENTICAL to the plain launches -- in direct mode, in poly mode, for several
+    blocks, for chain lengths with every remainder mod 6, on a cache hit and after switching back to plain launches
+    (the stream-K epochs of captured launches restart in every replay).  The launch count shows that the graph ran."""
+    from paper_2310_20103_b200 import polyfit
+    for prob, L0 in ((p0, 60), (p1, 40)):
+        cfg = prob.cfg
+        nch = cfg.n_chains
+        with _ctx(prob) as ctx:
+            for (L, blk, poly) in ((L0, cfg.block, False), (L0 + 1, cfg.block, False), (L0 + 3, max(2, cfg.block // 2), False),
+                                   (18, cfg.block, True)):
+                if poly:
+                    lo, hi = polyfit.range_from_spectrum(ctx, prob.eps_v, prob.eps_c, steps=20)
+                    ctx.set_polynomial(6, polyfit.sqrt_chebyshev(6, lo, hi), lo, hi)
+                    ctx.set_chains(prob.n_idx, prob.m_idx)
+                ctx.set_profiling(1)
+                n0 = ctx.get_launch_count()
+                ref = ctx.lanczos(nch, L, blk, 0)
+                sig_ref, _ = ctx.selfenergy(prob.omega, DLT, nch)
+                n_plain = ctx.get_launch_count() - n0
+                ctx.set_profiling(0)
+                for rep in range(2):                                      # capture, then cache hit
+                    n0 = ctx.get_launch_count()
+                    out = ctx.lanczos(nch, L, blk, 0)
+                    sig, _ = ctx.selfenergy(prob.omega, DLT, nch)
+                    n_graph = ctx.get_launch_count() - n0
+                    assert all(np.array_equal(x, y) for x, y in zip(out, ref)), (cfg.name, L, blk, poly, rep)
+                    assert np.array_equal(sig, sig_ref)
+                    pfx = (L - 2) % 6 + 2
+                    n_blocks = -(-nch // blk)
+                    assert n_graph == n_plain + n_blocks * (1 + (L - pfx) // 6)   # set_int + one add_int per replay
+                ctx.set_profiling(1)
+                again = ctx.lanczos(nch, L, blk, 0)                       # plain launches after the replays
+                assert all(np.array_equal(x, y) for x, y in zip(again, ref))
+
+
 def test_chain_sharded_state_on_one_gpu(p0):
     """SURVEY.md §8(f)-2 on the GPU path: the slices two ranks would take (runtime.shard_range), run one after the
     other on this GPU through runtime.gwl_local_sigma_sum, add up to gwl_selfenergy_state; a single process
