@@ -52,6 +52,7 @@ def parse():
                     help="context run, not the bench line: the complex-orbital Tamm-Dancoff variant (SURVEY 8(f)-3) on a "
                          "synthetic periodic problem of that shape, e.g. 4,64,1024,6144; block = --chains (default 128), "
                          "L = --lanczos-steps (default 10)")
+    ap.add_argument("--block", type=int, default=0, help="with --paper-setting: chains per block (default 256)")
     ap.add_argument("--rpa", action="store_true",
                     help="with --tdc: the full RPA for complex orbitals (pseudo-Hermitian Lanczos on C^RPA(q), PAPER.md:159): every "
                          "chain is a pair [x; y] = two GEMM columns, one product with Omega^ per step")
@@ -185,7 +186,7 @@ def run_paper_setting(args):
     from paper_2310_20103_b200 import gwl, polyfit, synth
 
     n_v, n_c, n_mu = (int(x) for x in args.paper_setting.split(","))
-    g, n_iter, block = 7, 8, 256
+    g, n_iter, block = 7, 8, (args.block or 256)
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
     gwl.load_library()

@@ -181,6 +181,23 @@ def sigma_chain_rpa(alpha, beta, norm2, length, omega, eps_n, sgn_n, dlt, prefac
     return prefactor * norm2 * out
 
 
+def resolvent_chain(alpha, beta, norm2, length, zeta):
+    """<u|(zeta - H)^{-1}|u>_O by Eq. 14 on the tridiagonal of lanczos_pseudo_hermitian: both branches +-Omega_s."""
+    return tdp.continued_fraction(alpha, beta, norm2, zeta, length)
+
+
+def resolvent_exact_rpa(A, B, u1, u2, zeta):
+    """The same matrix element by dense solves: u^H Omega^ (zeta - F Omega^)^{-1} u."""
+    n = A.shape[0]
+    Oh = omega_hat_dense(A, B)
+    H = tdp.casida_rpa_block(A, B)
+    u = np.concatenate([u1, u2])
+    out = np.zeros(len(zeta), dtype=np.complex128)
+    for i, z in enumerate(np.asarray(zeta, dtype=np.complex128)):
+        out[i] = np.vdot(u, Oh @ np.linalg.solve(z * np.eye(2 * n) - H, u))
+    return out
+
+
 def run_chains_rpa(psi_v, psi_cq, eps_v, eps_cq, V, chains, steps, omega, dlt, n_q=1, reorth=False):
     """S1-S7 for chains [(kn, n_idx, km, m_idx), ...] in the RPA with complex orbitals."""
     delta = tdp.delta_kvc(eps_v, eps_cq)

@@ -172,3 +172,25 @@ def test_prpa_cluster_scale_sampled():
     assert np.abs(ar - r1["alpha"]).max() <= 1e-9 * bs
     assert (np.abs(br - r1["beta"]) <= 1e-9 * np.abs(r1["beta"])).all()
     assert np.abs(sig - r1["sigma"]).max() <= 1e-6
+
+
+def test_prpa_resolvent_against_oracle_and_dense_solve():
+    """gwl_resolvent on a complex-RPA run: <u|(zeta - C^RPA)^-1|u>_O by Eq. 14, against the oracle's continued fraction at the
+    same length and, at full length, against the dense solve u^H Omega^ (zeta - F Omega^)^-1 u."""
+    p = synth.make_periodic(2, 2, 5, 20, seed=12, n_chains=3)
+    zeta = np.array([3.0 + 0.5j, -7.0 + 0.2j, 0.1j, 25.0 - 1.0j])
+    delta = tdp.delta_kvc(p.eps_v, p.eps_cq)
+    K = tdp.pair_matrix(p.psi_v, p.psi_cq)
+    A, B = tdp.tda_dense(delta, K, p.V), tdp.coupling_B(K, p.V)
+    with _ctx(p) as ctx:
+        ctx.lanczos(3, 12, 3, 1)
+        r12 = ctx.resolvent(zeta, 3)
+        ctx.lanczos(3, 2 * p.n_kvc, 3, 1)
+        rfull = ctx.resolvent(zeta, 3)
+    ref = rpa.run_chains_rpa(p.psi_v, p.psi_cq, p.eps_v, p.eps_cq, p.V, p.chains, 12, p.omega, DLT, reorth=True)
+    for j, (kn, n_idx, km, m_idx) in enumerate(p.chains):
+        cf = rpa.resolvent_chain(ref["alpha"][j], ref["beta"][j], ref["norm2"][j], ref["len"][j], zeta)
+        assert np.abs(r12[j] - cf).max() <= 1e-9 * np.abs(cf).max()
+        u1, u2 = rpa.start_vector_rpa(*rpa.printed_elements(p.psi_v, p.psi_cq, p.V, kn, n_idx, km, m_idx))
+        ex = rpa.resolvent_exact_rpa(A, B, u1, u2, zeta)
+        assert np.abs(rfull[j] - ex).max() <= 1e-8 * np.abs(ex).max()

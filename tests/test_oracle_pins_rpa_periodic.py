@@ -220,3 +220,28 @@ def test_short_lanczos_converges_towards_the_pole_sum():
         r = rpa.run_chains_rpa(p.psi_v, p.psi_cq, p.eps_v, p.eps_cq, p.V, p.chains[:1], L, p.omega, 0.5, n_q=1, reorth=True)
         errs.append(np.abs(r["sigma"][0] - exact).max())
     assert errs[1] < 0.2 * errs[0]
+
+
+def test_resolvent_of_the_pseudo_hermitian_matrix_by_eq14():
+    """<u|(zeta - H)^-1|u>_O: the continued fraction of the full-length tridiagonal equals the dense solve, and its partial
+    fractions carry BOTH branches: sum_s |lambda_s| |d^H v_s|^2 / (zeta - lambda_s) over +Omega_s (v = [X; Y]) and -Omega_s
+    (v = [Y^*; X^*])."""
+    p = synth.make_periodic(2, 2, 3, 10, seed=31)
+    delta, K, A, B = _dense(p)
+    n = delta.size
+    Oh = rpa.omega_hat_dense(A, B)
+    P1, P2 = rpa.printed_elements(p.psi_v, p.psi_cq, p.V, 0, 0, 0, 1)
+    u1, u2 = rpa.start_vector_rpa(P1, P2)
+    a, b, n2, ln = rpa.lanczos_pseudo_hermitian(lambda x, y: tuple(np.split(Oh @ np.concatenate([x, y]), 2)), u1, u2, 2 * n,
+                                                reorth=True)
+    zeta = np.array([3.0 + 0.5j, -7.0 + 0.2j, 0.1j, 25.0 - 1.0j])
+    cf = rpa.resolvent_chain(a, b, n2, ln, zeta)
+    ex = rpa.resolvent_exact_rpa(A, B, u1, u2, zeta)
+    assert np.abs(cf - ex).max() <= 1e-9 * np.abs(ex).max()
+    om, X, Y = rpa.rpa_eig(A, B)
+    d = np.conj(np.concatenate([P1, P2]))
+    wp = np.abs(d.conj() @ np.concatenate([X, Y], axis=0)) ** 2
+    wm = np.abs(d.conj() @ np.concatenate([Y.conj(), X.conj()], axis=0)) ** 2
+    pf = (om[None, :] * wp[None, :] / (zeta[:, None] - om[None, :])).sum(axis=1) \
+        + (om[None, :] * wm[None, :] / (zeta[:, None] + om[None, :])).sum(axis=1)
+    assert np.abs(pf - ex).max() <= 1e-9 * np.abs(ex).max()
