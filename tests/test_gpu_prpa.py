@@ -194,3 +194,35 @@ def test_prpa_resolvent_against_oracle_and_dense_solve():
         u1, u2 = rpa.start_vector_rpa(*rpa.printed_elements(p.psi_v, p.psi_cq, p.V, kn, n_idx, km, m_idx))
         ex = rpa.resolvent_exact_rpa(A, B, u1, u2, zeta)
         assert np.abs(rfull[j] - ex).max() <= 1e-8 * np.abs(ex).max()
+
+
+def test_complex_config2_scale_sampled():
+    """262 144 complex pairs (N_k = 4, N_v = 64, N_c = 1024, N_mu = 6144: the shape of `bench.py --tdc 4,64,1024,6144`), 64 chain
+    pairs = 128 GEMM columns on the GPU in the launch configuration that arm times; the oracle (about 15 s per product with
+    Omega^ at this size) follows one sampled pair of the product, of A(q) x in the Tamm-Dancoff operator, and the leading steps of
+    one sampled chain of the pseudo-Hermitian Lanczos."""
+    p = synth.make_periodic(4, 64, 1024, 6144, box=20.0, seed=0, n_chains=64, n_omega=101)
+    delta = tdp.delta_kvc(p.eps_v, p.eps_cq)
+    X = synth.random_complex_block(p.n_kvc, 64, seed=3)
+    Y = synth.random_complex_block(p.n_kvc, 64, seed=4)
+    idx = np.array([37])
+    j = np.array([21])
+    L = 3
+    with _ctx(p) as ctx:
+        ox, oy = ctx.matvec_rpa(X, Y)
+        a, b, n2, ln = ctx.lanczos(64, L, 64, 0)
+        sig, _ = ctx.selfenergy(p.omega, DLT, 64)
+        ctx.set_approximation(gwl.GWL_TDA)
+        Ax = ctx.matvec(X)
+    rx, ry = rpa.omega_hat_factored(p.psi_v, p.psi_cq, p.V, delta, X[idx], Y[idx])
+    scale = max(np.abs(rx).max(), np.abs(ry).max())
+    assert np.abs(ox[idx] - rx).max() <= 1e-12 * scale and np.abs(oy[idx] - ry).max() <= 1e-12 * scale
+    # A x is the upper half of Omega^ [x; 0]: by linearity rx = A x + B y, so compare A x with rx - B y through a second product
+    zx, _ = rpa.omega_hat_factored(p.psi_v, p.psi_cq, p.V, delta, X[idx], np.zeros_like(Y[idx]))
+    assert _relmax(Ax[idx], zx) <= 1e-12
+    r0 = rpa.run_chains_rpa(p.psi_v, p.psi_cq, p.eps_v, p.eps_cq, p.V, p.chains[j], L, p.omega, DLT, reorth=False)
+    bs = np.abs(r0["beta"]).max()
+    assert abs(n2[j[0]] - r0["norm2"][0]) <= 1e-12 * r0["norm2"][0]
+    assert np.abs(a[j] - r0["alpha"]).max() <= 1e-9 * bs
+    assert (np.abs(b[j] - r0["beta"]) <= 1e-9 * np.abs(r0["beta"])).all()
+    assert np.abs(sig[j] - r0["sigma"]).max() <= 1e-6
