@@ -273,8 +273,16 @@ class SymmetricProblem:
 
     @property
     def V_wf(self) -> np.ndarray:
-        """[n_w][g][n_w]: rows of V_full for the wedge points against every image, V(r_mu, h r_nu) (a slice, no arithmetic)."""
-        return np.ascontiguousarray(self.V_full[:self.n_w].reshape(self.n_w, self.g, self.n_w))
+        """[n_w][g][n_w]: rows of V_full for the wedge points against every image, V(r_mu, h r_nu): the same kernel formula
+        evaluated for those rows only (the full g n_w x g n_w matrix is not needed to feed the library)."""
+        if self._V is not None:
+            rows = self._V[:self.n_w]
+        else:
+            rows = np.empty((self.n_w, self.g * self.n_w))
+            for i in range(0, self.n_w, 1024):
+                d = self.r_w[i:i + 1024, None, :] - self.r_full[None, :, :]
+                rows[i:i + 1024] = 14.4 / np.sqrt(np.einsum("ijk,ijk->ij", d, d) + 0.25)
+        return np.ascontiguousarray(rows.reshape(self.n_w, self.g, self.n_w))
 
 
 def make_symmetric(n_refl: int, nv_irrep, nc_irrep, n_w: int, box: float = 12.0, seed: int = 0,

@@ -254,3 +254,35 @@ def test_sym_exchange_spectrum_bounds_and_quasiparticle_state():
     assert np.abs(sc - ref_c).max() <= 1e-6
     e_ref, z_ref, _ = orc.qp_solve(p.eps_v[m], -9.0, orc.exchange_eq6(phi_v, phi_c, p.V_full, m), ref_c, p.omega)
     assert abs(e_qp[0] - e_ref) <= 1e-6 and abs(z_qp[0] - z_ref) <= 1e-6
+
+
+def test_sym_config4_scale_sampled():
+    """The sizes of BASELINE.json:configs[4] with a group of order 8 (the shape of `bench.py --sym 3`: N_v = 1024, N_c = 4096,
+    wedge of 2560 of the 20 480 points, 524 288 pairs per block), one block of 128 chains on the GPU in the launch configuration
+    that arm times; the oracle follows sampled columns of the block product and one sampled chain (no reorthogonalisation:
+    inside a block two correct FP64 runs stay together)."""
+    p = synth.make_symmetric(3, [128] * 8, [512] * 8, 2560, box=40.0, seed=0, n_omega=101)
+    gamma, m = 1, 0
+    irr = np.concatenate([p.irrep_v, p.irrep_c])
+    n_idx = np.array([n for n in range(irr.size) if irr[n] ^ irr[m] == gamma][:128], dtype=np.int32)
+    m_idx = np.full(128, m, dtype=np.int32)
+    cols = np.array([5, 127])
+    j = np.array([77])
+    L = 10
+    with _ctx(p) as ctx:
+        n_pairs = ctx.select(gamma)
+        assert n_pairs == 8 * 128 * 512
+        X = np.random.default_rng(9).standard_normal((128, n_pairs))
+        Y = ctx.matvec(X)
+        ctx.set_chains(n_idx, m_idx)
+        a, b, n2, ln = ctx.lanczos(128, L, 128, 0)
+        sig, _ = ctx.selfenergy(p.omega, DLT, 128)
+    V_wf = p.V_wf
+    ref = sym.block_matvec(p.phi_v_w, p.phi_c_w, p.eps_v, p.eps_c, p.irrep_v, p.irrep_c, V_wf, gamma, X[cols])
+    assert np.abs(Y[cols] - ref).max() <= 1e-12 * np.abs(ref).max()
+    r0 = sym.run_chains_sym(p.phi_v_w, p.phi_c_w, p.eps_v, p.eps_c, p.irrep_v, p.irrep_c, V_wf, n_idx[j], m_idx[j], L, p.omega, DLT,
+                            reorth=False)
+    assert abs(n2[j[0]] - r0["norm2"][0]) <= 1e-12 * r0["norm2"][0]
+    assert (np.abs(a[j] - r0["alpha"]) <= 1e-9 * np.abs(r0["alpha"])).all()
+    assert (np.abs(b[j] - r0["beta"]) <= 1e-9 * np.abs(r0["beta"])).all()
+    assert np.abs(sig[j] - r0["sigma"]).max() <= 1e-6

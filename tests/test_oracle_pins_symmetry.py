@@ -71,6 +71,8 @@ def test_group_facts():
     for gamma in range(p.g):
         Vg = sym.reduced_kernel(p.V_wf, gamma)
         assert np.abs(Vg - Vg.T).max() <= 1e-12 * np.abs(Vg).max()
+    p2 = synth.make_symmetric(2, [1, 1, 1, 1], [1, 1, 1, 1], 5, seed=44)          # wedge rows computed without the full matrix
+    assert np.array_equal(p2.V_wf, p.V_full[:n_w].reshape(n_w, p.g, n_w))
     p1 = synth.make_symmetric(0, [2], [3], 6, seed=45)
     assert np.array_equal(sym.reduced_kernel(p1.V_wf, 0), p1.V_full)
 
