@@ -286,3 +286,32 @@ def test_sym_config4_scale_sampled():
     assert (np.abs(a[j] - r0["alpha"]) <= 1e-9 * np.abs(r0["alpha"])).all()
     assert (np.abs(b[j] - r0["beta"]) <= 1e-9 * np.abs(r0["beta"])).all()
     assert np.abs(sig[j] - r0["sigma"]).max() <= 1e-6
+
+
+def test_sym_device_pointer_mode_and_empty_chain_list():
+    """Device-pointer mode of gwl_sym_matvec and gwl_sym_selfenergy_state (what bench.py uses) gives the bits of the host-pointer
+    calls; an empty chain list is accepted."""
+    import torch
+    p = synth.make_symmetric(2, [3, 2, 2, 1], [6, 5, 9, 4], 40, seed=67, n_omega=61)
+    gamma, m = 2, 1
+    with _ctx(p) as ctx:
+        n_pairs = ctx.select(gamma)
+        X = np.random.default_rng(1).standard_normal((3, n_pairs))
+        Y = ctx.matvec(X)
+        s_host = ctx.selfenergy_state(m, 10, 4, 0, p.omega, DLT)
+        ctx.select(gamma)
+        ctx.set_chains(np.zeros(0, dtype=np.int32), np.zeros(0, dtype=np.int32))
+        a, b, n2, ln = ctx.lanczos(0, 5, 4, 0)
+        assert a.shape == (0, 5)
+        ctx.set_pointer_mode(1)
+        ctx.set_stream(torch.cuda.current_stream().cuda_stream)
+        xd = torch.from_numpy(X).cuda()
+        yd = torch.empty_like(xd)
+        ctx.matvec(xd, yd)
+        om = torch.from_numpy(p.omega).cuda()
+        sd = torch.empty(len(p.omega), 2, dtype=torch.float64, device="cuda")
+        ctx.selfenergy_state(m, 10, 4, 0, om, DLT, out=sd)
+        torch.cuda.synchronize()
+    assert np.array_equal(yd.cpu().numpy(), Y)
+    sdev = sd.cpu().numpy()
+    assert np.array_equal(sdev[:, 0] + 1j * sdev[:, 1], s_host)
