@@ -204,6 +204,13 @@ gwl_status gwl_tdc_matvec(gwl_ctx* ctx, const double* x, double* y, int64_t nvec
  * vectors, each [nvec][n_k][n_v][n_c][2] (pointer mode applies); inputs and outputs must not overlap.  Either approximation. */
 gwl_status gwl_tdc_matvec_rpa(gwl_ctx* ctx, const double* x, const double* y, double* ox, double* oy, int64_t nvec);
 
+/* The q-term of Sigma^corr_{mk,mk}(omega) (PAPER.md:288 / :310) summed over ALL n = 0 .. n_v+n_c-1 of slot kn (the orbitals of
+ * momentum k-q): one chain per n from (n kn, m km), in the context's approximation (GWL_TDA or GWL_RPA), prefactor 2/(N_q N_k)
+ * included; the sum over q is the caller's (one context per q).  Equivalent to gwl_tdc_set_chains(all n) + gwl_lanczos +
+ * gwl_selfenergy(sum only) and leaves the context in that state.  omega [n_omega], sigma_mm [n_omega][2] (pointer mode applies). */
+gwl_status gwl_tdc_selfenergy_state(gwl_ctx* ctx, int32_t kn, int32_t km, int32_t m_idx, int64_t steps, int64_t block, int reorth,
+                                    const double* omega, int64_t n_omega, double eta, double* sigma_mm);
+
 /* ---- interpolative separable density fitting front end -------------------------------------------
  * PAPER.md:115-128 (Eq. 15-17): phi_n(r) phi_m(r) ~ sum_mu zeta_mu(r) C^mu_nm with C^mu_nm = phi_n(r_mu) phi_m(r_mu) at given
  * interpolation points r_mu = r[idx[mu]] (ISDF, refs. [62, 63]); zeta is the least-squares solution

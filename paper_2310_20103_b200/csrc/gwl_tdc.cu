@@ -195,4 +195,26 @@ gwl_status gwl_tdc_matvec_rpa(gwl_ctx* ctx, const double* x, const double* y, do
     return GWL_OK;
 }
 
+gwl_status gwl_tdc_selfenergy_state(gwl_ctx* ctx, int32_t kn, int32_t km, int32_t m_idx, int64_t steps, int64_t block, int reorth,
+                                    const double* omega, int64_t n_omega, double eta, double* sigma_mm) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    DeviceGuard dg(ctx);
+    if (!ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_tdc_selfenergy_state: not a gwl_tdc_create context");
+    if (sigma_mm == nullptr || omega == nullptr || n_omega < 1)
+        return ctx->fail(GWL_EINVAL, "gwl_tdc_selfenergy_state: bad arguments");
+    const int n_orb = ctx->nv_k + ctx->n_c;
+    std::vector<int32_t> chains((size_t)4 * n_orb);
+    for (int n = 0; n < n_orb; ++n) {
+        chains[4 * n] = kn;
+        chains[4 * n + 1] = n;
+        chains[4 * n + 2] = km;
+        chains[4 * n + 3] = m_idx;
+    }
+    gwl_status rs = gwl_tdc_set_chains(ctx, n_orb, chains.data());
+    if (rs != GWL_OK) return rs;
+    rs = gwl_lanczos(ctx, n_orb, steps, block, reorth, nullptr, nullptr, nullptr, nullptr);
+    if (rs != GWL_OK) return rs;
+    return gwl_selfenergy(ctx, omega, n_omega, eta, nullptr, sigma_mm);
+}
+
 }  // extern "C"

@@ -49,6 +49,8 @@ SIGNATURES = {
     "gwl_tdc_set_chains": (c_int, [c_void_p, c_int64, c_void_p]),
     "gwl_tdc_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
     "gwl_tdc_matvec_rpa": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int64]),
+    "gwl_tdc_selfenergy_state": (c_int, [c_void_p, c_int32, c_int32, c_int32, c_int64, c_int64, c_int, c_void_p, c_int64, c_double,
+                                         c_void_p]),
     "gwl_sym_create": (c_int, [POINTER(c_void_p), c_int, c_void_p, c_void_p, c_int64]),
     "gwl_sym_set_orbitals": (c_int, [c_void_p, c_void_p, c_void_p]),
     "gwl_sym_set_kernel": (c_int, [c_void_p, c_void_p]),
@@ -423,6 +425,19 @@ class TdcContext(Context):
         yh = np.empty_like(xh)
         self._ck(self._lib.gwl_tdc_matvec(self._h, _ptr(xh), _ptr(yh), xh.size // self.n_kvc))
         return yh
+
+    def selfenergy_state(self, kn: int, km: int, m_idx: int, steps: int, block: int, reorth: int, omega, eta: float, out=None):
+        """The q-term of Sigma_{mk,mk}(omega) summed over all n of slot kn (PAPER.md:288 / :310).  Host mode: complex numpy
+        [n_omega]; device mode: omega and out [n_omega, 2] torch CUDA tensors."""
+        if self.device_ptrs:
+            self._ck(self._lib.gwl_tdc_selfenergy_state(self._h, int(kn), int(km), int(m_idx), steps, block, reorth, _ptr(omega),
+                                                        omega.numel(), float(eta), _ptr(out)))
+            return out
+        om = _host(omega)
+        ss = np.zeros(om.size, dtype=np.complex128)
+        self._ck(self._lib.gwl_tdc_selfenergy_state(self._h, int(kn), int(km), int(m_idx), steps, block, reorth, _ptr(om), om.size,
+                                                    float(eta), _ptr(ss)))
+        return ss
 
     def matvec_rpa(self, x, y, ox=None, oy=None):
         """[ox; oy] = Omega^ [x; y] = [A x + B y; B^* x + A^* y].  Host mode: complex numpy arrays

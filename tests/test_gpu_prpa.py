@@ -226,3 +226,20 @@ def test_complex_config2_scale_sampled():
     assert np.abs(a[j] - r0["alpha"]).max() <= 1e-9 * bs
     assert (np.abs(b[j] - r0["beta"]) <= 1e-9 * np.abs(r0["beta"])).all()
     assert np.abs(sig[j] - r0["sigma"]).max() <= 1e-6
+
+
+def test_tdc_selfenergy_state_both_approximations():
+    """gwl_tdc_selfenergy_state: all n of one slot, Eq. 10-like sum on the device, Tamm-Dancoff and RPA, against the oracles."""
+    p = synth.make_periodic(2, 3, 7, 48, seed=13, n_omega=81)
+    n_orb = p.n_v + p.n_c
+    kn, km, m, L = 1, 0, p.n_v - 1, 14
+    chains = np.array([(kn, n, km, m) for n in range(n_orb)], dtype=np.int32)
+    with _ctx(p, n_q=2, chains=False) as ctx:
+        s_rpa = ctx.selfenergy_state(kn, km, m, L, 4, 1, p.omega, DLT)          # blocks of 4, 4, 2
+        ctx.set_approximation(gwl.GWL_TDA)
+        s_tda = ctx.selfenergy_state(kn, km, m, L, 16, 1, p.omega, DLT)
+    r_rpa = rpa.run_chains_rpa(p.psi_v, p.psi_cq, p.eps_v, p.eps_cq, p.V, chains, L, p.omega, DLT, n_q=2, reorth=True)
+    r_tda = tdp.run_chains(p.psi_v, p.psi_cq, p.eps_v, p.eps_cq, p.V, chains, L, p.omega, DLT, n_q=2, reorth=True)
+    assert np.abs(s_rpa - r_rpa["sigma_sum"]).max() <= 1e-6
+    assert np.abs(s_tda - r_tda["sigma_sum"]).max() <= 1e-6
+    assert np.abs(s_rpa - s_tda).max() > 1e-4                                     # the two approximations differ
