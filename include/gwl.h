@@ -292,6 +292,38 @@ gwl_status gwl_get_kernel_times(gwl_ctx* ctx, double* ms, int64_t* count);
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 gwl_status gwl_get_launch_count(gwl_ctx* ctx, int64_t* n_launches);
 
+/* The one entry point that allocates nothing: norm2[j] = <P_j|P_j> = sum_vc p[j][vc]^2, the numerator of the continued
+ * fraction (Eq. 14) and the same quantity gwl_lanczos returns as `norm2`.
+ *
+ * It is for host programs that cannot let a library call cudaMalloc: a driver that has given all of HBM to its own pool
+ * (a later cudaMalloc fails or fragments the remainder), or one that keeps other streams busy (cudaMalloc / cudaFree
+ * synchronise the whole device and would stall them).  Everything else in this header needs a gwl_ctx, whose buffers come
+ * from cudaMalloc; this call needs no context and calls no cudaMalloc, cudaFree or allocating library routine.  The partial
+ * sums of its two-stage reduction go into a fixed array of GWL_STATIC_SCRATCH_BYTES that is part of the library image: every
+ * GPU that loads the library's kernels holds those bytes until the process exits.
+ *
+ *   p      [n_chains][n_vc]  DEVICE pointer, read only, contiguous (row stride n_vc)
+ *   norm2  [n_chains]        DEVICE pointer, written; must not overlap p
+ *   cuda_stream              cudaStream_t the two kernels are enqueued on (NULL = legacy default stream); the call does not
+ *                            synchronise: norm2 is valid once the stream has reached this point
+ *   err, err_len             optional caller-owned buffer for a NUL-terminated description of a failure ("" on success);
+ *                            err may be NULL
+ * p and norm2 must live on the CURRENT device (cudaSetDevice); the caller owns them.
+ * Limits: 0 <= n_chains <= GWL_STATIC_MAX_CHAINS, 1 <= n_vc <= GWL_STATIC_MAX_NVC, else GWL_EINVAL with the limit named in
+ * err; nothing is launched then.  n_chains = 0 is a no-op.  A failed set-up or launch returns GWL_ECUDA.
+ * First call on each device: the library looks up the device address of its scratch array once (cudaGetSymbolAddress, with
+ * that device current) and keeps it.  Make that first call during start-up, outside any stream capture.
+ * Sharing: all calls in the process use the same array on a given device.  It keeps the previous call's partial sums; that
+ * is harmless because each call writes every slot before it reads it (nothing has to start at zero).  Two calls whose
+ * kernels can overlap on one GPU (different streams, or different host threads) race on the array and give wrong norms:
+ * order them on one stream or with events.
+ * Results repeat bit for bit for the same arguments and agree with gwl_lanczos's norm2 to rounding (1e-12 relative). */
+#define GWL_STATIC_SCRATCH_BYTES 262144          /* 32 768 doubles */
+#define GWL_STATIC_MAX_CHAINS 4096
+#define GWL_STATIC_MAX_NVC 4294967296LL          /* 2^32 pairs */
+gwl_status gwl_chain_norms_static(const double* p, int64_t n_chains, int64_t n_vc, double* norm2, void* cuda_stream,
+                                  char* err, int64_t err_len);
+
 /* Measurement helper, not part of the method: run a register-resident mma.sync.m8n8k4.f64 (kind 0) or
  * DFMA (kind 1) loop on every SM of the current device and return the achieved FP64 TFLOP/s.
  * This is the denominator DESIGN.md uses for the FP64 tensor roofline. */

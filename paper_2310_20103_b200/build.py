@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgwl.so")
-SOURCES = ["gwl_api.cu", "gwl_driver.cu", "gwl_tdc.cu", "gwl_sym.cu", "gwl_isdf_api.cu", "kr_gemm.cu", "kr_gemm_c.cu", "isdf.cu", "vec_kernels.cu", "prpa_kernels.cu", "sym_kernels.cu", "spectral_kernels.cu", "ritz_dc.cu", "probe.cu"]
+SOURCES = ["gwl_api.cu", "gwl_driver.cu", "gwl_tdc.cu", "gwl_sym.cu", "gwl_isdf_api.cu", "kr_gemm.cu", "kr_gemm_c.cu", "isdf.cu", "vec_kernels.cu", "prpa_kernels.cu", "sym_kernels.cu", "spectral_kernels.cu", "ritz_dc.cu", "probe.cu", "noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC"]

@@ -65,6 +65,7 @@ SIGNATURES = {
     "gwl_get_kernel_times": (c_int, [c_void_p, POINTER(c_double), POINTER(c_int64)]),
     "gwl_get_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
     "gwl_probe_fp64_peak": (c_int, [c_int, POINTER(c_double)]),
+    "gwl_chain_norms_static": (c_int, [c_void_p, c_int64, c_int64, c_void_p, c_void_p, c_char_p, c_int64]),
 }
 
 
@@ -121,6 +122,29 @@ def probe_fp64_peak(kind: int = 0) -> float:
     if st != GWL_OK:
         raise GwlError(st, "gwl_probe_fp64_peak failed")
     return out.value
+
+
+def chain_norms_static(p, norm2, n_chains: int | None = None, n_vc: int | None = None, cuda_stream: int | None = None):
+    """norm2[j] = <P_j|P_j> through gwl_chain_norms_static, the entry point for callers that must not trigger a
+    cudaMalloc (all of HBM already in the caller's pool, or other streams that a device-wide synchronisation would
+    stall).  p [n_chains, n_vc] and norm2 [n_chains] are contiguous torch CUDA float64 tensors on the current device;
+    norm2 is written in place on `cuda_stream` (default: the legacy default stream) and returned.  The scratch is a
+    fixed 256 KB array inside libgwl.so shared by all calls: do not let two calls overlap on one GPU.  Sizes may be
+    given explicitly when p is a flat buffer; limits: n_chains <= 4096, n_vc <= 2^32 (GwlError otherwise)."""
+    lib = load_library()
+    if n_chains is None or n_vc is None:
+        if p.dim() != 2:
+            raise GwlError(GWL_EINVAL, "chain_norms_static: p must be [n_chains, n_vc] (or pass the sizes)")
+        n_chains, n_vc = p.shape
+    if not (_is_torch(p) and _is_torch(norm2) and p.is_cuda and norm2.is_cuda and p.is_contiguous()
+            and norm2.is_contiguous()) or p.numel() < n_chains * n_vc or norm2.numel() < n_chains:
+        raise GwlError(GWL_EINVAL, "chain_norms_static: p, norm2 must be contiguous torch CUDA float64 tensors of "
+                                   "at least n_chains * n_vc and n_chains elements")
+    err = ctypes.create_string_buffer(256)
+    st = lib.gwl_chain_norms_static(_ptr(p), int(n_chains), int(n_vc), _ptr(norm2), c_void_p(cuda_stream or 0), err, 256)
+    if st != GWL_OK:
+        raise GwlError(st, err.value.decode())
+    return norm2
 
 
 class Context:
