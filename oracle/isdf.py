@@ -30,7 +30,9 @@ def fit(phi_a, phi_b, idx):
 
 def coulomb_grid(r, weight, soft):
     """Quadrature form of 1/|r - r'| on the grid points, softened at short range (stand-in for the Poisson solve of the
-    real-space code): G[i, j] = weight^2 14.4 / sqrt(|r_i - r_j|^2 + soft^2)  (eV Angstrom units as in synth.py)."""
+    real-space code): G[i, j] = weight^2 14.4 / sqrt(|r_i - r_j|^2 + soft^2)  (eV Angstrom units as in synth.py).
+    Pinned by the Coulomb energy of two Gaussian charges (erf closed form and its softened one-dimensional integral),
+    tests/test_oracle_pins_isdf.py::test_coulomb_grid_reproduces_the_coulomb_energy_of_two_gaussian_charges."""
     d = r[:, None, :] - r[None, :, :]
     return weight * weight * 14.4 / np.sqrt(np.einsum("ijk,ijk->ij", d, d) + soft * soft)
 
