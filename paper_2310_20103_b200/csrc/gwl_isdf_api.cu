@@ -33,16 +33,17 @@ gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, c
     CK(PhiMu.ensure((size_t)n_mu * nop * 8 + (size_t)n_mu * n_orb * 8, st));
     CK(Y.ensure((size_t)n_mu * nrp * 8, st));
     CK(S.ensure((size_t)n_mu * ldm * 8 + (size_t)n_r * 24 + 8 + (size_t)n_mu * 4 + 16, st));
-    CK(G.ensure((size_t)n_r * nrp * 8, st));
+    // G also stages the finished (alpha|beta): the context's own V and orbitals are only touched once every step that can
+    // fail on the inputs (a singular C C^T) has passed, so a failed build leaves a ready context exactly as it was.
+    const size_t v_bytes = (size_t)n_mu * ldm * 8;
+    CK(G.ensure(std::max((size_t)n_r * nrp * 8, v_bytes), st));
     CK(U.ensure((size_t)n_mu * nrp * 8, st));
-    CK(ctx->V.ensure((size_t)n_mu * ldm * 8, st));
     CK(cudaMemsetAsync(Phi.p, 0, Phi.bytes, st));
     CK(cudaMemsetAsync(PhiMu.p, 0, PhiMu.bytes, st));
     CK(cudaMemsetAsync(Y.p, 0, Y.bytes, st));
     CK(cudaMemsetAsync(S.p, 0, S.bytes, st));
     CK(cudaMemsetAsync(G.p, 0, G.bytes, st));
     CK(cudaMemsetAsync(U.p, 0, U.bytes, st));
-    CK(cudaMemsetAsync(ctx->V.p, 0, ctx->V.bytes, st));
     double* dS = S.as<double>();
     double* d_r = dS + (size_t)n_mu * ldm;
     double* d_scale = d_r + (size_t)n_r * 3;
@@ -75,8 +76,24 @@ gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, c
     CKL(4, launch_coulomb_grid(d_r, nr, weight, soft, G.as<double>(), nrp, st));
     rs = plain_gemm(ctx, G.as<double>(), nrp, Y.as<double>(), nrp, nr, n_mu, (int)(nrp / BK), U.as<double>(), nrp, 1);
     if (rs != GWL_OK) return rs;
-    rs = plain_gemm(ctx, Y.as<double>(), nrp, U.as<double>(), nrp, n_mu, n_mu, (int)(nrp / BK), ctx->V.as<double>(), ldm, 1);
+    CK(cudaMemsetAsync(G.p, 0, v_bytes, st));  // G itself is consumed; its head becomes the staging copy of V (zero padding)
+    rs = plain_gemm(ctx, Y.as<double>(), nrp, U.as<double>(), nrp, n_mu, n_mu, (int)(nrp / BK), G.as<double>(), ldm, 1);
     if (rs != GWL_OK) return rs;
+    // Commit.  From here on only a CUDA failure can stop the call; if one does, the context is left "not ready"
+    // (GWL_ESTATE from the next product) instead of holding a kernel and orbitals that do not belong together.
+    struct CommitGuard {
+        gwl_ctx* c;
+        bool done = false;
+        ~CommitGuard() {
+            if (!done) {
+                c->have_V = false;
+                c->have_orb = false;
+                invalidate_run(c);
+            }
+        }
+    } commit{ctx};
+    CK(ctx->V.ensure(v_bytes, st));
+    CK(cudaMemcpyAsync(ctx->V.p, G.p, v_bytes, cudaMemcpyDeviceToDevice, st));
     // the orbitals at the interpolation points become the context's orbitals
     double* compact = PhiMu.as<double>() + (size_t)n_mu * nop;  // [n_mu][n_v] then [n_mu][n_c]
     CK(cudaMemcpy2DAsync(compact, (size_t)ctx->n_v * 8, PhiMu.p, (size_t)nop * 8, (size_t)ctx->n_v * 8, (size_t)n_mu,
@@ -92,6 +109,7 @@ gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, c
         CK(cudaMemcpy2DAsync(V_out, (size_t)n_mu * 8, ctx->V.p, (size_t)ldm * 8, (size_t)n_mu * 8, (size_t)n_mu,
                              cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    commit.done = true;
     ctx->have_orb = true;
     ctx->have_V = true;
     invalidate_run(ctx);

@@ -20,7 +20,11 @@ def _problem(n_grid, n_v, n_c, n_mu, seed=1):
     return r, phi, w, idx
 
 
-@pytest.mark.parametrize("n_grid,n_v,n_c,n_mu,seed", [(8, 2, 4, 14, 1), (10, 3, 6, 24, 5), (12, 4, 9, 40, 0)])
+# The last case reaches the blocked paths of the factorisation and the solves: N_mu = 256 is eight Cholesky blocks of 32
+# (seven panels and trailing updates), n_r = 20^3 = 8000 grid points, 72 orbitals.  The pair products of 72 box states have
+# numerical rank 413, and at these points cond(C C^T) = 3.2e5 (same range as the small cases: the 1e-8 bar is kept).
+@pytest.mark.parametrize("n_grid,n_v,n_c,n_mu,seed", [(8, 2, 4, 14, 1), (10, 3, 6, 24, 5), (12, 4, 9, 40, 0),
+                                                      (20, 16, 56, 256, 1)])
 def test_isdf_fit_and_two_center_integrals(n_grid, n_v, n_c, n_mu, seed):
     r, phi, w, idx = _problem(n_grid, n_v, n_c, n_mu, seed)
     soft = 0.5
@@ -83,6 +87,30 @@ def test_isdf_rejects_bad_points_and_rank_deficient_fits():
         assert e.value.status == gwl.GWL_EINVAL and "positive definite" in str(e.value)
         with pytest.raises(gwl.GwlError):
             ctx.casida_matvec(np.zeros((1, 2, 3)))                        # nothing was installed
+
+
+def test_failed_isdf_build_leaves_a_ready_context_untouched():
+    """A context that already holds an operator (set_orbitals / set_energies / set_kernel) keeps exactly that operator when a
+    later gwl_isdf_build fails on its inputs (singular C C^T): the product before and after is bit-identical.  The build
+    stages (alpha|beta) in scratch and touches the context's V and orbitals only after the factorisation has succeeded."""
+    p = synth.make_custom(2, 3, 20, seed=3)
+    r, phi, w, idx = _problem(8, 2, 3, 20)
+    X = synth.random_block(p.cfg, 2)
+    with gwl.Context(2, 3, 20) as ctx:
+        ctx.set_orbitals(p.phi_v, p.phi_c)
+        ctx.set_energies(p.eps_v, p.eps_c)
+        ctx.set_kernel(p.V)
+        y0 = ctx.casida_matvec(X)
+        with pytest.raises(gwl.GwlError) as e:
+            ctx.isdf_build(phi[:, :2], phi[:, 2:], r, w, 0.5, idx)          # rank-deficient, as in the test above
+        assert e.value.status == gwl.GWL_EINVAL and "positive definite" in str(e.value)
+        y1 = ctx.casida_matvec(X)
+        ctx.set_chains(p.n_idx, p.m_idx)
+        a, b, n2, ln = ctx.lanczos(len(p.n_idx), 6, 4, 0)
+    assert np.array_equal(y0, y1)
+    ref = orc.casida_matvec_factored(p.phi_v, p.phi_c, p.V, orc.delta_vc(p.eps_v, p.eps_c), X)
+    assert np.abs(y1 - ref).max() <= 1e-12 * np.abs(ref).max()
+    assert (n2 > 0).all() and np.isfinite(a).all()
 
 
 def test_cvt_point_selection_matches_oracle_and_feeds_the_fit():
