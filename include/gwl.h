@@ -112,14 +112,17 @@ gwl_status gwl_set_start_vectors(gwl_ctx* ctx, int64_t n_chains, const double* p
 
 /* Lanczos tridiagonalisation of Op (C, or p_g(C) in poly mode) for the first n_chains chains set
  * above, `block` chains at a time (the last block may be short), PAPER.md:87-90 (Eq. 13).
- * steps = number of Op applications = dimension of T_L.  reorth: 0 off, 1 two-pass full
- * reorthogonalisation against all previous Lanczos vectors of the same chain.
+ * steps = number of Op applications = dimension of T_L (1..100000).  reorth: 0 off, 1 two-pass full
+ * reorthogonalisation against all previous Lanczos vectors of the same chain; then steps <= GWL_MAX_REORTH_STEPS
+ * (GWL_EINVAL above it: the kernels keep one projection coefficient per earlier vector in shared memory, and the
+ * basis of steps x block x N_vc doubles has to fit in HBM anyway).
  * Outputs (may be NULL to skip; the context keeps its own copy for gwl_resolvent/gwl_selfenergy):
  *   alpha [n_chains][steps]  a_0 .. a_{L-1}
  *   beta  [n_chains][steps]  beta[k] = b_{k+1}; beta[steps-1] is returned but not part of T_L
  *   norm2 [n_chains]         <P|P>
  *   len   [n_chains]         effective length <= steps: on breakdown (b_{k+1} <= 1e-12 max_i(|a_i|+b_i))
  *                            len = k+1, b_{k+1} is stored as 0 and the tail is zero-filled. */
+#define GWL_MAX_REORTH_STEPS 8192
 gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t block, int reorth,
                        double* alpha, double* beta, double* norm2, int32_t* len);
 
@@ -186,6 +189,7 @@ gwl_status gwl_qp_solve(gwl_ctx* ctx, int64_t n_states, const double* eps_m, con
  * exact at L = 2 N_k N_v N_c.  One step costs one product with Omega^ (2 K, 1 V, 2 K^H contractions: twice a TDA step).
  * gwl_lanczos then returns the alpha, beta of that T_L and norm2 = <u,u>_O; gwl_selfenergy evaluates the sum above (with the
  * prefactor); gwl_resolvent gives <u|(zeta - C^RPA)^{-1}|u>_O by Eq. 14 (both branches). */
+#define GWL_TDC_MAX_KV 65535 /* n_k * n_v of a complex context (the (k, v) planes are a grid dimension); GWL_EINVAL above it */
 gwl_status gwl_tdc_create(gwl_ctx** out, int64_t n_k, int64_t n_v, int64_t n_c, int64_t n_mu, int64_t n_q);
 /* psi_v [n_k][n_mu][n_v][2] = psi_{v k}(r_mu); psi_cq [n_k][n_mu][n_c][2] = psi_{c k+q}(r_mu) (slot k holds the conduction
  * orbitals of momentum k+q: the caller does the momentum bookkeeping).  Host. */
@@ -278,7 +282,10 @@ gwl_status gwl_sym_selfenergy_state(gwl_ctx* ctx, int32_t m_idx, int64_t steps, 
  * vector kernels (S4) and overall.  Any pointer may be NULL.  Synchronises the stream. */
 gwl_status gwl_get_timing(gwl_ctx* ctx, double* ms_matvec, double* ms_vecops, double* ms_total);
 
-/* Profiling level: 0 no events; 1 (default) one CUDA-event triple per Lanczos step (feeds gwl_get_timing);
+/* Profiling level: 0 no events -- this is also the switch for the CUDA-graph replay of the step loop: at level 0 gwl_lanczos
+ * replays six steps at a time from a captured graph when the problem is launch-bound (N_vc <= 65 536, reorth = 0, real
+ * orbitals, steps >= 16, at most 8 chain blocks per call); the results are bit-identical to plain launches, which every
+ * other level uses; 1 (default) one CUDA-event triple per Lanczos step (feeds gwl_get_timing);
  * 2 additionally an event pair around every kernel launch, tagged with its class (feeds gwl_get_kernel_times). */
 gwl_status gwl_set_profiling(gwl_ctx* ctx, int level);
 /* Per-class device time (ms) and launch count since the start of the last gwl_lanczos (including later

@@ -644,14 +644,21 @@ gwl_status gwl_lanczos(gwl_ctx* ctx, int64_t n_chains, int64_t steps, int64_t bl
     DeviceGuard dg(ctx);
     if (n_chains < 0 || steps < 1 || steps > 100000 || block < 1 || (reorth != 0 && reorth != 1))
         return ctx->fail(GWL_EINVAL, "gwl_lanczos: bad arguments");
+    if (reorth == 1 && steps > GWL_MAX_REORTH_STEPS)
+        return ctx->fail(GWL_EINVAL, "gwl_lanczos: reorth = 1 needs steps <= GWL_MAX_REORTH_STEPS = " + std::to_string(GWL_MAX_REORTH_STEPS) +
+                                         " (the projection coefficients of all earlier vectors sit in shared memory)");
     if (!ready(ctx)) return ctx->fail(GWL_ESTATE, "gwl_lanczos: orbitals, energies and kernel must be set");
     if (ctx->chain_mode == 0) return ctx->fail(GWL_ESTATE, "gwl_lanczos: no chains set");
     if (n_chains > ctx->n_chains_set) return ctx->fail(GWL_EINVAL, "gwl_lanczos: more chains than were set");
     // Step graphs (small problems, no profiling events, no reorthogonalisation): the whole call runs on an internal stream
     // fenced against the caller's stream on both sides, because the caller's stream may be the legacy default stream.
-    static const bool graphs_allowed = std::getenv("GWL_NO_GRAPH") == nullptr;
-    const bool want_graph = graphs_allowed && !ctx->graph_off && ctx->prof_level == 0 && reorth == 0 && !ctx->cplx && steps >= 16 &&
-                            n_chains > 0 && lanczos_fused_fits(ctx->n_vc);
+    // A captured graph is tied to its chain block (the alpha/beta bases of the block are baked into the kernel arguments),
+    // and the context caches eight of them: with more blocks than that every block would re-capture on every call, which
+    // costs more than the replay saves, so such calls use plain launches.  Switch: gwl_set_profiling(ctx, 0) enables the
+    // replay, any other level (the default is 1) disables it.
+    const int64_t n_blocks = (n_chains + block - 1) / block;
+    const bool want_graph = !ctx->graph_off && ctx->prof_level == 0 && reorth == 0 && !ctx->cplx && steps >= 16 &&
+                            n_chains > 0 && n_blocks <= 8 && lanczos_fused_fits(ctx->n_vc);
     if (!want_graph) return lanczos_impl(ctx, n_chains, steps, block, reorth, alpha, beta, norm2, len, false);
     if (ctx->gstream == nullptr) {
         CK(cudaStreamCreateWithFlags(&ctx->gstream, cudaStreamNonBlocking));

@@ -460,6 +460,9 @@ gwl_status create_common(gwl_ctx** out, int64_t n_k, int64_t n_v, int64_t n_c, i
     if (n_v < 1 || n_c < 1 || n_mu < 1 || n_k < 1 || n_q < 1 || n_k > 4096 || n_k * n_v > (1 << 20) || n_c > (1 << 20) ||
         n_mu > (1 << 24))
         return GWL_EINVAL;
+    // the complex Khatri-Rao GEMMs index the (k, v) planes through grid.z (kr_gemm_c.cu): reject here, where the caller can
+    // see why, instead of failing every later product with an opaque CUDA error (include/gwl.h states the limit)
+    if (cplx && n_k * n_v > GWL_TDC_MAX_KV) return GWL_EINVAL;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) {
         cudaGetLastError();

@@ -56,6 +56,8 @@ def test_create_validates_and_fails_loudly_without_gpu(lib):
         assert not h.value
         with pytest.raises(gwl.GwlError):
             gwl.Context(2, 2, 2)
+    # complex contexts: n_k * n_v beyond GWL_TDC_MAX_KV is refused at creation (it is a grid dimension of the complex GEMMs)
+    assert lib.gwl_tdc_create(ctypes.byref(h), 64, 1100, 8, 16, 1) == gwl.GWL_EINVAL and not h.value
     lib.gwl_destroy(None)                       # NULL-safe
     assert lib.gwl_last_error(None) == b""
     assert lib.gwl_set_pointer_mode(None, 0) == gwl.GWL_EINVAL

@@ -326,10 +326,31 @@ def test_state_and_argument_errors(p0):
             ctx.lanczos(5, 5, 1, 0)                                   # more chains than set
         with pytest.raises(gwl.GwlError):
             ctx.lanczos(1, 0, 1, 0)                                   # steps < 1
+        with pytest.raises(gwl.GwlError) as e:
+            ctx.lanczos(1, 8193, 1, 1)                                # reorth beyond GWL_MAX_REORTH_STEPS: named, not ECUDA
+        assert e.value.status == gwl.GWL_EINVAL and "GWL_MAX_REORTH_STEPS" in str(e.value)
         a, b, n2, ln = ctx.lanczos(0, 5, 4, 0)                        # empty run is fine
         assert a.shape == (0, 5)
         assert ctx.casida_matvec(np.zeros((0, cfg.n_v, cfg.n_c))).shape == (0, cfg.n_v, cfg.n_c)
         assert ctx.get_launch_count() > 0
+
+
+def test_spectrum_bounds_after_breakdown_match_the_oracle():
+    """Breakdown inside the range probe: with V = 0 and only three distinct Delta the Krylov space of any start vector is
+    three-dimensional, the fourth beta vanishes, and the bounds are the exact extreme eigenvalues min / max Delta^2 with a
+    zero residual term -- on the GPU (b_last = 0 when len < steps) and in the oracle (beta[len-1] stored as 0) alike."""
+    p = synth.make_custom(4, 6, 16, seed=2)
+    eps_v = np.full(4, -7.0)
+    eps_c = np.array([1.0, 1.0, 2.5, 2.5, 6.0, 6.0])
+    delta = orc.delta_vc(eps_v, eps_c)
+    with gwl.Context(4, 6, 16) as ctx:
+        ctx.set_orbitals(p.phi_v, p.phi_c)
+        ctx.set_energies(eps_v, eps_c)
+        ctx.set_kernel(np.zeros((16, 16)))
+        lo, hi = ctx.spectrum_bounds(10)
+    olo, ohi = orc.spectrum_bounds_lanczos(lambda x: delta ** 2 * x, delta.size, 10)
+    for got in ((lo, hi), (olo, ohi)):
+        assert abs(got[0] - 64.0) <= 1e-10 * 64.0 and abs(got[1] - 169.0) <= 1e-10 * 169.0
 
 
 def test_launches_and_timing_reported(p0):
