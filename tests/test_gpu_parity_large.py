@@ -132,24 +132,31 @@ def test_lanczos_config2_block_invariance():
 def test_poly_mode_config2_paper_parameters_sampled_chains():
     """The paper's own route at the 128x128-tile size: Lanczos on p_g(C) with g = 7, N_iter = 8, every C-apply
     ending in the fused Chebyshev epilogue, the whole block of 256 chains on the GPU (reorthogonalisation off, two-kernel
-    update); the oracle follows sampled chains with the same polynomial (fitting range from gwl_spectrum_bounds: the
-    heuristic range does not contain this spectrum, Q23).  alpha/beta 1e-9, Sigma (Eq. 12 + 14) 1e-6 eV."""
+    update); the oracle follows sampled chains on the fitting range of ITS OWN Lanczos bound (the heuristic range does not
+    contain this spectrum, Q23) with its own least-squares coefficients.  alpha/beta 1e-9, Sigma (Eq. 12 + 14) 1e-6 eV."""
     from paper_2310_20103_b200 import polyfit
     p = _problem(2)
     cfg = p.cfg
     g, L = 7, 8
     idx = np.array([3, 200])
+    # The fitting range comes from the ORACLE's own 24-step Lanczos on the oracle's factored product; the GPU's
+    # gwl_spectrum_bounds is asserted against it, never consumed (inputs flow oracle -> GPU only).  Each side fits its
+    # own coefficients on that range: polyfit.sqrt_chebyshev (closed form) for the GPU, orc.fit_sqrt_chebyshev (lstsq).
+    delta = orc.delta_vc(p.eps_v, p.eps_c)
+    _, top = orc.spectrum_bounds_lanczos(
+        lambda x: orc.casida_matvec_factored(p.phi_v, p.phi_c, p.V, delta, x[None])[0], delta.size, 24)
+    lo, hi = 0.8 * (delta ** 2).min(), 1.02 * top
     with _ctx(p, chains=False) as ctx:
-        lo, hi = polyfit.range_from_spectrum(ctx, p.eps_v, p.eps_c, steps=24)
-        c = polyfit.sqrt_chebyshev(g, lo, hi)
-        ctx.set_polynomial(g, c, lo, hi)
+        glo, ghi = polyfit.range_from_spectrum(ctx, p.eps_v, p.eps_c, steps=24)
+        assert abs(glo - lo) <= 1e-12 * lo and abs(ghi - hi) <= 1e-6 * hi
+        ctx.set_polynomial(g, polyfit.sqrt_chebyshev(g, lo, hi), lo, hi)
         ctx.set_chains(p.n_idx, p.m_idx)
         a, b, n2, ln = ctx.lanczos(cfg.block, L, cfg.block, 0)
         sig, _ = ctx.selfenergy(p.omega, DLT, cfg.block)
     lam_max_heuristic = polyfit.default_range(p.eps_v, p.eps_c)[1]
     assert hi > 1.5 * lam_max_heuristic                                # the case the advisor flagged in round 1
     ref = orc.run_chains(p.phi_v, p.phi_c, p.eps_v, p.eps_c, p.V, p.n_idx[idx], p.m_idx[idx], L, p.omega, DLT, reorth=False,
-                         poly=(c, lo, hi))
+                         poly=(orc.fit_sqrt_chebyshev(g, lo, hi), lo, hi))
     assert (ln[idx] == ref["len"]).all()
     assert (np.abs(n2[idx] - ref["norm2"]) <= 1e-12 * ref["norm2"]).all()
     _check_ab(a[idx], b[idx], ref["alpha"], ref["beta"], L)
