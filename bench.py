@@ -451,6 +451,9 @@ def cublas_dgemm_tflops(dev, n=8192, reps=3):
     return 2.0 * n ** 3 / (best * 1e-3) / 1e12
 
 
+SHARD_QUANTUM = 128   # chain shards are cut at multiples of the GEMM column tile (runtime.shard_range)
+
+
 def run_sharded_state(args):
     """Sigma^corr_mm(omega) of ONE state with its N_v+N_c chains partitioned over the ranks
     (runtime.shard_range), direct mode, L steps each, ONE all-reduce (NCCL) of the omega grid.  Strong scaling:
@@ -483,7 +486,7 @@ def run_sharded_state(args):
     local = runtime.gwl_local_sigma_sum(ctx, m, L, cfg.block, 0, om, cfg.eta)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
     for _ in range(args.warmup):
-        runtime.sharded_sigma_state(local, n_orb)
+        runtime.sharded_sigma_state(local, n_orb, SHARD_QUANTUM)
     torch.cuda.synchronize()
     sampler = runtime.ClockSampler(local_rank).start()
     if world > 1:
@@ -495,7 +498,7 @@ def run_sharded_state(args):
         flush.zero_()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        sig = runtime.sharded_sigma_state(local, n_orb)
+        sig = runtime.sharded_sigma_state(local, n_orb, SHARD_QUANTUM)
         e1.record(stream)
         pairs.append((e0, e1))
     torch.cuda.synchronize()
@@ -503,7 +506,7 @@ def run_sharded_state(args):
         dist.barrier()
     clocks = sampler.stop()
     elapsed = sum(a.elapsed_time(b) for a, b in pairs) * 1e-3
-    lo, hi = runtime.shard_range(n_orb, rank, world)
+    lo, hi = runtime.shard_range(n_orb, rank, world, SHARD_QUANTUM)
     units, tmax = runtime.aggregate_throughput(float(args.steps) * (hi - lo) * L, elapsed, dev)
     if rank == 0:
         line = {"metric": METRIC, "value": units / tmax, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -518,6 +521,8 @@ def run_sharded_state(args):
                            "l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB write)"},
                 "clocks": clocks, "gpu_launches": int(ctx.get_launch_count() - n0),
                 "allreduce_bytes_per_step": int(cfg.n_omega * 16) if world > 1 else 0,
+                "chains_per_rank": [b - a for a, b in (runtime.shard_range(n_orb, r, world, SHARD_QUANTUM) for r in range(world))],
+                "shard_quantum": SHARD_QUANTUM, "tile_efficiency": runtime.tile_efficiency(n_orb, world, SHARD_QUANTUM),
                 "sigma_checksum": float(sig.abs().sum().item())}
         print(json.dumps(line), flush=True)
     ctx.close()

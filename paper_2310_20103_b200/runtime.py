@@ -41,22 +41,40 @@ def whole_job_value(units_local: float, elapsed_s_local: float, device=None) -> 
     return u / t if t > 0 else 0.0
 
 
-def shard_range(n: int, rank: int, world: int):
-    """Contiguous, balanced slice [lo, hi) of n items for `rank` of `world` (first n % world ranks get one more)."""
-    base, rem = divmod(int(n), int(world))
-    lo = rank * base + min(rank, rem)
-    return lo, lo + base + (1 if rank < rem else 0)
+def shard_range(n: int, rank: int, world: int, quantum: int = 1):
+    """Contiguous slice [lo, hi) of n items for `rank` of `world`.
+    quantum = 1: balanced to +-1 item (the first n % world ranks get one more).
+    quantum = q > 1: whole tiles of q items are handed out, balanced to +-1 TILE, and the ragged last tile goes with its
+    rank; every cut is a multiple of q.  This is the cut for Lanczos chains: a block of chains costs whole GEMM column
+    tiles (q = 128 for the wide kernels), so 160 chains cost two tiles exactly like 256 do, and the
+    step time of the job is the LARGEST tile count of any rank -- ceil(ceil(n/q) / world), which this cut attains.  Ranks
+    beyond the tile count get an empty slice (they could only shorten the job by taking part of a tile, which costs a
+    whole one)."""
+    n, rank, world, q = int(n), int(rank), int(world), max(1, int(quantum))
+    tiles = -(-n // q)
+    base, rem = divmod(tiles, world)
+    t_lo = rank * base + min(rank, rem)
+    t_hi = t_lo + base + (1 if rank < rem else 0)
+    return min(t_lo * q, n), min(t_hi * q, n)
 
 
-def sharded_sigma_state(local_sigma_sum, n_orb: int):
+def tile_efficiency(n: int, world: int, quantum: int) -> float:
+    """Useful columns / columns paid for on the critical path: n / (world * quantum * max tiles of any rank)."""
+    q = max(1, int(quantum))
+    worst = max(-(-(hi - lo) // q) for lo, hi in (shard_range(n, r, world, q) for r in range(int(world))))
+    return float(n) / float(world * q * worst) if worst else 1.0
+
+
+def sharded_sigma_state(local_sigma_sum, n_orb: int, quantum: int = 1):
     """Sigma^corr_mm(omega) = sum over all n (Eq. 10) with the chains n partitioned over the ranks.
     local_sigma_sum(lo, hi) -> float64 tensor [n_omega, 2] holding the sum over n in [lo, hi) (zeros if empty),
-    on the device of the process group's backend.  Returns the all-reduced tensor (same on every rank)."""
+    on the device of the process group's backend.  `quantum`: see shard_range (128 for the GPU path).
+    Returns the all-reduced tensor (same on every rank)."""
     import torch.distributed as dist
     on = dist.is_available() and dist.is_initialized()
     rank = dist.get_rank() if on else 0
     world = dist.get_world_size() if on else 1
-    lo, hi = shard_range(n_orb, rank, world)
+    lo, hi = shard_range(n_orb, rank, world, quantum)
     part = local_sigma_sum(lo, hi)
     if on and world > 1:
         dist.all_reduce(part, op=dist.ReduceOp.SUM)

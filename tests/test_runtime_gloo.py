@@ -106,3 +106,24 @@ def test_shard_range_covers_everything():
             assert cuts[0][0] == 0 and cuts[-1][1] == n
             assert all(a[1] == b[0] for a, b in zip(cuts, cuts[1:]))
             assert max(h - l for l, h in cuts) - min(h - l for l, h in cuts) <= 1
+
+
+def test_tile_aligned_shards():
+    """runtime.shard_range with quantum = 128 (the GEMM column tile): cuts at multiples of 128, whole tiles balanced to +-1,
+    everything covered once, and the largest tile count of any rank is the optimum ceil(tiles / world) -- for the chain
+    counts of config 2 (1280), config 3 (5120) and the Si86H76-shaped state (1730) on 8 / 8 / 4 ranks."""
+    from paper_2310_20103_b200 import runtime
+    q = 128
+    for n, w in ((1280, 8), (5120, 8), (1730, 4), (160, 8), (100, 3), (0, 2), (129, 2)):
+        cuts = [runtime.shard_range(n, r, w, q) for r in range(w)]
+        assert cuts[0][0] == 0 and cuts[-1][1] == n
+        assert all(cuts[i][1] == cuts[i + 1][0] for i in range(w - 1))
+        assert all(lo % q == 0 and (hi % q == 0 or hi == n) for lo, hi in cuts)
+        tiles = [-(-(hi - lo) // q) for lo, hi in cuts]
+        assert max(tiles) == -(-(-(-n // q)) // w) and max(tiles) - min(tiles) <= 1
+    assert [hi - lo for lo, hi in (runtime.shard_range(1280, r, 8, q) for r in range(8))] == [256, 256, 128, 128, 128, 128, 128, 128]
+    assert [hi - lo for lo, hi in (runtime.shard_range(1730, r, 4, q) for r in range(4))] == [512, 512, 384, 322]
+    # the +-1-chain cut of config 2 on 8 ranks pays two tiles for 160 chains on every rank: 62.5 %; the aligned cut, with
+    # the same two-tile critical path, is honest about it, and 5120 chains on 8 ranks lose nothing
+    assert abs(runtime.tile_efficiency(1280, 8, q) - 0.625) < 1e-12 and runtime.tile_efficiency(5120, 8, q) == 1.0
+    assert runtime.shard_range(10, 1, 3) == (4, 7)                              # quantum 1: the old balanced cut
