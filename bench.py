@@ -63,6 +63,10 @@ def parse():
     ap.add_argument("--sharded-state", action="store_true",
                     help="SURVEY 8(f)-2 arm, its own line: the N_v+N_c chains of ONE state partitioned over the ranks "
                          "(runtime.shard_range), one NCCL all-reduce of the omega grid; strong scaling")
+    ap.add_argument("--isdf", default="", metavar="NGRID,NORB,NMU[,SEED]",
+                    help="context run, not the bench line: the ISDF front end (SURVEY 8(f)-4; gwl_isdf_build) on NORB particle-in-"
+                         "a-box orbitals on an NGRID^3 grid (n_r = NGRID^3 <= 65535) with NMU interpolation points, e.g. 40,256,1024: "
+                         "seconds per build, flop model and fraction of the DMMA peak")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -451,6 +455,56 @@ def cublas_dgemm_tflops(dev, n=8192, reps=3):
     return 2.0 * n ** 3 / (best * 1e-3) / 1e12
 
 
+def run_isdf(args):
+    """gwl_isdf_build timed end to end through the C ABI with HOST buffers (the call is synchronous:
+    H2D of the orbitals and points, Z C^T and C C^T on the DMMA GEMM, Cholesky + solves, the dense Coulomb quadrature
+    matrix G, G zeta and zeta^T G zeta on the DMMA GEMM, D2H of (alpha|beta)).  Prints its own JSON line."""
+    import time
+
+    import numpy as np
+    import torch
+
+    from paper_2310_20103_b200 import gwl, synth
+
+    parts = [int(x) for x in args.isdf.split(",")]
+    n_grid, n_orb, n_mu = parts[:3]
+    seed = parts[3] if len(parts) > 3 else 1
+    n_v = max(1, n_orb // 4)
+    n_c = n_orb - n_v
+    torch.cuda.set_device(0)
+    gwl.load_library()
+    r, phi, w = synth.box_orbitals(n_grid, n_orb)
+    n_r = r.shape[0]
+    idx = synth.stride_points(n_r, n_mu, seed)
+    pv, pc = np.ascontiguousarray(phi[:, :n_v]), np.ascontiguousarray(phi[:, n_v:])
+    peak = gwl.probe_fp64_peak(0)
+    flop = {"ZCt": 2.0 * n_r * n_mu * n_orb, "cholesky": n_mu ** 3 / 3.0, "solves": 2.0 * n_mu ** 2 * n_r,
+            "G_zeta": 2.0 * float(n_r) ** 2 * n_mu, "zetaT_G_zeta": 2.0 * n_r * float(n_mu) ** 2}
+    times = []
+    with gwl.Context(n_v, n_c, n_mu) as ctx:
+        for i in range(args.warmup + args.steps):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            _, V = ctx.isdf_build(pv, pc, r, w, 0.5, idx, want_zeta=False)
+            torch.cuda.synchronize()
+            if i >= args.warmup:
+                times.append(time.perf_counter() - t0)
+        launches = ctx.get_launch_count()
+    t = float(np.median(times))
+    total = sum(flop.values())
+    line = {"arm": "isdf (SURVEY 8(f)-4): not the headline bench line", "metric": "isdf_build_seconds", "value": t, "unit": "s",
+            "higher_is_better": False, "steps": args.steps, "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"gwl_isdf_build: {n_orb} box orbitals ({n_v} + {n_c}) on a {n_grid}^3 grid, n_r = {n_r}, "
+                                   f"N_mu = {n_mu} stride points (seed {seed}), softened Coulomb quadrature (soft 0.5)",
+                       "n_r": n_r, "n_orb": n_orb, "n_mu": n_mu},
+            "flop_model": flop, "flop_total": total, "tflops_whole_call": total / t * 1e-12,
+            "frac_of_dmma_peak_whole_call": total / t * 1e-12 / peak, "dmma_peak_tflops": peak,
+            "host_bytes_in": int(pv.nbytes + pc.nbytes + r.nbytes + idx.nbytes), "host_bytes_out": int(V.nbytes),
+            "gpu_launches_per_build": int(launches // (args.warmup + args.steps)),
+            "V_checksum": float(np.abs(V).sum()), "V_asymmetry": float(np.abs(V - V.T).max() / np.abs(V).max())}
+    print(json.dumps(line), flush=True)
+
+
 SHARD_QUANTUM = 128   # chain shards are cut at multiples of the GEMM column tile (runtime.shard_range)
 
 
@@ -544,6 +598,9 @@ def main():
         return
     if args.sharded_state:
         run_sharded_state(args)
+        return
+    if args.isdf:
+        run_isdf(args)
         return
     if args.sym >= 0 and not args.paper_setting:
         run_sym(args)

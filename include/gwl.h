@@ -73,6 +73,18 @@ gwl_status gwl_set_kernel(gwl_ctx* ctx, const double* V);
  * NULL) clears it: Op = C and gwl_selfenergy evaluates Eq. 11 on the Ritz pairs of T_L ("direct mode"). */
 gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo, double hi);
 
+/* Coefficients for gwl_set_polynomial: cheb[0..g] (HOST, caller-allocated) of the least-squares fit of sqrt(x) at the
+ * 4 (g + 1) Chebyshev nodes of [lo, hi] -- "a polynomial function p_g(x) ... fitted to sqrt(x)" with the coefficients found "via
+ * least-squares fitting", g = 7 in the paper's runs.  Host arithmetic only (closed form
+ * in the Chebyshev basis); needs no context and no GPU.  GWL_EINVAL unless 1 <= g <= 64 and 0 < lo < hi. */
+gwl_status gwl_fit_sqrt_polynomial(int g, double lo, double hi, double* cheb);
+/* The fitting range for it.  steps = 0: the heuristic [0.8 min Delta^2, 1.25 max Delta^2] from the energies of
+ * gwl_set_energies, no GPU work.  steps >= 2: lo = 0.8 min Delta^2 (a lower bound of C when V is positive semidefinite) and
+ * hi = (1 + margin) max(lam_max of gwl_spectrum_bounds(steps), max Delta^2); margin (e.g. 0.02) cushions an unconverged top
+ * Ritz value and is a heuristic, not a bound.  Like gwl_spectrum_bounds this replaces the chain list and synchronises.
+ * lo, hi HOST outputs.  Real-orbital contexts with energies set (GWL_ESTATE otherwise). */
+gwl_status gwl_sqrt_fit_range(gwl_ctx* ctx, int64_t steps, double margin, double* lo, double* hi);
+
 /* Extremal eigenvalues of the operator for the fitting range of p_g: "One can use standard Lanczos algorithm to
  * determine the extremal eigenvalues min(Omega_s^2) and max(Omega_s^2) of C".  Runs `steps`
  * (2..512; 30-60 is plenty) Lanczos steps on the operator itself (C, or A in the TDA; never p_g(C)) from a generic

@@ -179,6 +179,55 @@ gwl_status gwl_set_polynomial(gwl_ctx* ctx, int g, const double* cheb, double lo
     return GWL_OK;
 }
 
+// Least-squares fit of sqrt(x) at the M = 4 (g + 1) first-kind Chebyshev nodes of [lo, hi] (
+// DESIGN.md Q13).  In the Chebyshev basis the normal equations are diagonal -- sum_k T_i(t_k) T_j(t_k) = (M/2) delta_ij
+// (M for i = j = 0) on the nodes t_k = cos(pi (k + 1/2) / M) -- so c_j = (2/M) sum_k sqrt(x_k) cos(j theta_k), c_0 halved.
+// Host arithmetic only: no context, no device.
+gwl_status gwl_fit_sqrt_polynomial(int g, double lo, double hi, double* cheb) {
+    if (cheb == nullptr || g < 1 || g > 64 || !(lo > 0.0) || !(hi > lo) || !std::isfinite(hi)) return GWL_EINVAL;
+    const int M = 4 * (g + 1);
+    const double pi = 3.14159265358979323846;
+    std::vector<double> f((size_t)M), th((size_t)M);
+    for (int k = 0; k < M; ++k) {
+        th[k] = pi * (k + 0.5) / M;
+        f[k] = std::sqrt(0.5 * (hi + lo) + 0.5 * (hi - lo) * std::cos(th[k]));
+    }
+    for (int j = 0; j <= g; ++j) {
+        double acc = 0.0;
+        for (int k = 0; k < M; ++k) acc += f[k] * std::cos(j * th[k]);
+        cheb[j] = (j == 0 ? 1.0 : 2.0) * acc / M;
+    }
+    return GWL_OK;
+}
+
+// Fitting range of p_g.  steps = 0: the paper's heuristic [0.8 min Delta^2, 1.25 max Delta^2] (reading Q12).
+// steps >= 2: lo as before (a true lower bound of C when V is positive semidefinite), hi = (1 + margin) max(Lanczos
+// estimate of gwl_spectrum_bounds, max Delta^2) (reading Q23: the heuristic upper end is not a bound once the coupling is
+// strong).  The margin is a cushion for an unconverged top Ritz value, not a guarantee.
+gwl_status gwl_sqrt_fit_range(gwl_ctx* ctx, int64_t steps, double margin, double* lo, double* hi) {
+    if (ctx == nullptr) return GWL_EINVAL;
+    if (lo == nullptr || hi == nullptr || !(margin >= 0.0) || steps < 0 || steps == 1)
+        return ctx->fail(GWL_EINVAL, "gwl_sqrt_fit_range: need lo, hi != NULL, margin >= 0 and steps = 0 or >= 2");
+    if (ctx->cplx) return ctx->fail(GWL_ESTATE, "gwl_sqrt_fit_range: the polynomial square root applies to real-orbital contexts");
+    if (!ctx->have_eps || ctx->h_eps_v.empty() || ctx->h_eps_c.empty())
+        return ctx->fail(GWL_ESTATE, "gwl_sqrt_fit_range: energies must be set");
+    const double v_min = *std::min_element(ctx->h_eps_v.begin(), ctx->h_eps_v.end());
+    const double v_max = *std::max_element(ctx->h_eps_v.begin(), ctx->h_eps_v.end());
+    const double c_min = *std::min_element(ctx->h_eps_c.begin(), ctx->h_eps_c.end());
+    const double c_max = *std::max_element(ctx->h_eps_c.begin(), ctx->h_eps_c.end());
+    const double d_min = c_min - v_max, d_max = c_max - v_min;
+    *lo = 0.8 * d_min * d_min;
+    if (steps == 0) {
+        *hi = 1.25 * d_max * d_max;
+        return GWL_OK;
+    }
+    double lam_min = 0.0, lam_max = 0.0;
+    const gwl_status rs = gwl_spectrum_bounds(ctx, steps, &lam_min, &lam_max);
+    if (rs != GWL_OK) return rs;
+    *hi = (1.0 + margin) * std::max(lam_max, d_max * d_max);
+    return GWL_OK;
+}
+
 gwl_status gwl_set_approximation(gwl_ctx* ctx, int approximation) {
     if (ctx == nullptr || (approximation != GWL_RPA && approximation != GWL_TDA)) return GWL_EINVAL;
     DeviceGuard dg(ctx);

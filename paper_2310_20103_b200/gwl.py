@@ -32,6 +32,8 @@ SIGNATURES = {
     "gwl_set_kernel": (c_int, [c_void_p, c_void_p]),
     "gwl_set_polynomial": (c_int, [c_void_p, c_int, c_void_p, c_double, c_double]),
     "gwl_set_approximation": (c_int, [c_void_p, c_int]),
+    "gwl_fit_sqrt_polynomial": (c_int, [c_int, c_double, c_double, c_void_p]),
+    "gwl_sqrt_fit_range": (c_int, [c_void_p, c_int64, c_double, POINTER(c_double), POINTER(c_double)]),
     "gwl_spectrum_bounds": (c_int, [c_void_p, c_int64, POINTER(c_double), POINTER(c_double)]),
     "gwl_casida_matvec": (c_int, [c_void_p, c_void_p, c_void_p, c_int64]),
     "gwl_set_chains": (c_int, [c_void_p, c_int64, c_void_p, c_void_p]),
@@ -147,6 +149,15 @@ def chain_norms_static(p, norm2, n_chains: int | None = None, n_vc: int | None =
     return norm2
 
 
+def fit_sqrt_polynomial(g: int, lo: float, hi: float) -> np.ndarray:
+    """cheb[0..g] of p_g(x) ~ sqrt(x) on [lo, hi] (gwl_fit_sqrt_polynomial: host arithmetic inside libgwl.so)."""
+    c = np.zeros(int(g) + 1 if g >= 0 else 1)
+    st = load_library().gwl_fit_sqrt_polynomial(int(g), float(lo), float(hi), _ptr(c))
+    if st != GWL_OK:
+        raise GwlError(st, "gwl_fit_sqrt_polynomial: need 1 <= g <= 64 and 0 < lo < hi")
+    return c
+
+
 class Context:
     """gwl_ctx wrapper.  Method names follow the C ABI without the gwl_ prefix."""
 
@@ -222,6 +233,12 @@ class Context:
     def set_approximation(self, approximation: int):
         """0 = RPA (operator C, default), 1 = Tamm-Dancoff (operator A)."""
         self._ck(self._lib.gwl_set_approximation(self._h, int(approximation)))
+
+    def sqrt_fit_range(self, steps: int = 40, margin: float = 0.02):
+        """(lo, hi) for gwl_set_polynomial: steps = 0 the paper's heuristic range, else from gwl_spectrum_bounds."""
+        lo, hi = c_double(0.0), c_double(0.0)
+        self._ck(self._lib.gwl_sqrt_fit_range(self._h, int(steps), float(margin), byref(lo), byref(hi)))
+        return lo.value, hi.value
 
     def spectrum_bounds(self, steps: int = 40):
         """(lam_min, lam_max) estimates of the operator's spectrum from a short Lanczos run."""

@@ -1,10 +1,9 @@
-"""Host helper for the optional polynomial mode: coefficients of p_g(x) ~ sqrt(x) for
-gwl_set_polynomial.  PAPER.md:85, :284, :317: least-squares fit at the Chebyshev nodes of the fitting range,
-range [0.8 min(eps_c - eps_v)^2, 1.25 max(eps_c - eps_v)^2] (readings Q12, Q13).
+"""Python face of the polynomial-mode helpers of the C ABI: coefficients of p_g(x) ~ sqrt(x) and the
+fitting range for gwl_set_polynomial.  PAPER.md:85, :284, :317 (readings Q12, Q13, Q23).
 
-The fit is done in the Chebyshev basis, where it has a closed form: first-kind Chebyshev polynomials are orthogonal on
-the M first-kind nodes t_k = cos(pi (k + 1/2) / M), sum_k T_i(t_k) T_j(t_k) = M/2 delta_ij (M for i = j = 0), so the
-least-squares coefficients are c_j = (2 / M) sum_k f(x_k) T_j(t_k), c_0 halved.  No oracle code is used or imported.
+The arithmetic lives in libgwl.so -- gwl_fit_sqrt_polynomial (the least-squares fit at the Chebyshev nodes, closed form in the
+Chebyshev basis) and gwl_sqrt_fit_range (heuristic range, or the Lanczos estimate of gwl_spectrum_bounds) -- so a C caller can
+run the paper's route (g = 7, N_iter = 8) without this file.  The functions here only forward.  No oracle code is used.
 """
 from __future__ import annotations
 
@@ -34,10 +33,7 @@ def range_from_spectrum(ctx, eps_v, eps_c, steps: int = 40, margin: float = 0.02
     estimates agree to well inside the margin.
     lo = the paper's 0.8 min Delta^2, which IS a lower bound of C whenever V is positive semidefinite
     (C - diag(Delta^2) is then positive semidefinite).  Call before the chain list is set (the probe replaces it)."""
-    d_min = float(np.min(eps_c) - np.max(eps_v))
-    d_max = float(np.max(eps_c) - np.min(eps_v))
-    _, lam_max = ctx.spectrum_bounds(steps)
-    return 0.8 * d_min * d_min, (1.0 + margin) * max(lam_max, d_max * d_max)
+    return ctx.sqrt_fit_range(steps, margin)            # eps_v, eps_c: the context already holds them (gwl_set_energies)
 
 
 def sqrt_chebyshev(g: int, lo: float, hi: float, nodes_per_coefficient: int = 4) -> np.ndarray:
@@ -45,9 +41,7 @@ def sqrt_chebyshev(g: int, lo: float, hi: float, nodes_per_coefficient: int = 4)
     M = nodes_per_coefficient (g + 1) Chebyshev nodes of [lo, hi]."""
     if g < 1 or not (hi > lo > 0.0):
         raise ValueError("need g >= 1 and hi > lo > 0")
-    M = nodes_per_coefficient * (g + 1)
-    theta = np.pi * (np.arange(M) + 0.5) / M
-    f = np.sqrt(0.5 * (hi + lo) + 0.5 * (hi - lo) * np.cos(theta))
-    c = np.array([(2.0 / M) * np.sum(f * np.cos(j * theta)) for j in range(g + 1)])
-    c[0] *= 0.5
-    return c
+    if nodes_per_coefficient != 4:
+        raise ValueError("gwl_fit_sqrt_polynomial fits at 4 (g + 1) nodes (DESIGN.md Q13)")
+    from . import gwl
+    return gwl.fit_sqrt_polynomial(g, lo, hi)

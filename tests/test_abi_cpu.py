@@ -89,8 +89,24 @@ def test_synth_configs_match_baseline():
     assert abs(synth.CONFIGS[2].flop_per_vector() - 6.52e9) < 0.01e9
 
 
+def test_fit_sqrt_polynomial_through_the_c_abi(lib):
+    """gwl_fit_sqrt_polynomial called through ctypes (host arithmetic, no GPU): equals the oracle's lstsq fit, and rejects
+    bad arguments.  PAPER.md:85, :284, :317."""
+    from oracle import gw_oracle as orc
+    for g, lo, hi in ((7, 5.0, 1125.0), (1, 0.3, 0.9), (64, 1.0, 4.0e4)):
+        c = np.zeros(g + 1)
+        assert lib.gwl_fit_sqrt_polynomial(g, lo, hi, c.ctypes.data_as(ctypes.c_void_p)) == gwl.GWL_OK
+        ref = orc.fit_sqrt_chebyshev(g, lo, hi)
+        assert np.abs(c - ref).max() <= 1e-12 * np.abs(ref).max()
+    c = np.zeros(8)
+    p = c.ctypes.data_as(ctypes.c_void_p)
+    for g, lo, hi, ptr in ((0, 1.0, 2.0, p), (65, 1.0, 2.0, p), (3, 0.0, 2.0, p), (3, 2.0, 2.0, p), (3, 1.0, 2.0, None)):
+        assert lib.gwl_fit_sqrt_polynomial(g, lo, hi, ptr) == gwl.GWL_EINVAL
+    assert lib.gwl_sqrt_fit_range(None, 0, 0.02, None, None) == gwl.GWL_EINVAL
+
+
 def test_polyfit_helper_closed_form_equals_least_squares():
-    """paper_2310_20103_b200/polyfit.py (discrete-orthogonality closed form) against the oracle's lstsq fit and
+    """paper_2310_20103_b200/polyfit.py (a call-through to gwl_fit_sqrt_polynomial) against the oracle's lstsq fit and
     against sqrt itself on the range."""
     import numpy as np
     from oracle import gw_oracle as orc

@@ -335,6 +335,19 @@ def test_state_and_argument_errors(p0):
         assert ctx.get_launch_count() > 0
 
 
+def test_sqrt_fit_range_heuristic_and_lanczos(p0):
+    """gwl_sqrt_fit_range: steps = 0 is the paper's heuristic [0.8 min Delta^2, 1.25 max Delta^2] (PAPER.md:284, Q12);
+    steps > 0 takes hi from the Lanczos estimate, against the oracle's own bound on the oracle's product."""
+    delta = orc.delta_vc(p0.eps_v, p0.eps_c)
+    with _ctx(p0, chains=False) as ctx:
+        lo, hi = ctx.sqrt_fit_range(0)
+        assert abs(lo - 0.8 * (delta ** 2).min()) <= 1e-12 * lo and abs(hi - 1.25 * (delta ** 2).max()) <= 1e-12 * hi
+        lo2, hi2 = ctx.sqrt_fit_range(40, 0.02)
+    _, top = orc.spectrum_bounds_lanczos(
+        lambda x: orc.casida_matvec_factored(p0.phi_v, p0.phi_c, p0.V, delta, x[None])[0], delta.size, 40)
+    assert lo2 == lo and abs(hi2 - 1.02 * max(top, (delta ** 2).max())) <= 1e-6 * hi2
+
+
 def test_spectrum_bounds_after_breakdown_match_the_oracle():
     """Breakdown inside the range probe: with V = 0 and only three distinct Delta the Krylov space of any start vector is
     three-dimensional, the fourth beta vanishes, and the bounds are the exact extreme eigenvalues min / max Delta^2 with a
