@@ -704,12 +704,15 @@ def test_state_selfenergy_exchange_and_qp_solve_config1(p1):
 
 
 def test_out_of_memory_is_reported_and_context_survives():
-    """A reorthogonalised run whose basis (100 001 x 4 x 65 536 doubles = 210 GB) cannot be allocated returns
-    GWL_ENOMEM from a single failed cudaMalloc; the context keeps working afterwards."""
+    """A reorthogonalised run whose basis (8192 + 1 vectors x 64 chains x 65 536 doubles = 275 GB, at the largest step count
+    reorth = 1 accepts, GWL_MAX_REORTH_STEPS) cannot be allocated returns GWL_ENOMEM from a single failed cudaMalloc; the
+    context keeps working afterwards."""
     p = synth.make_custom(8, 8192, 32, seed=2)
     with _ctx(p) as ctx:
+        ctx.set_chains(np.arange(64, dtype=np.int32), np.full(64, 7, dtype=np.int32))
         with pytest.raises(gwl.GwlError) as e:
-            ctx._ck(ctx._lib.gwl_lanczos(ctx._h, 4, 100000, 4, 1, None, None, None, None))
+            ctx._ck(ctx._lib.gwl_lanczos(ctx._h, 64, 8192, 64, 1, None, None, None, None))
         assert e.value.status == gwl.GWL_ENOMEM
+        ctx.set_chains(p.n_idx, p.m_idx)
         a, b, n2, ln = ctx.lanczos(4, 10, 4, 1)
         assert (ln == 10).all() and np.isfinite(a).all() and (b > 0).all()
