@@ -63,9 +63,9 @@ def parse():
     ap.add_argument("--sharded-state", action="store_true",
                     help="SURVEY 8(f)-2 arm, its own line: the N_v+N_c chains of ONE state partitioned over the ranks "
                          "(runtime.shard_range), one NCCL all-reduce of the omega grid; strong scaling")
-    ap.add_argument("--isdf", default="", metavar="NGRID,NORB,NMU[,SEED]",
+    ap.add_argument("--isdf", default="", metavar="NGRID,NORB,NMU[,SEED]",  # SEED < 0: pick the first well-conditioned stride-point set
                     help="context run, not the bench line: the ISDF front end (SURVEY 8(f)-4; gwl_isdf_build) on NORB particle-in-"
-                         "a-box orbitals on an NGRID^3 grid (n_r = NGRID^3 <= 65535) with NMU interpolation points, e.g. 40,256,1024: "
+                         "a-box orbitals on an NGRID^3 grid with NMU interpolation points, e.g. 40,256,1024: "
                          "seconds per build, flop model and fraction of the DMMA peak")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -475,6 +475,13 @@ def run_isdf(args):
     gwl.load_library()
     r, phi, w = synth.box_orbitals(n_grid, n_orb)
     n_r = r.shape[0]
+    if seed < 0:                                     # first stride-point set on which C C^T is safely positive definite
+        for seed in range(16):
+            idx = synth.stride_points(n_r, n_mu, seed)
+            P = phi[idx] @ phi[idx].T
+            ev = np.linalg.eigvalsh(P * P)
+            if ev[0] > 0 and ev[-1] / ev[0] < 1e9:
+                break
     idx = synth.stride_points(n_r, n_mu, seed)
     pv, pc = np.ascontiguousarray(phi[:, :n_v]), np.ascontiguousarray(phi[:, n_v:])
     peak = gwl.probe_fp64_peak(0)

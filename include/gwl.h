@@ -236,10 +236,12 @@ gwl_status gwl_tdc_selfenergy_state(gwl_ctx* ctx, int32_t kn, int32_t km, int32_
  * sum_ij zeta_alpha(r_i) G_ij zeta_beta(r_j), G_ij = weight^2 14.4 / sqrt(|r_i - r_j|^2 + soft^2) eV (softened at short range:
  * the stand-in for the real-space Poisson solve).  The paper's code runs this part on CPUs.
  * Inputs (host): phi_v_grid [n_r][n_v], phi_c_grid [n_r][n_c] orbitals on the real-space grid, r [n_r][3] grid points
- * (Angstrom), weight = h^3, soft > 0, idx [n_mu] distinct grid indices.  n_mu <= n_r <= 65535.
+ * (Angstrom), weight = h^3, soft > 0, idx [n_mu] distinct grid indices.  n_mu <= n_r <= GWL_ISDF_MAX_NR.  Device memory is about
+ * 8 n_r (n_v + n_c + 3 n_mu + 8192) bytes: G is generated in panels of 8192 rows that feed the G zeta GEMM (GWL_ENOMEM if it does not fit).
  * Effect: the context's orbitals become the grid orbitals at the interpolation points and its kernel becomes (alpha|beta),
  * exactly as after gwl_set_orbitals + gwl_set_kernel (gwl_set_energies is still needed).  Optional host outputs:
  * zeta_t [n_mu][n_r] (zeta transposed) and V_out [n_mu][n_mu]; either may be NULL. */
+#define GWL_ISDF_MAX_NR 4194304 /* grid points of gwl_isdf_build; the Coulomb quadrature matrix is walked in row panels, never held */
 gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, const double* phi_c_grid, const double* r,
                           double weight, double soft, const int32_t* idx, double* zeta_t, double* V_out);
 

@@ -271,7 +271,8 @@ cudaError_t launch_gather_rows(const double* src, int64_t ld_src, int n_cols, co
 cudaError_t launch_hadamard(double* y, const double* x, int64_t n, cudaStream_t st);
 cudaError_t launch_gather_cols(const double* Y, int64_t ld_y, const int32_t* idx, int n_mu, double* S, int64_t ld_s,
                                cudaStream_t st);
-cudaError_t launch_coulomb_grid(const double* r, int n_r, double weight, double soft, double* G, int64_t ld, cudaStream_t st);
+cudaError_t launch_coulomb_grid(const double* r, int n_r, int i0, int rows, double weight, double soft, double* G, int64_t ld,
+                                cudaStream_t st);  // rows i0 .. i0+rows-1 of the quadrature matrix into G[0..rows-1][*], rows <= 65535
 // S = L L^T in place (lower triangle, upper zeroed inside the diagonal blocks); *info (zero on entry) = 1-based index of the
 // first pivot that is not above 1e-13 max_i S_ii (scale: one device double of scratch)
 cudaError_t launch_cholesky(double* S, int64_t ld, int n, double* scale, int* info, cudaStream_t st);

@@ -14,8 +14,8 @@ gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, c
     if (ctx->sym) return ctx->fail(GWL_ESTATE, "gwl_isdf_build: symmetry-block (gwl_sym_create) context: not available on a symmetry-block context");
     if (phi_v_grid == nullptr || phi_c_grid == nullptr || r == nullptr || idx == nullptr)
         return ctx->fail(GWL_EINVAL, "gwl_isdf_build: NULL input");
-    if (n_r < ctx->n_mu || n_r > 65535 || !(weight > 0.0) || !(soft > 0.0))
-        return ctx->fail(GWL_EINVAL, "gwl_isdf_build: need n_mu <= n_r <= 65535, weight > 0, soft > 0");
+    if (n_r < ctx->n_mu || n_r > GWL_ISDF_MAX_NR || !(weight > 0.0) || !(soft > 0.0))
+        return ctx->fail(GWL_EINVAL, "gwl_isdf_build: need n_mu <= n_r <= GWL_ISDF_MAX_NR (4 194 304), weight > 0, soft > 0");
     const int n_mu = ctx->n_mu, n_orb = ctx->n_v + ctx->n_c, nr = (int)n_r;
     {
         std::vector<char> seen((size_t)n_r, 0);
@@ -36,7 +36,10 @@ gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, c
     // G also stages the finished (alpha|beta): the context's own V and orbitals are only touched once every step that can
     // fail on the inputs (a singular C C^T) has passed, so a failed build leaves a ready context exactly as it was.
     const size_t v_bytes = (size_t)n_mu * ldm * 8;
-    CK(G.ensure(std::max((size_t)n_r * nrp * 8, v_bytes), st));
+    // The Coulomb quadrature matrix is walked in row panels of G_PANEL rows: memory scales as N_r N_mu, not N_r^2.
+    constexpr int G_PANEL = 8192;
+    const int g_rows = std::min(nr, G_PANEL);
+    CK(G.ensure(std::max((size_t)g_rows * nrp * 8, v_bytes), st));
     CK(U.ensure((size_t)n_mu * nrp * 8, st));
     CK(cudaMemsetAsync(Phi.p, 0, Phi.bytes, st));
     CK(cudaMemsetAsync(PhiMu.p, 0, PhiMu.bytes, st));
@@ -73,9 +76,14 @@ gwl_status gwl_isdf_build(gwl_ctx* ctx, int64_t n_r, const double* phi_v_grid, c
                                          "): the interpolation points do not resolve the pair products");
     CKL(4, launch_cholesky_solve(dS, ldm, n_mu, Y.as<double>(), nrp, nr, st));
     // (alpha|beta) = zeta^T G zeta with the Coulomb quadrature matrix of the grid
-    CKL(4, launch_coulomb_grid(d_r, nr, weight, soft, G.as<double>(), nrp, st));
-    rs = plain_gemm(ctx, G.as<double>(), nrp, Y.as<double>(), nrp, nr, n_mu, (int)(nrp / BK), U.as<double>(), nrp, 1);
-    if (rs != GWL_OK) return rs;
+    // U[mu][i] = sum_j G[i][j] zeta_mu(r_j), panel of rows i by panel (G is symmetric; each panel is generated, used, dropped;
+    // the padding columns n_r .. nrp of a panel stay zero from the memset above, no kernel writes them)
+    for (int i0 = 0; i0 < nr; i0 += G_PANEL) {
+        const int rows = std::min(G_PANEL, nr - i0);
+        CKL(4, launch_coulomb_grid(d_r, nr, i0, rows, weight, soft, G.as<double>(), nrp, st));
+        rs = plain_gemm(ctx, G.as<double>(), nrp, Y.as<double>(), nrp, rows, n_mu, (int)(nrp / BK), U.as<double>() + i0, nrp, 1);
+        if (rs != GWL_OK) return rs;
+    }
     CK(cudaMemsetAsync(G.p, 0, v_bytes, st));  // G itself is consumed; its head becomes the staging copy of V (zero padding)
     rs = plain_gemm(ctx, Y.as<double>(), nrp, U.as<double>(), nrp, n_mu, n_mu, (int)(nrp / BK), G.as<double>(), ldm, 1);
     if (rs != GWL_OK) return rs;

@@ -37,13 +37,15 @@ __global__ void k_gather_cols(const double* __restrict__ Y, int64_t ld_y, const 
 }
 
 // G[i][j] = w^2 * 14.4 / sqrt(|r_i - r_j|^2 + soft^2): the grid quadrature of 1/|r - r'| (eV Angstrom)
-__global__ void k_coulomb_grid(const double* __restrict__ r, int n_r, double w2, double soft2, double* __restrict__ G,
+// One launch fills the row panel i0 .. i0 + gridDim.y - 1 into G[0 .. gridDim.y - 1][*]: the full N_r x N_r matrix is never
+// held (gwl_isdf_build walks it in panels that feed the G zeta GEMM).
+__global__ void k_coulomb_grid(const double* __restrict__ r, int n_r, int i0, double w2, double soft2, double* __restrict__ G,
                                int64_t ld) {
-    const int i = blockIdx.y;
+    const int i = i0 + blockIdx.y;
     const double xi = r[3 * i], yi = r[3 * i + 1], zi = r[3 * i + 2];
     for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n_r; j += gridDim.x * blockDim.x) {
         const double dx = xi - r[3 * j], dy = yi - r[3 * j + 1], dz = zi - r[3 * j + 2];
-        G[(int64_t)i * ld + j] = w2 * 14.4 / sqrt(dx * dx + dy * dy + dz * dz + soft2);
+        G[(int64_t)blockIdx.y * ld + j] = w2 * 14.4 / sqrt(dx * dx + dy * dy + dz * dz + soft2);
     }
 }
 
@@ -355,10 +357,12 @@ cudaError_t launch_gather_cols(const double* Y, int64_t ld_y, const int32_t* idx
     return cudaGetLastError();
 }
 
-cudaError_t launch_coulomb_grid(const double* r, int n_r, double weight, double soft, double* G, int64_t ld, cudaStream_t st) {
-    dim3 grid((unsigned)std::min<int64_t>(ceil_div(n_r, 256), 64), (unsigned)n_r);
-    if (n_r > 65535) return cudaErrorInvalidValue;
-    k_coulomb_grid<<<grid, 256, 0, st>>>(r, n_r, weight * weight, soft * soft, G, ld);
+cudaError_t launch_coulomb_grid(const double* r, int n_r, int i0, int rows, double weight, double soft, double* G, int64_t ld,
+                                cudaStream_t st) {
+    if (rows <= 0) return cudaSuccess;
+    if (rows > 65535 || i0 < 0 || i0 + rows > n_r) return cudaErrorInvalidValue;
+    dim3 grid((unsigned)std::min<int64_t>(ceil_div(n_r, 256), 64), (unsigned)rows);
+    k_coulomb_grid<<<grid, 256, 0, st>>>(r, n_r, i0, weight * weight, soft * soft, G, ld);
     count_launch();
     return cudaGetLastError();
 }

@@ -44,6 +44,29 @@ def test_isdf_fit_and_two_center_integrals(n_grid, n_v, n_c, n_mu, seed):
     assert np.abs(zt[:, idx] - np.eye(n_mu)).max() <= 1e-7
 
 
+def test_isdf_coulomb_matrix_in_row_panels():
+    """n_r = 22^3 = 10 648 grid points: the Coulomb quadrature matrix is generated in two row panels (8192 + a ragged 2456)
+    that feed the G zeta GEMM one after the other.  30 orbitals, N_mu = 64; the stride-point seed is the first whose
+    cond(C C^T) is below 1e5 (decided here from the inputs alone), so that the 1e-8 bar of the other cases applies."""
+    n_grid, n_v, n_c, n_mu = 22, 8, 22, 64
+    r, phi, w = synth.box_orbitals(n_grid, n_v + n_c)
+    for seed in range(8):
+        idx = synth.stride_points(r.shape[0], n_mu, seed)
+        P = phi[idx] @ phi[idx].T
+        ev = np.linalg.eigvalsh(P * P)
+        if ev[0] > 0 and ev[-1] / ev[0] < 1e5:
+            break
+    else:
+        pytest.fail("no well-conditioned stride-point set among 8 seeds")
+    with gwl.Context(n_v, n_c, n_mu) as ctx:
+        zt, V = ctx.isdf_build(phi[:, :n_v], phi[:, n_v:], r, w, 0.5, idx)
+    zeta = isdf.fit(phi, phi, idx)
+    Vref = isdf.two_center(zeta, isdf.coulomb_grid(r, w, 0.5))
+    assert np.abs(zt.T - zeta).max() <= 1e-8 * np.abs(zeta).max()
+    assert np.abs(V - Vref).max() <= 1e-8 * np.abs(Vref).max()
+    assert np.abs(V - V.T).max() <= 1e-10 * np.abs(V).max()
+
+
 def test_isdf_built_context_runs_the_hot_path():
     """gwl_isdf_build installs Phi(r_mu) and (alpha|beta): the Casida product, Lanczos and Sigma on that context against
     the oracle fed with the ORACLE's own fit."""
